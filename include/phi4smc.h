@@ -1,0 +1,186 @@
+/*
+ * phi4smc.h -- C ABI of libphi4smc.so: the batched tempered-particle update of
+ * "Particle Monte Carlo methods for Lattice Field Theory" (arxiv 2511.15196; PAPER.md) for
+ * 2D phi^4 theory, as hand-written CUDA for sm_100a (NVIDIA B200).
+ *
+ * Model (PAPER.md:27-29 Eq. 1, :43): periodic L x L lattice, V = L*L sites, x = r*L + c,
+ *   S_E(phi) = sum_x [ 1/2 (phi_{x+1hat}-phi_x)^2 + 1/2 (phi_{x+2hat}-phi_x)^2
+ *                      + 1/2 m0sq phi_x^2 + lambda phi_x^4 ],
+ *   U0(phi) = 1/2 sum_x phi_x^2,   p_beta(phi) ~ exp(-[U0 + beta S_E]),  beta in [0,1].
+ * log Z means log int N(phi;0,I) exp(-S_E(phi)) dphi (reading A1).
+ *
+ * Conventions
+ *  - Every function returns PHI4_OK (0) or a negative PHI4_E* code; nothing throws, aborts or
+ *    prints.  phi4_strerror(code) names a code.  There is NO CPU fallback: without a CUDA device
+ *    every compute entry point returns PHI4_ECUDA.
+ *  - Pointers named d_* are DEVICE pointers, h_* are HOST pointers; everything else is by value.
+ *  - The caller owns the device workspace (one allocation of *_workspace_bytes, 256-byte aligned)
+ *    and the CUDA stream (a cudaStream_t passed as void*; NULL = the legacy default stream).  The
+ *    library owns the opaque handle, keeps all state inside the workspace and never allocates
+ *    device memory after *_init.  The workspace must outlive the handle.
+ *  - Work is enqueued on the handle's stream.  A function synchronises the stream only when it
+ *    returns host values (an info struct, a host array, a double); this is stated per function.
+ *  - Host-visible particle arrays are fp32, site-major and dense: h_phi[x*N + i], x = site,
+ *    i = particle.  (Inside the workspace the particle stride is padded; not visible here.)
+ *  - Random numbers: Philox4x32-10, key = (seed lo32, seed hi32), counter = (site quad or 0,
+ *    slot, step counter, stream tag); readings R1/R2 fix the streams so that a CPU
+ *    oracle can reproduce every draw.
+ */
+#ifndef PHI4SMC_H
+#define PHI4SMC_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PHI4_OK 0
+#define PHI4_EINVAL (-1)  /* bad argument, NULL handle, wrong sampler kind, workspace too small   */
+#define PHI4_ENOMEM (-2)  /* host allocation failed                                               */
+#define PHI4_ENOTPD (-3)  /* particle covariance not positive definite even after the jitter retry */
+#define PHI4_ENAN (-4)    /* a non-finite action or weight was produced                           */
+#define PHI4_ECUDA (-5)   /* a CUDA call failed or no device; see phi4_last_cuda_error()          */
+
+#define PHI4_HIST_BINS 80 /* B = 80 bins; fixed range [-1.6, 1.6] (reading A13)     */
+#define PHI4_MAX_HOOK_STEPS 64 /* largest k accepted by smc_mutate when flags/margins are wanted  */
+
+typedef struct phi4smc phi4smc; /* opaque sampler handle (SMC or NS) */
+
+/* Free parameters of the outer kernel. */
+typedef struct {
+  int k_steps;      /* MCMC steps per tempering transition, n_MCMC >= 1           */
+  float ess_target; /* target ESS fraction in (0,1) for adaptive tempering        */
+  float step_scale; /* s in phi' = phi + s*Lc*z; 0 selects 2.38/sqrt(V) (A3)       */
+  int mutation_path; /* 0 = automatic, 1 = generic (any V), 2 = fused tcgen05 (if it supports V) */
+} smc_params;
+
+/* One tempering transition, filled when smc_step is given a non-NULL pointer. */
+typedef struct {
+  double beta;        /* inverse temperature after the step                                      */
+  double delta;       /* increment chosen by the ESS bisection (P1)                              */
+  double ess_frac;    /* ESS/N of the incremental weights at delta                               */
+  double dlogZ;       /* logsumexp(-delta S_E) - log N (P2)                                      */
+  double logZ;        /* running sum of dlogZ                                                    */
+  double accept_rate; /* mean Metropolis acceptance over the k_steps mutations    */
+  int n_unique;       /* distinct ancestors chosen by the resampler                              */
+  int chol_status;    /* 0 plain, 1 jitter retry used, -1 failed                                 */
+  int temp_index;     /* 0-based index of this temperature                                       */
+  int done;           /* 1 when beta == 1                                                        */
+} smc_step_info;
+
+typedef struct {
+  double logX;           /* log prior volume after this iteration (reading A6)                   */
+  double logZ;           /* log evidence accumulated from dead points (live term added when done) */
+  double S_star;         /* likelihood threshold of this iteration: constraint S_E < S_star      */
+  double accept_rate;    /* acceptance of the constrained walk                                   */
+  double remaining_frac; /* X mean_live(e^-S) / (Z + X mean_live(e^-S))                          */
+  int chol_status;
+  int iter_index;
+  int done; /* 1 when remaining_frac < stop_frac; the live term has then been added to logZ      */
+} ns_step_info;
+
+typedef struct {
+  double absM;         /* <|M|>, M = (1/V) sum_x phi_x                             */
+  double M2;           /* <M^2>                                                                  */
+  double chi;          /* V (<M^2> - <|M|>^2)                                                    */
+  double mean_SE;      /* <S_E>                                                                  */
+  double mode_balance; /* #(M>0) / #(M<0), zeros ignored, +inf if no negatives    */
+  double hist[PHI4_HIST_BINS]; /* normalised (weighted) histogram of M on [-1.6, 1.6]            */
+} phi4_observables;
+
+const char* phi4_strerror(int code);
+/* Text of the last CUDA error seen by this handle ("" if none); valid until the next call. */
+const char* phi4_last_cuda_error(const phi4smc* h);
+
+/* ---------------------------------------------------------------- SMC-RW (PAPER.md:53(i)) ----
+ * smc_workspace_bytes: bytes of device memory smc_init needs for an L x L lattice and N particles
+ * (0 if L < 1 or N < 2).  Sized for 180 GB parts: C4 (L=64, N=131072) needs about 9 GB.          */
+size_t smc_workspace_bytes(int L, int N);
+
+/* Creates an SMC sampler: particles phi_i ~ N(0,I) from Philox stream INIT, S_E and U0 evaluated,
+ * beta = 0, logZ = 0, Lc = I, defaults k_steps = 10, ess_target = 0.5, step_scale = 0 (2.38/sqrt V).
+ * d_workspace: device memory of >= smc_workspace_bytes(L,N).  Enqueues on cuda_stream, no sync.  */
+int smc_init(phi4smc** out, int L, float m0sq, float lambda, int N, uint64_t seed,
+             void* d_workspace, size_t workspace_bytes, void* cuda_stream);
+/* Re-initialises an existing handle (SMC or NS) with a new seed exactly as *_init would: fresh
+ * particles from stream INIT, beta = 0, logZ = 0 (NS: -inf, logX = 0), Lc = I, history cleared.
+ * Device work only (no host allocation); enqueue only.                                          */
+int smc_reset(phi4smc* h, uint64_t seed);
+int smc_destroy(phi4smc* h); /* synchronises the stream, frees host resources; NULL is a no-op    */
+int smc_set_params(phi4smc* h, const smc_params* p);
+
+/* One temperature (SURVEY 8(a) P1,P2,P3,P4,C1,C2,(M1-M4) x k_steps):
+ * bisection for delta at the target ESS, incremental weights and log Z, systematic resampling,
+ * gather, covariance + Cholesky of the resampled particles (A4), k_steps fused RW-Metropolis
+ * mutations at the new beta.  info == NULL: enqueue only.  info != NULL: synchronises and fills
+ * it.  Calling it when beta == 1 is a no-op that reports done = 1.                               */
+int smc_step(phi4smc* h, smc_step_info* info);
+
+/* Runs smc_step until beta == 1 or max_temps transitions were made; termination is decided on
+ * the device, the host only polls a flag.  Synchronises.  *n_temps (may be NULL) = transitions
+ * made by this call.  Returns PHI4_ENOTPD / PHI4_ENAN if a step failed.                          */
+int smc_run(phi4smc* h, int max_temps, int* n_temps);
+
+/* Per-temperature records of all transitions made so far (at most cap entries are copied;
+ * returns the number available through *n).  Synchronises.                                       */
+int smc_get_history(phi4smc* h, smc_step_info* h_info, int cap, int* n);
+
+/* C1 + C2 from the current, equally weighted particles: mean, centred covariance with 1/(N-1),
+ * lower Cholesky factor (readings A4, R6).  Enqueue only.                                        */
+int estimate_cov_chol(phi4smc* h);
+
+/* Magnetisation observables of the current particles (SMC: equal weights; NS: dead points and
+ * live points with their nested-sampling weights).  Synchronises.                                */
+int observables(phi4smc* h, phi4_observables* out);
+
+/* Synchronises; SMC: sum of dlogZ so far; NS: log evidence (with the live term once done).
+ * NaN if h is NULL.                                                                              */
+double log_Z(const phi4smc* h);
+
+/* ------------------------------------------------ nested sampling (PAPER.md:53(iv), :170) ---- */
+size_t ns_workspace_bytes(int L, int n_live, int k_delete, int max_iters);
+
+/* n_live points ~ N(0,I), likelihood exp(-S_E); per iteration the k_delete lowest-likelihood
+ * points are deleted and each replaced by an n_walk-step covariance-preconditioned constrained
+ * walk (accept iff S_E' < S_star and log u < -dU0, reading A5).  stop_frac: remaining-evidence
+ * fraction at which the run ends (BASELINE configs: 1e-3).  max_iters bounds the dead-point log.
+ * Requires 2 <= n_live <= 16384 and 1 <= k_delete < n_live.                                      */
+int ns_init(phi4smc** out, int L, float m0sq, float lambda, int n_live, int k_delete, int n_walk,
+            uint64_t seed, double stop_frac, int max_iters, void* d_workspace,
+            size_t workspace_bytes, void* cuda_stream);
+/* One iteration N1-N4.  info != NULL synchronises.  No-op once done.              */
+int ns_step(phi4smc* h, ns_step_info* info);
+int ns_run(phi4smc* h, int max_iters, int* n_iters); /* until done; synchronises                 */
+
+/* ------------------------------------------------- test / checkpoint hooks (all synchronise) --
+ * Needed for lockstep parity with the oracle; they also serve as checkpoint / resume, since the
+ * RNG is counter-based: the whole sampler state is (phi, beta, logZ, step counter).
+ * Any output pointer may be NULL.  N below is the particle count (n_live for NS).               */
+int smc_get_state(phi4smc* h, float* h_phi, float* h_SE, float* h_U0, double* beta,
+                  uint64_t* step_counter);
+/* Replaces the particles (S_E, U0 are recomputed on the device), beta and the step counter.      */
+int smc_set_state(phi4smc* h, const float* h_phi, double beta, uint64_t step_counter);
+int smc_get_chol(phi4smc* h, float* h_Lc /* V*V row-major, strict upper = 0 */);
+int smc_set_chol(phi4smc* h, const float* h_Lc);
+int smc_get_cov(phi4smc* h, float* h_Sigma /* V*V row-major */);
+/* M1-M4 only: k mutation steps at the current beta and Lc; step counters continue from the
+ * handle's counter.  h_accept[j*N+i] in {0,1}, h_margin[j*N+i] = g of reading R4 as the kernel
+ * computed it (fp32).  k <= PHI4_MAX_HOOK_STEPS when either array is wanted.                     */
+int smc_mutate(phi4smc* h, int k, uint8_t* h_accept, float* h_margin);
+/* P1+P2 at the current beta: delta < 0 selects the bisection, otherwise the given delta is used.
+ * Advances beta and logZ; h_w receives the max-shifted fp32 weights (max = 1).                   */
+int smc_reweight(phi4smc* h, double delta, float* h_w, smc_step_info* info);
+/* P3+P4: systematic resampling of the device weights (or of h_w if non-NULL) with the Philox
+ * offset of the current temperature index, then the gather.  h_ancestors receives a_j.           */
+int smc_resample(phi4smc* h, const float* h_w, int32_t* h_ancestors);
+/* NS hooks: the last iteration's dead indices (k_delete, by decreasing S_E) and the dead-point
+ * log so far (S_E, M, log w per dead point; n_dead = iterations * k_delete).                     */
+int ns_get_dead(phi4smc* h, int32_t* h_last_dead_idx, float* h_dead_S, float* h_dead_M,
+                double* h_dead_logw, int cap, int* n_dead);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PHI4SMC_H */

@@ -60,7 +60,7 @@ def lib():
         "orc_init_particles": (None, [C.c_uint64, C.c_int, C.c_int, _dp]),
         "orc_mutate": (None, [_dp, _dp, _dp, C.c_int, C.c_int, C.c_double, C.c_double, _dp,
                               C.c_double, C.c_double, C.c_int, C.c_double, C.c_uint64,
-                              C.c_uint32, C.c_uint32, C.c_uint32, C.c_int, vp, vp, vp]),
+                              C.c_uint32, C.c_uint32, C.c_uint32, C.c_int, vp, vp, vp, vp]),
         "orc_lse_neg": (C.c_double, [_dp, C.c_int, C.c_double]),
         "orc_ess_frac": (C.c_double, [_dp, C.c_int, C.c_double]),
         "orc_next_delta": (C.c_double, [_dp, C.c_int, C.c_double, C.c_double, C.POINTER(C.c_int)]),
@@ -157,20 +157,23 @@ def init_particles(seed, N, V):
 
 
 def mutate(phi, S, U0, L, m0sq, lam, Lc, s, beta, seed, t0, k, mode=MODE_SMC, S_star=0.0,
-           tag_prop=None, tag_acc=None):
+           tag_prop=None, tag_acc=None, slots=None):
     """k RW-Metropolis steps in place on copies; returns (phi, S, U0, accept[k,N], margin[k,N],
-    cmargin[k,N])."""
+    cmargin[k,N]).  slots: optional Philox slot of each column (default: column index)."""
     phi, S, U0 = _f64(phi).copy(), _f64(S).copy(), _f64(U0).copy()
     V, N = phi.shape
     if tag_prop is None:
         tag_prop = TAG_PROP if mode == MODE_SMC else TAG_NS_PROP
     if tag_acc is None:
         tag_acc = TAG_ACC if mode == MODE_SMC else TAG_NS_ACC
+    if slots is not None:
+        slots = np.ascontiguousarray(slots, np.int32)
+        assert slots.shape == (N,)
     acc = np.zeros((k, N), np.uint8)
     mar = np.zeros((k, N))
     cmar = np.zeros((k, N))
     lib().orc_mutate(phi, S, U0, N, L, m0sq, lam, _f64(Lc), s, beta, mode, S_star, seed,
-                     tag_prop, tag_acc, t0, k, _ptr(acc), _ptr(mar), _ptr(cmar))
+                     tag_prop, tag_acc, t0, k, _ptr(acc), _ptr(mar), _ptr(cmar), _ptr(slots))
     return phi, S, U0, acc, mar, cmar
 
 

@@ -234,12 +234,15 @@ void orc_init_particles(uint64_t seed, int N, int V, double* phi) {
  *   accept iff g > 0 (and the constraint in NS mode); u from tag_acc.
  * accept_out[j*N+i] (0/1) and margin_out[j*N+i] (= g; in NS mode also
  * cmargin_out = S_star - S') may be NULL.  phi, S, U0 are updated in place.
+ * slots (may be NULL = identity) gives the Philox slot of column i (R1:
+ * streams are keyed by slot), so that a sub-sample of a large population
+ * can be replayed with its own streams.
  * ---------------------------------------------------------------------- */
 void orc_mutate(double* phi, double* S, double* U0, int N, int L, double m0sq,
                 double lam, const double* Lc, double s, double beta, int mode,
                 double S_star, uint64_t seed, uint32_t tag_prop,
                 uint32_t tag_acc, uint32_t t0, int k, uint8_t* accept_out,
-                double* margin_out, double* cmargin_out) {
+                double* margin_out, double* cmargin_out, const int32_t* slots) {
   int V = L * L;
 #pragma omp parallel
   {
@@ -250,9 +253,10 @@ void orc_mutate(double* phi, double* S, double* U0, int N, int L, double m0sq,
     for (int i = 0; i < N; ++i) {
       orc_get_field(phi, N, V, i, f);
       double Si = S[i], Ui = U0[i];
+      const uint32_t slot = slots ? (uint32_t)slots[i] : (uint32_t)i;
       for (int j = 0; j < k; ++j) {
         uint32_t t = t0 + (uint32_t)j;
-        orc_normals(seed, tag_prop, t, (uint32_t)i, V, z);
+        orc_normals(seed, tag_prop, t, slot, V, z);
         for (int x = 0; x < V; ++x) {
           double d = 0.0;
           for (int y = 0; y <= x; ++y) d += Lc[(size_t)x * V + y] * z[y];
@@ -260,7 +264,7 @@ void orc_mutate(double* phi, double* S, double* U0, int N, int L, double m0sq,
         }
         double Sp = orc_action_field(fp, L, m0sq, lam, NULL);
         double Up = orc_u0_field(fp, V);
-        double u = orc_uniform(seed, tag_acc, t, (uint32_t)i);
+        double u = orc_uniform(seed, tag_acc, t, slot);
         double g;
         int acc;
         if (mode == ORC_MODE_SMC) {
@@ -524,7 +528,7 @@ int orc_smc_run(int L, double m0sq, double lam, int N, uint64_t seed, int k,
     int st = orc_cov_chol(phi, N, V, Sigma, Lc);
     if (st < 0) { rc = -1; break; }
     orc_mutate(phi, S, U0, N, L, m0sq, lam, Lc, s, beta_new, ORC_MODE_SMC, 0.0,
-               seed, ORC_TAG_PROP, ORC_TAG_ACC, t + 1, k, acc, NULL, NULL);
+               seed, ORC_TAG_PROP, ORC_TAG_ACC, t + 1, k, acc, NULL, NULL, NULL);
     t += (uint32_t)k;
     double nacc = 0.0;
     for (size_t m = 0; m < (size_t)k * N; ++m) nacc += acc[m];
@@ -642,7 +646,8 @@ int orc_ns_run(int L, double m0sq, double lam, int n, int k_del, int n_walk,
     }
     orc_mutate(wphi, wS, wU, k_del, L, m0sq, lam, Lc, s, 0.0, ORC_MODE_NS,
                S_star, seed, ORC_TAG_NS_PROP, ORC_TAG_NS_ACC,
-               (uint32_t)it * (uint32_t)n_walk + 1u, n_walk, acc, NULL, NULL);
+               (uint32_t)it * (uint32_t)n_walk + 1u, n_walk, acc, NULL, NULL,
+               NULL);
     for (int j = 0; j < k_del; ++j) {
       int d = dead[j];
       for (int x = 0; x < V; ++x)

@@ -1,0 +1,675 @@
+// api.cu -- the C ABI of include/phi4smc.h: handle, workspace carve-up, step sequencing.
+// No torch types, no device allocation: all device state lives in the caller's workspace.
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <new>
+
+#include "../../include/phi4smc.h"
+#include "kernels.cuh"
+
+#define PHI4_API extern "C" __attribute__((visibility("default")))
+
+using namespace phi4;
+
+namespace {
+constexpr int KIND_SMC = 0, KIND_NS = 1;
+constexpr int MAX_RECORDS = 4096;       // per-temperature records kept on the device (SMC)
+constexpr size_t ALIGN = 256;
+
+struct Carver {                         // bump allocator over the caller's workspace
+  char* base;
+  size_t off;
+  template <typename T>
+  T* take(size_t count) {
+    off = (off + ALIGN - 1) / ALIGN * ALIGN;
+    T* p = base ? reinterpret_cast<T*>(base + off) : nullptr;
+    off += count * sizeof(T);
+    return p;
+  }
+};
+}  // namespace
+
+struct phi4smc {
+  int kind;
+  Model md;
+  int N, ld;                 // particles (n_live for NS) and padded stride
+  uint64_t seed;
+  smc_params prm;
+  float s;                   // step scale actually used
+  cudaStream_t st;
+  // device state (inside the workspace)
+  float* phi[2]; float* S[2]; float* U0[2];
+  int cur;
+  float *phip, *Z, *w, *mu, *Sigma, *Lc, *partial, *M, *margins;
+  unsigned long long* C;
+  int32_t* anc;
+  uint8_t* acc_flags;
+  Ctrl* ctrl;
+  StepRecord* rec;
+  int max_rec;
+  double* obs_out;
+  // nested sampling
+  int k_del, n_walk, max_iters, ldw;
+  double stop_frac;
+  float *wphi, *wS, *wU, *dead_S, *dead_M, *M_all, *S_all;
+  double *dead_logw, *logw_all;
+  int32_t *dead, *surv, *start;
+  // host side
+  uint64_t step_counter;     // mutation steps enqueued so far (next step uses counter + 1)
+  uint32_t iters_enqueued;   // NS iterations enqueued
+  int known_done;
+  Ctrl* h_ctrl;              // pinned staging
+  StepRecord* h_rec;         // pinned staging (one record)
+  double* h_obs;             // pinned staging (85 doubles)
+  char err[256];
+};
+
+#define CU(call)                                                                     \
+  do {                                                                               \
+    cudaError_t e_ = (call);                                                         \
+    if (e_ != cudaSuccess) {                                                         \
+      snprintf(h->err, sizeof(h->err), "%s: %s", #call, cudaGetErrorString(e_));     \
+      return PHI4_ECUDA;                                                             \
+    }                                                                                \
+  } while (0)
+
+static int carve_smc(phi4smc* h, char* base, size_t* total) {
+  const int V = h->md.V, ld = h->ld, N = h->N;
+  Carver c{base, 0};
+  const size_t field = (size_t)V * ld;
+  for (int b = 0; b < 2; ++b) {
+    h->phi[b] = c.take<float>(field);
+    h->S[b] = c.take<float>(ld);
+    h->U0[b] = c.take<float>(ld);
+  }
+  h->phip = c.take<float>(field);
+  h->Z = c.take<float>(field);
+  h->w = c.take<float>(ld);
+  h->M = c.take<float>(ld);
+  h->C = c.take<unsigned long long>(ld);
+  h->anc = c.take<int32_t>(ld);
+  h->mu = c.take<float>(V);
+  h->Sigma = c.take<float>((size_t)V * V);
+  h->Lc = c.take<float>((size_t)V * V);
+  h->partial = c.take<float>(cov_partial_floats(V, N));
+  h->acc_flags = c.take<uint8_t>((size_t)PHI4_MAX_HOOK_STEPS * N);
+  h->margins = c.take<float>((size_t)PHI4_MAX_HOOK_STEPS * N);
+  h->ctrl = c.take<Ctrl>(1);
+  h->rec = c.take<StepRecord>(h->max_rec);
+  h->obs_out = c.take<double>(5 + PHI4_HIST_BINS);
+  *total = c.off + ALIGN;
+  return 0;
+}
+
+static int carve_ns(phi4smc* h, char* base, size_t* total) {
+  const int V = h->md.V, ld = h->ld, N = h->N, kd = h->k_del, ldw = h->ldw;
+  Carver c{base, 0};
+  h->phi[0] = c.take<float>((size_t)V * ld);
+  h->S[0] = c.take<float>(ld);
+  h->U0[0] = c.take<float>(ld);
+  h->phi[1] = nullptr; h->S[1] = nullptr; h->U0[1] = nullptr;
+  h->wphi = c.take<float>((size_t)V * ldw);
+  h->wS = c.take<float>(ldw);
+  h->wU = c.take<float>(ldw);
+  h->phip = c.take<float>((size_t)V * ldw);
+  h->Z = c.take<float>((size_t)V * ldw);
+  h->mu = c.take<float>(V);
+  h->Sigma = c.take<float>((size_t)V * V);
+  h->Lc = c.take<float>((size_t)V * V);
+  h->partial = c.take<float>(cov_partial_floats(V, N));
+  h->dead = c.take<int32_t>(kd);
+  h->surv = c.take<int32_t>(N);
+  h->start = c.take<int32_t>(kd);
+  const size_t nlog = (size_t)h->max_iters * kd;
+  h->dead_S = c.take<float>(nlog);
+  h->dead_M = c.take<float>(nlog);
+  h->dead_logw = c.take<double>(nlog);
+  h->M_all = c.take<float>(nlog + N);
+  h->S_all = c.take<float>(nlog + N);
+  h->logw_all = c.take<double>(nlog + N);
+  h->acc_flags = c.take<uint8_t>((size_t)PHI4_MAX_HOOK_STEPS * kd);
+  h->margins = c.take<float>((size_t)PHI4_MAX_HOOK_STEPS * kd);
+  h->ctrl = c.take<Ctrl>(1);
+  h->rec = c.take<StepRecord>(h->max_rec);
+  h->obs_out = c.take<double>(5 + PHI4_HIST_BINS);
+  *total = c.off + ALIGN;
+  return 0;
+}
+
+static phi4smc* new_handle(int kind, int L, float m0sq, float lambda, int N, uint64_t seed) {
+  phi4smc* h = new (std::nothrow) phi4smc;
+  if (!h) return nullptr;
+  memset(h, 0, sizeof(*h));
+  h->kind = kind;
+  h->md.L = L; h->md.V = L * L; h->md.m0sq = m0sq; h->md.lam = lambda;
+  h->N = N; h->ld = round_up(N, 128);
+  h->seed = seed;
+  h->prm.k_steps = 10; h->prm.ess_target = 0.5f; h->prm.step_scale = 0.f; h->prm.mutation_path = 0;
+  h->s = 2.38f / sqrtf((float)h->md.V);
+  return h;
+}
+
+PHI4_API const char* phi4_strerror(int code) {
+  switch (code) {
+    case PHI4_OK: return "ok";
+    case PHI4_EINVAL: return "invalid argument";
+    case PHI4_ENOMEM: return "out of host memory";
+    case PHI4_ENOTPD: return "particle covariance not positive definite";
+    case PHI4_ENAN: return "non-finite action or weight";
+    case PHI4_ECUDA: return "CUDA error or no device";
+    default: return "unknown error";
+  }
+}
+
+PHI4_API const char* phi4_last_cuda_error(const phi4smc* h) { return h ? h->err : ""; }
+
+PHI4_API size_t smc_workspace_bytes(int L, int N) {
+  if (L < 1 || N < 2 || L > 4096) return 0;
+  phi4smc tmp;
+  memset(&tmp, 0, sizeof(tmp));
+  tmp.md.L = L; tmp.md.V = L * L; tmp.N = N; tmp.ld = round_up(N, 128); tmp.max_rec = MAX_RECORDS;
+  size_t total = 0;
+  carve_smc(&tmp, nullptr, &total);
+  return total;
+}
+
+PHI4_API size_t ns_workspace_bytes(int L, int n_live, int k_delete, int max_iters) {
+  if (L < 1 || n_live < 2 || k_delete < 1 || k_delete >= n_live || max_iters < 1) return 0;
+  phi4smc tmp;
+  memset(&tmp, 0, sizeof(tmp));
+  tmp.md.L = L; tmp.md.V = L * L; tmp.N = n_live; tmp.ld = round_up(n_live, 128);
+  tmp.k_del = k_delete; tmp.ldw = round_up(k_delete, 128); tmp.max_iters = max_iters;
+  tmp.max_rec = max_iters;
+  size_t total = 0;
+  carve_ns(&tmp, nullptr, &total);
+  return total;
+}
+
+static int host_staging(phi4smc* h) {
+  CU(cudaMallocHost((void**)&h->h_ctrl, sizeof(Ctrl)));
+  CU(cudaMallocHost((void**)&h->h_rec, sizeof(StepRecord)));
+  CU(cudaMallocHost((void**)&h->h_obs, sizeof(double) * (5 + PHI4_HIST_BINS)));
+  return PHI4_OK;
+}
+
+static int have_device(phi4smc* h) {
+  int n = 0;
+  cudaError_t e = cudaGetDeviceCount(&n);
+  if (e != cudaSuccess || n < 1) {
+    snprintf(h->err, sizeof(h->err), "no CUDA device: %s", cudaGetErrorString(e));
+    return PHI4_ECUDA;
+  }
+  return PHI4_OK;
+}
+
+// Pull the control block to the host (synchronises) and map device flags to error codes.
+static int sync_ctrl(phi4smc* h) {
+  CU(cudaMemcpyAsync(h->h_ctrl, h->ctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost, h->st));
+  CU(cudaStreamSynchronize(h->st));
+  CU(cudaGetLastError());
+  if (h->h_ctrl->done) h->known_done = 1;
+  if (h->h_ctrl->nan_flag) return PHI4_ENAN;
+  if (h->h_ctrl->chol_status < 0) return PHI4_ENOTPD;
+  return PHI4_OK;
+}
+
+static int push_ctrl(phi4smc* h) {
+  CU(cudaMemcpyAsync(h->ctrl, h->h_ctrl, sizeof(Ctrl), cudaMemcpyHostToDevice, h->st));
+  CU(cudaStreamSynchronize(h->st));
+  return PHI4_OK;
+}
+
+// ------------------------------------------------------------------------------ SMC ----------
+PHI4_API int smc_init(phi4smc** out, int L, float m0sq, float lambda, int N, uint64_t seed,
+                        void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (!out) return PHI4_EINVAL;
+  *out = nullptr;
+  size_t need = smc_workspace_bytes(L, N);
+  if (need == 0 || !d_workspace || workspace_bytes < need ||
+      (reinterpret_cast<uintptr_t>(d_workspace) % ALIGN) != 0)
+    return PHI4_EINVAL;
+  phi4smc* h = new_handle(KIND_SMC, L, m0sq, lambda, N, seed);
+  if (!h) return PHI4_ENOMEM;
+  h->st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  h->max_rec = MAX_RECORDS;
+  int rc = have_device(h);
+  if (rc == PHI4_OK) rc = host_staging(h);
+  if (rc != PHI4_OK) { delete h; return rc; }
+  size_t total;
+  carve_smc(h, static_cast<char*>(d_workspace), &total);
+  *out = h;
+  CU(cudaMemsetAsync(d_workspace, 0, need, h->st));
+  launch_init_particles(h->phi[0], N, h->ld, h->md.V, seed, h->st);
+  launch_action(h->phi[0], N, h->ld, h->md, h->S[0], h->U0[0], h->ctrl, h->st);
+  launch_set_identity(h->Lc, h->md.V, h->st);
+  CU(cudaGetLastError());
+  return PHI4_OK;
+}
+
+PHI4_API int smc_reset(phi4smc* h, uint64_t seed) {
+  if (!h) return PHI4_EINVAL;
+  h->seed = seed;
+  h->cur = 0;
+  h->step_counter = 0;
+  h->iters_enqueued = 0;
+  h->known_done = 0;
+  // h_ctrl is pinned staging that an earlier async copy may still be reading: use a memset for
+  // the zero state and a tiny kernel-free patch for the NS evidence (-inf) via a second copy.
+  CU(cudaMemsetAsync(h->ctrl, 0, sizeof(Ctrl), h->st));
+  if (h->kind == KIND_NS) {
+    static const double neg_inf = -INFINITY;
+    CU(cudaMemcpyAsync(&h->ctrl->logZ, &neg_inf, sizeof(double), cudaMemcpyHostToDevice, h->st));
+  }
+  launch_init_particles(h->phi[0], h->N, h->ld, h->md.V, seed, h->st);
+  launch_action(h->phi[0], h->N, h->ld, h->md, h->S[0], h->U0[0], h->ctrl, h->st);
+  launch_set_identity(h->Lc, h->md.V, h->st);
+  CU(cudaGetLastError());
+  return PHI4_OK;
+}
+
+PHI4_API int smc_destroy(phi4smc* h) {
+  if (!h) return PHI4_OK;
+  cudaStreamSynchronize(h->st);
+  if (h->h_ctrl) cudaFreeHost(h->h_ctrl);
+  if (h->h_rec) cudaFreeHost(h->h_rec);
+  if (h->h_obs) cudaFreeHost(h->h_obs);
+  delete h;
+  return PHI4_OK;
+}
+
+PHI4_API int smc_set_params(phi4smc* h, const smc_params* p) {
+  if (!h || !p) return PHI4_EINVAL;
+  if (p->k_steps < 1 || !(p->ess_target > 0.f && p->ess_target < 1.f) || p->step_scale < 0.f ||
+      p->mutation_path < 0 || p->mutation_path > 2)
+    return PHI4_EINVAL;
+  h->prm = *p;
+  h->s = p->step_scale > 0.f ? p->step_scale : 2.38f / sqrtf((float)h->md.V);
+  return PHI4_OK;
+}
+
+static MutateArgs smc_mutate_args(phi4smc* h, int k, uint8_t* acc, float* mar, int respect_done) {
+  MutateArgs a;
+  a.phi = h->phi[h->cur]; a.phip = h->phip; a.Z = h->Z;
+  a.S = h->S[h->cur]; a.U0 = h->U0[h->cur]; a.Lc = h->Lc; a.ctrl = h->ctrl;
+  a.acc_out = acc; a.margin_out = mar;
+  a.N = h->N; a.ld = h->ld; a.md = h->md; a.s = h->s; a.mode = MODE_SMC; a.seed = h->seed;
+  a.tag_prop = TAG_PROP; a.tag_acc = TAG_ACC;
+  a.t0 = (uint32_t)(h->step_counter + 1); a.k = k; a.respect_done = respect_done;
+  return a;
+}
+
+static void enqueue_mutation(phi4smc* h, const MutateArgs& a) {
+  launch_mutate_generic(a, h->st);
+}
+
+static CovCholArgs cov_args(phi4smc* h, int respect_done) {
+  CovCholArgs c;
+  c.phi = h->phi[h->cur]; c.N = h->N; c.ld = h->ld; c.V = h->md.V;
+  c.mu = h->mu; c.Sigma = h->Sigma; c.Lc = h->Lc; c.partial = h->partial; c.ctrl = h->ctrl;
+  c.respect_done = respect_done;
+  return c;
+}
+
+static void enqueue_resample(phi4smc* h) {
+  launch_quantise_scan(h->w, h->N, h->C, h->ctrl, h->st);
+  launch_ancestors(h->C, h->N, h->seed, h->anc, h->ctrl, h->st);
+  const int o = h->cur ^ 1;
+  launch_gather(h->phi[h->cur], h->phi[o], h->S[h->cur], h->S[o], h->U0[h->cur], h->U0[o], h->anc,
+                h->N, h->ld, h->md.V, h->ctrl, h->st);
+  h->cur = o;
+}
+
+static void enqueue_smc_step(phi4smc* h) {
+  launch_next_delta_reweight(h->S[h->cur], h->N, h->prm.ess_target, -1.0, h->w, h->ctrl, h->st);
+  enqueue_resample(h);
+  launch_cov_chol(cov_args(h, 1), h->st);
+  enqueue_mutation(h, smc_mutate_args(h, h->prm.k_steps, nullptr, nullptr, 1));
+  h->step_counter += (uint64_t)h->prm.k_steps;
+  launch_finish_step(h->ctrl, h->rec, h->max_rec, h->prm.k_steps, h->N, h->st);
+}
+
+static void fill_info(const StepRecord& r, smc_step_info* info) {
+  info->beta = r.beta; info->delta = r.delta; info->ess_frac = r.ess_frac; info->dlogZ = r.dlogZ;
+  info->logZ = r.logZ; info->accept_rate = r.accept_rate; info->n_unique = r.n_unique;
+  info->chol_status = r.chol_status; info->temp_index = r.index; info->done = r.done;
+}
+
+static int fetch_record(phi4smc* h, int index, StepRecord* out) {
+  if (index < 0 || index >= h->max_rec) return PHI4_EINVAL;
+  CU(cudaMemcpyAsync(h->h_rec, h->rec + index, sizeof(StepRecord), cudaMemcpyDeviceToHost, h->st));
+  CU(cudaStreamSynchronize(h->st));
+  *out = *h->h_rec;
+  return PHI4_OK;
+}
+
+PHI4_API int smc_step(phi4smc* h, smc_step_info* info) {
+  if (!h || h->kind != KIND_SMC) return PHI4_EINVAL;
+  if (!h->known_done) enqueue_smc_step(h);
+  if (!info) {
+    CU(cudaGetLastError());
+    return PHI4_OK;
+  }
+  int rc = sync_ctrl(h);
+  if (rc == PHI4_ECUDA) return rc;
+  memset(info, 0, sizeof(*info));
+  int last = h->h_ctrl->temp_index - 1;
+  if (last >= 0) {
+    StepRecord r;
+    int rr = fetch_record(h, last < h->max_rec ? last : h->max_rec - 1, &r);
+    if (rr != PHI4_OK) return rr;
+    fill_info(r, info);
+  }
+  info->done = h->h_ctrl->done ? 1 : 0;
+  return rc;
+}
+
+PHI4_API int smc_run(phi4smc* h, int max_temps, int* n_temps) {
+  if (!h || h->kind != KIND_SMC || max_temps < 0) return PHI4_EINVAL;
+  int rc = sync_ctrl(h);
+  if (rc != PHI4_OK) return rc;
+  const int start = h->h_ctrl->temp_index;
+  int enq = 0;
+  while (!h->known_done && enq < max_temps) {
+    // the device decides when beta hits 1; the host polls the control block between batches
+    int batch = 1;
+    for (int b = 0; b < batch && enq < max_temps; ++b, ++enq) enqueue_smc_step(h);
+    rc = sync_ctrl(h);
+    if (rc != PHI4_OK) break;
+  }
+  const int made = h->h_ctrl->temp_index - start;
+  // steps enqueued past beta = 1 were no-ops: take them out of the step counter
+  if (enq > made) h->step_counter -= (uint64_t)(enq - made) * (uint64_t)h->prm.k_steps;
+  if (n_temps) *n_temps = made;
+  return rc;
+}
+
+PHI4_API int smc_get_history(phi4smc* h, smc_step_info* h_info, int cap, int* n) {
+  if (!h || h->kind != KIND_SMC) return PHI4_EINVAL;
+  int rc = sync_ctrl(h);
+  if (rc == PHI4_ECUDA) return rc;
+  int avail = h->h_ctrl->temp_index < h->max_rec ? h->h_ctrl->temp_index : h->max_rec;
+  if (n) *n = avail;
+  int m = avail < cap ? avail : cap;
+  if (h_info && m > 0) {
+    StepRecord* tmp = (StepRecord*)malloc(sizeof(StepRecord) * m);
+    if (!tmp) return PHI4_ENOMEM;
+    cudaError_t e = cudaMemcpy(tmp, h->rec, sizeof(StepRecord) * m, cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) { free(tmp); snprintf(h->err, sizeof(h->err), "history: %s", cudaGetErrorString(e)); return PHI4_ECUDA; }
+    for (int i = 0; i < m; ++i) fill_info(tmp[i], &h_info[i]);
+    free(tmp);
+  }
+  return PHI4_OK;
+}
+
+PHI4_API int estimate_cov_chol(phi4smc* h) {
+  if (!h) return PHI4_EINVAL;
+  launch_cov_chol(cov_args(h, 0), h->st);
+  CU(cudaGetLastError());
+  return PHI4_OK;
+}
+
+static NsArgs ns_args(phi4smc* h);
+
+PHI4_API int observables(phi4smc* h, phi4_observables* out) {
+  if (!h || !out) return PHI4_EINVAL;
+  const int V = h->md.V;
+  if (h->kind == KIND_SMC) {
+    launch_magnetisation(h->phi[h->cur], h->N, h->ld, V, h->M, h->st);
+    launch_observables_reduce(h->M, h->S[h->cur], nullptr, h->N, V, h->obs_out, h->st);
+  } else {
+    int rc = sync_ctrl(h);
+    if (rc == PHI4_ECUDA) return rc;
+    int iters = h->h_ctrl->temp_index < h->max_iters ? h->h_ctrl->temp_index : h->max_iters;
+    int n_dead = iters * h->k_del;
+    launch_magnetisation(h->phi[0], h->N, h->ld, V, h->M_all + n_dead, h->st);
+    launch_ns_obs_inputs(ns_args(h), n_dead, h->M_all, h->S_all, h->logw_all, h->st);
+    launch_observables_reduce(h->M_all, h->S_all, h->logw_all, n_dead + h->N, V, h->obs_out, h->st);
+  }
+  CU(cudaMemcpyAsync(h->h_obs, h->obs_out, sizeof(double) * (5 + PHI4_HIST_BINS),
+                     cudaMemcpyDeviceToHost, h->st));
+  CU(cudaStreamSynchronize(h->st));
+  CU(cudaGetLastError());
+  out->absM = h->h_obs[0]; out->M2 = h->h_obs[1]; out->chi = h->h_obs[2];
+  out->mean_SE = h->h_obs[3]; out->mode_balance = h->h_obs[4];
+  for (int b = 0; b < PHI4_HIST_BINS; ++b) out->hist[b] = h->h_obs[5 + b];
+  return PHI4_OK;
+}
+
+PHI4_API double log_Z(const phi4smc* hc) {
+  phi4smc* h = const_cast<phi4smc*>(hc);
+  if (!h) return NAN;
+  if (sync_ctrl(h) == PHI4_ECUDA) return NAN;
+  return h->h_ctrl->logZ;
+}
+
+// ------------------------------------------------------------------- nested sampling ---------
+static NsArgs ns_args(phi4smc* h) {
+  NsArgs a;
+  a.phi = h->phi[0]; a.S = h->S[0]; a.U0 = h->U0[0];
+  a.wphi = h->wphi; a.wS = h->wS; a.wU = h->wU;
+  a.n = h->N; a.ld = h->ld; a.k_del = h->k_del; a.ldw = h->ldw; a.V = h->md.V;
+  a.seed = h->seed; a.dead = h->dead; a.surv = h->surv; a.start = h->start;
+  a.dead_S = h->dead_S; a.dead_M = h->dead_M; a.dead_logw = h->dead_logw;
+  a.max_iters = h->max_iters; a.stop_frac = h->stop_frac; a.ctrl = h->ctrl;
+  return a;
+}
+
+PHI4_API int ns_init(phi4smc** out, int L, float m0sq, float lambda, int n_live, int k_delete,
+                       int n_walk, uint64_t seed, double stop_frac, int max_iters,
+                       void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (!out) return PHI4_EINVAL;
+  *out = nullptr;
+  if (n_live > 16384 || k_delete > 1024 || n_walk < 1 || !(stop_frac > 0.0)) return PHI4_EINVAL;
+  size_t need = ns_workspace_bytes(L, n_live, k_delete, max_iters);
+  if (need == 0 || !d_workspace || workspace_bytes < need ||
+      (reinterpret_cast<uintptr_t>(d_workspace) % ALIGN) != 0)
+    return PHI4_EINVAL;
+  phi4smc* h = new_handle(KIND_NS, L, m0sq, lambda, n_live, seed);
+  if (!h) return PHI4_ENOMEM;
+  h->st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  h->k_del = k_delete; h->ldw = round_up(k_delete, 128); h->n_walk = n_walk;
+  h->max_iters = max_iters; h->max_rec = max_iters; h->stop_frac = stop_frac;
+  int rc = have_device(h);
+  if (rc == PHI4_OK) rc = host_staging(h);
+  if (rc != PHI4_OK) { delete h; return rc; }
+  size_t total;
+  carve_ns(h, static_cast<char*>(d_workspace), &total);
+  *out = h;
+  CU(cudaMemsetAsync(d_workspace, 0, need, h->st));
+  memset(h->h_ctrl, 0, sizeof(Ctrl));
+  h->h_ctrl->logZ = -INFINITY;
+  CU(cudaMemcpyAsync(h->ctrl, h->h_ctrl, sizeof(Ctrl), cudaMemcpyHostToDevice, h->st));
+  launch_init_particles(h->phi[0], n_live, h->ld, h->md.V, seed, h->st);
+  launch_action(h->phi[0], n_live, h->ld, h->md, h->S[0], h->U0[0], h->ctrl, h->st);
+  launch_set_identity(h->Lc, h->md.V, h->st);
+  CU(cudaStreamSynchronize(h->st));
+  CU(cudaGetLastError());
+  return PHI4_OK;
+}
+
+static void enqueue_ns_step(phi4smc* h) {
+  NsArgs a = ns_args(h);
+  launch_cov_chol(cov_args(h, 1), h->st);
+  launch_ns_select_evidence(a, h->st);
+  launch_ns_load_walkers(a, h->st);
+  MutateArgs m;
+  m.phi = h->wphi; m.phip = h->phip; m.Z = h->Z; m.S = h->wS; m.U0 = h->wU; m.Lc = h->Lc;
+  m.ctrl = h->ctrl; m.acc_out = nullptr; m.margin_out = nullptr;
+  m.N = h->k_del; m.ld = h->ldw; m.md = h->md; m.s = h->s; m.mode = MODE_NS; m.seed = h->seed;
+  m.tag_prop = TAG_NS_PROP; m.tag_acc = TAG_NS_ACC;
+  m.t0 = h->iters_enqueued * (uint32_t)h->n_walk + 1u; m.k = h->n_walk; m.respect_done = 1;
+  enqueue_mutation(h, m);
+  launch_ns_store_walkers(a, h->st);
+  launch_ns_finish(a, h->rec, h->n_walk, h->st);
+  h->iters_enqueued += 1;
+}
+
+static void fill_ns_info(const StepRecord& r, ns_step_info* info) {
+  info->logX = r.beta; info->S_star = r.delta; info->remaining_frac = r.ess_frac;
+  info->logZ = r.logZ; info->accept_rate = r.accept_rate; info->chol_status = r.chol_status;
+  info->iter_index = r.index; info->done = r.done;
+}
+
+PHI4_API int ns_step(phi4smc* h, ns_step_info* info) {
+  if (!h || h->kind != KIND_NS) return PHI4_EINVAL;
+  if (!h->known_done) enqueue_ns_step(h);
+  if (!info) {
+    CU(cudaGetLastError());
+    return PHI4_OK;
+  }
+  int rc = sync_ctrl(h);
+  if (rc == PHI4_ECUDA) return rc;
+  memset(info, 0, sizeof(*info));
+  int last = h->h_ctrl->temp_index - 1;
+  if (last >= 0 && last < h->max_rec) {
+    StepRecord r;
+    int rr = fetch_record(h, last, &r);
+    if (rr != PHI4_OK) return rr;
+    fill_ns_info(r, info);
+  }
+  info->done = h->h_ctrl->done ? 1 : 0;
+  return rc;
+}
+
+PHI4_API int ns_run(phi4smc* h, int max_iters, int* n_iters) {
+  if (!h || h->kind != KIND_NS || max_iters < 0) return PHI4_EINVAL;
+  int rc = sync_ctrl(h);
+  if (rc != PHI4_OK) return rc;
+  const int start = h->h_ctrl->temp_index;
+  int enq = 0;
+  while (!h->known_done && enq < max_iters) {
+    int batch = 8;   // iterations are short and latency-bound: poll the stop flag every 8
+    for (int b = 0; b < batch && enq < max_iters; ++b, ++enq) enqueue_ns_step(h);
+    rc = sync_ctrl(h);
+    if (rc != PHI4_OK) break;
+  }
+  const int made = h->h_ctrl->temp_index - start;
+  if (enq > made) h->iters_enqueued -= (uint32_t)(enq - made);
+  if (n_iters) *n_iters = made;
+  return rc;
+}
+
+PHI4_API int ns_get_dead(phi4smc* h, int32_t* h_last_dead_idx, float* h_dead_S, float* h_dead_M,
+                           double* h_dead_logw, int cap, int* n_dead) {
+  if (!h || h->kind != KIND_NS) return PHI4_EINVAL;
+  int rc = sync_ctrl(h);
+  if (rc == PHI4_ECUDA) return rc;
+  int iters = h->h_ctrl->temp_index < h->max_iters ? h->h_ctrl->temp_index : h->max_iters;
+  int nd = iters * h->k_del;
+  if (n_dead) *n_dead = nd;
+  int m = nd < cap ? nd : cap;
+  if (h_last_dead_idx) CU(cudaMemcpy(h_last_dead_idx, h->dead, sizeof(int32_t) * h->k_del, cudaMemcpyDeviceToHost));
+  if (h_dead_S && m > 0) CU(cudaMemcpy(h_dead_S, h->dead_S, sizeof(float) * m, cudaMemcpyDeviceToHost));
+  if (h_dead_M && m > 0) CU(cudaMemcpy(h_dead_M, h->dead_M, sizeof(float) * m, cudaMemcpyDeviceToHost));
+  if (h_dead_logw && m > 0) CU(cudaMemcpy(h_dead_logw, h->dead_logw, sizeof(double) * m, cudaMemcpyDeviceToHost));
+  return PHI4_OK;
+}
+
+// ------------------------------------------------------------------------ hooks --------------
+PHI4_API int smc_get_state(phi4smc* h, float* h_phi, float* h_SE, float* h_U0, double* beta,
+                             uint64_t* step_counter) {
+  if (!h) return PHI4_EINVAL;
+  int rc = sync_ctrl(h);
+  if (rc == PHI4_ECUDA) return rc;
+  const int V = h->md.V, N = h->N, c = h->cur;
+  if (h_phi)
+    CU(cudaMemcpy2D(h_phi, sizeof(float) * N, h->phi[c], sizeof(float) * h->ld, sizeof(float) * N,
+                    V, cudaMemcpyDeviceToHost));
+  if (h_SE) CU(cudaMemcpy(h_SE, h->S[c], sizeof(float) * N, cudaMemcpyDeviceToHost));
+  if (h_U0) CU(cudaMemcpy(h_U0, h->U0[c], sizeof(float) * N, cudaMemcpyDeviceToHost));
+  if (beta) *beta = h->h_ctrl->beta;
+  if (step_counter)
+    *step_counter = h->kind == KIND_SMC ? h->step_counter
+                                        : (uint64_t)h->iters_enqueued * (uint64_t)h->n_walk;
+  return PHI4_OK;
+}
+
+PHI4_API int smc_set_state(phi4smc* h, const float* h_phi, double beta, uint64_t step_counter) {
+  if (!h || !h_phi || !(beta >= 0.0 && beta <= 1.0)) return PHI4_EINVAL;
+  int rc = sync_ctrl(h);
+  if (rc == PHI4_ECUDA) return rc;
+  const int V = h->md.V, N = h->N, c = h->cur;
+  CU(cudaMemcpy2DAsync(h->phi[c], sizeof(float) * h->ld, h_phi, sizeof(float) * N,
+                       sizeof(float) * N, V, cudaMemcpyHostToDevice, h->st));
+  h->h_ctrl->beta = beta;
+  h->h_ctrl->done = (h->kind == KIND_SMC && beta >= 1.0) ? 1 : 0;
+  h->h_ctrl->nan_flag = 0;
+  h->known_done = h->h_ctrl->done;
+  rc = push_ctrl(h);
+  if (rc != PHI4_OK) return rc;
+  launch_action(h->phi[c], N, h->ld, h->md, h->S[c], h->U0[c], h->ctrl, h->st);
+  if (h->kind == KIND_SMC) h->step_counter = step_counter;
+  else h->iters_enqueued = (uint32_t)(step_counter / (uint64_t)h->n_walk);
+  CU(cudaStreamSynchronize(h->st));
+  CU(cudaGetLastError());
+  return PHI4_OK;
+}
+
+PHI4_API int smc_get_chol(phi4smc* h, float* h_Lc) {
+  if (!h || !h_Lc) return PHI4_EINVAL;
+  CU(cudaStreamSynchronize(h->st));
+  CU(cudaMemcpy(h_Lc, h->Lc, sizeof(float) * h->md.V * h->md.V, cudaMemcpyDeviceToHost));
+  return PHI4_OK;
+}
+
+PHI4_API int smc_set_chol(phi4smc* h, const float* h_Lc) {
+  if (!h || !h_Lc) return PHI4_EINVAL;
+  CU(cudaMemcpyAsync(h->Lc, h_Lc, sizeof(float) * h->md.V * h->md.V, cudaMemcpyHostToDevice, h->st));
+  launch_zero_upper(h->Lc, h->md.V, h->st);
+  CU(cudaStreamSynchronize(h->st));
+  return PHI4_OK;
+}
+
+PHI4_API int smc_get_cov(phi4smc* h, float* h_Sigma) {
+  if (!h || !h_Sigma) return PHI4_EINVAL;
+  CU(cudaStreamSynchronize(h->st));
+  CU(cudaMemcpy(h_Sigma, h->Sigma, sizeof(float) * h->md.V * h->md.V, cudaMemcpyDeviceToHost));
+  return PHI4_OK;
+}
+
+PHI4_API int smc_mutate(phi4smc* h, int k, uint8_t* h_accept, float* h_margin) {
+  if (!h || h->kind != KIND_SMC || k < 1) return PHI4_EINVAL;
+  const bool want = h_accept || h_margin;
+  if (want && k > PHI4_MAX_HOOK_STEPS) return PHI4_EINVAL;
+  launch_reset_counters(h->ctrl, h->st);
+  enqueue_mutation(h, smc_mutate_args(h, k, want ? h->acc_flags : nullptr,
+                                      want ? h->margins : nullptr, 0));
+  h->step_counter += (uint64_t)k;
+  const size_t n = (size_t)k * h->N;
+  if (h_accept) CU(cudaMemcpyAsync(h_accept, h->acc_flags, n, cudaMemcpyDeviceToHost, h->st));
+  if (h_margin) CU(cudaMemcpyAsync(h_margin, h->margins, n * sizeof(float), cudaMemcpyDeviceToHost, h->st));
+  launch_reset_counters(h->ctrl, h->st);
+  CU(cudaStreamSynchronize(h->st));
+  CU(cudaGetLastError());
+  return PHI4_OK;
+}
+
+PHI4_API int smc_reweight(phi4smc* h, double delta, float* h_w, smc_step_info* info) {
+  if (!h || h->kind != KIND_SMC) return PHI4_EINVAL;
+  launch_next_delta_reweight(h->S[h->cur], h->N, h->prm.ess_target, delta < 0.0 ? -1.0 : delta,
+                             h->w, h->ctrl, h->st);
+  if (h_w) CU(cudaMemcpyAsync(h_w, h->w, sizeof(float) * h->N, cudaMemcpyDeviceToHost, h->st));
+  int rc = sync_ctrl(h);
+  if (rc == PHI4_ECUDA) return rc;
+  if (info) {
+    memset(info, 0, sizeof(*info));
+    info->beta = h->h_ctrl->beta; info->delta = h->h_ctrl->delta;
+    info->ess_frac = h->h_ctrl->ess_frac; info->dlogZ = h->h_ctrl->dlogZ;
+    info->logZ = h->h_ctrl->logZ; info->temp_index = h->h_ctrl->temp_index;
+    info->done = h->h_ctrl->beta >= 1.0;
+  }
+  return rc;
+}
+
+PHI4_API int smc_resample(phi4smc* h, const float* h_w, int32_t* h_ancestors) {
+  if (!h || h->kind != KIND_SMC) return PHI4_EINVAL;
+  if (h_w) CU(cudaMemcpyAsync(h->w, h_w, sizeof(float) * h->N, cudaMemcpyHostToDevice, h->st));
+  launch_reset_counters(h->ctrl, h->st);
+  enqueue_resample(h);
+  if (h_ancestors)
+    CU(cudaMemcpyAsync(h_ancestors, h->anc, sizeof(int32_t) * h->N, cudaMemcpyDeviceToHost, h->st));
+  return sync_ctrl(h);
+}

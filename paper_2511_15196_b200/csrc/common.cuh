@@ -1,0 +1,83 @@
+// common.cuh -- shared declarations of the sm_100a kernels behind include/phi4smc.h.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace phi4 {
+
+// Philox stream tags (reading R1).
+enum : uint32_t {
+  TAG_INIT = 0, TAG_PROP = 1, TAG_ACC = 2, TAG_RESAMPLE = 3,
+  TAG_NS_START = 4, TAG_NS_PROP = 5, TAG_NS_ACC = 6
+};
+enum : int { MODE_SMC = 0, MODE_NS = 1 };
+
+// Device-resident control block: everything a temperature / NS iteration decides lives here so
+// that a step can be enqueued without a host round trip.
+struct Ctrl {
+  double beta;        // current inverse temperature
+  double delta;       // last increment
+  double ess_frac;    // ESS/N at delta
+  double dlogZ;
+  double logZ;        // SMC: running sum; NS: log evidence from dead points (-inf at start)
+  double logX;        // NS: log prior volume
+  double S_star;      // NS: current threshold
+  double remaining;   // NS: remaining evidence fraction
+  float S_min;        // min S_E of the population at the last reweight
+  int done;           // beta == 1 (SMC) / stop rule fired (NS)
+  int temp_index;     // transitions / iterations completed
+  int chol_fail;      // bit 0: plain attempt hit a pivot <= 0; bit 1: the jittered retry did too
+  float trace;        // tr(Sigma) of the last covariance (jitter scale, reading A4)
+  int chol_status;    // 0 plain, 1 jitter used, -1 failed
+  int nan_flag;       // non-finite weight sum or action seen
+  unsigned int n_accept;  // acceptances of the current mutation batch
+  unsigned int n_unique;  // distinct ancestors of the last resampling
+  unsigned long long q_total;  // T of reading R5
+};
+
+// One record per temperature / iteration, written by the device at the end of each step.
+struct StepRecord {
+  double beta, delta, ess_frac, dlogZ, logZ, accept_rate;   // NS: logX, logZ, S_star, acc, rem
+  int n_unique, chol_status, index, done;
+};
+
+struct Model {
+  int L, V;
+  float m0sq, lam;
+};
+
+__host__ __device__ inline int round_up(int a, int b) { return (a + b - 1) / b * b; }
+
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+__device__ __forceinline__ float warp_min(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fminf(v, __shfl_xor_sync(0xffffffffu, v, o));
+  return v;
+}
+
+// Block-wide sum of doubles; result valid in every thread.  scratch: >= 33 doubles of smem.
+__device__ inline double block_sum(double v, double* scratch) {
+  int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+  v = warp_sum(v);
+  __syncthreads();
+  if (lane == 0) scratch[w] = v;
+  __syncthreads();
+  if (w == 0) {
+    double t = lane < nw ? scratch[lane] : 0.0;
+    t = warp_sum(t);
+    if (lane == 0) scratch[32] = t;
+  }
+  __syncthreads();
+  return scratch[32];
+}
+
+}  // namespace phi4

@@ -1,0 +1,348 @@
+// covchol.cu -- C1 (particle covariance) and C2 (Cholesky), readings A4 / R6.
+//   mu_x = (1/N) sum_i phi[x][i];  Sigma = (1/(N-1)) sum_i (phi_i - mu)(phi_i - mu)^T
+//   Sigma (+ jitter on retry) = Lc Lc^T, Lc lower-triangular, strict upper = 0.
+// FP32 SIMT version: 64x64 "NT" tiles (both operands contiguous along the contraction index),
+// lower-triangular tiles only, deterministic split-K for small V.  One CTA factorises V <= 160 in
+// shared memory; larger V use a blocked right-looking factorisation (64-wide panels: diagonal
+// block, row solves, trailing update with the same NT tile).
+#include "kernels.cuh"
+
+namespace phi4 {
+
+__global__ void __launch_bounds__(256)
+mean_kernel(const float* __restrict__ phi, int N, int ld, float* __restrict__ mu,
+            const Ctrl* ctrl, int respect_done) {
+  __shared__ double scratch[33];
+  if (respect_done && ctrl->done) return;
+  const float* row = phi + (size_t)blockIdx.x * ld;
+  double a = 0.0;
+  for (int i = threadIdx.x; i < N; i += blockDim.x) a += (double)row[i];
+  a = block_sum(a, scratch);
+  if (threadIdx.x == 0) mu[blockIdx.x] = (float)(a / (double)N);
+}
+
+// acc[p][r] += sum_{k in [kb,ke)} (A[(x0+ty*4+p)*lda + k] - mx) (A[(y0+tx*4+r)*lda + k] - my)
+// Rows >= M and columns k >= kvalid contribute zero.  VEC: lda % 4 == 0 and kb % 16 == 0.
+template <bool VEC>
+__device__ __forceinline__ void nt_tile(const float* __restrict__ A, size_t lda, int x0, int y0,
+                                        int M, int kb, int ke, int kvalid,
+                                        const float* __restrict__ mu, float (&acc)[4][4],
+                                        float (&As)[16][68], float (&Bs)[16][68]) {
+  const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
+  const int lr = threadIdx.x >> 2, lk = (threadIdx.x & 3) * 4;
+  const int xr = x0 + lr, yr = y0 + lr;
+  const float mx = (mu && xr < M) ? mu[xr] : 0.f;
+  const float my = (mu && yr < M) ? mu[yr] : 0.f;
+  for (int k0 = kb; k0 < ke; k0 += 16) {
+    float va[4], vb[4];
+    if (VEC) {
+      float4 a4 = make_float4(0.f, 0.f, 0.f, 0.f), b4 = a4;
+      if (xr < M) a4 = *reinterpret_cast<const float4*>(A + (size_t)xr * lda + k0 + lk);
+      if (yr < M) b4 = *reinterpret_cast<const float4*>(A + (size_t)yr * lda + k0 + lk);
+      va[0] = a4.x; va[1] = a4.y; va[2] = a4.z; va[3] = a4.w;
+      vb[0] = b4.x; vb[1] = b4.y; vb[2] = b4.z; vb[3] = b4.w;
+    } else {
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        int k = k0 + lk + j;
+        va[j] = (xr < M && k < ke) ? A[(size_t)xr * lda + k] : 0.f;
+        vb[j] = (yr < M && k < ke) ? A[(size_t)yr * lda + k] : 0.f;
+      }
+    }
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      int k = k0 + lk + j;
+      bool ok = k < kvalid && k < ke;
+      As[lk + j][lr] = (ok && xr < M) ? va[j] - mx : 0.f;
+      Bs[lk + j][lr] = (ok && yr < M) ? vb[j] - my : 0.f;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int kk = 0; kk < 16; ++kk) {
+      float a[4], b[4];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) { a[j] = As[kk][ty * 4 + j]; b[j] = Bs[kk][tx * 4 + j]; }
+#pragma unroll
+      for (int p = 0; p < 4; ++p)
+#pragma unroll
+        for (int r = 0; r < 4; ++r) acc[p][r] = fmaf(a[p], b[r], acc[p][r]);
+    }
+    __syncthreads();
+  }
+}
+
+// linear index t -> lower-triangular tile (tr, tc), tc <= tr
+__device__ __forceinline__ void tri_tile(int t, int& tr, int& tc) {
+  tr = (int)((sqrtf(8.f * (float)t + 1.f) - 1.f) * 0.5f);
+  while ((tr + 1) * (tr + 2) / 2 <= t) ++tr;
+  while (tr * (tr + 1) / 2 > t) --tr;
+  tc = t - tr * (tr + 1) / 2;
+}
+
+// Split-K partial covariance sums: partial[z][x][y] over the particle chunk z.
+__global__ void __launch_bounds__(256)
+syrk_partial_kernel(const float* __restrict__ phi, int N, int ld, int V,
+                    const float* __restrict__ mu, float* __restrict__ partial, int chunk,
+                    const Ctrl* ctrl, int respect_done) {
+  if (respect_done && ctrl->done) return;
+  __shared__ float As[16][68], Bs[16][68];
+  int tr, tc;
+  tri_tile(blockIdx.x, tr, tc);
+  const int x0 = tr * 64, y0 = tc * 64;
+  const int kb = blockIdx.y * chunk, ke = min(ld, kb + chunk);
+  float acc[4][4];
+#pragma unroll
+  for (int p = 0; p < 4; ++p)
+#pragma unroll
+    for (int r = 0; r < 4; ++r) acc[p][r] = 0.f;
+  nt_tile<true>(phi, (size_t)ld, x0, y0, V, kb, ke, N, mu, acc, As, Bs);
+  const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
+  float* out = partial + (size_t)blockIdx.y * V * V;
+#pragma unroll
+  for (int p = 0; p < 4; ++p)
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+      int x = x0 + ty * 4 + p, y = y0 + tx * 4 + r;
+      if (x < V && y < V) out[(size_t)x * V + y] = acc[p][r];
+    }
+}
+
+// Sigma[x][y] = Sigma[y][x] = (sum_z partial[z][x][y]) / (N-1) for y <= x, fixed summation order.
+__global__ void syrk_reduce_kernel(const float* __restrict__ partial, int nsplit, int V, int N,
+                                   float* __restrict__ Sigma, const Ctrl* ctrl, int respect_done) {
+  if (respect_done && ctrl->done) return;
+  int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= V * V) return;
+  int x = idx / V, y = idx - x * V;
+  if (y > x) return;
+  float a = 0.f;
+  for (int z = 0; z < nsplit; ++z) a += partial[(size_t)z * V * V + idx];
+  a /= (float)(N - 1);
+  Sigma[(size_t)x * V + y] = a;
+  Sigma[(size_t)y * V + x] = a;
+}
+
+__global__ void __launch_bounds__(256)
+trace_kernel(const float* __restrict__ Sigma, int V, Ctrl* ctrl, int respect_done) {
+  __shared__ double scratch[33];
+  if (respect_done && ctrl->done) return;
+  double a = 0.0;
+  for (int x = threadIdx.x; x < V; x += blockDim.x) a += (double)Sigma[(size_t)x * V + x];
+  a = block_sum(a, scratch);
+  if (threadIdx.x == 0) { ctrl->trace = (float)a; ctrl->chol_fail = 0; }
+}
+
+// attempt 0: plain; attempt 1: runs only if attempt 0 failed, adds 1e-6 tr/V to the diagonal.
+__device__ __forceinline__ bool chol_skip(const Ctrl* ctrl, int attempt, int respect_done) {
+  if (respect_done && ctrl->done) return true;
+  return attempt == 1 && !(ctrl->chol_fail & 1);
+}
+
+// ------------------------------------------------------------------ small V: one CTA ---------
+__global__ void __launch_bounds__(256)
+chol_small_kernel(const float* __restrict__ Sigma, float* __restrict__ Lc, int V, Ctrl* ctrl,
+                  int attempt, int respect_done) {
+  extern __shared__ float sm[];   // V x (V+1)
+  if (chol_skip(ctrl, attempt, respect_done)) return;
+  const int P = V + 1;
+  const float add = attempt ? 1e-6f * ctrl->trace / (float)V : 0.f;
+  for (int idx = threadIdx.x; idx < V * V; idx += blockDim.x) {
+    int x = idx / V, y = idx - x * V;
+    sm[x * P + y] = Sigma[idx] + (x == y ? add : 0.f);
+  }
+  __syncthreads();
+  int failed = 0;
+  for (int j = 0; j < V; ++j) {
+    float d = sm[j * P + j];
+    if (!(d > 0.f)) { failed = 1; d = 1.f; }
+    float inv = 1.f / sqrtf(d);
+    __syncthreads();
+    for (int r = j + threadIdx.x; r < V; r += blockDim.x) {
+      float v = sm[r * P + j];
+      sm[r * P + j] = (r == j) ? sqrtf(d) : v * inv;
+    }
+    __syncthreads();
+    // trailing update of the lower triangle: a_rc -= l_rj l_cj, j < c <= r
+    const int m = V - j - 1;
+    for (int e = threadIdx.x; e < m * m; e += blockDim.x) {
+      int rr = e / m, cc = e - rr * m;
+      if (cc <= rr) {
+        int r = j + 1 + rr, c = j + 1 + cc;
+        sm[r * P + c] = fmaf(-sm[r * P + j], sm[c * P + j], sm[r * P + c]);
+      }
+    }
+    __syncthreads();
+  }
+  for (int idx = threadIdx.x; idx < V * V; idx += blockDim.x) {
+    int x = idx / V, y = idx - x * V;
+    Lc[idx] = (y <= x) ? sm[x * P + y] : 0.f;
+  }
+  if (threadIdx.x == 0 && failed) atomicOr(&ctrl->chol_fail, attempt ? 2 : 1);
+}
+
+// ------------------------------------------------------------------ large V: blocked ---------
+__global__ void chol_copy_kernel(const float* __restrict__ Sigma, float* __restrict__ Lc, int V,
+                                 const Ctrl* ctrl, int attempt, int respect_done) {
+  if (chol_skip(ctrl, attempt, respect_done)) return;
+  int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= V * V) return;
+  int x = idx / V, y = idx - x * V;
+  float add = (attempt && x == y) ? 1e-6f * ctrl->trace / (float)V : 0.f;
+  Lc[idx] = (y <= x) ? Sigma[idx] + add : 0.f;
+}
+
+// Diagonal block [j0, j0+nb) factorised in shared memory by one CTA of 64 threads (thread = row).
+__global__ void __launch_bounds__(64)
+chol_diag_kernel(float* __restrict__ A, int V, int j0, Ctrl* ctrl, int attempt,
+                 int respect_done) {
+  __shared__ float T[64][65];
+  if (chol_skip(ctrl, attempt, respect_done)) return;
+  const int nb = min(64, V - j0), r = threadIdx.x;
+  for (int c = 0; c < nb; ++c) T[r][c] = (r < nb && c <= r) ? A[(size_t)(j0 + r) * V + j0 + c] : 0.f;
+  __syncthreads();
+  int failed = 0;
+  for (int j = 0; j < nb; ++j) {
+    float d = T[j][j];
+    if (!(d > 0.f)) { failed = 1; d = 1.f; }
+    float sq = sqrtf(d);
+    __syncthreads();
+    if (r == j) T[r][j] = sq;
+    else if (r > j && r < nb) T[r][j] = T[r][j] / sq;
+    __syncthreads();
+    if (r > j && r < nb) {
+      float lrj = T[r][j];
+      for (int c = j + 1; c <= r; ++c) T[r][c] = fmaf(-lrj, T[c][j], T[r][c]);
+    }
+    __syncthreads();
+  }
+  for (int c = 0; c < nb; ++c)
+    if (r < nb && c <= r) A[(size_t)(j0 + r) * V + j0 + c] = T[r][c];
+  if (r == 0 && failed) atomicOr(&ctrl->chol_fail, attempt ? 2 : 1);
+}
+
+// Rows below the diagonal block: X L11^T = A21, one thread per row, L11 in shared memory.
+__global__ void __launch_bounds__(64)
+chol_trsm_kernel(float* __restrict__ A, int V, int j0, const Ctrl* ctrl, int attempt,
+                 int respect_done) {
+  __shared__ float T[64][65];
+  if (chol_skip(ctrl, attempt, respect_done)) return;
+  const int nb = min(64, V - j0);
+  for (int c = 0; c < nb; ++c)
+    T[threadIdx.x][c] = (threadIdx.x < nb && c <= threadIdx.x)
+                            ? A[(size_t)(j0 + threadIdx.x) * V + j0 + c] : 0.f;
+  __syncthreads();
+  const int row = j0 + nb + blockIdx.x * 64 + threadIdx.x;
+  if (row >= V) return;
+  float x[64];
+  float* a = A + (size_t)row * V + j0;
+#pragma unroll
+  for (int c = 0; c < 64; ++c) x[c] = c < nb ? a[c] : 0.f;
+#pragma unroll
+  for (int c = 0; c < 64; ++c) {
+    if (c < nb) {
+      float v = x[c];
+#pragma unroll
+      for (int m = 0; m < 64; ++m)
+        if (m < c) v = fmaf(-x[m], T[c][m], v);
+      x[c] = v / T[c][c];
+    }
+  }
+#pragma unroll
+  for (int c = 0; c < 64; ++c)
+    if (c < nb) a[c] = x[c];
+}
+
+// Trailing update A22 -= L21 L21^T on the lower-triangular 64x64 tiles of rows/cols >= j1.
+__global__ void __launch_bounds__(256)
+chol_update_kernel(float* __restrict__ A, int V, int j0, int j1, const Ctrl* ctrl, int attempt,
+                   int respect_done) {
+  if (chol_skip(ctrl, attempt, respect_done)) return;
+  __shared__ float As[16][68], Bs[16][68];
+  int tr, tc;
+  tri_tile(blockIdx.x, tr, tc);
+  const int x0 = j1 + tr * 64, y0 = j1 + tc * 64;
+  float acc[4][4];
+#pragma unroll
+  for (int p = 0; p < 4; ++p)
+#pragma unroll
+    for (int r = 0; r < 4; ++r) acc[p][r] = 0.f;
+  nt_tile<false>(A, (size_t)V, x0, y0, V, j0, j1, V, nullptr, acc, As, Bs);
+  const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
+#pragma unroll
+  for (int p = 0; p < 4; ++p)
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+      int x = x0 + ty * 4 + p, y = y0 + tx * 4 + r;
+      if (x < V && y <= x) A[(size_t)x * V + y] -= acc[p][r];
+    }
+}
+
+__global__ void chol_finalize_kernel(Ctrl* ctrl, int respect_done) {
+  if (respect_done && ctrl->done) return;
+  int f = ctrl->chol_fail;
+  ctrl->chol_status = (f == 0) ? 0 : ((f & 2) ? -1 : 1);
+  ctrl->chol_fail = 0;
+}
+
+void launch_cholesky(const float* Sigma, float* Lc, int V, Ctrl* ctrl, int respect_done,
+                     cudaStream_t st) {
+  trace_kernel<<<1, 256, 0, st>>>(Sigma, V, ctrl, respect_done);
+  for (int attempt = 0; attempt < 2; ++attempt) {
+    if (V <= 160) {
+      size_t smem = (size_t)V * (V + 1) * sizeof(float);
+      static bool attr_done = false;
+      if (!attr_done) {
+        cudaFuncSetAttribute(chol_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             160 * 161 * (int)sizeof(float));
+        attr_done = true;
+      }
+      chol_small_kernel<<<1, 256, smem, st>>>(Sigma, Lc, V, ctrl, attempt, respect_done);
+    } else {
+      chol_copy_kernel<<<(V * V + 255) / 256, 256, 0, st>>>(Sigma, Lc, V, ctrl, attempt,
+                                                            respect_done);
+      for (int j0 = 0; j0 < V; j0 += 64) {
+        int j1 = min(V, j0 + 64);
+        chol_diag_kernel<<<1, 64, 0, st>>>(Lc, V, j0, ctrl, attempt, respect_done);
+        int rows = V - j1;
+        if (rows > 0) {
+          chol_trsm_kernel<<<(rows + 63) / 64, 64, 0, st>>>(Lc, V, j0, ctrl, attempt,
+                                                            respect_done);
+          int nt = (rows + 63) / 64;
+          chol_update_kernel<<<nt * (nt + 1) / 2, 256, 0, st>>>(Lc, V, j0, j1, ctrl, attempt,
+                                                                respect_done);
+        }
+      }
+    }
+  }
+  chol_finalize_kernel<<<1, 1, 0, st>>>(ctrl, respect_done);
+}
+
+static int cov_nsplit(int V, int N) {
+  int nt = (V + 63) / 64;
+  int tiles = nt * (nt + 1) / 2;
+  int want = (2 * 148 + tiles - 1) / tiles;
+  int maxsplit = (round_up(N, 128) + 255) / 256;   // chunks of >= 256 particles
+  int ns = want < 1 ? 1 : want;
+  if (ns > maxsplit) ns = maxsplit;
+  if (ns > 128) ns = 128;
+  return ns;
+}
+
+size_t cov_partial_floats(int V, int N) { return (size_t)cov_nsplit(V, N) * V * V; }
+
+void launch_cov_chol(const CovCholArgs& a, cudaStream_t st) {
+  const int V = a.V;
+  mean_kernel<<<V, 256, 0, st>>>(a.phi, a.N, a.ld, a.mu, a.ctrl, a.respect_done);
+  int ns = cov_nsplit(V, a.N);
+  int chunk = round_up((a.ld + ns - 1) / ns, 16);
+  ns = (a.ld + chunk - 1) / chunk;
+  int nt = (V + 63) / 64;
+  dim3 grid(nt * (nt + 1) / 2, ns);
+  syrk_partial_kernel<<<grid, 256, 0, st>>>(a.phi, a.N, a.ld, V, a.mu, a.partial, chunk, a.ctrl,
+                                            a.respect_done);
+  syrk_reduce_kernel<<<(V * V + 255) / 256, 256, 0, st>>>(a.partial, ns, V, a.N, a.Sigma, a.ctrl,
+                                                          a.respect_done);
+  launch_cholesky(a.Sigma, a.Lc, V, a.ctrl, a.respect_done, st);
+}
+
+}  // namespace phi4

@@ -1,0 +1,99 @@
+// kernels.cuh -- host-side launchers of the kernels (one .cu per group), used by api.cu.
+// Particles are site-major with a padded stride: phi[x*ld + i], ld = round_up(N,128); the pad
+// particles i in [N, ld) hold zeros and never enter a reduction.
+#pragma once
+#include "common.cuh"
+
+namespace phi4 {
+
+// field.cu -- M1 (INIT stream) and the full action (Eq. 1; U0)
+void launch_init_particles(float* phi, int N, int ld, int V, uint64_t seed, cudaStream_t st);
+void launch_action(const float* phi, int N, int ld, Model md, float* S, float* U0,
+                   Ctrl* ctrl, cudaStream_t st);
+
+void launch_set_identity(float* A, int V, cudaStream_t st);
+void launch_zero_upper(float* A, int V, cudaStream_t st);
+void launch_reset_counters(Ctrl* ctrl, cudaStream_t st);
+
+// mutate_generic.cu -- M1-M4 for any V, one step = normals -> proposal GEMM -> accept/commit
+struct MutateArgs {
+  float* phi;        // [V][ld] current particles (updated in place)
+  float* phip;       // [V][ld] scratch: proposals
+  float* Z;          // [V][ld] scratch: normals
+  float* S;          // [ld] cached S_E
+  float* U0;         // [ld] cached U0
+  const float* Lc;   // [V][V] row-major lower Cholesky factor, strict upper = 0
+  Ctrl* ctrl;        // beta / S_star / done are read from here
+  uint8_t* acc_out;  // optional [k][N] accept flags
+  float* margin_out; // optional [k][N] margins g (R4)
+  int N, ld;
+  Model md;
+  float s;           // step scale
+  int mode;          // MODE_SMC / MODE_NS
+  uint64_t seed;
+  uint32_t tag_prop, tag_acc;
+  uint32_t t0;       // step counter of the first step
+  int k;             // number of steps
+  int respect_done;  // 1: every kernel is a no-op once ctrl->done is set
+};
+void launch_mutate_generic(const MutateArgs& a, cudaStream_t st);
+
+// population.cu -- P1-P4
+void launch_next_delta_reweight(const float* S, int N, float ess_target, double delta_fixed,
+                                float* w, Ctrl* ctrl, cudaStream_t st);
+void launch_quantise_scan(const float* w, int N, unsigned long long* C, Ctrl* ctrl,
+                          cudaStream_t st);
+void launch_ancestors(const unsigned long long* C, int N, uint64_t seed, int32_t* anc, Ctrl* ctrl,
+                      cudaStream_t st);
+void launch_gather(const float* phi_in, float* phi_out, const float* S_in, float* S_out,
+                   const float* U_in, float* U_out, const int32_t* anc, int N, int ld, int V,
+                   Ctrl* ctrl, cudaStream_t st);
+void launch_finish_step(Ctrl* ctrl, StepRecord* rec, int max_rec, int k, int N, cudaStream_t st);
+
+// covchol.cu -- C1, C2
+struct CovCholArgs {
+  const float* phi;  // [V][ld]
+  int N, ld, V;
+  float* mu;         // [V]
+  float* Sigma;      // [V][V]
+  float* Lc;         // [V][V]
+  float* partial;    // split-K scratch, >= cov_partial_floats(V, N) floats
+  Ctrl* ctrl;
+  int respect_done;
+};
+size_t cov_partial_floats(int V, int N);
+void launch_cov_chol(const CovCholArgs& a, cudaStream_t st);
+void launch_cholesky(const float* Sigma, float* Lc, int V, Ctrl* ctrl, int respect_done,
+                     cudaStream_t st);
+
+// observables.cu -- O
+void launch_magnetisation(const float* phi, int N, int ld, int V, float* M, cudaStream_t st);
+// out: 5 + 80 doubles (absM, M2, chi, mean_SE, mode_balance, hist); logw may be NULL
+void launch_observables_reduce(const float* M, const float* S, const double* logw, int n, int V,
+                               double* out, cudaStream_t st);
+
+// ns.cu -- N1-N4
+struct NsArgs {
+  float* phi; float* S; float* U0;       // live set [V][ld], [ld], [ld]
+  float* wphi; float* wS; float* wU;     // walkers [V][ldw], [ldw], [ldw]
+  int n, ld, k_del, ldw, V;
+  uint64_t seed;
+  int32_t* dead;                         // [k_del] by decreasing S_E
+  int32_t* surv;                         // [n] survivors in index order
+  int32_t* start;                        // [k_del] chosen start points
+  float* dead_S; float* dead_M; double* dead_logw;   // dead-point log [max_iters*k_del]
+  int max_iters;
+  double stop_frac;
+  Ctrl* ctrl;
+};
+void launch_ns_select_evidence(const NsArgs& a, cudaStream_t st);   // N1 + N2 + start choice
+void launch_ns_load_walkers(const NsArgs& a, cudaStream_t st);      // N3 gather
+void launch_ns_store_walkers(const NsArgs& a, cudaStream_t st);     // N3 scatter
+void launch_ns_finish(const NsArgs& a, StepRecord* rec, int n_walk, cudaStream_t st);  // N4
+
+}  // namespace phi4
+
+namespace phi4 {
+void launch_ns_obs_inputs(const NsArgs& a, int n_dead, float* M_all, float* S_all,
+                          double* logw_all, cudaStream_t st);
+}

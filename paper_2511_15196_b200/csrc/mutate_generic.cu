@@ -1,0 +1,186 @@
+// mutate_generic.cu -- M1-M4 for any lattice size, one launch triple per step:
+//   normals_kernel   z[y][i]  (Philox, never reused across steps)
+//   propose_kernel   phi'[x][i] = phi[x][i] + s * sum_{y<=x} Lc[x][y] z[y][i]   (FP32 SIMT GEMM)
+//   accept_kernel    per-site action differences, Metropolis / constrained accept, commit
+// This is the size-agnostic path (and the reference point for the fused tcgen05 kernel): its HBM
+// traffic is per step, not per temperature.
+#include "kernels.cuh"
+#include "philox.cuh"
+
+namespace phi4 {
+
+__global__ void normals_kernel(float* __restrict__ Z, int N, int ld, int V, uint64_t seed,
+                               uint32_t tag, uint32_t t, const Ctrl* ctrl, int respect_done) {
+  if (respect_done && ctrl->done) return;
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  int q = blockIdx.y;
+  if (i >= ld) return;
+  float z[4] = {0.f, 0.f, 0.f, 0.f};
+  if (i < N) normals4(seed, tag, t, (uint32_t)i, (uint32_t)q, z);
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    int x = 4 * q + j;
+    if (x < V) Z[(size_t)x * ld + i] = z[j];
+  }
+}
+
+// C[x][i] = phi[x][i] + s * sum_y Lc[x][y] Z[y][i].  64x64 tile, BK=16, 4x4 per thread.  Lc is
+// lower-triangular, so the y loop of a tile ends at its last row.
+__global__ void __launch_bounds__(256)
+propose_kernel(const float* __restrict__ Lc, const float* __restrict__ Z,
+               const float* __restrict__ phi, float* __restrict__ phip, int V, int ld, float s,
+               const Ctrl* ctrl, int respect_done) {
+  if (respect_done && ctrl->done) return;
+  __shared__ float As[16][64 + 4];
+  __shared__ __align__(16) float Bs[16][64];
+  const int x0 = blockIdx.y * 64, i0 = blockIdx.x * 64;
+  const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
+  float acc[4][4];
+#pragma unroll
+  for (int a = 0; a < 4; ++a)
+#pragma unroll
+    for (int b = 0; b < 4; ++b) acc[a][b] = 0.f;
+  const int kend = min(V, x0 + 64);
+  const int am = threadIdx.x >> 2, ak = (threadIdx.x & 3) * 4;  // A loader: row am, 4 k's
+  const int bk = threadIdx.x >> 4, bn = (threadIdx.x & 15) * 4; // B loader: row bk, 4 i's
+  for (int k0 = 0; k0 < kend; k0 += 16) {
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      int x = x0 + am, y = k0 + ak + j;
+      As[ak + j][am] = (x < V && y < V) ? Lc[(size_t)x * V + y] : 0.f;
+    }
+    {
+      int y = k0 + bk;
+      float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (y < V) v = *reinterpret_cast<const float4*>(Z + (size_t)y * ld + i0 + bn);
+      *reinterpret_cast<float4*>(&Bs[bk][bn]) = v;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int kk = 0; kk < 16; ++kk) {
+      float a[4], b[4];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) a[j] = As[kk][ty * 4 + j];
+      float4 bv = *reinterpret_cast<const float4*>(&Bs[kk][tx * 4]);
+      b[0] = bv.x; b[1] = bv.y; b[2] = bv.z; b[3] = bv.w;
+#pragma unroll
+      for (int p = 0; p < 4; ++p)
+#pragma unroll
+        for (int r = 0; r < 4; ++r) acc[p][r] = fmaf(a[p], b[r], acc[p][r]);
+    }
+    __syncthreads();
+  }
+#pragma unroll
+  for (int p = 0; p < 4; ++p) {
+    int x = x0 + ty * 4 + p;
+    if (x < V) {
+      size_t o = (size_t)x * ld + i0 + tx * 4;
+      float4 f = *reinterpret_cast<const float4*>(phi + o);
+      f.x = fmaf(s, acc[p][0], f.x);
+      f.y = fmaf(s, acc[p][1], f.y);
+      f.z = fmaf(s, acc[p][2], f.z);
+      f.w = fmaf(s, acc[p][3], f.w);
+      *reinterpret_cast<float4*>(phip + o) = f;
+    }
+  }
+}
+
+// Per-site differences of Eq. 1 and U0 between phi' and phi, written so that nothing cancels
+// (SURVEY H3): with a = phi_x, b / c its forward neighbours and primes for the proposal,
+//   d kin  = 1/2 [(e'-e)(e'+e) + (f'-f)(f'+f)],  e = b-a, f = c-a
+//   d mass + d quartic = (a'^2-a^2) (1/2 m0^2 + lambda (a'^2+a^2)),   dU0 = 1/2 (a'^2-a^2)
+__device__ __forceinline__ void site_diff(float a, float b, float c, float a2, float b2, float c2,
+                                          float hm, float lam, float& dS, float& dU) {
+  float q = (a2 - a) * (a2 + a);
+  float e = b - a, e2 = b2 - a2, f = c - a, f2 = c2 - a2;
+  dS += 0.5f * ((e2 - e) * (e2 + e) + (f2 - f) * (f2 + f)) + q * (hm + lam * (a2 * a2 + a * a));
+  dU += 0.5f * q;
+}
+
+// Block = 32 particles x 8 row groups (one warp per group).  Phase 1: partial dS, dU0 over the
+// group's lattice rows.  Phase 2: warp 0 decides (R4 margin; NS: also S' < S_star).  Phase 3:
+// every group commits its rows of the accepted particles.
+__global__ void __launch_bounds__(256)
+accept_kernel(float* __restrict__ phi, const float* __restrict__ phip, float* __restrict__ S,
+              float* __restrict__ U0, int N, int ld, Model md, int mode, uint64_t seed,
+              uint32_t tag_acc, uint32_t t, Ctrl* ctrl, uint8_t* __restrict__ acc_out,
+              float* __restrict__ margin_out, int respect_done) {
+  if (respect_done && ctrl->done) return;
+  __shared__ float ps[8][32], pu[8][32];
+  __shared__ int flag[32];
+  const int lane = threadIdx.x & 31, g = threadIdx.x >> 5;
+  const int i = blockIdx.x * 32 + lane;
+  const int L = md.L;
+  const float hm = 0.5f * md.m0sq, lam = md.lam;
+  float dS = 0.f, dU = 0.f;
+  if (i < N) {
+    for (int r = g; r < L; r += 8) {
+      int rn = (r + 1 == L) ? 0 : r + 1;
+      size_t ro = (size_t)r * L * ld + i, rno = (size_t)rn * L * ld + i;
+      float a = phi[ro], a2 = phip[ro];
+      for (int c = 0; c < L; ++c) {
+        int cn = (c + 1 == L) ? 0 : c + 1;
+        float b = phi[ro + (size_t)cn * ld], b2 = phip[ro + (size_t)cn * ld];
+        float d = phi[rno + (size_t)c * ld], d2 = phip[rno + (size_t)c * ld];
+        site_diff(a, b, d, a2, b2, d2, hm, lam, dS, dU);
+        a = b;
+        a2 = b2;
+      }
+    }
+  }
+  ps[g][lane] = dS;
+  pu[g][lane] = dU;
+  __syncthreads();
+  if (g == 0) {
+    int acc = 0;
+    if (i < N) {
+      float tS = 0.f, tU = 0.f;
+#pragma unroll
+      for (int m = 0; m < 8; ++m) { tS += ps[m][lane]; tU += pu[m][lane]; }
+      float lu = log_uniform(seed, tag_acc, t, (uint32_t)i);
+      float Si = S[i], margin;
+      if (mode == MODE_SMC) {
+        margin = -(tU + (float)ctrl->beta * tS) - lu;
+        acc = margin > 0.f;
+      } else {
+        margin = -tU - lu;
+        acc = (margin > 0.f) && (Si + tS < (float)ctrl->S_star);
+      }
+      if (acc) {
+        S[i] = Si + tS;
+        U0[i] += tU;
+      }
+      if (acc_out) acc_out[i] = (uint8_t)acc;
+      if (margin_out) margin_out[i] = margin;
+    }
+    flag[lane] = acc;
+    unsigned m = __ballot_sync(0xffffffffu, acc);
+    if (lane == 0 && m) atomicAdd(&ctrl->n_accept, (unsigned)__popc(m));
+  }
+  __syncthreads();
+  if (i < N && flag[lane]) {
+    for (int r = g; r < L; r += 8) {
+      size_t ro = (size_t)r * L * ld + i;
+      for (int c = 0; c < L; ++c) phi[ro + (size_t)c * ld] = phip[ro + (size_t)c * ld];
+    }
+  }
+}
+
+void launch_mutate_generic(const MutateArgs& a, cudaStream_t st) {
+  const int V = a.md.V;
+  dim3 gz((a.ld + 127) / 128, (V + 3) / 4);
+  dim3 gp(a.ld / 64, (V + 63) / 64);
+  for (int j = 0; j < a.k; ++j) {
+    uint32_t t = a.t0 + (uint32_t)j;
+    normals_kernel<<<gz, 128, 0, st>>>(a.Z, a.N, a.ld, V, a.seed, a.tag_prop, t, a.ctrl,
+                                       a.respect_done);
+    propose_kernel<<<gp, 256, 0, st>>>(a.Lc, a.Z, a.phi, a.phip, V, a.ld, a.s, a.ctrl,
+                                       a.respect_done);
+    accept_kernel<<<a.ld / 32, 256, 0, st>>>(
+        a.phi, a.phip, a.S, a.U0, a.N, a.ld, a.md, a.mode, a.seed, a.tag_acc, t, a.ctrl,
+        a.acc_out ? a.acc_out + (size_t)j * a.N : nullptr,
+        a.margin_out ? a.margin_out + (size_t)j * a.N : nullptr, a.respect_done);
+  }
+}
+
+}  // namespace phi4

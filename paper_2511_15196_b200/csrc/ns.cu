@@ -1,0 +1,268 @@
+// ns.cu -- nested-sampling population step N1-N4 (PAPER.md:53(iv), :161, :170, :174; readings
+// A5, A6; volume bookkeeping after Skilling 2006, PAPER.md:141 ref [37]).
+#include "kernels.cuh"
+#include "philox.cuh"
+
+namespace phi4 {
+
+__device__ __forceinline__ double logaddexp_d(double a, double b) {
+  if (a == -INFINITY) return b;
+  if (b == -INFINITY) return a;
+  double m = fmax(a, b);
+  return m + log(exp(a - m) + exp(b - m));
+}
+
+// N1 + N2 + survivors + start choice in one CTA.
+//  N1: 64-bit keys (descending S_E, ascending index) bitonic-sorted in shared memory; the first
+//      k_del are the dead points, S_star = smallest S_E among them.
+//  N2: logX_j = logX_{j-1} - 1/(n-j+1), w_j = X_{j-1} - X_j, Z += w_j e^{-S_j}; the logX offsets
+//      do not depend on the data, so the batch is one parallel log-sum-exp.
+//  N3 (choice): survivors in index order by a flag scan; walker j starts from survivor number
+//      (word0 mod (n - k_del)) of Philox stream NS_START (c1 = j, c2 = iteration).
+__global__ void __launch_bounds__(1024)
+ns_select_evidence_kernel(NsArgs a) {
+  extern __shared__ unsigned long long keys[];   // npow2 keys; later reused as int flags
+  __shared__ double scratch[33];
+  __shared__ int wsum[32];
+  Ctrl* ctrl = a.ctrl;
+  if (ctrl->done) return;
+  const int n = a.n, kd = a.k_del, tid = threadIdx.x, nt = blockDim.x;
+  int np2 = 1;
+  while (np2 < n) np2 <<= 1;
+  for (int i = tid; i < np2; i += nt) {
+    unsigned long long key = ~0ull;
+    if (i < n) {
+      uint32_t b = __float_as_uint(a.S[i]);
+      uint32_t asc = (b & 0x80000000u) ? ~b : (b | 0x80000000u);   // ascending-orderable
+      key = ((unsigned long long)(~asc) << 32) | (uint32_t)i;        // descending S, ascending i
+    }
+    keys[i] = key;
+  }
+  __syncthreads();
+  for (int k = 2; k <= np2; k <<= 1) {
+    for (int j = k >> 1; j > 0; j >>= 1) {
+      for (int i = tid; i < np2; i += nt) {
+        int p = i ^ j;
+        if (p > i) {
+          unsigned long long x = keys[i], y = keys[p];
+          bool up = (i & k) == 0;
+          if ((x > y) == up) { keys[i] = y; keys[p] = x; }
+        }
+      }
+      __syncthreads();
+    }
+  }
+  const int it = ctrl->temp_index;
+  const double logX0 = ctrl->logX;
+  // dead list, threshold
+  for (int j = tid; j < kd; j += nt) a.dead[j] = (int)(uint32_t)keys[j];
+  const float S_star = a.S[(int)(uint32_t)keys[kd - 1]];
+  // evidence of the batch
+  double best = -INFINITY;
+  double term_mine[1];   // kd <= 1024 = blockDim: one dead point per thread at most
+  term_mine[0] = -INFINITY;
+  if (tid < kd) {
+    double lx = logX0;
+    for (int m = 1; m <= tid; ++m) lx -= 1.0 / (double)(n - m + 1);      // logX_{j-1}, j = tid+1
+    double step = 1.0 / (double)(n - tid);                                // 1/(n-j+1)
+    double logw = lx + log1p(-exp(-step));
+    int d = (int)(uint32_t)keys[tid];
+    float Sd = a.S[d];
+    term_mine[0] = logw - (double)Sd;
+    if (it < a.max_iters) {
+      size_t slot = (size_t)it * kd + tid;
+      a.dead_S[slot] = Sd;
+      a.dead_logw[slot] = logw;
+    }
+    best = term_mine[0];
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) best = fmax(best, __shfl_xor_sync(0xffffffffu, best, o));
+  if ((tid & 31) == 0) scratch[tid >> 5] = best;
+  __syncthreads();
+  if (tid == 0) {
+    double m = -INFINITY;
+    for (int k = 0; k < (nt >> 5); ++k) m = fmax(m, scratch[k]);
+    scratch[32] = m;
+  }
+  __syncthreads();
+  best = scratch[32];
+  double e = (tid < kd) ? exp(term_mine[0] - best) : 0.0;
+  e = block_sum(e, scratch);
+  __syncthreads();
+  // survivors: flags over n, contiguous run per thread, block scan
+  int* flags = reinterpret_cast<int*>(keys);
+  unsigned long long mykey = (tid < kd) ? keys[tid] : 0ull;
+  __syncthreads();
+  for (int i = tid; i < n; i += nt) flags[i] = 1;
+  __syncthreads();
+  if (tid < kd) flags[(int)(uint32_t)mykey] = 0;
+  __syncthreads();
+  const int ipt = (n + nt - 1) / nt;
+  const int lo = min(n, tid * ipt), hi = min(n, lo + ipt);
+  int run = 0;
+  for (int i = lo; i < hi; ++i) run += flags[i];
+  int inc = run;
+  const int lane = tid & 31, wid = tid >> 5;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    int v = __shfl_up_sync(0xffffffffu, inc, o);
+    if (lane >= o) inc += v;
+  }
+  if (lane == 31) wsum[wid] = inc;
+  __syncthreads();
+  if (wid == 0) {
+    int v = wsum[lane], s = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      int u = __shfl_up_sync(0xffffffffu, s, o);
+      if (lane >= o) s += u;
+    }
+    wsum[lane] = s - v;
+  }
+  __syncthreads();
+  int pos = wsum[wid] + inc - run;
+  for (int i = lo; i < hi; ++i)
+    if (flags[i]) a.surv[pos++] = i;
+  __syncthreads();
+  __threadfence_block();
+  const int ns = n - kd;
+  for (int j = tid; j < kd; j += nt) {
+    uint32_t r = philox_draw(a.seed, TAG_NS_START, (uint32_t)it, (uint32_t)j, 0u).x;
+    a.start[j] = a.surv[r % (uint32_t)ns];
+  }
+  if (tid == 0) {
+    double lx = logX0;
+    for (int m = 1; m <= kd; ++m) lx -= 1.0 / (double)(n - m + 1);
+    ctrl->logX = lx;
+    ctrl->logZ = logaddexp_d(ctrl->logZ, best + log(e));
+    ctrl->S_star = (double)S_star;
+  }
+}
+
+void launch_ns_select_evidence(const NsArgs& a, cudaStream_t st) {
+  int np2 = 1;
+  while (np2 < a.n) np2 <<= 1;
+  size_t smem = (size_t)np2 * sizeof(unsigned long long);
+  static bool attr_done = false;
+  if (!attr_done) {
+    cudaFuncSetAttribute(ns_select_evidence_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                         16384 * (int)sizeof(unsigned long long));
+    attr_done = true;
+  }
+  ns_select_evidence_kernel<<<1, 1024, smem, st>>>(a);
+}
+
+// N3 gather: walker j <- live point start[j]; also logs the magnetisation of dead point j.
+__global__ void ns_load_walkers_kernel(NsArgs a) {
+  if (a.ctrl->done) return;
+  int j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= a.ldw) return;
+  const bool live = j < a.k_del;
+  const int src = live ? a.start[j] : 0, d = live ? a.dead[j] : 0;
+  float m = 0.f;
+  for (int x = 0; x < a.V; ++x) {
+    const float* row = a.phi + (size_t)x * a.ld;
+    a.wphi[(size_t)x * a.ldw + j] = live ? row[src] : 0.f;
+    if (live) m += row[d];
+  }
+  a.wS[j] = live ? a.S[src] : 0.f;
+  a.wU[j] = live ? a.U0[src] : 0.f;
+  const int it = a.ctrl->temp_index;
+  if (live && it < a.max_iters) a.dead_M[(size_t)it * a.k_del + j] = m / (float)a.V;
+}
+
+void launch_ns_load_walkers(const NsArgs& a, cudaStream_t st) {
+  ns_load_walkers_kernel<<<(a.ldw + 127) / 128, 128, 0, st>>>(a);
+}
+
+// N3 scatter: dead slot dead[j] <- walker j.
+__global__ void ns_store_walkers_kernel(NsArgs a) {
+  if (a.ctrl->done) return;
+  int j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= a.k_del) return;
+  const int d = a.dead[j];
+  for (int x = 0; x < a.V; ++x) a.phi[(size_t)x * a.ld + d] = a.wphi[(size_t)x * a.ldw + j];
+  a.S[d] = a.wS[j];
+  a.U0[d] = a.wU[j];
+}
+
+void launch_ns_store_walkers(const NsArgs& a, cudaStream_t st) {
+  ns_store_walkers_kernel<<<(a.k_del + 127) / 128, 128, 0, st>>>(a);
+}
+
+// N4: remaining = X mean_live(e^-S) / (Z + X mean_live(e^-S)); record; stop rule; live term.
+__global__ void __launch_bounds__(1024)
+ns_finish_kernel(NsArgs a, StepRecord* rec, int n_walk) {
+  __shared__ double scratch[33];
+  __shared__ float smin_s[33];
+  Ctrl* ctrl = a.ctrl;
+  if (ctrl->done) return;
+  float m = INFINITY;
+  for (int i = threadIdx.x; i < a.n; i += blockDim.x) m = fminf(m, a.S[i]);
+  m = warp_min(m);
+  if ((threadIdx.x & 31) == 0) smin_s[threadIdx.x >> 5] = m;
+  __syncthreads();
+  if (threadIdx.x < 32) {
+    float v = threadIdx.x < (blockDim.x >> 5) ? smin_s[threadIdx.x] : INFINITY;
+    v = warp_min(v);
+    if (threadIdx.x == 0) smin_s[32] = v;
+  }
+  __syncthreads();
+  const double smin = (double)smin_s[32];
+  double acc = 0.0;
+  for (int i = threadIdx.x; i < a.n; i += blockDim.x) acc += exp(-((double)a.S[i] - smin));
+  acc = block_sum(acc, scratch);
+  if (threadIdx.x == 0) {
+    double log_live = ctrl->logX + (-smin + log(acc)) - log((double)a.n);
+    double rem = exp(log_live - logaddexp_d(ctrl->logZ, log_live));
+    int it = ctrl->temp_index;
+    int fin = rem < a.stop_frac;
+    if (it < a.max_iters) {
+      StepRecord r;
+      r.beta = ctrl->logX; r.delta = ctrl->S_star; r.ess_frac = rem; r.dlogZ = log_live;
+      r.logZ = ctrl->logZ;
+      r.accept_rate = (double)ctrl->n_accept / ((double)n_walk * (double)a.k_del);
+      r.n_unique = 0; r.chol_status = ctrl->chol_status; r.index = it; r.done = fin;
+      rec[it] = r;
+    }
+    ctrl->remaining = rem;
+    ctrl->temp_index = it + 1;
+    ctrl->n_accept = 0u;
+    if (!isfinite(rem)) ctrl->nan_flag = 1;
+    if (fin) {
+      ctrl->logZ = logaddexp_d(ctrl->logZ, log_live);
+      ctrl->done = 1;
+    } else if (it + 1 >= a.max_iters) {
+      ctrl->done = 2;   // dead-point log is full: stop without the live term
+    }
+  }
+}
+
+void launch_ns_finish(const NsArgs& a, StepRecord* rec, int n_walk, cudaStream_t st) {
+  ns_finish_kernel<<<1, 1024, 0, st>>>(a, rec, n_walk);
+}
+
+// Posterior sample for `observables`: dead points (weight w_j e^{-S_j}) followed by the live
+// points (weight X/n e^{-S_i}).  M_all[n_dead..] must already hold the live magnetisations.
+__global__ void ns_obs_inputs_kernel(NsArgs a, int n_dead, float* M_all, float* S_all,
+                                     double* logw_all) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n_dead) {
+    M_all[i] = a.dead_M[i];
+    S_all[i] = a.dead_S[i];
+    logw_all[i] = a.dead_logw[i] - (double)a.dead_S[i];
+  } else if (i < n_dead + a.n) {
+    int l = i - n_dead;
+    S_all[i] = a.S[l];
+    logw_all[i] = a.ctrl->logX - log((double)a.n) - (double)a.S[l];
+  }
+}
+
+void launch_ns_obs_inputs(const NsArgs& a, int n_dead, float* M_all, float* S_all,
+                          double* logw_all, cudaStream_t st) {
+  int tot = n_dead + a.n;
+  ns_obs_inputs_kernel<<<(tot + 255) / 256, 256, 0, st>>>(a, n_dead, M_all, S_all, logw_all);
+}
+
+}  // namespace phi4

@@ -1,0 +1,62 @@
+// philox.cuh -- device Philox4x32-10 and the integer -> normal / uniform maps.
+// Counter-based streams as fixed by DESIGN.md readings R1 (layout) and R2 (maps):
+//   key = (seed lo32, seed hi32); counter = (c0 = site quad q or 0, c1 = slot, c2 = step t,
+//   c3 = stream tag).  One call yields the normals of sites 4q..4q+3.
+#pragma once
+#include "common.cuh"
+
+namespace phi4 {
+
+struct U4 { uint32_t x, y, z, w; };
+
+__device__ __forceinline__ U4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                            uint32_t k0, uint32_t k1) {
+  constexpr uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u;
+  constexpr uint32_t W0 = 0x9E3779B9u, W1 = 0xBB67AE85u;
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    uint32_t h0 = __umulhi(M0, c0), l0 = M0 * c0;
+    uint32_t h1 = __umulhi(M1, c2), l1 = M1 * c2;
+    c0 = h1 ^ c1 ^ k0;
+    c2 = h0 ^ c3 ^ k1;
+    c1 = l1;
+    c3 = l0;
+    k0 += W0;
+    k1 += W1;
+  }
+  return U4{c0, c1, c2, c3};
+}
+
+__device__ __forceinline__ U4 philox_draw(uint64_t seed, uint32_t tag, uint32_t t, uint32_t slot,
+                                          uint32_t q) {
+  return philox4x32_10(q, slot, t, tag, (uint32_t)seed, (uint32_t)(seed >> 32));
+}
+
+// R2: radius uniform (k+1) 2^-24 in (0,1] (exact in fp32), angle 2 pi k' 2^-24.  Accurate
+// logf / sincospif (no fast-math intrinsics); the angle is handed to sincospi as k' 2^-23 so
+// that no rounded multiple of pi enters the argument.
+__device__ __forceinline__ void box_muller(uint32_t xa, uint32_t xb, float& za, float& zb) {
+  float ur = (float)((xa >> 8) + 1u) * 5.9604644775390625e-8f;  // 2^-24
+  float r = sqrtf(-2.0f * logf(ur));
+  float sn, cs;
+  sincospif((float)(xb >> 8) * 1.1920928955078125e-7f, &sn, &cs);  // 2^-23
+  za = r * cs;
+  zb = r * sn;
+}
+
+// The four normals of site quad q for (seed, tag, t, slot).
+__device__ __forceinline__ void normals4(uint64_t seed, uint32_t tag, uint32_t t, uint32_t slot,
+                                         uint32_t q, float z[4]) {
+  U4 w = philox_draw(seed, tag, t, slot, q);
+  box_muller(w.x, w.y, z[0], z[1]);
+  box_muller(w.z, w.w, z[2], z[3]);
+}
+
+// R2: accept uniform u = (k+1) 2^-24 from word 0 of the c0 = 0 draw; returns ln u.
+__device__ __forceinline__ float log_uniform(uint64_t seed, uint32_t tag, uint32_t t,
+                                             uint32_t slot) {
+  U4 w = philox_draw(seed, tag, t, slot, 0u);
+  return logf((float)((w.x >> 8) + 1u) * 5.9604644775390625e-8f);
+}
+
+}  // namespace phi4

@@ -1,0 +1,251 @@
+// population.cu -- the population step P1-P4: next beta by ESS bisection,
+// incremental weights + log Z, exact integer systematic resampling, gather.
+#include "kernels.cuh"
+#include "philox.cuh"
+
+namespace phi4 {
+
+// ---------------------------------------------------------------------------------------------
+// P1 + P2 in one CTA (N <= a few 1e5 floats: the vector is L2/L1 resident).
+// R3: f(d) = ESS(d)/N - target, ESS(d) = (sum e^{-d S})^2 / sum e^{-2 d S}; if f(1-beta) >= 0 the
+// step is final (beta' = 1), else 48 halvings of [0, 1-beta].  exp in fp32 on max-shifted
+// arguments, sums in fp64.  Then w_i = exp(-d (S_i - S_min)) (max w = 1) and
+// dlogZ = -d S_min + log sum w - log N   (U0 cancels between p_beta and p_beta').
+// ---------------------------------------------------------------------------------------------
+__device__ inline double ess_frac_eval(const float* __restrict__ S, int N, float smin, double d,
+                                       double* scratch, double* sum_out) {
+  float df = (float)d;
+  double a = 0.0, b = 0.0;
+  for (int i = threadIdx.x; i < N; i += blockDim.x) {
+    float e = expf(-df * (S[i] - smin));
+    a += (double)e;
+    b += (double)e * (double)e;
+  }
+  a = block_sum(a, scratch);
+  b = block_sum(b, scratch);
+  if (sum_out) *sum_out = a;
+  return a * a / (b * (double)N);
+}
+
+__global__ void __launch_bounds__(1024)
+next_delta_reweight_kernel(const float* __restrict__ S, int N, float ess_target,
+                           double delta_fixed, float* __restrict__ w, Ctrl* ctrl) {
+  __shared__ double scratch[33];
+  __shared__ float smin_s[33];
+  if (ctrl->done) return;
+  // S_min
+  float m = INFINITY;
+  for (int i = threadIdx.x; i < N; i += blockDim.x) m = fminf(m, S[i]);
+  m = warp_min(m);
+  if ((threadIdx.x & 31) == 0) smin_s[threadIdx.x >> 5] = m;
+  __syncthreads();
+  if (threadIdx.x < 32) {
+    float v = threadIdx.x < (blockDim.x >> 5) ? smin_s[threadIdx.x] : INFINITY;
+    v = warp_min(v);
+    if (threadIdx.x == 0) smin_s[32] = v;
+  }
+  __syncthreads();
+  const float smin = smin_s[32];
+  const double beta = ctrl->beta;
+  const double rest = 1.0 - beta;
+  double delta;
+  int final_step;
+  if (delta_fixed >= 0.0) {
+    delta = delta_fixed;
+    final_step = (beta + delta >= 1.0);
+  } else if (ess_frac_eval(S, N, smin, rest, scratch, nullptr) - (double)ess_target >= 0.0) {
+    delta = rest;
+    final_step = 1;
+  } else {
+    double lo = 0.0, hi = rest;
+    for (int it = 0; it < 48; ++it) {
+      double mid = 0.5 * (lo + hi);
+      if (ess_frac_eval(S, N, smin, mid, scratch, nullptr) - (double)ess_target > 0.0) lo = mid;
+      else hi = mid;
+    }
+    delta = 0.5 * (lo + hi);
+    final_step = 0;
+  }
+  // weights and the final sums
+  const float df = (float)delta;
+  double a = 0.0, b = 0.0;
+  for (int i = threadIdx.x; i < N; i += blockDim.x) {
+    float e = expf(-df * (S[i] - smin));
+    w[i] = e;
+    a += (double)e;
+    b += (double)e * (double)e;
+  }
+  a = block_sum(a, scratch);
+  b = block_sum(b, scratch);
+  if (threadIdx.x == 0) {
+    double dlz = -delta * (double)smin + log(a) - log((double)N);
+    ctrl->delta = delta;
+    ctrl->beta = final_step ? 1.0 : beta + delta;
+    ctrl->ess_frac = a * a / (b * (double)N);
+    ctrl->dlogZ = dlz;
+    ctrl->logZ += dlz;
+    ctrl->S_min = smin;
+    if (!isfinite(dlz)) ctrl->nan_flag = 1;
+  }
+}
+
+void launch_next_delta_reweight(const float* S, int N, float ess_target, double delta_fixed,
+                                float* w, Ctrl* ctrl, cudaStream_t st) {
+  next_delta_reweight_kernel<<<1, 1024, 0, st>>>(S, N, ess_target, delta_fixed, w, ctrl);
+}
+
+// ---------------------------------------------------------------------------------------------
+// P3, reading R5: q_i = floor(w_i 2^40) (exact: a power-of-two scaling of an fp32), inclusive
+// integer scan C_i, T = C_{N-1}.  Integer addition is associative, so the result is the same
+// for every scan shape: one CTA, each thread a contiguous run, warp-shuffle scan of the run sums.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(1024)
+quantise_scan_kernel(const float* __restrict__ w, int N, unsigned long long* __restrict__ C,
+                     Ctrl* ctrl) {
+  __shared__ unsigned long long wsum[32];
+  if (ctrl->done) return;
+  const int ipt = (N + blockDim.x - 1) / blockDim.x;
+  const int lo = min(N, (int)threadIdx.x * ipt), hi = min(N, lo + ipt);
+  unsigned long long run = 0;
+  for (int i = lo; i < hi; ++i) run += (unsigned long long)((double)w[i] * 1099511627776.0);
+  // inclusive scan of run over the block
+  unsigned long long inc = run;
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    unsigned long long v = __shfl_up_sync(0xffffffffu, inc, o);
+    if (lane >= o) inc += v;
+  }
+  if (lane == 31) wsum[wid] = inc;
+  __syncthreads();
+  if (wid == 0) {
+    unsigned long long v = wsum[lane], s = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      unsigned long long u = __shfl_up_sync(0xffffffffu, s, o);
+      if (lane >= o) s += u;
+    }
+    wsum[lane] = s - v;  // exclusive
+  }
+  __syncthreads();
+  unsigned long long pre = wsum[wid] + inc - run;
+  for (int i = lo; i < hi; ++i) {
+    pre += (unsigned long long)((double)w[i] * 1099511627776.0);
+    C[i] = pre;
+  }
+  if (threadIdx.x == blockDim.x - 1) {
+    ctrl->q_total = pre;
+    if (pre == 0ull) ctrl->nan_flag = 1;
+  }
+}
+
+void launch_quantise_scan(const float* w, int N, unsigned long long* C, Ctrl* ctrl,
+                          cudaStream_t st) {
+  quantise_scan_kernel<<<1, 1024, 0, st>>>(w, N, C, ctrl);
+}
+
+// a_j = #{i : C_i <= t_j}, t_j = floor(((j 2^32 + U) T) / (N 2^32)), clamped to N-1; U = word 0
+// of the RESAMPLE stream at the current temperature index.  Once the run is done the map is the
+// identity, so that a step enqueued past beta = 1 leaves the particles unchanged.
+__global__ void ancestors_kernel(const unsigned long long* __restrict__ C, int N, uint64_t seed,
+                                 int32_t* __restrict__ anc, const Ctrl* ctrl) {
+  int j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= N) return;
+  if (ctrl->done || ctrl->q_total == 0ull) { anc[j] = j; return; }
+  const uint32_t U = philox_draw(seed, TAG_RESAMPLE, (uint32_t)ctrl->temp_index, 0u, 0u).x;
+  const unsigned long long T = ctrl->q_total;
+  unsigned __int128 num = (unsigned __int128)(((unsigned long long)j << 32) + U) *
+                          (unsigned __int128)T;
+  unsigned long long tj = (unsigned long long)(num / ((unsigned __int128)((unsigned long long)N << 32)));
+  int lo = 0, hi = N;  // first index with C > tj
+  while (lo < hi) {
+    int mid = (lo + hi) >> 1;
+    if (C[mid] <= tj) lo = mid + 1; else hi = mid;
+  }
+  anc[j] = min(lo, N - 1);
+}
+
+void launch_ancestors(const unsigned long long* C, int N, uint64_t seed, int32_t* anc, Ctrl* ctrl,
+                      cudaStream_t st) {
+  ancestors_kernel<<<(N + 255) / 256, 256, 0, st>>>(C, N, seed, anc, ctrl);
+}
+
+// ---------------------------------------------------------------------------------------------
+// P4: phi_out[x][j] = phi_in[x][a_j] (and S, U0).  A thread owns 4 consecutive slots j: four
+// scalar gathers (a is monotone, so a warp reads a near-contiguous span) and one 16-byte store
+// per site row.  grid.y splits the V rows.  HBM bound: 8 N V bytes.
+// ---------------------------------------------------------------------------------------------
+constexpr int GATHER_ROWS = 16;
+__global__ void __launch_bounds__(256)
+gather_kernel(const float* __restrict__ pin, float* __restrict__ pout,
+              const float* __restrict__ Sin, float* __restrict__ Sout,
+              const float* __restrict__ Uin, float* __restrict__ Uout,
+              const int32_t* __restrict__ anc, int N, int ld, int V, Ctrl* ctrl) {
+  const int j0 = (blockIdx.x * blockDim.x + threadIdx.x) * 4;
+  if (j0 >= ld) return;
+  int a[4];
+#pragma unroll
+  for (int m = 0; m < 4; ++m) a[m] = (j0 + m < N) ? anc[j0 + m] : -1;
+  const int x0 = blockIdx.y * GATHER_ROWS, x1 = min(V, x0 + GATHER_ROWS);
+  for (int x = x0; x < x1; ++x) {
+    const float* src = pin + (size_t)x * ld;
+    float4 v;
+    v.x = a[0] >= 0 ? src[a[0]] : 0.f;
+    v.y = a[1] >= 0 ? src[a[1]] : 0.f;
+    v.z = a[2] >= 0 ? src[a[2]] : 0.f;
+    v.w = a[3] >= 0 ? src[a[3]] : 0.f;
+    *reinterpret_cast<float4*>(pout + (size_t)x * ld + j0) = v;
+  }
+  if (blockIdx.y == 0) {
+    float4 s, u;
+    s.x = a[0] >= 0 ? Sin[a[0]] : 0.f; u.x = a[0] >= 0 ? Uin[a[0]] : 0.f;
+    s.y = a[1] >= 0 ? Sin[a[1]] : 0.f; u.y = a[1] >= 0 ? Uin[a[1]] : 0.f;
+    s.z = a[2] >= 0 ? Sin[a[2]] : 0.f; u.z = a[2] >= 0 ? Uin[a[2]] : 0.f;
+    s.w = a[3] >= 0 ? Sin[a[3]] : 0.f; u.w = a[3] >= 0 ? Uin[a[3]] : 0.f;
+    *reinterpret_cast<float4*>(Sout + j0) = s;
+    *reinterpret_cast<float4*>(Uout + j0) = u;
+    // distinct ancestors: a is non-decreasing, count the rises
+    int prev = (j0 > 0 && j0 - 1 < N) ? anc[j0 - 1] : -1;
+    int cnt = 0;
+#pragma unroll
+    for (int m = 0; m < 4; ++m)
+      if (a[m] >= 0) { cnt += (a[m] != prev); prev = a[m]; }
+    unsigned tot = (unsigned)cnt;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) tot += __shfl_xor_sync(0xffffffffu, tot, o);
+    if ((threadIdx.x & 31) == 0 && tot) atomicAdd(&ctrl->n_unique, tot);
+  }
+}
+
+void launch_gather(const float* phi_in, float* phi_out, const float* S_in, float* S_out,
+                   const float* U_in, float* U_out, const int32_t* anc, int N, int ld, int V,
+                   Ctrl* ctrl, cudaStream_t st) {
+  dim3 grid((ld / 4 + 255) / 256, (V + GATHER_ROWS - 1) / GATHER_ROWS);
+  gather_kernel<<<grid, 256, 0, st>>>(phi_in, phi_out, S_in, S_out, U_in, U_out, anc, N, ld, V,
+                                      ctrl);
+}
+
+// End of a temperature: record it, advance the index, latch done at beta == 1.
+__global__ void finish_step_kernel(Ctrl* ctrl, StepRecord* rec, int max_rec, int k, int N) {
+  if (ctrl->done) return;
+  int t = ctrl->temp_index;
+  if (t < max_rec) {
+    StepRecord r;
+    r.beta = ctrl->beta; r.delta = ctrl->delta; r.ess_frac = ctrl->ess_frac;
+    r.dlogZ = ctrl->dlogZ; r.logZ = ctrl->logZ;
+    r.accept_rate = (double)ctrl->n_accept / ((double)k * (double)N);
+    r.n_unique = (int)ctrl->n_unique; r.chol_status = ctrl->chol_status;
+    r.index = t; r.done = ctrl->beta >= 1.0;
+    rec[t] = r;
+  }
+  ctrl->temp_index = t + 1;
+  ctrl->n_accept = 0u;
+  ctrl->n_unique = 0u;
+  if (ctrl->beta >= 1.0) ctrl->done = 1;
+}
+
+void launch_finish_step(Ctrl* ctrl, StepRecord* rec, int max_rec, int k, int N, cudaStream_t st) {
+  finish_step_kernel<<<1, 1, 0, st>>>(ctrl, rec, max_rec, k, N);
+}
+
+}  // namespace phi4
