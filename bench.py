@@ -1,0 +1,302 @@
+#!/usr/bin/env python
+"""bench.py -- site-updates/s and SMC wall-clock to beta=1 of the batched tempered-particle update.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload C1]
+
+A "step" is one pass of the whole hot path: a complete adaptive-tempering SMC-RW run from fresh
+N(0,I) particles to beta = 1 (P1-P4, C1, C2 and k x (M1-M4) per temperature) on BASELINE.json's
+configuration (default C1 = configs[1]: L=10, N=16384, k=20, ESS 0.5).  value = N*V*(mutation steps
+executed) / time, summed over ranks.  The path does not shard ("replicas only"): with
+--gpus N every rank runs an independent replica with its own seed, no collective on the data path.
+
+One JSON line on stdout (rank 0).  --impl reference times the FP64 CPU oracle on the host cores.
+"""
+import argparse
+import json
+import math
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+ALU_OPS_PER_SITE_UPDATE = 40          # Philox ~20 int + Box-Muller ~6 + action ~14
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return {"hbm_gbs": d["hbm_gbs"], "bf16_tflops": d["bf16_tflops"],
+                "bf16_tflops_sustained": d.get("bf16_tflops_sustained", d["bf16_tflops"]),
+                "sm_max_mhz": d.get("sm_max_mhz", 1965.0), "source": "measured"}
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0,
+            "sm_max_mhz": 1965.0, "source": "fallback"}
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.stop_flag, self.samples, self.reasons, self.max_mhz = index, False, [], set(), None
+
+    def run(self):
+        try:
+            import pynvml as nv
+            nv.nvmlInit()
+            h = nv.nvmlDeviceGetHandleByIndex(self.index)
+            self.max_mhz = nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM)
+            names = {nv.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown",
+                     nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
+                     nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown",
+                     nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap"}
+            while not self.stop_flag:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(h)
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+                time.sleep(0.02)
+        except Exception as e:                      # pragma: no cover - depends on the box
+            self.reasons.add("nvml_unavailable:%s" % type(e).__name__)
+
+    def result(self):
+        s = sorted(self.samples)
+        return {"sm_mhz": s[len(s) // 2] if s else None, "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons)}
+
+
+def oracle_run(cfg, n_sample, seed):
+    """One oracle SMC run on a reduced population; returns (site_updates, seconds, T, threads)."""
+    from oracle import oracle as O
+    t0 = time.perf_counter()
+    r = O.smc_run(cfg["L"], cfg["m0sq"], cfg["lam"], n_sample, seed, cfg["k"], ess_target=cfg["ess"])
+    dt = time.perf_counter() - t0
+    V = cfg["L"] ** 2
+    return n_sample * V * cfg["k"] * r["T"], dt, r["T"], O.num_threads()
+
+
+def run_reference(args, cfg):
+    """--impl reference: the oracle as it stands, on the host cores, bounded sample per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    n_sample = min(cfg["N"], args.ref_particles)
+    for w in range(args.warmup):
+        oracle_run(cfg, n_sample, 1000 + w)
+    tot_su, tot_t, Ts = 0, 0.0, []
+    for s in range(args.steps):
+        su, dt, T, thr = oracle_run(cfg, n_sample, s)
+        tot_su += su
+        tot_t += dt
+        Ts.append(T)
+    value = tot_su / tot_t
+    sample = "N=%d of %d particles, full adaptive tempering run to beta=1 per step" % (n_sample, cfg["N"])
+    line = {"impl": "reference", "metric": "site-updates/s", "value": value, "unit": "site-updates/s",
+            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": 1e3 * tot_t / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_config(args, cfg, temps=Ts),
+            "cpu_baseline": {"value": value, "unit": "site-updates/s", "cores": thr, "kind": "oracle",
+                             "sample": sample},
+            "e2e": {"value": value, "unit": "site-updates/s", "h2d_bytes_per_step": 0,
+                    "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def workload_config(args, cfg, temps=None):
+    c = {"workload": "%s: phi^4 L=%d (V=%d) m0sq=%g lambda=%g, N=%d particles from N(0,I), adaptive "
+                     "tempering to beta=1 at ESS %.2f, %d RW-Metropolis steps per temperature, "
+                     "systematic resampling, dense VxV covariance-Cholesky proposal"
+                     % (args.workload, cfg["L"], cfg["L"] ** 2, cfg["m0sq"], cfg["lam"], cfg["N"],
+                        cfg["ess"], cfg["k"]),
+         "L": cfg["L"], "V": cfg["L"] ** 2, "N": cfg["N"], "k_steps": cfg["k"], "ess_target": cfg["ess"],
+         "parallelism": "replicas x%d (no sharding)" % args.gpus,
+         "l2": "flushed between timed steps (256 MiB write)"}
+    if temps is not None:
+        c["temperatures_per_step"] = temps
+    return c
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=8)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="C1")
+    ap.add_argument("--path", type=int, default=0, help="mutation path: 0 auto, 1 generic, 2 fused")
+    ap.add_argument("--ref-particles", type=int, default=16384)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 0)
+
+    from paper_2511_15196_b200 import inputs
+    cfg = inputs.CONFIGS[args.workload]
+    assert cfg["kind"] == "smc", "bench.py times SMC workloads (C0, C0g, C1, C3, C4)"
+    if args.impl == "reference":
+        run_reference(args, cfg)
+        return
+
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_2511_15196_b200 import binding as B
+    from paper_2511_15196_b200 import build
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --impl ours needs a CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = "cuda:%d" % local
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(dev))
+    if rank == 0:
+        build.build()
+    if world > 1:
+        dist.barrier()
+    B.load()
+
+    L, N, k, V = cfg["L"], cfg["N"], cfg["k"], cfg["L"] ** 2
+    h = B.smc_init(L, cfg["m0sq"], cfg["lam"], N, 0, device=dev)
+    B.smc_set_params(h, k_steps=k, ess_target=cfg["ess"], mutation_path=args.path)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    def device_step(seed):
+        """inputs resident in HBM: particles are drawn on the device by the INIT Philox stream."""
+        flush.fill_(seed & 0xFF)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        B.smc_reset(h, seed)
+        T = B.smc_run(h)
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1), T
+
+    # ---- device-resident timing -------------------------------------------------------------
+    for w in range(args.warmup):
+        device_step(1000 + w + 7919 * rank)
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    l0 = B.phi4_kernel_launches()
+    ms, Ts = 0.0, []
+    for s in range(args.steps):
+        dt, T = device_step(s + 7919 * rank)
+        ms += dt
+        Ts.append(T)
+    launches = B.phi4_kernel_launches() - l0
+    barrier()
+    sampler.stop_flag = True
+    sampler.join()
+    site_updates = float(N) * V * k * sum(Ts)
+    logZ = B.log_Z(h)
+
+    # ---- end to end through the C ABI with HOST buffers ---------------------------------------
+    h_in = torch.empty((V, N), dtype=torch.float32, pin_memory=True)
+    h_in.normal_(generator=torch.Generator().manual_seed(1234 + rank))
+    phi_in = h_in.numpy()
+
+    def e2e_step(seed):
+        flush.fill_(seed & 0xFF)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        B.smc_reset(h, seed)
+        B.smc_set_state(h, phi_in, 0.0, 0)            # H2D: V*N fp32 initial particles
+        T = B.smc_run(h)
+        st = B.smc_get_state(h)                       # D2H: final particles, S_E, U0
+        lz = B.log_Z(h)
+        torch.cuda.synchronize()
+        return (time.perf_counter() - t0) * 1e3, T, lz
+
+    e2e_step(999)
+    e2e_ms, e2e_T = 0.0, []
+    barrier()
+    for s in range(args.steps):
+        dt, T, _ = e2e_step(s + 7919 * rank)
+        e2e_ms += dt
+        e2e_T.append(T)
+    barrier()
+    e2e_su = float(N) * V * k * sum(e2e_T)
+
+    # ---- dominant kernel: the mutation, timed alone at a mid-schedule state -------------------
+    B.smc_reset(h, 4242)
+    for _ in range(3):
+        B.smc_step(h, want_info=False)
+    torch.cuda.synchronize()
+    for _ in range(2):
+        B.smc_mutate(h, k, want=False)
+    reps = 5
+    l1 = B.phi4_kernel_launches()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(reps):
+        B.smc_mutate(h, k, want=False)
+    e1.record()
+    torch.cuda.synchronize()
+    mut_ms = e0.elapsed_time(e1) / reps                       # k steps
+    mut_launches = (B.phi4_kernel_launches() - l1) // reps
+
+    # ---- reduce over ranks ----------------------------------------------------------------------
+    stats = torch.tensor([ms, site_updates, e2e_ms, e2e_su, mut_ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        mx = stats.clone()
+        dist.all_reduce(mx, op=dist.ReduceOp.MAX)
+        sm = stats.clone()
+        dist.all_reduce(sm, op=dist.ReduceOp.SUM)
+        ms, e2e_ms, mut_ms = mx[0].item(), mx[2].item(), mx[4].item()
+        site_updates, e2e_su = sm[1].item(), sm[3].item()
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    pk = peaks()
+    # Roofline of the mutation: algorithmic work per site-update =
+    # (V+1) flop for the triangular proposal product + 40 plain ALU ops (RNG, Box-Muller, action).
+    work = (V + 1 + ALU_OPS_PER_SITE_UPDATE) * float(N) * V * k
+    alu_peak = 148 * 128 * 2 * pk["sm_max_mhz"] * 1e6 / 1e12       # TFLOP/s, FP32 FMA pipes
+    achieved = work / (mut_ms * 1e-3) / 1e12
+    roofline = {"bound": "alu", "kernel": "mutation x%d steps (%d launches)" % (k, mut_launches),
+                "achieved": achieved, "peak": alu_peak, "unit": "TFLOP/s", "frac": achieved / alu_peak,
+                "traffic": None, "peak_source": "derived: 148 SM x 128 lanes x 2 x %.0f MHz (%s clocks)"
+                % (pk["sm_max_mhz"], pk["source"]),
+                "site_updates_per_s": float(N) * V * k / (mut_ms * 1e-3), "ms": mut_ms}
+
+    cpu = None
+    if not args.no_cpu_baseline:
+        n_s = min(N, args.ref_particles)
+        su, dt, T, thr = oracle_run(cfg, n_s, 0)
+        cpu = {"value": su / dt, "unit": "site-updates/s", "cores": thr, "kind": "oracle",
+               "sample": "N=%d of %d particles, one full tempering run (%d temperatures, %.1f s)"
+               % (n_s, N, T, dt)}
+
+    line = {"metric": "site-updates/s", "value": site_updates / (ms * 1e-3), "unit": "site-updates/s",
+            "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+            "data": "synthetic", "config": workload_config(args, cfg, temps=Ts),
+            "smc_wall_clock_ms_to_beta1": ms / args.steps, "logZ_last": logZ,
+            "e2e": {"value": e2e_su / (e2e_ms * 1e-3), "unit": "site-updates/s",
+                    "h2d_bytes_per_step": V * N * 4, "d2h_bytes_per_step": V * N * 4 + 8 * N + 8,
+                    "ms_per_step": e2e_ms / args.steps},
+            "gpu_launches": int(launches), "clocks": sampler.result(), "roofline": roofline,
+            "cpu_baseline": cpu}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -93,6 +93,8 @@ typedef struct {
 const char* phi4_strerror(int code);
 /* Text of the last CUDA error seen by this handle ("" if none); valid until the next call. */
 const char* phi4_last_cuda_error(const phi4smc* h);
+/* Diagnostic: number of CUDA kernels this library has launched in this process so far. */
+uint64_t phi4_kernel_launches(void);
 
 /* ---------------------------------------------------------------- SMC-RW (PAPER.md:53(i)) ----
  * smc_workspace_bytes: bytes of device memory smc_init needs for an L x L lattice and N particles

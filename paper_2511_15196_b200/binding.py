@@ -65,6 +65,7 @@ _vp, _i, _f, _d, _u64, _sz = C.c_void_p, C.c_int, C.c_float, C.c_double, C.c_uin
 SIGNATURES = {
     "phi4_strerror": (C.c_char_p, [_i]),
     "phi4_last_cuda_error": (C.c_char_p, [_vp]),
+    "phi4_kernel_launches": (_u64, []),
     "smc_workspace_bytes": (_sz, [_i, _i]),
     "smc_init": (_i, [C.POINTER(_vp), _i, _f, _f, _i, _u64, _vp, _sz, _vp]),
     "smc_reset": (_i, [_vp, _u64]),
@@ -153,6 +154,10 @@ def _stream_ptr(device):
 def _aligned(ws):
     p = ws.data_ptr()
     return (p + 255) // 256 * 256
+
+
+def phi4_kernel_launches():
+    return load().phi4_kernel_launches()
 
 
 def smc_workspace_bytes(L, N):

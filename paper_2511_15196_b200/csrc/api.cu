@@ -14,6 +14,8 @@
 
 using namespace phi4;
 
+namespace phi4 { unsigned long long g_launches = 0; }
+
 namespace {
 constexpr int KIND_SMC = 0, KIND_NS = 1;
 constexpr int MAX_RECORDS = 4096;       // per-temperature records kept on the device (SMC)
@@ -163,6 +165,8 @@ PHI4_API const char* phi4_strerror(int code) {
     default: return "unknown error";
   }
 }
+
+PHI4_API uint64_t phi4_kernel_launches(void) { return g_launches; }
 
 PHI4_API const char* phi4_last_cuda_error(const phi4smc* h) { return h ? h->err : ""; }
 

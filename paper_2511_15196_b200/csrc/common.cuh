@@ -5,6 +5,9 @@
 
 namespace phi4 {
 
+// Number of kernels this library has launched (diagnostic; bench.py reports it as gpu_launches).
+extern unsigned long long g_launches;
+
 // Philox stream tags (reading R1).
 enum : uint32_t {
   TAG_INIT = 0, TAG_PROP = 1, TAG_ACC = 2, TAG_RESAMPLE = 3,

@@ -286,7 +286,7 @@ __global__ void chol_finalize_kernel(Ctrl* ctrl, int respect_done) {
 
 void launch_cholesky(const float* Sigma, float* Lc, int V, Ctrl* ctrl, int respect_done,
                      cudaStream_t st) {
-  trace_kernel<<<1, 256, 0, st>>>(Sigma, V, ctrl, respect_done);
+  ++g_launches; trace_kernel<<<1, 256, 0, st>>>(Sigma, V, ctrl, respect_done);
   for (int attempt = 0; attempt < 2; ++attempt) {
     if (V <= 160) {
       size_t smem = (size_t)V * (V + 1) * sizeof(float);
@@ -296,25 +296,25 @@ void launch_cholesky(const float* Sigma, float* Lc, int V, Ctrl* ctrl, int respe
                              160 * 161 * (int)sizeof(float));
         attr_done = true;
       }
-      chol_small_kernel<<<1, 256, smem, st>>>(Sigma, Lc, V, ctrl, attempt, respect_done);
+      ++g_launches; chol_small_kernel<<<1, 256, smem, st>>>(Sigma, Lc, V, ctrl, attempt, respect_done);
     } else {
-      chol_copy_kernel<<<(V * V + 255) / 256, 256, 0, st>>>(Sigma, Lc, V, ctrl, attempt,
+      ++g_launches; chol_copy_kernel<<<(V * V + 255) / 256, 256, 0, st>>>(Sigma, Lc, V, ctrl, attempt,
                                                             respect_done);
       for (int j0 = 0; j0 < V; j0 += 64) {
         int j1 = min(V, j0 + 64);
-        chol_diag_kernel<<<1, 64, 0, st>>>(Lc, V, j0, ctrl, attempt, respect_done);
+        ++g_launches; chol_diag_kernel<<<1, 64, 0, st>>>(Lc, V, j0, ctrl, attempt, respect_done);
         int rows = V - j1;
         if (rows > 0) {
-          chol_trsm_kernel<<<(rows + 63) / 64, 64, 0, st>>>(Lc, V, j0, ctrl, attempt,
+          ++g_launches; chol_trsm_kernel<<<(rows + 63) / 64, 64, 0, st>>>(Lc, V, j0, ctrl, attempt,
                                                             respect_done);
           int nt = (rows + 63) / 64;
-          chol_update_kernel<<<nt * (nt + 1) / 2, 256, 0, st>>>(Lc, V, j0, j1, ctrl, attempt,
+          ++g_launches; chol_update_kernel<<<nt * (nt + 1) / 2, 256, 0, st>>>(Lc, V, j0, j1, ctrl, attempt,
                                                                 respect_done);
         }
       }
     }
   }
-  chol_finalize_kernel<<<1, 1, 0, st>>>(ctrl, respect_done);
+  ++g_launches; chol_finalize_kernel<<<1, 1, 0, st>>>(ctrl, respect_done);
 }
 
 static int cov_nsplit(int V, int N) {
@@ -332,15 +332,15 @@ size_t cov_partial_floats(int V, int N) { return (size_t)cov_nsplit(V, N) * V * 
 
 void launch_cov_chol(const CovCholArgs& a, cudaStream_t st) {
   const int V = a.V;
-  mean_kernel<<<V, 256, 0, st>>>(a.phi, a.N, a.ld, a.mu, a.ctrl, a.respect_done);
+  ++g_launches; mean_kernel<<<V, 256, 0, st>>>(a.phi, a.N, a.ld, a.mu, a.ctrl, a.respect_done);
   int ns = cov_nsplit(V, a.N);
   int chunk = round_up((a.ld + ns - 1) / ns, 16);
   ns = (a.ld + chunk - 1) / chunk;
   int nt = (V + 63) / 64;
   dim3 grid(nt * (nt + 1) / 2, ns);
-  syrk_partial_kernel<<<grid, 256, 0, st>>>(a.phi, a.N, a.ld, V, a.mu, a.partial, chunk, a.ctrl,
+  ++g_launches; syrk_partial_kernel<<<grid, 256, 0, st>>>(a.phi, a.N, a.ld, V, a.mu, a.partial, chunk, a.ctrl,
                                             a.respect_done);
-  syrk_reduce_kernel<<<(V * V + 255) / 256, 256, 0, st>>>(a.partial, ns, V, a.N, a.Sigma, a.ctrl,
+  ++g_launches; syrk_reduce_kernel<<<(V * V + 255) / 256, 256, 0, st>>>(a.partial, ns, V, a.N, a.Sigma, a.ctrl,
                                                           a.respect_done);
   launch_cholesky(a.Sigma, a.Lc, V, a.ctrl, a.respect_done, st);
 }

@@ -21,7 +21,7 @@ __global__ void init_particles_kernel(float* __restrict__ phi, int N, int ld, in
 
 void launch_init_particles(float* phi, int N, int ld, int V, uint64_t seed, cudaStream_t st) {
   dim3 grid((ld + 127) / 128, (V + 3) / 4);
-  init_particles_kernel<<<grid, 128, 0, st>>>(phi, N, ld, V, seed);
+  ++g_launches; init_particles_kernel<<<grid, 128, 0, st>>>(phi, N, ld, V, seed);
 }
 
 // Eq. 1 and U0 for every particle.  A block is 32 particles x 8 row
@@ -68,7 +68,7 @@ action_kernel(const float* __restrict__ phi, int N, int ld, Model md, float* __r
 
 void launch_action(const float* phi, int N, int ld, Model md, float* S, float* U0, Ctrl* ctrl,
                    cudaStream_t st) {
-  action_kernel<<<ld / 32, 256, 0, st>>>(phi, N, ld, md, S, U0, ctrl);
+  ++g_launches; action_kernel<<<ld / 32, 256, 0, st>>>(phi, N, ld, md, S, U0, ctrl);
 }
 
 __global__ void set_identity_kernel(float* __restrict__ A, int V) {
@@ -77,7 +77,7 @@ __global__ void set_identity_kernel(float* __restrict__ A, int V) {
 }
 
 void launch_set_identity(float* A, int V, cudaStream_t st) {
-  set_identity_kernel<<<(V * V + 255) / 256, 256, 0, st>>>(A, V);
+  ++g_launches; set_identity_kernel<<<(V * V + 255) / 256, 256, 0, st>>>(A, V);
 }
 
 // Strict upper triangle := 0 (the proposal GEMM relies on it to stop each tile at its last row).
@@ -87,7 +87,7 @@ __global__ void zero_upper_kernel(float* __restrict__ A, int V) {
 }
 
 void launch_zero_upper(float* A, int V, cudaStream_t st) {
-  zero_upper_kernel<<<(V * V + 255) / 256, 256, 0, st>>>(A, V);
+  ++g_launches; zero_upper_kernel<<<(V * V + 255) / 256, 256, 0, st>>>(A, V);
 }
 
 __global__ void reset_counters_kernel(Ctrl* ctrl) { ctrl->n_accept = 0u; ctrl->n_unique = 0u; }

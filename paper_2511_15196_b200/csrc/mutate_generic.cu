@@ -172,11 +172,11 @@ void launch_mutate_generic(const MutateArgs& a, cudaStream_t st) {
   dim3 gp(a.ld / 64, (V + 63) / 64);
   for (int j = 0; j < a.k; ++j) {
     uint32_t t = a.t0 + (uint32_t)j;
-    normals_kernel<<<gz, 128, 0, st>>>(a.Z, a.N, a.ld, V, a.seed, a.tag_prop, t, a.ctrl,
+    ++g_launches; normals_kernel<<<gz, 128, 0, st>>>(a.Z, a.N, a.ld, V, a.seed, a.tag_prop, t, a.ctrl,
                                        a.respect_done);
-    propose_kernel<<<gp, 256, 0, st>>>(a.Lc, a.Z, a.phi, a.phip, V, a.ld, a.s, a.ctrl,
+    ++g_launches; propose_kernel<<<gp, 256, 0, st>>>(a.Lc, a.Z, a.phi, a.phip, V, a.ld, a.s, a.ctrl,
                                        a.respect_done);
-    accept_kernel<<<a.ld / 32, 256, 0, st>>>(
+    ++g_launches; accept_kernel<<<a.ld / 32, 256, 0, st>>>(
         a.phi, a.phip, a.S, a.U0, a.N, a.ld, a.md, a.mode, a.seed, a.tag_acc, t, a.ctrl,
         a.acc_out ? a.acc_out + (size_t)j * a.N : nullptr,
         a.margin_out ? a.margin_out + (size_t)j * a.N : nullptr, a.respect_done);

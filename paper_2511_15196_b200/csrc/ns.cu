@@ -150,7 +150,7 @@ void launch_ns_select_evidence(const NsArgs& a, cudaStream_t st) {
                          16384 * (int)sizeof(unsigned long long));
     attr_done = true;
   }
-  ns_select_evidence_kernel<<<1, 1024, smem, st>>>(a);
+  ++g_launches; ns_select_evidence_kernel<<<1, 1024, smem, st>>>(a);
 }
 
 // N3 gather: walker j <- live point start[j]; also logs the magnetisation of dead point j.
@@ -173,7 +173,7 @@ __global__ void ns_load_walkers_kernel(NsArgs a) {
 }
 
 void launch_ns_load_walkers(const NsArgs& a, cudaStream_t st) {
-  ns_load_walkers_kernel<<<(a.ldw + 127) / 128, 128, 0, st>>>(a);
+  ++g_launches; ns_load_walkers_kernel<<<(a.ldw + 127) / 128, 128, 0, st>>>(a);
 }
 
 // N3 scatter: dead slot dead[j] <- walker j.
@@ -188,7 +188,7 @@ __global__ void ns_store_walkers_kernel(NsArgs a) {
 }
 
 void launch_ns_store_walkers(const NsArgs& a, cudaStream_t st) {
-  ns_store_walkers_kernel<<<(a.k_del + 127) / 128, 128, 0, st>>>(a);
+  ++g_launches; ns_store_walkers_kernel<<<(a.k_del + 127) / 128, 128, 0, st>>>(a);
 }
 
 // N4: remaining = X mean_live(e^-S) / (Z + X mean_live(e^-S)); record; stop rule; live term.
@@ -240,7 +240,7 @@ ns_finish_kernel(NsArgs a, StepRecord* rec, int n_walk) {
 }
 
 void launch_ns_finish(const NsArgs& a, StepRecord* rec, int n_walk, cudaStream_t st) {
-  ns_finish_kernel<<<1, 1024, 0, st>>>(a, rec, n_walk);
+  ++g_launches; ns_finish_kernel<<<1, 1024, 0, st>>>(a, rec, n_walk);
 }
 
 // Posterior sample for `observables`: dead points (weight w_j e^{-S_j}) followed by the live
@@ -262,7 +262,7 @@ __global__ void ns_obs_inputs_kernel(NsArgs a, int n_dead, float* M_all, float* 
 void launch_ns_obs_inputs(const NsArgs& a, int n_dead, float* M_all, float* S_all,
                           double* logw_all, cudaStream_t st) {
   int tot = n_dead + a.n;
-  ns_obs_inputs_kernel<<<(tot + 255) / 256, 256, 0, st>>>(a, n_dead, M_all, S_all, logw_all);
+  ++g_launches; ns_obs_inputs_kernel<<<(tot + 255) / 256, 256, 0, st>>>(a, n_dead, M_all, S_all, logw_all);
 }
 
 }  // namespace phi4

@@ -14,7 +14,7 @@ __global__ void magnetisation_kernel(const float* __restrict__ phi, int N, int l
 }
 
 void launch_magnetisation(const float* phi, int N, int ld, int V, float* M, cudaStream_t st) {
-  magnetisation_kernel<<<(N + 127) / 128, 128, 0, st>>>(phi, N, ld, V, M);
+  ++g_launches; magnetisation_kernel<<<(N + 127) / 128, 128, 0, st>>>(phi, N, ld, V, M);
 }
 
 // out[0..4] = <|M|>, <M^2>, chi, <S_E>, mode balance; out[5..84] = normalised weighted histogram
@@ -75,7 +75,7 @@ observables_reduce_kernel(const float* __restrict__ M, const float* __restrict__
 
 void launch_observables_reduce(const float* M, const float* S, const double* logw, int n, int V,
                                double* out, cudaStream_t st) {
-  observables_reduce_kernel<<<1, 1024, 0, st>>>(M, S, logw, n, V, out);
+  ++g_launches; observables_reduce_kernel<<<1, 1024, 0, st>>>(M, S, logw, n, V, out);
 }
 
 }  // namespace phi4

@@ -91,7 +91,7 @@ next_delta_reweight_kernel(const float* __restrict__ S, int N, float ess_target,
 
 void launch_next_delta_reweight(const float* S, int N, float ess_target, double delta_fixed,
                                 float* w, Ctrl* ctrl, cudaStream_t st) {
-  next_delta_reweight_kernel<<<1, 1024, 0, st>>>(S, N, ess_target, delta_fixed, w, ctrl);
+  ++g_launches; next_delta_reweight_kernel<<<1, 1024, 0, st>>>(S, N, ess_target, delta_fixed, w, ctrl);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -141,7 +141,7 @@ quantise_scan_kernel(const float* __restrict__ w, int N, unsigned long long* __r
 
 void launch_quantise_scan(const float* w, int N, unsigned long long* C, Ctrl* ctrl,
                           cudaStream_t st) {
-  quantise_scan_kernel<<<1, 1024, 0, st>>>(w, N, C, ctrl);
+  ++g_launches; quantise_scan_kernel<<<1, 1024, 0, st>>>(w, N, C, ctrl);
 }
 
 // a_j = #{i : C_i <= t_j}, t_j = floor(((j 2^32 + U) T) / (N 2^32)), clamped to N-1; U = word 0
@@ -167,7 +167,7 @@ __global__ void ancestors_kernel(const unsigned long long* __restrict__ C, int N
 
 void launch_ancestors(const unsigned long long* C, int N, uint64_t seed, int32_t* anc, Ctrl* ctrl,
                       cudaStream_t st) {
-  ancestors_kernel<<<(N + 255) / 256, 256, 0, st>>>(C, N, seed, anc, ctrl);
+  ++g_launches; ancestors_kernel<<<(N + 255) / 256, 256, 0, st>>>(C, N, seed, anc, ctrl);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -221,7 +221,7 @@ void launch_gather(const float* phi_in, float* phi_out, const float* S_in, float
                    const float* U_in, float* U_out, const int32_t* anc, int N, int ld, int V,
                    Ctrl* ctrl, cudaStream_t st) {
   dim3 grid((ld / 4 + 255) / 256, (V + GATHER_ROWS - 1) / GATHER_ROWS);
-  gather_kernel<<<grid, 256, 0, st>>>(phi_in, phi_out, S_in, S_out, U_in, U_out, anc, N, ld, V,
+  ++g_launches; gather_kernel<<<grid, 256, 0, st>>>(phi_in, phi_out, S_in, S_out, U_in, U_out, anc, N, ld, V,
                                       ctrl);
 }
 
@@ -245,7 +245,7 @@ __global__ void finish_step_kernel(Ctrl* ctrl, StepRecord* rec, int max_rec, int
 }
 
 void launch_finish_step(Ctrl* ctrl, StepRecord* rec, int max_rec, int k, int N, cudaStream_t st) {
-  finish_step_kernel<<<1, 1, 0, st>>>(ctrl, rec, max_rec, k, N);
+  ++g_launches; finish_step_kernel<<<1, 1, 0, st>>>(ctrl, rec, max_rec, k, N);
 }
 
 }  // namespace phi4

@@ -19,7 +19,7 @@ def lib():
 def header_functions():
     src = open(os.path.join(ROOT, "include", "phi4smc.h")).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    names = re.findall(r"^\s*(?:const\s+char\s*\*|size_t|int|double)\s+(\w+)\s*\(", src, flags=re.M)
+    names = re.findall(r"^\s*(?:const\s+char\s*\*|size_t|int|double|uint64_t)\s+(\w+)\s*\(", src, flags=re.M)
     return sorted(set(names))
 
 
@@ -37,7 +37,7 @@ def test_struct_sizes_match_header(lib):
     from paper_2511_15196_b200 import binding as B
     assert C.sizeof(B.smc_params) == 16
     assert C.sizeof(B.smc_step_info) == 6 * 8 + 4 * 4
-    assert C.sizeof(B.ns_step_info) == 5 * 8 + 4 * 4 - 4 + 4   # 5 doubles + 3 ints, padded to 8
+    assert C.sizeof(B.ns_step_info) == 56   # 5 doubles + 3 ints, padded to 8
     assert C.sizeof(B.phi4_observables) == (5 + 80) * 8
 
 
