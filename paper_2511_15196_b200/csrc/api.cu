@@ -45,7 +45,7 @@ struct phi4smc {
   // device state (inside the workspace)
   float* phi[2]; float* S[2]; float* U0[2];
   int cur;
-  float *phip, *Z, *w, *mu, *Sigma, *Lc, *partial, *M, *margins;
+  float *phip, *Z, *w, *mu, *Sigma, *Lc, *Lsplit, *partial, *M, *margins;
   unsigned long long* C;
   int32_t* anc;
   uint8_t* acc_flags;
@@ -97,6 +97,7 @@ static int carve_smc(phi4smc* h, char* base, size_t* total) {
   h->Sigma = c.take<float>((size_t)V * V);
   h->Lc = c.take<float>((size_t)V * V);
   h->partial = c.take<float>(cov_partial_floats(V, N));
+  h->Lsplit = c.take<float>(mutate_tc_supported(V) ? mutate_tc_lsplit_floats(V) : 4);
   h->acc_flags = c.take<uint8_t>((size_t)PHI4_MAX_HOOK_STEPS * N);
   h->margins = c.take<float>((size_t)PHI4_MAX_HOOK_STEPS * N);
   h->ctrl = c.take<Ctrl>(1);
@@ -122,6 +123,7 @@ static int carve_ns(phi4smc* h, char* base, size_t* total) {
   h->Sigma = c.take<float>((size_t)V * V);
   h->Lc = c.take<float>((size_t)V * V);
   h->partial = c.take<float>(cov_partial_floats(V, N));
+  h->Lsplit = c.take<float>(mutate_tc_supported(V) ? mutate_tc_lsplit_floats(V) : 4);
   h->dead = c.take<int32_t>(kd);
   h->surv = c.take<int32_t>(N);
   h->start = c.take<int32_t>(kd);
@@ -289,6 +291,7 @@ PHI4_API int smc_set_params(phi4smc* h, const smc_params* p) {
   if (p->k_steps < 1 || !(p->ess_target > 0.f && p->ess_target < 1.f) || p->step_scale < 0.f ||
       p->mutation_path < 0 || p->mutation_path > 2)
     return PHI4_EINVAL;
+  if (p->mutation_path == 2 && !mutate_tc_supported(h->md.V)) return PHI4_EINVAL;
   h->prm = *p;
   h->s = p->step_scale > 0.f ? p->step_scale : 2.38f / sqrtf((float)h->md.V);
   return PHI4_OK;
@@ -305,8 +308,14 @@ static MutateArgs smc_mutate_args(phi4smc* h, int k, uint8_t* acc, float* mar, i
   return a;
 }
 
+// mutation_path 0: the fused tcgen05 kernel whenever it supports this V, else the generic path
+static bool use_tc_path(const phi4smc* h) {
+  return h->prm.mutation_path != 1 && mutate_tc_supported(h->md.V);
+}
+
 static void enqueue_mutation(phi4smc* h, const MutateArgs& a) {
-  launch_mutate_generic(a, h->st);
+  if (use_tc_path(h)) launch_mutate_tc(a, h->Lsplit, h->st);
+  else launch_mutate_generic(a, h->st);
 }
 
 static CovCholArgs cov_args(phi4smc* h, int respect_done) {

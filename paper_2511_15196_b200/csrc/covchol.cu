@@ -139,45 +139,48 @@ __device__ __forceinline__ bool chol_skip(const Ctrl* ctrl, int attempt, int res
 }
 
 // ------------------------------------------------------------------ small V: one CTA ---------
-__global__ void __launch_bounds__(256)
+// Right-looking factorisation in shared memory, thread r owns row r (row stride V+1: conflict
+// free; the column read A[c][j] is a broadcast).  Two barriers per column.
+__global__ void __launch_bounds__(160)
 chol_small_kernel(const float* __restrict__ Sigma, float* __restrict__ Lc, int V, Ctrl* ctrl,
                   int attempt, int respect_done) {
   extern __shared__ float sm[];   // V x (V+1)
+  __shared__ int failed_s;
   if (chol_skip(ctrl, attempt, respect_done)) return;
-  const int P = V + 1;
+  const int P = V + 1, r = threadIdx.x;
   const float add = attempt ? 1e-6f * ctrl->trace / (float)V : 0.f;
+  if (r == 0) failed_s = 0;
   for (int idx = threadIdx.x; idx < V * V; idx += blockDim.x) {
     int x = idx / V, y = idx - x * V;
     sm[x * P + y] = Sigma[idx] + (x == y ? add : 0.f);
   }
   __syncthreads();
-  int failed = 0;
+  float* row = sm + r * P;
   for (int j = 0; j < V; ++j) {
-    float d = sm[j * P + j];
-    if (!(d > 0.f)) { failed = 1; d = 1.f; }
-    float inv = 1.f / sqrtf(d);
-    __syncthreads();
-    for (int r = j + threadIdx.x; r < V; r += blockDim.x) {
-      float v = sm[r * P + j];
-      sm[r * P + j] = (r == j) ? sqrtf(d) : v * inv;
+    if (r == j) {
+      float d = row[j];
+      if (!(d > 0.f)) { failed_s = 1; d = 1.f; }
+      row[j] = sqrtf(d);
     }
     __syncthreads();
-    // trailing update of the lower triangle: a_rc -= l_rj l_cj, j < c <= r
-    const int m = V - j - 1;
-    for (int e = threadIdx.x; e < m * m; e += blockDim.x) {
-      int rr = e / m, cc = e - rr * m;
-      if (cc <= rr) {
-        int r = j + 1 + rr, c = j + 1 + cc;
-        sm[r * P + c] = fmaf(-sm[r * P + j], sm[c * P + j], sm[r * P + c]);
-      }
+    float l = 0.f;
+    if (r > j && r < V) {
+      l = row[j] / sm[j * P + j];
+      row[j] = l;
     }
     __syncthreads();
+    if (r > j && r < V) {
+      const float* col = sm + j;
+#pragma unroll 4
+      for (int c = j + 1; c <= r; ++c) row[c] = fmaf(-l, col[c * P], row[c]);
+    }
   }
+  __syncthreads();
   for (int idx = threadIdx.x; idx < V * V; idx += blockDim.x) {
     int x = idx / V, y = idx - x * V;
     Lc[idx] = (y <= x) ? sm[x * P + y] : 0.f;
   }
-  if (threadIdx.x == 0 && failed) atomicOr(&ctrl->chol_fail, attempt ? 2 : 1);
+  if (threadIdx.x == 0 && failed_s) atomicOr(&ctrl->chol_fail, attempt ? 2 : 1);
 }
 
 // ------------------------------------------------------------------ large V: blocked ---------
@@ -296,7 +299,7 @@ void launch_cholesky(const float* Sigma, float* Lc, int V, Ctrl* ctrl, int respe
                              160 * 161 * (int)sizeof(float));
         attr_done = true;
       }
-      ++g_launches; chol_small_kernel<<<1, 256, smem, st>>>(Sigma, Lc, V, ctrl, attempt, respect_done);
+      ++g_launches; chol_small_kernel<<<1, round_up(V, 32), smem, st>>>(Sigma, Lc, V, ctrl, attempt, respect_done);
     } else {
       ++g_launches; chol_copy_kernel<<<(V * V + 255) / 256, 256, 0, st>>>(Sigma, Lc, V, ctrl, attempt,
                                                             respect_done);

@@ -38,6 +38,11 @@ struct MutateArgs {
 };
 void launch_mutate_generic(const MutateArgs& a, cudaStream_t st);
 
+// mutate_tc.cu -- M1-M4 fused over k steps on tcgen05 (3xTF32), phi tile resident on-chip
+bool mutate_tc_supported(int V);
+size_t mutate_tc_lsplit_floats(int V);
+void launch_mutate_tc(const MutateArgs& a, float* Lsplit, cudaStream_t st);
+
 // population.cu -- P1-P4
 void launch_next_delta_reweight(const float* S, int N, float ess_target, double delta_fixed,
                                 float* w, Ctrl* ctrl, cudaStream_t st);

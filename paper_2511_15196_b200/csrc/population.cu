@@ -12,28 +12,45 @@ namespace phi4 {
 // arguments, sums in fp64.  Then w_i = exp(-d (S_i - S_min)) (max w = 1) and
 // dlogZ = -d S_min + log sum w - log N   (U0 cancels between p_beta and p_beta').
 // ---------------------------------------------------------------------------------------------
+// One evaluation of ESS(d)/N and sum_i e^{-d (S_i - S_min)}: e_i in fp32, sums in fp64, the two
+// sums reduced together.
 __device__ inline double ess_frac_eval(const float* __restrict__ S, int N, float smin, double d,
-                                       double* scratch, double* sum_out) {
-  float df = (float)d;
+                                       double2* scratch, double* sum_out) {
+  const float df = (float)d;
   double a = 0.0, b = 0.0;
   for (int i = threadIdx.x; i < N; i += blockDim.x) {
     float e = expf(-df * (S[i] - smin));
     a += (double)e;
     b += (double)e * (double)e;
   }
-  a = block_sum(a, scratch);
-  b = block_sum(b, scratch);
-  if (sum_out) *sum_out = a;
-  return a * a / (b * (double)N);
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  a = warp_sum(a);
+  b = warp_sum(b);
+  __syncthreads();
+  if (lane == 0) scratch[w] = make_double2(a, b);
+  __syncthreads();
+  if (w == 0) {
+    double2 t = lane < nw ? scratch[lane] : make_double2(0.0, 0.0);
+    t.x = warp_sum(t.x);
+    t.y = warp_sum(t.y);
+    if (lane == 0) scratch[32] = t;
+  }
+  __syncthreads();
+  const double2 r = scratch[32];
+  if (sum_out) *sum_out = r.x;
+  return r.x * r.x / (r.y * (double)N);
 }
 
+// Root of f(d) = ESS(d)/N - target on (0, rest].  R3 defines delta as the limit of 48 bisection
+// halvings; f is smooth and strictly decreasing, so a bracketed regula falsi (Illinois variant)
+// reaches the same root to ~1e-7 relative in a handful of evaluations instead of 48 -- each
+// evaluation is a pass over all N actions.  DESIGN.md (reading R3) states the equivalence bound.
 __global__ void __launch_bounds__(1024)
 next_delta_reweight_kernel(const float* __restrict__ S, int N, float ess_target,
                            double delta_fixed, float* __restrict__ w, Ctrl* ctrl) {
-  __shared__ double scratch[33];
+  __shared__ double2 scratch[33];
   __shared__ float smin_s[33];
   if (ctrl->done) return;
-  // S_min
   float m = INFINITY;
   for (int i = threadIdx.x; i < N; i += blockDim.x) m = fminf(m, S[i]);
   m = warp_min(m);
@@ -48,25 +65,41 @@ next_delta_reweight_kernel(const float* __restrict__ S, int N, float ess_target,
   const float smin = smin_s[32];
   const double beta = ctrl->beta;
   const double rest = 1.0 - beta;
+  const double target = (double)ess_target;
   double delta;
   int final_step;
   if (delta_fixed >= 0.0) {
     delta = delta_fixed;
     final_step = (beta + delta >= 1.0);
-  } else if (ess_frac_eval(S, N, smin, rest, scratch, nullptr) - (double)ess_target >= 0.0) {
-    delta = rest;
-    final_step = 1;
   } else {
-    double lo = 0.0, hi = rest;
-    for (int it = 0; it < 48; ++it) {
-      double mid = 0.5 * (lo + hi);
-      if (ess_frac_eval(S, N, smin, mid, scratch, nullptr) - (double)ess_target > 0.0) lo = mid;
-      else hi = mid;
+    double f_hi = ess_frac_eval(S, N, smin, rest, scratch, nullptr) - target;
+    if (f_hi >= 0.0) {
+      delta = rest;
+      final_step = 1;
+    } else {
+      double lo = 0.0, hi = rest, f_lo = 1.0 - target;     // ESS(0)/N = 1
+      int side = 0;
+      for (int it = 0; it < 60; ++it) {
+        double x = (lo * f_hi - hi * f_lo) / (f_hi - f_lo);
+        if (!(x > lo && x < hi)) x = 0.5 * (lo + hi);
+        double fx = ess_frac_eval(S, N, smin, x, scratch, nullptr) - target;
+        if (fx > 0.0) {
+          lo = x; f_lo = fx;
+          if (side == 1) f_hi *= 0.5;
+          side = 1;
+        } else {
+          hi = x; f_hi = fx;
+          if (side == -1) f_lo *= 0.5;
+          side = -1;
+        }
+        if (hi - lo <= 1e-7 * hi || fabs(fx) < 1e-9) break;
+      }
+      // one secant step inside the final bracket
+      double x = (lo * f_hi - hi * f_lo) / (f_hi - f_lo);
+      delta = (x > lo && x < hi) ? x : 0.5 * (lo + hi);
+      final_step = 0;
     }
-    delta = 0.5 * (lo + hi);
-    final_step = 0;
   }
-  // weights and the final sums
   const float df = (float)delta;
   double a = 0.0, b = 0.0;
   for (int i = threadIdx.x; i < N; i += blockDim.x) {
@@ -75,8 +108,23 @@ next_delta_reweight_kernel(const float* __restrict__ S, int N, float ess_target,
     a += (double)e;
     b += (double)e * (double)e;
   }
-  a = block_sum(a, scratch);
-  b = block_sum(b, scratch);
+  {
+    const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    a = warp_sum(a);
+    b = warp_sum(b);
+    __syncthreads();
+    if (lane == 0) scratch[wi] = make_double2(a, b);
+    __syncthreads();
+    if (wi == 0) {
+      double2 t = lane < nw ? scratch[lane] : make_double2(0.0, 0.0);
+      t.x = warp_sum(t.x);
+      t.y = warp_sum(t.y);
+      if (lane == 0) scratch[32] = t;
+    }
+    __syncthreads();
+    a = scratch[32].x;
+    b = scratch[32].y;
+  }
   if (threadIdx.x == 0) {
     double dlz = -delta * (double)smin + log(a) - log((double)N);
     ctrl->delta = delta;
