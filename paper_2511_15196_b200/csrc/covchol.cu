@@ -15,8 +15,14 @@ mean_kernel(const float* __restrict__ phi, int N, int ld, float* __restrict__ mu
   __shared__ double scratch[33];
   if (respect_done && ctrl->done) return;
   const float* row = phi + (size_t)blockIdx.x * ld;
-  double a = 0.0;
-  for (int i = threadIdx.x; i < N; i += blockDim.x) a += (double)row[i];
+  // ld is a multiple of 128 and pad particles hold zeros: whole float4s, four partial sums
+  double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+  const float4* row4 = reinterpret_cast<const float4*>(row);
+  for (int i = threadIdx.x; i < ld / 4; i += blockDim.x) {
+    float4 v = row4[i];
+    a0 += (double)v.x; a1 += (double)v.y; a2 += (double)v.z; a3 += (double)v.w;
+  }
+  double a = (a0 + a1) + (a2 + a3);
   a = block_sum(a, scratch);
   if (threadIdx.x == 0) mu[blockIdx.x] = (float)(a / (double)N);
 }
@@ -170,9 +176,21 @@ chol_small_kernel(const float* __restrict__ Sigma, float* __restrict__ Lc, int V
     }
     __syncthreads();
     if (r > j && r < V) {
+      // batches of 8 with all loads issued before the stores (row and column alias in smem, so
+      // the compiler would otherwise serialise load -> fma -> store per element)
       const float* col = sm + j;
-#pragma unroll 4
-      for (int c = j + 1; c <= r; ++c) row[c] = fmaf(-l, col[c * P], row[c]);
+      for (int c0 = j + 1; c0 <= r; c0 += 8) {
+        float cv[8], rv[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+          int c = c0 + u;
+          cv[u] = c <= r ? col[c * P] : 0.f;
+          rv[u] = c <= r ? row[c] : 0.f;
+        }
+#pragma unroll
+        for (int u = 0; u < 8; ++u)
+          if (c0 + u <= r) row[c0 + u] = fmaf(-l, cv[u], rv[u]);
+      }
     }
   }
   __syncthreads();

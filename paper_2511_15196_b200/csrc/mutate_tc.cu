@@ -26,30 +26,48 @@ namespace phi4 {
 namespace tc {
 
 constexpr int TILE = 128;            // particles per CTA = TMEM lanes
-constexpr int STAGES = 4;            // Z ring depth (K-steps in flight)
-constexpr int EPI_WARPS = 4;
+constexpr int STAGES = 4;            // Z ring depth; one stage = two K-steps (K = 16)
+constexpr int EPI_FILLS = 2;         // ring stages per step filled by the epilogue warps (<= 2)
+constexpr int EPI_PARTS = 4;         // warps per TMEM lane quarter (sites split four ways)
+constexpr int EPI_WARPS = 4 * EPI_PARTS;
 constexpr int PROD_WARPS = 8;
-constexpr int MMA_WARP = EPI_WARPS;  // warp 4
-constexpr int THREADS = (EPI_WARPS + 1 + PROD_WARPS) * 32;
-constexpr int SLAB_BYTES = 2 * 2 * TILE * 16;   // {hi,lo} x 2 K-chunks x 128 rows x 16 B
+constexpr int PROD_WARP0 = EPI_WARPS;               // warps 16..23
+constexpr int MMA_WARP = EPI_WARPS + PROD_WARPS;    // warp 24: the scheduler favours high warp ids
+constexpr int THREADS = (EPI_WARPS + 1 + PROD_WARPS) * 32;   // 800
+constexpr int CHUNK_BYTES = TILE * 16;           // one 16-byte K-chunk of all 128 rows
+constexpr int SLAB_BYTES = 2 * 4 * CHUNK_BYTES;  // {hi,lo} x 4 K-chunks
 constexpr int MAX_SMEM = 232448;
 
 __host__ __device__ inline int vn_of(int V) { return round_up(V, 16); }
 __host__ __device__ inline int kp_of(int V) { return round_up(V, 8); }
+// Lc is lower-triangular: K-step ks (columns y in [8 ks, 8 ks + 8)) only has non-zero rows
+// x >= 8 ks, so only rows [xs(ks), Vn) are stored and multiplied, xs = 8 ks rounded down to 16.
+__host__ __device__ inline int xs_of(int ks) { return (8 * ks) & ~15; }
+// rows stored before K-step ks (each K-step block holds 2 chunks x (Vn - xs) rows x 16 B)
+__host__ __device__ inline int rows_before(int ks, int Vn) {
+  int r = 0;
+  for (int j = 0; j < ks; ++j) r += Vn - xs_of(j);
+  return r;
+}
+__host__ __device__ inline size_t l_floats(int V) {     // floats per hi / lo part
+  return (size_t)rows_before(kp_of(V) / 8, vn_of(V)) * 8;
+}
 
 struct Smem {
-  size_t tile0, tile1, lhi, llo, zring, bars, total;
+  size_t tile0, tile1, lhi, llo, zring, part, dtab, bars, total;
 };
 __host__ __device__ inline Smem smem_layout(int V) {
   Smem s;
   size_t o = 0;
-  const size_t tile = (size_t)V * TILE * 4, lmat = (size_t)kp_of(V) * vn_of(V) * 4;
+  const size_t tile = (size_t)V * TILE * 4, lmat = l_floats(V) * 4;
   s.tile0 = o; o += round_up((int)tile, 128);
   s.tile1 = o; o += round_up((int)tile, 128);
   s.lhi = o; o += round_up((int)lmat, 128);
   s.llo = o; o += round_up((int)lmat, 128);
   s.zring = o; o += (size_t)STAGES * SLAB_BYTES;
-  s.bars = o; o += 256;
+  s.part = o; o += (size_t)EPI_PARTS * TILE * 8 + TILE * 4;   // partial (dS, dU0) per part and particle; ln u
+  s.dtab = o; o += 32 * 32;                        // per-K-step operand descriptors
+  s.bars = o; o += 128;
   s.total = o;
   return s;
 }
@@ -63,6 +81,9 @@ __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
 }
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_n(uint32_t bar, uint32_t n) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(n) : "memory");
 }
 __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes)
@@ -78,6 +99,21 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
       "bra WAIT_%=;\n\t"
       "DONE_%=:\n\t"
       "}" ::"r"(bar), "r"(parity)
+      : "memory");
+}
+// Same, for waiters that are not on the critical path: the thread is suspended by the hardware
+// until the phase completes (or the time hint expires), so that a waiting warp takes no issue
+// slots from the warps doing the arithmetic.
+__device__ __forceinline__ void mbar_wait_relaxed(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n\t"
+      ".reg .pred p;\n\t"
+      "WAITR_%=:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n\t"
+      "@p bra DONER_%=;\n\t"
+      "bra WAITR_%=;\n\t"
+      "DONER_%=:\n\t"
+      "}" ::"r"(bar), "r"(parity), "r"(1000000u)
       : "memory");
 }
 __device__ __forceinline__ void fence_proxy_async() {
@@ -134,6 +170,8 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&r)[16]) {
         "=r"(r[14]), "=r"(r[15])
       : "r"(taddr)
       : "memory");
+}
+__device__ __forceinline__ void tmem_ld_wait() {
   asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 }
 
@@ -159,6 +197,14 @@ __device__ __forceinline__ float tf32_rna(float x) {
 
 }  // namespace tc
 
+#ifdef PHI4_TC_TRACE
+// Debug build only (never defined by build.py): per-role clock64 stamps of CTA 0.
+__device__ long long g_tc_trace[3 * 4096];
+#define TC_TRACE(role, cnt) do { if (blockIdx.x == 0 && (cnt) < 4096) g_tc_trace[(role) * 4096 + (cnt)++] = clock64(); } while (0)
+#else
+#define TC_TRACE(role, cnt) do { } while (0)
+#endif
+
 struct TcParams {
   float* phi; float* S; float* U0;
   const float* Lsplit;         // [2][Kp/4][Vn][4]: s*Lc split hi/lo, UMMA K-major interleave layout
@@ -172,30 +218,109 @@ struct TcParams {
   int k, respect_done;
 };
 
-// (s Lc) -> hi/lo TF32 split in the layout the MMA reads: element (x, y) of part h at
-// ((h*(Kp/4) + y/4) * Vn + x) * 4 + y%4; zero outside the lower triangle / beyond V.
+// (s Lc) -> hi/lo TF32 split in the layout the MMA reads.  K-step ks is a block of two 16-byte
+// K-chunks over the rows [xs(ks), Vn): element (x, y), ks = y / 8, sits at float offset
+//   8 rows_before(ks) + ((y % 8) / 4) (Vn - xs) 4 + (x - xs) 4 + y % 4
+// of its part (hi, then lo after l_floats(V) floats).  Zero beyond V (the strict upper triangle
+// inside a block is zero in Lc itself).
 __global__ void lsplit_kernel(const float* __restrict__ Lc, int V, int Vn, int Kp, float s,
                               float* __restrict__ out, const Ctrl* ctrl, int respect_done) {
   if (respect_done && ctrl->done) return;
   int idx = blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= Kp * Vn) return;
-  int y = idx / Vn, x = idx - y * Vn;
+  const int y = idx / Vn, x = idx - y * Vn;
+  const int ks = y >> 3, xs = tc::xs_of(ks);
+  if (x < xs) return;
   float v = (x < V && y < V && y <= x) ? s * Lc[(size_t)x * V + y] : 0.f;
   float hi = tc::tf32_rna(v);
   float lo = tc::tf32_rna(v - hi);
-  size_t o = ((size_t)(y >> 2) * Vn + x) * 4 + (y & 3);
+  const int rows = Vn - xs;
+  size_t o = (size_t)tc::rows_before(ks, Vn) * 8 + (size_t)((y & 7) >> 2) * rows * 4 +
+             (size_t)(x - xs) * 4 + (y & 3);
   out[o] = hi;
-  out[(size_t)Kp * Vn + o] = lo;
+  out[tc::l_floats(V) + o] = lo;
 }
 
+// Per-site difference of Eq. 1 between phi' (a2; forward neighbours b2, c2) and phi (a; b, c) in
+// the lattice-Laplacian form: on the periodic lattice
+//   S_E = sum_x [ (2 + m0^2/2) phi_x^2 + lambda phi_x^4 - phi_x (phi_{x+1} + phi_{x+2}) ],
+// which is Eq. 1 with the squares expanded (each site appears in four bonds).  With
+// q = a2^2 - a^2 formed as (a2-a)(a2+a), the potential part does not cancel; the bond part
+// a2 (b2+c2) - a (b+c) carries an fp32 rounding of ~3e-7 per site, 3e-6 over the V <= 112 sites
+// of this kernel -- far inside the 1e-4 decision band.  (The generic path, used up to V = 4096,
+// keeps the fully difference-based form.)
 __device__ __forceinline__ void tc_site_diff(float a, float b, float c, float a2, float b2,
-                                             float c2, float hm, float lam, float& dS, float& dU) {
-  float q = (a2 - a) * (a2 + a);
-  float e = b - a, e2 = b2 - a2, f = c - a, f2 = c2 - a2;
-  dS += 0.5f * ((e2 - e) * (e2 + e) + (f2 - f) * (f2 + f)) + q * (hm + lam * (a2 * a2 + a * a));
-  dU += 0.5f * q;
+                                             float c2, float c2m, float lam, float& dS, float& dU) {
+  const float q = (a2 - a) * (a2 + a);
+  dS = fmaf(q, fmaf(lam, fmaf(a2, a2, a * a), c2m), dS);
+  dS = fmaf(a, b + c, dS);
+  dS = fmaf(-a2, b2 + c2, dS);
+  dU = fmaf(0.5f, q, dU);
 }
 
+// Differences of Eq. 1 / U0 over the lattice rows r = g, g + EPI_PARTS, ... of one particle
+// (column `pr` of the site-major tiles).  LT > 0: the lattice size is a compile-time constant, a
+// row is fully unrolled -- all 4 LT shared-memory loads of a row (immediate offsets) are in
+// flight before the arithmetic.  LT = 0: any L, one site at a time.
+template <int LT>
+__device__ __forceinline__ void tc_stencil(const float* cur, const float* oth, int g, int Lrt,
+                                           float c2m, float lam, float& dS, float& dU) {
+  using namespace tc;
+  if constexpr (LT > 0) {
+    float s0 = 0.f, u0 = 0.f, s1 = 0.f, u1 = 0.f;
+    for (int r = g; r < LT; r += EPI_PARTS) {
+      const int rn = (r + 1 == LT) ? 0 : r + 1;
+      const float* c0 = cur + r * LT * TILE; const float* c1 = cur + rn * LT * TILE;
+      const float* o0 = oth + r * LT * TILE; const float* o1 = oth + rn * LT * TILE;
+      float a[LT], a2[LT], d[LT], d2[LT];
+#pragma unroll
+      for (int c = 0; c < LT; ++c) {
+        a[c] = c0[c * TILE]; a2[c] = o0[c * TILE];
+        d[c] = c1[c * TILE]; d2[c] = o1[c * TILE];
+      }
+#pragma unroll
+      for (int c = 0; c < LT; ++c) {
+        constexpr int dummy = 0; (void)dummy;
+        const int cn = (c + 1 == LT) ? 0 : c + 1;
+        if (c & 1) tc_site_diff(a[c], a[cn], d[c], a2[c], a2[cn], d2[c], c2m, lam, s1, u1);
+        else tc_site_diff(a[c], a[cn], d[c], a2[c], a2[cn], d2[c], c2m, lam, s0, u0);
+      }
+    }
+    dS = s0 + s1;
+    dU = u0 + u1;
+  } else {
+    const int L = Lrt;
+    for (int r = g; r < L; r += EPI_PARTS) {
+      const int rn = (r + 1 == L) ? 0 : r + 1;
+      const float* c0 = cur + r * L * TILE; const float* c1 = cur + rn * L * TILE;
+      const float* o0 = oth + r * L * TILE; const float* o1 = oth + rn * L * TILE;
+      float a = c0[0], a2 = o0[0];
+      for (int c = 0; c < L; ++c) {
+        const int cn = (c + 1 == L) ? 0 : c + 1;
+        float b = c0[cn * TILE], b2 = o0[cn * TILE];
+        float d = c1[c * TILE], d2 = o1[c * TILE];
+        tc_site_diff(a, b, d, a2, b2, d2, c2m, lam, dS, dU);
+        a = b;
+        a2 = b2;
+      }
+    }
+  }
+}
+
+__device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
+  asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+
+// Warp roles (800 threads, one CTA per SM):
+//   warps 0..15   epilogue.  Warp w serves TMEM lane quarter Q = w % 4 (the hardware lets a warp
+//                 read only lanes 32 (w % 4) .. +31) and site part g = w / 4: the four warps of a
+//                 quarter split the 16-column TMEM blocks and the lattice rows of their 32
+//                 particles and meet at named barrier 1 + Q.
+//   warps 16..23  normal producers: thread (particle row, half) draws two Philox quads per ring
+//                 stage, two stages (four independent chains) per pass.
+//   warp 24       one thread issues every tcgen05.mma and the bulk copy of Lc; the operand
+//                 descriptors of all K-steps are tabulated once in shared memory by its 32 lanes.
+template <int LT>
 __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParams p) {
   using namespace tc;
   extern __shared__ __align__(1024) uint8_t smem[];
@@ -203,8 +328,9 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
   const Smem lay = smem_layout(p.V);
   float* tile0 = reinterpret_cast<float*>(smem + lay.tile0);
   float* tile1 = reinterpret_cast<float*>(smem + lay.tile1);
+  float2* part = reinterpret_cast<float2*>(smem + lay.part);
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + lay.bars);
-  // barrier slots: zfull[4] zempty[4] dfull[2] dempty[2] lfull, then the TMEM base slot
+  // barrier slots: zfull[S] zempty[S] dfull[2] dempty[2] lfull, then the TMEM base slot
   const uint32_t bar0 = smem_u32(bars);
   auto zfull = [&](int s) { return bar0 + 8u * s; };
   auto zempty = [&](int s) { return bar0 + 8u * (STAGES + s); };
@@ -214,13 +340,16 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * STAGES + 5);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int V = p.V, Vn = p.Vn, Kp = p.Kp, nk8 = Kp >> 3;
+  const int V = p.V, Vn = p.Vn, Kp = p.Kp, nk8 = Kp >> 3, nit = (nk8 + 1) >> 1;
+  // the last nitE ring fills of every step are produced by the epilogue warps (one quad per
+  // thread), the first nitP by the dedicated producers (two quads per thread)
+  const int nitE = min(EPI_FILLS, nit - 1), nitP = nit - nitE;
   const int i0 = blockIdx.x * TILE;
   uint32_t ncols = 32;
   while ((int)ncols < 2 * Vn) ncols <<= 1;
 
   if (warp == MMA_WARP && lane == 0) {
-    for (int s = 0; s < STAGES; ++s) { mbar_init(zfull(s), PROD_WARPS); mbar_init(zempty(s), 1); }
+    for (int s = 0; s < STAGES; ++s) { mbar_init(zfull(s), EPI_WARPS); mbar_init(zempty(s), 1); }
     for (int b = 0; b < 2; ++b) { mbar_init(dfull(b), 1); mbar_init(dempty(b), EPI_WARPS); }
     mbar_init(lfull, 1);
     fence_mbar_init();
@@ -233,124 +362,245 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
 
   if (warp == MMA_WARP) {
     // ================================ MMA issuer (one thread) =================================
+    // per-K-step table: {b_hi, b_lo, idesc, first row xs}; lane ks fills entry ks
+    struct KStep { uint64_t b_hi, b_lo; uint32_t idesc, xs, pad0, pad1; };
+    KStep* tab = reinterpret_cast<KStep*>(smem + lay.dtab);
+    {
+      const uint32_t lhi = smem_u32(smem + lay.lhi), llo = smem_u32(smem + lay.llo);
+      for (int ks = lane; ks < nk8; ks += 32) {
+        const int xs = xs_of(ks);
+        const uint32_t lbo_b = (uint32_t)(Vn - xs) * 16;
+        const uint32_t boff = (uint32_t)rows_before(ks, Vn) * 32;
+        KStep e;
+        e.b_hi = smem_desc(lhi + boff, lbo_b, 128);
+        e.b_lo = smem_desc(llo + boff, lbo_b, 128);
+        e.idesc = instr_desc(TILE, Vn - xs);
+        e.xs = (uint32_t)xs; e.pad0 = 0; e.pad1 = 0;
+        tab[ks] = e;
+      }
+    }
+    __syncwarp();
     if (lane == 0) {
-      const uint32_t lbytes = (uint32_t)Kp * Vn * 4;
+      const uint32_t lbytes = (uint32_t)l_floats(V) * 4;
       mbar_expect_tx(lfull, 2 * lbytes);
       bulk_g2s(smem_u32(smem + lay.lhi), p.Lsplit, lbytes, lfull);
-      bulk_g2s(smem_u32(smem + lay.llo), p.Lsplit + (size_t)Kp * Vn, lbytes, lfull);
+      bulk_g2s(smem_u32(smem + lay.llo), p.Lsplit + l_floats(V), lbytes, lfull);
       mbar_wait(lfull, 0);
-      const uint32_t lhi = smem_u32(smem + lay.lhi), llo = smem_u32(smem + lay.llo);
-      const uint32_t zr = smem_u32(smem + lay.zring);
-      const uint32_t lbo_b = (uint32_t)Vn * 16;
+      // A descriptors differ only in the start address: slot s, K-step kk, hi / lo part
+      const uint64_t a_base = smem_desc(smem_u32(smem + lay.zring), CHUNK_BYTES, 128);
       int s = 0;
       uint32_t ph = 0;
+      int tr = 0; (void)tr;
       for (int t = 0; t < p.k; ++t) {
         const int buf = t & 1;
+        TC_TRACE(0, tr);
         mbar_wait(dempty(buf), ((t >> 1) & 1) ^ 1);
         tc_fence_after();
-        for (int ks = 0; ks < nk8; ++ks) {
+        TC_TRACE(0, tr);
+        const uint32_t dbase = taddr + (uint32_t)(buf * Vn);
+        for (int it = 0; it < nit; ++it) {
+          const KStep e0 = tab[2 * it];
+          const KStep e1 = tab[min(2 * it + 1, nk8 - 1)];
+          const uint64_t a0 = a_base + (uint64_t)((uint32_t)s * (SLAB_BYTES >> 4));
           mbar_wait(zfull(s), ph);
           tc_fence_after();
-          // rows x < 8 ks of this K-step are zero: start at the 16-aligned row below
-          const int xs = (8 * ks) & ~15;
-          const int n = Vn - xs;
-          const uint32_t idesc = instr_desc(TILE, n);
-          const uint32_t d = taddr + (uint32_t)(buf * Vn + xs);
-          const uint32_t za = zr + (uint32_t)s * SLAB_BYTES;
-          const uint64_t a_hi = smem_desc(za, TILE * 16, 128);
-          const uint64_t a_lo = smem_desc(za + 2 * TILE * 16, TILE * 16, 128);
-          const uint32_t boff = (uint32_t)(2 * ks) * lbo_b + (uint32_t)xs * 16;
-          const uint64_t b_hi = smem_desc(lhi + boff, lbo_b, 128);
-          const uint64_t b_lo = smem_desc(llo + boff, lbo_b, 128);
+          TC_TRACE(0, tr);
           // the first K-step (xs = 0) overwrites all Vn columns; later ones accumulate
-          tc_mma_tf32(d, a_lo, b_hi, idesc, ks > 0);
-          tc_mma_tf32(d, a_hi, b_lo, idesc, 1);
-          tc_mma_tf32(d, a_hi, b_hi, idesc, 1);
+          tc_mma_tf32(dbase + e0.xs, a0 + (4 * CHUNK_BYTES >> 4), e0.b_hi, e0.idesc, it > 0);
+          tc_mma_tf32(dbase + e0.xs, a0, e0.b_lo, e0.idesc, 1);
+          tc_mma_tf32(dbase + e0.xs, a0, e0.b_hi, e0.idesc, 1);
+          if (2 * it + 1 < nk8) {
+            const uint64_t a1 = a0 + (2 * CHUNK_BYTES >> 4);
+            tc_mma_tf32(dbase + e1.xs, a1 + (4 * CHUNK_BYTES >> 4), e1.b_hi, e1.idesc, 1);
+            tc_mma_tf32(dbase + e1.xs, a1, e1.b_lo, e1.idesc, 1);
+            tc_mma_tf32(dbase + e1.xs, a1, e1.b_hi, e1.idesc, 1);
+          }
           tc_commit(zempty(s));
+          TC_TRACE(0, tr);
           if (++s == STAGES) { s = 0; ph ^= 1; }
         }
         tc_commit(dfull(buf));
       }
     }
     __syncwarp();
-  } else if (warp > MMA_WARP) {
+  } else if (warp >= PROD_WARP0) {
     // ================================ normal producers =======================================
-    const int j = threadIdx.x - (MMA_WARP + 1) * 32;     // 0..255
+    const int j = threadIdx.x - PROD_WARP0 * 32;         // 0..255
     const int pr = j & (TILE - 1), half = j >> 7;
     const int i = i0 + pr;
     const int nq = (V + 3) >> 2;
     uint8_t* zr = smem + lay.zring;
-    int s = 0;
-    uint32_t ph = 0;
+    int tr = (j == 0) ? 0 : 4096; (void)tr;
     for (int t = 0; t < p.k; ++t) {
-      for (int ks = 0; ks < nk8; ++ks) {
-        const int q = 2 * ks + half;
-        float z[4] = {0.f, 0.f, 0.f, 0.f};
-        if (q < nq && i < p.N) normals4(p.seed, p.tag_prop, p.t0 + (uint32_t)t, (uint32_t)i, (uint32_t)q, z);
-        float4 hi, lo;
-        hi.x = tf32_rna(z[0]); lo.x = tf32_rna(z[0] - hi.x);
-        hi.y = tf32_rna(z[1]); lo.y = tf32_rna(z[1] - hi.y);
-        hi.z = tf32_rna(z[2]); lo.z = tf32_rna(z[2] - hi.z);
-        hi.w = tf32_rna(z[3]); lo.w = tf32_rna(z[3] - hi.w);
-        mbar_wait(zempty(s), ph ^ 1);
-        uint8_t* slab = zr + (size_t)s * SLAB_BYTES + (size_t)half * (TILE * 16) + (size_t)pr * 16;
-        *reinterpret_cast<float4*>(slab) = hi;
-        *reinterpret_cast<float4*>(slab + 2 * TILE * 16) = lo;
-        fence_proxy_async();
-        __syncwarp();
-        if (lane == 0) mbar_arrive(zfull(s));
-        if (++s == STAGES) { s = 0; ph ^= 1; }
+      const uint32_t tt = p.t0 + (uint32_t)t;
+      // two ring stages (four Philox chains) per pass: the chains are independent, so their
+      // latencies overlap inside the warp
+      for (int it = 0; it < nitP; it += 2) {
+        TC_TRACE(1, tr);
+        const bool second = it + 1 < nitP;
+        U4 w[4];
+        bool ok[4];
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+          const int q = 4 * (it + (c >> 1)) + 2 * (c & 1) + half;   // stage it + c/2, chunk 2 (c%2) + half
+          ok[c] = (i < p.N) && (q < nq) && (c < 2 || second);
+        }
+        if (second) {
+#pragma unroll
+          for (int c = 0; c < 4; ++c)
+            w[c] = philox_draw(p.seed, p.tag_prop, tt, (uint32_t)i, (uint32_t)(4 * (it + (c >> 1)) + 2 * (c & 1) + half));
+        } else {
+#pragma unroll
+          for (int c = 0; c < 2; ++c)
+            w[c] = philox_draw(p.seed, p.tag_prop, tt, (uint32_t)i, (uint32_t)(4 * it + 2 * c + half));
+          w[2] = w[0]; w[3] = w[1];
+        }
+        TC_TRACE(1, tr);
+#pragma unroll
+        for (int st2 = 0; st2 < 2; ++st2) {
+          if (st2 == 1 && !second) break;
+          float4 hv[2], lv[2];
+#pragma unroll
+          for (int e = 0; e < 2; ++e) {
+            const int c = 2 * st2 + e;
+            float z[4] = {0.f, 0.f, 0.f, 0.f};
+            if (ok[c]) {
+              box_muller_fast(w[c].x, w[c].y, z[0], z[1]);
+              box_muller_fast(w[c].z, w[c].w, z[2], z[3]);
+            }
+            // hi = rna_tf32(z); lo = z - hi is exact and |lo| <= 2^-12 |z|: the tensor core's own
+            // truncation of lo to 11 bits costs 2^-23 |z|, below the dropped lo*lo term
+            hv[e].x = tf32_rna(z[0]); lv[e].x = z[0] - hv[e].x;
+            hv[e].y = tf32_rna(z[1]); lv[e].y = z[1] - hv[e].y;
+            hv[e].z = tf32_rna(z[2]); lv[e].z = z[2] - hv[e].z;
+            hv[e].w = tf32_rna(z[3]); lv[e].w = z[3] - hv[e].w;
+          }
+          const int n = t * nit + it + st2, s = n % STAGES;    // ring slot and use of fill n
+          const uint32_t ph = (uint32_t)(n / STAGES) & 1u;
+          mbar_wait_relaxed(zempty(s), ph ^ 1);
+          uint8_t* st = zr + (size_t)s * SLAB_BYTES + (size_t)half * CHUNK_BYTES + (size_t)pr * 16;
+          *reinterpret_cast<float4*>(st) = hv[0];
+          *reinterpret_cast<float4*>(st + 2 * CHUNK_BYTES) = hv[1];
+          *reinterpret_cast<float4*>(st + 4 * CHUNK_BYTES) = lv[0];
+          *reinterpret_cast<float4*>(st + 6 * CHUNK_BYTES) = lv[1];
+          fence_proxy_async();
+          __syncwarp();
+          if (lane == 0) mbar_arrive_n(zfull(s), 2);         // 8 warps x 2 = the 16 expected
+        }
+        TC_TRACE(1, tr);
+        TC_TRACE(1, tr);
       }
     }
   } else {
-    // ================================ epilogue: thread = particle =============================
-    const int pr = threadIdx.x;                 // 0..127 = TMEM lane
+    // ================================ epilogue ==============================================
+    const int Q = warp & 3, g = warp >> 2;       // lane quarter, site part
+    const int pr = Q * 32 + lane;                // particle row = TMEM lane
     const int i = i0 + pr;
     const bool live = i < p.N;
-    const int L = p.L;
-    const float hm = 0.5f * p.m0sq, lam = p.lam;
+    const int L = LT > 0 ? LT : p.L;
+    const float hm = 2.0f + 0.5f * p.m0sq, lam = p.lam;   // coefficient of phi^2 in the Laplacian form
     float* cur = tile0 + pr;
     float* oth = tile1 + pr;
-    for (int x = 0; x < V; ++x) cur[x * TILE] = live ? p.phi[(size_t)x * p.ld + i] : 0.f;
+    for (int x = g; x < V; x += EPI_PARTS) cur[x * TILE] = live ? p.phi[(size_t)x * p.ld + i] : 0.f;
     float Si = live ? p.S[i] : 0.f, Ui = live ? p.U0[i] : 0.f;
     const float beta = (float)p.ctrl->beta, S_star = (float)p.ctrl->S_star;
     unsigned nacc = 0;
-    const uint32_t tlane = taddr + ((uint32_t)(warp * 32) << 16);
+    const uint32_t tlane = taddr + ((uint32_t)(Q * 32) << 16);
+    named_bar_sync(1 + Q, 32 * EPI_PARTS);
+    float* lus = reinterpret_cast<float*>(part + EPI_PARTS * TILE);
+    uint8_t* zr = smem + lay.zring;
+    const int nq = (V + 3) >> 2;
+    // this thread's share of the normals of step t: quad 4 it + g of its own particle row
+    auto fill = [&](int t) {
+      // up to EPI_FILLS (= 2) stages: both Philox chains first, then the maps and the stores
+      U4 w[2];
+#pragma unroll
+      for (int e = 0; e < 2; ++e)
+        if (e < nitE) w[e] = philox_draw(p.seed, p.tag_prop, p.t0 + (uint32_t)t, (uint32_t)i, (uint32_t)(4 * (nitP + e) + g));
+#pragma unroll
+      for (int e = 0; e < 2; ++e) {
+        if (e >= nitE) break;
+        const int it = nitP + e, q = 4 * it + g;
+        float z[4] = {0.f, 0.f, 0.f, 0.f};
+        if (live && q < nq) {
+          box_muller_fast(w[e].x, w[e].y, z[0], z[1]);
+          box_muller_fast(w[e].z, w[e].w, z[2], z[3]);
+        }
+        float4 hv, lv;
+        hv.x = tf32_rna(z[0]); lv.x = z[0] - hv.x;  hv.y = tf32_rna(z[1]); lv.y = z[1] - hv.y;
+        hv.z = tf32_rna(z[2]); lv.z = z[2] - hv.z;  hv.w = tf32_rna(z[3]); lv.w = z[3] - hv.w;
+        const int n = t * nit + it, s = n % STAGES;
+        const uint32_t ph = (uint32_t)(n / STAGES) & 1u;
+        mbar_wait_relaxed(zempty(s), ph ^ 1);
+        uint8_t* st = zr + (size_t)s * SLAB_BYTES + (size_t)g * CHUNK_BYTES + (size_t)pr * 16;
+        *reinterpret_cast<float4*>(st) = hv;
+        *reinterpret_cast<float4*>(st + 4 * CHUNK_BYTES) = lv;
+        fence_proxy_async();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(zfull(s));
+      }
+    };
+    fill(0);
+    int tr = (threadIdx.x == 0) ? 0 : 4096; (void)tr;
     for (int t = 0; t < p.k; ++t) {
       const int buf = t & 1;
-      mbar_wait(dfull(buf), (t >> 1) & 1);
+      TC_TRACE(2, tr);
+      mbar_wait_relaxed(dfull(buf), (t >> 1) & 1);
       tc_fence_after();
-      // pass 1: phi' = phi + d  (d already carries the step scale s)
-      for (int cb = 0; cb < Vn; cb += 16) {
-        uint32_t r[16];
-        tmem_ld16(tlane + (uint32_t)(buf * Vn + cb), r);
+      TC_TRACE(2, tr);
+      // pass 1: phi' = phi + d on this part's 16-column blocks (d carries the step scale s); two
+      // TMEM loads in flight per wait
+      for (int cb = 16 * g; cb < Vn; cb += 32 * EPI_PARTS) {
+        uint32_t r0[16], r1[16];
+        const int cb1 = cb + 16 * EPI_PARTS;
+        const bool two = cb1 < Vn;
+        tmem_ld16(tlane + (uint32_t)(buf * Vn + cb), r0);
+        if (two) tmem_ld16(tlane + (uint32_t)(buf * Vn + cb1), r1);
+        tmem_ld_wait();
+        const float* ci = cur + cb * TILE; float* oi = oth + cb * TILE;
+        if (cb + 16 <= V) {
 #pragma unroll
-        for (int jj = 0; jj < 16; ++jj) {
-          int x = cb + jj;
-          if (x < V) oth[x * TILE] = cur[x * TILE] + __uint_as_float(r[jj]);
+          for (int jj = 0; jj < 16; ++jj) oi[jj * TILE] = ci[jj * TILE] + __uint_as_float(r0[jj]);
+        } else {
+#pragma unroll
+          for (int jj = 0; jj < 16; ++jj)
+            if (cb + jj < V) oi[jj * TILE] = ci[jj * TILE] + __uint_as_float(r0[jj]);
+        }
+        if (two) {
+          ci = cur + cb1 * TILE; oi = oth + cb1 * TILE;
+          if (cb1 + 16 <= V) {
+#pragma unroll
+            for (int jj = 0; jj < 16; ++jj) oi[jj * TILE] = ci[jj * TILE] + __uint_as_float(r1[jj]);
+          } else {
+#pragma unroll
+            for (int jj = 0; jj < 16; ++jj)
+              if (cb1 + jj < V) oi[jj * TILE] = ci[jj * TILE] + __uint_as_float(r1[jj]);
+          }
         }
       }
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive(dempty(buf));
-      // pass 2: per-site differences of Eq. 1 and U0
+      TC_TRACE(2, tr);
+      named_bar_sync(1 + Q, 32 * EPI_PARTS);       // the whole proposal of these 32 particles is in smem
+      TC_TRACE(2, tr);
+      // pass 2: per-site differences of Eq. 1 and U0 over this part's lattice rows
       float dS = 0.f, dU = 0.f;
-      for (int r = 0; r < L; ++r) {
-        const int rn = (r + 1 == L) ? 0 : r + 1;
-        const float* c0 = cur + r * L * TILE; const float* c1 = cur + rn * L * TILE;
-        const float* o0 = oth + r * L * TILE; const float* o1 = oth + rn * L * TILE;
-        float a = c0[0], a2 = o0[0];
-        for (int c = 0; c < L; ++c) {
-          const int cn = (c + 1 == L) ? 0 : c + 1;
-          float b = c0[cn * TILE], b2 = o0[cn * TILE];
-          float d = c1[c * TILE], d2 = o1[c * TILE];
-          tc_site_diff(a, b, d, a2, b2, d2, hm, lam, dS, dU);
-          a = b;
-          a2 = b2;
-        }
+      tc_stencil<LT>(cur, oth, g, L, hm, lam, dS, dU);
+      part[g * TILE + pr] = make_float2(dS, dU);
+      if (g == 0) lus[pr] = log_uniform(p.seed, p.tag_acc, p.t0 + (uint32_t)t, (uint32_t)i);
+      TC_TRACE(2, tr);
+      named_bar_sync(1 + Q, 32 * EPI_PARTS);
+      TC_TRACE(2, tr);
+      // every part sums the four partials in the same order and takes the same decision (M4)
+      dS = 0.f; dU = 0.f;
+#pragma unroll
+      for (int m = 0; m < EPI_PARTS; ++m) {
+        float2 v = part[m * TILE + pr];
+        dS += v.x;
+        dU += v.y;
       }
-      // M4
-      const float lu = log_uniform(p.seed, p.tag_acc, p.t0 + (uint32_t)t, (uint32_t)i);
+      const float lu = lus[pr];
       float margin;
       bool acc;
       if (p.mode == MODE_SMC) {
@@ -367,19 +617,21 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
         Ui += dU;
         ++nacc;
       }
-      if (live) {
+      if (live && g == 0) {
         if (p.acc_out) p.acc_out[(size_t)t * p.N + i] = (uint8_t)acc;
         if (p.margin_out) p.margin_out[(size_t)t * p.N + i] = margin;
       }
+      if (t + 1 < p.k) fill(t + 1);
     }
     if (live) {
-      for (int x = 0; x < V; ++x) p.phi[(size_t)x * p.ld + i] = cur[x * TILE];
-      p.S[i] = Si;
-      p.U0[i] = Ui;
+      for (int x = g; x < V; x += EPI_PARTS) p.phi[(size_t)x * p.ld + i] = cur[x * TILE];
+      if (g == 0) { p.S[i] = Si; p.U0[i] = Ui; }
     }
+    if (g == 0) {
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) nacc += __shfl_xor_sync(0xffffffffu, nacc, o);
-    if (lane == 0 && nacc) atomicAdd(&p.ctrl->n_accept, nacc);
+      for (int o = 16; o > 0; o >>= 1) nacc += __shfl_xor_sync(0xffffffffu, nacc, o);
+      if (lane == 0 && nacc) atomicAdd(&p.ctrl->n_accept, nacc);
+    }
   }
   tc_fence_before();
   __syncthreads();
@@ -390,7 +642,13 @@ bool mutate_tc_supported(int V) {
   return V >= 1 && tc::vn_of(V) <= 256 && tc::smem_layout(V).total <= (size_t)tc::MAX_SMEM;
 }
 
-size_t mutate_tc_lsplit_floats(int V) { return (size_t)2 * tc::kp_of(V) * tc::vn_of(V); }
+size_t mutate_tc_lsplit_floats(int V) { return 2 * tc::l_floats(V); }
+
+#ifdef PHI4_TC_TRACE
+extern "C" __attribute__((visibility("default"))) int phi4_debug_tc_trace(long long* out) {
+  return (int)cudaMemcpyFromSymbol(out, g_tc_trace, sizeof(long long) * 3 * 4096);
+}
+#endif
 
 void launch_mutate_tc(const MutateArgs& a, float* Lsplit, cudaStream_t st) {
   const int V = a.md.V, Vn = tc::vn_of(V), Kp = tc::kp_of(V);
@@ -406,11 +664,17 @@ void launch_mutate_tc(const MutateArgs& a, float* Lsplit, cudaStream_t st) {
   const size_t smem = tc::smem_layout(V).total;
   static bool attr_done = false;
   if (!attr_done) {
-    cudaFuncSetAttribute(mutate_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                         tc::MAX_SMEM);
+    cudaFuncSetAttribute(mutate_tc_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::MAX_SMEM);
+    cudaFuncSetAttribute(mutate_tc_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::MAX_SMEM);
+    cudaFuncSetAttribute(mutate_tc_kernel<10>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::MAX_SMEM);
     attr_done = true;
   }
-  ++g_launches; mutate_tc_kernel<<<a.ld / tc::TILE, tc::THREADS, smem, st>>>(p);
+  const dim3 grid(a.ld / tc::TILE);
+  ++g_launches;
+  // lattice sizes of the BASELINE configs get a fully unrolled stencil; any other L the loop
+  if (p.L == 10) mutate_tc_kernel<10><<<grid, tc::THREADS, smem, st>>>(p);
+  else if (p.L == 4) mutate_tc_kernel<4><<<grid, tc::THREADS, smem, st>>>(p);
+  else mutate_tc_kernel<0><<<grid, tc::THREADS, smem, st>>>(p);
 }
 
 }  // namespace phi4

@@ -15,12 +15,13 @@ __device__ __forceinline__ U4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c
   constexpr uint32_t W0 = 0x9E3779B9u, W1 = 0xBB67AE85u;
 #pragma unroll
   for (int r = 0; r < 10; ++r) {
-    uint32_t h0 = __umulhi(M0, c0), l0 = M0 * c0;
-    uint32_t h1 = __umulhi(M1, c2), l1 = M1 * c2;
-    c0 = h1 ^ c1 ^ k0;
-    c2 = h0 ^ c3 ^ k1;
-    c1 = l1;
-    c3 = l0;
+    // one 32x32->64 multiply per product (IMAD.WIDE), one 3-input XOR (LOP3) per word
+    const uint64_t p0 = (uint64_t)M0 * (uint64_t)c0;
+    const uint64_t p1 = (uint64_t)M1 * (uint64_t)c2;
+    c0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0;
+    c2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
+    c1 = (uint32_t)p1;
+    c3 = (uint32_t)p0;
     k0 += W0;
     k1 += W1;
   }
@@ -42,6 +43,34 @@ __device__ __forceinline__ void box_muller(uint32_t xa, uint32_t xb, float& za, 
   sincospif((float)(xb >> 8) * 1.1920928955078125e-7f, &sn, &cs);  // 2^-23
   za = r * cs;
   zb = r * sn;
+}
+
+// Same map on the special-function unit, for the fused mutation kernel whose issue slots the
+// normals dominate: lg2.approx on u in (0,1] (absolute error 2^-22 on [0.5,1), 2 ulp below),
+// sqrt.approx, sin/cos.approx on the angle reduced exactly (in integers) to [-pi, pi).  The last
+// 2^12 radius codes (u > 1 - 2.4e-4, where the absolute error of lg2 would dominate r) take the
+// accurate logf.  Resulting |dz| vs the exact map: ~5e-7 typical, < 1e-5 worst case, i.e. a
+// proposal perturbation of the order of the fp32 rounding of phi' itself (R2).
+__device__ __forceinline__ void box_muller_fast(uint32_t xa, uint32_t xb, float& za, float& zb) {
+  const uint32_t m = (xa >> 8) + 1u;                             // 1 .. 2^24
+  const float ur = (float)m * 5.9604644775390625e-8f;            // exact
+  float w;
+  if (m > 16777216u - 4096u) w = -2.0f * logf(ur);
+  else w = -1.3862943611198906f * __log2f(ur);
+  float r;
+  asm("sqrt.approx.f32 %0, %1;" : "=f"(r) : "f"(w));
+  const uint32_t kb = xb >> 8;                                   // angle code, 24 bits
+  const int sk = (int)kb - (int)((kb & 0x800000u) << 1);         // same angle in [-2^23, 2^23)
+  const float th = (float)sk * 3.7450702829238413e-7f;           // 2 pi 2^-24
+  za = r * __cosf(th);
+  zb = r * __sinf(th);
+}
+
+__device__ __forceinline__ void normals4_fast(uint64_t seed, uint32_t tag, uint32_t t,
+                                              uint32_t slot, uint32_t q, float z[4]) {
+  U4 w = philox_draw(seed, tag, t, slot, q);
+  box_muller_fast(w.x, w.y, z[0], z[1]);
+  box_muller_fast(w.z, w.w, z[2], z[3]);
 }
 
 // The four normals of site quad q for (seed, tag, t, slot).
