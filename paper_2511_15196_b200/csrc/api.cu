@@ -64,6 +64,8 @@ struct phi4smc {
   uint32_t iters_enqueued;   // NS iterations enqueued
   int known_done;
   Ctrl* h_ctrl;              // pinned staging
+  Ctrl* h_poll;              // pinned, 2 slots: smc_run / ns_run poll one step behind the GPU
+  cudaEvent_t poll_ev[2];
   StepRecord* h_rec;         // pinned staging (one record)
   double* h_obs;             // pinned staging (85 doubles)
   char err[256];
@@ -196,6 +198,8 @@ PHI4_API size_t ns_workspace_bytes(int L, int n_live, int k_delete, int max_iter
 
 static int host_staging(phi4smc* h) {
   CU(cudaMallocHost((void**)&h->h_ctrl, sizeof(Ctrl)));
+  CU(cudaMallocHost((void**)&h->h_poll, 2 * sizeof(Ctrl)));
+  for (int e = 0; e < 2; ++e) CU(cudaEventCreateWithFlags(&h->poll_ev[e], cudaEventDisableTiming));
   CU(cudaMallocHost((void**)&h->h_rec, sizeof(StepRecord)));
   CU(cudaMallocHost((void**)&h->h_obs, sizeof(double) * (5 + PHI4_HIST_BINS)));
   return PHI4_OK;
@@ -280,6 +284,8 @@ PHI4_API int smc_destroy(phi4smc* h) {
   if (!h) return PHI4_OK;
   cudaStreamSynchronize(h->st);
   if (h->h_ctrl) cudaFreeHost(h->h_ctrl);
+  if (h->h_poll) cudaFreeHost(h->h_poll);
+  for (int e = 0; e < 2; ++e) if (h->poll_ev[e]) cudaEventDestroy(h->poll_ev[e]);
   if (h->h_rec) cudaFreeHost(h->h_rec);
   if (h->h_obs) cudaFreeHost(h->h_obs);
   delete h;
@@ -379,19 +385,37 @@ PHI4_API int smc_step(phi4smc* h, smc_step_info* info) {
   return rc;
 }
 
+// Shared by smc_run / ns_run: keep one step queued behind the one whose control block the host
+// is looking at, so the GPU never idles on the host's poll.  `enqueue` enqueues one step.
+template <typename F>
+static int run_pipelined(phi4smc* h, int max_steps, int* enq_out, F enqueue) {
+  int enq = 0, rc = PHI4_OK;
+  while (!h->known_done && enq < max_steps) {
+    enqueue(h);
+    const int slot = enq & 1;
+    ++enq;
+    CU(cudaMemcpyAsync(&h->h_poll[slot], h->ctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost, h->st));
+    CU(cudaEventRecord(h->poll_ev[slot], h->st));
+    if (enq >= 2) {
+      const int prev = (enq - 2) & 1;            // the step before the one just enqueued
+      CU(cudaEventSynchronize(h->poll_ev[prev]));
+      const Ctrl& c = h->h_poll[prev];
+      if (c.done) h->known_done = 1;
+      if (c.nan_flag || c.chol_status < 0) break;
+    }
+  }
+  *enq_out = enq;
+  rc = sync_ctrl(h);
+  return rc;
+}
+
 PHI4_API int smc_run(phi4smc* h, int max_temps, int* n_temps) {
   if (!h || h->kind != KIND_SMC || max_temps < 0) return PHI4_EINVAL;
   int rc = sync_ctrl(h);
   if (rc != PHI4_OK) return rc;
   const int start = h->h_ctrl->temp_index;
   int enq = 0;
-  while (!h->known_done && enq < max_temps) {
-    // the device decides when beta hits 1; the host polls the control block between batches
-    int batch = 1;
-    for (int b = 0; b < batch && enq < max_temps; ++b, ++enq) enqueue_smc_step(h);
-    rc = sync_ctrl(h);
-    if (rc != PHI4_OK) break;
-  }
+  rc = run_pipelined(h, max_temps, &enq, enqueue_smc_step);
   const int made = h->h_ctrl->temp_index - start;
   // steps enqueued past beta = 1 were no-ops: take them out of the step counter
   if (enq > made) h->step_counter -= (uint64_t)(enq - made) * (uint64_t)h->prm.k_steps;
@@ -553,12 +577,7 @@ PHI4_API int ns_run(phi4smc* h, int max_iters, int* n_iters) {
   if (rc != PHI4_OK) return rc;
   const int start = h->h_ctrl->temp_index;
   int enq = 0;
-  while (!h->known_done && enq < max_iters) {
-    int batch = 8;   // iterations are short and latency-bound: poll the stop flag every 8
-    for (int b = 0; b < batch && enq < max_iters; ++b, ++enq) enqueue_ns_step(h);
-    rc = sync_ctrl(h);
-    if (rc != PHI4_OK) break;
-  }
+  rc = run_pipelined(h, max_iters, &enq, enqueue_ns_step);
   const int made = h->h_ctrl->temp_index - start;
   if (enq > made) h->iters_enqueued -= (uint32_t)(enq - made);
   if (n_iters) *n_iters = made;

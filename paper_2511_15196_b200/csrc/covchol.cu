@@ -145,60 +145,113 @@ __device__ __forceinline__ bool chol_skip(const Ctrl* ctrl, int attempt, int res
 }
 
 // ------------------------------------------------------------------ small V: one CTA ---------
-// Right-looking factorisation in shared memory, thread r owns row r (row stride V+1: conflict
-// free; the column read A[c][j] is a broadcast).  Two barriers per column.
-__global__ void __launch_bounds__(160)
+// Panel-blocked right-looking factorisation in shared memory (row stride V+1: conflict free).
+// Per 8-column panel: every row thread re-factorises the 8x8 diagonal block in registers (170
+// FMAs, no barrier) and solves its own row against it; then all 1024 threads apply the rank-8
+// update to the trailing lower triangle.  Three barriers per panel instead of two per column.
+// Both attempts of reading A4 (plain, then jitter 1e-6 tr/V) run inside this one launch.
+constexpr int CS_NB = 8;
+__global__ void __launch_bounds__(1024)
 chol_small_kernel(const float* __restrict__ Sigma, float* __restrict__ Lc, int V, Ctrl* ctrl,
-                  int attempt, int respect_done) {
+                  int respect_done) {
   extern __shared__ float sm[];   // V x (V+1)
   __shared__ int failed_s;
-  if (chol_skip(ctrl, attempt, respect_done)) return;
-  const int P = V + 1, r = threadIdx.x;
-  const float add = attempt ? 1e-6f * ctrl->trace / (float)V : 0.f;
-  if (r == 0) failed_s = 0;
-  for (int idx = threadIdx.x; idx < V * V; idx += blockDim.x) {
-    int x = idx / V, y = idx - x * V;
-    sm[x * P + y] = Sigma[idx] + (x == y ? add : 0.f);
-  }
-  __syncthreads();
-  float* row = sm + r * P;
-  for (int j = 0; j < V; ++j) {
-    if (r == j) {
-      float d = row[j];
-      if (!(d > 0.f)) { failed_s = 1; d = 1.f; }
-      row[j] = sqrtf(d);
+  __shared__ double red[33];
+  if (respect_done && ctrl->done) return;
+  const int P = V + 1, tid = threadIdx.x;
+  // tr(Sigma) for the jitter scale
+  double tr = 0.0;
+  for (int x = tid; x < V; x += blockDim.x) tr += (double)Sigma[(size_t)x * V + x];
+  tr = block_sum(tr, red);
+  int status = 0;
+  for (int attempt = 0; attempt < 2; ++attempt) {
+    const float add = attempt ? 1e-6f * (float)tr / (float)V : 0.f;
+    if (tid == 0) failed_s = 0;
+    for (int idx = tid; idx < V * V; idx += blockDim.x) {
+      int x = idx / V, y = idx - x * V;
+      sm[x * P + y] = Sigma[idx] + (x == y ? add : 0.f);
     }
     __syncthreads();
-    float l = 0.f;
-    if (r > j && r < V) {
-      l = row[j] / sm[j * P + j];
-      row[j] = l;
-    }
-    __syncthreads();
-    if (r > j && r < V) {
-      // batches of 8 with all loads issued before the stores (row and column alias in smem, so
-      // the compiler would otherwise serialise load -> fma -> store per element)
-      const float* col = sm + j;
-      for (int c0 = j + 1; c0 <= r; c0 += 8) {
-        float cv[8], rv[8];
+    for (int jb = 0; jb < V; jb += CS_NB) {
+      // ---- panel: rows r >= jb, one thread per row
+      const int r = jb + tid;
+      float D[CS_NB][CS_NB], x[CS_NB];
+      if (r < V) {
 #pragma unroll
-        for (int u = 0; u < 8; ++u) {
-          int c = c0 + u;
-          cv[u] = c <= r ? col[c * P] : 0.f;
-          rv[u] = c <= r ? row[c] : 0.f;
+        for (int i = 0; i < CS_NB; ++i)
+#pragma unroll
+          for (int k = 0; k < CS_NB; ++k)
+            if (k <= i) D[i][k] = (jb + i < V) ? sm[(jb + i) * P + jb + k] : (i == k ? 1.f : 0.f);
+#pragma unroll
+        for (int k = 0; k < CS_NB; ++k) x[k] = (jb + k < V) ? sm[r * P + jb + k] : 0.f;
+      }
+      __syncthreads();        // every thread has read the diagonal block before its rows change
+      if (r < V) {
+        bool bad = false;
+#pragma unroll
+        for (int k = 0; k < CS_NB; ++k) {
+          float d = D[k][k];
+          if (!(d > 0.f)) { bad = true; d = 1.f; }
+          const float sd = sqrtf(d), inv = 1.0f / sd;
+          D[k][k] = sd;
+#pragma unroll
+          for (int i = k + 1; i < CS_NB; ++i) D[i][k] *= inv;
+#pragma unroll
+          for (int i = k + 1; i < CS_NB; ++i)
+#pragma unroll
+            for (int c = k + 1; c <= i; ++c) D[i][c] = fmaf(-D[i][k], D[c][k], D[i][c]);
+        }
+        if (bad && tid == 0) failed_s = 1;
+        const int ri = r - jb;               // row inside the diagonal block if < CS_NB
+#pragma unroll
+        for (int k = 0; k < CS_NB; ++k) {
+          float v = x[k];
+#pragma unroll
+          for (int m = 0; m < k; ++m) v = fmaf(-x[m], D[k][m], v);
+          v = v / D[k][k];
+          // rows of the diagonal block take the factor itself (their solve reproduces it up to
+          // rounding; use the shared value so that every thread sees the same l_ck)
+          if (ri < CS_NB) {
+            float dv = 0.f;
+#pragma unroll
+            for (int i = 0; i < CS_NB; ++i) if (i == ri) dv = (k <= i) ? D[i][k] : 0.f;
+            v = dv;
+          }
+          x[k] = v;
         }
 #pragma unroll
-        for (int u = 0; u < 8; ++u)
-          if (c0 + u <= r) row[c0 + u] = fmaf(-l, cv[u], rv[u]);
+        for (int k = 0; k < CS_NB; ++k)
+          if (jb + k < V) sm[r * P + jb + k] = x[k];
       }
+      __syncthreads();
+      // ---- trailing update: A[r][c] -= sum_k l_rk l_ck for jb+8 <= c <= r < V
+      const int j1 = jb + CS_NB;
+      if (j1 < V) {
+        const int tx = tid & 31, ty = tid >> 5;
+        for (int rr = j1 + ty; rr < V; rr += 32) {
+          float lr[CS_NB];
+#pragma unroll
+          for (int k = 0; k < CS_NB; ++k) lr[k] = sm[rr * P + jb + k];
+          for (int cc = j1 + tx; cc <= rr; cc += 32) {
+            float acc = sm[rr * P + cc];
+#pragma unroll
+            for (int k = 0; k < CS_NB; ++k) acc = fmaf(-lr[k], sm[cc * P + jb + k], acc);
+            sm[rr * P + cc] = acc;
+          }
+        }
+      }
+      __syncthreads();
     }
+    const int failed = failed_s;
+    __syncthreads();
+    if (!failed) { status = attempt; break; }
+    status = -1;
   }
-  __syncthreads();
-  for (int idx = threadIdx.x; idx < V * V; idx += blockDim.x) {
+  for (int idx = tid; idx < V * V; idx += blockDim.x) {
     int x = idx / V, y = idx - x * V;
     Lc[idx] = (y <= x) ? sm[x * P + y] : 0.f;
   }
-  if (threadIdx.x == 0 && failed_s) atomicOr(&ctrl->chol_fail, attempt ? 2 : 1);
+  if (tid == 0) { ctrl->chol_status = status; ctrl->chol_fail = 0; ctrl->trace = (float)tr; }
 }
 
 // ------------------------------------------------------------------ large V: blocked ---------
@@ -307,31 +360,31 @@ __global__ void chol_finalize_kernel(Ctrl* ctrl, int respect_done) {
 
 void launch_cholesky(const float* Sigma, float* Lc, int V, Ctrl* ctrl, int respect_done,
                      cudaStream_t st) {
+  if (V <= 160) {
+    size_t smem = (size_t)V * (V + 1) * sizeof(float);
+    static bool attr_done = false;
+    if (!attr_done) {
+      cudaFuncSetAttribute(chol_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                           160 * 161 * (int)sizeof(float));
+      attr_done = true;
+    }
+    ++g_launches; chol_small_kernel<<<1, 1024, smem, st>>>(Sigma, Lc, V, ctrl, respect_done);
+    return;
+  }
   ++g_launches; trace_kernel<<<1, 256, 0, st>>>(Sigma, V, ctrl, respect_done);
   for (int attempt = 0; attempt < 2; ++attempt) {
-    if (V <= 160) {
-      size_t smem = (size_t)V * (V + 1) * sizeof(float);
-      static bool attr_done = false;
-      if (!attr_done) {
-        cudaFuncSetAttribute(chol_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             160 * 161 * (int)sizeof(float));
-        attr_done = true;
-      }
-      ++g_launches; chol_small_kernel<<<1, round_up(V, 32), smem, st>>>(Sigma, Lc, V, ctrl, attempt, respect_done);
-    } else {
-      ++g_launches; chol_copy_kernel<<<(V * V + 255) / 256, 256, 0, st>>>(Sigma, Lc, V, ctrl, attempt,
-                                                            respect_done);
-      for (int j0 = 0; j0 < V; j0 += 64) {
-        int j1 = min(V, j0 + 64);
-        ++g_launches; chol_diag_kernel<<<1, 64, 0, st>>>(Lc, V, j0, ctrl, attempt, respect_done);
-        int rows = V - j1;
-        if (rows > 0) {
-          ++g_launches; chol_trsm_kernel<<<(rows + 63) / 64, 64, 0, st>>>(Lc, V, j0, ctrl, attempt,
-                                                            respect_done);
-          int nt = (rows + 63) / 64;
-          ++g_launches; chol_update_kernel<<<nt * (nt + 1) / 2, 256, 0, st>>>(Lc, V, j0, j1, ctrl, attempt,
-                                                                respect_done);
-        }
+    ++g_launches; chol_copy_kernel<<<(V * V + 255) / 256, 256, 0, st>>>(Sigma, Lc, V, ctrl, attempt,
+                                                          respect_done);
+    for (int j0 = 0; j0 < V; j0 += 64) {
+      int j1 = min(V, j0 + 64);
+      ++g_launches; chol_diag_kernel<<<1, 64, 0, st>>>(Lc, V, j0, ctrl, attempt, respect_done);
+      int rows = V - j1;
+      if (rows > 0) {
+        ++g_launches; chol_trsm_kernel<<<(rows + 63) / 64, 64, 0, st>>>(Lc, V, j0, ctrl, attempt,
+                                                          respect_done);
+        int nt = (rows + 63) / 64;
+        ++g_launches; chol_update_kernel<<<nt * (nt + 1) / 2, 256, 0, st>>>(Lc, V, j0, j1, ctrl, attempt,
+                                                              respect_done);
       }
     }
   }

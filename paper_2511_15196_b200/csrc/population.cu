@@ -16,10 +16,14 @@ namespace phi4 {
 // sums reduced together.
 __device__ inline double ess_frac_eval(const float* __restrict__ S, int N, float smin, double d,
                                        double2* scratch, double* sum_out) {
-  const float df = (float)d;
+  // ex2.approx on the max-shifted argument: relative error ~1e-6 |x| on weights that matter
+  // (|x| < ~20), i.e. ~1e-6 on f -- far below the 1e-4 tolerance of the root (R3).  The weights
+  // themselves (P2) use the accurate expf.
+  const float df = (float)d * 1.4426950408889634f;
   double a = 0.0, b = 0.0;
   for (int i = threadIdx.x; i < N; i += blockDim.x) {
-    float e = expf(-df * (S[i] - smin));
+    float e;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(-df * (S[i] - smin)));
     a += (double)e;
     b += (double)e * (double)e;
   }
@@ -155,7 +159,19 @@ quantise_scan_kernel(const float* __restrict__ w, int N, unsigned long long* __r
   const int ipt = (N + blockDim.x - 1) / blockDim.x;
   const int lo = min(N, (int)threadIdx.x * ipt), hi = min(N, lo + ipt);
   unsigned long long run = 0;
-  for (int i = lo; i < hi; ++i) run += (unsigned long long)((double)w[i] * 1099511627776.0);
+  const bool vec = (ipt & 3) == 0 && hi - lo == ipt;     // whole, 16-byte aligned runs
+  if (vec) {
+    const float4* w4 = reinterpret_cast<const float4*>(w + lo);
+    for (int i = 0; i < ipt / 4; ++i) {
+      float4 v = w4[i];
+      run += (unsigned long long)((double)v.x * 1099511627776.0) +
+             (unsigned long long)((double)v.y * 1099511627776.0) +
+             (unsigned long long)((double)v.z * 1099511627776.0) +
+             (unsigned long long)((double)v.w * 1099511627776.0);
+    }
+  } else {
+    for (int i = lo; i < hi; ++i) run += (unsigned long long)((double)w[i] * 1099511627776.0);
+  }
   // inclusive scan of run over the block
   unsigned long long inc = run;
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
@@ -177,9 +193,24 @@ quantise_scan_kernel(const float* __restrict__ w, int N, unsigned long long* __r
   }
   __syncthreads();
   unsigned long long pre = wsum[wid] + inc - run;
-  for (int i = lo; i < hi; ++i) {
-    pre += (unsigned long long)((double)w[i] * 1099511627776.0);
-    C[i] = pre;
+  if (vec) {
+    const float4* w4 = reinterpret_cast<const float4*>(w + lo);
+    ulonglong2* C2 = reinterpret_cast<ulonglong2*>(C + lo);
+    for (int i = 0; i < ipt / 4; ++i) {
+      float4 v = w4[i];
+      ulonglong2 c0, c1;
+      pre += (unsigned long long)((double)v.x * 1099511627776.0); c0.x = pre;
+      pre += (unsigned long long)((double)v.y * 1099511627776.0); c0.y = pre;
+      pre += (unsigned long long)((double)v.z * 1099511627776.0); c1.x = pre;
+      pre += (unsigned long long)((double)v.w * 1099511627776.0); c1.y = pre;
+      C2[2 * i] = c0;
+      C2[2 * i + 1] = c1;
+    }
+  } else {
+    for (int i = lo; i < hi; ++i) {
+      pre += (unsigned long long)((double)w[i] * 1099511627776.0);
+      C[i] = pre;
+    }
   }
   if (threadIdx.x == blockDim.x - 1) {
     ctrl->q_total = pre;
