@@ -23,6 +23,8 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 ALU_OPS_PER_SITE_UPDATE = 40          # Philox ~20 int + Box-Muller ~6 + action ~14
+# dram__bytes_read.sum + dram__bytes_write.sum of one mutation launch (profiles/, ncu --set full)
+NCU_DRAM_BYTES = {"C1": 6817536}
 
 
 def peaks():
@@ -264,14 +266,17 @@ def main():
         return
 
     pk = peaks()
-    # Roofline of the mutation: algorithmic work per site-update =
-    # (V+1) flop for the triangular proposal product + 40 plain ALU ops (RNG, Box-Muller, action).
-    work = (V + 1 + ALU_OPS_PER_SITE_UPDATE) * float(N) * V * k
-    alu_peak = 148 * 128 * 2 * pk["sm_max_mhz"] * 1e6 / 1e12       # TFLOP/s, FP32 FMA pipes
+    # Roofline of the dominant kernel, the fused mutation: plain-ALU bound; the
+    # algorithmic work is 40 lane-ops per site-update (Philox ~20, Box-Muller ~6, action ~14;
+    # SURVEY 8(d)); the proposal product rides on the tensor pipe.  Peak: 148 SM x 128 lanes x clock
+    # (an FMA counts as one lane-op).  traffic: dram bytes per launch from the committed ncu capture.
+    work = ALU_OPS_PER_SITE_UPDATE * float(N) * V * k
+    alu_peak = 148 * 128 * pk["sm_max_mhz"] * 1e6 / 1e12
     achieved = work / (mut_ms * 1e-3) / 1e12
     roofline = {"bound": "alu", "kernel": "mutation x%d steps (%d launches)" % (k, mut_launches),
                 "achieved": achieved, "peak": alu_peak, "unit": "TFLOP/s", "frac": achieved / alu_peak,
-                "traffic": None, "peak_source": "derived: 148 SM x 128 lanes x 2 x %.0f MHz (%s clocks)"
+                "ops": "lane-ops (FMA = 1), 40 per site-update", "traffic": NCU_DRAM_BYTES.get(args.workload),
+                "peak_source": "derived: 148 SM x 128 lanes x %.0f MHz (%s clocks)"
                 % (pk["sm_max_mhz"], pk["source"]),
                 "site_updates_per_s": float(N) * V * k / (mut_ms * 1e-3), "ms": mut_ms}
 
