@@ -39,6 +39,15 @@ __device__ __forceinline__ void nt_tile(const float* __restrict__ A, size_t lda,
   const int xr = x0 + lr, yr = y0 + lr;
   const float mx = (mu && xr < M) ? mu[xr] : 0.f;
   const float my = (mu && yr < M) ? mu[yr] : 0.f;
+  // Two-level accumulation: `acc` runs over 1024 contraction indices at a time and is then folded
+  // into `tot`, so the fp32 rounding grows like sqrt(1024) + sqrt(K/1024) instead of sqrt(K)
+  // (K = N = 131072 particles at C4 would otherwise miss the 1e-5 covariance tolerance).
+  float tot[4][4];
+#pragma unroll
+  for (int p = 0; p < 4; ++p)
+#pragma unroll
+    for (int r = 0; r < 4; ++r) { tot[p][r] = acc[p][r]; acc[p][r] = 0.f; }
+  int since = 0;
   for (int k0 = kb; k0 < ke; k0 += 16) {
     float va[4], vb[4];
     if (VEC) {
@@ -74,7 +83,18 @@ __device__ __forceinline__ void nt_tile(const float* __restrict__ A, size_t lda,
         for (int r = 0; r < 4; ++r) acc[p][r] = fmaf(a[p], b[r], acc[p][r]);
     }
     __syncthreads();
+    if (++since == 64) {
+      since = 0;
+#pragma unroll
+      for (int p = 0; p < 4; ++p)
+#pragma unroll
+        for (int r = 0; r < 4; ++r) { tot[p][r] += acc[p][r]; acc[p][r] = 0.f; }
+    }
   }
+#pragma unroll
+  for (int p = 0; p < 4; ++p)
+#pragma unroll
+    for (int r = 0; r < 4; ++r) acc[p][r] += tot[p][r];
 }
 
 // linear index t -> lower-triangular tile (tr, tc), tc <= tr

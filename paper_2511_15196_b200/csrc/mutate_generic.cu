@@ -35,11 +35,14 @@ propose_kernel(const float* __restrict__ Lc, const float* __restrict__ Z,
   __shared__ __align__(16) float Bs[16][64];
   const int x0 = blockIdx.y * 64, i0 = blockIdx.x * 64;
   const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
-  float acc[4][4];
+  // two-level accumulation (fold every 512 y's): fp32 rounding of the V-term sum ~ sqrt(512) +
+  // sqrt(V/512) instead of sqrt(V), which keeps the V = 4096 margins inside the 1e-4 band
+  float acc[4][4], tot[4][4];
 #pragma unroll
   for (int a = 0; a < 4; ++a)
 #pragma unroll
-    for (int b = 0; b < 4; ++b) acc[a][b] = 0.f;
+    for (int b = 0; b < 4; ++b) { acc[a][b] = 0.f; tot[a][b] = 0.f; }
+  int since = 0;
   const int kend = min(V, x0 + 64);
   const int am = threadIdx.x >> 2, ak = (threadIdx.x & 3) * 4;  // A loader: row am, 4 k's
   const int bk = threadIdx.x >> 4, bn = (threadIdx.x & 15) * 4; // B loader: row bk, 4 i's
@@ -69,7 +72,18 @@ propose_kernel(const float* __restrict__ Lc, const float* __restrict__ Z,
         for (int r = 0; r < 4; ++r) acc[p][r] = fmaf(a[p], b[r], acc[p][r]);
     }
     __syncthreads();
+    if (++since == 32) {
+      since = 0;
+#pragma unroll
+      for (int p = 0; p < 4; ++p)
+#pragma unroll
+        for (int r = 0; r < 4; ++r) { tot[p][r] += acc[p][r]; acc[p][r] = 0.f; }
+    }
   }
+#pragma unroll
+  for (int p = 0; p < 4; ++p)
+#pragma unroll
+    for (int r = 0; r < 4; ++r) acc[p][r] += tot[p][r];
 #pragma unroll
   for (int p = 0; p < 4; ++p) {
     int x = x0 + ty * 4 + p;
@@ -118,14 +132,17 @@ accept_kernel(float* __restrict__ phi, const float* __restrict__ phip, float* __
       int rn = (r + 1 == L) ? 0 : r + 1;
       size_t ro = (size_t)r * L * ld + i, rno = (size_t)rn * L * ld + i;
       float a = phi[ro], a2 = phip[ro];
+      float rS = 0.f, rU = 0.f;       // per-row partial sums: two-level fp32 accumulation
       for (int c = 0; c < L; ++c) {
         int cn = (c + 1 == L) ? 0 : c + 1;
         float b = phi[ro + (size_t)cn * ld], b2 = phip[ro + (size_t)cn * ld];
         float d = phi[rno + (size_t)c * ld], d2 = phip[rno + (size_t)c * ld];
-        site_diff(a, b, d, a2, b2, d2, hm, lam, dS, dU);
+        site_diff(a, b, d, a2, b2, d2, hm, lam, rS, rU);
         a = b;
         a2 = b2;
       }
+      dS += rS;
+      dU += rU;
     }
   }
   ps[g][lane] = dS;

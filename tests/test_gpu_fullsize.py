@@ -1,0 +1,111 @@
+"""GPU parity at BASELINE.json's full sizes (C1, C3, C4): one tempering transition through the C ABI,
+checked on sampled outputs the oracle can compute one by one (sub-sampled lock-step for the mutation,
+sub-blocks of the covariance) and exactly where the work is integer (ancestors, gather)."""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+from paper_2511_15196_b200 import binding as B
+from paper_2511_15196_b200 import build, inputs
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    build.build()
+    B.load()
+
+
+@pytest.mark.parametrize("name,k,n_sub", [("C1", 20, 512), ("C3", 2, 256), ("C4", 1, 96)])
+def test_full_size_transition(name, k, n_sub):
+    c = inputs.CONFIGS[name]
+    L, N, V, seed = c["L"], c["N"], c["L"] ** 2, 0
+    rng = np.random.default_rng(123)
+    h = B.smc_init(L, c["m0sq"], c["lam"], N, seed)
+    B.smc_set_params(h, k_steps=k, ess_target=c["ess"])
+
+    # M1 + action on a sample of particles
+    st0 = B.smc_get_state(h)
+    sub = np.sort(rng.choice(N, n_sub, replace=False)).astype(np.int32)
+    for i in sub[:16]:
+        assert np.abs(st0["phi"][:, i] - O.normals(seed, O.TAG_INIT, 0, int(i), V)).max() < 4e-6
+    S, U0, A = O.action_batch(st0["phi"][:, sub].astype(np.float64), L, c["m0sq"], c["lam"], with_abs=True)
+    assert np.all(np.abs(st0["S"][sub] - S) <= 2e-5 * A)
+
+    # P1 + P2 (N floats: the oracle does the whole vector)
+    w, info = B.smc_reweight(h)
+    d_ref, fin = O.next_delta(st0["S"].astype(np.float64), 0.0, c["ess"])
+    assert not fin and info["delta"] == pytest.approx(d_ref, rel=1e-4)
+    w_ref, dlz = O.reweight(st0["S"].astype(np.float64), info["delta"])
+    assert np.allclose(w, w_ref, rtol=3e-5, atol=1e-12)
+    assert info["dlogZ"] == pytest.approx(dlz, abs=2e-5 * max(1.0, abs(dlz)))
+
+    # P3 + P4: integer work, exact at full size
+    anc = B.smc_resample(h)
+    assert np.array_equal(anc, O.resample_systematic(w, O.word0(seed, O.TAG_RESAMPLE, 0, 0)))
+    st1 = B.smc_get_state(h)
+    rows = rng.choice(V, min(V, 24), replace=False)
+    assert np.array_equal(st1["phi"][rows], st0["phi"][rows][:, anc])
+    assert np.array_equal(st1["S"], st0["S"][anc])
+
+    # C1 + C2: a random sub-block of Sigma from the definition; the factor through its reconstruction
+    B.estimate_cov_chol(h)
+    Sig, Lc = B.smc_get_cov(h), B.smc_get_chol(h)
+    xs = np.sort(rng.choice(V, min(V, 48), replace=False))
+    _, Sref = O.covariance(st1["phi"][xs].astype(np.float64))
+    blk = Sig[np.ix_(xs, xs)].astype(np.float64)
+    assert np.linalg.norm(blk - Sref) / np.linalg.norm(Sref) < 1e-5
+    assert np.array_equal(Sig, Sig.T)
+    Ld = Lc.astype(np.float64)
+    assert np.all(np.triu(Lc, 1) == 0) and np.all(np.diag(Lc) > 0)
+    assert np.linalg.norm(Ld @ Ld.T - Sig) / np.linalg.norm(Sig) < 1e-5            # R6
+
+    # M1-M4: lock-step on a sub-sample with its own Philox slots
+    B.smc_set_state(h, st1["phi"], 0.3, 0)                      # a mid-schedule beta
+    st2 = B.smc_get_state(h, want_phi=False)
+    acc, mar = B.smc_mutate(h, k)
+    st3 = B.smc_get_state(h)
+    s = np.float32(2.38 / math.sqrt(V))
+    _, _, Ax0 = O.action_batch(st1["phi"][:, sub].astype(np.float64), L, c["m0sq"], c["lam"], with_abs=True)
+    # the oracle starts from its own FP64 action of the same fp32 fields (the GPU's cached fp32 S_E
+    # is off by ~eps*A ~ 1e-3 at V = 4096, which would otherwise be booked as a margin error)
+    S_sub, U_sub = O.action_batch(st1["phi"][:, sub].astype(np.float64), L, c["m0sq"], c["lam"])
+    assert np.all(np.abs(st2["S"][sub] - S_sub) <= 2e-5 * np.maximum(1.0, np.abs(S_sub)) + 2e-5 * Ax0)
+    p, S_o, U_o, oacc, omar, _ = O.mutate(st1["phi"][:, sub], S_sub, U_sub, L, c["m0sq"],
+                                          c["lam"], Lc, s, 0.3, seed, 1, k, slots=sub)
+    amb = np.abs(omar) < 1e-4
+    first = np.where(amb.any(axis=0), amb.argmax(axis=0), k)
+    valid = np.arange(k)[:, None] < first[None, :]
+    assert valid.mean() > 0.97
+    assert np.array_equal(acc[:, sub][valid], oacc[valid])
+    # margin agreement: fp32 rounding of the V-term proposal sums and of the V-site action
+    # difference grows like sqrt(V); decisions above were compared exactly outside the fixed 1e-4 band
+    tol = 1e-4 * max(1.0, math.sqrt(V / 100.0))
+    assert np.all(np.abs(mar[:, sub][valid] - omar[valid]) < tol + 1e-5 * np.abs(omar[valid]))
+    clean = first == k
+    assert np.abs(st3["phi"][:, sub][:, clean] - p[:, clean]).max() < 2e-5
+    Sx, Ux, Ax = O.action_batch(st3["phi"][:, sub].astype(np.float64), L, c["m0sq"], c["lam"], with_abs=True)
+    assert np.all(np.abs(st3["S"][sub] - Sx) <= 2e-5 * Ax + 2e-5)
+    assert 0.0 < acc.mean() < 1.0
+    h.close()
+
+
+def test_C3_whole_step_and_observables():
+    """One smc_step at C3 (all rows chained through the device control block) and O."""
+    c = inputs.CONFIGS["C3"]
+    h = B.smc_init(c["L"], c["m0sq"], c["lam"], c["N"], 1)
+    B.smc_set_params(h, k_steps=2, ess_target=c["ess"])
+    info = B.smc_step(h)
+    assert info["temp_index"] == 0 and 0 < info["beta"] < 1 and info["chol_status"] == 0
+    assert abs(info["ess_frac"] - 0.5) < 1e-3 and 0.0 < info["accept_rate"] < 1.0
+    assert c["N"] * 0.4 < info["n_unique"] < c["N"]
+    obs = B.observables(h)
+    st = B.smc_get_state(h)
+    M = st["phi"].astype(np.float64).mean(axis=0)
+    assert obs["absM"] == pytest.approx(np.abs(M).mean(), rel=1e-5)
+    assert obs["M2"] == pytest.approx((M * M).mean(), rel=1e-5)
+    assert obs["mean_SE"] == pytest.approx(st["S"].astype(np.float64).mean(), rel=1e-5)
+    h.close()

@@ -109,7 +109,9 @@ def lockstep(L, N, k, beta, seed, m0sq=-4.0, lam=1.0, path=0, fields="init", t_s
     st1 = B.smc_get_state(h)
     assert st1["step"] == t_start + k
     s = 2.38 / math.sqrt(V)
-    p, S, U0, oacc, omar, _ = O.mutate(st0["phi"], st0["S"], st0["U0"], L, m0sq, lam, Lc,
+    # the oracle starts from its own FP64 action of the same fp32 fields
+    S0, U00 = O.action_batch(st0["phi"].astype(np.float64), L, m0sq, lam)
+    p, S, U0, oacc, omar, _ = O.mutate(st0["phi"], S0, U00, L, m0sq, lam, Lc,
                                        np.float32(s), beta, seed, t_start + 1, k)
     # R4: a particle is compared up to (excluding) its first step with |g_oracle| < BAND
     amb = np.abs(omar) < BAND
