@@ -98,7 +98,7 @@ uint64_t phi4_kernel_launches(void);
 
 /* ---------------------------------------------------------------- SMC-RW (PAPER.md:53(i)) ----
  * smc_workspace_bytes: bytes of device memory smc_init needs for an L x L lattice and N particles
- * (0 if L < 1 or N < 2).  Sized for 180 GB parts: C4 (L=64, N=131072) needs about 9 GB.          */
+ * (0 if L < 1 or N < 2).  Sized for 180 GB parts: C4 (L=64, N=131072) needs about 11 GB.          */
 size_t smc_workspace_bytes(int L, int N);
 
 /* Creates an SMC sampler: particles phi_i ~ N(0,I) from Philox stream INIT, S_E and U0 evaluated,

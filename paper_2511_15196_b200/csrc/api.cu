@@ -90,7 +90,7 @@ static int carve_smc(phi4smc* h, char* base, size_t* total) {
     h->U0[b] = c.take<float>(ld);
   }
   h->phip = c.take<float>(field);
-  h->Z = c.take<float>(field);
+  h->Z = c.take<float>(propose_tc_supported(V) ? propose_tc_zsplit_floats(V, ld) : field);
   h->w = c.take<float>(ld);
   h->M = c.take<float>(ld);
   h->C = c.take<unsigned long long>(ld);
@@ -99,7 +99,7 @@ static int carve_smc(phi4smc* h, char* base, size_t* total) {
   h->Sigma = c.take<float>((size_t)V * V);
   h->Lc = c.take<float>((size_t)V * V);
   h->partial = c.take<float>(cov_partial_floats(V, N));
-  h->Lsplit = c.take<float>(mutate_tc_supported(V) ? mutate_tc_lsplit_floats(V) : 4);
+  h->Lsplit = c.take<float>((mutate_tc_supported(V) || propose_tc_supported(V)) ? mutate_tc_lsplit_floats(V) : 4);
   h->acc_flags = c.take<uint8_t>((size_t)PHI4_MAX_HOOK_STEPS * N);
   h->margins = c.take<float>((size_t)PHI4_MAX_HOOK_STEPS * N);
   h->ctrl = c.take<Ctrl>(1);
@@ -120,12 +120,12 @@ static int carve_ns(phi4smc* h, char* base, size_t* total) {
   h->wS = c.take<float>(ldw);
   h->wU = c.take<float>(ldw);
   h->phip = c.take<float>((size_t)V * ldw);
-  h->Z = c.take<float>((size_t)V * ldw);
+  h->Z = c.take<float>(propose_tc_supported(V) ? propose_tc_zsplit_floats(V, ldw) : (size_t)V * ldw);
   h->mu = c.take<float>(V);
   h->Sigma = c.take<float>((size_t)V * V);
   h->Lc = c.take<float>((size_t)V * V);
   h->partial = c.take<float>(cov_partial_floats(V, N));
-  h->Lsplit = c.take<float>(mutate_tc_supported(V) ? mutate_tc_lsplit_floats(V) : 4);
+  h->Lsplit = c.take<float>((mutate_tc_supported(V) || propose_tc_supported(V)) ? mutate_tc_lsplit_floats(V) : 4);
   h->dead = c.take<int32_t>(kd);
   h->surv = c.take<int32_t>(N);
   h->start = c.take<int32_t>(kd);
@@ -297,7 +297,8 @@ PHI4_API int smc_set_params(phi4smc* h, const smc_params* p) {
   if (p->k_steps < 1 || !(p->ess_target > 0.f && p->ess_target < 1.f) || p->step_scale < 0.f ||
       p->mutation_path < 0 || p->mutation_path > 2)
     return PHI4_EINVAL;
-  if (p->mutation_path == 2 && !mutate_tc_supported(h->md.V)) return PHI4_EINVAL;
+  if (p->mutation_path == 2 && !mutate_tc_supported(h->md.V) && !propose_tc_supported(h->md.V))
+    return PHI4_EINVAL;
   h->prm = *p;
   h->s = p->step_scale > 0.f ? p->step_scale : 2.38f / sqrtf((float)h->md.V);
   return PHI4_OK;
@@ -319,9 +320,14 @@ static bool use_tc_path(const phi4smc* h) {
   return h->prm.mutation_path != 1 && mutate_tc_supported(h->md.V);
 }
 
+// large V: tcgen05 proposal GEMM + the generic accept step
+static bool use_tc_propose(const phi4smc* h) {
+  return h->prm.mutation_path != 1 && propose_tc_supported(h->md.V);
+}
+
 static void enqueue_mutation(phi4smc* h, const MutateArgs& a) {
   if (use_tc_path(h)) launch_mutate_tc(a, h->Lsplit, h->st);
-  else launch_mutate_generic(a, h->st);
+  else launch_mutate_generic(a, use_tc_propose(h) ? h->Lsplit : nullptr, h->st);
 }
 
 static CovCholArgs cov_args(phi4smc* h, int respect_done) {

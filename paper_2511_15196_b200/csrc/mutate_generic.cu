@@ -183,16 +183,24 @@ accept_kernel(float* __restrict__ phi, const float* __restrict__ phip, float* __
   }
 }
 
-void launch_mutate_generic(const MutateArgs& a, cudaStream_t st) {
+// Lsplit != nullptr selects the tcgen05 proposal (propose_tc.cu) for M1 + M2; a.Z must then hold
+// 2 V ld floats.  The accept / commit step is the same either way.
+void launch_mutate_generic(const MutateArgs& a, float* Lsplit, cudaStream_t st) {
   const int V = a.md.V;
   dim3 gz((a.ld + 127) / 128, (V + 3) / 4);
   dim3 gp(a.ld / 64, (V + 63) / 64);
+  if (Lsplit) launch_lsplit(a.Lc, V, a.s, Lsplit, a.ctrl, a.respect_done, st);
   for (int j = 0; j < a.k; ++j) {
     uint32_t t = a.t0 + (uint32_t)j;
-    ++g_launches; normals_kernel<<<gz, 128, 0, st>>>(a.Z, a.N, a.ld, V, a.seed, a.tag_prop, t, a.ctrl,
-                                       a.respect_done);
-    ++g_launches; propose_kernel<<<gp, 256, 0, st>>>(a.Lc, a.Z, a.phi, a.phip, V, a.ld, a.s, a.ctrl,
-                                       a.respect_done);
+    if (Lsplit) {
+      launch_normals_split(a.Z, a.N, a.ld, V, a.seed, a.tag_prop, t, a.ctrl, a.respect_done, st);
+      launch_propose_tc(a.phi, a.phip, a.Z, Lsplit, a.ld, V, a.ctrl, a.respect_done, st);
+    } else {
+      ++g_launches; normals_kernel<<<gz, 128, 0, st>>>(a.Z, a.N, a.ld, V, a.seed, a.tag_prop, t, a.ctrl,
+                                         a.respect_done);
+      ++g_launches; propose_kernel<<<gp, 256, 0, st>>>(a.Lc, a.Z, a.phi, a.phip, V, a.ld, a.s, a.ctrl,
+                                         a.respect_done);
+    }
     ++g_launches; accept_kernel<<<a.ld / 32, 256, 0, st>>>(
         a.phi, a.phip, a.S, a.U0, a.N, a.ld, a.md, a.mode, a.seed, a.tag_acc, t, a.ctrl,
         a.acc_out ? a.acc_out + (size_t)j * a.N : nullptr,

@@ -20,6 +20,7 @@
 // BASELINE.json north_star (3xTF32 tcgen05 proposal product, tile kept on-chip across k steps).
 #include "kernels.cuh"
 #include "philox.cuh"
+#include "tcgen05.cuh"
 
 namespace phi4 {
 
@@ -38,21 +39,6 @@ constexpr int CHUNK_BYTES = TILE * 16;           // one 16-byte K-chunk of all 1
 constexpr int SLAB_BYTES = 2 * 4 * CHUNK_BYTES;  // {hi,lo} x 4 K-chunks
 constexpr int MAX_SMEM = 232448;
 
-__host__ __device__ inline int vn_of(int V) { return round_up(V, 16); }
-__host__ __device__ inline int kp_of(int V) { return round_up(V, 8); }
-// Lc is lower-triangular: K-step ks (columns y in [8 ks, 8 ks + 8)) only has non-zero rows
-// x >= 8 ks, so only rows [xs(ks), Vn) are stored and multiplied, xs = 8 ks rounded down to 16.
-__host__ __device__ inline int xs_of(int ks) { return (8 * ks) & ~15; }
-// rows stored before K-step ks (each K-step block holds 2 chunks x (Vn - xs) rows x 16 B)
-__host__ __device__ inline int rows_before(int ks, int Vn) {
-  int r = 0;
-  for (int j = 0; j < ks; ++j) r += Vn - xs_of(j);
-  return r;
-}
-__host__ __device__ inline size_t l_floats(int V) {     // floats per hi / lo part
-  return (size_t)rows_before(kp_of(V) / 8, vn_of(V)) * 8;
-}
-
 struct Smem {
   size_t tile0, tile1, lhi, llo, zring, part, dtab, bars, total;
 };
@@ -70,129 +56,6 @@ __host__ __device__ inline Smem smem_layout(int V) {
   s.bars = o; o += 128;
   s.total = o;
   return s;
-}
-
-// ------------------------------------------------------------------ PTX wrappers -------------
-__device__ __forceinline__ uint32_t smem_u32(const void* p) {
-  return (uint32_t)__cvta_generic_to_shared(p);
-}
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
-}
-__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
-  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_n(uint32_t bar, uint32_t n) {
-  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(n) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes)
-               : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-  asm volatile(
-      "{\n\t"
-      ".reg .pred p;\n\t"
-      "WAIT_%=:\n\t"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
-      "@p bra DONE_%=;\n\t"
-      "bra WAIT_%=;\n\t"
-      "DONE_%=:\n\t"
-      "}" ::"r"(bar), "r"(parity)
-      : "memory");
-}
-// Same, for waiters that are not on the critical path: the thread is suspended by the hardware
-// until the phase completes (or the time hint expires), so that a waiting warp takes no issue
-// slots from the warps doing the arithmetic.
-__device__ __forceinline__ void mbar_wait_relaxed(uint32_t bar, uint32_t parity) {
-  asm volatile(
-      "{\n\t"
-      ".reg .pred p;\n\t"
-      "WAITR_%=:\n\t"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n\t"
-      "@p bra DONER_%=;\n\t"
-      "bra WAITR_%=;\n\t"
-      "DONER_%=:\n\t"
-      "}" ::"r"(bar), "r"(parity), "r"(1000000u)
-      : "memory");
-}
-__device__ __forceinline__ void fence_proxy_async() {
-  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-}
-__device__ __forceinline__ void fence_mbar_init() {
-  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-}
-__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes,
-                                         uint32_t bar) {
-  asm volatile(
-      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::
-          "r"(dst), "l"(src), "r"(bytes), "r"(bar)
-      : "memory");
-}
-__device__ __forceinline__ void tc_fence_before() {
-  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-}
-__device__ __forceinline__ void tc_fence_after() {
-  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-}
-__device__ __forceinline__ void tmem_alloc(uint32_t slot, uint32_t ncols) {
-  asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(slot),
-               "r"(ncols)
-               : "memory");
-  asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
-}
-__device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t ncols) {
-  asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols)
-               : "memory");
-}
-__device__ __forceinline__ void tc_commit(uint32_t bar) {
-  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::
-                   "r"(bar)
-               : "memory");
-}
-// D[tmem] (+)= A[smem] * B[smem]^T, kind::tf32, one CTA.
-__device__ __forceinline__ void tc_mma_tf32(uint32_t d, uint64_t a, uint64_t b, uint32_t idesc,
-                                            uint32_t accumulate) {
-  asm volatile(
-      "{\n\t"
-      ".reg .pred p;\n\t"
-      "setp.ne.b32 p, %4, 0;\n\t"
-      "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t"
-      "}" ::"r"(d), "l"(a), "l"(b), "r"(idesc), "r"(accumulate)
-      : "memory");
-}
-__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&r)[16]) {
-  asm volatile(
-      "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
-      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
-      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]),
-        "=r"(r[7]), "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]),
-        "=r"(r[14]), "=r"(r[15])
-      : "r"(taddr)
-      : "memory");
-}
-__device__ __forceinline__ void tmem_ld_wait() {
-  asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-}
-
-// Shared-memory matrix descriptor, K-major, no swizzle ("interleave"): core matrix = 8 rows x
-// 16 B stored contiguously; LBO = byte distance between the two 16-byte K-chunks of one MMA,
-// SBO = byte distance between 8-row groups.  (Field layout: start>>4 [0,14), LBO>>4 [16,30),
-// SBO>>4 [32,46), version=1 [46,48), layout type 0 [61,64).)
-__device__ __forceinline__ uint64_t smem_desc(uint32_t addr, uint32_t lbo, uint32_t sbo) {
-  return (uint64_t)((addr >> 4) & 0x3FFFu) | ((uint64_t)((lbo >> 4) & 0x3FFFu) << 16) |
-         ((uint64_t)((sbo >> 4) & 0x3FFFu) << 32) | (1ull << 46);
-}
-// Instruction descriptor: D = F32 [4,6)=1, A = B = TF32 [7,10)=[10,13)=2, both K-major,
-// N>>3 at [17,23), M>>4 at [24,29).
-__device__ __forceinline__ uint32_t instr_desc(int M, int N) {
-  return (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(N >> 3) << 17) |
-         ((uint32_t)(M >> 4) << 24);
-}
-__device__ __forceinline__ float tf32_rna(float x) {
-  uint32_t u;
-  asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(u) : "f"(x));
-  return __uint_as_float(u);
 }
 
 }  // namespace tc
@@ -650,10 +513,17 @@ extern "C" __attribute__((visibility("default"))) int phi4_debug_tc_trace(long l
 }
 #endif
 
+void launch_lsplit(const float* Lc, int V, float s, float* Lsplit, const Ctrl* ctrl, int respect_done,
+                   cudaStream_t st) {
+  const int Vn = tc::vn_of(V), Kp = tc::kp_of(V);
+  ++g_launches;
+  lsplit_kernel<<<(unsigned)(((size_t)Kp * Vn + 255) / 256), 256, 0, st>>>(Lc, V, Vn, Kp, s, Lsplit, ctrl,
+                                                                         respect_done);
+}
+
 void launch_mutate_tc(const MutateArgs& a, float* Lsplit, cudaStream_t st) {
   const int V = a.md.V, Vn = tc::vn_of(V), Kp = tc::kp_of(V);
-  ++g_launches; lsplit_kernel<<<(Kp * Vn + 255) / 256, 256, 0, st>>>(a.Lc, V, Vn, Kp, a.s, Lsplit, a.ctrl,
-                                                      a.respect_done);
+  launch_lsplit(a.Lc, V, a.s, Lsplit, a.ctrl, a.respect_done, st);
   TcParams p;
   p.phi = a.phi; p.S = a.S; p.U0 = a.U0; p.Lsplit = Lsplit; p.ctrl = a.ctrl;
   p.acc_out = a.acc_out; p.margin_out = a.margin_out;

@@ -1,0 +1,246 @@
+// propose_tc.cu -- M1 + M2 for large lattices (V >= 128, V % 16 == 0): the proposal product
+//   phi'[x][i] = phi[x][i] + sum_{y<=x} (s Lc)[x][y] z[y][i]
+// as a persistent tcgen05 GEMM in 3xTF32 split precision (BASELINE.json north_star: "the N x V x V
+// proposal product L*z ... as tcgen05/TMEM tiles in 3xTF32 split precision"; PAPER.md:53(i), :172).
+//
+//   normals_split_kernel  Philox normals of one step, split hi/lo, written straight in the UMMA
+//                         K-major interleave layout, tile-major: Zs[part][particle tile][K-chunk]
+//                         [128 rows][4] -- a ring stage is one contiguous 8 KB run per part.
+//   propose_tc_kernel     one CTA per SM loops over (particle tile 128) x (site tile 256) output
+//                         tiles.  Warp 4 streams A (normals) and B (s Lc, packed lower-triangular
+//                         blocks of tcgen05.cuh) into a 4-stage shared-memory ring with
+//                         cp.async.bulk + mbarrier; warp 5 issues tcgen05.mma kind::tf32 (three
+//                         products per K-step into one FP32 TMEM accumulator, K-steps above the
+//                         diagonal skipped, N shrunk inside the diagonal block); warps 0-3 read the
+//                         accumulator with tcgen05.ld (lane = particle) and write phi' = phi + d,
+//                         coalesced along particles.  The accumulator is double-buffered (2 x 256
+//                         TMEM columns), so the epilogue of a tile overlaps the MMAs of the next.
+// The accept step stays in accept_kernel (mutate_generic.cu): it needs whole lattice rows of phi'.
+#include "kernels.cuh"
+#include "philox.cuh"
+#include "tcgen05.cuh"
+
+namespace phi4 {
+
+namespace lg {
+constexpr int TILE = 128;                    // particles per output tile = TMEM lanes
+constexpr int TN = 256;                      // sites per output tile = TMEM columns per buffer
+constexpr int STAGES = 4;
+constexpr int CHUNK_A = TILE * 16;           // one 16-byte K-chunk of 128 rows
+constexpr int CHUNK_B = TN * 16;
+constexpr int A_PART = 4 * CHUNK_A;          // K = 16 per stage: 4 chunks per hi / lo part
+constexpr int B_PART = 4 * CHUNK_B;
+constexpr int STAGE_BYTES = 2 * A_PART + 2 * B_PART;   // 48 KB
+constexpr int THREADS = 192;                 // 4 epilogue warps, producer warp, MMA warp
+constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 256;
+}  // namespace lg
+
+// z of step t for every particle, hi/lo split, tile-major interleave layout:
+// float4 index ((part * ntm + m) * nkc + q) * 128 + pr, part 0 = hi, 1 = lo.
+__global__ void __launch_bounds__(128)
+normals_split_kernel(float4* __restrict__ Zs, int N, int ntm, int V, uint64_t seed, uint32_t tag,
+                     uint32_t t, const Ctrl* ctrl, int respect_done) {
+  if (respect_done && ctrl->done) return;
+  const int m = blockIdx.x, q = blockIdx.y, pr = threadIdx.x;
+  const int i = m * lg::TILE + pr, nkc = V >> 2;
+  float z[4] = {0.f, 0.f, 0.f, 0.f};
+  if (i < N) normals4(seed, tag, t, (uint32_t)i, (uint32_t)q, z);
+  float4 hi, lo;
+  hi.x = tc::tf32_rna(z[0]); lo.x = z[0] - hi.x;
+  hi.y = tc::tf32_rna(z[1]); lo.y = z[1] - hi.y;
+  hi.z = tc::tf32_rna(z[2]); lo.z = z[2] - hi.z;
+  hi.w = tc::tf32_rna(z[3]); lo.w = z[3] - hi.w;
+  const size_t o = ((size_t)m * nkc + q) * lg::TILE + pr;
+  Zs[o] = hi;
+  Zs[(size_t)ntm * nkc * lg::TILE + o] = lo;
+}
+
+struct ProposeTcParams {
+  const float* phi; float* phip;     // [V][ld]
+  const float* Zs;                   // normals_split_kernel output
+  const float* Lsplit;               // packed s*Lc hi | lo (tcgen05.cuh layout)
+  const Ctrl* ctrl;
+  int ld, V, ntm, ntn;
+  int respect_done;
+};
+
+__global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const ProposeTcParams p) {
+  using namespace tc;
+  using namespace lg;
+  extern __shared__ __align__(1024) uint8_t smem[];
+  if (p.respect_done && p.ctrl->done) return;
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + STAGES * STAGE_BYTES);
+  const uint32_t bar0 = smem_u32(bars);
+  auto full = [&](int s) { return bar0 + 8u * s; };
+  auto empty = [&](int s) { return bar0 + 8u * (STAGES + s); };
+  auto dfull = [&](int b) { return bar0 + 8u * (2 * STAGES + b); };
+  auto dempty = [&](int b) { return bar0 + 8u * (2 * STAGES + 2 + b); };
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * STAGES + 4);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int V = p.V, nkc = V >> 2, ntiles = p.ntm * p.ntn;
+
+  if (warp == 4 && lane == 0) {
+    for (int s = 0; s < STAGES; ++s) { mbar_init(full(s), 1); mbar_init(empty(s), 1); }
+    for (int b = 0; b < 2; ++b) { mbar_init(dfull(b), 1); mbar_init(dempty(b), 4); }
+    fence_mbar_init();
+  }
+  if (warp == 0) tmem_alloc(smem_u32(tmem_slot), 2 * TN);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t taddr = *tmem_slot;
+  const uint32_t ring = smem_u32(smem);
+
+  if (warp == 4) {
+    // ================================ producer: bulk copies into the ring =====================
+    if (lane == 0) {
+      const size_t lpart = l_floats(V);
+      int s = 0;
+      uint32_t ph = 0;
+      for (int tl = blockIdx.x; tl < ntiles; tl += gridDim.x) {
+        const int m = tl / p.ntn, n0 = (tl % p.ntn) * TN;
+        const int nst = (n0 + TN) >> 4;                       // K-stages up to the tile's last row
+        for (int it = 0; it < nst; ++it) {
+          mbar_wait(empty(s), ph ^ 1);
+          const uint32_t st = ring + (uint32_t)s * STAGE_BYTES;
+          // bytes of this stage: A is always whole, B shrinks inside the diagonal block
+          uint32_t bytes = 2 * A_PART;
+          int rowstart[2], nrows[2];
+#pragma unroll
+          for (int kk = 0; kk < 2; ++kk) {
+            const int xs = xs_of(2 * it + kk);
+            rowstart[kk] = max(n0, xs);
+            nrows[kk] = n0 + TN - rowstart[kk];
+            bytes += 4u * (uint32_t)nrows[kk] * 16u;            // 2 chunks x hi, lo
+          }
+          mbar_expect_tx(full(s), bytes);
+#pragma unroll
+          for (int h = 0; h < 2; ++h) {
+            const float* za = p.Zs + (((size_t)h * p.ntm + m) * nkc + 4 * it) * (TILE * 4);
+            bulk_g2s(st + (uint32_t)h * A_PART, za, A_PART, full(s));
+          }
+#pragma unroll
+          for (int kk = 0; kk < 2; ++kk) {
+            const int ks = 2 * it + kk, xs = xs_of(ks);
+            const size_t blk = (size_t)rows_before(ks, V) * 8;
+#pragma unroll
+            for (int c = 0; c < 2; ++c)
+#pragma unroll
+              for (int h = 0; h < 2; ++h) {
+                const float* src = p.Lsplit + (size_t)h * lpart + blk + (size_t)c * (V - xs) * 4 +
+                                   (size_t)(rowstart[kk] - xs) * 4;
+                const uint32_t dst = st + 2 * A_PART + (uint32_t)h * B_PART +
+                                     (uint32_t)(kk * 2 + c) * CHUNK_B +
+                                     (uint32_t)(rowstart[kk] - n0) * 16u;
+                bulk_g2s(dst, src, (uint32_t)nrows[kk] * 16u, full(s));
+              }
+          }
+          if (++s == STAGES) { s = 0; ph ^= 1; }
+        }
+      }
+    }
+    __syncwarp();
+  } else if (warp == 5) {
+    // ================================ MMA issuer ==============================================
+    if (lane == 0) {
+      int s = 0, cnt = 0;
+      uint32_t ph = 0;
+      const uint64_t a_base = smem_desc(ring, CHUNK_A, 128);
+      const uint64_t b_base = smem_desc(ring + 2 * A_PART, CHUNK_B, 128);
+      for (int tl = blockIdx.x; tl < ntiles; tl += gridDim.x, ++cnt) {
+        const int n0 = (tl % p.ntn) * TN;
+        const int nst = (n0 + TN) >> 4;
+        const int buf = cnt & 1;
+        mbar_wait(dempty(buf), ((cnt >> 1) & 1) ^ 1);
+        tc_fence_after();
+        const uint32_t dbase = taddr + (uint32_t)(buf * TN);
+        for (int it = 0; it < nst; ++it) {
+          mbar_wait(full(s), ph);
+          tc_fence_after();
+          const uint32_t so = (uint32_t)s * (STAGE_BYTES >> 4);
+#pragma unroll
+          for (int kk = 0; kk < 2; ++kk) {
+            const int xs = xs_of(2 * it + kk);
+            const int rowstart = max(n0, xs), nrows = n0 + TN - rowstart;
+            const uint32_t idesc = instr_desc(TILE, nrows);
+            const uint32_t d = dbase + (uint32_t)(rowstart - n0);
+            const uint64_t a_hi = a_base + so + (uint32_t)(2 * kk) * (CHUNK_A >> 4);
+            const uint64_t a_lo = a_hi + (A_PART >> 4);
+            const uint64_t b_hi = b_base + so + (uint32_t)(2 * kk) * (CHUNK_B >> 4) +
+                                  (uint32_t)(rowstart - n0);
+            const uint64_t b_lo = b_hi + (B_PART >> 4);
+            // the first K-step of a tile covers all TN columns and overwrites the accumulator
+            tc_mma_tf32(d, a_lo, b_hi, idesc, (it | kk) != 0);
+            tc_mma_tf32(d, a_hi, b_lo, idesc, 1);
+            tc_mma_tf32(d, a_hi, b_hi, idesc, 1);
+          }
+          tc_commit(empty(s));
+          if (++s == STAGES) { s = 0; ph ^= 1; }
+        }
+        tc_commit(dfull(buf));
+      }
+    }
+    __syncwarp();
+  } else {
+    // ================================ epilogue: phi' = phi + d ================================
+    int cnt = 0;
+    const uint32_t tlane = taddr + ((uint32_t)(warp * 32) << 16);
+    for (int tl = blockIdx.x; tl < ntiles; tl += gridDim.x, ++cnt) {
+      const int m = tl / p.ntn, n0 = (tl % p.ntn) * TN;
+      const int buf = cnt & 1;
+      const size_t col = (size_t)m * TILE + warp * 32 + lane;
+      mbar_wait_relaxed(dfull(buf), (cnt >> 1) & 1);
+      tc_fence_after();
+      for (int cb = 0; cb < TN; cb += 16) {
+        uint32_t r[16];
+        tmem_ld16(tlane + (uint32_t)(buf * TN + cb), r);
+        float f[16];
+#pragma unroll
+        for (int jj = 0; jj < 16; ++jj) f[jj] = p.phi[(size_t)(n0 + cb + jj) * p.ld + col];
+        tmem_ld_wait();
+#pragma unroll
+        for (int jj = 0; jj < 16; ++jj)
+          p.phip[(size_t)(n0 + cb + jj) * p.ld + col] = f[jj] + __uint_as_float(r[jj]);
+      }
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(dempty(buf));
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 0) tmem_dealloc(taddr, 2 * TN);
+}
+
+bool propose_tc_supported(int V) { return V >= 256 && (V % lg::TN) == 0; }
+
+size_t propose_tc_zsplit_floats(int V, int ld) { return (size_t)2 * V * ld; }
+
+void launch_normals_split(float* Zs, int N, int ld, int V, uint64_t seed, uint32_t tag, uint32_t t,
+                          const Ctrl* ctrl, int respect_done, cudaStream_t st) {
+  dim3 grid(ld / lg::TILE, V / 4);
+  ++g_launches;
+  normals_split_kernel<<<grid, 128, 0, st>>>(reinterpret_cast<float4*>(Zs), N, ld / lg::TILE, V, seed,
+                                             tag, t, ctrl, respect_done);
+}
+
+void launch_propose_tc(const float* phi, float* phip, const float* Zs, const float* Lsplit, int ld,
+                       int V, const Ctrl* ctrl, int respect_done, cudaStream_t st) {
+  static int num_sms = 0;
+  if (!num_sms) {
+    cudaFuncSetAttribute(propose_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                         lg::SMEM_BYTES);
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev);
+  }
+  ProposeTcParams p;
+  p.phi = phi; p.phip = phip; p.Zs = Zs; p.Lsplit = Lsplit; p.ctrl = ctrl;
+  p.ld = ld; p.V = V; p.ntm = ld / lg::TILE; p.ntn = V / lg::TN; p.respect_done = respect_done;
+  const int ntiles = p.ntm * p.ntn;
+  const int grid = ntiles < num_sms ? ntiles : num_sms;
+  ++g_launches;
+  propose_tc_kernel<<<grid, lg::THREADS, lg::SMEM_BYTES, st>>>(p);
+}
+
+}  // namespace phi4
