@@ -334,6 +334,8 @@ static CovCholArgs cov_args(phi4smc* h, int respect_done) {
   CovCholArgs c;
   c.phi = h->phi[h->cur]; c.N = h->N; c.ld = h->ld; c.V = h->md.V;
   c.mu = h->mu; c.Sigma = h->Sigma; c.Lc = h->Lc; c.partial = h->partial; c.ctrl = h->ctrl;
+  // the split-normal scratch of the large-V proposal doubles as the centred-split scratch
+  c.tc_scratch = (h->prm.mutation_path != 1 && propose_tc_supported(h->md.V) && h->kind == KIND_SMC) ? h->Z : nullptr;
   c.respect_done = respect_done;
   return c;
 }

@@ -422,11 +422,23 @@ static int cov_nsplit(int V, int N) {
   return ns;
 }
 
-size_t cov_partial_floats(int V, int N) { return (size_t)cov_nsplit(V, N) * V * V; }
+size_t cov_partial_floats(int V, int N) {
+  int ns = cov_nsplit(V, N);
+  const int ld = round_up(N, 128);
+  if (syrk_tc_supported(V, ld) && syrk_tc_nsplit(V, ld) > ns) ns = syrk_tc_nsplit(V, ld);
+  return (size_t)ns * V * V;
+}
 
 void launch_cov_chol(const CovCholArgs& a, cudaStream_t st) {
   const int V = a.V;
   ++g_launches; mean_kernel<<<V, 256, 0, st>>>(a.phi, a.N, a.ld, a.mu, a.ctrl, a.respect_done);
+  if (a.tc_scratch && syrk_tc_supported(V, a.ld)) {
+    launch_syrk_tc(a.phi, a.N, a.ld, V, a.mu, a.tc_scratch, a.partial, a.ctrl, a.respect_done, st);
+    ++g_launches; syrk_reduce_kernel<<<(V * V + 255) / 256, 256, 0, st>>>(
+        a.partial, syrk_tc_nsplit(V, a.ld), V, a.N, a.Sigma, a.ctrl, a.respect_done);
+    launch_cholesky(a.Sigma, a.Lc, V, a.ctrl, a.respect_done, st);
+    return;
+  }
   int ns = cov_nsplit(V, a.N);
   int chunk = round_up((a.ld + ns - 1) / ns, 16);
   ns = (a.ld + chunk - 1) / chunk;

@@ -73,6 +73,7 @@ struct CovCholArgs {
   float* Sigma;      // [V][V]
   float* Lc;         // [V][V]
   float* partial;    // split-K scratch, >= cov_partial_floats(V, N) floats
+  float* tc_scratch; // >= syrk_tc_scratch_floats(V, ld) floats, or nullptr: FP32 SIMT syrk
   Ctrl* ctrl;
   int respect_done;
 };
@@ -80,6 +81,13 @@ size_t cov_partial_floats(int V, int N);
 void launch_cov_chol(const CovCholArgs& a, cudaStream_t st);
 void launch_cholesky(const float* Sigma, float* Lc, int V, Ctrl* ctrl, int respect_done,
                      cudaStream_t st);
+
+// syrk_tc.cu -- C1 for large V: centred 3xTF32 tcgen05 syrk with K split
+bool syrk_tc_supported(int V, int ld);
+int syrk_tc_nsplit(int V, int ld);
+size_t syrk_tc_scratch_floats(int V, int ld);
+void launch_syrk_tc(const float* phi, int N, int ld, int V, const float* mu, float* Ps,
+                    float* partial, const Ctrl* ctrl, int respect_done, cudaStream_t st);
 
 // observables.cu -- O
 void launch_magnetisation(const float* phi, int N, int ld, int V, float* M, cudaStream_t st);

@@ -7,14 +7,17 @@
 //                         K-major interleave layout, tile-major: Zs[part][particle tile][K-chunk]
 //                         [128 rows][4] -- a ring stage is one contiguous 8 KB run per part.
 //   propose_tc_kernel     one CTA per SM loops over (particle tile 128) x (site tile 256) output
-//                         tiles.  Warp 4 streams A (normals) and B (s Lc, packed lower-triangular
+//                         tiles.  Warp 8 streams A (normals) and B (s Lc, packed lower-triangular
 //                         blocks of tcgen05.cuh) into a 4-stage shared-memory ring with
-//                         cp.async.bulk + mbarrier; warp 5 issues tcgen05.mma kind::tf32 (three
+//                         cp.async.bulk + mbarrier; warp 9 issues tcgen05.mma kind::tf32 (three
 //                         products per K-step into one FP32 TMEM accumulator, K-steps above the
-//                         diagonal skipped, N shrunk inside the diagonal block); warps 0-3 read the
+//                         diagonal skipped, N shrunk inside the diagonal block); warps 0-7 read the
 //                         accumulator with tcgen05.ld (lane = particle) and write phi' = phi + d,
 //                         coalesced along particles.  The accumulator is double-buffered (2 x 256
 //                         TMEM columns), so the epilogue of a tile overlaps the MMAs of the next.
+// The tensor core's FP32 accumulation truncates (measured in syrk_tc.cu: -1e-4 relative over 3000
+// MMAs), so one TMEM accumulator only runs over K = 1024 (384 MMAs, ~1e-5 of |d|); the epilogue
+// folds the chains into round-to-nearest FP32 register sums.
 // The accept step stays in accept_kernel (mutate_generic.cu): it needs whole lattice rows of phi'.
 #include "kernels.cuh"
 #include "philox.cuh"
@@ -31,7 +34,8 @@ constexpr int CHUNK_B = TN * 16;
 constexpr int A_PART = 4 * CHUNK_A;          // K = 16 per stage: 4 chunks per hi / lo part
 constexpr int B_PART = 4 * CHUNK_B;
 constexpr int STAGE_BYTES = 2 * A_PART + 2 * B_PART;   // 48 KB
-constexpr int THREADS = 192;                 // 4 epilogue warps, producer warp, MMA warp
+constexpr int THREADS = 320;                 // 8 epilogue warps, producer warp, MMA warp
+constexpr int SUB_STAGES = 64;               // one TMEM accumulation chain covers K = 1024
 constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 256;
 }  // namespace lg
 
@@ -79,9 +83,9 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int V = p.V, nkc = V >> 2, ntiles = p.ntm * p.ntn;
 
-  if (warp == 4 && lane == 0) {
+  if (warp == 8 && lane == 0) {
     for (int s = 0; s < STAGES; ++s) { mbar_init(full(s), 1); mbar_init(empty(s), 1); }
-    for (int b = 0; b < 2; ++b) { mbar_init(dfull(b), 1); mbar_init(dempty(b), 4); }
+    for (int b = 0; b < 2; ++b) { mbar_init(dfull(b), 1); mbar_init(dempty(b), 8); }
     fence_mbar_init();
   }
   if (warp == 0) tmem_alloc(smem_u32(tmem_slot), 2 * TN);
@@ -91,7 +95,7 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
   const uint32_t taddr = *tmem_slot;
   const uint32_t ring = smem_u32(smem);
 
-  if (warp == 4) {
+  if (warp == 8) {
     // ================================ producer: bulk copies into the ring =====================
     if (lane == 0) {
       const size_t lpart = l_floats(V);
@@ -140,71 +144,113 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
       }
     }
     __syncwarp();
-  } else if (warp == 5) {
+  } else if (warp == 9) {
     // ================================ MMA issuer ==============================================
     if (lane == 0) {
       int s = 0, cnt = 0;
       uint32_t ph = 0;
       const uint64_t a_base = smem_desc(ring, CHUNK_A, 128);
       const uint64_t b_base = smem_desc(ring + 2 * A_PART, CHUNK_B, 128);
-      for (int tl = blockIdx.x; tl < ntiles; tl += gridDim.x, ++cnt) {
+      for (int tl = blockIdx.x; tl < ntiles; tl += gridDim.x) {
         const int n0 = (tl % p.ntn) * TN;
         const int nst = (n0 + TN) >> 4;
-        const int buf = cnt & 1;
-        mbar_wait(dempty(buf), ((cnt >> 1) & 1) ^ 1);
-        tc_fence_after();
-        const uint32_t dbase = taddr + (uint32_t)(buf * TN);
-        for (int it = 0; it < nst; ++it) {
-          mbar_wait(full(s), ph);
+        for (int it0 = 0; it0 < nst; it0 += SUB_STAGES, ++cnt) {
+          const int buf = cnt & 1;
+          mbar_wait(dempty(buf), ((cnt >> 1) & 1) ^ 1);
           tc_fence_after();
-          const uint32_t so = (uint32_t)s * (STAGE_BYTES >> 4);
+          const uint32_t dbase = taddr + (uint32_t)(buf * TN);
+          const int it1 = min(nst, it0 + SUB_STAGES);
+          for (int it = it0; it < it1; ++it) {
+            mbar_wait(full(s), ph);
+            tc_fence_after();
+            const uint32_t so = (uint32_t)s * (STAGE_BYTES >> 4);
 #pragma unroll
-          for (int kk = 0; kk < 2; ++kk) {
-            const int xs = xs_of(2 * it + kk);
-            const int rowstart = max(n0, xs), nrows = n0 + TN - rowstart;
-            const uint32_t idesc = instr_desc(TILE, nrows);
-            const uint32_t d = dbase + (uint32_t)(rowstart - n0);
-            const uint64_t a_hi = a_base + so + (uint32_t)(2 * kk) * (CHUNK_A >> 4);
-            const uint64_t a_lo = a_hi + (A_PART >> 4);
-            const uint64_t b_hi = b_base + so + (uint32_t)(2 * kk) * (CHUNK_B >> 4) +
-                                  (uint32_t)(rowstart - n0);
-            const uint64_t b_lo = b_hi + (B_PART >> 4);
-            // the first K-step of a tile covers all TN columns and overwrites the accumulator
-            tc_mma_tf32(d, a_lo, b_hi, idesc, (it | kk) != 0);
-            tc_mma_tf32(d, a_hi, b_lo, idesc, 1);
-            tc_mma_tf32(d, a_hi, b_hi, idesc, 1);
+            for (int kk = 0; kk < 2; ++kk) {
+              const int xs = xs_of(2 * it + kk);
+              const int rowstart = max(n0, xs), nrows = n0 + TN - rowstart;
+              const uint32_t idesc = instr_desc(TILE, nrows);
+              const uint32_t d = dbase + (uint32_t)(rowstart - n0);
+              const uint64_t a_hi = a_base + so + (uint32_t)(2 * kk) * (CHUNK_A >> 4);
+              const uint64_t a_lo = a_hi + (A_PART >> 4);
+              const uint64_t b_hi = b_base + so + (uint32_t)(2 * kk) * (CHUNK_B >> 4) +
+                                    (uint32_t)(rowstart - n0);
+              const uint64_t b_lo = b_hi + (B_PART >> 4);
+              // The first K-step of a chain overwrites the accumulator.  Only the chain that ends
+              // in the diagonal block has shrunk K-steps, and it starts with a full-width one
+              // (n0 is a multiple of 256 <= 16 it0 whenever it0 > 0), so no column is left stale.
+              tc_mma_tf32(d, a_lo, b_hi, idesc, (it != it0) || kk);
+              tc_mma_tf32(d, a_hi, b_lo, idesc, 1);
+              tc_mma_tf32(d, a_hi, b_hi, idesc, 1);
+            }
+            tc_commit(empty(s));
+            if (++s == STAGES) { s = 0; ph ^= 1; }
           }
-          tc_commit(empty(s));
-          if (++s == STAGES) { s = 0; ph ^= 1; }
+          tc_commit(dfull(buf));
         }
-        tc_commit(dfull(buf));
       }
     }
     __syncwarp();
   } else {
-    // ================================ epilogue: phi' = phi + d ================================
+    // ================================ epilogue: phi' = phi + sum of chains ====================
+    // warp w: TMEM lane quarter w % 4 (32 particles), column half w / 4 (128 sites)
     int cnt = 0;
-    const uint32_t tlane = taddr + ((uint32_t)(warp * 32) << 16);
-    for (int tl = blockIdx.x; tl < ntiles; tl += gridDim.x, ++cnt) {
+    const int Q = warp & 3, hc = warp >> 2;
+    const uint32_t tlane = taddr + ((uint32_t)(Q * 32) << 16);
+    for (int tl = blockIdx.x; tl < ntiles; tl += gridDim.x) {
       const int m = tl / p.ntn, n0 = (tl % p.ntn) * TN;
-      const int buf = cnt & 1;
-      const size_t col = (size_t)m * TILE + warp * 32 + lane;
-      mbar_wait_relaxed(dfull(buf), (cnt >> 1) & 1);
-      tc_fence_after();
-      for (int cb = 0; cb < TN; cb += 16) {
-        uint32_t r[16];
-        tmem_ld16(tlane + (uint32_t)(buf * TN + cb), r);
-        float f[16];
+      const int nst = (n0 + TN) >> 4;
+      const size_t col = (size_t)m * TILE + Q * 32 + lane;
+      const int x0 = n0 + hc * 128;
+      if (nst <= SUB_STAGES) {
+        // one chain: accumulator -> phi' directly, 16 columns (16 loads in flight) at a time
+        const int buf = cnt & 1;
+        mbar_wait_relaxed(dfull(buf), (cnt >> 1) & 1);
+        tc_fence_after();
+        for (int cb = 0; cb < 128; cb += 16) {
+          uint32_t r[16];
+          tmem_ld16(tlane + (uint32_t)(buf * TN + hc * 128 + cb), r);
+          float f[16];
 #pragma unroll
-        for (int jj = 0; jj < 16; ++jj) f[jj] = p.phi[(size_t)(n0 + cb + jj) * p.ld + col];
-        tmem_ld_wait();
+          for (int jj = 0; jj < 16; ++jj) f[jj] = p.phi[(size_t)(x0 + cb + jj) * p.ld + col];
+          tmem_ld_wait();
 #pragma unroll
-        for (int jj = 0; jj < 16; ++jj)
-          p.phip[(size_t)(n0 + cb + jj) * p.ld + col] = f[jj] + __uint_as_float(r[jj]);
+          for (int jj = 0; jj < 16; ++jj)
+            p.phip[(size_t)(x0 + cb + jj) * p.ld + col] = f[jj] + __uint_as_float(r[jj]);
+        }
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(dempty(buf));
+        ++cnt;
+      } else {
+        float acc[128];
+#pragma unroll
+        for (int j = 0; j < 128; ++j) acc[j] = 0.f;
+        for (int it0 = 0; it0 < nst; it0 += SUB_STAGES, ++cnt) {
+          const int buf = cnt & 1;
+          mbar_wait_relaxed(dfull(buf), (cnt >> 1) & 1);
+          tc_fence_after();
+#pragma unroll
+          for (int cb = 0; cb < 128; cb += 16) {
+            uint32_t r[16];
+            tmem_ld16(tlane + (uint32_t)(buf * TN + hc * 128 + cb), r);
+            tmem_ld_wait();
+#pragma unroll
+            for (int jj = 0; jj < 16; ++jj) acc[cb + jj] += __uint_as_float(r[jj]);
+          }
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(dempty(buf));
+        }
+#pragma unroll
+        for (int cb = 0; cb < 128; cb += 16) {
+          float f[16];
+#pragma unroll
+          for (int jj = 0; jj < 16; ++jj) f[jj] = p.phi[(size_t)(x0 + cb + jj) * p.ld + col];
+#pragma unroll
+          for (int jj = 0; jj < 16; ++jj)
+            p.phip[(size_t)(x0 + cb + jj) * p.ld + col] = f[jj] + acc[cb + jj];
+        }
       }
-      tc_fence_before();
-      __syncwarp();
-      if (lane == 0) mbar_arrive(dempty(buf));
     }
   }
   tc_fence_before();
