@@ -171,27 +171,12 @@ __device__ __forceinline__ bool chol_skip(const Ctrl* ctrl, int attempt, int res
 // update to the trailing lower triangle.  Three barriers per panel instead of two per column.
 // Both attempts of reading A4 (plain, then jitter 1e-6 tr/V) run inside this one launch.
 constexpr int CS_NB = 8;
-__global__ void __launch_bounds__(1024)
-chol_small_kernel(const float* __restrict__ Sigma, float* __restrict__ Lc, int V, Ctrl* ctrl,
-                  int respect_done) {
-  extern __shared__ float sm[];   // V x (V+1)
-  __shared__ int failed_s;
-  __shared__ double red[33];
-  if (respect_done && ctrl->done) return;
-  const int P = V + 1, tid = threadIdx.x;
-  // tr(Sigma) for the jitter scale
-  double tr = 0.0;
-  for (int x = tid; x < V; x += blockDim.x) tr += (double)Sigma[(size_t)x * V + x];
-  tr = block_sum(tr, red);
-  int status = 0;
-  for (int attempt = 0; attempt < 2; ++attempt) {
-    const float add = attempt ? 1e-6f * (float)tr / (float)V : 0.f;
-    if (tid == 0) failed_s = 0;
-    for (int idx = tid; idx < V * V; idx += blockDim.x) {
-      int x = idx / V, y = idx - x * V;
-      sm[x * P + y] = Sigma[idx] + (x == y ? add : 0.f);
-    }
-    __syncthreads();
+// In-place lower Cholesky of the n x n matrix in shared memory (row stride P), 8-column panels:
+// every row thread re-factorises the 8x8 diagonal block in registers and solves its own row,
+// then the whole block applies the rank-8 update to the trailing lower triangle.  *failed_s is
+// set if a pivot is <= 0 (the factorisation then continues with a unit pivot).
+__device__ __forceinline__ void chol_panels(float* sm, int P, int V, int* failed_s) {
+  const int tid = threadIdx.x;
     for (int jb = 0; jb < V; jb += CS_NB) {
       // ---- panel: rows r >= jb, one thread per row
       const int r = jb + tid;
@@ -221,7 +206,7 @@ chol_small_kernel(const float* __restrict__ Sigma, float* __restrict__ Lc, int V
 #pragma unroll
             for (int c = k + 1; c <= i; ++c) D[i][c] = fmaf(-D[i][k], D[c][k], D[i][c]);
         }
-        if (bad && tid == 0) failed_s = 1;
+        if (bad) *failed_s = 1;
         const int ri = r - jb;               // row inside the diagonal block if < CS_NB
 #pragma unroll
         for (int k = 0; k < CS_NB; ++k) {
@@ -248,7 +233,7 @@ chol_small_kernel(const float* __restrict__ Sigma, float* __restrict__ Lc, int V
       const int j1 = jb + CS_NB;
       if (j1 < V) {
         const int tx = tid & 31, ty = tid >> 5;
-        for (int rr = j1 + ty; rr < V; rr += 32) {
+        for (int rr = j1 + ty; rr < V; rr += (int)(blockDim.x >> 5)) {
           float lr[CS_NB];
 #pragma unroll
           for (int k = 0; k < CS_NB; ++k) lr[k] = sm[rr * P + jb + k];
@@ -262,6 +247,30 @@ chol_small_kernel(const float* __restrict__ Sigma, float* __restrict__ Lc, int V
       }
       __syncthreads();
     }
+}
+
+__global__ void __launch_bounds__(1024)
+chol_small_kernel(const float* __restrict__ Sigma, float* __restrict__ Lc, int V, Ctrl* ctrl,
+                  int respect_done) {
+  extern __shared__ float sm[];   // V x (V+1)
+  __shared__ int failed_s;
+  __shared__ double red[33];
+  if (respect_done && ctrl->done) return;
+  const int P = V + 1, tid = threadIdx.x;
+  // tr(Sigma) for the jitter scale
+  double tr = 0.0;
+  for (int x = tid; x < V; x += blockDim.x) tr += (double)Sigma[(size_t)x * V + x];
+  tr = block_sum(tr, red);
+  int status = 0;
+  for (int attempt = 0; attempt < 2; ++attempt) {
+    const float add = attempt ? 1e-6f * (float)tr / (float)V : 0.f;
+    if (tid == 0) failed_s = 0;
+    for (int idx = tid; idx < V * V; idx += blockDim.x) {
+      int x = idx / V, y = idx - x * V;
+      sm[x * P + y] = Sigma[idx] + (x == y ? add : 0.f);
+    }
+    __syncthreads();
+    chol_panels(sm, P, V, &failed_s);
     const int failed = failed_s;
     __syncthreads();
     if (!failed) { status = attempt; break; }
@@ -285,33 +294,27 @@ __global__ void chol_copy_kernel(const float* __restrict__ Sigma, float* __restr
   Lc[idx] = (y <= x) ? Sigma[idx] + add : 0.f;
 }
 
-// Diagonal block [j0, j0+nb) factorised in shared memory by one CTA of 64 threads (thread = row).
-__global__ void __launch_bounds__(64)
+// Diagonal block [j0, j0+nb) factorised in shared memory by one CTA (panel algorithm above).
+__global__ void __launch_bounds__(256)
 chol_diag_kernel(float* __restrict__ A, int V, int j0, Ctrl* ctrl, int attempt,
                  int respect_done) {
-  __shared__ float T[64][65];
+  __shared__ float T[64 * 65];
+  __shared__ int failed_s;
   if (chol_skip(ctrl, attempt, respect_done)) return;
-  const int nb = min(64, V - j0), r = threadIdx.x;
-  for (int c = 0; c < nb; ++c) T[r][c] = (r < nb && c <= r) ? A[(size_t)(j0 + r) * V + j0 + c] : 0.f;
-  __syncthreads();
-  int failed = 0;
-  for (int j = 0; j < nb; ++j) {
-    float d = T[j][j];
-    if (!(d > 0.f)) { failed = 1; d = 1.f; }
-    float sq = sqrtf(d);
-    __syncthreads();
-    if (r == j) T[r][j] = sq;
-    else if (r > j && r < nb) T[r][j] = T[r][j] / sq;
-    __syncthreads();
-    if (r > j && r < nb) {
-      float lrj = T[r][j];
-      for (int c = j + 1; c <= r; ++c) T[r][c] = fmaf(-lrj, T[c][j], T[r][c]);
-    }
-    __syncthreads();
+  const int nb = min(64, V - j0);
+  if (threadIdx.x == 0) failed_s = 0;
+  for (int e = threadIdx.x; e < nb * nb; e += blockDim.x) {
+    const int r = e / nb, c = e - r * nb;
+    T[r * 65 + c] = (c <= r) ? A[(size_t)(j0 + r) * V + j0 + c] : 0.f;
   }
-  for (int c = 0; c < nb; ++c)
-    if (r < nb && c <= r) A[(size_t)(j0 + r) * V + j0 + c] = T[r][c];
-  if (r == 0 && failed) atomicOr(&ctrl->chol_fail, attempt ? 2 : 1);
+  __syncthreads();
+  chol_panels(T, 65, nb, &failed_s);
+  __syncthreads();
+  for (int e = threadIdx.x; e < nb * nb; e += blockDim.x) {
+    const int r = e / nb, c = e - r * nb;
+    if (c <= r) A[(size_t)(j0 + r) * V + j0 + c] = T[r * 65 + c];
+  }
+  if (threadIdx.x == 0 && failed_s) atomicOr(&ctrl->chol_fail, attempt ? 2 : 1);
 }
 
 // Rows below the diagonal block: X L11^T = A21, one thread per row, L11 in shared memory.
@@ -397,7 +400,7 @@ void launch_cholesky(const float* Sigma, float* Lc, int V, Ctrl* ctrl, int respe
                                                           respect_done);
     for (int j0 = 0; j0 < V; j0 += 64) {
       int j1 = min(V, j0 + 64);
-      ++g_launches; chol_diag_kernel<<<1, 64, 0, st>>>(Lc, V, j0, ctrl, attempt, respect_done);
+      ++g_launches; chol_diag_kernel<<<1, 256, 0, st>>>(Lc, V, j0, ctrl, attempt, respect_done);
       int rows = V - j1;
       if (rows > 0) {
         ++g_launches; chol_trsm_kernel<<<(rows + 63) / 64, 64, 0, st>>>(Lc, V, j0, ctrl, attempt,
