@@ -57,7 +57,7 @@ struct phi4smc {
   int k_del, n_walk, max_iters, ldw;
   double stop_frac;
   float *wphi, *wS, *wU, *dead_S, *dead_M, *M_all, *S_all;
-  double *dead_logw, *logw_all;
+  double *dead_logw, *logw_all, *hsum;
   int32_t *dead, *surv, *start;
   // host side
   uint64_t step_counter;     // mutation steps enqueued so far (next step uses counter + 1)
@@ -133,6 +133,7 @@ static int carve_ns(phi4smc* h, char* base, size_t* total) {
   h->dead_S = c.take<float>(nlog);
   h->dead_M = c.take<float>(nlog);
   h->dead_logw = c.take<double>(nlog);
+  h->hsum = c.take<double>(kd + 1);
   h->M_all = c.take<float>(nlog + N);
   h->S_all = c.take<float>(nlog + N);
   h->logw_all = c.take<double>(nlog + N);
@@ -498,7 +499,7 @@ static NsArgs ns_args(phi4smc* h) {
   a.n = h->N; a.ld = h->ld; a.k_del = h->k_del; a.ldw = h->ldw; a.V = h->md.V;
   a.seed = h->seed; a.dead = h->dead; a.surv = h->surv; a.start = h->start;
   a.dead_S = h->dead_S; a.dead_M = h->dead_M; a.dead_logw = h->dead_logw;
-  a.max_iters = h->max_iters; a.stop_frac = h->stop_frac; a.ctrl = h->ctrl;
+  a.max_iters = h->max_iters; a.stop_frac = h->stop_frac; a.ctrl = h->ctrl; a.hsum = h->hsum;
   return a;
 }
 
@@ -527,6 +528,7 @@ PHI4_API int ns_init(phi4smc** out, int L, float m0sq, float lambda, int n_live,
   memset(h->h_ctrl, 0, sizeof(Ctrl));
   h->h_ctrl->logZ = -INFINITY;
   CU(cudaMemcpyAsync(h->ctrl, h->h_ctrl, sizeof(Ctrl), cudaMemcpyHostToDevice, h->st));
+  launch_ns_hsum(h->hsum, n_live, k_delete, h->st);
   launch_init_particles(h->phi[0], n_live, h->ld, h->md.V, seed, h->st);
   launch_action(h->phi[0], n_live, h->ld, h->md, h->S[0], h->U0[0], h->ctrl, h->st);
   launch_set_identity(h->Lc, h->md.V, h->st);

@@ -79,6 +79,7 @@ struct TcParams {
   uint64_t seed;
   uint32_t tag_prop, tag_acc, t0;
   int k, respect_done;
+  PhiloxKeys rk;               // round keys of `seed` (constant-bank operands of the Philox XORs)
 };
 
 // (s Lc) -> hi/lo TF32 split in the layout the MMA reads.  K-step ks is a block of two 16-byte
@@ -311,11 +312,11 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
         if (second) {
 #pragma unroll
           for (int c = 0; c < 4; ++c)
-            w[c] = philox_draw(p.seed, p.tag_prop, tt, (uint32_t)i, (uint32_t)(4 * (it + (c >> 1)) + 2 * (c & 1) + half));
+            w[c] = philox4x32_10_rk((uint32_t)(4 * (it + (c >> 1)) + 2 * (c & 1) + half), (uint32_t)i, tt, p.tag_prop, p.rk);
         } else {
 #pragma unroll
           for (int c = 0; c < 2; ++c)
-            w[c] = philox_draw(p.seed, p.tag_prop, tt, (uint32_t)i, (uint32_t)(4 * it + 2 * c + half));
+            w[c] = philox4x32_10_rk((uint32_t)(4 * it + 2 * c + half), (uint32_t)i, tt, p.tag_prop, p.rk);
           w[2] = w[0]; w[3] = w[1];
         }
         TC_TRACE(1, tr);
@@ -379,7 +380,7 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
       U4 w[2];
 #pragma unroll
       for (int e = 0; e < 2; ++e)
-        if (e < nitE) w[e] = philox_draw(p.seed, p.tag_prop, p.t0 + (uint32_t)t, (uint32_t)i, (uint32_t)(4 * (nitP + e) + g));
+        if (e < nitE) w[e] = philox4x32_10_rk((uint32_t)(4 * (nitP + e) + g), (uint32_t)i, p.t0 + (uint32_t)t, p.tag_prop, p.rk);
 #pragma unroll
       for (int e = 0; e < 2; ++e) {
         if (e >= nitE) break;
@@ -531,6 +532,7 @@ void launch_mutate_tc(const MutateArgs& a, float* Lsplit, cudaStream_t st) {
   p.m0sq = a.md.m0sq; p.lam = a.md.lam; p.mode = a.mode; p.seed = a.seed;
   p.tag_prop = a.tag_prop; p.tag_acc = a.tag_acc; p.t0 = a.t0; p.k = a.k;
   p.respect_done = a.respect_done;
+  p.rk = philox_round_keys(a.seed);
   const size_t smem = tc::smem_layout(V).total;
   static bool attr_done = false;
   if (!attr_done) {

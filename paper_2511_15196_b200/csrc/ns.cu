@@ -62,8 +62,7 @@ ns_select_evidence_kernel(NsArgs a) {
   double term_mine[1];   // kd <= 1024 = blockDim: one dead point per thread at most
   term_mine[0] = -INFINITY;
   if (tid < kd) {
-    double lx = logX0;
-    for (int m = 1; m <= tid; ++m) lx -= 1.0 / (double)(n - m + 1);      // logX_{j-1}, j = tid+1
+    const double lx = logX0 - a.hsum[tid];                                // logX_{j-1}, j = tid+1
     double step = 1.0 / (double)(n - tid);                                // 1/(n-j+1)
     double logw = lx + log1p(-exp(-step));
     int d = (int)(uint32_t)keys[tid];
@@ -132,9 +131,7 @@ ns_select_evidence_kernel(NsArgs a) {
     a.start[j] = a.surv[r % (uint32_t)ns];
   }
   if (tid == 0) {
-    double lx = logX0;
-    for (int m = 1; m <= kd; ++m) lx -= 1.0 / (double)(n - m + 1);
-    ctrl->logX = lx;
+    ctrl->logX = logX0 - a.hsum[kd];
     ctrl->logZ = logaddexp_d(ctrl->logZ, best + log(e));
     ctrl->S_star = (double)S_star;
   }
@@ -153,42 +150,70 @@ void launch_ns_select_evidence(const NsArgs& a, cudaStream_t st) {
   ++g_launches; ns_select_evidence_kernel<<<1, 1024, smem, st>>>(a);
 }
 
-// N3 gather: walker j <- live point start[j]; also logs the magnetisation of dead point j.
+// hsum[j] = sum_{m=1..j} 1/(n-m+1), j = 0..k_del: the data-independent volume shrinkage of
+// reading A6, tabulated once at ns_init.
+__global__ void ns_hsum_kernel(double* hsum, int n, int k_del) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  double acc = 0.0;
+  hsum[0] = 0.0;
+  for (int m = 1; m <= k_del; ++m) { acc += 1.0 / (double)(n - m + 1); hsum[m] = acc; }
+}
+void launch_ns_hsum(double* hsum, int n, int k_del, cudaStream_t st) {
+  ++g_launches; ns_hsum_kernel<<<1, 32, 0, st>>>(hsum, n, k_del);
+}
+
+// N3 gather: walker j <- live point start[j].  One thread per (site, walker): the walker index is
+// the fast one, so the stores are coalesced and the gathers hit 512 distinct columns of one row.
 __global__ void ns_load_walkers_kernel(NsArgs a) {
   if (a.ctrl->done) return;
-  int j = blockIdx.x * blockDim.x + threadIdx.x;
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  const int x = blockIdx.y;
   if (j >= a.ldw) return;
   const bool live = j < a.k_del;
-  const int src = live ? a.start[j] : 0, d = live ? a.dead[j] : 0;
-  float m = 0.f;
-  for (int x = 0; x < a.V; ++x) {
-    const float* row = a.phi + (size_t)x * a.ld;
-    a.wphi[(size_t)x * a.ldw + j] = live ? row[src] : 0.f;
-    if (live) m += row[d];
+  const int src = live ? a.start[j] : 0;
+  a.wphi[(size_t)x * a.ldw + j] = live ? a.phi[(size_t)x * a.ld + src] : 0.f;
+  if (x == 0) {
+    a.wS[j] = live ? a.S[src] : 0.f;
+    a.wU[j] = live ? a.U0[src] : 0.f;
   }
-  a.wS[j] = live ? a.S[src] : 0.f;
-  a.wU[j] = live ? a.U0[src] : 0.f;
+}
+
+// Magnetisation of the dead points (logged for the posterior observables): one warp per point.
+__global__ void ns_dead_M_kernel(NsArgs a) {
+  if (a.ctrl->done) return;
+  const int j = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  if (j >= a.k_del) return;
+  const int d = a.dead[j];
+  float m = 0.f;
+  for (int x = lane; x < a.V; x += 32) m += a.phi[(size_t)x * a.ld + d];
+  m = warp_sum(m);
   const int it = a.ctrl->temp_index;
-  if (live && it < a.max_iters) a.dead_M[(size_t)it * a.k_del + j] = m / (float)a.V;
+  if (lane == 0 && it < a.max_iters) a.dead_M[(size_t)it * a.k_del + j] = m / (float)a.V;
 }
 
 void launch_ns_load_walkers(const NsArgs& a, cudaStream_t st) {
-  ++g_launches; ns_load_walkers_kernel<<<(a.ldw + 127) / 128, 128, 0, st>>>(a);
+  ++g_launches; ns_dead_M_kernel<<<(a.k_del * 32 + 127) / 128, 128, 0, st>>>(a);
+  dim3 grid((a.ldw + 127) / 128, a.V);
+  ++g_launches; ns_load_walkers_kernel<<<grid, 128, 0, st>>>(a);
 }
 
-// N3 scatter: dead slot dead[j] <- walker j.
+// N3 scatter: dead slot dead[j] <- walker j, one thread per (site, walker).
 __global__ void ns_store_walkers_kernel(NsArgs a) {
   if (a.ctrl->done) return;
-  int j = blockIdx.x * blockDim.x + threadIdx.x;
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  const int x = blockIdx.y;
   if (j >= a.k_del) return;
   const int d = a.dead[j];
-  for (int x = 0; x < a.V; ++x) a.phi[(size_t)x * a.ld + d] = a.wphi[(size_t)x * a.ldw + j];
-  a.S[d] = a.wS[j];
-  a.U0[d] = a.wU[j];
+  a.phi[(size_t)x * a.ld + d] = a.wphi[(size_t)x * a.ldw + j];
+  if (x == 0) {
+    a.S[d] = a.wS[j];
+    a.U0[d] = a.wU[j];
+  }
 }
 
 void launch_ns_store_walkers(const NsArgs& a, cudaStream_t st) {
-  ++g_launches; ns_store_walkers_kernel<<<(a.k_del + 127) / 128, 128, 0, st>>>(a);
+  dim3 grid((a.k_del + 127) / 128, a.V);
+  ++g_launches; ns_store_walkers_kernel<<<grid, 128, 0, st>>>(a);
 }
 
 // N4: remaining = X mean_live(e^-S) / (Z + X mean_live(e^-S)); record; stop rule; live term.

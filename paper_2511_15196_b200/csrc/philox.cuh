@@ -28,6 +28,33 @@ __device__ __forceinline__ U4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c
   return U4{c0, c1, c2, c3};
 }
 
+// Round keys k + r * Weyl for r = 0..9, tabulated on the host and passed in kernel-parameter
+// space: the per-round XOR then takes its key straight from the constant bank instead of
+// spending two integer adds per round per chain.
+struct PhiloxKeys { uint32_t k0[10], k1[10]; };
+
+inline PhiloxKeys philox_round_keys(uint64_t seed) {
+  PhiloxKeys rk;
+  uint32_t a = (uint32_t)seed, b = (uint32_t)(seed >> 32);
+  for (int r = 0; r < 10; ++r) { rk.k0[r] = a; rk.k1[r] = b; a += 0x9E3779B9u; b += 0xBB67AE85u; }
+  return rk;
+}
+
+__device__ __forceinline__ U4 philox4x32_10_rk(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                               const PhiloxKeys& rk) {
+  constexpr uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u;
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    const uint64_t p0 = (uint64_t)M0 * (uint64_t)c0;
+    const uint64_t p1 = (uint64_t)M1 * (uint64_t)c2;
+    c0 = (uint32_t)(p1 >> 32) ^ c1 ^ rk.k0[r];
+    c2 = (uint32_t)(p0 >> 32) ^ c3 ^ rk.k1[r];
+    c1 = (uint32_t)p1;
+    c3 = (uint32_t)p0;
+  }
+  return U4{c0, c1, c2, c3};
+}
+
 __device__ __forceinline__ U4 philox_draw(uint64_t seed, uint32_t tag, uint32_t t, uint32_t slot,
                                           uint32_t q) {
   return philox4x32_10(q, slot, t, tag, (uint32_t)seed, (uint32_t)(seed >> 32));
@@ -55,15 +82,24 @@ __device__ __forceinline__ void box_muller_fast(uint32_t xa, uint32_t xb, float&
   const uint32_t m = (xa >> 8) + 1u;                             // 1 .. 2^24
   const float ur = (float)m * 5.9604644775390625e-8f;            // exact
   float w;
-  if (m > 16777216u - 4096u) w = -2.0f * logf(ur);
-  else w = -1.3862943611198906f * __log2f(ur);
-  float r;
-  asm("sqrt.approx.f32 %0, %1;" : "=f"(r) : "f"(w));
+  // .ftz forms: every argument here is zero or a normal number (ur >= 2^-24, w >= 0,
+  // |th| <= pi), so the subnormal fix-up code of the default forms would never fire
+  if (m > 16777216u - 4096u) {
+    w = -2.0f * logf(ur);
+  } else {
+    float l2;
+    asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(l2) : "f"(ur));
+    w = -1.3862943611198906f * l2;
+  }
+  float r, cs, sn;
+  asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(w));
   const uint32_t kb = xb >> 8;                                   // angle code, 24 bits
   const int sk = (int)kb - (int)((kb & 0x800000u) << 1);         // same angle in [-2^23, 2^23)
   const float th = (float)sk * 3.7450702829238413e-7f;           // 2 pi 2^-24
-  za = r * __cosf(th);
-  zb = r * __sinf(th);
+  asm("cos.approx.ftz.f32 %0, %1;" : "=f"(cs) : "f"(th));
+  asm("sin.approx.ftz.f32 %0, %1;" : "=f"(sn) : "f"(th));
+  za = r * cs;
+  zb = r * sn;
 }
 
 __device__ __forceinline__ void normals4_fast(uint64_t seed, uint32_t tag, uint32_t t,
