@@ -121,6 +121,9 @@ def workload_config(args, cfg, temps=None):
          "l2": "flushed between timed steps (256 MiB write)"}
     if temps is not None:
         c["temperatures_per_step"] = temps
+    if cfg["L"] ** 2 >= 1024:
+        c["note"] = "full schedule to beta=1 takes 100+ temperatures at this size: each step runs the first max_temps"
+
     return c
 
 
@@ -134,6 +137,9 @@ def main():
     ap.add_argument("--path", type=int, default=0, help="mutation path: 0 auto, 1 generic, 2 fused")
     ap.add_argument("--ref-particles", type=int, default=16384)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--max-temps", type=int, default=-1,
+                    help="temperatures per step; -1: to beta=1 (C0-C2), 6 for C3/C4 whose full schedule "
+                         "takes 100+ temperatures")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
 
@@ -166,6 +172,7 @@ def main():
     B.load()
 
     L, N, k, V = cfg["L"], cfg["N"], cfg["k"], cfg["L"] ** 2
+    max_temps = args.max_temps if args.max_temps > 0 else (6 if V >= 1024 else 4096)
     h = B.smc_init(L, cfg["m0sq"], cfg["lam"], N, 0, device=dev)
     B.smc_set_params(h, k_steps=k, ess_target=cfg["ess"], mutation_path=args.path)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
@@ -182,7 +189,7 @@ def main():
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record()
         B.smc_reset(h, seed)
-        T = B.smc_run(h)
+        T = B.smc_run(h, max_temps)
         e1.record()
         torch.cuda.synchronize()
         return e0.elapsed_time(e1), T
@@ -217,7 +224,7 @@ def main():
         t0 = time.perf_counter()
         B.smc_reset(h, seed)
         B.smc_set_state(h, phi_in, 0.0, 0)            # H2D: V*N fp32 initial particles
-        T = B.smc_run(h)
+        T = B.smc_run(h, max_temps)
         st = B.smc_get_state(h)                       # D2H: final particles, S_E, U0
         lz = B.log_Z(h)
         torch.cuda.synchronize()
@@ -251,6 +258,17 @@ def main():
     mut_ms = e0.elapsed_time(e1) / reps                       # k steps
     mut_launches = (B.phi4_kernel_launches() - l1) // reps
 
+    # ---- population step: resample (integer scan, ancestors) + gather, device-resident weights ----
+    B.smc_reweight(h)                                          # weights at the ESS target
+    B.smc_resample(h)
+    pe0, pe1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    pe0.record()
+    for _ in range(reps):
+        B.smc_resample(h)                                      # P3 + P4 (+ N int32 ancestors to the host)
+    pe1.record()
+    torch.cuda.synchronize()
+    pop_ms = pe0.elapsed_time(pe1) / reps
+
     # ---- reduce over ranks ----------------------------------------------------------------------
     stats = torch.tensor([ms, site_updates, e2e_ms, e2e_su, mut_ms], dtype=torch.float64, device=dev)
     if world > 1:
@@ -273,12 +291,34 @@ def main():
     work = ALU_OPS_PER_SITE_UPDATE * float(N) * V * k
     alu_peak = 148 * 128 * pk["sm_max_mhz"] * 1e6 / 1e12
     achieved = work / (mut_ms * 1e-3) / 1e12
-    roofline = {"bound": "alu", "kernel": "mutation x%d steps (%d launches)" % (k, mut_launches),
-                "achieved": achieved, "peak": alu_peak, "unit": "TFLOP/s", "frac": achieved / alu_peak,
-                "ops": "lane-ops (FMA = 1), 40 per site-update", "traffic": NCU_DRAM_BYTES.get(args.workload),
-                "peak_source": "derived: 148 SM x 128 lanes x %.0f MHz (%s clocks)"
-                % (pk["sm_max_mhz"], pk["source"]),
-                "site_updates_per_s": float(N) * V * k / (mut_ms * 1e-3), "ms": mut_ms}
+    if V <= 112:
+        roofline = {"bound": "alu", "kernel": "mutation x%d steps (%d launches)" % (k, mut_launches),
+                    "achieved": achieved, "peak": alu_peak, "unit": "TFLOP/s", "frac": achieved / alu_peak,
+                    "ops": "lane-ops (FMA = 1), 40 per site-update",
+                    "traffic": NCU_DRAM_BYTES.get(args.workload),
+                    "peak_source": "derived: 148 SM x 128 lanes x %.0f MHz (%s clocks)"
+                    % (pk["sm_max_mhz"], pk["source"]),
+                    "site_updates_per_s": float(N) * V * k / (mut_ms * 1e-3), "ms": mut_ms}
+    else:
+        # Large V: the mutation is the 3xTF32 tcgen05 proposal GEMM plus HBM-bound
+        # normals / accept kernels.  Algorithmic work = the triangular product, (V+1) flop per
+        # site-update in FP32-equivalent flop; every such flop costs three TF32 MMAs, so 1/3 is the
+        # ceiling of this fraction.  Peak: measured dense BF16 x 1/2 (nominal TF32 : BF16 ratio).
+        tf32_peak = 0.5 * pk["bf16_tflops"]
+        achieved = (V + 1) * float(N) * V * k / (mut_ms * 1e-3) / 1e12
+        roofline = {"bound": "tensor", "kernel": "mutation x%d steps (%d launches)" % (k, mut_launches),
+                    "achieved": achieved, "peak": tf32_peak, "unit": "TFLOP/s", "frac": achieved / tf32_peak,
+                    "ops": "FP32-equivalent flop of the triangular L*z, (V+1) per site-update; 3xTF32 "
+                           "issues 3 MMAs per flop (ceiling 1/3)",
+                    "traffic": NCU_DRAM_BYTES.get(args.workload),
+                    "peak_source": "%s bf16 %.0f TFLOP/s x 1/2" % (pk["source"], pk["bf16_tflops"]),
+                    "site_updates_per_s": float(N) * V * k / (mut_ms * 1e-3), "ms": mut_ms}
+    # Population step (P3 + P4): 8 bytes per site (4 read + 4 written) + 12 bytes per particle.
+    pop_bytes = 8.0 * N * V + 12.0 * N
+    population = {"bound": "hbm", "kernel": "resample + gather", "achieved": pop_bytes / (pop_ms * 1e-3) / 1e9,
+                  "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": pop_bytes / (pop_ms * 1e-3) / 1e9 / pk["hbm_gbs"],
+                  "ms": pop_ms, "state_in_l2": bool(8.0 * N * V < 126e6),
+                  "note": "includes the integer CDF scan, the ancestor search and a 4N-byte D2H copy"}
 
     cpu = None
     if not args.no_cpu_baseline:
@@ -297,7 +337,7 @@ def main():
                     "h2d_bytes_per_step": V * N * 4, "d2h_bytes_per_step": V * N * 4 + 8 * N + 8,
                     "ms_per_step": e2e_ms / args.steps},
             "gpu_launches": int(launches), "clocks": sampler.result(), "roofline": roofline,
-            "cpu_baseline": cpu}
+            "population_step": population, "cpu_baseline": cpu}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
