@@ -48,7 +48,8 @@ normals_split_kernel(float4* __restrict__ Zs, int N, int ntm, int V, uint64_t se
   const int m = blockIdx.x, q = blockIdx.y, pr = threadIdx.x;
   const int i = m * lg::TILE + pr, nkc = V >> 2;
   float z[4] = {0.f, 0.f, 0.f, 0.f};
-  if (i < N) normals4(seed, tag, t, (uint32_t)i, (uint32_t)q, z);
+  // SFU Box-Muller (philox.cuh, R2): this kernel is instruction-issue bound
+  if (i < N) normals4_fast(seed, tag, t, (uint32_t)i, (uint32_t)q, z);
   float4 hi, lo;
   hi.x = tc::tf32_rna(z[0]); lo.x = z[0] - hi.x;
   hi.y = tc::tf32_rna(z[1]); lo.y = z[1] - hi.y;
