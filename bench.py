@@ -71,11 +71,12 @@ class ClockSampler(threading.Thread):
                 "reasons": sorted(self.reasons)}
 
 
-def oracle_run(cfg, n_sample, seed):
+def oracle_run(cfg, n_sample, seed, max_temps=4096):
     """One oracle SMC run on a reduced population; returns (site_updates, seconds, T, threads)."""
     from oracle import oracle as O
     t0 = time.perf_counter()
-    r = O.smc_run(cfg["L"], cfg["m0sq"], cfg["lam"], n_sample, seed, cfg["k"], ess_target=cfg["ess"])
+    r = O.smc_run(cfg["L"], cfg["m0sq"], cfg["lam"], n_sample, seed, cfg["k"], ess_target=cfg["ess"],
+                  max_temps=max_temps)
     dt = time.perf_counter() - t0
     V = cfg["L"] ** 2
     return n_sample * V * cfg["k"] * r["T"], dt, r["T"], O.num_threads()
@@ -86,12 +87,14 @@ def run_reference(args, cfg):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    n_sample = min(cfg["N"], args.ref_particles)
+    V = cfg["L"] ** 2
+    n_sample = min(cfg["N"], args.ref_particles if V < 1024 else 256)
+    max_temps = args.max_temps if args.max_temps > 0 else (6 if V >= 1024 else 4096)
     for w in range(args.warmup):
-        oracle_run(cfg, n_sample, 1000 + w)
+        oracle_run(cfg, n_sample, 1000 + w, max_temps)
     tot_su, tot_t, Ts = 0, 0.0, []
     for s in range(args.steps):
-        su, dt, T, thr = oracle_run(cfg, n_sample, s)
+        su, dt, T, thr = oracle_run(cfg, n_sample, s, max_temps)
         tot_su += su
         tot_t += dt
         Ts.append(T)
@@ -154,11 +157,9 @@ def main():
     import torch
     import torch.distributed as dist
     from paper_2511_15196_b200 import binding as B
-    from paper_2511_15196_b200 import build
+    from paper_2511_15196_b200 import build, replicas
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    rank, world, local = replicas.rank_info()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py --impl ours needs a CUDA device (there is no CPU fallback)")
     torch.cuda.set_device(local)
@@ -196,14 +197,14 @@ def main():
 
     # ---- device-resident timing -------------------------------------------------------------
     for w in range(args.warmup):
-        device_step(1000 + w + 7919 * rank)
+        device_step(replicas.replica_seed(1000 + w, rank))
     barrier()
     sampler = ClockSampler(local)
     sampler.start()
     l0 = B.phi4_kernel_launches()
     ms, Ts = 0.0, []
     for s in range(args.steps):
-        dt, T = device_step(s + 7919 * rank)
+        dt, T = device_step(replicas.replica_seed(s, rank))
         ms += dt
         Ts.append(T)
     launches = B.phi4_kernel_launches() - l0
@@ -234,7 +235,7 @@ def main():
     e2e_ms, e2e_T = 0.0, []
     barrier()
     for s in range(args.steps):
-        dt, T, _ = e2e_step(s + 7919 * rank)
+        dt, T, _ = e2e_step(replicas.replica_seed(s, rank))
         e2e_ms += dt
         e2e_T.append(T)
     barrier()
@@ -269,15 +270,11 @@ def main():
     torch.cuda.synchronize()
     pop_ms = pe0.elapsed_time(pe1) / reps
 
-    # ---- reduce over ranks ----------------------------------------------------------------------
-    stats = torch.tensor([ms, site_updates, e2e_ms, e2e_su, mut_ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        mx = stats.clone()
-        dist.all_reduce(mx, op=dist.ReduceOp.MAX)
-        sm = stats.clone()
-        dist.all_reduce(sm, op=dist.ReduceOp.SUM)
-        ms, e2e_ms, mut_ms = mx[0].item(), mx[2].item(), mx[4].item()
-        site_updates, e2e_su = sm[1].item(), sm[3].item()
+    # ---- reduce over ranks: MAX of the times, SUM of the work (no data-path collective) ---------
+    tmax, usum = replicas.reduce_stats({"ms": ms, "e2e_ms": e2e_ms, "mut_ms": mut_ms, "pop_ms": pop_ms},
+                                       {"su": site_updates, "e2e_su": e2e_su}, device=dev)
+    ms, e2e_ms, mut_ms, pop_ms = tmax["ms"], tmax["e2e_ms"], tmax["mut_ms"], tmax["pop_ms"]
+    site_updates, e2e_su = usum["su"], usum["e2e_su"]
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -322,11 +319,18 @@ def main():
 
     cpu = None
     if not args.no_cpu_baseline:
-        n_s = min(N, args.ref_particles)
-        su, dt, T, thr = oracle_run(cfg, n_s, 0)
-        cpu = {"value": su / dt, "unit": "site-updates/s", "cores": thr, "kind": "oracle",
-               "sample": "N=%d of %d particles, one full tempering run (%d temperatures, %.1f s)"
-               % (n_s, N, T, dt)}
+        # the oracle as it stands on the host cores: full runs of the same workload until ~10 s of
+        # CPU work (large lattices: a reduced population, the per-particle work is independent)
+        n_s = min(N, args.ref_particles if V < 1024 else 256)
+        su_tot, dt_tot, runs, T, thr = 0.0, 0.0, 0, 0, 1
+        while dt_tot < 10.0 and runs < 12:
+            su, dt, T, thr = oracle_run(cfg, n_s, runs, max_temps)
+            su_tot += su
+            dt_tot += dt
+            runs += 1
+        cpu = {"value": su_tot / dt_tot, "unit": "site-updates/s", "cores": thr, "kind": "oracle",
+               "sample": "%d oracle runs of N=%d of %d particles, %d temperatures each, %.1f s of CPU time"
+               % (runs, n_s, N, T, dt_tot)}
 
     line = {"metric": "site-updates/s", "value": site_updates / (ms * 1e-3), "unit": "site-updates/s",
             "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,

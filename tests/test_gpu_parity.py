@@ -242,3 +242,61 @@ def test_observables(L, N):
     assert np.abs(obs["hist"] - ref["hist"]).sum() < 4.0 / N + 1e-12
     assert obs["hist"].sum() == pytest.approx(1.0, abs=1e-12)
     h.close()
+
+
+# ------------------------------------------------------------------ edge cases ----------------
+def test_argument_errors_on_device():
+    h = new_smc(4, 256)
+    with pytest.raises(B.Phi4Error):
+        B.smc_mutate(h, B.MAX_HOOK_STEPS + 1)              # flags wanted for more steps than the buffer
+    B.smc_mutate(h, B.MAX_HOOK_STEPS + 1, want=False)       # fine without flags
+    with pytest.raises(B.Phi4Error):
+        B.smc_set_params(h, k_steps=0)
+    with pytest.raises(B.Phi4Error):
+        B.smc_set_params(h, ess_target=1.5)
+    with pytest.raises(B.Phi4Error):
+        B.ns_step(h)                                       # SMC handle given to an NS call
+    h.close()
+    with pytest.raises(B.Phi4Error):
+        B.ns_init(4, -4.0, 1.0, 64, 64, 5, 0)              # k_delete must be < n_live
+    with pytest.raises(B.Phi4Error):
+        B.smc_init(4, -4.0, 1.0, 1, 0)                     # N >= 2
+
+
+def test_smallest_population_and_reset():
+    """A ragged single tile (N = 48) on L = 1, 2, 4 lattices; smc_reset reproduces smc_init exactly.
+    (N = 2 itself is covered by the init and resampling cases: at ESS target 0.5 = 1/N it collapses
+    onto one particle by construction.)"""
+    for L in (1, 2, 4):
+        h = new_smc(L, 48, seed=9, k=3)
+        a = B.smc_get_state(h)
+        T = B.smc_run(h, 50)
+        assert T >= 1 and np.all(np.isfinite(B.smc_get_state(h)["phi"]))
+        lz = B.log_Z(h)
+        B.smc_reset(h, 9)
+        b = B.smc_get_state(h)
+        assert np.array_equal(a["phi"], b["phi"]) and b["beta"] == 0.0 and b["step"] == 0
+        assert B.smc_run(h, 50) == T and B.log_Z(h) == lz
+        h.close()
+
+
+def test_degenerate_weights_and_collapsed_population():
+    """All mass on one particle: every ancestor is that particle; the covariance of the collapsed
+    population is singular, the jitter retry (A4) cannot rescue an all-zero matrix -> ENOTPD."""
+    h = new_smc(4, 300, seed=2)
+    w = np.zeros(300, np.float32)
+    w[123] = 1.0
+    anc = B.smc_resample(h, w)
+    assert np.all(anc == 123)
+    st = B.smc_get_state(h)
+    assert np.all(st["phi"] == st["phi"][:, :1])
+    B.estimate_cov_chol(h)
+    with pytest.raises(B.Phi4Error) as e:
+        B.smc_step(h)
+    assert e.value.code == -3
+    h.close()
+    h = new_smc(4, 64, seed=2)
+    with pytest.raises(B.Phi4Error) as e:                  # all weights quantise to zero: ENAN
+        B.smc_resample(h, np.zeros(64, np.float32))
+    assert e.value.code == -4
+    h.close()
