@@ -90,7 +90,14 @@ static int carve_smc(phi4smc* h, char* base, size_t* total) {
     h->U0[b] = c.take<float>(ld);
   }
   h->phip = c.take<float>(field);
-  h->Z = c.take<float>(propose_tc_supported(V) ? propose_tc_zsplit_floats(V, ld) : field);
+  {
+    // normal scratch: [V][ld] (generic path), or the split normals / centred-split particles of
+    // the tcgen05 paths, whichever is larger
+    size_t zf = field;
+    if (propose_tc_supported(V) && propose_tc_zsplit_floats(V, ld) > zf) zf = propose_tc_zsplit_floats(V, ld);
+    if (syrk_tc_supported(V, ld) && syrk_tc_scratch_floats(V, ld) > zf) zf = syrk_tc_scratch_floats(V, ld);
+    h->Z = c.take<float>(zf);
+  }
   h->w = c.take<float>(ld);
   h->M = c.take<float>(ld);
   h->C = c.take<unsigned long long>(ld);
@@ -99,7 +106,7 @@ static int carve_smc(phi4smc* h, char* base, size_t* total) {
   h->Sigma = c.take<float>((size_t)V * V);
   h->Lc = c.take<float>((size_t)V * V);
   h->partial = c.take<float>(cov_partial_floats(V, N));
-  h->Lsplit = c.take<float>((mutate_tc_supported(V) || propose_tc_supported(V)) ? mutate_tc_lsplit_floats(V) : 4);
+  h->Lsplit = c.take<float>(mutate_tc_supported(V) ? mutate_tc_lsplit_floats(V) : (propose_tc_supported(V) ? propose_tc_lsplit_floats(V) : 4));
   h->acc_flags = c.take<uint8_t>((size_t)PHI4_MAX_HOOK_STEPS * N);
   h->margins = c.take<float>((size_t)PHI4_MAX_HOOK_STEPS * N);
   h->ctrl = c.take<Ctrl>(1);
@@ -125,7 +132,7 @@ static int carve_ns(phi4smc* h, char* base, size_t* total) {
   h->Sigma = c.take<float>((size_t)V * V);
   h->Lc = c.take<float>((size_t)V * V);
   h->partial = c.take<float>(cov_partial_floats(V, N));
-  h->Lsplit = c.take<float>((mutate_tc_supported(V) || propose_tc_supported(V)) ? mutate_tc_lsplit_floats(V) : 4);
+  h->Lsplit = c.take<float>(mutate_tc_supported(V) ? mutate_tc_lsplit_floats(V) : (propose_tc_supported(V) ? propose_tc_lsplit_floats(V) : 4));
   h->dead = c.take<int32_t>(kd);
   h->surv = c.take<int32_t>(N);
   h->start = c.take<int32_t>(kd);

@@ -42,12 +42,14 @@ void launch_mutate_generic(const MutateArgs& a, float* Lsplit, cudaStream_t st);
 bool mutate_tc_supported(int V);
 size_t mutate_tc_lsplit_floats(int V);
 void launch_mutate_tc(const MutateArgs& a, float* Lsplit, cudaStream_t st);
-void launch_lsplit(const float* Lc, int V, float s, float* Lsplit, const Ctrl* ctrl, int respect_done,
-                   cudaStream_t st);
+void launch_lsplit(const float* Lc, int V, int Vn, int Kp, float s, float* Lsplit, const Ctrl* ctrl,
+                   int respect_done, cudaStream_t st);
 
 // propose_tc.cu -- M1 + M2 for large V: persistent 3xTF32 tcgen05 GEMM, normals in UMMA layout
 bool propose_tc_supported(int V);
 size_t propose_tc_zsplit_floats(int V, int ld);
+size_t propose_tc_lsplit_floats(int V);
+void propose_tc_dims(int V, int* Vn, int* Kp);
 void launch_normals_split(float* Zs, int N, int ld, int V, uint64_t seed, uint32_t tag, uint32_t t,
                           const Ctrl* ctrl, int respect_done, cudaStream_t st);
 void launch_propose_tc(const float* phi, float* phip, const float* Zs, const float* Lsplit, int ld,

@@ -88,11 +88,12 @@ struct TcParams {
 // of its part (hi, then lo after l_floats(V) floats).  Zero beyond V (the strict upper triangle
 // inside a block is zero in Lc itself).
 __global__ void lsplit_kernel(const float* __restrict__ Lc, int V, int Vn, int Kp, float s,
-                              float* __restrict__ out, const Ctrl* ctrl, int respect_done) {
+                              float* __restrict__ out, size_t lpart, const Ctrl* ctrl,
+                              int respect_done) {
   if (respect_done && ctrl->done) return;
-  int idx = blockIdx.x * blockDim.x + threadIdx.x;
-  if (idx >= Kp * Vn) return;
-  const int y = idx / Vn, x = idx - y * Vn;
+  const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= (size_t)Kp * Vn) return;
+  const int y = (int)(idx / Vn), x = (int)(idx - (size_t)y * Vn);
   const int ks = y >> 3, xs = tc::xs_of(ks);
   if (x < xs) return;
   float v = (x < V && y < V && y <= x) ? s * Lc[(size_t)x * V + y] : 0.f;
@@ -102,7 +103,7 @@ __global__ void lsplit_kernel(const float* __restrict__ Lc, int V, int Vn, int K
   size_t o = (size_t)tc::rows_before(ks, Vn) * 8 + (size_t)((y & 7) >> 2) * rows * 4 +
              (size_t)(x - xs) * 4 + (y & 3);
   out[o] = hi;
-  out[tc::l_floats(V) + o] = lo;
+  out[lpart + o] = lo;
 }
 
 // Per-site difference of Eq. 1 between phi' (a2; forward neighbours b2, c2) and phi (a; b, c) in
@@ -514,17 +515,18 @@ extern "C" __attribute__((visibility("default"))) int phi4_debug_tc_trace(long l
 }
 #endif
 
-void launch_lsplit(const float* Lc, int V, float s, float* Lsplit, const Ctrl* ctrl, int respect_done,
-                   cudaStream_t st) {
-  const int Vn = tc::vn_of(V), Kp = tc::kp_of(V);
+// Packed hi / lo split of s*Lc with Vn rows (>= V, multiple of 16) and Kp columns (>= V, multiple
+// of 8); the lo part starts l_floats_vk(Vn, Kp) floats after the hi part.
+void launch_lsplit(const float* Lc, int V, int Vn, int Kp, float s, float* Lsplit, const Ctrl* ctrl,
+                   int respect_done, cudaStream_t st) {
   ++g_launches;
-  lsplit_kernel<<<(unsigned)(((size_t)Kp * Vn + 255) / 256), 256, 0, st>>>(Lc, V, Vn, Kp, s, Lsplit, ctrl,
-                                                                         respect_done);
+  lsplit_kernel<<<(unsigned)(((size_t)Kp * Vn + 255) / 256), 256, 0, st>>>(
+      Lc, V, Vn, Kp, s, Lsplit, tc::l_floats_vk(Vn, Kp), ctrl, respect_done);
 }
 
 void launch_mutate_tc(const MutateArgs& a, float* Lsplit, cudaStream_t st) {
   const int V = a.md.V, Vn = tc::vn_of(V), Kp = tc::kp_of(V);
-  launch_lsplit(a.Lc, V, a.s, Lsplit, a.ctrl, a.respect_done, st);
+  launch_lsplit(a.Lc, V, Vn, Kp, a.s, Lsplit, a.ctrl, a.respect_done, st);
   TcParams p;
   p.phi = a.phi; p.S = a.S; p.U0 = a.U0; p.Lsplit = Lsplit; p.ctrl = a.ctrl;
   p.acc_out = a.acc_out; p.margin_out = a.margin_out;

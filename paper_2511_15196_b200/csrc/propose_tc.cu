@@ -1,4 +1,5 @@
-// propose_tc.cu -- M1 + M2 for large lattices (V >= 128, V % 16 == 0): the proposal product
+// propose_tc.cu -- M1 + M2 for lattices beyond the fused kernel (V > 112, any V: the packed
+// operands are zero-padded to 256 rows / 16 columns): the proposal product
 //   phi'[x][i] = phi[x][i] + sum_{y<=x} (s Lc)[x][y] z[y][i]
 // as a persistent tcgen05 GEMM in 3xTF32 split precision (BASELINE.json north_star: "the N x V x V
 // proposal product L*z ... as tcgen05/TMEM tiles in 3xTF32 split precision"; PAPER.md:53(i), :172).
@@ -42,14 +43,15 @@ constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 256;
 // z of step t for every particle, hi/lo split, tile-major interleave layout:
 // float4 index ((part * ntm + m) * nkc + q) * 128 + pr, part 0 = hi, 1 = lo.
 __global__ void __launch_bounds__(128)
-normals_split_kernel(float4* __restrict__ Zs, int N, int ntm, int V, uint64_t seed, uint32_t tag,
-                     uint32_t t, const Ctrl* ctrl, int respect_done) {
+normals_split_kernel(float4* __restrict__ Zs, int N, int ntm, int V, int Kp, uint64_t seed,
+                     uint32_t tag, uint32_t t, const Ctrl* ctrl, int respect_done) {
   if (respect_done && ctrl->done) return;
   const int m = blockIdx.x, q = blockIdx.y, pr = threadIdx.x;
-  const int i = m * lg::TILE + pr, nkc = V >> 2;
+  const int i = m * lg::TILE + pr, nkc = Kp >> 2;
   float z[4] = {0.f, 0.f, 0.f, 0.f};
-  // SFU Box-Muller (philox.cuh, R2): this kernel is instruction-issue bound
-  if (i < N) normals4_fast(seed, tag, t, (uint32_t)i, (uint32_t)q, z);
+  // SFU Box-Muller (philox.cuh, R2): this kernel is instruction-issue bound.  Quads
+  // beyond the lattice (K padding) stay zero; sites >= V inside the last quad meet zero columns.
+  if (i < N && 4 * q < V) normals4_fast(seed, tag, t, (uint32_t)i, (uint32_t)q, z);
   float4 hi, lo;
   hi.x = tc::tf32_rna(z[0]); lo.x = z[0] - hi.x;
   hi.y = tc::tf32_rna(z[1]); lo.y = z[1] - hi.y;
@@ -65,7 +67,7 @@ struct ProposeTcParams {
   const float* Zs;                   // normals_split_kernel output
   const float* Lsplit;               // packed s*Lc hi | lo (tcgen05.cuh layout)
   const Ctrl* ctrl;
-  int ld, V, ntm, ntn;
+  int ld, V, Vn, Kp, ntm, ntn;       // Vn = V rounded up to 256 rows, Kp = V rounded up to 16
   int respect_done;
 };
 
@@ -82,7 +84,7 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
   auto dempty = [&](int b) { return bar0 + 8u * (2 * STAGES + 2 + b); };
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * STAGES + 4);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int V = p.V, nkc = V >> 2, ntiles = p.ntm * p.ntn;
+  const int V = p.V, Vn = p.Vn, Kp = p.Kp, nkc = Kp >> 2, ntiles = p.ntm * p.ntn;
 
   if (warp == 8 && lane == 0) {
     for (int s = 0; s < STAGES; ++s) { mbar_init(full(s), 1); mbar_init(empty(s), 1); }
@@ -99,12 +101,12 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
   if (warp == 8) {
     // ================================ producer: bulk copies into the ring =====================
     if (lane == 0) {
-      const size_t lpart = l_floats(V);
+      const size_t lpart = l_floats_vk(Vn, Kp);
       int s = 0;
       uint32_t ph = 0;
       for (int tl = blockIdx.x; tl < ntiles; tl += gridDim.x) {
         const int m = tl / p.ntn, n0 = (tl % p.ntn) * TN;
-        const int nst = (n0 + TN) >> 4;                       // K-stages up to the tile's last row
+        const int nst = min(n0 + TN, Kp) >> 4;               // K-stages up to the tile's last row
         for (int it = 0; it < nst; ++it) {
           mbar_wait(empty(s), ph ^ 1);
           const uint32_t st = ring + (uint32_t)s * STAGE_BYTES;
@@ -127,12 +129,12 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
 #pragma unroll
           for (int kk = 0; kk < 2; ++kk) {
             const int ks = 2 * it + kk, xs = xs_of(ks);
-            const size_t blk = (size_t)rows_before(ks, V) * 8;
+            const size_t blk = (size_t)rows_before(ks, Vn) * 8;
 #pragma unroll
             for (int c = 0; c < 2; ++c)
 #pragma unroll
               for (int h = 0; h < 2; ++h) {
-                const float* src = p.Lsplit + (size_t)h * lpart + blk + (size_t)c * (V - xs) * 4 +
+                const float* src = p.Lsplit + (size_t)h * lpart + blk + (size_t)c * (Vn - xs) * 4 +
                                    (size_t)(rowstart[kk] - xs) * 4;
                 const uint32_t dst = st + 2 * A_PART + (uint32_t)h * B_PART +
                                      (uint32_t)(kk * 2 + c) * CHUNK_B +
@@ -154,7 +156,7 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
       const uint64_t b_base = smem_desc(ring + 2 * A_PART, CHUNK_B, 128);
       for (int tl = blockIdx.x; tl < ntiles; tl += gridDim.x) {
         const int n0 = (tl % p.ntn) * TN;
-        const int nst = (n0 + TN) >> 4;
+        const int nst = min(n0 + TN, Kp) >> 4;
         for (int it0 = 0; it0 < nst; it0 += SUB_STAGES, ++cnt) {
           const int buf = cnt & 1;
           mbar_wait(dempty(buf), ((cnt >> 1) & 1) ^ 1);
@@ -199,7 +201,7 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
     const uint32_t tlane = taddr + ((uint32_t)(Q * 32) << 16);
     for (int tl = blockIdx.x; tl < ntiles; tl += gridDim.x) {
       const int m = tl / p.ntn, n0 = (tl % p.ntn) * TN;
-      const int nst = (n0 + TN) >> 4;
+      const int nst = min(n0 + TN, Kp) >> 4;
       const size_t col = (size_t)m * TILE + Q * 32 + lane;
       const int x0 = n0 + hc * 128;
       if (nst <= SUB_STAGES) {
@@ -212,11 +214,13 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
           tmem_ld16(tlane + (uint32_t)(buf * TN + hc * 128 + cb), r);
           float f[16];
 #pragma unroll
-          for (int jj = 0; jj < 16; ++jj) f[jj] = p.phi[(size_t)(x0 + cb + jj) * p.ld + col];
+          for (int jj = 0; jj < 16; ++jj)
+            f[jj] = (x0 + cb + jj < V) ? p.phi[(size_t)(x0 + cb + jj) * p.ld + col] : 0.f;
           tmem_ld_wait();
 #pragma unroll
           for (int jj = 0; jj < 16; ++jj)
-            p.phip[(size_t)(x0 + cb + jj) * p.ld + col] = f[jj] + __uint_as_float(r[jj]);
+            if (x0 + cb + jj < V)
+              p.phip[(size_t)(x0 + cb + jj) * p.ld + col] = f[jj] + __uint_as_float(r[jj]);
         }
         tc_fence_before();
         __syncwarp();
@@ -246,10 +250,11 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
         for (int cb = 0; cb < 128; cb += 16) {
           float f[16];
 #pragma unroll
-          for (int jj = 0; jj < 16; ++jj) f[jj] = p.phi[(size_t)(x0 + cb + jj) * p.ld + col];
+          for (int jj = 0; jj < 16; ++jj)
+            f[jj] = (x0 + cb + jj < V) ? p.phi[(size_t)(x0 + cb + jj) * p.ld + col] : 0.f;
 #pragma unroll
           for (int jj = 0; jj < 16; ++jj)
-            p.phip[(size_t)(x0 + cb + jj) * p.ld + col] = f[jj] + acc[cb + jj];
+            if (x0 + cb + jj < V) p.phip[(size_t)(x0 + cb + jj) * p.ld + col] = f[jj] + acc[cb + jj];
         }
       }
     }
@@ -259,16 +264,26 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
   if (warp == 0) tmem_dealloc(taddr, 2 * TN);
 }
 
-bool propose_tc_supported(int V) { return V >= 256 && (V % lg::TN) == 0; }
+bool propose_tc_supported(int V) { return V > 112; }
 
-size_t propose_tc_zsplit_floats(int V, int ld) { return (size_t)2 * V * ld; }
+void propose_tc_dims(int V, int* Vn, int* Kp) {
+  *Vn = round_up(V, lg::TN);
+  *Kp = round_up(V, 16);
+}
+
+size_t propose_tc_zsplit_floats(int V, int ld) { return (size_t)2 * round_up(V, 16) * ld; }
+
+size_t propose_tc_lsplit_floats(int V) {
+  return 2 * tc::l_floats_vk(round_up(V, lg::TN), round_up(V, 16));
+}
 
 void launch_normals_split(float* Zs, int N, int ld, int V, uint64_t seed, uint32_t tag, uint32_t t,
                           const Ctrl* ctrl, int respect_done, cudaStream_t st) {
-  dim3 grid(ld / lg::TILE, V / 4);
+  const int Kp = round_up(V, 16);
+  dim3 grid(ld / lg::TILE, Kp / 4);
   ++g_launches;
-  normals_split_kernel<<<grid, 128, 0, st>>>(reinterpret_cast<float4*>(Zs), N, ld / lg::TILE, V, seed,
-                                             tag, t, ctrl, respect_done);
+  normals_split_kernel<<<grid, 128, 0, st>>>(reinterpret_cast<float4*>(Zs), N, ld / lg::TILE, V, Kp,
+                                             seed, tag, t, ctrl, respect_done);
 }
 
 void launch_propose_tc(const float* phi, float* phip, const float* Zs, const float* Lsplit, int ld,
@@ -283,7 +298,9 @@ void launch_propose_tc(const float* phi, float* phip, const float* Zs, const flo
   }
   ProposeTcParams p;
   p.phi = phi; p.phip = phip; p.Zs = Zs; p.Lsplit = Lsplit; p.ctrl = ctrl;
-  p.ld = ld; p.V = V; p.ntm = ld / lg::TILE; p.ntn = V / lg::TN; p.respect_done = respect_done;
+  p.ld = ld; p.V = V;
+  propose_tc_dims(V, &p.Vn, &p.Kp);
+  p.ntm = ld / lg::TILE; p.ntn = p.Vn / lg::TN; p.respect_done = respect_done;
   const int ntiles = p.ntm * p.ntn;
   const int grid = ntiles < num_sms ? ntiles : num_sms;
   ++g_launches;

@@ -1,4 +1,5 @@
-// syrk_tc.cu -- C1 for large lattices (V % 256 == 0): the centred particle covariance
+// syrk_tc.cu -- C1 for lattices beyond the single-CTA sizes (V > 112; operands zero-padded to
+// 256 rows and 256 particles): the centred particle covariance
 //   Sigma = (1/(N-1)) sum_i (phi_i - mu)(phi_i - mu)^T
 // as a tcgen05 GEMM in 3xTF32 split precision (BASELINE.json north_star: "the V x V covariance
 // syrk as tcgen05/TMEM tiles in 3xTF32 split precision"; readings A4, R6).
@@ -34,7 +35,7 @@ constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 256;
 
 // Block = 32 sites x 128 particles.  Pad particles (i >= N) contribute exact zeros.
 __global__ void __launch_bounds__(256)
-centre_split_kernel(const float* __restrict__ phi, int N, int ld, int V,
+centre_split_kernel(const float* __restrict__ phi, int N, int ld, int V, int Vn, int ldp,
                     const float* __restrict__ mu, float4* __restrict__ Ps, const Ctrl* ctrl,
                     int respect_done) {
   if (respect_done && ctrl->done) return;
@@ -42,11 +43,11 @@ centre_split_kernel(const float* __restrict__ phi, int N, int ld, int V,
   const int x0 = blockIdx.y * 32, i0 = blockIdx.x * 128;
   for (int e = threadIdx.x; e < 32 * 128; e += 256) {
     const int xr = e >> 7, ic = e & 127;
-    const int i = i0 + ic;
-    tile[xr][ic] = i < N ? phi[(size_t)(x0 + xr) * ld + i] - mu[x0 + xr] : 0.f;
+    const int i = i0 + ic, x = x0 + xr;
+    tile[xr][ic] = (i < N && x < V) ? phi[(size_t)x * ld + i] - mu[x] : 0.f;   // zero padding
   }
   __syncthreads();
-  const size_t part = (size_t)(ld >> 2) * V;             // float4s per hi / lo part
+  const size_t part = (size_t)(ldp >> 2) * Vn;           // float4s per hi / lo part
   for (int e = threadIdx.x; e < 32 * 32; e += 256) {
     const int kc = e >> 5, xr = e & 31;                  // lanes along x: 512 B contiguous stores
     float4 hi, lo;
@@ -56,7 +57,7 @@ centre_split_kernel(const float* __restrict__ phi, int N, int ld, int V,
     hi.y = tc::tf32_rna(v1); lo.y = v1 - hi.y;
     hi.z = tc::tf32_rna(v2); lo.z = v2 - hi.z;
     hi.w = tc::tf32_rna(v3); lo.w = v3 - hi.w;
-    const size_t o = (size_t)((i0 >> 2) + kc) * V + x0 + xr;
+    const size_t o = (size_t)((i0 >> 2) + kc) * Vn + x0 + xr;
     Ps[o] = hi;
     Ps[part + o] = lo;
   }
@@ -66,7 +67,7 @@ struct SyrkTcParams {
   const float* Ps;       // centre_split_kernel output
   float* partial;        // [nsplit][V][V]
   const Ctrl* ctrl;
-  int V, nkc, ntm, nsplit, chunks_per_split, nitems;
+  int V, Vn, nkc, ntm, nsplit, chunks_per_split, nitems;   // Vn = V rounded up to 256
   int respect_done;
 };
 
@@ -78,7 +79,8 @@ __device__ __forceinline__ void syrk_item(const SyrkTcParams& p, int item, int& 
   // enumerate tm = 0..ntm-1, tn = 0..floor((tm*128+127)/256)
   int tm = 0;
   for (;;) {
-    const int cnt = ((tm * sy::TM + sy::TM - 1) / sy::TN) + 1;
+    const int last = min(tm * sy::TM + sy::TM - 1, p.V - 1);     // last real row of this tile row
+    const int cnt = last / sy::TN + 1;
     if (t < cnt) break;
     t -= cnt;
     ++tm;
@@ -100,7 +102,7 @@ __global__ void __launch_bounds__(sy::THREADS, 1) syrk_tc_kernel(const SyrkTcPar
   auto dempty = [&](int b) { return bar0 + 8u * (2 * STAGES + 2 + b); };
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * STAGES + 4);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int V = p.V;
+  const int V = p.V, Vn = p.Vn;
 
   if (warp == 8 && lane == 0) {
     for (int s = 0; s < STAGES; ++s) { mbar_init(full(s), 1); mbar_init(empty(s), 1); }
@@ -117,7 +119,7 @@ __global__ void __launch_bounds__(sy::THREADS, 1) syrk_tc_kernel(const SyrkTcPar
 
   if (warp == 8) {
     if (lane == 0) {
-      const size_t part = (size_t)p.nkc * V * 4;           // floats per hi / lo part
+      const size_t part = (size_t)p.nkc * Vn * 4;          // floats per hi / lo part
       int s = 0;
       uint32_t ph = 0;
       for (int item = blockIdx.x; item < p.nitems; item += gridDim.x) {
@@ -130,7 +132,7 @@ __global__ void __launch_bounds__(sy::THREADS, 1) syrk_tc_kernel(const SyrkTcPar
           mbar_expect_tx(full(s), STAGE_BYTES);
 #pragma unroll
           for (int c = 0; c < 4; ++c) {
-            const size_t row = (size_t)(kc0 + 4 * it + c) * V;
+            const size_t row = (size_t)(kc0 + 4 * it + c) * Vn;
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
               const float* base = p.Ps + (size_t)h * part + row * 4;
@@ -207,10 +209,19 @@ __global__ void __launch_bounds__(sy::THREADS, 1) syrk_tc_kernel(const SyrkTcPar
         __syncwarp();
         if (lane == 0) mbar_arrive(dempty(buf));
       }
-      float* out = p.partial + (size_t)z * V * V + (size_t)(m0 + Q * 32 + lane) * V + n0 + hc * 128;
+      const int x = m0 + Q * 32 + lane, y0 = n0 + hc * 128;
+      if (x < V) {
+        float* out = p.partial + (size_t)z * V * V + (size_t)x * V + y0;
+        if ((V & 3) == 0 && y0 + 128 <= V) {
 #pragma unroll
-      for (int j = 0; j < 128; j += 4)
-        *reinterpret_cast<float4*>(out + j) = make_float4(acc[j], acc[j + 1], acc[j + 2], acc[j + 3]);
+          for (int j = 0; j < 128; j += 4)
+            *reinterpret_cast<float4*>(out + j) = make_float4(acc[j], acc[j + 1], acc[j + 2], acc[j + 3]);
+        } else {
+#pragma unroll
+          for (int j = 0; j < 128; ++j)
+            if (y0 + j < V) out[j] = acc[j];
+        }
+      }
     }
   }
   tc_fence_before();
@@ -218,26 +229,30 @@ __global__ void __launch_bounds__(sy::THREADS, 1) syrk_tc_kernel(const SyrkTcPar
   if (warp == 0) tmem_dealloc(taddr, 2 * TN);
 }
 
-bool syrk_tc_supported(int V, int ld) {
-  return V >= 256 && (V % sy::TN) == 0 && (ld % (16 * sy::SUB_STAGES)) == 0;
-}
+bool syrk_tc_supported(int V, int ld) { return V > 112 && ld >= 256; }
 
 static int syrk_tc_tiles(int V) {
   int t = 0;
-  for (int tm = 0; tm < V / sy::TM; ++tm) t += ((tm * sy::TM + sy::TM - 1) / sy::TN) + 1;
+  for (int tm = 0; tm * sy::TM < V; ++tm) {
+    int last = tm * sy::TM + sy::TM - 1;
+    if (last > V - 1) last = V - 1;
+    t += last / sy::TN + 1;
+  }
   return t;
 }
 
-// K split: enough items for ~2 waves of 148 SMs; every split is a whole number of K = 16 stages.
+// K split: enough items for ~2 waves of 148 SMs; every split is a whole number of K = 256 chains.
 int syrk_tc_nsplit(int V, int ld) {
-  const int nkc = ld >> 2, tiles = syrk_tc_tiles(V);
+  const int nkc = round_up(ld, 256) >> 2, tiles = syrk_tc_tiles(V);
   int ns = (2 * 148 + tiles - 1) / tiles;
   if (ns < 1) ns = 1;
-  while (ns > 1 && (nkc % (4 * sy::SUB_STAGES * ns)) != 0) --ns;   // whole K = 256 sub-chunks
+  while (ns > 1 && (nkc % (4 * sy::SUB_STAGES * ns)) != 0) --ns;
   return ns;
 }
 
-size_t syrk_tc_scratch_floats(int V, int ld) { return (size_t)2 * V * ld; }
+size_t syrk_tc_scratch_floats(int V, int ld) {
+  return (size_t)2 * round_up(V, sy::TN) * round_up(ld, 256);
+}
 
 void launch_syrk_tc(const float* phi, int N, int ld, int V, const float* mu, float* Ps,
                     float* partial, const Ctrl* ctrl, int respect_done, cudaStream_t st) {
@@ -249,12 +264,14 @@ void launch_syrk_tc(const float* phi, int N, int ld, int V, const float* mu, flo
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev);
   }
-  dim3 gc(ld / 128, V / 32);
+  const int Vn = round_up(V, sy::TN), ldp = round_up(ld, 256);
+  dim3 gc(ldp / 128, Vn / 32);
   ++g_launches;
-  centre_split_kernel<<<gc, 256, 0, st>>>(phi, N, ld, V, mu, reinterpret_cast<float4*>(Ps), ctrl,
-                                          respect_done);
+  centre_split_kernel<<<gc, 256, 0, st>>>(phi, N, ld, V, Vn, ldp, mu, reinterpret_cast<float4*>(Ps),
+                                          ctrl, respect_done);
   SyrkTcParams p;
-  p.Ps = Ps; p.partial = partial; p.ctrl = ctrl; p.V = V; p.nkc = ld >> 2; p.ntm = V / sy::TM;
+  p.Ps = Ps; p.partial = partial; p.ctrl = ctrl; p.V = V; p.Vn = Vn; p.nkc = ldp >> 2;
+  p.ntm = Vn / sy::TM;
   p.nsplit = syrk_tc_nsplit(V, ld);
   p.chunks_per_split = p.nkc / p.nsplit;
   p.nitems = syrk_tc_tiles(V) * p.nsplit;

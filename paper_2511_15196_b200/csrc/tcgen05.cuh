@@ -19,9 +19,11 @@ __host__ __device__ inline long long rows_before(int ks, int Vn) {
   const long long sum_half = (ks & 1) ? m * m : m * (m - 1);      // sum_{j<ks} floor(j/2)
   return (long long)ks * Vn - 16 * sum_half;
 }
-__host__ __device__ inline size_t l_floats(int V) {     // floats per hi / lo part
-  return (size_t)rows_before(kp_of(V) / 8, vn_of(V)) * 8;
+// floats per hi / lo part of the packed factor with Vn rows and Kp columns
+__host__ __device__ inline size_t l_floats_vk(int Vn, int Kp) {
+  return (size_t)rows_before(Kp / 8, Vn) * 8;
 }
+__host__ __device__ inline size_t l_floats(int V) { return l_floats_vk(vn_of(V), kp_of(V)); }
 
 
 // ------------------------------------------------------------------ PTX wrappers -------------

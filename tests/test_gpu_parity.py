@@ -58,7 +58,8 @@ def test_set_state_roundtrip_and_action_large_fields():
 
 
 # ------------------------------------------------------------------ C1 + C2 -------------------
-@pytest.mark.parametrize("L,N", [(4, 1024), (10, 16384), (10, 1000), (15, 2000), (16, 4096)])
+@pytest.mark.parametrize("L,N", [(4, 1024), (10, 16384), (10, 1000), (15, 2000), (16, 4096), (18, 5000),
+                                 (11, 700), (12, 400)])
 def test_cov_chol(L, N):
     V = L * L
     phi = inputs.smooth_fields(L, N, seed=L)
@@ -138,22 +139,22 @@ def lockstep(L, N, k, beta, seed, m0sq=-4.0, lam=1.0, path=0, fields="init", t_s
 @pytest.mark.parametrize("L,N,k,beta,fields", [
     (4, 1024, 10, 0.4, "init"), (10, 16384, 20, 0.3, "smooth"), (10, 1000, 5, 1.0, "smooth"),
     (5, 333, 8, 0.7, "smooth"), (1, 200, 6, 1.0, "init"), (2, 129, 6, 0.5, "init"),
-    (9, 640, 7, 0.6, "smooth"), (16, 2048, 4, 0.2, "smooth")])
+    (9, 640, 7, 0.6, "smooth"), (16, 2048, 4, 0.2, "smooth"), (15, 700, 3, 0.5, "smooth"),
+    (18, 1500, 3, 0.4, "smooth"), (11, 300, 4, 0.5, "smooth")])
 def test_mutation_lockstep(L, N, k, beta, fields, path):
     """Both mutation paths -- the generic per-step kernels and the fused tcgen05 kernel (3xTF32
     proposal, tile resident over the k steps) -- in lock-step with the oracle."""
-    V = L * L
-    if path == 2 and V > 112 and V % 256 != 0:
-        pytest.skip("tcgen05 paths: fused kernel for V <= 112, proposal GEMM for V % 256 == 0")
     rate = lockstep(L, N, k, beta, seed=7 + L, fields=fields, t_start=3 * k, path=path)
     assert 0.0 < rate < 1.0
 
 
-def test_fused_path_rejected_when_unsupported():
-    h = B.smc_init(15, -4.0, 1.0, 256, 0)           # V = 225: neither tcgen05 path applies
-    with pytest.raises(B.Phi4Error):
+def test_every_lattice_size_has_a_tensor_core_path():
+    """V <= 112: fused kernel; V > 112: tcgen05 proposal GEMM on zero-padded operands (the paper's
+    own sizes L = 15, 18 included)."""
+    for L in (1, 4, 10, 11, 15, 18):
+        h = B.smc_init(L, -4.0, 1.0, 256, 0)
         B.smc_set_params(h, mutation_path=2)
-    h.close()
+        h.close()
 
 
 # ------------------------------------------------------------------ P1 + P2 -------------------
