@@ -88,17 +88,19 @@ def test_smc_gaussian_L4_closed_form_and_oracle():
         assert all(abs(x["ess_frac"] - 0.9) < 1e-3 for x in r["hist"][:-1])
 
 
-@pytest.mark.parametrize("name", ["C0", "C0g"])
+@pytest.mark.parametrize("name", ["C0", "C0g", "C1"])
 def test_smc_statistical_parity_16_seeds(name):
-    """BASELINE configs[0] and its Gaussian variant: <|M|>, <M^2>, histogram and log Z of 16 GPU
-    runs vs 16 oracle runs within 3 combined standard errors."""
+    """BASELINE configs[0], its Gaussian variant and configs[1] (L=10, N=16384, k=20; also chi): <|M|>,
+    <M^2>, histogram and log Z of 16 GPU runs vs 16 oracle runs within 3 combined standard errors."""
     c = inputs.CONFIGS[name]
     g = [gpu_smc(c["L"], c["N"], s, c["k"], c["ess"], c["m0sq"], c["lam"]) for s in range(16)]
     o = [O.smc_run(c["L"], c["m0sq"], c["lam"], c["N"], s, c["k"], ess_target=c["ess"]) for s in range(16)]
     oobs = [O.observables(r["phi"], r["S"]) for r in o]
     pairs = {"logZ": ([r["logZ"] for r in g], [r["logZ"] for r in o]),
              "absM": ([r["obs"]["absM"] for r in g], [x["absM"] for x in oobs]),
-             "M2": ([r["obs"]["M2"] for r in g], [x["M2"] for x in oobs])}
+             "M2": ([r["obs"]["M2"] for r in g], [x["M2"] for x in oobs]),
+             "chi": ([r["obs"]["chi"] for r in g], [x["chi"] for x in oobs]),
+             "mean_SE": ([r["obs"]["mean_SE"] for r in g], [x["mean_SE"] for x in oobs])}
     for key, (a, b) in pairs.items():
         (ma, sa), (mb, sb) = mean_se(a), mean_se(b)
         assert abs(ma - mb) < 3 * math.hypot(sa, sb), (key, ma, sa, mb, sb)
