@@ -193,12 +193,14 @@ __device__ __forceinline__ void chol_panels(float* sm, int P, int V, int* failed
       __syncthreads();        // every thread has read the diagonal block before its rows change
       if (r < V) {
         bool bad = false;
+        float invd[CS_NB];                   // 1 / l_kk: the solves multiply instead of dividing
 #pragma unroll
         for (int k = 0; k < CS_NB; ++k) {
           float d = D[k][k];
           if (!(d > 0.f)) { bad = true; d = 1.f; }
           const float sd = sqrtf(d), inv = 1.0f / sd;
           D[k][k] = sd;
+          invd[k] = inv;
 #pragma unroll
           for (int i = k + 1; i < CS_NB; ++i) D[i][k] *= inv;
 #pragma unroll
@@ -213,7 +215,7 @@ __device__ __forceinline__ void chol_panels(float* sm, int P, int V, int* failed
           float v = x[k];
 #pragma unroll
           for (int m = 0; m < k; ++m) v = fmaf(-x[m], D[k][m], v);
-          v = v / D[k][k];
+          v = v * invd[k];
           // rows of the diagonal block take the factor itself (their solve reproduces it up to
           // rounding; use the shared value so that every thread sees the same l_ck)
           if (ri < CS_NB) {

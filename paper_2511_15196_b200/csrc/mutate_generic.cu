@@ -126,9 +126,12 @@ accept_kernel(float* __restrict__ phi, const float* __restrict__ phip, float* __
   const int i = blockIdx.x * 32 + lane;
   const int L = md.L;
   const float hm = 0.5f * md.m0sq, lam = md.lam;
+  // each warp owns a contiguous band of lattice rows: the "down" row of one iteration is the
+  // row of the next one, so it is re-read from L1 instead of DRAM
+  const int band = (L + 7) >> 3, r_lo = g * band, r_hi = min(L, r_lo + band);
   float dS = 0.f, dU = 0.f;
   if (i < N) {
-    for (int r = g; r < L; r += 8) {
+    for (int r = r_lo; r < r_hi; ++r) {
       int rn = (r + 1 == L) ? 0 : r + 1;
       size_t ro = (size_t)r * L * ld + i, rno = (size_t)rn * L * ld + i;
       float a = phi[ro], a2 = phip[ro];
@@ -176,7 +179,7 @@ accept_kernel(float* __restrict__ phi, const float* __restrict__ phip, float* __
   }
   __syncthreads();
   if (i < N && flag[lane]) {
-    for (int r = g; r < L; r += 8) {
+    for (int r = r_lo; r < r_hi; ++r) {
       size_t ro = (size_t)r * L * ld + i;
       for (int c = 0; c < L; ++c) phi[ro + (size_t)c * ld] = phip[ro + (size_t)c * ld];
     }
