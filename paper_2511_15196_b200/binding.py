@@ -319,9 +319,9 @@ def smc_reweight(h, delta=-1.0):
     return w, info.asdict()
 
 
-def smc_resample(h, w=None):
+def smc_resample(h, w=None, want=True):
     w = None if w is None else np.ascontiguousarray(w, np.float32)
-    anc = np.empty(h.N, np.int32)
+    anc = np.empty(h.N, np.int32) if want else None
     h._check(load().smc_resample(h.ptr, _np_ptr(w), _np_ptr(anc)), "smc_resample")
     return anc
 

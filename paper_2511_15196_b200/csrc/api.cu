@@ -100,7 +100,7 @@ static int carve_smc(phi4smc* h, char* base, size_t* total) {
   }
   h->w = c.take<float>(ld);
   h->M = c.take<float>(ld);
-  h->C = c.take<unsigned long long>(ld);
+  h->C = c.take<unsigned long long>(ld + 256);            // + block sums of the two-launch scan
   h->anc = c.take<int32_t>(ld);
   h->mu = c.take<float>(V);
   h->Sigma = c.take<float>((size_t)V * V);

@@ -151,6 +151,17 @@ void launch_next_delta_reweight(const float* S, int N, float ess_target, double 
 // integer scan C_i, T = C_{N-1}.  Integer addition is associative, so the result is the same
 // for every scan shape: one CTA, each thread a contiguous run, warp-shuffle scan of the run sums.
 // ---------------------------------------------------------------------------------------------
+// floor(w 2^40) for an fp32 w in [0, 1], from the bits: w = m 2^(e-150), so q = m 2^(e-110).
+// Exact (this is reading R5's quantisation; the oracle forms floor((double)w * 2^40)).
+__device__ __forceinline__ unsigned long long quantise40(float w) {
+  const uint32_t b = __float_as_uint(w);
+  const int e = (int)((b >> 23) & 0xffu);
+  if (e == 0 || (b >> 31)) return 0ull;                       // zero, subnormal (< 2^-126) or negative
+  const unsigned long long m = (unsigned long long)((b & 0x7fffffu) | 0x800000u);
+  const int sh = e - 110;
+  return sh >= 0 ? (m << sh) : (sh > -24 ? (m >> (-sh)) : 0ull);
+}
+
 __global__ void __launch_bounds__(1024)
 quantise_scan_kernel(const float* __restrict__ w, int N, unsigned long long* __restrict__ C,
                      Ctrl* ctrl) {
@@ -164,13 +175,13 @@ quantise_scan_kernel(const float* __restrict__ w, int N, unsigned long long* __r
     const float4* w4 = reinterpret_cast<const float4*>(w + lo);
     for (int i = 0; i < ipt / 4; ++i) {
       float4 v = w4[i];
-      run += (unsigned long long)((double)v.x * 1099511627776.0) +
-             (unsigned long long)((double)v.y * 1099511627776.0) +
-             (unsigned long long)((double)v.z * 1099511627776.0) +
-             (unsigned long long)((double)v.w * 1099511627776.0);
+      run += quantise40(v.x) +
+             quantise40(v.y) +
+             quantise40(v.z) +
+             quantise40(v.w);
     }
   } else {
-    for (int i = lo; i < hi; ++i) run += (unsigned long long)((double)w[i] * 1099511627776.0);
+    for (int i = lo; i < hi; ++i) run += quantise40(w[i]);
   }
   // inclusive scan of run over the block
   unsigned long long inc = run;
@@ -199,16 +210,16 @@ quantise_scan_kernel(const float* __restrict__ w, int N, unsigned long long* __r
     for (int i = 0; i < ipt / 4; ++i) {
       float4 v = w4[i];
       ulonglong2 c0, c1;
-      pre += (unsigned long long)((double)v.x * 1099511627776.0); c0.x = pre;
-      pre += (unsigned long long)((double)v.y * 1099511627776.0); c0.y = pre;
-      pre += (unsigned long long)((double)v.z * 1099511627776.0); c1.x = pre;
-      pre += (unsigned long long)((double)v.w * 1099511627776.0); c1.y = pre;
+      pre += quantise40(v.x); c0.x = pre;
+      pre += quantise40(v.y); c0.y = pre;
+      pre += quantise40(v.z); c1.x = pre;
+      pre += quantise40(v.w); c1.y = pre;
       C2[2 * i] = c0;
       C2[2 * i + 1] = c1;
     }
   } else {
     for (int i = lo; i < hi; ++i) {
-      pre += (unsigned long long)((double)w[i] * 1099511627776.0);
+      pre += quantise40(w[i]);
       C[i] = pre;
     }
   }
@@ -218,9 +229,86 @@ quantise_scan_kernel(const float* __restrict__ w, int N, unsigned long long* __r
   }
 }
 
+// Large N: two launches.  Blocks of 256 threads x 16 weights; (1) block sums, (2) every block adds
+// the sums of the blocks before it (at most 256 of them: N <= 2^20) and scans its own 4096 weights.
+constexpr int SCAN_BLOCK = 4096;
+__global__ void __launch_bounds__(256)
+scan_block_sums_kernel(const float* __restrict__ w, int N, unsigned long long* __restrict__ bsum,
+                       const Ctrl* ctrl) {
+  __shared__ unsigned long long ws[8];
+  if (ctrl->done) return;
+  const int base = blockIdx.x * SCAN_BLOCK + threadIdx.x * 16;
+  unsigned long long run = 0;
+#pragma unroll
+  for (int j = 0; j < 16; ++j) run += (base + j < N) ? quantise40(w[base + j]) : 0ull;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) run += __shfl_xor_sync(0xffffffffu, run, o);
+  if ((threadIdx.x & 31) == 0) ws[threadIdx.x >> 5] = run;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    unsigned long long t = 0;
+    for (int k = 0; k < 8; ++k) t += ws[k];
+    bsum[blockIdx.x] = t;
+  }
+}
+
+__global__ void __launch_bounds__(256)
+scan_apply_kernel(const float* __restrict__ w, int N, const unsigned long long* __restrict__ bsum,
+                  unsigned long long* __restrict__ C, Ctrl* ctrl) {
+  __shared__ unsigned long long ws[8];
+  __shared__ unsigned long long off_s;
+  if (ctrl->done) return;
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  // exclusive prefix of the block sums before this block
+  unsigned long long pre = ((int)threadIdx.x < (int)blockIdx.x) ? bsum[threadIdx.x] : 0ull;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) pre += __shfl_xor_sync(0xffffffffu, pre, o);
+  if (lane == 0) ws[wid] = pre;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    unsigned long long t = 0;
+    for (int k = 0; k < 8; ++k) t += ws[k];
+    off_s = t;
+  }
+  __syncthreads();
+  const int base = blockIdx.x * SCAN_BLOCK + threadIdx.x * 16;
+  unsigned long long q[16], run = 0;
+#pragma unroll
+  for (int j = 0; j < 16; ++j) { q[j] = (base + j < N) ? quantise40(w[base + j]) : 0ull; run += q[j]; }
+  unsigned long long inc = run;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    unsigned long long v = __shfl_up_sync(0xffffffffu, inc, o);
+    if (lane >= o) inc += v;
+  }
+  __syncthreads();
+  if (lane == 31) ws[wid] = inc;
+  __syncthreads();
+  unsigned long long wpre = 0;
+  for (int k = 0; k < wid; ++k) wpre += ws[k];
+  unsigned long long acc = off_s + wpre + inc - run;
+#pragma unroll
+  for (int j = 0; j < 16; ++j) {
+    acc += q[j];
+    if (base + j < N) C[base + j] = acc;
+  }
+  if (blockIdx.x == gridDim.x - 1 && threadIdx.x == blockDim.x - 1) {
+    ctrl->q_total = acc;
+    if (acc == 0ull) ctrl->nan_flag = 1;
+  }
+}
+
 void launch_quantise_scan(const float* w, int N, unsigned long long* C, Ctrl* ctrl,
                           cudaStream_t st) {
-  ++g_launches; quantise_scan_kernel<<<1, 1024, 0, st>>>(w, N, C, ctrl);
+  if (N <= 32768 || N > 256 * SCAN_BLOCK) {
+    ++g_launches; quantise_scan_kernel<<<1, 1024, 0, st>>>(w, N, C, ctrl);
+    return;
+  }
+  const int nb = (N + SCAN_BLOCK - 1) / SCAN_BLOCK;
+  // block sums live in the pad of C: C has ld = round_up(N,128) entries plus 256 spare (api.cu)
+  unsigned long long* sums = C + round_up(N, 128);
+  ++g_launches; scan_block_sums_kernel<<<nb, 256, 0, st>>>(w, N, sums, ctrl);
+  ++g_launches; scan_apply_kernel<<<nb, 256, 0, st>>>(w, N, sums, C, ctrl);
 }
 
 // a_j = #{i : C_i <= t_j}, t_j = floor(((j 2^32 + U) T) / (N 2^32)), clamped to N-1; U = word 0
