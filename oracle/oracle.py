@@ -76,6 +76,14 @@ def lib():
         "orc_smc_run": (C.c_int, [C.c_int, C.c_double, C.c_double, C.c_int, C.c_uint64, C.c_int,
                                   C.c_double, C.c_double, C.c_int, _dp, _dp, _dp,
                                   C.POINTER(C.c_double), vp]),
+        "orc_hmc_mutate": (None, [_dp, _dp, _dp, C.c_int, C.c_int, C.c_double, C.c_double, _dp,
+                                  C.c_double, C.c_int, C.c_double, C.c_uint64, C.c_uint32, C.c_int,
+                                  vp, vp, vp]),
+        "orc_leapfrog": (C.c_double, [_dp, _dp, C.c_int, C.c_double, C.c_double, _dp, C.c_double,
+                                      C.c_int, C.c_double]),
+        "orc_smc_hmc_run": (C.c_int, [C.c_int, C.c_double, C.c_double, C.c_int, C.c_uint64, C.c_int,
+                                      C.c_double, C.c_double, C.c_int, C.c_int, _dp, _dp, _dp,
+                                      C.POINTER(C.c_double), vp]),
         "orc_ns_select": (None, [_dp, C.c_int, C.c_int, _ip]),
         "orc_ns_run": (C.c_int, [C.c_int, C.c_double, C.c_double, C.c_int, C.c_int, C.c_int,
                                  C.c_uint64, C.c_double, C.c_double, C.c_int, _dp, _dp, _dp,
@@ -312,3 +320,34 @@ def ns_run(L, m0sq, lam, n_live, k_del, n_walk, seed, step_scale=0.0, stop_frac=
     n = it * k_del
     return {"iters": it, "logZ": logZ.value, "logX": logX.value, "phi": phi, "S": S, "U0": U0,
             "dead_S": dS[:n], "dead_M": dM[:n], "dead_logw": dW[:n], "info": info[:it]}
+
+
+# ---------------------------------------------------------------- NEXT row f1: SMC-HMC ----
+def hmc_mutate(phi, S, U0, L, m0sq, lam, var, eps, nfrog, beta, seed, t0, k, slots=None):
+    """k HMC transitions (reading A14) on copies; returns (phi, S, U0, accept[k,N], margin[k,N])."""
+    phi, S, U0 = _f64(phi).copy(), _f64(S).copy(), _f64(U0).copy()
+    V, N = phi.shape
+    if slots is not None:
+        slots = np.ascontiguousarray(slots, np.int32)
+    acc = np.zeros((k, N), np.uint8)
+    mar = np.zeros((k, N))
+    lib().orc_hmc_mutate(phi, S, U0, N, L, m0sq, lam, _f64(var), eps, nfrog, beta, seed, t0, k,
+                         _ptr(acc), _ptr(mar), _ptr(slots))
+    return phi, S, U0, acc, mar
+
+
+def leapfrog(q, p, L, m0sq, lam, var, eps, nfrog, beta):
+    """One trajectory of a single field; returns (q_new, p_new, H_new - H_old)."""
+    q, p = _f64(q).reshape(-1).copy(), _f64(p).reshape(-1).copy()
+    dH = lib().orc_leapfrog(q, p, L, m0sq, lam, _f64(var), eps, nfrog, beta)
+    return q, p, dH
+
+
+def smc_hmc_run(L, m0sq, lam, N, seed, k, ess_target=0.5, eps=0.1, nfrog=20, max_temps=4096):
+    V = L * L
+    phi, S, U0 = np.zeros((V, N)), np.zeros(N), np.zeros(N)
+    info = np.zeros((max_temps, 8))
+    logZ = C.c_double(0.0)
+    T = lib().orc_smc_hmc_run(L, m0sq, lam, N, seed, k, ess_target, eps, nfrog, max_temps, phi, S,
+                              U0, C.byref(logZ), _ptr(info))
+    return {"T": T, "logZ": logZ.value, "phi": phi, "S": S, "U0": U0, "info": info[:T]}

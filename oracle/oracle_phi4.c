@@ -676,3 +676,155 @@ int orc_ns_run(int L, double m0sq, double lam, int n, int k_del, int n_walk,
   free(surv); free(isdead); free(acc);
   return rc < 0 ? rc : it;
 }
+
+/* ------------------------------------------------------------------------
+ * NEXT row f1 -- SMC-HMC rejuvenation (PAPER.md:53(iii), :172): "short HMC
+ * trajectories", "diagonal mass matrix", "fixed trajectory of 20 leapfrog
+ * steps".  Reading A14: target U(phi) = U0 + beta S_E; mass matrix
+ * M = diag(1/var_x) with var_x the particle variance of site x (the diagonal
+ * of the covariance of reading A4); momentum p = z / sqrt(var) with z the
+ * PROP-stream normals; nfrog leapfrog steps of size eps:
+ *     p <- p - eps/2 grad U;  nfrog x { phi <- phi + eps var p;
+ *     p <- p - eps grad U (eps/2 after the last position update) };
+ * H = U + 1/2 sum var_x p_x^2; margin g = (H_old - H_new) - ln u (ACC stream),
+ * accept iff g > 0.  grad U = phi + beta grad S_E (orc_action_grad_field).
+ * Same outputs / slot keying as orc_mutate.
+ * ---------------------------------------------------------------------- */
+static void orc_grad_u(const double* f, int L, double m0sq, double lam,
+                       double beta, double* g) {
+  orc_action_grad_field(f, L, m0sq, lam, g);
+  for (int x = 0; x < L * L; ++x) g[x] = f[x] + beta * g[x];
+}
+
+void orc_hmc_mutate(double* phi, double* S, double* U0, int N, int L,
+                    double m0sq, double lam, const double* var, double eps,
+                    int nfrog, double beta, uint64_t seed, uint32_t t0, int k,
+                    uint8_t* accept_out, double* margin_out,
+                    const int32_t* slots) {
+  int V = L * L;
+#pragma omp parallel
+  {
+    double* f = (double*)malloc(sizeof(double) * V);
+    double* q = (double*)malloc(sizeof(double) * V);
+    double* p = (double*)malloc(sizeof(double) * V);
+    double* g = (double*)malloc(sizeof(double) * V);
+    double* z = (double*)malloc(sizeof(double) * V);
+#pragma omp for
+    for (int i = 0; i < N; ++i) {
+      orc_get_field(phi, N, V, i, f);
+      double Si = S[i], Ui = U0[i];
+      const uint32_t slot = slots ? (uint32_t)slots[i] : (uint32_t)i;
+      for (int j = 0; j < k; ++j) {
+        uint32_t t = t0 + (uint32_t)j;
+        orc_normals(seed, ORC_TAG_PROP, t, slot, V, z);
+        double K0 = 0.0;
+        for (int x = 0; x < V; ++x) {
+          p[x] = z[x] / sqrt(var[x]);
+          K0 += 0.5 * var[x] * p[x] * p[x];
+          q[x] = f[x];
+        }
+        orc_grad_u(q, L, m0sq, lam, beta, g);
+        for (int x = 0; x < V; ++x) p[x] -= 0.5 * eps * g[x];
+        for (int s = 0; s < nfrog; ++s) {
+          for (int x = 0; x < V; ++x) q[x] += eps * var[x] * p[x];
+          orc_grad_u(q, L, m0sq, lam, beta, g);
+          double h = (s + 1 == nfrog) ? 0.5 * eps : eps;
+          for (int x = 0; x < V; ++x) p[x] -= h * g[x];
+        }
+        double K1 = 0.0;
+        for (int x = 0; x < V; ++x) K1 += 0.5 * var[x] * p[x] * p[x];
+        double Sp = orc_action_field(q, L, m0sq, lam, NULL);
+        double Up = orc_u0_field(q, V);
+        double u = orc_uniform(seed, ORC_TAG_ACC, t, slot);
+        double gm = ((Ui + beta * Si + K0) - (Up + beta * Sp + K1)) - log(u);
+        int acc = gm > 0.0;
+        if (margin_out) margin_out[(size_t)j * N + i] = gm;
+        if (accept_out) accept_out[(size_t)j * N + i] = (uint8_t)acc;
+        if (acc) {
+          memcpy(f, q, sizeof(double) * V);
+          Si = Sp;
+          Ui = Up;
+        }
+      }
+      orc_put_field(phi, N, V, i, f);
+      S[i] = Si;
+      U0[i] = Ui;
+    }
+    free(f); free(q); free(p); free(g); free(z);
+  }
+}
+
+/* One leapfrog trajectory of a single field with given momentum (pin helper:
+ * reversibility and energy-error scaling).  q, p are updated in place;
+ * returns H_new - H_old. */
+double orc_leapfrog(double* q, double* p, int L, double m0sq, double lam,
+                    const double* var, double eps, int nfrog, double beta) {
+  int V = L * L;
+  double* g = (double*)malloc(sizeof(double) * V);
+  double H0 = orc_u0_field(q, V) + beta * orc_action_field(q, L, m0sq, lam, NULL);
+  for (int x = 0; x < V; ++x) H0 += 0.5 * var[x] * p[x] * p[x];
+  orc_grad_u(q, L, m0sq, lam, beta, g);
+  for (int x = 0; x < V; ++x) p[x] -= 0.5 * eps * g[x];
+  for (int s = 0; s < nfrog; ++s) {
+    for (int x = 0; x < V; ++x) q[x] += eps * var[x] * p[x];
+    orc_grad_u(q, L, m0sq, lam, beta, g);
+    double h = (s + 1 == nfrog) ? 0.5 * eps : eps;
+    for (int x = 0; x < V; ++x) p[x] -= h * g[x];
+  }
+  double H1 = orc_u0_field(q, V) + beta * orc_action_field(q, L, m0sq, lam, NULL);
+  for (int x = 0; x < V; ++x) H1 += 0.5 * var[x] * p[x] * p[x];
+  free(g);
+  return H1 - H0;
+}
+
+/* SMC with HMC rejuvenation: orc_smc_run with step 2(e) replaced by k HMC
+ * transitions; var = diag of the covariance of the resampled particles. */
+int orc_smc_hmc_run(int L, double m0sq, double lam, int N, uint64_t seed, int k,
+                    double ess_target, double eps, int nfrog, int max_temps,
+                    double* phi, double* S, double* U0, double* logZ_out,
+                    double* info) {
+  int V = L * L;
+  double* tmp = (double*)malloc(sizeof(double) * (size_t)V * N);
+  double* Sigma = (double*)malloc(sizeof(double) * (size_t)V * V);
+  double* mu = (double*)malloc(sizeof(double) * V);
+  double* var = (double*)malloc(sizeof(double) * V);
+  float* w = (float*)malloc(sizeof(float) * N);
+  int32_t* anc = (int32_t*)malloc(sizeof(int32_t) * N);
+  uint8_t* acc = (uint8_t*)malloc((size_t)k * N);
+  orc_init_particles(seed, N, V, phi);
+  orc_action_batch(phi, N, L, m0sq, lam, S, U0, NULL);
+  double beta = 0.0, logZ = 0.0;
+  uint32_t t = 0;
+  int T = 0;
+  while (beta < 1.0 && T < max_temps) {
+    int final;
+    double delta = orc_next_delta(S, N, beta, ess_target, &final);
+    double beta_new = final ? 1.0 : beta + delta;
+    double ess = orc_ess_frac(S, N, delta);
+    double dlz = orc_reweight(S, N, delta, w);
+    logZ += dlz;
+    uint32_t U = orc_word0(seed, ORC_TAG_RESAMPLE, (uint32_t)T, 0u);
+    orc_resample_systematic(w, N, U, anc);
+    orc_gather(phi, N, V, anc, tmp);
+    memcpy(phi, tmp, sizeof(double) * (size_t)V * N);
+    orc_gather(S, N, 1, anc, tmp);  memcpy(S, tmp, sizeof(double) * N);
+    orc_gather(U0, N, 1, anc, tmp); memcpy(U0, tmp, sizeof(double) * N);
+    orc_covariance(phi, N, V, mu, Sigma);
+    for (int x = 0; x < V; ++x) var[x] = Sigma[(size_t)x * V + x];
+    orc_hmc_mutate(phi, S, U0, N, L, m0sq, lam, var, eps, nfrog, beta_new, seed,
+                   t + 1, k, acc, NULL, NULL);
+    t += (uint32_t)k;
+    double nacc = 0.0;
+    for (size_t m = 0; m < (size_t)k * N; ++m) nacc += acc[m];
+    if (info) {
+      double* o = info + 8 * T;
+      o[0] = beta_new; o[1] = delta; o[2] = ess; o[3] = dlz;
+      o[4] = nacc / ((double)k * N); o[5] = 0; o[6] = 0; o[7] = 0.0;
+    }
+    beta = beta_new;
+    ++T;
+  }
+  *logZ_out = logZ;
+  free(tmp); free(Sigma); free(mu); free(var); free(w); free(anc); free(acc);
+  return T;
+}
