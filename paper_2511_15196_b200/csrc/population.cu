@@ -152,7 +152,7 @@ void launch_next_delta_reweight(const float* S, int N, float ess_target, double 
 // for every scan shape: one CTA, each thread a contiguous run, warp-shuffle scan of the run sums.
 // ---------------------------------------------------------------------------------------------
 // floor(w 2^40) for an fp32 w in [0, 1], from the bits: w = m 2^(e-150), so q = m 2^(e-110).
-// Exact (this is reading R5's quantisation; the oracle forms floor((double)w * 2^40)).
+// Exact (reading R5: identical to floor((double)w * 2^40)).
 __device__ __forceinline__ unsigned long long quantise40(float w) {
   const uint32_t b = __float_as_uint(w);
   const int e = (int)((b >> 23) & 0xffu);
