@@ -54,6 +54,13 @@ typedef struct {
   float ess_target; /* target ESS fraction in (0,1) for adaptive tempering        */
   float step_scale; /* s in phi' = phi + s*Lc*z; 0 selects 2.38/sqrt(V) (A3)       */
   int mutation_path; /* 0 = automatic, 1 = generic (any V), 2 = fused tcgen05 (if it supports V) */
+  /* Rejuvenation kernel: 0 = RW-Metropolis (i), 1 = HMC (iii, :172; reading A14).
+   * HMC: mass matrix diag(1/var_x) from the particle covariance, hmc_leapfrog >= 1 leapfrog steps
+   * of size hmc_eps > 0 per transition, k_steps transitions per temperature.  The HMC kernel
+   * keeps 32 particles x 3 fields in shared memory: L*L <= 512, else PHI4_EINVAL.               */
+  int kernel;
+  float hmc_eps;
+  int hmc_leapfrog;
 } smc_params;
 
 /* One tempering transition, filled when smc_step is given a non-NULL pointer. */
@@ -91,7 +98,8 @@ typedef struct {
 } phi4_observables;
 
 const char* phi4_strerror(int code);
-/* Text of the last CUDA error seen by this handle ("" if none); valid until the next call. */
+/* Text of the last CUDA error seen by this handle ("" if none); valid until the next call.
+ * h == NULL: the message of the last smc_init / ns_init that failed in this process.        */
 const char* phi4_last_cuda_error(const phi4smc* h);
 /* Diagnostic: number of CUDA kernels this library has launched in this process so far. */
 uint64_t phi4_kernel_launches(void);

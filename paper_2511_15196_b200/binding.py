@@ -27,7 +27,8 @@ class Phi4Error(RuntimeError):
 
 class smc_params(C.Structure):
     _fields_ = [("k_steps", C.c_int), ("ess_target", C.c_float), ("step_scale", C.c_float),
-                ("mutation_path", C.c_int)]
+                ("mutation_path", C.c_int), ("kernel", C.c_int), ("hmc_eps", C.c_float),
+                ("hmc_leapfrog", C.c_int)]
 
 
 class smc_step_info(C.Structure):
@@ -179,7 +180,7 @@ def smc_init(L, m0sq, lam, N, seed, device="cuda:0"):
     rc = lib.smc_init(C.byref(ptr), L, m0sq, lam, N, seed, C.c_void_p(base),
                       nbytes, _stream_ptr(device))
     if rc != 0:
-        detail = lib.phi4_last_cuda_error(ptr).decode() if ptr else ""
+        detail = lib.phi4_last_cuda_error(ptr if ptr else None).decode()
         if ptr:
             lib.smc_destroy(ptr)
         raise Phi4Error(rc, "smc_init", detail)
@@ -198,7 +199,7 @@ def ns_init(L, m0sq, lam, n_live, k_delete, n_walk, seed, stop_frac=1e-3, max_it
     rc = lib.ns_init(C.byref(ptr), L, m0sq, lam, n_live, k_delete, n_walk, seed, stop_frac,
                      max_iters, C.c_void_p(base), nbytes, _stream_ptr(device))
     if rc != 0:
-        detail = lib.phi4_last_cuda_error(ptr).decode() if ptr else ""
+        detail = lib.phi4_last_cuda_error(ptr if ptr else None).decode()
         if ptr:
             lib.smc_destroy(ptr)
         raise Phi4Error(rc, "ns_init", detail)
@@ -213,8 +214,9 @@ def smc_destroy(h):
     h.close()
 
 
-def smc_set_params(h, k_steps=10, ess_target=0.5, step_scale=0.0, mutation_path=0):
-    p = smc_params(k_steps, ess_target, step_scale, mutation_path)
+def smc_set_params(h, k_steps=10, ess_target=0.5, step_scale=0.0, mutation_path=0, kernel=0,
+                   hmc_eps=0.1, hmc_leapfrog=20):
+    p = smc_params(k_steps, ess_target, step_scale, mutation_path, kernel, hmc_eps, hmc_leapfrog)
     h._check(load().smc_set_params(h.ptr, C.byref(p)), "smc_set_params")
 
 

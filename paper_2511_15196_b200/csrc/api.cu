@@ -162,6 +162,7 @@ static phi4smc* new_handle(int kind, int L, float m0sq, float lambda, int N, uin
   h->N = N; h->ld = round_up(N, 128);
   h->seed = seed;
   h->prm.k_steps = 10; h->prm.ess_target = 0.5f; h->prm.step_scale = 0.f; h->prm.mutation_path = 0;
+  h->prm.kernel = 0; h->prm.hmc_eps = 0.1f; h->prm.hmc_leapfrog = 20;
   h->s = 2.38f / sqrtf((float)h->md.V);
   return h;
 }
@@ -180,7 +181,15 @@ PHI4_API const char* phi4_strerror(int code) {
 
 PHI4_API uint64_t phi4_kernel_launches(void) { return g_launches; }
 
-PHI4_API const char* phi4_last_cuda_error(const phi4smc* h) { return h ? h->err : ""; }
+// a failed *_init has no handle to carry its message: kept here, read with a NULL handle
+static char g_init_err[256] = "";
+static int init_failed(phi4smc* h, int rc) {
+  snprintf(g_init_err, sizeof(g_init_err), "%s", h->err);
+  delete h;
+  return rc;
+}
+
+PHI4_API const char* phi4_last_cuda_error(const phi4smc* h) { return h ? h->err : g_init_err; }
 
 PHI4_API size_t smc_workspace_bytes(int L, int N) {
   if (L < 1 || N < 2 || L > 4096) return 0;
@@ -255,7 +264,7 @@ PHI4_API int smc_init(phi4smc** out, int L, float m0sq, float lambda, int N, uin
   h->max_rec = MAX_RECORDS;
   int rc = have_device(h);
   if (rc == PHI4_OK) rc = host_staging(h);
-  if (rc != PHI4_OK) { delete h; return rc; }
+  if (rc != PHI4_OK) return init_failed(h, rc);
   size_t total;
   carve_smc(h, static_cast<char*>(d_workspace), &total);
   *out = h;
@@ -307,6 +316,10 @@ PHI4_API int smc_set_params(phi4smc* h, const smc_params* p) {
     return PHI4_EINVAL;
   if (p->mutation_path == 2 && !mutate_tc_supported(h->md.V) && !propose_tc_supported(h->md.V))
     return PHI4_EINVAL;
+  if (p->kernel < 0 || p->kernel > 1) return PHI4_EINVAL;
+  if (p->kernel == 1 && (h->kind != KIND_SMC || !hmc_supported(h->md.V) || !(p->hmc_eps > 0.f) ||
+                         p->hmc_leapfrog < 1))
+    return PHI4_EINVAL;
   h->prm = *p;
   h->s = p->step_scale > 0.f ? p->step_scale : 2.38f / sqrtf((float)h->md.V);
   return PHI4_OK;
@@ -334,6 +347,11 @@ static bool use_tc_propose(const phi4smc* h) {
 }
 
 static void enqueue_mutation(phi4smc* h, const MutateArgs& a) {
+  if (h->prm.kernel == 1 && a.mode == MODE_SMC) {
+    launch_hmc(a.phi, a.S, a.U0, h->Sigma, a.N, a.ld, a.md, h->prm.hmc_eps, h->prm.hmc_leapfrog,
+               a.seed, a.t0, a.k, a.ctrl, a.acc_out, a.margin_out, a.respect_done, h->st);
+    return;
+  }
   if (use_tc_path(h)) launch_mutate_tc(a, h->Lsplit, h->st);
   else launch_mutate_generic(a, use_tc_propose(h) ? h->Lsplit : nullptr, h->st);
 }
@@ -527,7 +545,7 @@ PHI4_API int ns_init(phi4smc** out, int L, float m0sq, float lambda, int n_live,
   h->max_iters = max_iters; h->max_rec = max_iters; h->stop_frac = stop_frac;
   int rc = have_device(h);
   if (rc == PHI4_OK) rc = host_staging(h);
-  if (rc != PHI4_OK) { delete h; return rc; }
+  if (rc != PHI4_OK) return init_failed(h, rc);
   size_t total;
   carve_ns(h, static_cast<char*>(d_workspace), &total);
   *out = h;

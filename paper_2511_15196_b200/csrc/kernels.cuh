@@ -121,6 +121,11 @@ void launch_ns_finish(const NsArgs& a, StepRecord* rec, int n_walk, cudaStream_t
 }  // namespace phi4
 
 namespace phi4 {
+// hmc.cu -- NEXT f1: k HMC transitions with mass matrix diag(1/Sigma_xx) (reading A14)
+bool hmc_supported(int V);
+void launch_hmc(float* phi, float* S, float* U0, const float* Sigma, int N, int ld, Model md,
+                float eps, int nfrog, uint64_t seed, uint32_t t0, int k, Ctrl* ctrl,
+                uint8_t* acc_out, float* margin_out, int respect_done, cudaStream_t st);
 void launch_ns_obs_inputs(const NsArgs& a, int n_dead, float* M_all, float* S_all,
                           double* logw_all, cudaStream_t st);
 }
