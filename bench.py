@@ -23,6 +23,9 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 ALU_OPS_PER_SITE_UPDATE = 40          # Philox ~20 int + Box-Muller ~6 + action ~14
+# HMC: per site per leapfrog step: neighbour sum 3, 4a-nb 1, a^2 1, lam4*a^2+m0sq 1,
+# *a 1, + 1, beta*gs+a 1, kick 1, drift 1
+ALU_OPS_PER_LEAPFROG_SITE = 11
 # dram__bytes_read.sum + dram__bytes_write.sum of one mutation launch (profiles/, ncu --set full)
 NCU_DRAM_BYTES = {"C1": 6817536}
 
@@ -75,11 +78,22 @@ def oracle_run(cfg, n_sample, seed, max_temps=4096):
     """One oracle SMC run on a reduced population; returns (site_updates, seconds, T, threads)."""
     from oracle import oracle as O
     t0 = time.perf_counter()
-    r = O.smc_run(cfg["L"], cfg["m0sq"], cfg["lam"], n_sample, seed, cfg["k"], ess_target=cfg["ess"],
-                  max_temps=max_temps)
+    if cfg.get("hmc"):
+        eps, nfrog = cfg["hmc"]
+        r = O.smc_hmc_run(cfg["L"], cfg["m0sq"], cfg["lam"], n_sample, seed, cfg["k"],
+                          ess_target=cfg["ess"], eps=eps, nfrog=nfrog, max_temps=max_temps)
+    else:
+        r = O.smc_run(cfg["L"], cfg["m0sq"], cfg["lam"], n_sample, seed, cfg["k"], ess_target=cfg["ess"],
+                      max_temps=max_temps)
     dt = time.perf_counter() - t0
     V = cfg["L"] ** 2
-    return n_sample * V * cfg["k"] * r["T"], dt, r["T"], O.num_threads()
+    return n_sample * V * cfg["k"] * units_per_step(cfg) * r["T"], dt, r["T"], O.num_threads()
+
+
+def units_per_step(cfg):
+    """Site-updates per site per mutation step: 1 for RW-Metropolis; an HMC transition updates every
+    site once per leapfrog step."""
+    return cfg["hmc"][1] if cfg.get("hmc") else 1
 
 
 def run_reference(args, cfg):
@@ -115,10 +129,13 @@ def run_reference(args, cfg):
 
 def workload_config(args, cfg, temps=None):
     c = {"workload": "%s: phi^4 L=%d (V=%d) m0sq=%g lambda=%g, N=%d particles from N(0,I), adaptive "
-                     "tempering to beta=1 at ESS %.2f, %d RW-Metropolis steps per temperature, "
-                     "systematic resampling, dense VxV covariance-Cholesky proposal"
+                     "tempering to beta=1 at ESS %.2f, %d %s per temperature, systematic resampling"
                      % (args.workload, cfg["L"], cfg["L"] ** 2, cfg["m0sq"], cfg["lam"], cfg["N"],
-                        cfg["ess"], cfg["k"]),
+                        cfg["ess"], cfg["k"],
+                        "HMC transitions (%d leapfrog steps of %g, diagonal mass matrix; a site-update "
+                        "is one site in one leapfrog step)" % (cfg["hmc"][1], cfg["hmc"][0])
+                        if cfg.get("hmc") else
+                        "RW-Metropolis steps, dense VxV covariance-Cholesky proposal"),
          "L": cfg["L"], "V": cfg["L"] ** 2, "N": cfg["N"], "k_steps": cfg["k"], "ess_target": cfg["ess"],
          "parallelism": "replicas x%d (no sharding)" % args.gpus,
          "l2": "flushed between timed steps (256 MiB write)"}
@@ -139,6 +156,11 @@ def main():
     ap.add_argument("--workload", default="C1")
     ap.add_argument("--path", type=int, default=0, help="mutation path: 0 auto, 1 generic, 2 fused")
     ap.add_argument("--ref-particles", type=int, default=16384)
+    ap.add_argument("--kernel", default="rw", choices=["rw", "hmc"],
+                    help="rejuvenation kernel: RW-Metropolis (BASELINE metric) or HMC (NEXT row f1)")
+    ap.add_argument("--k-steps", type=int, default=-1, help="override the workload's steps per temperature")
+    ap.add_argument("--hmc-eps", type=float, default=0.1)
+    ap.add_argument("--hmc-leapfrog", type=int, default=20)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--max-temps", type=int, default=-1,
                     help="temperatures per step; -1: to beta=1 (C0-C2), 6 for C3/C4 whose full schedule "
@@ -147,8 +169,13 @@ def main():
     args.warmup = max(args.warmup, 0)
 
     from paper_2511_15196_b200 import inputs
-    cfg = inputs.CONFIGS[args.workload]
-    assert cfg["kind"] == "smc", "bench.py times SMC workloads (C0, C0g, C1, C3, C4)"
+    cfg = dict(inputs.CONFIGS[args.workload])
+    assert cfg["kind"] == "smc", "bench.py times SMC workloads (C0, C0g, C1, C3, C4, P10, P15, P18)"
+    if args.kernel == "hmc":
+        cfg["hmc"] = (args.hmc_eps, args.hmc_leapfrog)
+        cfg["k"] = 2                                   # "short HMC trajectories"
+    if args.k_steps > 0:
+        cfg["k"] = args.k_steps
     if args.impl == "reference":
         run_reference(args, cfg)
         return
@@ -175,7 +202,12 @@ def main():
     L, N, k, V = cfg["L"], cfg["N"], cfg["k"], cfg["L"] ** 2
     max_temps = args.max_temps if args.max_temps > 0 else (6 if V >= 1024 else 4096)
     h = B.smc_init(L, cfg["m0sq"], cfg["lam"], N, 0, device=dev)
-    B.smc_set_params(h, k_steps=k, ess_target=cfg["ess"], mutation_path=args.path)
+    upm = units_per_step(cfg)
+    if cfg.get("hmc"):
+        B.smc_set_params(h, k_steps=k, ess_target=cfg["ess"], kernel=1, hmc_eps=cfg["hmc"][0],
+                         hmc_leapfrog=cfg["hmc"][1])
+    else:
+        B.smc_set_params(h, k_steps=k, ess_target=cfg["ess"], mutation_path=args.path)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
 
     def barrier():
@@ -211,7 +243,7 @@ def main():
     barrier()
     sampler.stop_flag = True
     sampler.join()
-    site_updates = float(N) * V * k * sum(Ts)
+    site_updates = float(N) * V * k * upm * sum(Ts)
     logZ = B.log_Z(h)
 
     # ---- end to end through the C ABI with HOST buffers ---------------------------------------
@@ -239,7 +271,7 @@ def main():
         e2e_ms += dt
         e2e_T.append(T)
     barrier()
-    e2e_su = float(N) * V * k * sum(e2e_T)
+    e2e_su = float(N) * V * k * upm * sum(e2e_T)
 
     # ---- dominant kernel: the mutation, timed alone at a mid-schedule state -------------------
     B.smc_reset(h, 4242)
@@ -288,7 +320,16 @@ def main():
     work = ALU_OPS_PER_SITE_UPDATE * float(N) * V * k
     alu_peak = 148 * 128 * pk["sm_max_mhz"] * 1e6 / 1e12
     achieved = work / (mut_ms * 1e-3) / 1e12
-    if V <= 112:
+    if cfg.get("hmc"):
+        work = ALU_OPS_PER_LEAPFROG_SITE * float(N) * V * k * upm
+        achieved = work / (mut_ms * 1e-3) / 1e12
+        roofline = {"bound": "alu", "kernel": "hmc_kernel x%d transitions (%d launches)" % (k, mut_launches),
+                    "achieved": achieved, "peak": alu_peak, "unit": "TFLOP/s", "frac": achieved / alu_peak,
+                    "ops": "lane-ops (FMA = 1), 11 per site per leapfrog step", "traffic": None,
+                    "peak_source": "derived: 148 SM x 128 lanes x %.0f MHz (%s clocks)"
+                    % (pk["sm_max_mhz"], pk["source"]),
+                    "site_updates_per_s": float(N) * V * k * upm / (mut_ms * 1e-3), "ms": mut_ms}
+    elif V <= 112:
         roofline = {"bound": "alu", "kernel": "mutation x%d steps (%d launches)" % (k, mut_launches),
                     "achieved": achieved, "peak": alu_peak, "unit": "TFLOP/s", "frac": achieved / alu_peak,
                     "ops": "lane-ops (FMA = 1), 40 per site-update",

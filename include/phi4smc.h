@@ -57,7 +57,8 @@ typedef struct {
   /* Rejuvenation kernel: 0 = RW-Metropolis (i), 1 = HMC (iii, :172; reading A14).
    * HMC: mass matrix diag(1/var_x) from the particle covariance, hmc_leapfrog >= 1 leapfrog steps
    * of size hmc_eps > 0 per transition, k_steps transitions per temperature.  The HMC kernel
-   * keeps 32 particles x 3 fields in shared memory: L*L <= 512, else PHI4_EINVAL.               */
+   * is instantiated per lattice side (three 32-particle tiles in shared memory): L <= 22, else
+   * PHI4_EINVAL.                                                                               */
   int kernel;
   float hmc_eps;
   int hmc_leapfrog;

@@ -6,175 +6,252 @@
 // normals.  One transition: half kick, nfrog x (drift phi += eps var p, kick p -= eps grad U, the
 // last kick halved), then g = (H_old - H_new) - ln u, accept iff g > 0.
 //
-// No dense contraction here: the kernel is stencil / ALU bound.  A block owns 32 particles for all
-// k transitions; phi, the trajectory position q and the momentum p live in shared memory as
-// site-major [V][32] tiles (a warp reads 32 consecutive particles of one site: conflict free),
-// eight warps split the lattice rows, two barriers per leapfrog step.  HBM traffic: phi read and
-// written once per temperature.
+// No dense contraction here (the diagonal mass matrix makes the drift elementwise): the kernel is
+// bound by the FP32 pipe.  A CTA owns 32 particles for all k transitions; lane = particle, warp w
+// owns a band of lattice rows (two by default) whose position, momentum and eps*var live in REGISTERS for the
+// whole trajectory (the lattice side is a template parameter, every index is a compile-time
+// constant).  East/west neighbours come from registers, the two halo rows from a double-buffered
+// site-major [V][32] shared-memory tile into which every band publishes its rows after each
+// drift: one barrier, ~1 LDS + 1 STS and ~11 FP32 instructions per site per leapfrog step.
+// HBM traffic: phi read and written once per temperature.
 #include "kernels.cuh"
 #include "philox.cuh"
 
 namespace phi4 {
 
 namespace hm {
-constexpr int P = 32, G = 8, THREADS = P * G;
+constexpr int P = 32;                       // particles per CTA (one per lane)
+constexpr int MAX_L = 22;                   // three [V][32] fp32 tiles must fit in 200 KB
+// Band height per lattice side (measured at L = 10 and 16: even bands of few, tall warps win --
+// fewer halo rows and barrier partners -- as long as a thread's 3 x R x LT values stay in
+// registers): the tallest even split with R * LT <= 64 sites per thread, else the least ragged.
+__host__ __device__ constexpr int rows_per_band(int LT) {
+  constexpr int tab[23] = {1, 1, 2, 3, 4, 5, 6, 7, 8, 3, 5, 4, 4, 2, 2, 3, 4, 2, 3, 3, 3, 3, 2};
+  return tab[LT];
 }
-
-__device__ __forceinline__ float hmc_grad_u(const float* q, int x, int r, int c, int L, float beta,
-                                            float m0sq, float lam4) {
-  const int cw = c == 0 ? L - 1 : c - 1, ce = c + 1 == L ? 0 : c + 1;
-  const int rn = r == 0 ? L - 1 : r - 1, rs = r + 1 == L ? 0 : r + 1;
-  const float a = q[x * hm::P];
-  const float nb = q[(r * L + ce) * hm::P] + q[(r * L + cw) * hm::P] + q[(rs * L + c) * hm::P] +
-                   q[(rn * L + c) * hm::P];
-  // grad S_E = (4 a - neighbours) + m0^2 a + 4 lambda a^3;  grad U = a + beta grad S_E
-  const float gs = fmaf(4.0f, a, -nb) + a * fmaf(lam4, a * a, m0sq);
-  return fmaf(beta, gs, a);
+__host__ __device__ constexpr int bands(int LT) {
+  return (LT + rows_per_band(LT) - 1) / rows_per_band(LT);
 }
+}  // namespace hm
 
-__global__ void __launch_bounds__(hm::THREADS)
-hmc_kernel(float* __restrict__ phi, float* __restrict__ S, float* __restrict__ U0,
-           const float* __restrict__ Sigma, int N, int ld, Model md, float eps, int nfrog,
-           uint64_t seed, uint32_t t0, int k, Ctrl* ctrl, uint8_t* __restrict__ acc_out,
-           float* __restrict__ margin_out, int respect_done) {
-  using namespace hm;
-  extern __shared__ __align__(16) float sm[];
-  if (respect_done && ctrl->done) return;
-  const int V = md.V, L = md.L;
-  float4* red = reinterpret_cast<float4*>(sm);   // [G][32] partial (K0, K1, S', U0')
-  float* cur = sm + 4 * G * P;     // [V][32] current particles
-  float* q = cur + V * P;          // trajectory position
-  float* p = q + V * P;            // momentum
-  float* var = p + V * P;          // [V]
-  float* isd = var + V;            // [V] 1/sqrt(var)
-  __shared__ int flag[P];
-  const int lane = threadIdx.x & 31, g = threadIdx.x >> 5;
-  const int i = blockIdx.x * P + lane;
-  const bool live = i < N;
-  const float beta = (float)ctrl->beta, m0sq = md.m0sq, lam = md.lam, lam4 = 4.0f * md.lam;
-  const int nq = (V + 3) >> 2;
+struct HmcArgs {
+  float* phi; float* S; float* U0; const float* Sigma;
+  int N, ld; Model md; float eps; int nfrog;
+  uint64_t seed; uint32_t t0; int k; Ctrl* ctrl;
+  uint8_t* acc_out; float* margin_out; int respect_done;
+};
 
-  for (int x = threadIdx.x; x < V; x += THREADS) {
-    const float v = Sigma[(size_t)x * V + x];
-    var[x] = v;
-    isd[x] = rsqrtf(v);
-  }
-  for (int x = g; x < V; x += G) cur[x * P + lane] = live ? phi[(size_t)x * ld + i] : 0.f;
-  float Si = live ? S[i] : 0.f, Ui = live ? U0[i] : 0.f;
-  unsigned nacc = 0;
-  __syncthreads();
-  const float* cq = q + lane;
-  for (int j = 0; j < k; ++j) {
-    const uint32_t t = t0 + (uint32_t)j;
-    // momentum refresh (quads q ~ g) and q <- cur (rows ~ g)
-    float K0 = 0.f;
-    for (int qd = g; qd < nq; qd += G) {
-      float z[4] = {0.f, 0.f, 0.f, 0.f};
-      if (live) normals4(seed, TAG_PROP, t, (uint32_t)i, (uint32_t)qd, z);
+// bands of different height run different instantiations of the same barrier sequence
+__device__ __forceinline__ void cta_sync() { asm volatile("bar.sync 0;" ::: "memory"); }
+
+// p -= h * grad U on a band of NR rows.  hn / hs: this lane's column of the halo rows north of
+// the band's first row and south of its last row (stride P per site).
+template <int LT, int NR, int R>
+__device__ __forceinline__ void hmc_kick(const float (&q)[R * LT], float (&p)[R * LT],
+                                         const float* hn, const float* hs, float h, float beta,
+                                         float m0sq, float lam4) {
 #pragma unroll
-      for (int e = 0; e < 4; ++e) {
-        const int x = 4 * qd + e;
-        if (x < V) {
-          p[x * P + lane] = z[e] * isd[x];
-          K0 = fmaf(0.5f * z[e], z[e], K0);
-        }
-      }
+  for (int jr = 0; jr < NR; ++jr)
+#pragma unroll
+    for (int c = 0; c < LT; ++c) {
+      const int j = jr * LT + c;
+      const float a = q[j];
+      const float e = q[jr * LT + (c + 1) % LT], w = q[jr * LT + (c + LT - 1) % LT];
+      const float n = jr == 0 ? hn[c * hm::P] : q[jr == 0 ? j : j - LT];
+      const float s = jr == NR - 1 ? hs[c * hm::P] : q[jr == NR - 1 ? j : j + LT];
+      // grad S_E = (4 a - neighbours) + m0^2 a + 4 lambda a^3;  grad U = a + beta grad S_E
+      const float gs = fmaf(4.0f, a, -((e + w) + (n + s))) + a * fmaf(lam4, a * a, m0sq);
+      p[j] = fmaf(-h, fmaf(beta, gs, a), p[j]);
     }
-    for (int x = g; x < V; x += G) q[x * P + lane] = cur[x * P + lane];
-    __syncthreads();
-    // half kick
-    for (int r = g; r < L; r += G)
-      for (int c = 0; c < L; ++c) {
-        const int x = r * L + c;
-        p[x * P + lane] -= 0.5f * eps * hmc_grad_u(cq, x, r, c, L, beta, m0sq, lam4);
-      }
-    for (int s = 0; s < nfrog; ++s) {
-      // other warps may still be reading this warp's rows of q in their kick
-      __syncthreads();
-      // drift on this warp's rows (only its own p), then everyone needs the new q
-      for (int r = g; r < L; r += G)
-        for (int c = 0; c < L; ++c) {
-          const int x = r * L + c;
-          q[x * P + lane] = fmaf(eps * var[x], p[x * P + lane], q[x * P + lane]);
-        }
-      __syncthreads();
-      const float h = (s + 1 == nfrog) ? 0.5f * eps : eps;
-      for (int r = g; r < L; r += G)
-        for (int c = 0; c < L; ++c) {
-          const int x = r * L + c;
-          p[x * P + lane] -= h * hmc_grad_u(cq, x, r, c, L, beta, m0sq, lam4);
-        }
+}
+
+template <int LT, int NR>
+__device__ __forceinline__ void hmc_band(const HmcArgs& A, float* cur, float* hal0, float* hal1,
+                                         const float* var_s, const float* isd_s, float4* red,
+                                         int* flag) {
+  using namespace hm;
+  constexpr int V = LT * LT, NB = bands(LT), R = rows_per_band(LT), NS = NR * LT;
+  constexpr int nq = (V + 3) >> 2;
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const int i = blockIdx.x * P + lane;
+  const bool live = i < A.N;
+  const int r0 = w * R, x0 = r0 * LT;
+  const int rn = (r0 + LT - 1) % LT, rs = (r0 + NR) % LT;       // halo rows
+  const float beta = (float)A.ctrl->beta, m0sq = A.md.m0sq, lam = A.md.lam, lam4 = 4.0f * A.md.lam;
+  const float eps = A.eps;
+  float q[R * LT], p[R * LT], ev[R * LT];
+#pragma unroll
+  for (int j = 0; j < NS; ++j) ev[j] = eps * var_s[x0 + j];
+  float Si = live ? A.S[i] : 0.f, Ui = live ? A.U0[i] : 0.f;
+  unsigned nacc = 0;
+  float* const own0 = hal0 + x0 * P + lane;
+  float* const own1 = hal1 + x0 * P + lane;
+  float* const ownc = cur + x0 * P + lane;
+#pragma unroll
+  for (int j = 0; j < NS; ++j) q[j] = live ? A.phi[(size_t)(x0 + j) * A.ld + i] : 0.f;
+#pragma unroll
+  for (int j = 0; j < NS; ++j) ownc[j * P] = q[j];
+
+  for (int jt = 0; jt < A.k; ++jt) {
+    const uint32_t t = A.t0 + (uint32_t)jt;
+    // momentum normals by quad (shared evenly between the bands), staged in hal1
+    for (int qd = w; qd < nq; qd += NB) {
+      float z[4] = {0.f, 0.f, 0.f, 0.f};
+      if (live) normals4(A.seed, TAG_PROP, t, (uint32_t)i, (uint32_t)qd, z);
+#pragma unroll
+      for (int e = 0; e < 4; ++e)
+        if (4 * qd + e < V) hal1[(4 * qd + e) * P + lane] = z[e];
     }
-    // H_new: kinetic, S_E (Eq. 1, forward neighbours), U0 over this warp's rows
+#pragma unroll
+    for (int j = 0; j < NS; ++j) {
+      q[j] = ownc[j * P];
+      own0[j * P] = q[j];
+    }
+    cta_sync();
+    float K0 = 0.f;
+#pragma unroll
+    for (int j = 0; j < NS; ++j) {
+      const float z = own1[j * P];
+      p[j] = z * isd_s[x0 + j];
+      K0 = fmaf(0.5f * z, z, K0);
+    }
+    hmc_kick<LT, NR, R>(q, p, hal0 + rn * LT * P + lane, hal0 + rs * LT * P + lane, 0.5f * eps, beta,
+                     m0sq, lam4);
+    cta_sync();                       // hal1 (the staged normals) is free from here on
+    for (int s = 0; s < A.nfrog; ++s) {
+      float* const own = (s & 1) ? own0 : own1;
+      const float* const hb = (s & 1) ? hal0 : hal1;
+#pragma unroll
+      for (int j = 0; j < NS; ++j) {
+        q[j] = fmaf(ev[j], p[j], q[j]);
+        own[j * P] = q[j];
+      }
+      cta_sync();
+      hmc_kick<LT, NR, R>(q, p, hb + rn * LT * P + lane, hb + rs * LT * P + lane,
+                       (s + 1 == A.nfrog) ? 0.5f * eps : eps, beta, m0sq, lam4);
+    }
+    // H_new: kinetic, S_E (Eq. 1, forward neighbours), U0 over this band
+    const float* const hs = (((A.nfrog - 1) & 1) ? hal0 : hal1) + rs * LT * P + lane;
     float K1 = 0.f, Sp = 0.f, Up = 0.f;
-    for (int r = g; r < L; r += G) {
-      const int rs = r + 1 == L ? 0 : r + 1;
-      float rowS = 0.f, rowU = 0.f, rowK = 0.f;
-      for (int c = 0; c < L; ++c) {
-        const int x = r * L + c, ce = c + 1 == L ? 0 : c + 1;
-        const float a = cq[x * P], b = cq[(r * L + ce) * P], d = cq[(rs * L + c) * P];
-        const float e1 = b - a, e2 = d - a, a2 = a * a, pp = p[x * P + lane];
+#pragma unroll
+    for (int jr = 0; jr < NR; ++jr) {
+      float rowS = 0.f;
+#pragma unroll
+      for (int c = 0; c < LT; ++c) {
+        const int j = jr * LT + c;
+        const float a = q[j], b = q[jr * LT + (c + 1) % LT];
+        const float d = jr == NR - 1 ? hs[c * P] : q[jr == NR - 1 ? j : j + LT];
+        const float e1 = b - a, e2 = d - a, a2 = a * a;
         rowS += 0.5f * (e1 * e1 + e2 * e2) + a2 * (0.5f * m0sq + lam * a2);
-        rowU = fmaf(0.5f, a2, rowU);
-        rowK = fmaf(0.5f * var[x] * pp, pp, rowK);
+        Up = fmaf(0.5f, a2, Up);
+        K1 = fmaf(0.5f * ev[j] * p[j], p[j], K1);
       }
-      Sp += rowS; Up += rowU; K1 += rowK;
+      Sp += rowS;
     }
-    red[g * P + lane] = make_float4(K0, K1, Sp, Up);
-    __syncthreads();
-    if (g == 0) {
+    red[w * P + lane] = make_float4(K0, K1 / eps, Sp, Up);       // ev = eps * var
+    cta_sync();
+    if (w == 0) {
       float4 tot = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
-      for (int m = 0; m < G; ++m) {
+      for (int m = 0; m < NB; ++m) {
         const float4 v = red[m * P + lane];
         tot.x += v.x; tot.y += v.y; tot.z += v.z; tot.w += v.w;
       }
       int acc = 0;
       if (live) {
-        const float lu = log_uniform(seed, TAG_ACC, t, (uint32_t)i);
+        const float lu = log_uniform(A.seed, TAG_ACC, t, (uint32_t)i);
         // (H_old - H_new) - ln u with the differences taken term by term
         const float margin = ((Ui - tot.w) + beta * (Si - tot.z) + (tot.x - tot.y)) - lu;
         acc = margin > 0.f;
         if (acc) { Si = tot.z; Ui = tot.w; ++nacc; }
-        if (acc_out) acc_out[(size_t)j * N + i] = (uint8_t)acc;
-        if (margin_out) margin_out[(size_t)j * N + i] = margin;
+        if (A.acc_out) A.acc_out[(size_t)jt * A.N + i] = (uint8_t)acc;
+        if (A.margin_out) A.margin_out[(size_t)jt * A.N + i] = margin;
       }
       flag[lane] = acc;
     }
-    __syncthreads();
-    if (flag[lane])
-      for (int x = g; x < V; x += G) cur[x * P + lane] = q[x * P + lane];
-    __syncthreads();
+    cta_sync();
+    if (flag[lane]) {
+#pragma unroll
+      for (int j = 0; j < NS; ++j) ownc[j * P] = q[j];
+    }
+    // the next transition's staging writes hal1 / own0, which every warp finished reading before
+    // the barrier above; flag[] is rewritten only two barriers further on
   }
   if (live) {
-    for (int x = g; x < V; x += G) phi[(size_t)x * ld + i] = cur[x * P + lane];
-    if (g == 0) { S[i] = Si; U0[i] = Ui; }
+#pragma unroll
+    for (int j = 0; j < NS; ++j) A.phi[(size_t)(x0 + j) * A.ld + i] = ownc[j * P];
+    if (w == 0) { A.S[i] = Si; A.U0[i] = Ui; }
   }
-  if (g == 0) {
+  if (w == 0) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) nacc += __shfl_xor_sync(0xffffffffu, nacc, o);
-    if (lane == 0 && nacc) atomicAdd(&ctrl->n_accept, nacc);
+    if (lane == 0 && nacc) atomicAdd(&A.ctrl->n_accept, nacc);
   }
 }
 
-static size_t hmc_smem_bytes(int V) {
-  return ((size_t)3 * V * hm::P + 2 * V) * sizeof(float) + (size_t)hm::G * hm::P * sizeof(float4);
+template <int LT>
+__global__ void __launch_bounds__(32 * hm::bands(LT)) hmc_kernel(const HmcArgs A) {
+  using namespace hm;
+  constexpr int V = LT * LT, NB = bands(LT), R = rows_per_band(LT);
+  extern __shared__ __align__(16) float sm[];
+  __shared__ int flag[P];
+  if (A.respect_done && A.ctrl->done) return;
+  float4* red = reinterpret_cast<float4*>(sm);   // [NB][32] partial (K0, K1, S', U0')
+  float* cur = sm + 4 * NB * P;                  // [V][32] current particles
+  float* hal0 = cur + V * P;                     // [V][32] published positions, double-buffered
+  float* hal1 = hal0 + V * P;
+  float* var_s = hal1 + V * P;                   // [V]
+  float* isd_s = var_s + V;                      // [V] 1/sqrt(var)
+  const int w = threadIdx.x >> 5;
+  for (int x = threadIdx.x; x < V; x += 32 * NB) {
+    const float v = A.Sigma[(size_t)x * V + x];
+    var_s[x] = v;
+    isd_s[x] = rsqrtf(v);
+  }
+  cta_sync();
+  constexpr int LAST = LT - (NB - 1) * R;        // height of the last band
+  if (LAST != R && w == NB - 1)
+    hmc_band<LT, LAST>(A, cur, hal0, hal1, var_s, isd_s, red, flag);
+  else
+    hmc_band<LT, R>(A, cur, hal0, hal1, var_s, isd_s, red, flag);
 }
 
-bool hmc_supported(int V) { return hmc_smem_bytes(V) <= 200 * 1024; }
+static size_t hmc_smem_bytes(int L) {
+  const int V = L * L;
+  return ((size_t)3 * V * hm::P + 2 * V) * sizeof(float) +
+         (size_t)hm::bands(L) * hm::P * sizeof(float4);
+}
+
+bool hmc_supported(int V) {
+  int L = 1;
+  while (L * L < V) ++L;
+  return L * L == V && L <= hm::MAX_L;
+}
+
+template <int LT>
+static void launch_hmc_lt(const HmcArgs& a, cudaStream_t st) {
+  static bool attr_done = false;
+  if (!attr_done) {
+    cudaFuncSetAttribute(hmc_kernel<LT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                         (int)hmc_smem_bytes(LT));
+    attr_done = true;
+  }
+  hmc_kernel<LT><<<(a.N + hm::P - 1) / hm::P, 32 * hm::bands(LT), hmc_smem_bytes(LT), st>>>(a);
+}
+
+template <int LT>
+static void dispatch_hmc(const HmcArgs& a, cudaStream_t st) {
+  if (a.md.L == LT) launch_hmc_lt<LT>(a, st);
+  else if constexpr (LT > 1) dispatch_hmc<LT - 1>(a, st);
+}
 
 void launch_hmc(float* phi, float* S, float* U0, const float* Sigma, int N, int ld, Model md,
                 float eps, int nfrog, uint64_t seed, uint32_t t0, int k, Ctrl* ctrl,
                 uint8_t* acc_out, float* margin_out, int respect_done, cudaStream_t st) {
-  static bool attr_done = false;
-  if (!attr_done) {
-    cudaFuncSetAttribute(hmc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-    attr_done = true;
-  }
+  HmcArgs a{phi, S, U0, Sigma, N, ld, md, eps, nfrog, seed, t0, k, ctrl, acc_out, margin_out,
+            respect_done};
   ++g_launches;
-  hmc_kernel<<<(N + hm::P - 1) / hm::P, hm::THREADS, hmc_smem_bytes(md.V), st>>>(
-      phi, S, U0, Sigma, N, ld, md, eps, nfrog, seed, t0, k, ctrl, acc_out, margin_out,
-      respect_done);
+  dispatch_hmc<hm::MAX_L>(a, st);
 }
 
 }  // namespace phi4

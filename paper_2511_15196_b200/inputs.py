@@ -15,6 +15,11 @@ CONFIGS = {
                stop_frac=1e-3),
     "C3": dict(kind="smc", L=32, N=65536, k=20, m0sq=-4.0, lam=1.0, ess=0.5),
     "C4": dict(kind="smc", L=64, N=131072, k=10, m0sq=-4.0, lam=1.0, ess=0.5),
+    # paper-scale settings (N = 5000, n_MCMC = 3V, ESS target 0.9; L in {10,15,18}
+    # of :208, :236-242) -- a second workload whose wall-clock can be set beside Tables 1-3
+    "P10": dict(kind="smc", L=10, N=5000, k=300, m0sq=-4.0, lam=1.0, ess=0.9),
+    "P15": dict(kind="smc", L=15, N=5000, k=675, m0sq=-4.0, lam=1.0, ess=0.9),
+    "P18": dict(kind="smc", L=18, N=5000, k=972, m0sq=-4.0, lam=1.0, ess=0.9),
 }
 
 
