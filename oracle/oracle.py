@@ -84,6 +84,10 @@ def lib():
         "orc_smc_hmc_run": (C.c_int, [C.c_int, C.c_double, C.c_double, C.c_int, C.c_uint64, C.c_int,
                                       C.c_double, C.c_double, C.c_int, C.c_int, _dp, _dp, _dp,
                                       C.POINTER(C.c_double), vp]),
+        "orc_irmh_mutate": (None, [_dp, _dp, _dp, C.c_int, C.c_int, C.c_double, C.c_double, _dp, _dp,
+                                   C.c_double, C.c_uint64, C.c_uint32, C.c_int, vp, vp, vp]),
+        "orc_smc_irmh_run": (C.c_int, [C.c_int, C.c_double, C.c_double, C.c_int, C.c_uint64, C.c_int,
+                                       C.c_double, C.c_int, _dp, _dp, _dp, C.POINTER(C.c_double), vp]),
         "orc_ns_select": (None, [_dp, C.c_int, C.c_int, _ip]),
         "orc_ns_run": (C.c_int, [C.c_int, C.c_double, C.c_double, C.c_int, C.c_int, C.c_int,
                                  C.c_uint64, C.c_double, C.c_double, C.c_int, _dp, _dp, _dp,
@@ -350,4 +354,30 @@ def smc_hmc_run(L, m0sq, lam, N, seed, k, ess_target=0.5, eps=0.1, nfrog=20, max
     logZ = C.c_double(0.0)
     T = lib().orc_smc_hmc_run(L, m0sq, lam, N, seed, k, ess_target, eps, nfrog, max_temps, phi, S,
                               U0, C.byref(logZ), _ptr(info))
+    return {"T": T, "logZ": logZ.value, "phi": phi, "S": S, "U0": U0, "info": info[:T]}
+
+
+def irmh_mutate(phi, S, U0, L, m0sq, lam, mu, Lc, beta, seed, t0, k, slots=None):
+    """k independent-MH steps from N(mu, Lc Lc^T) (reading A15) on copies; returns
+    (phi, S, U0, accept[k,N], margin[k,N])."""
+    phi, S, U0 = _f64(phi).copy(), _f64(S).copy(), _f64(U0).copy()
+    V, N = phi.shape
+    if slots is not None:
+        slots = np.ascontiguousarray(slots, np.int32)
+    acc = np.zeros((k, N), np.uint8)
+    mar = np.zeros((k, N))
+    lib().orc_irmh_mutate(phi, S, U0, N, L, m0sq, lam, _f64(mu), _f64(Lc), beta, seed, t0, k,
+                          _ptr(acc), _ptr(mar), _ptr(slots))
+    return phi, S, U0, acc, mar
+
+
+def smc_irmh_run(L, m0sq, lam, N, seed, k, ess_target=0.5, max_temps=4096):
+    V = L * L
+    phi, S, U0 = np.zeros((V, N)), np.zeros(N), np.zeros(N)
+    info = np.zeros((max_temps, 8))
+    logZ = C.c_double(0.0)
+    T = lib().orc_smc_irmh_run(L, m0sq, lam, N, seed, k, ess_target, max_temps, phi, S, U0,
+                               C.byref(logZ), _ptr(info))
+    if T < 0:
+        raise RuntimeError("oracle SMC-IRMH: covariance not positive definite")
     return {"T": T, "logZ": logZ.value, "phi": phi, "S": S, "U0": U0, "info": info[:T]}

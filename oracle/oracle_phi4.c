@@ -828,3 +828,122 @@ int orc_smc_hmc_run(int L, double m0sq, double lam, int N, uint64_t seed, int k,
   free(tmp); free(Sigma); free(mu); free(var); free(w); free(anc); free(acc);
   return T;
 }
+
+/* ------------------------------------------------------------------------
+ * NEXT row f2 -- SMC-IRMH rejuvenation (PAPER.md:53(ii): "independent
+ * Metropolis-Hastings, with a Gaussian proposal fitted to the particles";
+ * :200).  Reading A15: proposal q = N(mu, Sigma) with mu, Sigma
+ * the particle mean and covariance of reading A4, Sigma = Lc Lc^T;
+ *     phi' = mu + Lc z,  z = PROP-stream normals (same keying as orc_mutate);
+ *     log q(phi) = -1/2 |Lc^-1 (phi - mu)|^2 + const,  log q(phi') = -1/2 |z|^2 + const;
+ *     g = -[(U0' - U0) + beta (S' - S)] + 1/2 |z|^2 - 1/2 |w|^2 - ln u,
+ *     w = Lc^-1 (phi - mu) of the CURRENT state (forward substitution; after an
+ *     accepted move w = z), u from the ACC stream; accept iff g > 0.
+ * Same outputs / slot keying as orc_mutate.
+ * ---------------------------------------------------------------------- */
+void orc_irmh_mutate(double* phi, double* S, double* U0, int N, int L,
+                     double m0sq, double lam, const double* mu,
+                     const double* Lc, double beta, uint64_t seed, uint32_t t0,
+                     int k, uint8_t* accept_out, double* margin_out,
+                     const int32_t* slots) {
+  int V = L * L;
+#pragma omp parallel
+  {
+    double* f = (double*)malloc(sizeof(double) * V);
+    double* fp = (double*)malloc(sizeof(double) * V);
+    double* z = (double*)malloc(sizeof(double) * V);
+    double* w = (double*)malloc(sizeof(double) * V);
+#pragma omp for
+    for (int i = 0; i < N; ++i) {
+      orc_get_field(phi, N, V, i, f);
+      double Si = S[i], Ui = U0[i];
+      const uint32_t slot = slots ? (uint32_t)slots[i] : (uint32_t)i;
+      /* w = Lc^-1 (f - mu) */
+      double W2 = 0.0;
+      for (int x = 0; x < V; ++x) {
+        double a = f[x] - mu[x];
+        for (int y = 0; y < x; ++y) a -= Lc[(size_t)x * V + y] * w[y];
+        w[x] = a / Lc[(size_t)x * V + x];
+        W2 += w[x] * w[x];
+      }
+      for (int j = 0; j < k; ++j) {
+        uint32_t t = t0 + (uint32_t)j;
+        orc_normals(seed, ORC_TAG_PROP, t, slot, V, z);
+        double Z2 = 0.0;
+        for (int x = 0; x < V; ++x) {
+          double a = mu[x];
+          for (int y = 0; y <= x; ++y) a += Lc[(size_t)x * V + y] * z[y];
+          fp[x] = a;
+          Z2 += z[x] * z[x];
+        }
+        double Sp = orc_action_field(fp, L, m0sq, lam, NULL);
+        double Up = orc_u0_field(fp, V);
+        double u = orc_uniform(seed, ORC_TAG_ACC, t, slot);
+        double gm = -((Up - Ui) + beta * (Sp - Si)) + 0.5 * Z2 - 0.5 * W2 - log(u);
+        int acc = gm > 0.0;
+        if (margin_out) margin_out[(size_t)j * N + i] = gm;
+        if (accept_out) accept_out[(size_t)j * N + i] = (uint8_t)acc;
+        if (acc) {
+          memcpy(f, fp, sizeof(double) * V);
+          Si = Sp; Ui = Up; W2 = Z2;
+        }
+      }
+      orc_put_field(phi, N, V, i, f);
+      S[i] = Si;
+      U0[i] = Ui;
+    }
+    free(f); free(fp); free(z); free(w);
+  }
+}
+
+/* SMC with IRMH rejuvenation: orc_smc_run with step 2(e) replaced by k IRMH
+ * steps from N(mu, Sigma) of the resampled particles (A4 jitter rule). */
+int orc_smc_irmh_run(int L, double m0sq, double lam, int N, uint64_t seed, int k,
+                     double ess_target, int max_temps, double* phi, double* S,
+                     double* U0, double* logZ_out, double* info) {
+  int V = L * L;
+  double* tmp = (double*)malloc(sizeof(double) * (size_t)V * N);
+  double* Sigma = (double*)malloc(sizeof(double) * (size_t)V * V);
+  double* Lc = (double*)malloc(sizeof(double) * (size_t)V * V);
+  double* mu = (double*)malloc(sizeof(double) * V);
+  float* w = (float*)malloc(sizeof(float) * N);
+  int32_t* anc = (int32_t*)malloc(sizeof(int32_t) * N);
+  uint8_t* acc = (uint8_t*)malloc((size_t)k * N);
+  orc_init_particles(seed, N, V, phi);
+  orc_action_batch(phi, N, L, m0sq, lam, S, U0, NULL);
+  double beta = 0.0, logZ = 0.0;
+  uint32_t t = 0;
+  int T = 0, rc = 0;
+  while (beta < 1.0 && T < max_temps) {
+    int final;
+    double delta = orc_next_delta(S, N, beta, ess_target, &final);
+    double beta_new = final ? 1.0 : beta + delta;
+    double ess = orc_ess_frac(S, N, delta);
+    double dlz = orc_reweight(S, N, delta, w);
+    logZ += dlz;
+    uint32_t U = orc_word0(seed, ORC_TAG_RESAMPLE, (uint32_t)T, 0u);
+    orc_resample_systematic(w, N, U, anc);
+    orc_gather(phi, N, V, anc, tmp);
+    memcpy(phi, tmp, sizeof(double) * (size_t)V * N);
+    orc_gather(S, N, 1, anc, tmp);  memcpy(S, tmp, sizeof(double) * N);
+    orc_gather(U0, N, 1, anc, tmp); memcpy(U0, tmp, sizeof(double) * N);
+    orc_covariance(phi, N, V, mu, Sigma);
+    int st = orc_cov_chol(phi, N, V, Sigma, Lc);
+    if (st < 0) { rc = -1; break; }
+    orc_irmh_mutate(phi, S, U0, N, L, m0sq, lam, mu, Lc, beta_new, seed, t + 1, k,
+                    acc, NULL, NULL);
+    t += (uint32_t)k;
+    double nacc = 0.0;
+    for (size_t m = 0; m < (size_t)k * N; ++m) nacc += acc[m];
+    if (info) {
+      double* o = info + 8 * T;
+      o[0] = beta_new; o[1] = delta; o[2] = ess; o[3] = dlz;
+      o[4] = nacc / ((double)k * N); o[5] = 0; o[6] = st; o[7] = 0.0;
+    }
+    beta = beta_new;
+    ++T;
+  }
+  *logZ_out = logZ;
+  free(tmp); free(Sigma); free(Lc); free(mu); free(w); free(anc); free(acc);
+  return rc < 0 ? rc : T;
+}
