@@ -78,7 +78,10 @@ def oracle_run(cfg, n_sample, seed, max_temps=4096):
     """One oracle SMC run on a reduced population; returns (site_updates, seconds, T, threads)."""
     from oracle import oracle as O
     t0 = time.perf_counter()
-    if cfg.get("hmc"):
+    if cfg.get("irmh"):
+        r = O.smc_irmh_run(cfg["L"], cfg["m0sq"], cfg["lam"], n_sample, seed, cfg["k"],
+                           ess_target=cfg["ess"], max_temps=max_temps)
+    elif cfg.get("hmc"):
         eps, nfrog = cfg["hmc"]
         r = O.smc_hmc_run(cfg["L"], cfg["m0sq"], cfg["lam"], n_sample, seed, cfg["k"],
                           ess_target=cfg["ess"], eps=eps, nfrog=nfrog, max_temps=max_temps)
@@ -135,6 +138,7 @@ def workload_config(args, cfg, temps=None):
                         "HMC transitions (%d leapfrog steps of %g, diagonal mass matrix; a site-update "
                         "is one site in one leapfrog step)" % (cfg["hmc"][1], cfg["hmc"][0])
                         if cfg.get("hmc") else
+                        "independent-MH steps from the fitted Gaussian N(mu, Sigma)" if cfg.get("irmh") else
                         "RW-Metropolis steps, dense VxV covariance-Cholesky proposal"),
          "L": cfg["L"], "V": cfg["L"] ** 2, "N": cfg["N"], "k_steps": cfg["k"], "ess_target": cfg["ess"],
          "parallelism": "replicas x%d (no sharding)" % args.gpus,
@@ -156,8 +160,9 @@ def main():
     ap.add_argument("--workload", default="C1")
     ap.add_argument("--path", type=int, default=0, help="mutation path: 0 auto, 1 generic, 2 fused")
     ap.add_argument("--ref-particles", type=int, default=16384)
-    ap.add_argument("--kernel", default="rw", choices=["rw", "hmc"],
-                    help="rejuvenation kernel: RW-Metropolis (BASELINE metric) or HMC (NEXT row f1)")
+    ap.add_argument("--kernel", default="rw", choices=["rw", "hmc", "irmh"],
+                    help="rejuvenation kernel: RW-Metropolis (BASELINE metric), HMC (NEXT row f1) or "
+                         "independent MH (NEXT row f2)")
     ap.add_argument("--k-steps", type=int, default=-1, help="override the workload's steps per temperature")
     ap.add_argument("--hmc-eps", type=float, default=0.1)
     ap.add_argument("--hmc-leapfrog", type=int, default=20)
@@ -174,6 +179,8 @@ def main():
     if args.kernel == "hmc":
         cfg["hmc"] = (args.hmc_eps, args.hmc_leapfrog)
         cfg["k"] = 2                                   # "short HMC trajectories"
+    if args.kernel == "irmh":
+        cfg["irmh"] = True
     if args.k_steps > 0:
         cfg["k"] = args.k_steps
     if args.impl == "reference":
@@ -206,6 +213,8 @@ def main():
     if cfg.get("hmc"):
         B.smc_set_params(h, k_steps=k, ess_target=cfg["ess"], kernel=1, hmc_eps=cfg["hmc"][0],
                          hmc_leapfrog=cfg["hmc"][1])
+    elif cfg.get("irmh"):
+        B.smc_set_params(h, k_steps=k, ess_target=cfg["ess"], kernel=2)
     else:
         B.smc_set_params(h, k_steps=k, ess_target=cfg["ess"], mutation_path=args.path)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)

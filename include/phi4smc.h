@@ -54,7 +54,8 @@ typedef struct {
   float ess_target; /* target ESS fraction in (0,1) for adaptive tempering        */
   float step_scale; /* s in phi' = phi + s*Lc*z; 0 selects 2.38/sqrt(V) (A3)       */
   int mutation_path; /* 0 = automatic, 1 = generic (any V), 2 = fused tcgen05 (if it supports V) */
-  /* Rejuvenation kernel: 0 = RW-Metropolis (i), 1 = HMC (iii, :172; reading A14).
+  /* Rejuvenation kernel: 0 = RW-Metropolis (i), 1 = HMC (iii, :172; reading A14),
+   * 2 = independent MH from the fitted Gaussian N(mu, Sigma) (ii, :200; reading A15; L*L <= 800).
    * HMC: mass matrix diag(1/var_x) from the particle covariance, hmc_leapfrog >= 1 leapfrog steps
    * of size hmc_eps > 0 per transition, k_steps transitions per temperature.  The HMC kernel
    * is instantiated per lattice side (three 32-particle tiles in shared memory): L <= 22, else
@@ -176,6 +177,7 @@ int smc_set_state(phi4smc* h, const float* h_phi, double beta, uint64_t step_cou
 int smc_get_chol(phi4smc* h, float* h_Lc /* V*V row-major, strict upper = 0 */);
 int smc_set_chol(phi4smc* h, const float* h_Lc);
 int smc_get_cov(phi4smc* h, float* h_Sigma /* V*V row-major */);
+int smc_get_mean(phi4smc* h, float* h_mu /* V: particle mean of the last covariance estimate */);
 /* M1-M4 only: k mutation steps at the current beta and Lc; step counters continue from the
  * handle's counter.  h_accept[j*N+i] in {0,1}, h_margin[j*N+i] = g of reading R4 as the kernel
  * computed it (fp32).  k <= PHI4_MAX_HOOK_STEPS when either array is wanted.                     */

@@ -87,6 +87,7 @@ SIGNATURES = {
     "smc_get_chol": (_i, [_vp, _vp]),
     "smc_set_chol": (_i, [_vp, _vp]),
     "smc_get_cov": (_i, [_vp, _vp]),
+    "smc_get_mean": (_i, [_vp, _vp]),
     "smc_mutate": (_i, [_vp, _i, _vp, _vp]),
     "smc_reweight": (_i, [_vp, _d, _vp, C.POINTER(smc_step_info)]),
     "smc_resample": (_i, [_vp, _vp, _vp]),
@@ -305,6 +306,12 @@ def smc_get_cov(h):
     Sig = np.empty((h.V, h.V), np.float32)
     h._check(load().smc_get_cov(h.ptr, _np_ptr(Sig)), "smc_get_cov")
     return Sig
+
+
+def smc_get_mean(h):
+    mu = np.zeros(h.V, np.float32)
+    h._check(load().smc_get_mean(h.ptr, _np_ptr(mu)), "smc_get_mean")
+    return mu
 
 
 def smc_mutate(h, k, want=True):

@@ -45,7 +45,7 @@ struct phi4smc {
   // device state (inside the workspace)
   float* phi[2]; float* S[2]; float* U0[2];
   int cur;
-  float *phip, *Z, *w, *mu, *Sigma, *Lc, *Lsplit, *partial, *M, *margins;
+  float *phip, *Z, *w, *W2, *mu, *Sigma, *Lc, *Lsplit, *partial, *M, *margins;
   unsigned long long* C;
   int32_t* anc;
   uint8_t* acc_flags;
@@ -99,6 +99,7 @@ static int carve_smc(phi4smc* h, char* base, size_t* total) {
     h->Z = c.take<float>(zf);
   }
   h->w = c.take<float>(ld);
+  h->W2 = c.take<float>(ld);                               // IRMH: |Lc^-1 (phi - mu)|^2
   h->M = c.take<float>(ld);
   h->C = c.take<unsigned long long>(ld + 256);            // + block sums of the two-launch scan
   h->anc = c.take<int32_t>(ld);
@@ -316,7 +317,8 @@ PHI4_API int smc_set_params(phi4smc* h, const smc_params* p) {
     return PHI4_EINVAL;
   if (p->mutation_path == 2 && !mutate_tc_supported(h->md.V) && !propose_tc_supported(h->md.V))
     return PHI4_EINVAL;
-  if (p->kernel < 0 || p->kernel > 1) return PHI4_EINVAL;
+  if (p->kernel < 0 || p->kernel > 2) return PHI4_EINVAL;
+  if (p->kernel == 2 && (h->kind != KIND_SMC || !irmh_supported(h->md.V))) return PHI4_EINVAL;
   if (p->kernel == 1 && (h->kind != KIND_SMC || !hmc_supported(h->md.V) || !(p->hmc_eps > 0.f) ||
                          p->hmc_leapfrog < 1))
     return PHI4_EINVAL;
@@ -350,6 +352,10 @@ static void enqueue_mutation(phi4smc* h, const MutateArgs& a) {
   if (h->prm.kernel == 1 && a.mode == MODE_SMC) {
     launch_hmc(a.phi, a.S, a.U0, h->Sigma, a.N, a.ld, a.md, h->prm.hmc_eps, h->prm.hmc_leapfrog,
                a.seed, a.t0, a.k, a.ctrl, a.acc_out, a.margin_out, a.respect_done, h->st);
+    return;
+  }
+  if (h->prm.kernel == 2 && a.mode == MODE_SMC) {
+    launch_mutate_irmh(a, h->mu, h->W2, h->st);
     return;
   }
   if (use_tc_path(h)) launch_mutate_tc(a, h->Lsplit, h->st);
@@ -694,6 +700,13 @@ PHI4_API int smc_get_cov(phi4smc* h, float* h_Sigma) {
   if (!h || !h_Sigma) return PHI4_EINVAL;
   CU(cudaStreamSynchronize(h->st));
   CU(cudaMemcpy(h_Sigma, h->Sigma, sizeof(float) * h->md.V * h->md.V, cudaMemcpyDeviceToHost));
+  return PHI4_OK;
+}
+
+PHI4_API int smc_get_mean(phi4smc* h, float* h_mu) {
+  if (!h || !h_mu) return PHI4_EINVAL;
+  CU(cudaStreamSynchronize(h->st));
+  CU(cudaMemcpy(h_mu, h->mu, sizeof(float) * h->md.V, cudaMemcpyDeviceToHost));
   return PHI4_OK;
 }
 

@@ -13,7 +13,7 @@ enum : uint32_t {
   TAG_INIT = 0, TAG_PROP = 1, TAG_ACC = 2, TAG_RESAMPLE = 3,
   TAG_NS_START = 4, TAG_NS_PROP = 5, TAG_NS_ACC = 6
 };
-enum : int { MODE_SMC = 0, MODE_NS = 1 };
+enum : int { MODE_SMC = 0, MODE_NS = 1, MODE_IRMH = 2 };
 
 // Device-resident control block: everything a temperature / NS iteration decides lives here so
 // that a step can be enqueued without a host round trip.

@@ -37,6 +37,9 @@ struct MutateArgs {
   int respect_done;  // 1: every kernel is a no-op once ctrl->done is set
 };
 void launch_mutate_generic(const MutateArgs& a, float* Lsplit, cudaStream_t st);
+// NEXT f2: k independent-MH steps from N(mu, Lc Lc^T) (reading A15); W2 [ld] scratch
+bool irmh_supported(int V);
+void launch_mutate_irmh(const MutateArgs& a, const float* mu, float* W2, cudaStream_t st);
 
 // mutate_tc.cu -- M1-M4 fused over k steps on tcgen05 (3xTF32), phi tile resident on-chip
 bool mutate_tc_supported(int V);

@@ -24,12 +24,12 @@ __global__ void normals_kernel(float* __restrict__ Z, int N, int ld, int V, uint
   }
 }
 
-// C[x][i] = phi[x][i] + s * sum_y Lc[x][y] Z[y][i].  64x64 tile, BK=16, 4x4 per thread.  Lc is
+// C[x][i] = phi[x][i] (or mu[x]) + s * sum_y Lc[x][y] Z[y][i].  64x64 tile, BK=16, 4x4 per thread.  Lc is
 // lower-triangular, so the y loop of a tile ends at its last row.
 __global__ void __launch_bounds__(256)
 propose_kernel(const float* __restrict__ Lc, const float* __restrict__ Z,
                const float* __restrict__ phi, float* __restrict__ phip, int V, int ld, float s,
-               const Ctrl* ctrl, int respect_done) {
+               const float* __restrict__ mu, const Ctrl* ctrl, int respect_done) {
   if (respect_done && ctrl->done) return;
   __shared__ float As[16][64 + 4];
   __shared__ __align__(16) float Bs[16][64];
@@ -89,7 +89,9 @@ propose_kernel(const float* __restrict__ Lc, const float* __restrict__ Z,
     int x = x0 + ty * 4 + p;
     if (x < V) {
       size_t o = (size_t)x * ld + i0 + tx * 4;
-      float4 f = *reinterpret_cast<const float4*>(phi + o);
+      // independent proposal (IRMH): the base point is the particle mean, not the particle
+      float4 f = mu ? make_float4(mu[x], mu[x], mu[x], mu[x])
+                    : *reinterpret_cast<const float4*>(phi + o);
       f.x = fmaf(s, acc[p][0], f.x);
       f.y = fmaf(s, acc[p][1], f.y);
       f.z = fmaf(s, acc[p][2], f.z);
@@ -118,9 +120,10 @@ __global__ void __launch_bounds__(256)
 accept_kernel(float* __restrict__ phi, const float* __restrict__ phip, float* __restrict__ S,
               float* __restrict__ U0, int N, int ld, Model md, int mode, uint64_t seed,
               uint32_t tag_acc, uint32_t t, Ctrl* ctrl, uint8_t* __restrict__ acc_out,
-              float* __restrict__ margin_out, int respect_done) {
+              float* __restrict__ margin_out, int respect_done, const float* __restrict__ Z,
+              float* __restrict__ W2) {
   if (respect_done && ctrl->done) return;
-  __shared__ float ps[8][32], pu[8][32];
+  __shared__ float ps[8][32], pu[8][32], pz[8][32];
   __shared__ int flag[32];
   const int lane = threadIdx.x & 31, g = threadIdx.x >> 5;
   const int i = blockIdx.x * 32 + lane;
@@ -129,8 +132,14 @@ accept_kernel(float* __restrict__ phi, const float* __restrict__ phip, float* __
   // each warp owns a contiguous band of lattice rows: the "down" row of one iteration is the
   // row of the next one, so it is re-read from L1 instead of DRAM
   const int band = (L + 7) >> 3, r_lo = g * band, r_hi = min(L, r_lo + band);
-  float dS = 0.f, dU = 0.f;
+  float dS = 0.f, dU = 0.f, z2 = 0.f;
   if (i < N) {
+    if (mode == MODE_IRMH) {          // |z|^2 of this band: log q(phi') = -1/2 |z|^2 + const
+      for (int x = r_lo * L; x < r_hi * L; ++x) {
+        const float z = Z[(size_t)x * ld + i];
+        z2 = fmaf(z, z, z2);
+      }
+    }
     for (int r = r_lo; r < r_hi; ++r) {
       int rn = (r + 1 == L) ? 0 : r + 1;
       size_t ro = (size_t)r * L * ld + i, rno = (size_t)rn * L * ld + i;
@@ -150,6 +159,7 @@ accept_kernel(float* __restrict__ phi, const float* __restrict__ phip, float* __
   }
   ps[g][lane] = dS;
   pu[g][lane] = dU;
+  pz[g][lane] = z2;
   __syncthreads();
   if (g == 0) {
     int acc = 0;
@@ -162,6 +172,14 @@ accept_kernel(float* __restrict__ phi, const float* __restrict__ phip, float* __
       if (mode == MODE_SMC) {
         margin = -(tU + (float)ctrl->beta * tS) - lu;
         acc = margin > 0.f;
+      } else if (mode == MODE_IRMH) {
+        float tZ = 0.f;
+#pragma unroll
+        for (int m = 0; m < 8; ++m) tZ += pz[m][lane];
+        // log q(phi) - log q(phi') = 1/2 |z|^2 - 1/2 |w|^2, w = Lc^-1 (phi - mu) (reading A15)
+        margin = -(tU + (float)ctrl->beta * tS) + 0.5f * (tZ - W2[i]) - lu;
+        acc = margin > 0.f;
+        if (acc) W2[i] = tZ;
       } else {
         margin = -tU - lu;
         acc = (margin > 0.f) && (Si + tS < (float)ctrl->S_star);
@@ -205,13 +223,65 @@ void launch_mutate_generic(const MutateArgs& a, float* Lsplit, cudaStream_t st) 
     } else {
       ++g_launches; normals_kernel<<<gz, 128, 0, st>>>(a.Z, a.N, a.ld, V, a.seed, a.tag_prop, t, a.ctrl,
                                          a.respect_done);
-      ++g_launches; propose_kernel<<<gp, 256, 0, st>>>(a.Lc, a.Z, a.phi, a.phip, V, a.ld, a.s, a.ctrl,
-                                         a.respect_done);
+      ++g_launches; propose_kernel<<<gp, 256, 0, st>>>(a.Lc, a.Z, a.phi, a.phip, V, a.ld, a.s, nullptr,
+                                         a.ctrl, a.respect_done);
     }
     ++g_launches; accept_kernel<<<a.ld / 32, 256, 0, st>>>(
         a.phi, a.phip, a.S, a.U0, a.N, a.ld, a.md, a.mode, a.seed, a.tag_acc, t, a.ctrl,
         a.acc_out ? a.acc_out + (size_t)j * a.N : nullptr,
-        a.margin_out ? a.margin_out + (size_t)j * a.N : nullptr, a.respect_done);
+        a.margin_out ? a.margin_out + (size_t)j * a.N : nullptr, a.respect_done, nullptr, nullptr);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// NEXT row f2: independent Metropolis-Hastings from the fitted Gaussian N(mu, Lc Lc^T)
+// (PAPER.md:53(ii), :200; reading A15).  whiten_kernel: W2[i] = |Lc^-1 (phi_i - mu)|^2 by forward
+// substitution, one warp per 32 particles, w in shared memory; FP64 accumulation (once per
+// temperature: the solve amplifies rounding by cond(Lc), and W2 enters every margin).
+__global__ void __launch_bounds__(32)
+whiten_kernel(const float* __restrict__ phi, const float* __restrict__ mu,
+              const float* __restrict__ Lc, float* __restrict__ W2, int N, int ld, int V,
+              const Ctrl* ctrl, int respect_done) {
+  if (respect_done && ctrl->done) return;
+  extern __shared__ double wsm[];          // [V][32]
+  const int lane = threadIdx.x, i = blockIdx.x * 32 + lane;
+  if (i >= N) return;
+  double w2 = 0.0;
+  for (int x = 0; x < V; ++x) {
+    const float* row = Lc + (size_t)x * V;
+    double a = (double)phi[(size_t)x * ld + i] - (double)mu[x];
+    for (int y = 0; y < x; ++y) a -= (double)row[y] * wsm[y * 32 + lane];
+    a /= (double)row[x];
+    wsm[x * 32 + lane] = a;
+    w2 += a * a;
+  }
+  W2[i] = (float)w2;
+}
+
+bool irmh_supported(int V) { return (size_t)V * 32 * sizeof(double) <= 200 * 1024; }
+
+void launch_mutate_irmh(const MutateArgs& a, const float* mu, float* W2, cudaStream_t st) {
+  const int V = a.md.V;
+  static bool attr_done = false;
+  if (!attr_done) {
+    cudaFuncSetAttribute(whiten_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    attr_done = true;
+  }
+  ++g_launches;
+  whiten_kernel<<<(a.N + 31) / 32, 32, (size_t)V * 32 * sizeof(double), st>>>(
+      a.phi, mu, a.Lc, W2, a.N, a.ld, V, a.ctrl, a.respect_done);
+  dim3 gz((a.ld + 127) / 128, (V + 3) / 4);
+  dim3 gp(a.ld / 64, (V + 63) / 64);
+  for (int j = 0; j < a.k; ++j) {
+    uint32_t t = a.t0 + (uint32_t)j;
+    ++g_launches; normals_kernel<<<gz, 128, 0, st>>>(a.Z, a.N, a.ld, V, a.seed, a.tag_prop, t, a.ctrl,
+                                       a.respect_done);
+    ++g_launches; propose_kernel<<<gp, 256, 0, st>>>(a.Lc, a.Z, a.phi, a.phip, V, a.ld, 1.0f, mu,
+                                       a.ctrl, a.respect_done);
+    ++g_launches; accept_kernel<<<a.ld / 32, 256, 0, st>>>(
+        a.phi, a.phip, a.S, a.U0, a.N, a.ld, a.md, MODE_IRMH, a.seed, a.tag_acc, t, a.ctrl,
+        a.acc_out ? a.acc_out + (size_t)j * a.N : nullptr,
+        a.margin_out ? a.margin_out + (size_t)j * a.N : nullptr, a.respect_done, a.Z, W2);
   }
 }
 
