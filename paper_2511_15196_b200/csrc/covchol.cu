@@ -48,8 +48,10 @@ __device__ __forceinline__ void nt_tile(const float* __restrict__ A, size_t lda,
 #pragma unroll
     for (int r = 0; r < 4; ++r) { tot[p][r] = acc[p][r]; acc[p][r] = 0.f; }
   int since = 0;
-  for (int k0 = kb; k0 < ke; k0 += 16) {
-    float va[4], vb[4];
+  // the global loads of slab k0 + 16 are issued before the FMAs of slab k0 (register double
+  // buffer): their latency hides behind the 256 FMAs per thread instead of stalling every slab
+  float va[4], vb[4];
+  auto load_slab = [&](int k0) {
     if (VEC) {
       float4 a4 = make_float4(0.f, 0.f, 0.f, 0.f), b4 = a4;
       if (xr < M) a4 = *reinterpret_cast<const float4*>(A + (size_t)xr * lda + k0 + lk);
@@ -64,6 +66,9 @@ __device__ __forceinline__ void nt_tile(const float* __restrict__ A, size_t lda,
         vb[j] = (yr < M && k < ke) ? A[(size_t)yr * lda + k] : 0.f;
       }
     }
+  };
+  if (kb < ke) load_slab(kb);
+  for (int k0 = kb; k0 < ke; k0 += 16) {
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
       int k = k0 + lk + j;
@@ -72,11 +77,12 @@ __device__ __forceinline__ void nt_tile(const float* __restrict__ A, size_t lda,
       Bs[lk + j][lr] = (ok && yr < M) ? vb[j] - my : 0.f;
     }
     __syncthreads();
+    if (k0 + 16 < ke) load_slab(k0 + 16);
 #pragma unroll
     for (int kk = 0; kk < 16; ++kk) {
-      float a[4], b[4];
-#pragma unroll
-      for (int j = 0; j < 4; ++j) { a[j] = As[kk][ty * 4 + j]; b[j] = Bs[kk][tx * 4 + j]; }
+      const float4 a4 = *reinterpret_cast<const float4*>(&As[kk][ty * 4]);
+      const float4 b4 = *reinterpret_cast<const float4*>(&Bs[kk][tx * 4]);
+      const float a[4] = {a4.x, a4.y, a4.z, a4.w}, b[4] = {b4.x, b4.y, b4.z, b4.w};
 #pragma unroll
       for (int p = 0; p < 4; ++p)
 #pragma unroll
@@ -111,7 +117,7 @@ syrk_partial_kernel(const float* __restrict__ phi, int N, int ld, int V,
                     const float* __restrict__ mu, float* __restrict__ partial, int chunk,
                     const Ctrl* ctrl, int respect_done) {
   if (respect_done && ctrl->done) return;
-  __shared__ float As[16][68], Bs[16][68];
+  __shared__ __align__(16) float As[16][68], Bs[16][68];
   int tr, tc;
   tri_tile(blockIdx.x, tr, tc);
   const int x0 = tr * 64, y0 = tc * 64;
@@ -133,16 +139,22 @@ syrk_partial_kernel(const float* __restrict__ phi, int N, int ld, int V,
     }
 }
 
-// Sigma[x][y] = Sigma[y][x] = (sum_z partial[z][x][y]) / (N-1) for y <= x, fixed summation order.
+// Sigma[x][y] = Sigma[y][x] = (sum_z partial[z][x][y]) / (N-1) for y <= x, fixed summation order:
+// eight lanes per entry each sum every eighth split, then a fixed shuffle tree.
 __global__ void syrk_reduce_kernel(const float* __restrict__ partial, int nsplit, int V, int N,
                                    float* __restrict__ Sigma, const Ctrl* ctrl, int respect_done) {
   if (respect_done && ctrl->done) return;
-  int idx = blockIdx.x * blockDim.x + threadIdx.x;
-  if (idx >= V * V) return;
-  int x = idx / V, y = idx - x * V;
-  if (y > x) return;
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  const int idx = t >> 3, part = t & 7;
+  const bool in = idx < V * V;
+  const int x = in ? idx / V : 0, y = in ? idx - x * V : 1;
   float a = 0.f;
-  for (int z = 0; z < nsplit; ++z) a += partial[(size_t)z * V * V + idx];
+  if (in && y <= x)
+    for (int z = part; z < nsplit; z += 8) a += partial[(size_t)z * V * V + idx];
+  a += __shfl_xor_sync(0xffffffffu, a, 1);
+  a += __shfl_xor_sync(0xffffffffu, a, 2);
+  a += __shfl_xor_sync(0xffffffffu, a, 4);
+  if (!in || y > x || part) return;
   a /= (float)(N - 1);
   Sigma[(size_t)x * V + y] = a;
   Sigma[(size_t)y * V + x] = a;
@@ -171,6 +183,10 @@ __device__ __forceinline__ bool chol_skip(const Ctrl* ctrl, int attempt, int res
 // update to the trailing lower triangle.  Three barriers per panel instead of two per column.
 // Both attempts of reading A4 (plain, then jitter 1e-6 tr/V) run inside this one launch.
 constexpr int CS_NB = 8;
+#ifndef PHI4_CS_THREADS
+#define PHI4_CS_THREADS 1024
+#endif
+constexpr int CS_THREADS = PHI4_CS_THREADS;
 // In-place lower Cholesky of the n x n matrix in shared memory (row stride P), 8-column panels:
 // every row thread re-factorises the 8x8 diagonal block in registers and solves its own row,
 // then the whole block applies the rank-8 update to the trailing lower triangle.  *failed_s is
@@ -198,7 +214,11 @@ __device__ __forceinline__ void chol_panels(float* sm, int P, int V, int* failed
         for (int k = 0; k < CS_NB; ++k) {
           float d = D[k][k];
           if (!(d > 0.f)) { bad = true; d = 1.f; }
-          const float sd = sqrtf(d), inv = 1.0f / sd;
+          // 1/sqrt(d) from the SFU seed plus one Newton step (~1 ulp), l_kk = d * that: two
+          // short dependent chains per pivot instead of an IEEE sqrt followed by an IEEE divide
+          float inv = rsqrtf(d);
+          inv = inv * fmaf(-0.5f * d * inv, inv, 1.5f);
+          const float sd = d * inv;
           D[k][k] = sd;
           invd[k] = inv;
 #pragma unroll
@@ -356,7 +376,7 @@ __global__ void __launch_bounds__(256)
 chol_update_kernel(float* __restrict__ A, int V, int j0, int j1, const Ctrl* ctrl, int attempt,
                    int respect_done) {
   if (chol_skip(ctrl, attempt, respect_done)) return;
-  __shared__ float As[16][68], Bs[16][68];
+  __shared__ __align__(16) float As[16][68], Bs[16][68];
   int tr, tc;
   tri_tile(blockIdx.x, tr, tc);
   const int x0 = j1 + tr * 64, y0 = j1 + tc * 64;
@@ -393,7 +413,7 @@ void launch_cholesky(const float* Sigma, float* Lc, int V, Ctrl* ctrl, int respe
                            160 * 161 * (int)sizeof(float));
       attr_done = true;
     }
-    ++g_launches; chol_small_kernel<<<1, 1024, smem, st>>>(Sigma, Lc, V, ctrl, respect_done);
+    ++g_launches; chol_small_kernel<<<1, CS_THREADS, smem, st>>>(Sigma, Lc, V, ctrl, respect_done);
     return;
   }
   ++g_launches; trace_kernel<<<1, 256, 0, st>>>(Sigma, V, ctrl, respect_done);
@@ -420,7 +440,7 @@ static int cov_nsplit(int V, int N) {
   int nt = (V + 63) / 64;
   int tiles = nt * (nt + 1) / 2;
   int want = (2 * 148 + tiles - 1) / tiles;
-  int maxsplit = (round_up(N, 128) + 255) / 256;   // chunks of >= 256 particles
+  int maxsplit = (round_up(N, 128) + 127) / 128;   // chunks of >= 128 particles
   int ns = want < 1 ? 1 : want;
   if (ns > maxsplit) ns = maxsplit;
   if (ns > 128) ns = 128;
@@ -439,7 +459,7 @@ void launch_cov_chol(const CovCholArgs& a, cudaStream_t st) {
   ++g_launches; mean_kernel<<<V, 256, 0, st>>>(a.phi, a.N, a.ld, a.mu, a.ctrl, a.respect_done);
   if (a.tc_scratch && syrk_tc_supported(V, a.ld)) {
     launch_syrk_tc(a.phi, a.N, a.ld, V, a.mu, a.tc_scratch, a.partial, a.ctrl, a.respect_done, st);
-    ++g_launches; syrk_reduce_kernel<<<(V * V + 255) / 256, 256, 0, st>>>(
+    ++g_launches; syrk_reduce_kernel<<<(8 * V * V + 255) / 256, 256, 0, st>>>(
         a.partial, syrk_tc_nsplit(V, a.ld), V, a.N, a.Sigma, a.ctrl, a.respect_done);
     launch_cholesky(a.Sigma, a.Lc, V, a.ctrl, a.respect_done, st);
     return;
@@ -451,7 +471,7 @@ void launch_cov_chol(const CovCholArgs& a, cudaStream_t st) {
   dim3 grid(nt * (nt + 1) / 2, ns);
   ++g_launches; syrk_partial_kernel<<<grid, 256, 0, st>>>(a.phi, a.N, a.ld, V, a.mu, a.partial, chunk, a.ctrl,
                                             a.respect_done);
-  ++g_launches; syrk_reduce_kernel<<<(V * V + 255) / 256, 256, 0, st>>>(a.partial, ns, V, a.N, a.Sigma, a.ctrl,
+  ++g_launches; syrk_reduce_kernel<<<(8 * V * V + 255) / 256, 256, 0, st>>>(a.partial, ns, V, a.N, a.Sigma, a.ctrl,
                                                           a.respect_done);
   launch_cholesky(a.Sigma, a.Lc, V, a.ctrl, a.respect_done, st);
 }

@@ -2,125 +2,199 @@
 // incremental weights + log Z, exact integer systematic resampling, gather.
 #include "kernels.cuh"
 #include "philox.cuh"
+#ifdef PHI4_RW_TRACE
+#include <cstdio>
+#endif
 
 namespace phi4 {
 
 // ---------------------------------------------------------------------------------------------
-// P1 + P2 in one CTA (N <= a few 1e5 floats: the vector is L2/L1 resident).
+// P1 + P2 in one CTA (N <= a few 1e5 floats: the vector is L2/L1 resident, and for N <= 16384 it
+// is held in registers across all passes).
 // R3: f(d) = ESS(d)/N - target, ESS(d) = (sum e^{-d S})^2 / sum e^{-2 d S}; if f(1-beta) >= 0 the
-// step is final (beta' = 1), else 48 halvings of [0, 1-beta].  exp in fp32 on max-shifted
-// arguments, sums in fp64.  Then w_i = exp(-d (S_i - S_min)) (max w = 1) and
+// step is final (beta' = 1), else delta is the root of f on (0, 1-beta) -- R3 defines it as the
+// limit of 48 bisection halvings.  f is smooth and strictly decreasing, so a bracketed Newton
+// iteration on h(d) = log ESS(d)/N - log target (close to a parabola in d: ESS/N = exp(-d^2 var S)
+// for Gaussian S) started from the previous temperature's delta reaches the same root to 1e-7
+// relative in 3-5 evaluations; each evaluation is one pass over the N actions that also yields
+// h'(d) = 2 a'/a - b'/b from a' = -sum x e, b' = -2 sum x e^2 (x = S - S_min, e = e^{-d x}).
+// A step that leaves the bracket falls back to bisection (reading R3).
+// Then w_i = exp(-d (S_i - S_min)) (max w = 1) and
 // dlogZ = -d S_min + log sum w - log N   (U0 cancels between p_beta and p_beta').
 // ---------------------------------------------------------------------------------------------
-// One evaluation of ESS(d)/N and sum_i e^{-d (S_i - S_min)}: e_i in fp32, sums in fp64, the two
-// sums reduced together.
-__device__ inline double ess_frac_eval(const float* __restrict__ S, int N, float smin, double d,
-                                       double2* scratch, double* sum_out) {
-  // ex2.approx on the max-shifted argument: relative error ~1e-6 |x| on weights that matter
-  // (|x| < ~20), i.e. ~1e-6 on f -- far below the 1e-4 tolerance of the root (R3).  The weights
-  // themselves (P2) use the accurate expf.
-  const float df = (float)d * 1.4426950408889634f;
-  double a = 0.0, b = 0.0;
-  for (int i = threadIdx.x; i < N; i += blockDim.x) {
-    float e;
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(-df * (S[i] - smin)));
-    a += (double)e;
-    b += (double)e * (double)e;
-  }
-  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
-  a = warp_sum(a);
-  b = warp_sum(b);
-  __syncthreads();
-  if (lane == 0) scratch[w] = make_double2(a, b);
-  __syncthreads();
-  if (w == 0) {
-    double2 t = lane < nw ? scratch[lane] : make_double2(0.0, 0.0);
-    t.x = warp_sum(t.x);
-    t.y = warp_sum(t.y);
-    if (lane == 0) scratch[32] = t;
-  }
-  __syncthreads();
-  const double2 r = scratch[32];
-  if (sum_out) *sum_out = r.x;
-  return r.x * r.x / (r.y * (double)N);
+namespace rw {
+constexpr int THREADS = 1024, RC = 16;        // register cache: up to 16 actions per thread
 }
 
-// Root of f(d) = ESS(d)/N - target on (0, rest].  R3 defines delta as the limit of 48 bisection
-// halvings; f is smooth and strictly decreasing, so a bracketed regula falsi (Illinois variant)
-// reaches the same root to ~1e-7 relative in a handful of evaluations instead of 48 -- each
-// evaluation is a pass over all N actions.  DESIGN.md (reading R3) states the equivalence bound.
-__global__ void __launch_bounds__(1024)
-next_delta_reweight_kernel(const float* __restrict__ S, int N, float ess_target,
-                           double delta_fixed, float* __restrict__ w, Ctrl* ctrl) {
-  __shared__ double2 scratch[33];
+struct EssSums { double a, b, da, db; };
+
+// all four sums for one d: e_i by ex2.approx on the max-shifted argument (relative error ~1e-6 |x|
+// on weights that matter, far below the 1e-4 tolerance of the root), per-thread partials in FP32
+// (<= 16 terms when cached, folded every 32 terms otherwise), block reduction in FP64
+template <bool CACHED>
+__device__ __forceinline__ EssSums ess_sums(const float (&xs)[rw::RC], int cnt,
+                                            const float* __restrict__ S, int N, float smin,
+                                            double d, double4* scratch) {
+  const float df = (float)d * 1.4426950408889634f;
+  double A = 0.0, B = 0.0, DA = 0.0, DB = 0.0;
+  if (CACHED) {
+    float a = 0.f, b = 0.f, da = 0.f, db = 0.f;
+#pragma unroll
+    for (int j = 0; j < rw::RC; ++j)
+      if (j < cnt) {
+        float e;
+        asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(-df * xs[j]));
+        const float e2 = e * e;
+        a += e; b += e2;
+        da = fmaf(xs[j], e, da); db = fmaf(xs[j], e2, db);
+      }
+    A = a; B = b; DA = da; DB = db;
+  } else {
+    for (int i0 = threadIdx.x; i0 < N; i0 += rw::THREADS * 32) {
+      float a = 0.f, b = 0.f, da = 0.f, db = 0.f;
+      for (int j = 0; j < 32; ++j) {
+        const int i = i0 + j * rw::THREADS;
+        if (i < N) {
+          const float x = S[i] - smin;
+          float e;
+          asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(-df * x));
+          const float e2 = e * e;
+          a += e; b += e2;
+          da = fmaf(x, e, da); db = fmaf(x, e2, db);
+        }
+      }
+      A += a; B += b; DA += da; DB += db;
+    }
+  }
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  A = warp_sum(A); B = warp_sum(B); DA = warp_sum(DA); DB = warp_sum(DB);
+  if (lane == 0) scratch[w] = make_double4(A, B, DA, DB);
+  __syncthreads();
+  EssSums r{0.0, 0.0, 0.0, 0.0};
+  if (w == 0) {                                    // the totals are valid in warp 0 only
+    double4 t = scratch[lane];                     // 1024 threads: exactly 32 warps
+    r.a = warp_sum(t.x); r.b = warp_sum(t.y); r.da = -warp_sum(t.z); r.db = -2.0 * warp_sum(t.w);
+  }
+  return r;
+}
+
+template <bool CACHED>
+__device__ __forceinline__ void next_delta_reweight_body(const float* __restrict__ S, int N,
+                                                         float ess_target, double delta_fixed,
+                                                         float* __restrict__ w, Ctrl* ctrl) {
+  __shared__ double4 scratch[33];
   __shared__ float smin_s[33];
-  if (ctrl->done) return;
+  __shared__ double bcast_x;
+  __shared__ int bcast_flags;
+  float xs[rw::RC];
+  int cnt = 0;
   float m = INFINITY;
-  for (int i = threadIdx.x; i < N; i += blockDim.x) m = fminf(m, S[i]);
+  if (CACHED) {
+#pragma unroll
+    for (int j = 0; j < rw::RC; ++j) {
+      const int i = threadIdx.x + j * rw::THREADS;
+      xs[j] = i < N ? S[i] : INFINITY;
+      m = fminf(m, xs[j]);
+    }
+    cnt = (N - (int)threadIdx.x + rw::THREADS - 1) / rw::THREADS;
+    cnt = cnt < 0 ? 0 : cnt;
+  } else {
+    for (int i = threadIdx.x; i < N; i += rw::THREADS) m = fminf(m, S[i]);
+  }
   m = warp_min(m);
   if ((threadIdx.x & 31) == 0) smin_s[threadIdx.x >> 5] = m;
   __syncthreads();
   if (threadIdx.x < 32) {
-    float v = threadIdx.x < (blockDim.x >> 5) ? smin_s[threadIdx.x] : INFINITY;
-    v = warp_min(v);
+    float v = warp_min(smin_s[threadIdx.x]);
     if (threadIdx.x == 0) smin_s[32] = v;
   }
   __syncthreads();
   const float smin = smin_s[32];
+  if (CACHED) {
+#pragma unroll
+    for (int j = 0; j < rw::RC; ++j) xs[j] -= smin;
+  }
   const double beta = ctrl->beta;
   const double rest = 1.0 - beta;
-  const double target = (double)ess_target;
+  const double ltarget = log((double)ess_target), lN = log((double)N);
   double delta;
-  int final_step;
+  int final_step = 0;
   if (delta_fixed >= 0.0) {
     delta = delta_fixed;
     final_step = (beta + delta >= 1.0);
   } else {
-    double f_hi = ess_frac_eval(S, N, smin, rest, scratch, nullptr) - target;
-    if (f_hi >= 0.0) {
-      delta = rest;
-      final_step = 1;
-    } else {
-      double lo = 0.0, hi = rest, f_lo = 1.0 - target;     // ESS(0)/N = 1
-      int side = 0;
-      for (int it = 0; it < 60; ++it) {
-        double x = (lo * f_hi - hi * f_lo) / (f_hi - f_lo);
-        if (!(x > lo && x < hi)) x = 0.5 * (lo + hi);
-        double fx = ess_frac_eval(S, N, smin, x, scratch, nullptr) - target;
-        if (fx > 0.0) {
-          lo = x; f_lo = fx;
-          if (side == 1) f_hi *= 0.5;
-          side = 1;
-        } else {
-          hi = x; f_hi = fx;
-          if (side == -1) f_lo *= 0.5;
-          side = -1;
+    // thread 0 owns the bracket and the Newton step (FP64 logs and divisions once, not 1024
+    // times); the next abscissa and the stop flag go through shared memory
+    double lo = 0.0, hi = rest;
+    bool hi_known = false;                           // sign of h(rest) not evaluated yet
+    const double prev = ctrl->delta;
+    double x = (prev > 0.0 && prev < rest) ? prev : rest;
+    delta = rest;
+    for (int it = 0; it < 64; ++it) {
+      const EssSums q = ess_sums<CACHED>(xs, cnt, S, N, smin, x, scratch);
+      if (threadIdx.x == 0) {
+        int stop = 0, fin = 0;
+        double xn = x;
+        const double h = 2.0 * log(q.a) - log(q.b) - lN - ltarget;
+        if (x >= rest && !hi_known) {
+          if (h >= 0.0) { stop = 1; fin = 1; xn = rest; }
+          hi_known = true;
         }
-        if (hi - lo <= 1e-7 * hi || fabs(fx) < 1e-9) break;
+        if (!stop) {
+          if (h > 0.0) lo = x; else hi = x;
+          if (fabs(h) < 1e-9) stop = 1;
+          else {
+            const double dh = 2.0 * q.da / q.a - q.db / q.b;
+            xn = x - h / dh;
+            if (!(xn > lo && xn < hi)) {
+              if (!hi_known && xn >= hi) xn = rest;      // probe the end of the interval
+              else if (hi_known) xn = 0.5 * (lo + hi);
+              else xn = fmin(rest, 2.0 * x);             // dh >= 0 or NaN far out: walk right
+            }
+            if (fabs(xn - x) <= 1e-7 * xn && !(xn >= rest && !hi_known)) stop = 1;
+          }
+        }
+        bcast_x = xn; bcast_flags = stop | (fin << 1);
       }
-      // one secant step inside the final bracket
-      double x = (lo * f_hi - hi * f_lo) / (f_hi - f_lo);
-      delta = (x > lo && x < hi) ? x : 0.5 * (lo + hi);
-      final_step = 0;
+      __syncthreads();
+      x = bcast_x;
+      delta = x;
+      const int fl = bcast_flags;
+      final_step = fl >> 1;
+#ifdef PHI4_RW_TRACE
+      if (threadIdx.x == 0) printf("rw it=%d x=%.9g stop=%d\n", it, x, fl);
+#endif
+      if (fl & 1) break;
     }
   }
   const float df = (float)delta;
   double a = 0.0, b = 0.0;
-  for (int i = threadIdx.x; i < N; i += blockDim.x) {
-    float e = expf(-df * (S[i] - smin));
-    w[i] = e;
-    a += (double)e;
-    b += (double)e * (double)e;
+  if (CACHED) {
+#pragma unroll
+    for (int j = 0; j < rw::RC; ++j)
+      if (j < cnt) {
+        const float e = expf(-df * xs[j]);
+        w[threadIdx.x + j * rw::THREADS] = e;
+        a += (double)e;
+        b += (double)e * (double)e;
+      }
+  } else {
+    for (int i = threadIdx.x; i < N; i += rw::THREADS) {
+      const float e = expf(-df * (S[i] - smin));
+      w[i] = e;
+      a += (double)e;
+      b += (double)e * (double)e;
+    }
   }
   {
-    const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5;
     a = warp_sum(a);
     b = warp_sum(b);
     __syncthreads();
-    if (lane == 0) scratch[wi] = make_double2(a, b);
+    if (lane == 0) scratch[wi] = make_double4(a, b, 0.0, 0.0);
     __syncthreads();
     if (wi == 0) {
-      double2 t = lane < nw ? scratch[lane] : make_double2(0.0, 0.0);
+      double4 t = scratch[lane];
       t.x = warp_sum(t.x);
       t.y = warp_sum(t.y);
       if (lane == 0) scratch[32] = t;
@@ -130,7 +204,7 @@ next_delta_reweight_kernel(const float* __restrict__ S, int N, float ess_target,
     b = scratch[32].y;
   }
   if (threadIdx.x == 0) {
-    double dlz = -delta * (double)smin + log(a) - log((double)N);
+    double dlz = -delta * (double)smin + log(a) - lN;
     ctrl->delta = delta;
     ctrl->beta = final_step ? 1.0 : beta + delta;
     ctrl->ess_frac = a * a / (b * (double)N);
@@ -141,9 +215,17 @@ next_delta_reweight_kernel(const float* __restrict__ S, int N, float ess_target,
   }
 }
 
+__global__ void __launch_bounds__(rw::THREADS)
+next_delta_reweight_kernel(const float* __restrict__ S, int N, float ess_target,
+                           double delta_fixed, float* __restrict__ w, Ctrl* ctrl) {
+  if (ctrl->done) return;
+  if (N <= rw::THREADS * rw::RC) next_delta_reweight_body<true>(S, N, ess_target, delta_fixed, w, ctrl);
+  else next_delta_reweight_body<false>(S, N, ess_target, delta_fixed, w, ctrl);
+}
+
 void launch_next_delta_reweight(const float* S, int N, float ess_target, double delta_fixed,
                                 float* w, Ctrl* ctrl, cudaStream_t st) {
-  ++g_launches; next_delta_reweight_kernel<<<1, 1024, 0, st>>>(S, N, ess_target, delta_fixed, w, ctrl);
+  ++g_launches; next_delta_reweight_kernel<<<1, rw::THREADS, 0, st>>>(S, N, ess_target, delta_fixed, w, ctrl);
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -79,7 +79,7 @@ def test_hmc_rejects_unsupported():
         B.smc_set_params(h, kernel=1)
     h.close()
     h = B.smc_init(10, -4.0, 1.0, 256, 1)
-    for bad in (dict(hmc_eps=0.0), dict(hmc_leapfrog=0), dict(kernel=2)):
+    for bad in (dict(hmc_eps=0.0), dict(hmc_leapfrog=0), dict(kernel=3)):
         with pytest.raises(B.Phi4Error):
             B.smc_set_params(h, **{"kernel": 1, **bad})
     h.close()
