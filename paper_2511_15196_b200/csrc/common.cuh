@@ -83,4 +83,31 @@ __device__ inline double block_sum(double v, double* scratch) {
   return scratch[32];
 }
 
+// Programmatic dependent launch: a kernel launched through launch_pdl may be scheduled while its
+// predecessor in the stream is still running; pdl_enter() -- the first statement of every such
+// kernel -- lets the successor be scheduled in turn and then blocks until the predecessor has
+// completed and its writes are visible (a grid's CTAs are only scheduled once every CTA of its
+// predecessor has started, so waiting grids cannot starve the grids they wait for).  Stream order is unchanged; only the launch latency between
+// the short dependent kernels of one temperature overlaps.  Launched normally, pdl_enter() is a
+// no-op.  PHI4_NO_PDL=1 in the environment turns the attribute off.
+__device__ __forceinline__ void pdl_enter() {
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+
+bool pdl_enabled();
+
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem,
+                              cudaStream_t st, Args&&... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = pdl_enabled() ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
 }  // namespace phi4

@@ -12,6 +12,7 @@ namespace phi4 {
 __global__ void __launch_bounds__(256)
 mean_kernel(const float* __restrict__ phi, int N, int ld, float* __restrict__ mu,
             const Ctrl* ctrl, int respect_done) {
+  pdl_enter();
   __shared__ double scratch[33];
   if (respect_done && ctrl->done) return;
   const float* row = phi + (size_t)blockIdx.x * ld;
@@ -116,6 +117,7 @@ __global__ void __launch_bounds__(256)
 syrk_partial_kernel(const float* __restrict__ phi, int N, int ld, int V,
                     const float* __restrict__ mu, float* __restrict__ partial, int chunk,
                     const Ctrl* ctrl, int respect_done) {
+  pdl_enter();
   if (respect_done && ctrl->done) return;
   __shared__ __align__(16) float As[16][68], Bs[16][68];
   int tr, tc;
@@ -143,6 +145,7 @@ syrk_partial_kernel(const float* __restrict__ phi, int N, int ld, int V,
 // eight lanes per entry each sum every eighth split, then a fixed shuffle tree.
 __global__ void syrk_reduce_kernel(const float* __restrict__ partial, int nsplit, int V, int N,
                                    float* __restrict__ Sigma, const Ctrl* ctrl, int respect_done) {
+  pdl_enter();
   if (respect_done && ctrl->done) return;
   const int t = blockIdx.x * blockDim.x + threadIdx.x;
   const int idx = t >> 3, part = t & 7;
@@ -274,6 +277,7 @@ __device__ __forceinline__ void chol_panels(float* sm, int P, int V, int* failed
 __global__ void __launch_bounds__(1024)
 chol_small_kernel(const float* __restrict__ Sigma, float* __restrict__ Lc, int V, Ctrl* ctrl,
                   int respect_done) {
+  pdl_enter();
   extern __shared__ float sm[];   // V x (V+1)
   __shared__ int failed_s;
   __shared__ double red[33];
@@ -413,7 +417,7 @@ void launch_cholesky(const float* Sigma, float* Lc, int V, Ctrl* ctrl, int respe
                            160 * 161 * (int)sizeof(float));
       attr_done = true;
     }
-    ++g_launches; chol_small_kernel<<<1, CS_THREADS, smem, st>>>(Sigma, Lc, V, ctrl, respect_done);
+    ++g_launches; launch_pdl(chol_small_kernel, 1, CS_THREADS, smem, st, Sigma, Lc, V, ctrl, respect_done);
     return;
   }
   ++g_launches; trace_kernel<<<1, 256, 0, st>>>(Sigma, V, ctrl, respect_done);
@@ -456,10 +460,10 @@ size_t cov_partial_floats(int V, int N) {
 
 void launch_cov_chol(const CovCholArgs& a, cudaStream_t st) {
   const int V = a.V;
-  ++g_launches; mean_kernel<<<V, 256, 0, st>>>(a.phi, a.N, a.ld, a.mu, a.ctrl, a.respect_done);
+  ++g_launches; launch_pdl(mean_kernel, V, 256, 0, st, a.phi, a.N, a.ld, a.mu, a.ctrl, a.respect_done);
   if (a.tc_scratch && syrk_tc_supported(V, a.ld)) {
     launch_syrk_tc(a.phi, a.N, a.ld, V, a.mu, a.tc_scratch, a.partial, a.ctrl, a.respect_done, st);
-    ++g_launches; syrk_reduce_kernel<<<(8 * V * V + 255) / 256, 256, 0, st>>>(
+    ++g_launches; launch_pdl(syrk_reduce_kernel, (8 * V * V + 255) / 256, 256, 0, st, 
         a.partial, syrk_tc_nsplit(V, a.ld), V, a.N, a.Sigma, a.ctrl, a.respect_done);
     launch_cholesky(a.Sigma, a.Lc, V, a.ctrl, a.respect_done, st);
     return;
@@ -469,9 +473,9 @@ void launch_cov_chol(const CovCholArgs& a, cudaStream_t st) {
   ns = (a.ld + chunk - 1) / chunk;
   int nt = (V + 63) / 64;
   dim3 grid(nt * (nt + 1) / 2, ns);
-  ++g_launches; syrk_partial_kernel<<<grid, 256, 0, st>>>(a.phi, a.N, a.ld, V, a.mu, a.partial, chunk, a.ctrl,
+  ++g_launches; launch_pdl(syrk_partial_kernel, grid, 256, 0, st, a.phi, a.N, a.ld, V, a.mu, a.partial, chunk, a.ctrl,
                                             a.respect_done);
-  ++g_launches; syrk_reduce_kernel<<<(8 * V * V + 255) / 256, 256, 0, st>>>(a.partial, ns, V, a.N, a.Sigma, a.ctrl,
+  ++g_launches; launch_pdl(syrk_reduce_kernel, (8 * V * V + 255) / 256, 256, 0, st, a.partial, ns, V, a.N, a.Sigma, a.ctrl,
                                                           a.respect_done);
   launch_cholesky(a.Sigma, a.Lc, V, a.ctrl, a.respect_done, st);
 }

@@ -1,4 +1,5 @@
 // field.cu -- particle initialisation (Philox stream INIT) and the full lattice action.
+#include <cstdlib>
 #include "kernels.cuh"
 #include "philox.cuh"
 
@@ -91,6 +92,11 @@ void launch_zero_upper(float* A, int V, cudaStream_t st) {
 }
 
 __global__ void reset_counters_kernel(Ctrl* ctrl) { ctrl->n_accept = 0u; ctrl->n_unique = 0u; }
+bool pdl_enabled() {
+  static const bool on = [] { const char* e = getenv("PHI4_NO_PDL"); return !(e && e[0] == '1'); }();
+  return on;
+}
+
 void launch_reset_counters(Ctrl* ctrl, cudaStream_t st) { reset_counters_kernel<<<1, 1, 0, st>>>(ctrl); }
 
 }  // namespace phi4

@@ -90,6 +90,7 @@ struct TcParams {
 __global__ void lsplit_kernel(const float* __restrict__ Lc, int V, int Vn, int Kp, float s,
                               float* __restrict__ out, size_t lpart, const Ctrl* ctrl,
                               int respect_done) {
+  pdl_enter();
   if (respect_done && ctrl->done) return;
   const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= (size_t)Kp * Vn) return;
@@ -187,6 +188,7 @@ __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
 //                 descriptors of all K-steps are tabulated once in shared memory by its 32 lanes.
 template <int LT>
 __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParams p) {
+  pdl_enter();
   using namespace tc;
   extern __shared__ __align__(1024) uint8_t smem[];
   if (p.respect_done && p.ctrl->done) return;
@@ -520,7 +522,7 @@ extern "C" __attribute__((visibility("default"))) int phi4_debug_tc_trace(long l
 void launch_lsplit(const float* Lc, int V, int Vn, int Kp, float s, float* Lsplit, const Ctrl* ctrl,
                    int respect_done, cudaStream_t st) {
   ++g_launches;
-  lsplit_kernel<<<(unsigned)(((size_t)Kp * Vn + 255) / 256), 256, 0, st>>>(
+  launch_pdl(lsplit_kernel, (unsigned)(((size_t)Kp * Vn + 255) / 256), 256, 0, st, 
       Lc, V, Vn, Kp, s, Lsplit, tc::l_floats_vk(Vn, Kp), ctrl, respect_done);
 }
 
@@ -546,9 +548,9 @@ void launch_mutate_tc(const MutateArgs& a, float* Lsplit, cudaStream_t st) {
   const dim3 grid(a.ld / tc::TILE);
   ++g_launches;
   // lattice sizes of the BASELINE configs get a fully unrolled stencil; any other L the loop
-  if (p.L == 10) mutate_tc_kernel<10><<<grid, tc::THREADS, smem, st>>>(p);
-  else if (p.L == 4) mutate_tc_kernel<4><<<grid, tc::THREADS, smem, st>>>(p);
-  else mutate_tc_kernel<0><<<grid, tc::THREADS, smem, st>>>(p);
+  if (p.L == 10) launch_pdl(mutate_tc_kernel<10>, grid, tc::THREADS, smem, st, p);
+  else if (p.L == 4) launch_pdl(mutate_tc_kernel<4>, grid, tc::THREADS, smem, st, p);
+  else launch_pdl(mutate_tc_kernel<0>, grid, tc::THREADS, smem, st, p);
 }
 
 }  // namespace phi4

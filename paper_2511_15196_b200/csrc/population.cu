@@ -218,6 +218,7 @@ __device__ __forceinline__ void next_delta_reweight_body(const float* __restrict
 __global__ void __launch_bounds__(rw::THREADS)
 next_delta_reweight_kernel(const float* __restrict__ S, int N, float ess_target,
                            double delta_fixed, float* __restrict__ w, Ctrl* ctrl) {
+  pdl_enter();
   if (ctrl->done) return;
   if (N <= rw::THREADS * rw::RC) next_delta_reweight_body<true>(S, N, ess_target, delta_fixed, w, ctrl);
   else next_delta_reweight_body<false>(S, N, ess_target, delta_fixed, w, ctrl);
@@ -225,7 +226,7 @@ next_delta_reweight_kernel(const float* __restrict__ S, int N, float ess_target,
 
 void launch_next_delta_reweight(const float* S, int N, float ess_target, double delta_fixed,
                                 float* w, Ctrl* ctrl, cudaStream_t st) {
-  ++g_launches; next_delta_reweight_kernel<<<1, rw::THREADS, 0, st>>>(S, N, ess_target, delta_fixed, w, ctrl);
+  ++g_launches; launch_pdl(next_delta_reweight_kernel, 1, rw::THREADS, 0, st, S, N, ess_target, delta_fixed, w, ctrl);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -247,6 +248,7 @@ __device__ __forceinline__ unsigned long long quantise40(float w) {
 __global__ void __launch_bounds__(1024)
 quantise_scan_kernel(const float* __restrict__ w, int N, unsigned long long* __restrict__ C,
                      Ctrl* ctrl) {
+  pdl_enter();
   __shared__ unsigned long long wsum[32];
   if (ctrl->done) return;
   const int ipt = (N + blockDim.x - 1) / blockDim.x;
@@ -383,7 +385,7 @@ scan_apply_kernel(const float* __restrict__ w, int N, const unsigned long long* 
 void launch_quantise_scan(const float* w, int N, unsigned long long* C, Ctrl* ctrl,
                           cudaStream_t st) {
   if (N <= 32768 || N > 256 * SCAN_BLOCK) {
-    ++g_launches; quantise_scan_kernel<<<1, 1024, 0, st>>>(w, N, C, ctrl);
+    ++g_launches; launch_pdl(quantise_scan_kernel, 1, 1024, 0, st, w, N, C, ctrl);
     return;
   }
   const int nb = (N + SCAN_BLOCK - 1) / SCAN_BLOCK;
@@ -398,6 +400,7 @@ void launch_quantise_scan(const float* w, int N, unsigned long long* C, Ctrl* ct
 // identity, so that a step enqueued past beta = 1 leaves the particles unchanged.
 __global__ void ancestors_kernel(const unsigned long long* __restrict__ C, int N, uint64_t seed,
                                  int32_t* __restrict__ anc, const Ctrl* ctrl) {
+  pdl_enter();
   int j = blockIdx.x * blockDim.x + threadIdx.x;
   if (j >= N) return;
   if (ctrl->done || ctrl->q_total == 0ull) { anc[j] = j; return; }
@@ -416,7 +419,7 @@ __global__ void ancestors_kernel(const unsigned long long* __restrict__ C, int N
 
 void launch_ancestors(const unsigned long long* C, int N, uint64_t seed, int32_t* anc, Ctrl* ctrl,
                       cudaStream_t st) {
-  ++g_launches; ancestors_kernel<<<(N + 255) / 256, 256, 0, st>>>(C, N, seed, anc, ctrl);
+  ++g_launches; launch_pdl(ancestors_kernel, (N + 255) / 256, 256, 0, st, C, N, seed, anc, ctrl);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -430,6 +433,7 @@ gather_kernel(const float* __restrict__ pin, float* __restrict__ pout,
               const float* __restrict__ Sin, float* __restrict__ Sout,
               const float* __restrict__ Uin, float* __restrict__ Uout,
               const int32_t* __restrict__ anc, int N, int ld, int V, Ctrl* ctrl) {
+  pdl_enter();
   const int j0 = (blockIdx.x * blockDim.x + threadIdx.x) * 4;
   if (j0 >= ld) return;
   int a[4];
@@ -470,12 +474,13 @@ void launch_gather(const float* phi_in, float* phi_out, const float* S_in, float
                    const float* U_in, float* U_out, const int32_t* anc, int N, int ld, int V,
                    Ctrl* ctrl, cudaStream_t st) {
   dim3 grid((ld / 4 + 255) / 256, (V + GATHER_ROWS - 1) / GATHER_ROWS);
-  ++g_launches; gather_kernel<<<grid, 256, 0, st>>>(phi_in, phi_out, S_in, S_out, U_in, U_out, anc, N, ld, V,
+  ++g_launches; launch_pdl(gather_kernel, grid, 256, 0, st, phi_in, phi_out, S_in, S_out, U_in, U_out, anc, N, ld, V,
                                       ctrl);
 }
 
 // End of a temperature: record it, advance the index, latch done at beta == 1.
 __global__ void finish_step_kernel(Ctrl* ctrl, StepRecord* rec, int max_rec, int k, int N) {
+  pdl_enter();
   if (ctrl->done) return;
   int t = ctrl->temp_index;
   if (t < max_rec) {
@@ -494,7 +499,7 @@ __global__ void finish_step_kernel(Ctrl* ctrl, StepRecord* rec, int max_rec, int
 }
 
 void launch_finish_step(Ctrl* ctrl, StepRecord* rec, int max_rec, int k, int N, cudaStream_t st) {
-  ++g_launches; finish_step_kernel<<<1, 1, 0, st>>>(ctrl, rec, max_rec, k, N);
+  ++g_launches; launch_pdl(finish_step_kernel, 1, 1, 0, st, ctrl, rec, max_rec, k, N);
 }
 
 }  // namespace phi4
