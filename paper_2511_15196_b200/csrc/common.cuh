@@ -90,9 +90,13 @@ __device__ inline double block_sum(double v, double* scratch) {
 // predecessor has started, so waiting grids cannot starve the grids they wait for).  Stream order is unchanged; only the launch latency between
 // the short dependent kernels of one temperature overlaps.  Launched normally, pdl_enter() is a
 // no-op.  PHI4_NO_PDL=1 in the environment turns the attribute off.
-__device__ __forceinline__ void pdl_enter() {
+__device__ __forceinline__ void pdl_trigger() {
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-  asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_enter() {
+  pdl_trigger();
+  pdl_wait();
 }
 
 bool pdl_enabled();

@@ -188,10 +188,11 @@ __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
 //                 descriptors of all K-steps are tabulated once in shared memory by its 32 lanes.
 template <int LT>
 __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParams p) {
-  pdl_enter();
+  // programmatic dependent launch: barrier setup and the TMEM allocation touch nothing the
+  // predecessor writes, so they run before the wait
+  pdl_trigger();
   using namespace tc;
   extern __shared__ __align__(1024) uint8_t smem[];
-  if (p.respect_done && p.ctrl->done) return;
   const Smem lay = smem_layout(p.V);
   float* tile0 = reinterpret_cast<float*>(smem + lay.tile0);
   float* tile1 = reinterpret_cast<float*>(smem + lay.tile1);
@@ -226,6 +227,11 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
   __syncthreads();
   tc_fence_after();
   const uint32_t taddr = *tmem_slot;
+  pdl_wait();
+  if (p.respect_done && p.ctrl->done) {
+    if (warp == 0) tmem_dealloc(taddr, ncols);
+    return;
+  }
 
   if (warp == MMA_WARP) {
     // ================================ MMA issuer (one thread) =================================

@@ -21,6 +21,7 @@ __device__ __forceinline__ double logaddexp_d(double a, double b) {
 //      (word0 mod (n - k_del)) of Philox stream NS_START (c1 = j, c2 = iteration).
 __global__ void __launch_bounds__(1024)
 ns_select_evidence_kernel(NsArgs a) {
+  pdl_enter();
   extern __shared__ unsigned long long keys[];   // npow2 keys; later reused as int flags
   __shared__ double scratch[33];
   __shared__ int wsum[32];
@@ -147,7 +148,7 @@ void launch_ns_select_evidence(const NsArgs& a, cudaStream_t st) {
                          16384 * (int)sizeof(unsigned long long));
     attr_done = true;
   }
-  ++g_launches; ns_select_evidence_kernel<<<1, 1024, smem, st>>>(a);
+  ++g_launches; launch_pdl(ns_select_evidence_kernel, 1, 1024, smem, st, a);
 }
 
 // hsum[j] = sum_{m=1..j} 1/(n-m+1), j = 0..k_del: the data-independent volume shrinkage of
@@ -165,6 +166,7 @@ void launch_ns_hsum(double* hsum, int n, int k_del, cudaStream_t st) {
 // N3 gather: walker j <- live point start[j].  One thread per (site, walker): the walker index is
 // the fast one, so the stores are coalesced and the gathers hit 512 distinct columns of one row.
 __global__ void ns_load_walkers_kernel(NsArgs a) {
+  pdl_enter();
   if (a.ctrl->done) return;
   const int j = blockIdx.x * blockDim.x + threadIdx.x;
   const int x = blockIdx.y;
@@ -180,6 +182,7 @@ __global__ void ns_load_walkers_kernel(NsArgs a) {
 
 // Magnetisation of the dead points (logged for the posterior observables): one warp per point.
 __global__ void ns_dead_M_kernel(NsArgs a) {
+  pdl_enter();
   if (a.ctrl->done) return;
   const int j = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
   if (j >= a.k_del) return;
@@ -192,13 +195,14 @@ __global__ void ns_dead_M_kernel(NsArgs a) {
 }
 
 void launch_ns_load_walkers(const NsArgs& a, cudaStream_t st) {
-  ++g_launches; ns_dead_M_kernel<<<(a.k_del * 32 + 127) / 128, 128, 0, st>>>(a);
+  ++g_launches; launch_pdl(ns_dead_M_kernel, (a.k_del * 32 + 127) / 128, 128, 0, st, a);
   dim3 grid((a.ldw + 127) / 128, a.V);
-  ++g_launches; ns_load_walkers_kernel<<<grid, 128, 0, st>>>(a);
+  ++g_launches; launch_pdl(ns_load_walkers_kernel, grid, 128, 0, st, a);
 }
 
 // N3 scatter: dead slot dead[j] <- walker j, one thread per (site, walker).
 __global__ void ns_store_walkers_kernel(NsArgs a) {
+  pdl_enter();
   if (a.ctrl->done) return;
   const int j = blockIdx.x * blockDim.x + threadIdx.x;
   const int x = blockIdx.y;
@@ -213,12 +217,13 @@ __global__ void ns_store_walkers_kernel(NsArgs a) {
 
 void launch_ns_store_walkers(const NsArgs& a, cudaStream_t st) {
   dim3 grid((a.k_del + 127) / 128, a.V);
-  ++g_launches; ns_store_walkers_kernel<<<grid, 128, 0, st>>>(a);
+  ++g_launches; launch_pdl(ns_store_walkers_kernel, grid, 128, 0, st, a);
 }
 
 // N4: remaining = X mean_live(e^-S) / (Z + X mean_live(e^-S)); record; stop rule; live term.
 __global__ void __launch_bounds__(1024)
 ns_finish_kernel(NsArgs a, StepRecord* rec, int n_walk) {
+  pdl_enter();
   __shared__ double scratch[33];
   __shared__ float smin_s[33];
   Ctrl* ctrl = a.ctrl;
@@ -265,7 +270,7 @@ ns_finish_kernel(NsArgs a, StepRecord* rec, int n_walk) {
 }
 
 void launch_ns_finish(const NsArgs& a, StepRecord* rec, int n_walk, cudaStream_t st) {
-  ++g_launches; ns_finish_kernel<<<1, 1024, 0, st>>>(a, rec, n_walk);
+  ++g_launches; launch_pdl(ns_finish_kernel, 1, 1024, 0, st, a, rec, n_walk);
 }
 
 // Posterior sample for `observables`: dead points (weight w_j e^{-S_j}) followed by the live
