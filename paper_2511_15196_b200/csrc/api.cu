@@ -372,8 +372,8 @@ static CovCholArgs cov_args(phi4smc* h, int respect_done) {
   return c;
 }
 
-static void enqueue_resample(phi4smc* h) {
-  launch_quantise_scan(h->w, h->N, h->C, h->ctrl, h->st);
+static void enqueue_resample(phi4smc* h, bool scanned = false) {
+  if (!scanned) launch_quantise_scan(h->w, h->N, h->C, h->ctrl, h->st);
   launch_ancestors(h->C, h->N, h->seed, h->anc, h->ctrl, h->st);
   const int o = h->cur ^ 1;
   launch_gather(h->phi[h->cur], h->phi[o], h->S[h->cur], h->S[o], h->U0[h->cur], h->U0[o], h->anc,
@@ -382,8 +382,9 @@ static void enqueue_resample(phi4smc* h) {
 }
 
 static void enqueue_smc_step(phi4smc* h) {
-  launch_next_delta_reweight(h->S[h->cur], h->N, h->prm.ess_target, -1.0, h->w, h->ctrl, h->st);
-  enqueue_resample(h);
+  const bool scanned = launch_next_delta_reweight(h->S[h->cur], h->N, h->prm.ess_target, -1.0, h->w,
+                                                  h->C, h->ctrl, h->st);
+  enqueue_resample(h, scanned);
   launch_cov_chol(cov_args(h, 1), h->st);
   enqueue_mutation(h, smc_mutate_args(h, h->prm.k_steps, nullptr, nullptr, 1));
   h->step_counter += (uint64_t)h->prm.k_steps;
@@ -730,7 +731,7 @@ PHI4_API int smc_mutate(phi4smc* h, int k, uint8_t* h_accept, float* h_margin) {
 PHI4_API int smc_reweight(phi4smc* h, double delta, float* h_w, smc_step_info* info) {
   if (!h || h->kind != KIND_SMC) return PHI4_EINVAL;
   launch_next_delta_reweight(h->S[h->cur], h->N, h->prm.ess_target, delta < 0.0 ? -1.0 : delta,
-                             h->w, h->ctrl, h->st);
+                             h->w, nullptr, h->ctrl, h->st);
   if (h_w) CU(cudaMemcpyAsync(h_w, h->w, sizeof(float) * h->N, cudaMemcpyDeviceToHost, h->st));
   int rc = sync_ctrl(h);
   if (rc == PHI4_ECUDA) return rc;

@@ -59,8 +59,8 @@ void launch_propose_tc(const float* phi, float* phip, const float* Zs, const flo
                        int V, const Ctrl* ctrl, int respect_done, cudaStream_t st);
 
 // population.cu -- P1-P4
-void launch_next_delta_reweight(const float* S, int N, float ess_target, double delta_fixed,
-                                float* w, Ctrl* ctrl, cudaStream_t st);
+bool launch_next_delta_reweight(const float* S, int N, float ess_target, double delta_fixed,
+                                float* w, unsigned long long* C, Ctrl* ctrl, cudaStream_t st);
 void launch_quantise_scan(const float* w, int N, unsigned long long* C, Ctrl* ctrl,
                           cudaStream_t st);
 void launch_ancestors(const unsigned long long* C, int N, uint64_t seed, int32_t* anc, Ctrl* ctrl,

@@ -22,6 +22,17 @@ namespace phi4 {
 // Then w_i = exp(-d (S_i - S_min)) (max w = 1) and
 // dlogZ = -d S_min + log sum w - log N   (U0 cancels between p_beta and p_beta').
 // ---------------------------------------------------------------------------------------------
+// floor(w 2^40) for an fp32 w in [0, 1], from the bits: w = m 2^(e-150), so q = m 2^(e-110).
+// Exact (reading R5: identical to floor((double)w * 2^40)).
+__device__ __forceinline__ unsigned long long quantise40(float w) {
+  const uint32_t b = __float_as_uint(w);
+  const int e = (int)((b >> 23) & 0xffu);
+  if (e == 0 || (b >> 31)) return 0ull;                       // zero, subnormal (< 2^-126) or negative
+  const unsigned long long m = (unsigned long long)((b & 0x7fffffu) | 0x800000u);
+  const int sh = e - 110;
+  return sh >= 0 ? (m << sh) : (sh > -24 ? (m >> (-sh)) : 0ull);
+}
+
 namespace rw {
 constexpr int THREADS = 1024, RC = 16;        // register cache: up to 16 actions per thread
 }
@@ -81,7 +92,9 @@ __device__ __forceinline__ EssSums ess_sums(const float (&xs)[rw::RC], int cnt,
 template <bool CACHED>
 __device__ __forceinline__ void next_delta_reweight_body(const float* __restrict__ S, int N,
                                                          float ess_target, double delta_fixed,
-                                                         float* __restrict__ w, Ctrl* ctrl) {
+                                                         float* __restrict__ w,
+                                                         unsigned long long* __restrict__ C,
+                                                         Ctrl* ctrl) {
   __shared__ double4 scratch[33];
   __shared__ float smin_s[33];
   __shared__ double bcast_x;
@@ -89,15 +102,18 @@ __device__ __forceinline__ void next_delta_reweight_body(const float* __restrict
   float xs[rw::RC];
   int cnt = 0;
   float m = INFINITY;
+  // cached layout: warp w owns the contiguous span [w 32 ipt, (w+1) 32 ipt), lane l its elements
+  // l, l + 32, ...: every load / store instruction covers 32 consecutive entries, and the integer
+  // scan of P3 is a warp scan per row plus a running carry
+  const int ipt = min(rw::RC, (N + rw::THREADS - 1) / rw::THREADS);
+  const int run0 = (int)(threadIdx.x >> 5) * 32 * ipt + (int)(threadIdx.x & 31);
   if (CACHED) {
+    cnt = max(0, min(ipt, (N - run0 + 31) >> 5));
 #pragma unroll
     for (int j = 0; j < rw::RC; ++j) {
-      const int i = threadIdx.x + j * rw::THREADS;
-      xs[j] = i < N ? S[i] : INFINITY;
+      xs[j] = j < cnt ? S[run0 + 32 * j] : INFINITY;
       m = fminf(m, xs[j]);
     }
-    cnt = (N - (int)threadIdx.x + rw::THREADS - 1) / rw::THREADS;
-    cnt = cnt < 0 ? 0 : cnt;
   } else {
     for (int i = threadIdx.x; i < N; i += rw::THREADS) m = fminf(m, S[i]);
   }
@@ -170,14 +186,55 @@ __device__ __forceinline__ void next_delta_reweight_body(const float* __restrict
   const float df = (float)delta;
   double a = 0.0, b = 0.0;
   if (CACHED) {
+    unsigned long long run = 0;
 #pragma unroll
     for (int j = 0; j < rw::RC; ++j)
       if (j < cnt) {
         const float e = expf(-df * xs[j]);
-        w[threadIdx.x + j * rw::THREADS] = e;
+        xs[j] = e;                                   // kept for the scan below
+        w[run0 + 32 * j] = e;
         a += (double)e;
         b += (double)e * (double)e;
+        run += quantise40(e);
       }
+    if (C) {
+      // P3 fused (reading R5): inclusive integer scan of q_i = floor(w_i 2^40).  Warp totals ->
+      // exclusive offsets of the warp spans; inside a span, one warp scan per row of 32.
+      __shared__ unsigned long long wsum[32];
+      const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+      unsigned long long tot = run;
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) tot += __shfl_xor_sync(0xffffffffu, tot, o);
+      if (lane == 0) wsum[wid] = tot;
+      __syncthreads();
+      if (wid == 0) {
+        unsigned long long v = wsum[lane], sc = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+          unsigned long long u = __shfl_up_sync(0xffffffffu, sc, o);
+          if (lane >= o) sc += u;
+        }
+        wsum[lane] = sc - v;  // exclusive
+      }
+      __syncthreads();
+      unsigned long long carry = wsum[wid];
+#pragma unroll
+      for (int j = 0; j < rw::RC; ++j)
+        if (j < ipt) {                               // block-uniform bound: shuffles stay convergent
+          unsigned long long inc = j < cnt ? quantise40(xs[j]) : 0ull;
+#pragma unroll
+          for (int o = 1; o < 32; o <<= 1) {
+            unsigned long long v = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += v;
+          }
+          if (j < cnt) C[run0 + 32 * j] = carry + inc;
+          carry += __shfl_sync(0xffffffffu, inc, 31);
+        }
+      if (threadIdx.x == rw::THREADS - 1) {
+        ctrl->q_total = carry;
+        if (carry == 0ull) ctrl->nan_flag = 1;
+      }
+    }
   } else {
     for (int i = threadIdx.x; i < N; i += rw::THREADS) {
       const float e = expf(-df * (S[i] - smin));
@@ -217,16 +274,23 @@ __device__ __forceinline__ void next_delta_reweight_body(const float* __restrict
 
 __global__ void __launch_bounds__(rw::THREADS)
 next_delta_reweight_kernel(const float* __restrict__ S, int N, float ess_target,
-                           double delta_fixed, float* __restrict__ w, Ctrl* ctrl) {
+                           double delta_fixed, float* __restrict__ w,
+                           unsigned long long* __restrict__ C, Ctrl* ctrl) {
   pdl_enter();
   if (ctrl->done) return;
-  if (N <= rw::THREADS * rw::RC) next_delta_reweight_body<true>(S, N, ess_target, delta_fixed, w, ctrl);
-  else next_delta_reweight_body<false>(S, N, ess_target, delta_fixed, w, ctrl);
+  if (N <= rw::THREADS * rw::RC) next_delta_reweight_body<true>(S, N, ess_target, delta_fixed, w, C, ctrl);
+  else next_delta_reweight_body<false>(S, N, ess_target, delta_fixed, w, nullptr, ctrl);
 }
 
-void launch_next_delta_reweight(const float* S, int N, float ess_target, double delta_fixed,
-                                float* w, Ctrl* ctrl, cudaStream_t st) {
-  ++g_launches; launch_pdl(next_delta_reweight_kernel, 1, rw::THREADS, 0, st, S, N, ess_target, delta_fixed, w, ctrl);
+// C != nullptr and N <= 16384: the integer scan of P3 runs in the same kernel (the weights are
+// still in registers); returns whether it did, so that the caller can skip launch_quantise_scan.
+bool launch_next_delta_reweight(const float* S, int N, float ess_target, double delta_fixed,
+                                float* w, unsigned long long* C, Ctrl* ctrl, cudaStream_t st) {
+  const bool fused = C != nullptr && N <= rw::THREADS * rw::RC;
+  ++g_launches;
+  launch_pdl(next_delta_reweight_kernel, 1, rw::THREADS, 0, st, S, N, ess_target, delta_fixed, w,
+             fused ? C : (unsigned long long*)nullptr, ctrl);
+  return fused;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -234,17 +298,6 @@ void launch_next_delta_reweight(const float* S, int N, float ess_target, double 
 // integer scan C_i, T = C_{N-1}.  Integer addition is associative, so the result is the same
 // for every scan shape: one CTA, each thread a contiguous run, warp-shuffle scan of the run sums.
 // ---------------------------------------------------------------------------------------------
-// floor(w 2^40) for an fp32 w in [0, 1], from the bits: w = m 2^(e-150), so q = m 2^(e-110).
-// Exact (reading R5: identical to floor((double)w * 2^40)).
-__device__ __forceinline__ unsigned long long quantise40(float w) {
-  const uint32_t b = __float_as_uint(w);
-  const int e = (int)((b >> 23) & 0xffu);
-  if (e == 0 || (b >> 31)) return 0ull;                       // zero, subnormal (< 2^-126) or negative
-  const unsigned long long m = (unsigned long long)((b & 0x7fffffu) | 0x800000u);
-  const int sh = e - 110;
-  return sh >= 0 ? (m << sh) : (sh > -24 ? (m >> (-sh)) : 0ull);
-}
-
 __global__ void __launch_bounds__(1024)
 quantise_scan_kernel(const float* __restrict__ w, int N, unsigned long long* __restrict__ C,
                      Ctrl* ctrl) {
