@@ -141,26 +141,43 @@ syrk_partial_kernel(const float* __restrict__ phi, int N, int ld, int V,
     }
 }
 
-// Sigma[x][y] = Sigma[y][x] = (sum_z partial[z][x][y]) / (N-1) for y <= x, fixed summation order:
-// eight lanes per entry each sum every eighth split, then a fixed shuffle tree.
+// Sigma[x][y] = Sigma[y][x] = (sum_z partial[z][x][y]) / (N-1) for y <= x, fixed summation order.
+// LANES = 8 (small V: few entries, many splits): eight lanes per entry each sum every eighth split,
+// then a fixed shuffle tree.  LANES = 1 (large V): one thread per entry, coalesced along y.
+template <int LANES>
 __global__ void syrk_reduce_kernel(const float* __restrict__ partial, int nsplit, int V, int N,
                                    float* __restrict__ Sigma, const Ctrl* ctrl, int respect_done) {
   pdl_enter();
   if (respect_done && ctrl->done) return;
-  const int t = blockIdx.x * blockDim.x + threadIdx.x;
-  const int idx = t >> 3, part = t & 7;
-  const bool in = idx < V * V;
-  const int x = in ? idx / V : 0, y = in ? idx - x * V : 1;
+  const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const size_t idx = t / LANES;
+  const int part = (int)(t % LANES);
+  const bool in = idx < (size_t)V * V;
+  const int x = in ? (int)(idx / V) : 0, y = in ? (int)(idx - (size_t)x * V) : 1;
   float a = 0.f;
   if (in && y <= x)
-    for (int z = part; z < nsplit; z += 8) a += partial[(size_t)z * V * V + idx];
-  a += __shfl_xor_sync(0xffffffffu, a, 1);
-  a += __shfl_xor_sync(0xffffffffu, a, 2);
-  a += __shfl_xor_sync(0xffffffffu, a, 4);
+    for (int z = part; z < nsplit; z += LANES) a += partial[(size_t)z * V * V + idx];
+  if (LANES == 8) {
+    a += __shfl_xor_sync(0xffffffffu, a, 1);
+    a += __shfl_xor_sync(0xffffffffu, a, 2);
+    a += __shfl_xor_sync(0xffffffffu, a, 4);
+  }
   if (!in || y > x || part) return;
   a /= (float)(N - 1);
   Sigma[(size_t)x * V + y] = a;
   Sigma[(size_t)y * V + x] = a;
+}
+
+static void launch_syrk_reduce(const float* partial, int nsplit, int V, int N, float* Sigma,
+                               const Ctrl* ctrl, int respect_done, cudaStream_t st) {
+  ++g_launches;
+  const size_t e = (size_t)V * V;
+  if (V <= 128)
+    launch_pdl(syrk_reduce_kernel<8>, (unsigned)((8 * e + 255) / 256), 256, 0, st, partial, nsplit, V, N,
+               Sigma, ctrl, respect_done);
+  else
+    launch_pdl(syrk_reduce_kernel<1>, (unsigned)((e + 255) / 256), 256, 0, st, partial, nsplit, V, N, Sigma,
+               ctrl, respect_done);
 }
 
 __global__ void __launch_bounds__(256)
@@ -463,8 +480,7 @@ void launch_cov_chol(const CovCholArgs& a, cudaStream_t st) {
   ++g_launches; launch_pdl(mean_kernel, V, 256, 0, st, a.phi, a.N, a.ld, a.mu, a.ctrl, a.respect_done);
   if (a.tc_scratch && syrk_tc_supported(V, a.ld)) {
     launch_syrk_tc(a.phi, a.N, a.ld, V, a.mu, a.tc_scratch, a.partial, a.ctrl, a.respect_done, st);
-    ++g_launches; launch_pdl(syrk_reduce_kernel, (8 * V * V + 255) / 256, 256, 0, st, 
-        a.partial, syrk_tc_nsplit(V, a.ld), V, a.N, a.Sigma, a.ctrl, a.respect_done);
+    launch_syrk_reduce(a.partial, syrk_tc_nsplit(V, a.ld), V, a.N, a.Sigma, a.ctrl, a.respect_done, st);
     launch_cholesky(a.Sigma, a.Lc, V, a.ctrl, a.respect_done, st);
     return;
   }
@@ -475,8 +491,7 @@ void launch_cov_chol(const CovCholArgs& a, cudaStream_t st) {
   dim3 grid(nt * (nt + 1) / 2, ns);
   ++g_launches; launch_pdl(syrk_partial_kernel, grid, 256, 0, st, a.phi, a.N, a.ld, V, a.mu, a.partial, chunk, a.ctrl,
                                             a.respect_done);
-  ++g_launches; launch_pdl(syrk_reduce_kernel, (8 * V * V + 255) / 256, 256, 0, st, a.partial, ns, V, a.N, a.Sigma, a.ctrl,
-                                                          a.respect_done);
+  launch_syrk_reduce(a.partial, ns, V, a.N, a.Sigma, a.ctrl, a.respect_done, st);
   launch_cholesky(a.Sigma, a.Lc, V, a.ctrl, a.respect_done, st);
 }
 

@@ -116,6 +116,7 @@ __device__ __forceinline__ void site_diff(float a, float b, float c, float a2, f
 // Block = 32 particles x 8 row groups (one warp per group).  Phase 1: partial dS, dU0 over the
 // group's lattice rows.  Phase 2: warp 0 decides (R4 margin; NS: also S' < S_star).  Phase 3:
 // every group commits its rows of the accepted particles.
+template <bool IRMH>
 __global__ void __launch_bounds__(256)
 accept_kernel(float* __restrict__ phi, const float* __restrict__ phip, float* __restrict__ S,
               float* __restrict__ U0, int N, int ld, Model md, int mode, uint64_t seed,
@@ -123,7 +124,7 @@ accept_kernel(float* __restrict__ phi, const float* __restrict__ phip, float* __
               float* __restrict__ margin_out, int respect_done, const float* __restrict__ Z,
               float* __restrict__ W2) {
   if (respect_done && ctrl->done) return;
-  __shared__ float ps[8][32], pu[8][32], pz[8][32];
+  __shared__ float ps[8][32], pu[8][32], pz[IRMH ? 8 : 1][32];
   __shared__ int flag[32];
   const int lane = threadIdx.x & 31, g = threadIdx.x >> 5;
   const int i = blockIdx.x * 32 + lane;
@@ -134,7 +135,7 @@ accept_kernel(float* __restrict__ phi, const float* __restrict__ phip, float* __
   const int band = (L + 7) >> 3, r_lo = g * band, r_hi = min(L, r_lo + band);
   float dS = 0.f, dU = 0.f, z2 = 0.f;
   if (i < N) {
-    if (mode == MODE_IRMH) {          // |z|^2 of this band: log q(phi') = -1/2 |z|^2 + const
+    if (IRMH) {                       // |z|^2 of this band: log q(phi') = -1/2 |z|^2 + const
       for (int x = r_lo * L; x < r_hi * L; ++x) {
         const float z = Z[(size_t)x * ld + i];
         z2 = fmaf(z, z, z2);
@@ -159,7 +160,7 @@ accept_kernel(float* __restrict__ phi, const float* __restrict__ phip, float* __
   }
   ps[g][lane] = dS;
   pu[g][lane] = dU;
-  pz[g][lane] = z2;
+  if (IRMH) pz[g][lane] = z2;
   __syncthreads();
   if (g == 0) {
     int acc = 0;
@@ -169,10 +170,10 @@ accept_kernel(float* __restrict__ phi, const float* __restrict__ phip, float* __
       for (int m = 0; m < 8; ++m) { tS += ps[m][lane]; tU += pu[m][lane]; }
       float lu = log_uniform(seed, tag_acc, t, (uint32_t)i);
       float Si = S[i], margin;
-      if (mode == MODE_SMC) {
+      if (!IRMH && mode == MODE_SMC) {
         margin = -(tU + (float)ctrl->beta * tS) - lu;
         acc = margin > 0.f;
-      } else if (mode == MODE_IRMH) {
+      } else if (IRMH) {
         float tZ = 0.f;
 #pragma unroll
         for (int m = 0; m < 8; ++m) tZ += pz[m][lane];
@@ -226,7 +227,7 @@ void launch_mutate_generic(const MutateArgs& a, float* Lsplit, cudaStream_t st) 
       ++g_launches; propose_kernel<<<gp, 256, 0, st>>>(a.Lc, a.Z, a.phi, a.phip, V, a.ld, a.s, nullptr,
                                          a.ctrl, a.respect_done);
     }
-    ++g_launches; accept_kernel<<<a.ld / 32, 256, 0, st>>>(
+    ++g_launches; accept_kernel<false><<<a.ld / 32, 256, 0, st>>>(
         a.phi, a.phip, a.S, a.U0, a.N, a.ld, a.md, a.mode, a.seed, a.tag_acc, t, a.ctrl,
         a.acc_out ? a.acc_out + (size_t)j * a.N : nullptr,
         a.margin_out ? a.margin_out + (size_t)j * a.N : nullptr, a.respect_done, nullptr, nullptr);
@@ -278,7 +279,7 @@ void launch_mutate_irmh(const MutateArgs& a, const float* mu, float* W2, cudaStr
                                        a.respect_done);
     ++g_launches; propose_kernel<<<gp, 256, 0, st>>>(a.Lc, a.Z, a.phi, a.phip, V, a.ld, 1.0f, mu,
                                        a.ctrl, a.respect_done);
-    ++g_launches; accept_kernel<<<a.ld / 32, 256, 0, st>>>(
+    ++g_launches; accept_kernel<true><<<a.ld / 32, 256, 0, st>>>(
         a.phi, a.phip, a.S, a.U0, a.N, a.ld, a.md, MODE_IRMH, a.seed, a.tag_acc, t, a.ctrl,
         a.acc_out ? a.acc_out + (size_t)j * a.N : nullptr,
         a.margin_out ? a.margin_out + (size_t)j * a.N : nullptr, a.respect_done, a.Z, W2);
