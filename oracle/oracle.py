@@ -84,6 +84,13 @@ def lib():
         "orc_smc_hmc_run": (C.c_int, [C.c_int, C.c_double, C.c_double, C.c_int, C.c_uint64, C.c_int,
                                       C.c_double, C.c_double, C.c_int, C.c_int, _dp, _dp, _dp,
                                       C.POINTER(C.c_double), vp]),
+        "orc_ns_run_inner": (C.c_int, [C.c_int, C.c_double, C.c_double, C.c_int, C.c_int, C.c_int,
+                                       C.c_uint64, C.c_double, C.c_double, C.c_int, C.c_int,
+                                       C.c_double, C.c_int, C.c_int, _dp, _dp, _dp,
+                                       C.POINTER(C.c_double), C.POINTER(C.c_double), vp, vp, vp, vp]),
+        "orc_slice_walk": (None, [_dp, _dp, _dp, C.c_int, C.c_int, C.c_double, C.c_double, _dp,
+                                  C.c_double, C.c_int, C.c_int, C.c_double, C.c_uint64, C.c_uint32,
+                                  C.c_int, vp, vp, vp, vp, vp]),
         "orc_irmh_mutate": (None, [_dp, _dp, _dp, C.c_int, C.c_int, C.c_double, C.c_double, _dp, _dp,
                                    C.c_double, C.c_uint64, C.c_uint32, C.c_int, vp, vp, vp]),
         "orc_smc_irmh_run": (C.c_int, [C.c_int, C.c_double, C.c_double, C.c_int, C.c_uint64, C.c_int,
@@ -117,6 +124,11 @@ def philox(ctr, key):
     out = np.zeros(4, np.uint32)
     lib().orc_philox4x32_10(np.asarray(ctr, np.uint32), np.asarray(key, np.uint32), out)
     return out
+
+
+def draw(seed, tag, t, i, q):
+    """The four raw words of the R1 draw (c0, c1, c2, c3) = (q, i, t, tag) under key seed."""
+    return [int(v) for v in philox([q, i, t, tag], [seed & 0xFFFFFFFF, seed >> 32])]
 
 
 def normals(seed, tag, t, i, V):
@@ -310,15 +322,17 @@ NS_INFO = ("logX", "logZ", "S_star", "accept_rate", "remaining_frac", "chol_stat
 
 
 def ns_run(L, m0sq, lam, n_live, k_del, n_walk, seed, step_scale=0.0, stop_frac=1e-3,
-           max_iter=100000):
+           max_iter=100000, inner="rw", slice_w=1.0, m_expand=8, max_shrink=32):
+    """inner = "rw": constrained random walk (reading A5); "slice": slice sampling (reading A16)."""
     V = L * L
     phi, S, U0 = np.zeros((V, n_live)), np.zeros(n_live), np.zeros(n_live)
     info = np.zeros((max_iter, 6))
     dS, dM, dW = (np.zeros(max_iter * k_del) for _ in range(3))
     logZ, logX = C.c_double(0.0), C.c_double(0.0)
-    it = lib().orc_ns_run(L, m0sq, lam, n_live, k_del, n_walk, seed, step_scale, stop_frac,
-                          max_iter, phi, S, U0, C.byref(logZ), C.byref(logX), _ptr(dS), _ptr(dM),
-                          _ptr(dW), _ptr(info))
+    it = lib().orc_ns_run_inner(L, m0sq, lam, n_live, k_del, n_walk, seed, step_scale, stop_frac,
+                                max_iter, {"rw": 0, "slice": 1}[inner], slice_w, m_expand,
+                                max_shrink, phi, S, U0, C.byref(logZ), C.byref(logX), _ptr(dS),
+                                _ptr(dM), _ptr(dW), _ptr(info))
     if it < 0:
         raise RuntimeError("oracle NS: covariance not positive definite")
     n = it * k_del
@@ -381,3 +395,21 @@ def smc_irmh_run(L, m0sq, lam, N, seed, k, ess_target=0.5, max_temps=4096):
     if T < 0:
         raise RuntimeError("oracle SMC-IRMH: covariance not positive definite")
     return {"T": T, "logZ": logZ.value, "phi": phi, "S": S, "U0": U0, "info": info[:T]}
+
+
+# ---------------------------------------------------------------- NEXT row f3: NS slice ----
+def slice_walk(phi, S, U0, L, m0sq, lam, Lc, S_star, seed, t0, k, width=1.0, m_expand=8,
+               max_shrink=32, slots=None):
+    """k constrained slice-sampling steps (reading A16) on copies; returns
+    (phi, S, U0, t[k,N], n_expand[k,N], n_shrink[k,N], amb[k,N])."""
+    phi, S, U0 = _f64(phi).copy(), _f64(S).copy(), _f64(U0).copy()
+    V, N = phi.shape
+    if slots is not None:
+        slots = np.ascontiguousarray(slots, np.int32)
+    t = np.zeros((k, N))
+    nexp, nshr = np.zeros((k, N), np.int32), np.zeros((k, N), np.int32)
+    amb = np.zeros((k, N))
+    lib().orc_slice_walk(phi, S, U0, N, L, m0sq, lam, _f64(Lc), width, m_expand, max_shrink,
+                         S_star, seed, t0, k, _ptr(t), _ptr(nexp), _ptr(nshr), _ptr(amb),
+                         _ptr(slots))
+    return phi, S, U0, t, nexp, nshr, amb

@@ -593,11 +593,22 @@ static double orc_log_mean_like(const double* S, int n) {
  * {logX, logZ so far, S_star, accept rate, remaining fraction, chol status}.
  * Returns the number of iterations done, or -1.
  * ---------------------------------------------------------------------- */
-int orc_ns_run(int L, double m0sq, double lam, int n, int k_del, int n_walk,
-               uint64_t seed, double step_scale, double stop_frac,
-               int max_iter, double* phi, double* S, double* U0,
-               double* logZ_out, double* logX_out, double* dead_S,
-               double* dead_M, double* dead_logw, double* info) {
+void orc_slice_walk(double* phi, double* S, double* U0, int N, int L,
+                    double m0sq, double lam, const double* Lc, double width,
+                    int m_expand, int max_shrink, double S_star, uint64_t seed,
+                    uint32_t t0, int k, double* t_out, int32_t* nexp_out,
+                    int32_t* nshr_out, double* amb_out, const int32_t* slots);
+
+/* inner = 0: the constrained random walk of reading A5 (orc_mutate, MODE_NS);
+ * inner = 1: the slice-sampling kernel of reading A16 (orc_slice_walk) with
+ * bracket width slice_w, m_expand stepping-out moves, max_shrink shrinkages;
+ * info[3] is then the fraction of steps that moved. */
+int orc_ns_run_inner(int L, double m0sq, double lam, int n, int k_del, int n_walk,
+                     uint64_t seed, double step_scale, double stop_frac,
+                     int max_iter, int inner, double slice_w, int m_expand,
+                     int max_shrink, double* phi, double* S, double* U0,
+                     double* logZ_out, double* logX_out, double* dead_S,
+                     double* dead_M, double* dead_logw, double* info) {
   int V = L * L;
   double s = step_scale > 0.0 ? step_scale : 2.38 / sqrt((double)V);
   double* Sigma = (double*)malloc(sizeof(double) * (size_t)V * V);
@@ -644,10 +655,20 @@ int orc_ns_run(int L, double m0sq, double lam, int n, int k_del, int n_walk,
       wS[j] = S[src];
       wU[j] = U0[src];
     }
-    orc_mutate(wphi, wS, wU, k_del, L, m0sq, lam, Lc, s, 0.0, ORC_MODE_NS,
-               S_star, seed, ORC_TAG_NS_PROP, ORC_TAG_NS_ACC,
-               (uint32_t)it * (uint32_t)n_walk + 1u, n_walk, acc, NULL, NULL,
-               NULL);
+    if (inner == 0) {
+      orc_mutate(wphi, wS, wU, k_del, L, m0sq, lam, Lc, s, 0.0, ORC_MODE_NS,
+                 S_star, seed, ORC_TAG_NS_PROP, ORC_TAG_NS_ACC,
+                 (uint32_t)it * (uint32_t)n_walk + 1u, n_walk, acc, NULL, NULL,
+                 NULL);
+    } else {
+      double* tt = (double*)malloc(sizeof(double) * (size_t)n_walk * k_del);
+      orc_slice_walk(wphi, wS, wU, k_del, L, m0sq, lam, Lc, slice_w, m_expand,
+                     max_shrink, S_star, seed,
+                     (uint32_t)it * (uint32_t)n_walk + 1u, n_walk, tt, NULL,
+                     NULL, NULL, NULL);
+      for (size_t m = 0; m < (size_t)n_walk * k_del; ++m) acc[m] = tt[m] != 0.0;
+      free(tt);
+    }
     for (int j = 0; j < k_del; ++j) {
       int d = dead[j];
       for (int x = 0; x < V; ++x)
@@ -675,6 +696,16 @@ int orc_ns_run(int L, double m0sq, double lam, int n, int k_del, int n_walk,
   free(Sigma); free(Lc); free(wphi); free(wS); free(wU); free(dead);
   free(surv); free(isdead); free(acc);
   return rc < 0 ? rc : it;
+}
+
+int orc_ns_run(int L, double m0sq, double lam, int n, int k_del, int n_walk,
+               uint64_t seed, double step_scale, double stop_frac,
+               int max_iter, double* phi, double* S, double* U0,
+               double* logZ_out, double* logX_out, double* dead_S,
+               double* dead_M, double* dead_logw, double* info) {
+  return orc_ns_run_inner(L, m0sq, lam, n, k_del, n_walk, seed, step_scale,
+                          stop_frac, max_iter, 0, 0.0, 0, 0, phi, S, U0, logZ_out,
+                          logX_out, dead_S, dead_M, dead_logw, info);
 }
 
 /* ------------------------------------------------------------------------
@@ -946,4 +977,110 @@ int orc_smc_irmh_run(int L, double m0sq, double lam, int N, uint64_t seed, int k
   *logZ_out = logZ;
   free(tmp); free(Sigma); free(Lc); free(mu); free(w); free(anc); free(acc);
   return rc < 0 ? rc : T;
+}
+
+/* ------------------------------------------------------------------------
+ * NEXT row f3 -- the slice-sampling inner kernel of nested sampling
+ * (PAPER.md:53(iv), :174: "slice-sampling kernel (also tuned using the
+ * particle covariance)", "bracketing and shrinkage"; ref [47]).  Reading A16
+ * (DESIGN.md), one step of a walker at phi with S_E(phi) < S_star:
+ *   1. direction d = Lc z, z = NS_PROP-stream normals (tag 5, same keying as
+ *      orc_mutate); the particle covariance sets the scale of d.
+ *   2. one draw of the NS_SLICE stream (tag 7, c0 = 0): height
+ *      u_h = (w0>>8 + 1) 2^-24, bracket offset u_b = (w1>>8) 2^-24, stepping-out
+ *      split u_j = (w2>>8) 2^-24.  log y = -U0(phi) + ln u_h.
+ *      Inside(t) <=> S_E(phi + t d) < S_star and -U0(phi + t d) > log y
+ *      (slice of the reference density N(0,I) under the hard constraint).
+ *   3. bracket l = -width u_b, r = l + width; stepping out (Neal 2003, Fig. 3):
+ *      J = floor(m_expand u_j), K = m_expand - 1 - J; while J > 0 and Inside(l):
+ *      l -= width, --J; while K > 0 and Inside(r): r += width, --K.
+ *   4. shrinkage: for i = 0 .. max_shrink-1: u_i = ((w>>8) + 0.5) 2^-24 from
+ *      word i%4 of draw c0 = 1 + i/4; t = l + u_i (r - l); if Inside(t): move,
+ *      phi <- phi + t d, stop; else l = t if t < 0 else r = t.  No move after
+ *      max_shrink failures (t = 0).
+ * Outputs per (step, walker): t (0 = no move), expansions, shrinkages used and
+ * amb = the smallest |S_star - S_E| or |-U0 - log y| met in any Inside test
+ * (how close the nearest decision was to flipping).
+ * ---------------------------------------------------------------------- */
+#define ORC_TAG_NS_SLICE 7u
+
+typedef struct {
+  const double* f; const double* d; double* tmp;
+  int L; double m0sq, lam, S_star, logy, amb, S_last, U_last;
+} orc_slice_ctx;
+
+static int orc_slice_inside(orc_slice_ctx* c, double t) {
+  int V = c->L * c->L;
+  for (int x = 0; x < V; ++x) c->tmp[x] = c->f[x] + t * c->d[x];
+  double Sx = orc_action_field(c->tmp, c->L, c->m0sq, c->lam, NULL);
+  double Ux = orc_u0_field(c->tmp, V);
+  double a1 = fabs(c->S_star - Sx), a2 = fabs(-Ux - c->logy);
+  if (a1 < c->amb) c->amb = a1;
+  if (a2 < c->amb) c->amb = a2;
+  c->S_last = Sx; c->U_last = Ux;
+  return Sx < c->S_star && -Ux > c->logy;
+}
+
+void orc_slice_walk(double* phi, double* S, double* U0, int N, int L,
+                    double m0sq, double lam, const double* Lc, double width,
+                    int m_expand, int max_shrink, double S_star, uint64_t seed,
+                    uint32_t t0, int k, double* t_out, int32_t* nexp_out,
+                    int32_t* nshr_out, double* amb_out, const int32_t* slots) {
+  int V = L * L;
+#pragma omp parallel
+  {
+    double* f = (double*)malloc(sizeof(double) * V);
+    double* d = (double*)malloc(sizeof(double) * V);
+    double* z = (double*)malloc(sizeof(double) * V);
+    double* tmp = (double*)malloc(sizeof(double) * V);
+#pragma omp for
+    for (int i = 0; i < N; ++i) {
+      orc_get_field(phi, N, V, i, f);
+      double Si = S[i], Ui = U0[i];
+      const uint32_t slot = slots ? (uint32_t)slots[i] : (uint32_t)i;
+      for (int j = 0; j < k; ++j) {
+        uint32_t t = t0 + (uint32_t)j;
+        orc_normals(seed, ORC_TAG_NS_PROP, t, slot, V, z);
+        for (int x = 0; x < V; ++x) {
+          double a = 0.0;
+          for (int y = 0; y <= x; ++y) a += Lc[(size_t)x * V + y] * z[y];
+          d[x] = a;
+        }
+        uint32_t w[4];
+        orc_draw(seed, ORC_TAG_NS_SLICE, t, slot, 0u, w);
+        double u_h = ((double)(w[0] >> 8) + 1.0) * (1.0 / 16777216.0);
+        double u_b = (double)(w[1] >> 8) * (1.0 / 16777216.0);
+        double u_j = (double)(w[2] >> 8) * (1.0 / 16777216.0);
+        orc_slice_ctx c = {f, d, tmp, L, m0sq, lam, S_star, -Ui + log(u_h), INFINITY, Si, Ui};
+        double l = -width * u_b, r = l + width;
+        int J = (int)floor((double)m_expand * u_j), K = m_expand - 1 - J, nexp = 0;
+        while (J > 0 && orc_slice_inside(&c, l)) { l -= width; --J; ++nexp; }
+        while (K > 0 && orc_slice_inside(&c, r)) { r += width; --K; ++nexp; }
+        double tacc = 0.0;
+        int nshr = 0;
+        for (int m = 0; m < max_shrink; ++m) {
+          if ((m & 3) == 0) orc_draw(seed, ORC_TAG_NS_SLICE, t, slot, 1u + (uint32_t)(m >> 2), w);
+          double u = ((double)(w[m & 3] >> 8) + 0.5) * (1.0 / 16777216.0);
+          double tt = l + u * (r - l);
+          if (orc_slice_inside(&c, tt)) {
+            tacc = tt;
+            for (int x = 0; x < V; ++x) f[x] += tt * d[x];
+            Si = c.S_last; Ui = c.U_last;
+            break;
+          }
+          ++nshr;
+          if (tt < 0.0) l = tt; else r = tt;
+        }
+        size_t o = (size_t)j * N + i;
+        if (t_out) t_out[o] = tacc;
+        if (nexp_out) nexp_out[o] = nexp;
+        if (nshr_out) nshr_out[o] = nshr;
+        if (amb_out) amb_out[o] = c.amb;
+      }
+      orc_put_field(phi, N, V, i, f);
+      S[i] = Si;
+      U0[i] = Ui;
+    }
+    free(f); free(d); free(z); free(tmp);
+  }
 }
