@@ -65,6 +65,18 @@ typedef struct {
   int hmc_leapfrog;
 } smc_params;
 
+/* Inner kernel of nested sampling (PAPER.md:53(iv), :174).  inner = 0: constrained random walk of
+ * n_walk steps (reading A5, the BASELINE.json configuration).  inner = 1: slice sampling along
+ * covariance-drawn directions (reading A16): bracket of slice_width > 0 placed at random, at most
+ * max_expand - 1 stepping-out moves (1..64), at most max_shrink shrinkages (1..256) per step;
+ * n_walk is then the number of slice steps and accept_rate the fraction of steps that moved.   */
+typedef struct {
+  int inner;
+  float slice_width;
+  int max_expand;
+  int max_shrink;
+} ns_params;
+
 /* One tempering transition, filled when smc_step is given a non-NULL pointer. */
 typedef struct {
   double beta;        /* inverse temperature after the step                                      */
@@ -163,6 +175,7 @@ int ns_init(phi4smc** out, int L, float m0sq, float lambda, int n_live, int k_de
             uint64_t seed, double stop_frac, int max_iters, void* d_workspace,
             size_t workspace_bytes, void* cuda_stream);
 /* One iteration N1-N4.  info != NULL synchronises.  No-op once done.              */
+int ns_set_params(phi4smc* h, const ns_params* p); /* defaults: inner 0, width 1, 8, 32          */
 int ns_step(phi4smc* h, ns_step_info* info);
 int ns_run(phi4smc* h, int max_iters, int* n_iters); /* until done; synchronises                 */
 

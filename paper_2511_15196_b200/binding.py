@@ -31,6 +31,11 @@ class smc_params(C.Structure):
                 ("hmc_leapfrog", C.c_int)]
 
 
+class ns_params(C.Structure):
+    _fields_ = [("inner", C.c_int), ("slice_width", C.c_float), ("max_expand", C.c_int),
+                ("max_shrink", C.c_int)]
+
+
 class smc_step_info(C.Structure):
     _fields_ = [("beta", C.c_double), ("delta", C.c_double), ("ess_frac", C.c_double),
                 ("dlogZ", C.c_double), ("logZ", C.c_double), ("accept_rate", C.c_double),
@@ -80,6 +85,7 @@ SIGNATURES = {
     "log_Z": (_d, [_vp]),
     "ns_workspace_bytes": (_sz, [_i, _i, _i, _i]),
     "ns_init": (_i, [C.POINTER(_vp), _i, _f, _f, _i, _i, _i, _u64, _d, _i, _vp, _sz, _vp]),
+    "ns_set_params": (_i, [_vp, C.POINTER(ns_params)]),
     "ns_step": (_i, [_vp, C.POINTER(ns_step_info)]),
     "ns_run": (_i, [_vp, _i, C.POINTER(_i)]),
     "smc_get_state": (_i, [_vp, _vp, _vp, _vp, C.POINTER(_d), C.POINTER(_u64)]),
@@ -258,6 +264,11 @@ def log_Z(h):
     if math.isnan(v):
         raise Phi4Error(-5, "log_Z")
     return v
+
+
+def ns_set_params(h, inner=0, slice_width=1.0, max_expand=8, max_shrink=32):
+    p = ns_params(inner, slice_width, max_expand, max_shrink)
+    h._check(load().ns_set_params(h.ptr, C.byref(p)), "ns_set_params")
 
 
 def ns_step(h, want_info=True):

@@ -40,6 +40,7 @@ struct phi4smc {
   int N, ld;                 // particles (n_live for NS) and padded stride
   uint64_t seed;
   smc_params prm;
+  ns_params nsp;
   float s;                   // step scale actually used
   cudaStream_t st;
   // device state (inside the workspace)
@@ -164,6 +165,7 @@ static phi4smc* new_handle(int kind, int L, float m0sq, float lambda, int N, uin
   h->seed = seed;
   h->prm.k_steps = 10; h->prm.ess_target = 0.5f; h->prm.step_scale = 0.f; h->prm.mutation_path = 0;
   h->prm.kernel = 0; h->prm.hmc_eps = 0.1f; h->prm.hmc_leapfrog = 20;
+  h->nsp.inner = 0; h->nsp.slice_width = 1.0f; h->nsp.max_expand = 8; h->nsp.max_shrink = 32;
   h->s = 2.38f / sqrtf((float)h->md.V);
   return h;
 }
@@ -580,10 +582,21 @@ static void enqueue_ns_step(phi4smc* h) {
   m.N = h->k_del; m.ld = h->ldw; m.md = h->md; m.s = h->s; m.mode = MODE_NS; m.seed = h->seed;
   m.tag_prop = TAG_NS_PROP; m.tag_acc = TAG_NS_ACC;
   m.t0 = h->iters_enqueued * (uint32_t)h->n_walk + 1u; m.k = h->n_walk; m.respect_done = 1;
-  enqueue_mutation(h, m);
+  if (h->nsp.inner == 1) launch_ns_slice(m, h->nsp.slice_width, h->nsp.max_expand, h->nsp.max_shrink, h->st);
+  else enqueue_mutation(h, m);
   launch_ns_store_walkers(a, h->st);
   launch_ns_finish(a, h->rec, h->n_walk, h->st);
   h->iters_enqueued += 1;
+}
+
+PHI4_API int ns_set_params(phi4smc* h, const ns_params* p) {
+  if (!h || !p || h->kind != KIND_NS) return PHI4_EINVAL;
+  if (p->inner < 0 || p->inner > 1) return PHI4_EINVAL;
+  if (p->inner == 1 && (!(p->slice_width > 0.f) || p->max_expand < 1 || p->max_expand > 64 ||
+                        p->max_shrink < 1 || p->max_shrink > 256))
+    return PHI4_EINVAL;
+  h->nsp = *p;
+  return PHI4_OK;
 }
 
 static void fill_ns_info(const StepRecord& r, ns_step_info* info) {

@@ -37,6 +37,8 @@ struct MutateArgs {
   int respect_done;  // 1: every kernel is a no-op once ctrl->done is set
 };
 void launch_mutate_generic(const MutateArgs& a, float* Lsplit, cudaStream_t st);
+// NEXT f3: k constrained slice-sampling steps of the NS walkers (reading A16); a.phip = direction
+void launch_ns_slice(const MutateArgs& a, float width, int m_expand, int max_shrink, cudaStream_t st);
 // NEXT f2: k independent-MH steps from N(mu, Lc Lc^T) (reading A15); W2 [ld] scratch
 bool irmh_supported(int V);
 void launch_mutate_irmh(const MutateArgs& a, const float* mu, float* W2, cudaStream_t st);

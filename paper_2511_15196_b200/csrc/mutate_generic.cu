@@ -29,7 +29,7 @@ __global__ void normals_kernel(float* __restrict__ Z, int N, int ld, int V, uint
 __global__ void __launch_bounds__(256)
 propose_kernel(const float* __restrict__ Lc, const float* __restrict__ Z,
                const float* __restrict__ phi, float* __restrict__ phip, int V, int ld, float s,
-               const float* __restrict__ mu, const Ctrl* ctrl, int respect_done) {
+               const float* __restrict__ mu, int zero_base, const Ctrl* ctrl, int respect_done) {
   if (respect_done && ctrl->done) return;
   __shared__ float As[16][64 + 4];
   __shared__ __align__(16) float Bs[16][64];
@@ -90,8 +90,10 @@ propose_kernel(const float* __restrict__ Lc, const float* __restrict__ Z,
     if (x < V) {
       size_t o = (size_t)x * ld + i0 + tx * 4;
       // independent proposal (IRMH): the base point is the particle mean, not the particle
-      float4 f = mu ? make_float4(mu[x], mu[x], mu[x], mu[x])
-                    : *reinterpret_cast<const float4*>(phi + o);
+      // zero base (slice sampling): the output is the direction s * Lc z itself
+      float4 f = zero_base ? make_float4(0.f, 0.f, 0.f, 0.f)
+                 : mu      ? make_float4(mu[x], mu[x], mu[x], mu[x])
+                           : *reinterpret_cast<const float4*>(phi + o);
       f.x = fmaf(s, acc[p][0], f.x);
       f.y = fmaf(s, acc[p][1], f.y);
       f.z = fmaf(s, acc[p][2], f.z);
@@ -225,7 +227,7 @@ void launch_mutate_generic(const MutateArgs& a, float* Lsplit, cudaStream_t st) 
       ++g_launches; normals_kernel<<<gz, 128, 0, st>>>(a.Z, a.N, a.ld, V, a.seed, a.tag_prop, t, a.ctrl,
                                          a.respect_done);
       ++g_launches; propose_kernel<<<gp, 256, 0, st>>>(a.Lc, a.Z, a.phi, a.phip, V, a.ld, a.s, nullptr,
-                                         a.ctrl, a.respect_done);
+                                         0, a.ctrl, a.respect_done);
     }
     ++g_launches; accept_kernel<false><<<a.ld / 32, 256, 0, st>>>(
         a.phi, a.phip, a.S, a.U0, a.N, a.ld, a.md, a.mode, a.seed, a.tag_acc, t, a.ctrl,
@@ -278,11 +280,144 @@ void launch_mutate_irmh(const MutateArgs& a, const float* mu, float* W2, cudaStr
     ++g_launches; normals_kernel<<<gz, 128, 0, st>>>(a.Z, a.N, a.ld, V, a.seed, a.tag_prop, t, a.ctrl,
                                        a.respect_done);
     ++g_launches; propose_kernel<<<gp, 256, 0, st>>>(a.Lc, a.Z, a.phi, a.phip, V, a.ld, 1.0f, mu,
-                                       a.ctrl, a.respect_done);
+                                       0, a.ctrl, a.respect_done);
     ++g_launches; accept_kernel<true><<<a.ld / 32, 256, 0, st>>>(
         a.phi, a.phip, a.S, a.U0, a.N, a.ld, a.md, MODE_IRMH, a.seed, a.tag_acc, t, a.ctrl,
         a.acc_out ? a.acc_out + (size_t)j * a.N : nullptr,
         a.margin_out ? a.margin_out + (size_t)j * a.N : nullptr, a.respect_done, a.Z, W2);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// NEXT row f3: the slice-sampling inner kernel of nested sampling (PAPER.md:53(iv), :174; reading
+// A16).  Per step: normals_kernel, propose_kernel with a zero base (d = Lc z), slice_kernel.
+// Along the line phi + t d both S_E and U0 are polynomials in t (quartic / quadratic) whose
+// coefficients are eight lattice sums; every Inside(t) test of the stepping-out and shrinkage
+// loops is then O(1):
+//   U0(t)  = U0 + t A1 + t^2 A2/2,                      A1 = sum f d, A2 = sum d^2
+//   S_E(t) = S_E + t (K1 + m0^2 A1 + 4 lam Q1) + t^2 (K2/2 + m0^2 A2/2 + 6 lam Q2)
+//                + t^3 4 lam Q3 + t^4 lam Q4,
+//   K1 = sum_bonds (Df)(Dd), K2 = sum_bonds (Dd)^2, Q1..Q4 = sum f^3 d, f^2 d^2, f d^3, d^4.
+// Block = 32 walkers x 8 row groups: partial sums per group, warp 0 runs the (divergent) scalar
+// loops, every group then moves its rows of the walkers that found a point.
+__global__ void __launch_bounds__(256)
+slice_kernel(float* __restrict__ phi, const float* __restrict__ dir, float* __restrict__ S,
+             float* __restrict__ U0, int N, int ld, Model md, float width, int m_expand,
+             int max_shrink, uint64_t seed, uint32_t t, Ctrl* ctrl, int respect_done) {
+  if (respect_done && ctrl->done) return;
+  __shared__ float part[8][8][32];
+  __shared__ float tsel[32];
+  const int lane = threadIdx.x & 31, g = threadIdx.x >> 5;
+  const int i = blockIdx.x * 32 + lane;
+  const int L = md.L;
+  const int band = (L + 7) >> 3, r_lo = g * band, r_hi = min(L, r_lo + band);
+  float acc[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+  if (i < N) {
+    for (int r = r_lo; r < r_hi; ++r) {
+      const int rn = (r + 1 == L) ? 0 : r + 1;
+      const size_t ro = (size_t)r * L * ld + i, rno = (size_t)rn * L * ld + i;
+      float row[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};   // two-level fp32 accumulation
+      float f = phi[ro], d = dir[ro];
+      for (int c = 0; c < L; ++c) {
+        const int cn = (c + 1 == L) ? 0 : c + 1;
+        const float fe = phi[ro + (size_t)cn * ld], de = dir[ro + (size_t)cn * ld];
+        const float fs = phi[rno + (size_t)c * ld], ds = dir[rno + (size_t)c * ld];
+        const float dfe = fe - f, dde = de - d, dfs = fs - f, dds = ds - d;
+        const float f2 = f * f, d2 = d * d;
+        row[0] = fmaf(f, d, row[0]);
+        row[1] += d2;
+        row[2] += dfe * dde + dfs * dds;
+        row[3] += dde * dde + dds * dds;
+        row[4] = fmaf(f2 * f, d, row[4]);
+        row[5] = fmaf(f2, d2, row[5]);
+        row[6] = fmaf(f * d, d2, row[6]);
+        row[7] = fmaf(d2, d2, row[7]);
+        f = fe;
+        d = de;
+      }
+#pragma unroll
+      for (int q = 0; q < 8; ++q) acc[q] += row[q];
+    }
+  }
+#pragma unroll
+  for (int q = 0; q < 8; ++q) part[q][g][lane] = acc[q];
+  __syncthreads();
+  if (g == 0) {
+    float tacc = 0.f;
+    if (i < N) {
+      float v[8];
+#pragma unroll
+      for (int q = 0; q < 8; ++q) {
+        float a = 0.f;
+#pragma unroll
+        for (int m = 0; m < 8; ++m) a += part[q][m][lane];
+        v[q] = a;
+      }
+      const float lam = md.lam, m0 = md.m0sq;
+      const float c1 = v[2] + m0 * v[0] + 4.f * lam * v[4];
+      const float c2 = 0.5f * v[3] + 0.5f * m0 * v[1] + 6.f * lam * v[5];
+      const float c3 = 4.f * lam * v[6], c4 = lam * v[7];
+      const float u1 = v[0], u2 = 0.5f * v[1];
+      const float S0 = S[i], Ub = U0[i], S_star = (float)ctrl->S_star;
+      U4 w = philox_draw(seed, TAG_NS_SLICE, t, (uint32_t)i, 0u);
+      const float u_h = (float)((w.x >> 8) + 1u) * 5.9604644775390625e-8f;
+      const float u_b = (float)(w.y >> 8) * 5.9604644775390625e-8f;
+      const float u_j = (float)(w.z >> 8) * 5.9604644775390625e-8f;
+      const float logy = -Ub + logf(u_h);
+      float Sx = S0, Ux = Ub;
+      auto inside = [&](float tt) {
+        Sx = fmaf(tt, fmaf(tt, fmaf(tt, fmaf(tt, c4, c3), c2), c1), S0);
+        Ux = fmaf(tt, fmaf(tt, u2, u1), Ub);
+        return Sx < S_star && -Ux > logy;
+      };
+      float l = -width * u_b, r = l + width;
+      int J = (int)floorf((float)m_expand * u_j), K = m_expand - 1 - J;
+      while (J > 0 && inside(l)) { l -= width; --J; }
+      while (K > 0 && inside(r)) { r += width; --K; }
+      for (int m = 0; m < max_shrink; ++m) {
+        if ((m & 3) == 0) w = philox_draw(seed, TAG_NS_SLICE, t, (uint32_t)i, 1u + (uint32_t)(m >> 2));
+        const uint32_t wd = (m & 3) == 0 ? w.x : (m & 3) == 1 ? w.y : (m & 3) == 2 ? w.z : w.w;
+        const float u = ((float)(wd >> 8) + 0.5f) * 5.9604644775390625e-8f;
+        const float tt = fmaf(u, r - l, l);
+        if (inside(tt)) {
+          tacc = tt;
+          S[i] = Sx;
+          U0[i] = Ux;
+          break;
+        }
+        if (tt < 0.f) l = tt; else r = tt;
+      }
+    }
+    tsel[lane] = tacc;
+    const unsigned moved = __ballot_sync(0xffffffffu, tacc != 0.f);
+    if (lane == 0 && moved) atomicAdd(&ctrl->n_accept, (unsigned)__popc(moved));
+  }
+  __syncthreads();
+  const float tt = tsel[lane];
+  if (i < N && tt != 0.f) {
+    for (int r = r_lo; r < r_hi; ++r) {
+      const size_t ro = (size_t)r * L * ld + i;
+      for (int c = 0; c < L; ++c) {
+        const size_t o = ro + (size_t)c * ld;
+        phi[o] = fmaf(tt, dir[o], phi[o]);
+      }
+    }
+  }
+}
+
+// a.phip receives the direction; a.mode / a.s / acc_out / margin_out are unused
+void launch_ns_slice(const MutateArgs& a, float width, int m_expand, int max_shrink, cudaStream_t st) {
+  const int V = a.md.V;
+  dim3 gz((a.ld + 127) / 128, (V + 3) / 4);
+  dim3 gp(a.ld / 64, (V + 63) / 64);
+  for (int j = 0; j < a.k; ++j) {
+    const uint32_t t = a.t0 + (uint32_t)j;
+    ++g_launches; normals_kernel<<<gz, 128, 0, st>>>(a.Z, a.N, a.ld, V, a.seed, TAG_NS_PROP, t, a.ctrl,
+                                       a.respect_done);
+    ++g_launches; propose_kernel<<<gp, 256, 0, st>>>(a.Lc, a.Z, a.phi, a.phip, V, a.ld, 1.0f, nullptr, 1,
+                                       a.ctrl, a.respect_done);
+    ++g_launches; slice_kernel<<<a.ld / 32, 256, 0, st>>>(a.phi, a.phip, a.S, a.U0, a.N, a.ld, a.md, width,
+                                     m_expand, max_shrink, a.seed, t, a.ctrl, a.respect_done);
   }
 }
 

@@ -1,0 +1,121 @@
+"""GPU parity for the slice-sampling inner kernel of nested sampling (
+PAPER.md:53(iv), :174; reading A16): the CUDA path through the C ABI against the FP64 oracle.
+
+Tolerance.  The kernel evaluates S_E and U0 along the line phi + t d from polynomial coefficients
+in fp32, the oracle evaluates both directly in FP64; every stepping-out / shrinkage decision is a
+comparison of such a value against S_star or log y.  A walker is compared when the oracle's
+closest decision over all its steps was further than BAND_SLICE = 2e-3 from flipping (the
+oracle reports that distance); for those the whole decision sequence must agree, so the final
+fields agree to fp32 rounding."""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+from paper_2511_15196_b200 import binding as B
+from paper_2511_15196_b200 import build
+
+pytestmark = pytest.mark.gpu
+
+BAND_SLICE = 2e-3
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    build.build()
+    B.load()
+
+
+def gauss_a(L, m0sq):
+    k = np.arange(L)
+    kh = 4 * np.sin(np.pi * k / L) ** 2
+    return (m0sq + kh[:, None] + kh[None, :]).reshape(-1)
+
+
+@pytest.mark.parametrize("L,n,kd,nw,width,mexp", [(10, 4096, 512, 6, 1.0, 8), (4, 1024, 128, 8, 0.5, 4),
+                                                  (7, 600, 300, 5, 2.0, 8), (1, 256, 64, 6, 1.0, 8)])
+def test_slice_first_iteration_lockstep(L, n, kd, nw, width, mexp):
+    seed, m0sq, lam = 23 + L, -4.0, 1.0
+    h = B.ns_init(L, m0sq, lam, n, kd, nw, seed, max_iters=16)
+    B.ns_set_params(h, inner=1, slice_width=width, max_expand=mexp, max_shrink=32)
+    st0 = B.smc_get_state(h)
+    info = B.ns_step(h)
+    st1 = B.smc_get_state(h)
+    S0 = st0["S"].astype(np.float64)
+    dead = O.ns_select(S0, kd)
+    assert np.array_equal(B.ns_get_dead(h)["last_dead"], dead)
+    assert info["S_star"] == S0[dead[-1]]
+    Lc = B.smc_get_chol(h)
+    surv = np.setdiff1d(np.arange(n), dead)
+    start = np.array([surv[O.word0(seed, O.TAG_NS_START, 0, j) % (n - kd)] for j in range(kd)])
+    f0 = st0["phi"][:, start].astype(np.float64)
+    Ss, Us = O.action_batch(f0, L, m0sq, lam)
+    p, S, U0, t, nexp, nshr, amb = O.slice_walk(f0, Ss, Us, L, m0sq, lam, Lc, info["S_star"], seed, 1,
+                                                nw, width=np.float32(width), m_expand=mexp)
+    clean = amb.min(axis=0) > BAND_SLICE
+    assert clean.mean() > 0.6
+    got = st1["phi"][:, dead]
+    assert np.abs(got[:, clean] - p[:, clean]).max() < 1e-4
+    gS = st1["S"][dead]
+    A = O.action_batch(p, L, m0sq, lam, with_abs=True)[2]
+    assert np.all(np.abs(gS[clean] - S[clean]) <= 4e-5 * A[clean] + 1e-4)
+    assert np.all(st1["S"] < info["S_star"] + 1e-3)
+    keep = np.setdiff1d(np.arange(n), dead)
+    assert np.array_equal(st1["phi"][:, keep], st0["phi"][:, keep])          # survivors untouched
+    assert info["accept_rate"] == pytest.approx((t != 0).mean(), abs=0.02)
+    assert info["accept_rate"] > 0.8
+    h.close()
+
+
+def test_ns_set_params_validation():
+    h = B.ns_init(4, -4.0, 1.0, 256, 32, 5, 1, max_iters=8)
+    for bad in (dict(inner=2), dict(inner=1, slice_width=0.0), dict(inner=1, max_expand=0),
+                dict(inner=1, max_shrink=0), dict(inner=1, max_expand=65)):
+        with pytest.raises(B.Phi4Error):
+            B.ns_set_params(h, **bad)
+    h.close()
+    s = B.smc_init(4, -4.0, 1.0, 256, 1)
+    with pytest.raises(B.Phi4Error):
+        B.ns_set_params(s, inner=1)
+    s.close()
+
+
+def gpu_ns_slice(L, n, kd, nw, seed, m0sq=-4.0, lam=1.0, max_iters=4096):
+    h = B.ns_init(L, m0sq, lam, n, kd, nw, seed, max_iters=max_iters)
+    B.ns_set_params(h, inner=1)
+    it = B.ns_run(h, max_iters)
+    out = {"iters": it, "logZ": B.log_Z(h), "obs": B.observables(h)}
+    h.close()
+    return out
+
+
+def mean_se(v):
+    v = np.asarray(v, float)
+    return v.mean(), v.std(ddof=1) / math.sqrt(len(v))
+
+
+def test_ns_slice_gaussian_closed_form_and_oracle():
+    exact = -0.5 * np.sum(np.log1p(gauss_a(4, 1.0)))
+    g = [gpu_ns_slice(4, 1024, 128, 8, s, m0sq=1.0, lam=0.0) for s in range(8)]
+    m, se = mean_se([r["logZ"] for r in g])
+    assert abs(m - exact) < 3 * se + 0.02, (m, se)
+    o = [O.ns_run(4, 1.0, 0.0, 1024, 128, 8, s, inner="slice") for s in range(8)]
+    mo, so = mean_se([r["logZ"] for r in o])
+    assert abs(m - mo) < 3 * math.hypot(se, so) + 0.01
+    assert abs(np.mean([r["iters"] for r in g]) - np.mean([r["iters"] for r in o])) < 2.0
+    m2, s2 = mean_se([r["obs"]["M2"] for r in g])
+    assert abs(m2 - 1 / 32.0) < 4 * s2 + 5e-4
+
+
+def test_ns_slice_broken_phase_matches_oracle_and_the_walk_kernel():
+    L, n, kd, nw = 6, 2048, 1024, 10                  # the paper's delete fraction 0.5
+    g = [gpu_ns_slice(L, n, kd, nw, s) for s in range(4)]
+    o = [O.ns_run(L, -4.0, 1.0, n, kd, nw, s, inner="slice") for s in range(4)]
+    mg, sg = mean_se([r["logZ"] for r in g])
+    mo, so = mean_se([r["logZ"] for r in o])
+    assert abs(mg - mo) < 3 * math.hypot(sg, so) + 0.1, (mg, sg, mo, so)
+    ig, io = np.mean([r["iters"] for r in g]), np.mean([r["iters"] for r in o])
+    assert abs(ig - io) < 2.0
+    bal = np.mean([min(r["obs"]["mode_balance"], 1 / r["obs"]["mode_balance"]) for r in g])
+    assert bal > 0.5
