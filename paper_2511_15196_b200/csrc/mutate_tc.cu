@@ -28,7 +28,10 @@ namespace tc {
 
 constexpr int TILE = 128;            // particles per CTA = TMEM lanes
 constexpr int STAGES = 4;            // Z ring depth; one stage = two K-steps (K = 16)
-constexpr int EPI_FILLS = 2;         // ring stages per step filled by the epilogue warps (<= 2)
+// ring stages per step filled by the epilogue warps (measured per C1 temperature: 0 -> 242 us,
+// 1 -> 233, 2 -> 229, 3 -> 233)
+constexpr int EPI_FILLS = 2;
+static_assert(EPI_FILLS <= STAGES, "the epilogue fills of one step must fit the ring");
 constexpr int EPI_PARTS = 4;         // warps per TMEM lane quarter (sites split four ways)
 constexpr int EPI_WARPS = 4 * EPI_PARTS;
 constexpr int PROD_WARPS = 8;
@@ -209,8 +212,8 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int V = p.V, Vn = p.Vn, Kp = p.Kp, nk8 = Kp >> 3, nit = (nk8 + 1) >> 1;
-  // the last nitE ring fills of every step are produced by the epilogue warps (one quad per
-  // thread), the first nitP by the dedicated producers (two quads per thread)
+  // the first nitE ring fills of every step are produced by the epilogue warps (one quad per
+  // thread, two steps ahead), the other nitP by the dedicated producers (two quads per thread)
   const int nitE = min(EPI_FILLS, nit - 1), nitP = nit - nitE;
   const int i0 = blockIdx.x * TILE;
   uint32_t ncols = 32;
@@ -315,17 +318,17 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
         bool ok[4];
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
-          const int q = 4 * (it + (c >> 1)) + 2 * (c & 1) + half;   // stage it + c/2, chunk 2 (c%2) + half
+          const int q = 4 * (nitE + it + (c >> 1)) + 2 * (c & 1) + half;   // slab nitE + it + c/2, chunk 2 (c%2) + half
           ok[c] = (i < p.N) && (q < nq) && (c < 2 || second);
         }
         if (second) {
 #pragma unroll
           for (int c = 0; c < 4; ++c)
-            w[c] = philox4x32_10_rk((uint32_t)(4 * (it + (c >> 1)) + 2 * (c & 1) + half), (uint32_t)i, tt, p.tag_prop, p.rk);
+            w[c] = philox4x32_10_rk((uint32_t)(4 * (nitE + it + (c >> 1)) + 2 * (c & 1) + half), (uint32_t)i, tt, p.tag_prop, p.rk);
         } else {
 #pragma unroll
           for (int c = 0; c < 2; ++c)
-            w[c] = philox4x32_10_rk((uint32_t)(4 * it + 2 * c + half), (uint32_t)i, tt, p.tag_prop, p.rk);
+            w[c] = philox4x32_10_rk((uint32_t)(4 * (nitE + it) + 2 * c + half), (uint32_t)i, tt, p.tag_prop, p.rk);
           w[2] = w[0]; w[3] = w[1];
         }
         TC_TRACE(1, tr);
@@ -348,7 +351,7 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
             hv[e].z = tf32_rna(z[2]); lv[e].z = z[2] - hv[e].z;
             hv[e].w = tf32_rna(z[3]); lv[e].w = z[3] - hv[e].w;
           }
-          const int n = t * nit + it + st2, s = n % STAGES;    // ring slot and use of fill n
+          const int n = t * nit + nitE + it + st2, s = n % STAGES;    // ring slot and use of fill n
           const uint32_t ph = (uint32_t)(n / STAGES) & 1u;
           mbar_wait_relaxed(zempty(s), ph ^ 1);
           uint8_t* st = zr + (size_t)s * SLAB_BYTES + (size_t)half * CHUNK_BYTES + (size_t)pr * 16;
@@ -385,35 +388,40 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
     const int nq = (V + 3) >> 2;
     // this thread's share of the normals of step t: quad 4 it + g of its own particle row
     auto fill = [&](int t) {
-      // up to EPI_FILLS (= 2) stages: both Philox chains first, then the maps and the stores
-      U4 w[2];
+      // two stages per pass: both Philox chains first, then the maps and the stores
+      for (int e0 = 0; e0 < nitE; e0 += 2) {
+        U4 w[2];
 #pragma unroll
-      for (int e = 0; e < 2; ++e)
-        if (e < nitE) w[e] = philox4x32_10_rk((uint32_t)(4 * (nitP + e) + g), (uint32_t)i, p.t0 + (uint32_t)t, p.tag_prop, p.rk);
+        for (int e = 0; e < 2; ++e)
+          if (e0 + e < nitE) w[e] = philox4x32_10_rk((uint32_t)(4 * (e0 + e) + g), (uint32_t)i, p.t0 + (uint32_t)t, p.tag_prop, p.rk);
 #pragma unroll
-      for (int e = 0; e < 2; ++e) {
-        if (e >= nitE) break;
-        const int it = nitP + e, q = 4 * it + g;
-        float z[4] = {0.f, 0.f, 0.f, 0.f};
-        if (live && q < nq) {
-          box_muller_fast(w[e].x, w[e].y, z[0], z[1]);
-          box_muller_fast(w[e].z, w[e].w, z[2], z[3]);
+        for (int e = 0; e < 2; ++e) {
+          if (e0 + e >= nitE) break;
+          const int it = e0 + e, q = 4 * it + g;
+          float z[4] = {0.f, 0.f, 0.f, 0.f};
+          if (live && q < nq) {
+            box_muller_fast(w[e].x, w[e].y, z[0], z[1]);
+            box_muller_fast(w[e].z, w[e].w, z[2], z[3]);
+          }
+          float4 hv, lv;
+          hv.x = tf32_rna(z[0]); lv.x = z[0] - hv.x;  hv.y = tf32_rna(z[1]); lv.y = z[1] - hv.y;
+          hv.z = tf32_rna(z[2]); lv.z = z[2] - hv.z;  hv.w = tf32_rna(z[3]); lv.w = z[3] - hv.w;
+          const int n = t * nit + it, s = n % STAGES;
+          const uint32_t ph = (uint32_t)(n / STAGES) & 1u;
+          mbar_wait_relaxed(zempty(s), ph ^ 1);
+          uint8_t* st = zr + (size_t)s * SLAB_BYTES + (size_t)g * CHUNK_BYTES + (size_t)pr * 16;
+          *reinterpret_cast<float4*>(st) = hv;
+          *reinterpret_cast<float4*>(st + 4 * CHUNK_BYTES) = lv;
+          fence_proxy_async();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(zfull(s));
         }
-        float4 hv, lv;
-        hv.x = tf32_rna(z[0]); lv.x = z[0] - hv.x;  hv.y = tf32_rna(z[1]); lv.y = z[1] - hv.y;
-        hv.z = tf32_rna(z[2]); lv.z = z[2] - hv.z;  hv.w = tf32_rna(z[3]); lv.w = z[3] - hv.w;
-        const int n = t * nit + it, s = n % STAGES;
-        const uint32_t ph = (uint32_t)(n / STAGES) & 1u;
-        mbar_wait_relaxed(zempty(s), ph ^ 1);
-        uint8_t* st = zr + (size_t)s * SLAB_BYTES + (size_t)g * CHUNK_BYTES + (size_t)pr * 16;
-        *reinterpret_cast<float4*>(st) = hv;
-        *reinterpret_cast<float4*>(st + 4 * CHUNK_BYTES) = lv;
-        fence_proxy_async();
-        __syncwarp();
-        if (lane == 0) mbar_arrive(zfull(s));
       }
     };
+    // the epilogue warps produce the FIRST slabs of a step and run two steps ahead: the MMAs of
+    // step t + 1 then never wait for a warp that is itself waiting for the MMAs of step t
     fill(0);
+    if (p.k > 1) fill(1);
     int tr = (threadIdx.x == 0) ? 0 : 4096; (void)tr;
     for (int t = 0; t < p.k; ++t) {
       const int buf = t & 1;
@@ -494,7 +502,7 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
         if (p.acc_out) p.acc_out[(size_t)t * p.N + i] = (uint8_t)acc;
         if (p.margin_out) p.margin_out[(size_t)t * p.N + i] = margin;
       }
-      if (t + 1 < p.k) fill(t + 1);
+      if (t + 2 < p.k) fill(t + 2);
     }
     if (live) {
       for (int x = g; x < V; x += EPI_PARTS) p.phi[(size_t)x * p.ld + i] = cur[x * TILE];
