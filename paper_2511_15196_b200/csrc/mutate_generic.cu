@@ -118,15 +118,17 @@ __device__ __forceinline__ void site_diff(float a, float b, float c, float a2, f
 // Block = 32 particles x 8 row groups (one warp per group).  Phase 1: partial dS, dU0 over the
 // group's lattice rows.  Phase 2: warp 0 decides (R4 margin; NS: also S' < S_star).  Phase 3:
 // every group commits its rows of the accepted particles.
-template <bool IRMH>
-__global__ void __launch_bounds__(256)
+// G row groups (8 or 32 warps): a small population does not fill the GPU with 8-warp blocks and a
+// warp then walks a long band of rows with ~L2-latency per site; 32 groups shorten the band.
+template <bool IRMH, int G>
+__global__ void __launch_bounds__(32 * G)
 accept_kernel(float* __restrict__ phi, const float* __restrict__ phip, float* __restrict__ S,
               float* __restrict__ U0, int N, int ld, Model md, int mode, uint64_t seed,
               uint32_t tag_acc, uint32_t t, Ctrl* ctrl, uint8_t* __restrict__ acc_out,
               float* __restrict__ margin_out, int respect_done, const float* __restrict__ Z,
               float* __restrict__ W2) {
   if (respect_done && ctrl->done) return;
-  __shared__ float ps[8][32], pu[8][32], pz[IRMH ? 8 : 1][32];
+  __shared__ float ps[G][32], pu[G][32], pz[IRMH ? G : 1][32];
   __shared__ int flag[32];
   const int lane = threadIdx.x & 31, g = threadIdx.x >> 5;
   const int i = blockIdx.x * 32 + lane;
@@ -134,7 +136,7 @@ accept_kernel(float* __restrict__ phi, const float* __restrict__ phip, float* __
   const float hm = 0.5f * md.m0sq, lam = md.lam;
   // each warp owns a contiguous band of lattice rows: the "down" row of one iteration is the
   // row of the next one, so it is re-read from L1 instead of DRAM
-  const int band = (L + 7) >> 3, r_lo = g * band, r_hi = min(L, r_lo + band);
+  const int band = (L + G - 1) / G, r_lo = min(L, g * band), r_hi = min(L, r_lo + band);
   float dS = 0.f, dU = 0.f, z2 = 0.f;
   if (i < N) {
     if (IRMH) {                       // |z|^2 of this band: log q(phi') = -1/2 |z|^2 + const
@@ -169,7 +171,7 @@ accept_kernel(float* __restrict__ phi, const float* __restrict__ phip, float* __
     if (i < N) {
       float tS = 0.f, tU = 0.f;
 #pragma unroll
-      for (int m = 0; m < 8; ++m) { tS += ps[m][lane]; tU += pu[m][lane]; }
+      for (int m = 0; m < G; ++m) { tS += ps[m][lane]; tU += pu[m][lane]; }
       float lu = log_uniform(seed, tag_acc, t, (uint32_t)i);
       float Si = S[i], margin;
       if (!IRMH && mode == MODE_SMC) {
@@ -178,7 +180,7 @@ accept_kernel(float* __restrict__ phi, const float* __restrict__ phip, float* __
       } else if (IRMH) {
         float tZ = 0.f;
 #pragma unroll
-        for (int m = 0; m < 8; ++m) tZ += pz[m][lane];
+        for (int m = 0; m < G; ++m) tZ += pz[m][lane];
         // log q(phi) - log q(phi') = 1/2 |z|^2 - 1/2 |w|^2, w = Lc^-1 (phi - mu) (reading A15)
         margin = -(tU + (float)ctrl->beta * tS) + 0.5f * (tZ - W2[i]) - lu;
         acc = margin > 0.f;
@@ -211,6 +213,8 @@ accept_kernel(float* __restrict__ phi, const float* __restrict__ phip, float* __
 // 2 V ld floats.  The accept / commit step is the same either way.
 void launch_mutate_generic(const MutateArgs& a, float* Lsplit, cudaStream_t st) {
   const int V = a.md.V;
+  // fewer than two 8-warp blocks per SM and more than 8 lattice rows: one warp per row instead
+  const bool wide = a.md.L > 8 && a.ld / 32 < 2 * 148;
   dim3 gz((a.ld + 127) / 128, (V + 3) / 4);
   dim3 gp(a.ld / 64, (V + 63) / 64);
   if (Lsplit) {
@@ -229,10 +233,17 @@ void launch_mutate_generic(const MutateArgs& a, float* Lsplit, cudaStream_t st) 
       ++g_launches; propose_kernel<<<gp, 256, 0, st>>>(a.Lc, a.Z, a.phi, a.phip, V, a.ld, a.s, nullptr,
                                          0, a.ctrl, a.respect_done);
     }
-    ++g_launches; accept_kernel<false><<<a.ld / 32, 256, 0, st>>>(
-        a.phi, a.phip, a.S, a.U0, a.N, a.ld, a.md, a.mode, a.seed, a.tag_acc, t, a.ctrl,
-        a.acc_out ? a.acc_out + (size_t)j * a.N : nullptr,
-        a.margin_out ? a.margin_out + (size_t)j * a.N : nullptr, a.respect_done, nullptr, nullptr);
+    ++g_launches;
+    if (wide)
+      accept_kernel<false, 32><<<a.ld / 32, 1024, 0, st>>>(
+          a.phi, a.phip, a.S, a.U0, a.N, a.ld, a.md, a.mode, a.seed, a.tag_acc, t, a.ctrl,
+          a.acc_out ? a.acc_out + (size_t)j * a.N : nullptr,
+          a.margin_out ? a.margin_out + (size_t)j * a.N : nullptr, a.respect_done, nullptr, nullptr);
+    else
+      accept_kernel<false, 8><<<a.ld / 32, 256, 0, st>>>(
+          a.phi, a.phip, a.S, a.U0, a.N, a.ld, a.md, a.mode, a.seed, a.tag_acc, t, a.ctrl,
+          a.acc_out ? a.acc_out + (size_t)j * a.N : nullptr,
+          a.margin_out ? a.margin_out + (size_t)j * a.N : nullptr, a.respect_done, nullptr, nullptr);
   }
 }
 
@@ -281,7 +292,7 @@ void launch_mutate_irmh(const MutateArgs& a, const float* mu, float* W2, cudaStr
                                        a.respect_done);
     ++g_launches; propose_kernel<<<gp, 256, 0, st>>>(a.Lc, a.Z, a.phi, a.phip, V, a.ld, 1.0f, mu,
                                        0, a.ctrl, a.respect_done);
-    ++g_launches; accept_kernel<true><<<a.ld / 32, 256, 0, st>>>(
+    ++g_launches; accept_kernel<true, 8><<<a.ld / 32, 256, 0, st>>>(
         a.phi, a.phip, a.S, a.U0, a.N, a.ld, a.md, MODE_IRMH, a.seed, a.tag_acc, t, a.ctrl,
         a.acc_out ? a.acc_out + (size_t)j * a.N : nullptr,
         a.margin_out ? a.margin_out + (size_t)j * a.N : nullptr, a.respect_done, a.Z, W2);
