@@ -91,6 +91,10 @@ def lib():
         "orc_slice_walk": (None, [_dp, _dp, _dp, C.c_int, C.c_int, C.c_double, C.c_double, _dp,
                                   C.c_double, C.c_int, C.c_int, C.c_double, C.c_uint64, C.c_uint32,
                                   C.c_int, vp, vp, vp, vp, vp]),
+        "orc_z2_flip": (None, [_dp, C.c_int, C.c_int, C.c_uint64, C.c_uint32, vp]),
+        "orc_smc_run_z2": (C.c_int, [C.c_int, C.c_double, C.c_double, C.c_int, C.c_uint64, C.c_int,
+                                     C.c_double, C.c_double, C.c_int, _dp, _dp, _dp,
+                                     C.POINTER(C.c_double), vp]),
         "orc_irmh_mutate": (None, [_dp, _dp, _dp, C.c_int, C.c_int, C.c_double, C.c_double, _dp, _dp,
                                    C.c_double, C.c_uint64, C.c_uint32, C.c_int, vp, vp, vp]),
         "orc_smc_irmh_run": (C.c_int, [C.c_int, C.c_double, C.c_double, C.c_int, C.c_uint64, C.c_int,
@@ -299,12 +303,13 @@ def observables_from_M(M, S, logw, V):
 SMC_INFO = ("beta", "delta", "ess_frac", "dlogZ", "accept_rate", "n_unique", "chol_status", "_")
 
 
-def smc_run(L, m0sq, lam, N, seed, k, ess_target=0.5, step_scale=0.0, max_temps=4096):
+def smc_run(L, m0sq, lam, N, seed, k, ess_target=0.5, step_scale=0.0, max_temps=4096, z2_flip=False):
+    """z2_flip: flip each particle with probability 1/2 after every resampling (reading A17)."""
     V = L * L
     phi, S, U0 = np.zeros((V, N)), np.zeros(N), np.zeros(N)
     info = np.zeros((max_temps, 8))
     logZ = C.c_double(0.0)
-    T = lib().orc_smc_run(L, m0sq, lam, N, seed, k, ess_target, step_scale, max_temps, phi, S,
+    T = (lib().orc_smc_run_z2 if z2_flip else lib().orc_smc_run)(L, m0sq, lam, N, seed, k, ess_target, step_scale, max_temps, phi, S,
                           U0, C.byref(logZ), _ptr(info))
     if T < 0:
         raise RuntimeError("oracle SMC: covariance not positive definite")
@@ -413,3 +418,13 @@ def slice_walk(phi, S, U0, L, m0sq, lam, Lc, S_star, seed, t0, k, width=1.0, m_e
                          S_star, seed, t0, k, _ptr(t), _ptr(nexp), _ptr(nshr), _ptr(amb),
                          _ptr(slots))
     return phi, S, U0, t, nexp, nshr, amb
+
+
+# ---------------------------------------------------------------- NEXT row f4: Z2 flips ----
+def z2_flip(phi, seed, T):
+    """Flips of reading A17 on a copy; returns (phi, flipped[N])."""
+    phi = _f64(phi).copy()
+    V, N = phi.shape
+    fl = np.zeros(N, np.uint8)
+    lib().orc_z2_flip(phi, N, V, seed, T, _ptr(fl))
+    return phi, fl

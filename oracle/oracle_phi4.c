@@ -1084,3 +1084,76 @@ void orc_slice_walk(double* phi, double* S, double* U0, int N, int L,
     free(f); free(d); free(z); free(tmp);
   }
 }
+
+/* ------------------------------------------------------------------------
+ * NEXT row f4 -- global Z2 flips inside the particle method (PAPER.md:55,
+ * :85: "It is also possible to simply encode the Z2 symmetry into particle
+ * methods"; :176 describes the move for the AHMC control).  Reading A17
+ * (DESIGN.md): S_E and U0 are even in phi, so phi -> -phi is a symmetry of every
+ * p_beta and the flip is always accepted.  After the resampling of temperature
+ * T, the particle in slot j is flipped iff the top bit of word 0 of the draw
+ * (tag 8, t = T, slot j) is set.  S_E and U0 are unchanged.
+ * ---------------------------------------------------------------------- */
+#define ORC_TAG_Z2 8u
+void orc_z2_flip(double* phi, int N, int V, uint64_t seed, uint32_t T,
+                 uint8_t* flipped) {
+  for (int j = 0; j < N; ++j) {
+    uint32_t w = orc_word0(seed, ORC_TAG_Z2, T, (uint32_t)j);
+    int f = (int)(w >> 31);
+    if (flipped) flipped[j] = (uint8_t)f;
+    if (f)
+      for (int x = 0; x < V; ++x) phi[(size_t)x * N + j] = -phi[(size_t)x * N + j];
+  }
+}
+
+/* orc_smc_run with the Z2 flip of reading A17 after every resampling. */
+int orc_smc_run_z2(int L, double m0sq, double lam, int N, uint64_t seed, int k,
+                   double ess_target, double step_scale, int max_temps,
+                   double* phi, double* S, double* U0, double* logZ_out,
+                   double* info) {
+  int V = L * L;
+  double s = step_scale > 0.0 ? step_scale : 2.38 / sqrt((double)V);
+  double* tmp = (double*)malloc(sizeof(double) * (size_t)V * N);
+  double* Sigma = (double*)malloc(sizeof(double) * (size_t)V * V);
+  double* Lc = (double*)malloc(sizeof(double) * (size_t)V * V);
+  float* w = (float*)malloc(sizeof(float) * N);
+  int32_t* anc = (int32_t*)malloc(sizeof(int32_t) * N);
+  uint8_t* acc = (uint8_t*)malloc((size_t)k * N);
+  orc_init_particles(seed, N, V, phi);
+  orc_action_batch(phi, N, L, m0sq, lam, S, U0, NULL);
+  double beta = 0.0, logZ = 0.0;
+  uint32_t t = 0;
+  int T = 0, rc = 0;
+  while (beta < 1.0 && T < max_temps) {
+    int final;
+    double delta = orc_next_delta(S, N, beta, ess_target, &final);
+    double beta_new = final ? 1.0 : beta + delta;
+    double ess = orc_ess_frac(S, N, delta);
+    double dlz = orc_reweight(S, N, delta, w);
+    logZ += dlz;
+    uint32_t U = orc_word0(seed, ORC_TAG_RESAMPLE, (uint32_t)T, 0u);
+    orc_resample_systematic(w, N, U, anc);
+    orc_gather(phi, N, V, anc, tmp);
+    memcpy(phi, tmp, sizeof(double) * (size_t)V * N);
+    orc_gather(S, N, 1, anc, tmp);  memcpy(S, tmp, sizeof(double) * N);
+    orc_gather(U0, N, 1, anc, tmp); memcpy(U0, tmp, sizeof(double) * N);
+    orc_z2_flip(phi, N, V, seed, (uint32_t)T, NULL);
+    int st = orc_cov_chol(phi, N, V, Sigma, Lc);
+    if (st < 0) { rc = -1; break; }
+    orc_mutate(phi, S, U0, N, L, m0sq, lam, Lc, s, beta_new, ORC_MODE_SMC, 0.0,
+               seed, ORC_TAG_PROP, ORC_TAG_ACC, t + 1, k, acc, NULL, NULL, NULL);
+    t += (uint32_t)k;
+    double nacc = 0.0;
+    for (size_t m = 0; m < (size_t)k * N; ++m) nacc += acc[m];
+    if (info) {
+      double* o = info + 8 * T;
+      o[0] = beta_new; o[1] = delta; o[2] = ess; o[3] = dlz;
+      o[4] = nacc / ((double)k * N); o[5] = 0; o[6] = st; o[7] = 0.0;
+    }
+    beta = beta_new;
+    ++T;
+  }
+  *logZ_out = logZ;
+  free(tmp); free(Sigma); free(Lc); free(w); free(anc); free(acc);
+  return rc < 0 ? rc : T;
+}
