@@ -63,6 +63,9 @@ typedef struct {
   int kernel;
   float hmc_eps;
   int hmc_leapfrog;
+  /* 1: global Z2 flips phi -> -phi (reading A17): after every resampling each
+   * particle is flipped with probability 1/2 (always accepted: S_E and U0 are even).  0: off.   */
+  int z2_flip;
 } smc_params;
 
 /* Inner kernel of nested sampling (PAPER.md:53(iv), :174).  inner = 0: constrained random walk of

@@ -28,7 +28,7 @@ class Phi4Error(RuntimeError):
 class smc_params(C.Structure):
     _fields_ = [("k_steps", C.c_int), ("ess_target", C.c_float), ("step_scale", C.c_float),
                 ("mutation_path", C.c_int), ("kernel", C.c_int), ("hmc_eps", C.c_float),
-                ("hmc_leapfrog", C.c_int)]
+                ("hmc_leapfrog", C.c_int), ("z2_flip", C.c_int)]
 
 
 class ns_params(C.Structure):
@@ -222,8 +222,9 @@ def smc_destroy(h):
 
 
 def smc_set_params(h, k_steps=10, ess_target=0.5, step_scale=0.0, mutation_path=0, kernel=0,
-                   hmc_eps=0.1, hmc_leapfrog=20):
-    p = smc_params(k_steps, ess_target, step_scale, mutation_path, kernel, hmc_eps, hmc_leapfrog)
+                   hmc_eps=0.1, hmc_leapfrog=20, z2_flip=0):
+    p = smc_params(k_steps, ess_target, step_scale, mutation_path, kernel, hmc_eps, hmc_leapfrog,
+                   z2_flip)
     h._check(load().smc_set_params(h.ptr, C.byref(p)), "smc_set_params")
 
 

@@ -164,7 +164,7 @@ static phi4smc* new_handle(int kind, int L, float m0sq, float lambda, int N, uin
   h->N = N; h->ld = round_up(N, 128);
   h->seed = seed;
   h->prm.k_steps = 10; h->prm.ess_target = 0.5f; h->prm.step_scale = 0.f; h->prm.mutation_path = 0;
-  h->prm.kernel = 0; h->prm.hmc_eps = 0.1f; h->prm.hmc_leapfrog = 20;
+  h->prm.kernel = 0; h->prm.hmc_eps = 0.1f; h->prm.hmc_leapfrog = 20; h->prm.z2_flip = 0;
   h->nsp.inner = 0; h->nsp.slice_width = 1.0f; h->nsp.max_expand = 8; h->nsp.max_shrink = 32;
   h->s = 2.38f / sqrtf((float)h->md.V);
   return h;
@@ -319,7 +319,7 @@ PHI4_API int smc_set_params(phi4smc* h, const smc_params* p) {
     return PHI4_EINVAL;
   if (p->mutation_path == 2 && !mutate_tc_supported(h->md.V) && !propose_tc_supported(h->md.V))
     return PHI4_EINVAL;
-  if (p->kernel < 0 || p->kernel > 2) return PHI4_EINVAL;
+  if (p->kernel < 0 || p->kernel > 2 || p->z2_flip < 0 || p->z2_flip > 1) return PHI4_EINVAL;
   if (p->kernel == 2 && (h->kind != KIND_SMC || !irmh_supported(h->md.V))) return PHI4_EINVAL;
   if (p->kernel == 1 && (h->kind != KIND_SMC || !hmc_supported(h->md.V) || !(p->hmc_eps > 0.f) ||
                          p->hmc_leapfrog < 1))
@@ -376,9 +376,10 @@ static CovCholArgs cov_args(phi4smc* h, int respect_done) {
 
 static void enqueue_resample(phi4smc* h, bool scanned = false) {
   if (!scanned) launch_quantise_scan(h->w, h->N, h->C, h->ctrl, h->st);
-  launch_ancestors(h->C, h->N, h->seed, h->anc, h->ctrl, h->st);
+  // the accept-flag scratch of the hooks doubles as the per-slot Z2 flip bytes
+  launch_ancestors(h->C, h->N, h->seed, h->anc, h->acc_flags, h->prm.z2_flip, h->ctrl, h->st);
   const int o = h->cur ^ 1;
-  launch_gather(h->phi[h->cur], h->phi[o], h->S[h->cur], h->S[o], h->U0[h->cur], h->U0[o], h->anc,
+  launch_gather(h->phi[h->cur], h->phi[o], h->S[h->cur], h->S[o], h->U0[h->cur], h->U0[o], h->anc, h->acc_flags,
                 h->N, h->ld, h->md.V, h->ctrl, h->st);
   h->cur = o;
 }

@@ -11,7 +11,7 @@ extern unsigned long long g_launches;
 // Philox stream tags (reading R1).
 enum : uint32_t {
   TAG_INIT = 0, TAG_PROP = 1, TAG_ACC = 2, TAG_RESAMPLE = 3,
-  TAG_NS_START = 4, TAG_NS_PROP = 5, TAG_NS_ACC = 6, TAG_NS_SLICE = 7
+  TAG_NS_START = 4, TAG_NS_PROP = 5, TAG_NS_ACC = 6, TAG_NS_SLICE = 7, TAG_Z2 = 8
 };
 enum : int { MODE_SMC = 0, MODE_NS = 1, MODE_IRMH = 2 };
 

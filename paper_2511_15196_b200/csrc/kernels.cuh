@@ -65,11 +65,11 @@ bool launch_next_delta_reweight(const float* S, int N, float ess_target, double 
                                 float* w, unsigned long long* C, Ctrl* ctrl, cudaStream_t st);
 void launch_quantise_scan(const float* w, int N, unsigned long long* C, Ctrl* ctrl,
                           cudaStream_t st);
-void launch_ancestors(const unsigned long long* C, int N, uint64_t seed, int32_t* anc, Ctrl* ctrl,
-                      cudaStream_t st);
+void launch_ancestors(const unsigned long long* C, int N, uint64_t seed, int32_t* anc, uint8_t* flip,
+                      int z2, Ctrl* ctrl, cudaStream_t st);
 void launch_gather(const float* phi_in, float* phi_out, const float* S_in, float* S_out,
-                   const float* U_in, float* U_out, const int32_t* anc, int N, int ld, int V,
-                   Ctrl* ctrl, cudaStream_t st);
+                   const float* U_in, float* U_out, const int32_t* anc, const uint8_t* flip, int N,
+                   int ld, int V, Ctrl* ctrl, cudaStream_t st);
 void launch_finish_step(Ctrl* ctrl, StepRecord* rec, int max_rec, int k, int N, cudaStream_t st);
 
 // covchol.cu -- C1, C2

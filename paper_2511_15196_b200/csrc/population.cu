@@ -451,12 +451,17 @@ void launch_quantise_scan(const float* w, int N, unsigned long long* C, Ctrl* ct
 // a_j = #{i : C_i <= t_j}, t_j = floor(((j 2^32 + U) T) / (N 2^32)), clamped to N-1; U = word 0
 // of the RESAMPLE stream at the current temperature index.  Once the run is done the map is the
 // identity, so that a step enqueued past beta = 1 leaves the particles unchanged.
+// flip[j] (NEXT row f4, reading A17): with z2 set, slot j is sign-flipped by the gather iff the top
+// bit of word 0 of the Z2 stream at this temperature is set.
 __global__ void ancestors_kernel(const unsigned long long* __restrict__ C, int N, uint64_t seed,
-                                 int32_t* __restrict__ anc, const Ctrl* ctrl) {
+                                 int32_t* __restrict__ anc, uint8_t* __restrict__ flip, int z2,
+                                 const Ctrl* ctrl) {
   pdl_enter();
   int j = blockIdx.x * blockDim.x + threadIdx.x;
   if (j >= N) return;
-  if (ctrl->done || ctrl->q_total == 0ull) { anc[j] = j; return; }
+  if (ctrl->done || ctrl->q_total == 0ull) { anc[j] = j; flip[j] = 0; return; }
+  flip[j] = z2 ? (uint8_t)(philox_draw(seed, TAG_Z2, (uint32_t)ctrl->temp_index, (uint32_t)j, 0u).x >> 31)
+               : (uint8_t)0;
   const uint32_t U = philox_draw(seed, TAG_RESAMPLE, (uint32_t)ctrl->temp_index, 0u, 0u).x;
   const unsigned long long T = ctrl->q_total;
   unsigned __int128 num = (unsigned __int128)(((unsigned long long)j << 32) + U) *
@@ -470,9 +475,9 @@ __global__ void ancestors_kernel(const unsigned long long* __restrict__ C, int N
   anc[j] = min(lo, N - 1);
 }
 
-void launch_ancestors(const unsigned long long* C, int N, uint64_t seed, int32_t* anc, Ctrl* ctrl,
-                      cudaStream_t st) {
-  ++g_launches; launch_pdl(ancestors_kernel, (N + 255) / 256, 256, 0, st, C, N, seed, anc, ctrl);
+void launch_ancestors(const unsigned long long* C, int N, uint64_t seed, int32_t* anc, uint8_t* flip,
+                      int z2, Ctrl* ctrl, cudaStream_t st) {
+  ++g_launches; launch_pdl(ancestors_kernel, (N + 255) / 256, 256, 0, st, C, N, seed, anc, flip, z2, ctrl);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -485,21 +490,26 @@ __global__ void __launch_bounds__(256)
 gather_kernel(const float* __restrict__ pin, float* __restrict__ pout,
               const float* __restrict__ Sin, float* __restrict__ Sout,
               const float* __restrict__ Uin, float* __restrict__ Uout,
-              const int32_t* __restrict__ anc, int N, int ld, int V, Ctrl* ctrl) {
+              const int32_t* __restrict__ anc, const uint8_t* __restrict__ flip, int N, int ld,
+              int V, Ctrl* ctrl) {
   pdl_enter();
   const int j0 = (blockIdx.x * blockDim.x + threadIdx.x) * 4;
   if (j0 >= ld) return;
   int a[4];
+  float sg[4];                        // Z2 flip of the destination slot (S_E, U0 are even in phi)
 #pragma unroll
-  for (int m = 0; m < 4; ++m) a[m] = (j0 + m < N) ? anc[j0 + m] : -1;
+  for (int m = 0; m < 4; ++m) {
+    a[m] = (j0 + m < N) ? anc[j0 + m] : -1;
+    sg[m] = (j0 + m < N && flip[j0 + m]) ? -1.f : 1.f;
+  }
   const int x0 = blockIdx.y * GATHER_ROWS, x1 = min(V, x0 + GATHER_ROWS);
   for (int x = x0; x < x1; ++x) {
     const float* src = pin + (size_t)x * ld;
     float4 v;
-    v.x = a[0] >= 0 ? src[a[0]] : 0.f;
-    v.y = a[1] >= 0 ? src[a[1]] : 0.f;
-    v.z = a[2] >= 0 ? src[a[2]] : 0.f;
-    v.w = a[3] >= 0 ? src[a[3]] : 0.f;
+    v.x = a[0] >= 0 ? sg[0] * src[a[0]] : 0.f;
+    v.y = a[1] >= 0 ? sg[1] * src[a[1]] : 0.f;
+    v.z = a[2] >= 0 ? sg[2] * src[a[2]] : 0.f;
+    v.w = a[3] >= 0 ? sg[3] * src[a[3]] : 0.f;
     *reinterpret_cast<float4*>(pout + (size_t)x * ld + j0) = v;
   }
   if (blockIdx.y == 0) {
@@ -524,10 +534,10 @@ gather_kernel(const float* __restrict__ pin, float* __restrict__ pout,
 }
 
 void launch_gather(const float* phi_in, float* phi_out, const float* S_in, float* S_out,
-                   const float* U_in, float* U_out, const int32_t* anc, int N, int ld, int V,
-                   Ctrl* ctrl, cudaStream_t st) {
+                   const float* U_in, float* U_out, const int32_t* anc, const uint8_t* flip, int N,
+                   int ld, int V, Ctrl* ctrl, cudaStream_t st) {
   dim3 grid((ld / 4 + 255) / 256, (V + GATHER_ROWS - 1) / GATHER_ROWS);
-  ++g_launches; launch_pdl(gather_kernel, grid, 256, 0, st, phi_in, phi_out, S_in, S_out, U_in, U_out, anc, N, ld, V,
+  ++g_launches; launch_pdl(gather_kernel, grid, 256, 0, st, phi_in, phi_out, S_in, S_out, U_in, U_out, anc, flip, N, ld, V,
                                       ctrl);
 }
 

@@ -35,7 +35,7 @@ def test_header_symbols_are_exported_and_bound(lib):
 
 def test_struct_sizes_match_header(lib):
     from paper_2511_15196_b200 import binding as B
-    assert C.sizeof(B.smc_params) == 28
+    assert C.sizeof(B.smc_params) == 32
     assert C.sizeof(B.smc_step_info) == 6 * 8 + 4 * 4
     assert C.sizeof(B.ns_step_info) == 56   # 5 doubles + 3 ints, padded to 8
     assert C.sizeof(B.phi4_observables) == (5 + 80) * 8
