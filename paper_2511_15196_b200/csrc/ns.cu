@@ -12,6 +12,75 @@ __device__ __forceinline__ double logaddexp_d(double a, double b) {
   return m + log(exp(a - m) + exp(b - m));
 }
 
+// Ascending bitonic sort of 1024 E composite keys (descending S_E, ascending index; pad keys sort
+// last) by one block of 1024 threads.  Thread t holds keys t E .. t E + E - 1 in registers:
+// partners inside the thread are exchanged in registers, partners inside the warp by shuffles,
+// and only the strides that cross warps (j >= 32 E) go through shared memory -- 15 of the 78
+// stages at n = 4096 instead of a barrier after every stage.  The sorted keys end in `keys`.
+template <int E>
+__device__ __forceinline__ void bitonic_sort_block(const float* __restrict__ S, int n,
+                                                   unsigned long long* keys) {
+  const int tid = threadIdx.x, NP = 1024 * E;
+  unsigned long long kr[E];
+#pragma unroll
+  for (int e = 0; e < E; ++e) {
+    const int i = tid * E + e;
+    unsigned long long key = ~0ull;
+    if (i < n) {
+      uint32_t b = __float_as_uint(S[i]);
+      uint32_t asc = (b & 0x80000000u) ? ~b : (b | 0x80000000u);   // ascending-orderable
+      key = ((unsigned long long)(~asc) << 32) | (uint32_t)i;        // descending S, ascending i
+    }
+    kr[e] = key;
+  }
+  for (int k = 2; k <= NP; k <<= 1) {
+    for (int j = k >> 1; j >= E && j > 0; j >>= 1) {
+      if (j >= 32 * E) {
+        // partner in another warp: through shared memory
+#pragma unroll
+        for (int e = 0; e < E; ++e) keys[tid * E + e] = kr[e];
+        __syncthreads();
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+          const int i = tid * E + e;
+          const unsigned long long y = keys[i ^ j];
+          const bool keep_min = ((i & j) == 0) == ((i & k) == 0);
+          kr[e] = keep_min ? (kr[e] < y ? kr[e] : y) : (kr[e] > y ? kr[e] : y);
+        }
+        __syncthreads();
+      } else {
+        // partner in another lane of this warp, same register slot
+        const int lm = j / E;
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+          const int i = tid * E + e;
+          const unsigned long long y = __shfl_xor_sync(0xffffffffu, kr[e], lm);
+          const bool keep_min = ((i & j) == 0) == ((i & k) == 0);
+          kr[e] = keep_min ? (kr[e] < y ? kr[e] : y) : (kr[e] > y ? kr[e] : y);
+        }
+      }
+    }
+    // partners inside this thread: strides E/2 .. 1 (compile-time register indices)
+#pragma unroll
+    for (int jj = E >> 1; jj > 0; jj >>= 1) {
+      if (jj <= (k >> 1)) {
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+          if ((e & jj) == 0) {
+            const int i = tid * E + e;
+            const bool up = (i & k) == 0;
+            const unsigned long long x = kr[e], y = kr[e | jj];
+            if ((x > y) == up) { kr[e] = y; kr[e | jj] = x; }
+          }
+        }
+      }
+    }
+  }
+#pragma unroll
+  for (int e = 0; e < E; ++e) keys[tid * E + e] = kr[e];
+  __syncthreads();
+}
+
 // N1 + N2 + survivors + start choice in one CTA.
 //  N1: 64-bit keys (descending S_E, ascending index) bitonic-sorted in shared memory; the first
 //      k_del are the dead points, S_star = smallest S_E among them.
@@ -28,30 +97,14 @@ ns_select_evidence_kernel(NsArgs a) {
   Ctrl* ctrl = a.ctrl;
   if (ctrl->done) return;
   const int n = a.n, kd = a.k_del, tid = threadIdx.x, nt = blockDim.x;
-  int np2 = 1;
+  int np2 = 1024;                    // padded to the block: thread t holds keys t E .. t E + E - 1
   while (np2 < n) np2 <<= 1;
-  for (int i = tid; i < np2; i += nt) {
-    unsigned long long key = ~0ull;
-    if (i < n) {
-      uint32_t b = __float_as_uint(a.S[i]);
-      uint32_t asc = (b & 0x80000000u) ? ~b : (b | 0x80000000u);   // ascending-orderable
-      key = ((unsigned long long)(~asc) << 32) | (uint32_t)i;        // descending S, ascending i
-    }
-    keys[i] = key;
-  }
-  __syncthreads();
-  for (int k = 2; k <= np2; k <<= 1) {
-    for (int j = k >> 1; j > 0; j >>= 1) {
-      for (int i = tid; i < np2; i += nt) {
-        int p = i ^ j;
-        if (p > i) {
-          unsigned long long x = keys[i], y = keys[p];
-          bool up = (i & k) == 0;
-          if ((x > y) == up) { keys[i] = y; keys[p] = x; }
-        }
-      }
-      __syncthreads();
-    }
+  switch (np2 >> 10) {
+    case 1: bitonic_sort_block<1>(a.S, n, keys); break;
+    case 2: bitonic_sort_block<2>(a.S, n, keys); break;
+    case 4: bitonic_sort_block<4>(a.S, n, keys); break;
+    case 8: bitonic_sort_block<8>(a.S, n, keys); break;
+    default: bitonic_sort_block<16>(a.S, n, keys); break;
   }
   const int it = ctrl->temp_index;
   const double logX0 = ctrl->logX;
@@ -139,7 +192,7 @@ ns_select_evidence_kernel(NsArgs a) {
 }
 
 void launch_ns_select_evidence(const NsArgs& a, cudaStream_t st) {
-  int np2 = 1;
+  int np2 = 1024;
   while (np2 < a.n) np2 <<= 1;
   size_t smem = (size_t)np2 * sizeof(unsigned long long);
   static bool attr_done = false;
