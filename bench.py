@@ -291,14 +291,9 @@ def main():
         B.smc_mutate(h, k, want=False)
     reps = 5
     l1 = B.phi4_kernel_launches()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
-    for _ in range(reps):
-        B.smc_mutate(h, k, want=False)
-    e1.record()
-    torch.cuda.synchronize()
-    mut_ms = e0.elapsed_time(e1) / reps                       # k steps
-    mut_launches = (B.phi4_kernel_launches() - l1) // reps
+    # CUDA events on the library's own stream around `reps` back-to-back k-step mutations
+    mut_ms = B.smc_time_mutation(h, k, reps)                  # k steps
+    mut_launches = (B.phi4_kernel_launches() - l1 - 2) // reps    # minus the two counter resets
 
     # ---- population step: resample (integer scan, ancestors) + gather, device-resident weights ----
     B.smc_reweight(h)                                          # weights at the ESS target

@@ -200,6 +200,10 @@ int smc_get_mean(phi4smc* h, float* h_mu /* V: particle mean of the last covaria
 int smc_mutate(phi4smc* h, int k, uint8_t* h_accept, float* h_margin);
 /* P1+P2 at the current beta: delta < 0 selects the bisection, otherwise the given delta is used.
  * Advances beta and logZ; h_w receives the max-shifted fp32 weights (max = 1).                   */
+/* Measurement hook: enqueues `reps` back-to-back mutations of k steps each (as smc_mutate without
+ * flags, no host synchronisation in between) bracketed by CUDA events on the handle's stream and
+ * returns the average device time of one k-step mutation in milliseconds.                        */
+int smc_time_mutation(phi4smc* h, int k, int reps, float* h_ms_per_call);
 int smc_reweight(phi4smc* h, double delta, float* h_w, smc_step_info* info);
 /* P3+P4: systematic resampling of the device weights (or of h_w if non-NULL) with the Philox
  * offset of the current temperature index, then the gather.  h_ancestors receives a_j.           */

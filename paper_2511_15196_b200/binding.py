@@ -95,6 +95,7 @@ SIGNATURES = {
     "smc_get_cov": (_i, [_vp, _vp]),
     "smc_get_mean": (_i, [_vp, _vp]),
     "smc_mutate": (_i, [_vp, _i, _vp, _vp]),
+    "smc_time_mutation": (_i, [_vp, _i, _i, C.POINTER(_f)]),
     "smc_reweight": (_i, [_vp, _d, _vp, C.POINTER(smc_step_info)]),
     "smc_resample": (_i, [_vp, _vp, _vp]),
     "ns_get_dead": (_i, [_vp, _vp, _vp, _vp, _vp, _i, C.POINTER(_i)]),
@@ -331,6 +332,12 @@ def smc_mutate(h, k, want=True):
     mar = np.empty((k, h.N), np.float32) if want else None
     h._check(load().smc_mutate(h.ptr, k, _np_ptr(acc), _np_ptr(mar)), "smc_mutate")
     return acc, mar
+
+
+def smc_time_mutation(h, k, reps=5):
+    ms = C.c_float(0.0)
+    h._check(load().smc_time_mutation(h.ptr, k, reps, C.byref(ms)), "smc_time_mutation")
+    return ms.value
 
 
 def smc_reweight(h, delta=-1.0):

@@ -742,6 +742,29 @@ PHI4_API int smc_mutate(phi4smc* h, int k, uint8_t* h_accept, float* h_margin) {
   return PHI4_OK;
 }
 
+PHI4_API int smc_time_mutation(phi4smc* h, int k, int reps, float* h_ms_per_call) {
+  if (!h || h->kind != KIND_SMC || k < 1 || reps < 1 || !h_ms_per_call) return PHI4_EINVAL;
+  cudaEvent_t e0, e1;
+  CU(cudaEventCreate(&e0));
+  CU(cudaEventCreate(&e1));
+  launch_reset_counters(h->ctrl, h->st);
+  CU(cudaEventRecord(e0, h->st));
+  for (int r = 0; r < reps; ++r) {
+    enqueue_mutation(h, smc_mutate_args(h, k, nullptr, nullptr, 0));
+    h->step_counter += (uint64_t)k;
+  }
+  CU(cudaEventRecord(e1, h->st));
+  launch_reset_counters(h->ctrl, h->st);
+  CU(cudaStreamSynchronize(h->st));
+  float ms = 0.f;
+  CU(cudaEventElapsedTime(&ms, e0, e1));
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  CU(cudaGetLastError());
+  *h_ms_per_call = ms / (float)reps;
+  return PHI4_OK;
+}
+
 PHI4_API int smc_reweight(phi4smc* h, double delta, float* h_w, smc_step_info* info) {
   if (!h || h->kind != KIND_SMC) return PHI4_EINVAL;
   launch_next_delta_reweight(h->S[h->cur], h->N, h->prm.ess_target, delta < 0.0 ? -1.0 : delta,

@@ -97,6 +97,8 @@ bool pdl_enabled() {
   return on;
 }
 
-void launch_reset_counters(Ctrl* ctrl, cudaStream_t st) { reset_counters_kernel<<<1, 1, 0, st>>>(ctrl); }
+void launch_reset_counters(Ctrl* ctrl, cudaStream_t st) {
+  ++g_launches; reset_counters_kernel<<<1, 1, 0, st>>>(ctrl);
+}
 
 }  // namespace phi4
