@@ -134,8 +134,7 @@ accept_kernel(float* __restrict__ phi, const float* __restrict__ phip, float* __
   const int i = blockIdx.x * 32 + lane;
   const int L = md.L;
   const float hm = 0.5f * md.m0sq, lam = md.lam;
-  // each warp owns a contiguous band of lattice rows: the "down" row of one iteration is the
-  // row of the next one, so it is re-read from L1 instead of DRAM
+  // each warp owns a contiguous band of lattice rows
   const int band = (L + G - 1) / G, r_lo = min(L, g * band), r_hi = min(L, r_lo + band);
   float dS = 0.f, dU = 0.f, z2 = 0.f;
   if (i < N) {
@@ -145,21 +144,61 @@ accept_kernel(float* __restrict__ phi, const float* __restrict__ phip, float* __
         z2 = fmaf(z, z, z2);
       }
     }
-    for (int r = r_lo; r < r_hi; ++r) {
-      int rn = (r + 1 == L) ? 0 : r + 1;
-      size_t ro = (size_t)r * L * ld + i, rno = (size_t)rn * L * ld + i;
-      float a = phi[ro], a2 = phip[ro];
-      float rS = 0.f, rU = 0.f;       // per-row partial sums: two-level fp32 accumulation
-      for (int c = 0; c < L; ++c) {
-        int cn = (c + 1 == L) ? 0 : c + 1;
-        float b = phi[ro + (size_t)cn * ld], b2 = phip[ro + (size_t)cn * ld];
-        float d = phi[rno + (size_t)c * ld], d2 = phip[rno + (size_t)c * ld];
-        site_diff(a, b, d, a2, b2, d2, hm, lam, rS, rU);
-        a = b;
-        a2 = b2;
+    if (G == 8 && band <= 8 && ld >= 8192) {
+      // Column walk (large populations; a small one is latency-bound and prefers the row walk): the band's rows (<= 8) and the halo row below it are held for two adjacent
+      // lattice columns in registers, so every site of phi and phi' is loaded once (plus the
+      // halo row and the wrap-around column) instead of once as a site and again as the "down"
+      // neighbour of the row above -- the kernel is HBM-bound at C3 / C4.
+      const int nr = r_hi - r_lo;
+      const int rh = (r_hi == L) ? 0 : r_hi;              // halo row below the band
+      float A[9], A2[9], Bn[9], B2[9], rS[8], rU[8];
+#pragma unroll
+      for (int q = 0; q < 8; ++q) { rS[q] = 0.f; rU[q] = 0.f; }
+      auto load_col = [&](int c, float (&X)[9], float (&X2)[9]) {
+#pragma unroll
+        for (int q = 0; q < 8; ++q)
+          if (q < nr) {
+            const size_t o = ((size_t)(r_lo + q) * L + c) * ld + i;
+            X[q] = phi[o]; X2[q] = phip[o];
+          }
+        const size_t o = ((size_t)rh * L + c) * ld + i;
+        X[8] = phi[o]; X2[8] = phip[o];
+      };
+      if (nr > 0) {
+        load_col(0, A, A2);
+        for (int c = 0; c < L; ++c) {
+          load_col(c + 1 == L ? 0 : c + 1, Bn, B2);
+#pragma unroll
+          for (int q = 0; q < 8; ++q)
+            if (q < nr) {
+              const float d = (q + 1 < nr) ? A[q + 1 < 8 ? q + 1 : 8] : A[8];
+              const float d2 = (q + 1 < nr) ? A2[q + 1 < 8 ? q + 1 : 8] : A2[8];
+              site_diff(A[q], Bn[q], d, A2[q], B2[q], d2, hm, lam, rS[q], rU[q]);
+            }
+#pragma unroll
+          for (int q = 0; q < 9; ++q) { A[q] = Bn[q]; A2[q] = B2[q]; }
+        }
+#pragma unroll
+        for (int q = 0; q < 8; ++q)
+          if (q < nr) { dS += rS[q]; dU += rU[q]; }
       }
-      dS += rS;
-      dU += rU;
+    } else {
+      for (int r = r_lo; r < r_hi; ++r) {
+        int rn = (r + 1 == L) ? 0 : r + 1;
+        size_t ro = (size_t)r * L * ld + i, rno = (size_t)rn * L * ld + i;
+        float a = phi[ro], a2 = phip[ro];
+        float rS = 0.f, rU = 0.f;       // per-row partial sums: two-level fp32 accumulation
+        for (int c = 0; c < L; ++c) {
+          int cn = (c + 1 == L) ? 0 : c + 1;
+          float b = phi[ro + (size_t)cn * ld], b2 = phip[ro + (size_t)cn * ld];
+          float d = phi[rno + (size_t)c * ld], d2 = phip[rno + (size_t)c * ld];
+          site_diff(a, b, d, a2, b2, d2, hm, lam, rS, rU);
+          a = b;
+          a2 = b2;
+        }
+        dS += rS;
+        dU += rU;
+      }
     }
   }
   ps[g][lane] = dS;
