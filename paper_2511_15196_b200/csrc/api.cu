@@ -379,7 +379,8 @@ static void enqueue_resample(phi4smc* h, bool scanned = false) {
   // the accept-flag scratch of the hooks doubles as the per-slot Z2 flip bytes
   launch_ancestors(h->C, h->N, h->seed, h->anc, h->acc_flags, h->prm.z2_flip, h->ctrl, h->st);
   const int o = h->cur ^ 1;
-  launch_gather(h->phi[h->cur], h->phi[o], h->S[h->cur], h->S[o], h->U0[h->cur], h->U0[o], h->anc, h->acc_flags,
+  launch_gather(h->phi[h->cur], h->phi[o], h->S[h->cur], h->S[o], h->U0[h->cur], h->U0[o], h->anc,
+                h->prm.z2_flip ? h->acc_flags : nullptr,
                 h->N, h->ld, h->md.V, h->ctrl, h->st);
   h->cur = o;
 }

@@ -144,7 +144,7 @@ accept_kernel(float* __restrict__ phi, const float* __restrict__ phip, float* __
         z2 = fmaf(z, z, z2);
       }
     }
-    if (G == 8 && band <= 8 && ld >= 8192) {
+    if (G == 8 && band >= 4 && band <= 8 && ld >= 8192) {
       // Column walk (large populations; a small one is latency-bound and prefers the row walk): the band's rows (<= 8) and the halo row below it are held for two adjacent
       // lattice columns in registers, so every site of phi and phi' is loaded once (plus the
       // halo row and the wrap-around column) instead of once as a site and again as the "down"

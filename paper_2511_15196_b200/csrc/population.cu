@@ -486,6 +486,7 @@ void launch_ancestors(const unsigned long long* C, int N, uint64_t seed, int32_t
 // per site row.  grid.y splits the V rows.  HBM bound: 8 N V bytes.
 // ---------------------------------------------------------------------------------------------
 constexpr int GATHER_ROWS = 16;
+template <bool Z2>
 __global__ void __launch_bounds__(256)
 gather_kernel(const float* __restrict__ pin, float* __restrict__ pout,
               const float* __restrict__ Sin, float* __restrict__ Sout,
@@ -500,16 +501,17 @@ gather_kernel(const float* __restrict__ pin, float* __restrict__ pout,
 #pragma unroll
   for (int m = 0; m < 4; ++m) {
     a[m] = (j0 + m < N) ? anc[j0 + m] : -1;
-    sg[m] = (j0 + m < N && flip[j0 + m]) ? -1.f : 1.f;
+    sg[m] = (Z2 && j0 + m < N && flip[j0 + m]) ? -1.f : 1.f;
   }
   const int x0 = blockIdx.y * GATHER_ROWS, x1 = min(V, x0 + GATHER_ROWS);
   for (int x = x0; x < x1; ++x) {
     const float* src = pin + (size_t)x * ld;
     float4 v;
-    v.x = a[0] >= 0 ? sg[0] * src[a[0]] : 0.f;
-    v.y = a[1] >= 0 ? sg[1] * src[a[1]] : 0.f;
-    v.z = a[2] >= 0 ? sg[2] * src[a[2]] : 0.f;
-    v.w = a[3] >= 0 ? sg[3] * src[a[3]] : 0.f;
+    v.x = a[0] >= 0 ? src[a[0]] : 0.f;
+    v.y = a[1] >= 0 ? src[a[1]] : 0.f;
+    v.z = a[2] >= 0 ? src[a[2]] : 0.f;
+    v.w = a[3] >= 0 ? src[a[3]] : 0.f;
+    if (Z2) { v.x *= sg[0]; v.y *= sg[1]; v.z *= sg[2]; v.w *= sg[3]; }
     *reinterpret_cast<float4*>(pout + (size_t)x * ld + j0) = v;
   }
   if (blockIdx.y == 0) {
@@ -536,9 +538,15 @@ gather_kernel(const float* __restrict__ pin, float* __restrict__ pout,
 void launch_gather(const float* phi_in, float* phi_out, const float* S_in, float* S_out,
                    const float* U_in, float* U_out, const int32_t* anc, const uint8_t* flip, int N,
                    int ld, int V, Ctrl* ctrl, cudaStream_t st) {
+  // flip == nullptr: no Z2 move (the instantiation without the sign)
   dim3 grid((ld / 4 + 255) / 256, (V + GATHER_ROWS - 1) / GATHER_ROWS);
-  ++g_launches; launch_pdl(gather_kernel, grid, 256, 0, st, phi_in, phi_out, S_in, S_out, U_in, U_out, anc, flip, N, ld, V,
-                                      ctrl);
+  ++g_launches;
+  if (flip)
+    launch_pdl(gather_kernel<true>, grid, 256, 0, st, phi_in, phi_out, S_in, S_out, U_in, U_out, anc, flip, N,
+               ld, V, ctrl);
+  else
+    launch_pdl(gather_kernel<false>, grid, 256, 0, st, phi_in, phi_out, S_in, S_out, U_in, U_out, anc, flip, N,
+               ld, V, ctrl);
 }
 
 // End of a temperature: record it, advance the index, latch done at beta == 1.
