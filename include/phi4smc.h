@@ -57,9 +57,9 @@ typedef struct {
   /* Rejuvenation kernel: 0 = RW-Metropolis (i), 1 = HMC (iii, :172; reading A14),
    * 2 = independent MH from the fitted Gaussian N(mu, Sigma) (ii, :200; reading A15; L*L <= 800).
    * HMC: mass matrix diag(1/var_x) from the particle covariance, hmc_leapfrog >= 1 leapfrog steps
-   * of size hmc_eps > 0 per transition, k_steps transitions per temperature.  The HMC kernel
-   * is instantiated per lattice side (three 32-particle tiles in shared memory): L <= 22, else
-   * PHI4_EINVAL.                                                                               */
+   * of size hmc_eps > 0 per transition, k_steps transitions per temperature.  L <= 22 runs in one
+   * register/shared-memory resident kernel per temperature; larger lattices keep position and
+   * momentum in HBM scratch with one launch per leapfrog half-step.                             */
   int kernel;
   float hmc_eps;
   int hmc_leapfrog;

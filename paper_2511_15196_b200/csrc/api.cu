@@ -321,8 +321,7 @@ PHI4_API int smc_set_params(phi4smc* h, const smc_params* p) {
     return PHI4_EINVAL;
   if (p->kernel < 0 || p->kernel > 2 || p->z2_flip < 0 || p->z2_flip > 1) return PHI4_EINVAL;
   if (p->kernel == 2 && (h->kind != KIND_SMC || !irmh_supported(h->md.V))) return PHI4_EINVAL;
-  if (p->kernel == 1 && (h->kind != KIND_SMC || !hmc_supported(h->md.V) || !(p->hmc_eps > 0.f) ||
-                         p->hmc_leapfrog < 1))
+  if (p->kernel == 1 && (h->kind != KIND_SMC || !(p->hmc_eps > 0.f) || p->hmc_leapfrog < 1))
     return PHI4_EINVAL;
   h->prm = *p;
   h->s = p->step_scale > 0.f ? p->step_scale : 2.38f / sqrtf((float)h->md.V);
@@ -351,6 +350,12 @@ static bool use_tc_propose(const phi4smc* h) {
 }
 
 static void enqueue_mutation(phi4smc* h, const MutateArgs& a) {
+  if (h->prm.kernel == 1 && a.mode == MODE_SMC && !hmc_supported(a.md.V)) {
+    launch_hmc_generic(a.phi, a.S, a.U0, h->Sigma, a.phip, a.Z, h->W2, a.N, a.ld, a.md, h->prm.hmc_eps,
+                       h->prm.hmc_leapfrog, a.seed, a.t0, a.k, a.ctrl, a.acc_out, a.margin_out,
+                       a.respect_done, h->st);
+    return;
+  }
   if (h->prm.kernel == 1 && a.mode == MODE_SMC) {
     launch_hmc(a.phi, a.S, a.U0, h->Sigma, a.N, a.ld, a.md, h->prm.hmc_eps, h->prm.hmc_leapfrog,
                a.seed, a.t0, a.k, a.ctrl, a.acc_out, a.margin_out, a.respect_done, h->st);

@@ -255,3 +255,174 @@ void launch_hmc(float* phi, float* S, float* U0, const float* Sigma, int N, int 
 }
 
 }  // namespace phi4
+
+// ---------------------------------------------------------------------------------------------
+// Any lattice size: the fields of a trajectory no longer fit on one SM (L > 22), so position and
+// momentum live in HBM scratch ([V][ld] each) and every leapfrog half-step is its own launch
+// (the stencil needs the neighbours' updated positions: a grid-wide dependency).  HBM-bound:
+// ~28 B per site per leapfrog step.  Same arithmetic, streams and reading A14 as hmc_kernel.
+namespace phi4 {
+
+// momentum refresh, q <- phi, K0 = 1/2 sum z^2.  Block = 32 particles x 8 quad groups.
+__global__ void __launch_bounds__(256)
+hmc_g_init_kernel(const float* __restrict__ phi, float* __restrict__ q, float* __restrict__ p,
+                  const float* __restrict__ Sigma, float* __restrict__ K0, int N, int ld, int V,
+                  uint64_t seed, uint32_t t, const Ctrl* ctrl, int respect_done) {
+  if (respect_done && ctrl->done) return;
+  __shared__ float part[8][32];
+  const int lane = threadIdx.x & 31, g = threadIdx.x >> 5;
+  const int i = blockIdx.x * 32 + lane;
+  const int nq = (V + 3) >> 2;
+  float k0 = 0.f;
+  if (i < N) {
+    for (int qd = g; qd < nq; qd += 8) {
+      float z[4];
+      normals4(seed, TAG_PROP, t, (uint32_t)i, (uint32_t)qd, z);
+#pragma unroll
+      for (int e = 0; e < 4; ++e) {
+        const int x = 4 * qd + e;
+        if (x < V) {
+          const size_t o = (size_t)x * ld + i;
+          p[o] = z[e] * rsqrtf(Sigma[(size_t)x * V + x]);
+          q[o] = phi[o];
+          k0 = fmaf(0.5f * z[e], z[e], k0);
+        }
+      }
+    }
+  }
+  part[g][lane] = k0;
+  __syncthreads();
+  if (g == 0 && i < N) {
+    float a = 0.f;
+#pragma unroll
+    for (int m = 0; m < 8; ++m) a += part[m][lane];
+    K0[i] = a;
+  }
+}
+
+// p -= h grad U(q): one thread per (site, particle); blockIdx.y = site
+__global__ void __launch_bounds__(256)
+hmc_g_kick_kernel(const float* __restrict__ q, float* __restrict__ p, int N, int ld, Model md,
+                  float h, const Ctrl* ctrl, int respect_done) {
+  if (respect_done && ctrl->done) return;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= N) return;
+  const int L = md.L, x = blockIdx.y, r = x / L, c = x - r * L;
+  const int ce = c + 1 == L ? 0 : c + 1, cw = c == 0 ? L - 1 : c - 1;
+  const int rs = r + 1 == L ? 0 : r + 1, rn = r == 0 ? L - 1 : r - 1;
+  const float a = q[(size_t)x * ld + i];
+  const float e = q[(size_t)(r * L + ce) * ld + i], w = q[(size_t)(r * L + cw) * ld + i];
+  const float n = q[(size_t)(rn * L + c) * ld + i], s = q[(size_t)(rs * L + c) * ld + i];
+  const float beta = (float)ctrl->beta;
+  const float gs = fmaf(4.0f, a, -((e + w) + (n + s))) + a * fmaf(4.0f * md.lam, a * a, md.m0sq);
+  const size_t o = (size_t)x * ld + i;
+  p[o] = fmaf(-h, fmaf(beta, gs, a), p[o]);
+}
+
+// q += eps var p
+__global__ void __launch_bounds__(256)
+hmc_g_drift_kernel(float* __restrict__ q, const float* __restrict__ p,
+                   const float* __restrict__ Sigma, int N, int ld, int V, float eps,
+                   const Ctrl* ctrl, int respect_done) {
+  if (respect_done && ctrl->done) return;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= N) return;
+  const int x = blockIdx.y;
+  const size_t o = (size_t)x * ld + i;
+  q[o] = fmaf(eps * Sigma[(size_t)x * V + x], p[o], q[o]);
+}
+
+// H_new, margin, accept, commit.  Block = 32 particles x 8 row groups (as accept_kernel).
+__global__ void __launch_bounds__(256)
+hmc_g_accept_kernel(float* __restrict__ phi, const float* __restrict__ q,
+                    const float* __restrict__ p, const float* __restrict__ Sigma,
+                    const float* __restrict__ K0, float* __restrict__ S, float* __restrict__ U0,
+                    int N, int ld, Model md, uint64_t seed, uint32_t t, Ctrl* ctrl,
+                    uint8_t* __restrict__ acc_out, float* __restrict__ margin_out,
+                    int respect_done) {
+  if (respect_done && ctrl->done) return;
+  __shared__ float ps[8][32], pu[8][32], pk[8][32];
+  __shared__ int flag[32];
+  const int lane = threadIdx.x & 31, g = threadIdx.x >> 5;
+  const int i = blockIdx.x * 32 + lane;
+  const int L = md.L, V = md.V;
+  const float hm = 0.5f * md.m0sq, lam = md.lam;
+  const int band = (L + 7) >> 3, r_lo = min(L, g * band), r_hi = min(L, r_lo + band);
+  float Sp = 0.f, Up = 0.f, K1 = 0.f;
+  if (i < N) {
+    for (int r = r_lo; r < r_hi; ++r) {
+      const int rs = r + 1 == L ? 0 : r + 1;
+      float rowS = 0.f, rowU = 0.f, rowK = 0.f;       // two-level fp32 accumulation
+      float a = q[(size_t)(r * L) * ld + i];
+      for (int c = 0; c < L; ++c) {
+        const int x = r * L + c, ce = c + 1 == L ? 0 : c + 1;
+        const float b = q[(size_t)(r * L + ce) * ld + i], d = q[(size_t)(rs * L + c) * ld + i];
+        const float pp = p[(size_t)x * ld + i];
+        const float e1 = b - a, e2 = d - a, a2 = a * a;
+        rowS += 0.5f * (e1 * e1 + e2 * e2) + a2 * (hm + lam * a2);
+        rowU = fmaf(0.5f, a2, rowU);
+        rowK = fmaf(0.5f * Sigma[(size_t)x * V + x] * pp, pp, rowK);
+        a = b;
+      }
+      Sp += rowS; Up += rowU; K1 += rowK;
+    }
+  }
+  ps[g][lane] = Sp; pu[g][lane] = Up; pk[g][lane] = K1;
+  __syncthreads();
+  if (g == 0) {
+    int acc = 0;
+    if (i < N) {
+      float tS = 0.f, tU = 0.f, tK = 0.f;
+#pragma unroll
+      for (int m = 0; m < 8; ++m) { tS += ps[m][lane]; tU += pu[m][lane]; tK += pk[m][lane]; }
+      const float lu = log_uniform(seed, TAG_ACC, t, (uint32_t)i);
+      const float Si = S[i], Ui = U0[i];
+      const float margin = ((Ui - tU) + (float)ctrl->beta * (Si - tS) + (K0[i] - tK)) - lu;
+      acc = margin > 0.f;
+      if (acc) { S[i] = tS; U0[i] = tU; }
+      if (acc_out) acc_out[i] = (uint8_t)acc;
+      if (margin_out) margin_out[i] = margin;
+    }
+    flag[lane] = acc;
+    const unsigned m = __ballot_sync(0xffffffffu, acc);
+    if (lane == 0 && m) atomicAdd(&ctrl->n_accept, (unsigned)__popc(m));
+  }
+  __syncthreads();
+  if (i < N && flag[lane]) {
+    for (int r = r_lo; r < r_hi; ++r)
+      for (int c = 0; c < L; ++c) {
+        const size_t o = (size_t)(r * L + c) * ld + i;
+        phi[o] = q[o];
+      }
+  }
+}
+
+// q, p: [V][ld] scratch each; K0: [ld] scratch
+void launch_hmc_generic(float* phi, float* S, float* U0, const float* Sigma, float* q, float* p,
+                        float* K0, int N, int ld, Model md, float eps, int nfrog, uint64_t seed,
+                        uint32_t t0, int k, Ctrl* ctrl, uint8_t* acc_out, float* margin_out,
+                        int respect_done, cudaStream_t st) {
+  const int V = md.V;
+  const dim3 gs((N + 255) / 256, V);
+  for (int j = 0; j < k; ++j) {
+    const uint32_t t = t0 + (uint32_t)j;
+    ++g_launches;
+    hmc_g_init_kernel<<<ld / 32, 256, 0, st>>>(phi, q, p, Sigma, K0, N, ld, V, seed, t, ctrl, respect_done);
+    ++g_launches;
+    hmc_g_kick_kernel<<<gs, 256, 0, st>>>(q, p, N, ld, md, 0.5f * eps, ctrl, respect_done);
+    for (int s = 0; s < nfrog; ++s) {
+      ++g_launches;
+      hmc_g_drift_kernel<<<gs, 256, 0, st>>>(q, p, Sigma, N, ld, V, eps, ctrl, respect_done);
+      ++g_launches;
+      hmc_g_kick_kernel<<<gs, 256, 0, st>>>(q, p, N, ld, md, (s + 1 == nfrog) ? 0.5f * eps : eps, ctrl,
+                                            respect_done);
+    }
+    ++g_launches;
+    hmc_g_accept_kernel<<<ld / 32, 256, 0, st>>>(
+        phi, q, p, Sigma, K0, S, U0, N, ld, md, seed, t, ctrl,
+        acc_out ? acc_out + (size_t)j * N : nullptr, margin_out ? margin_out + (size_t)j * N : nullptr,
+        respect_done);
+  }
+}
+
+}  // namespace phi4

@@ -66,18 +66,16 @@ def hmc_lockstep(L, N, k, beta, seed, eps, nfrog, m0sq=-4.0, lam=1.0, t_start=0,
     (4, 1024, 4, 0.5, 0.1, 10, "init"), (5, 333, 3, 0.7, 0.15, 7, "smooth"),
     (1, 200, 5, 1.0, 0.1, 5, "init"), (2, 129, 4, 0.5, 0.1, 8, "init"),
     (9, 640, 2, 0.6, 0.1, 20, "smooth"), (16, 2048, 2, 0.2, 0.1, 20, "smooth"),
-    (22, 500, 1, 0.4, 0.05, 12, "smooth"), (11, 31, 2, 0.0, 0.1, 6, "init")])
+    (22, 500, 1, 0.4, 0.05, 12, "smooth"), (11, 31, 2, 0.0, 0.1, 6, "init"),
+    # L > 22: position and momentum in HBM scratch, one launch per leapfrog half-step
+    (23, 300, 2, 0.4, 0.05, 10, "smooth"), (32, 200, 1, 0.3, 0.04, 8, "smooth")])
 def test_hmc_lockstep(L, N, k, beta, eps, nfrog, fields):
     rate, _ = hmc_lockstep(L, N, k, beta, seed=31 + L, eps=eps, nfrog=nfrog, fields=fields,
                            t_start=5 * k)
     assert 0.0 < rate <= 1.0
 
 
-def test_hmc_rejects_unsupported():
-    h = B.smc_init(23, -4.0, 1.0, 256, 1)           # V = 529 > 512: three tiles do not fit
-    with pytest.raises(B.Phi4Error):
-        B.smc_set_params(h, kernel=1)
-    h.close()
+def test_hmc_rejects_bad_parameters():
     h = B.smc_init(10, -4.0, 1.0, 256, 1)
     for bad in (dict(hmc_eps=0.0), dict(hmc_leapfrog=0), dict(kernel=3)):
         with pytest.raises(B.Phi4Error):
