@@ -127,6 +127,7 @@ accept_kernel(float* __restrict__ phi, const float* __restrict__ phip, float* __
               uint32_t tag_acc, uint32_t t, Ctrl* ctrl, uint8_t* __restrict__ acc_out,
               float* __restrict__ margin_out, int respect_done, const float* __restrict__ Z,
               float* __restrict__ W2) {
+  pdl_enter();
   if (respect_done && ctrl->done) return;
   __shared__ float ps[G][32], pu[G][32], pz[IRMH ? G : 1][32];
   __shared__ int flag[32];
@@ -274,15 +275,17 @@ void launch_mutate_generic(const MutateArgs& a, float* Lsplit, cudaStream_t st) 
     }
     ++g_launches;
     if (wide)
-      accept_kernel<false, 32><<<a.ld / 32, 1024, 0, st>>>(
-          a.phi, a.phip, a.S, a.U0, a.N, a.ld, a.md, a.mode, a.seed, a.tag_acc, t, a.ctrl,
-          a.acc_out ? a.acc_out + (size_t)j * a.N : nullptr,
-          a.margin_out ? a.margin_out + (size_t)j * a.N : nullptr, a.respect_done, nullptr, nullptr);
+      launch_pdl(accept_kernel<false, 32>, a.ld / 32, 1024, 0, st,
+                 a.phi, a.phip, a.S, a.U0, a.N, a.ld, a.md, a.mode, a.seed, a.tag_acc, t, a.ctrl,
+                 a.acc_out ? a.acc_out + (size_t)j * a.N : nullptr,
+                 a.margin_out ? a.margin_out + (size_t)j * a.N : nullptr, a.respect_done,
+                 (const float*)nullptr, (float*)nullptr);
     else
-      accept_kernel<false, 8><<<a.ld / 32, 256, 0, st>>>(
-          a.phi, a.phip, a.S, a.U0, a.N, a.ld, a.md, a.mode, a.seed, a.tag_acc, t, a.ctrl,
-          a.acc_out ? a.acc_out + (size_t)j * a.N : nullptr,
-          a.margin_out ? a.margin_out + (size_t)j * a.N : nullptr, a.respect_done, nullptr, nullptr);
+      launch_pdl(accept_kernel<false, 8>, a.ld / 32, 256, 0, st,
+                 a.phi, a.phip, a.S, a.U0, a.N, a.ld, a.md, a.mode, a.seed, a.tag_acc, t, a.ctrl,
+                 a.acc_out ? a.acc_out + (size_t)j * a.N : nullptr,
+                 a.margin_out ? a.margin_out + (size_t)j * a.N : nullptr, a.respect_done,
+                 (const float*)nullptr, (float*)nullptr);
   }
 }
 

@@ -45,6 +45,7 @@ constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 256;
 __global__ void __launch_bounds__(128)
 normals_split_kernel(float4* __restrict__ Zs, int N, int ntm, int V, int Kp, uint64_t seed,
                      uint32_t tag, uint32_t t, const Ctrl* ctrl, int respect_done) {
+  pdl_enter();
   if (respect_done && ctrl->done) return;
   const int m = blockIdx.x, q = blockIdx.y, pr = threadIdx.x;
   const int i = m * lg::TILE + pr, nkc = Kp >> 2;
@@ -75,6 +76,7 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
   using namespace tc;
   using namespace lg;
   extern __shared__ __align__(1024) uint8_t smem[];
+  pdl_enter();
   if (p.respect_done && p.ctrl->done) return;
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + STAGES * STAGE_BYTES);
   const uint32_t bar0 = smem_u32(bars);
@@ -282,8 +284,8 @@ void launch_normals_split(float* Zs, int N, int ld, int V, uint64_t seed, uint32
   const int Kp = round_up(V, 16);
   dim3 grid(ld / lg::TILE, Kp / 4);
   ++g_launches;
-  normals_split_kernel<<<grid, 128, 0, st>>>(reinterpret_cast<float4*>(Zs), N, ld / lg::TILE, V, Kp,
-                                             seed, tag, t, ctrl, respect_done);
+  launch_pdl(normals_split_kernel, grid, 128, 0, st, reinterpret_cast<float4*>(Zs), N, ld / lg::TILE, V, Kp,
+             seed, tag, t, ctrl, respect_done);
 }
 
 void launch_propose_tc(const float* phi, float* phip, const float* Zs, const float* Lsplit, int ld,
@@ -304,7 +306,7 @@ void launch_propose_tc(const float* phi, float* phip, const float* Zs, const flo
   const int ntiles = p.ntm * p.ntn;
   const int grid = ntiles < num_sms ? ntiles : num_sms;
   ++g_launches;
-  propose_tc_kernel<<<grid, lg::THREADS, lg::SMEM_BYTES, st>>>(p);
+  launch_pdl(propose_tc_kernel, grid, lg::THREADS, lg::SMEM_BYTES, st, p);
 }
 
 }  // namespace phi4
