@@ -76,8 +76,8 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
   using namespace tc;
   using namespace lg;
   extern __shared__ __align__(1024) uint8_t smem[];
-  pdl_enter();
-  if (p.respect_done && p.ctrl->done) return;
+  // programmatic dependent launch: barrier setup and the TMEM allocation run before the wait
+  pdl_trigger();
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + STAGES * STAGE_BYTES);
   const uint32_t bar0 = smem_u32(bars);
   auto full = [&](int s) { return bar0 + 8u * s; };
@@ -99,6 +99,11 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
   tc_fence_after();
   const uint32_t taddr = *tmem_slot;
   const uint32_t ring = smem_u32(smem);
+  pdl_wait();
+  if (p.respect_done && p.ctrl->done) {
+    if (warp == 0) tmem_dealloc(taddr, 2 * TN);
+    return;
+  }
 
   if (warp == 8) {
     // ================================ producer: bulk copies into the ring =====================
