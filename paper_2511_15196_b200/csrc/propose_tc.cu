@@ -69,7 +69,33 @@ struct ProposeTcParams {
   const float* Lsplit;               // packed s*Lc hi | lo (tcgen05.cuh layout)
   const Ctrl* ctrl;
   int ld, V, Vn, Kp, ntm, ntn;       // Vn = V rounded up to 256 rows, Kp = V rounded up to 16
-  int respect_done;
+  int respect_done, pair;
+};
+
+// Tile order.  Work item w of a CTA (w = blockIdx.x, + gridDim.x, ...) is one half of a *pair* of
+// site tiles (j, ntn-1-j) of one particle tile m: a pair always spans ntn+1 K-blocks of 256, so the
+// CTAs stay in step, and the ceil(ntn/2) CTAs that hold the pairs of the same m at the same time
+// stream the same normal tile from K = 0 upwards together -- one HBM read, the rest L2 hits
+// (round 1 ran tile-index round robin: the 4 MB normal tile of a particle block at C4 was re-read
+// from HBM by every one of its 16 site tiles, 39 GB per launch against 8.6 GB of operands).
+// Populations with fewer tiles than SMs (pair = 0) keep one tile per CTA.
+struct TileIter {
+  int pair, np, nunits, ntn, u, half;
+  __device__ TileIter(int ntm, int ntn_, int pair_)
+      : pair(pair_), np(pair_ ? (ntn_ + 1) >> 1 : ntn_), nunits(ntm * np), ntn(ntn_),
+        u(blockIdx.x), half(0) {}
+  __device__ bool valid() const { return u < nunits; }
+  __device__ void tile(int& m, int& n) const {
+    m = u / np;
+    const int j = u % np;
+    n = half ? ntn - 1 - j : j;
+  }
+  __device__ void next() {
+    const int j = u % np;
+    if (pair && !half && ntn - 1 - j != j) { half = 1; return; }
+    half = 0;
+    u += gridDim.x;
+  }
 };
 
 __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const ProposeTcParams p) {
@@ -86,7 +112,7 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
   auto dempty = [&](int b) { return bar0 + 8u * (2 * STAGES + 2 + b); };
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * STAGES + 4);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int V = p.V, Vn = p.Vn, Kp = p.Kp, nkc = Kp >> 2, ntiles = p.ntm * p.ntn;
+  const int V = p.V, Vn = p.Vn, Kp = p.Kp, nkc = Kp >> 2;
 
   if (warp == 8 && lane == 0) {
     for (int s = 0; s < STAGES; ++s) { mbar_init(full(s), 1); mbar_init(empty(s), 1); }
@@ -111,8 +137,10 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
       const size_t lpart = l_floats_vk(Vn, Kp);
       int s = 0;
       uint32_t ph = 0;
-      for (int tl = blockIdx.x; tl < ntiles; tl += gridDim.x) {
-        const int m = tl / p.ntn, n0 = (tl % p.ntn) * TN;
+      for (TileIter ti(p.ntm, p.ntn, p.pair); ti.valid(); ti.next()) {
+        int m, tn;
+        ti.tile(m, tn);
+        const int n0 = tn * TN;
         const int nst = min(n0 + TN, Kp) >> 4;               // K-stages up to the tile's last row
         for (int it = 0; it < nst; ++it) {
           mbar_wait(empty(s), ph ^ 1);
@@ -161,8 +189,10 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
       uint32_t ph = 0;
       const uint64_t a_base = smem_desc(ring, CHUNK_A, 128);
       const uint64_t b_base = smem_desc(ring + 2 * A_PART, CHUNK_B, 128);
-      for (int tl = blockIdx.x; tl < ntiles; tl += gridDim.x) {
-        const int n0 = (tl % p.ntn) * TN;
+      for (TileIter ti(p.ntm, p.ntn, p.pair); ti.valid(); ti.next()) {
+        int m, tn;
+        ti.tile(m, tn);
+        const int n0 = tn * TN;
         const int nst = min(n0 + TN, Kp) >> 4;
         for (int it0 = 0; it0 < nst; it0 += SUB_STAGES, ++cnt) {
           const int buf = cnt & 1;
@@ -206,8 +236,10 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
     int cnt = 0;
     const int Q = warp & 3, hc = warp >> 2;
     const uint32_t tlane = taddr + ((uint32_t)(Q * 32) << 16);
-    for (int tl = blockIdx.x; tl < ntiles; tl += gridDim.x) {
-      const int m = tl / p.ntn, n0 = (tl % p.ntn) * TN;
+    for (TileIter ti(p.ntm, p.ntn, p.pair); ti.valid(); ti.next()) {
+      int m, tn;
+      ti.tile(m, tn);
+      const int n0 = tn * TN;
       const int nst = min(n0 + TN, Kp) >> 4;
       const size_t col = (size_t)m * TILE + Q * 32 + lane;
       const int x0 = n0 + hc * 128;
@@ -308,8 +340,9 @@ void launch_propose_tc(const float* phi, float* phip, const float* Zs, const flo
   p.ld = ld; p.V = V;
   propose_tc_dims(V, &p.Vn, &p.Kp);
   p.ntm = ld / lg::TILE; p.ntn = p.Vn / lg::TN; p.respect_done = respect_done;
-  const int ntiles = p.ntm * p.ntn;
-  const int grid = ntiles < num_sms ? ntiles : num_sms;
+  p.pair = p.ntm * p.ntn > num_sms;
+  const int nunits = p.ntm * (p.pair ? (p.ntn + 1) / 2 : p.ntn);
+  const int grid = nunits < num_sms ? nunits : num_sms;
   ++g_launches;
   launch_pdl(propose_tc_kernel, grid, lg::THREADS, lg::SMEM_BYTES, st, p);
 }
