@@ -54,6 +54,9 @@ def lib():
         "orc_uniform": (C.c_double, [C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32]),
         "orc_word0": (C.c_uint32, [C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32]),
         "orc_action_field": (C.c_double, [_dp, C.c_int, C.c_double, C.c_double, vp]),
+        "orc_set_kinetic": (None, [C.c_double]),
+        "orc_get_kinetic": (C.c_double, []),
+        "orc_action_eq2_field": (C.c_double, [_dp, C.c_int, C.c_double, C.c_double]),
         "orc_u0_field": (C.c_double, [_dp, C.c_int]),
         "orc_action_grad_field": (None, [_dp, C.c_int, C.c_double, C.c_double, _dp]),
         "orc_action_batch": (None, [_dp, C.c_int, C.c_int, C.c_double, C.c_double, _dp, _dp, vp]),
@@ -154,6 +157,35 @@ def action_field(f, L, m0sq, lam, with_abs=False):
     a = C.c_double(0.0)
     s = lib().orc_action_field(f, L, m0sq, lam, C.cast(C.byref(a), C.c_void_p))
     return (s, a.value) if with_abs else s
+
+
+class kinetic:
+    """`with kinetic(kappa):` -- every oracle call inside evaluates Eq. 1 with its kinetic term
+    multiplied by kappa (Eq. 2; reading A18).  Restores the previous value."""
+
+    def __init__(self, kappa):
+        self.kappa = float(kappa)
+
+    def __enter__(self):
+        self.prev = lib().orc_get_kinetic()
+        lib().orc_set_kinetic(self.kappa)
+        return self
+
+    def __exit__(self, *exc):
+        lib().orc_set_kinetic(self.prev)
+        return False
+
+
+def kl_to_eq1(kappa, lam):
+    """Eq. 2's (kappa, lambda) as Eq. 1 coefficients (Eq. 4): (kinetic, m0sq, lambda) and the
+    constant V*lambda per site that Eq. 5 drops (returned per site)."""
+    return float(kappa), 2.0 * (1.0 - 2.0 * lam), float(lam), float(lam)
+
+
+def action_eq2_field(f, L, kappa, lam):
+    """Eq. 2 verbatim, constant included."""
+    f = _f64(f).reshape(-1)
+    return lib().orc_action_eq2_field(f, L, kappa, lam)
 
 
 def u0_field(f):

@@ -144,6 +144,32 @@ uint32_t orc_word0(uint64_t seed, uint32_t tag, uint32_t t, uint32_t i) {
  * L = 1, 2).  If absum != NULL it receives sum_x(|kin_x|+|mass_x|+|quart_x|)
  * (the scale of reading A12's tolerance).
  * ---------------------------------------------------------------------- */
+/* Appendix G ("Alternative parameterizations"): a physical
+ * nearest-neighbour coupling kappa "that scales only the kinetic term",
+ *   Eq. 2: S_E(phi; kappa, lambda) = kappa/2 sum_{x,mu} (phi_{x+mu}-phi_x)^2
+ *                                    + sum_x [ phi_x^2 + lambda (phi_x^2-1)^2 ].
+ * By Eq. 4, phi^2 + lambda (phi^2-1)^2 = lambda phi^4 + (1-2 lambda) phi^2 + lambda, so
+ * Eq. 2 is Eq. 1 with the kinetic term multiplied by kappa, m0^2 = 2 (1 - 2 lambda), the
+ * same quartic coefficient, plus the constant V lambda (Eq. 5 drops it: it "only shifts
+ * log Z").  The oracle keeps one kinetic coefficient for the whole process (1 = Eq. 1);
+ * every action, gradient, mutation and run below reads it.  orc_action_eq2_field is
+ * Eq. 2 written out verbatim, constant included (reading A18). */
+static double orc_kappa = 1.0;
+void orc_set_kinetic(double kappa) { orc_kappa = kappa; }
+double orc_get_kinetic(void) { return orc_kappa; }
+
+double orc_action_eq2_field(const double* f, int L, double kappa, double lam) {
+  double S = 0.0;
+  for (int r = 0; r < L; ++r)
+    for (int c = 0; c < L; ++c) {
+      double p = f[r * L + c];
+      double pr = f[r * L + (c + 1) % L], pd = f[((r + 1) % L) * L + c];
+      S += 0.5 * kappa * ((pr - p) * (pr - p) + (pd - p) * (pd - p));
+      S += p * p + lam * (p * p - 1.0) * (p * p - 1.0);
+    }
+  return S;
+}
+
 double orc_action_field(const double* f, int L, double m0sq, double lam,
                         double* absum) {
   double S = 0.0, A = 0.0;
@@ -152,7 +178,7 @@ double orc_action_field(const double* f, int L, double m0sq, double lam,
       double p = f[r * L + c];
       double pr = f[r * L + (c + 1) % L];       /* x + 1-hat (next column) */
       double pd = f[((r + 1) % L) * L + c];     /* x + 2-hat (next row)    */
-      double kin = 0.5 * ((pr - p) * (pr - p) + (pd - p) * (pd - p));
+      double kin = 0.5 * orc_kappa * ((pr - p) * (pr - p) + (pd - p) * (pd - p));
       double mass = 0.5 * m0sq * p * p;
       double quart = lam * p * p * p * p;
       S += kin + mass + quart;
@@ -170,8 +196,8 @@ double orc_u0_field(const double* f, int V) {
   return 0.5 * u;
 }
 
-/* Gradient dS_E/dphi_x of Eq. 1 (used only by the finite-difference pin):
- * sum_mu (2 phi_x - phi_{x+mu} - phi_{x-mu}) + m0^2 phi_x + 4 lambda phi_x^3 */
+/* Gradient dS_E/dphi_x of Eq. 1 (finite-difference pin, HMC force):
+ * kappa sum_mu (2 phi_x - phi_{x+mu} - phi_{x-mu}) + m0^2 phi_x + 4 lambda phi_x^3 */
 void orc_action_grad_field(const double* f, int L, double m0sq, double lam,
                            double* g) {
   for (int r = 0; r < L; ++r)
@@ -179,7 +205,7 @@ void orc_action_grad_field(const double* f, int L, double m0sq, double lam,
       double p = f[r * L + c];
       double e = f[r * L + (c + 1) % L], w = f[r * L + (c + L - 1) % L];
       double s = f[((r + 1) % L) * L + c], n = f[((r + L - 1) % L) * L + c];
-      g[r * L + c] = (4.0 * p - e - w - s - n) + m0sq * p + 4.0 * lam * p * p * p;
+      g[r * L + c] = orc_kappa * (4.0 * p - e - w - s - n) + m0sq * p + 4.0 * lam * p * p * p;
     }
 }
 
