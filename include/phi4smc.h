@@ -131,6 +131,18 @@ size_t smc_workspace_bytes(int L, int N);
  * d_workspace: device memory of >= smc_workspace_bytes(L,N).  Enqueues on cuda_stream, no sync.  */
 int smc_init(phi4smc** out, int L, float m0sq, float lambda, int N, uint64_t seed,
              void* d_workspace, size_t workspace_bytes, void* cuda_stream);
+/* The kappa-lambda parameterisation (Appendix G; reading A18):
+ *   Eq. 2: S_E(phi; kappa, lambda) = kappa/2 sum_{x,mu} (phi_{x+mu}-phi_x)^2
+ *                                    + sum_x [ phi_x^2 + lambda (phi_x^2 - 1)^2 ],
+ * kappa >= 0 the physical nearest-neighbour coupling that "scales only the kinetic term".  By
+ * Eq. 4 this is Eq. 1's stencil with the kinetic term multiplied by kappa, m0sq = 2 (1 - 2 lambda)
+ * and the same quartic coefficient; the additive constant V*lambda is dropped as in Eq. 5, so
+ * every S_E and log_Z of such a handle refers to Eq. 5 (subtract V*lambda from log_Z for Eq. 2).
+ * U0, the tempering path and everything else are as for smc_init; the same kernels run (the
+ * kinetic coefficient is a model parameter of every stencil).  PHI4_EINVAL if kappa or lambda is
+ * negative or not finite.                                                                       */
+int smc_init_kl(phi4smc** out, int L, float kappa, float lambda, int N, uint64_t seed,
+                void* d_workspace, size_t workspace_bytes, void* cuda_stream);
 /* Re-initialises an existing handle (SMC or NS) with a new seed exactly as *_init would: fresh
  * particles from stream INIT, beta = 0, logZ = 0 (NS: -inf, logX = 0), Lc = I, history cleared.
  * Device work only (no host allocation); enqueue only.                                          */
@@ -177,6 +189,10 @@ size_t ns_workspace_bytes(int L, int n_live, int k_delete, int max_iters);
 int ns_init(phi4smc** out, int L, float m0sq, float lambda, int n_live, int k_delete, int n_walk,
             uint64_t seed, double stop_frac, int max_iters, void* d_workspace,
             size_t workspace_bytes, void* cuda_stream);
+/* ns_init for Eq. 2's (kappa, lambda); see smc_init_kl.                                         */
+int ns_init_kl(phi4smc** out, int L, float kappa, float lambda, int n_live, int k_delete,
+               int n_walk, uint64_t seed, double stop_frac, int max_iters, void* d_workspace,
+               size_t workspace_bytes, void* cuda_stream);
 /* One iteration N1-N4.  info != NULL synchronises.  No-op once done.              */
 int ns_set_params(phi4smc* h, const ns_params* p); /* defaults: inner 0, width 1, 8, 32          */
 int ns_step(phi4smc* h, ns_step_info* info);

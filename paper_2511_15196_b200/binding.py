@@ -74,6 +74,7 @@ SIGNATURES = {
     "phi4_kernel_launches": (_u64, []),
     "smc_workspace_bytes": (_sz, [_i, _i]),
     "smc_init": (_i, [C.POINTER(_vp), _i, _f, _f, _i, _u64, _vp, _sz, _vp]),
+    "smc_init_kl": (_i, [C.POINTER(_vp), _i, _f, _f, _i, _u64, _vp, _sz, _vp]),
     "smc_reset": (_i, [_vp, _u64]),
     "smc_destroy": (_i, [_vp]),
     "smc_set_params": (_i, [_vp, C.POINTER(smc_params)]),
@@ -85,6 +86,7 @@ SIGNATURES = {
     "log_Z": (_d, [_vp]),
     "ns_workspace_bytes": (_sz, [_i, _i, _i, _i]),
     "ns_init": (_i, [C.POINTER(_vp), _i, _f, _f, _i, _i, _i, _u64, _d, _i, _vp, _sz, _vp]),
+    "ns_init_kl": (_i, [C.POINTER(_vp), _i, _f, _f, _i, _i, _i, _u64, _d, _i, _vp, _sz, _vp]),
     "ns_set_params": (_i, [_vp, C.POINTER(ns_params)]),
     "ns_step": (_i, [_vp, C.POINTER(ns_step_info)]),
     "ns_run": (_i, [_vp, _i, C.POINTER(_i)]),
@@ -177,7 +179,7 @@ def ns_workspace_bytes(L, n_live, k_delete, max_iters):
     return load().ns_workspace_bytes(L, n_live, k_delete, max_iters)
 
 
-def smc_init(L, m0sq, lam, N, seed, device="cuda:0"):
+def smc_init(L, m0sq, lam, N, seed, device="cuda:0", _entry="smc_init"):
     lib = load()
     nbytes = lib.smc_workspace_bytes(L, N)
     if nbytes == 0:
@@ -185,18 +187,23 @@ def smc_init(L, m0sq, lam, N, seed, device="cuda:0"):
     ws = _device_workspace(nbytes, device)
     base = _aligned(ws)
     ptr = C.c_void_p()
-    rc = lib.smc_init(C.byref(ptr), L, m0sq, lam, N, seed, C.c_void_p(base),
-                      nbytes, _stream_ptr(device))
+    rc = getattr(lib, _entry)(C.byref(ptr), L, m0sq, lam, N, seed, C.c_void_p(base),
+                              nbytes, _stream_ptr(device))
     if rc != 0:
         detail = lib.phi4_last_cuda_error(ptr if ptr else None).decode()
         if ptr:
             lib.smc_destroy(ptr)
-        raise Phi4Error(rc, "smc_init", detail)
+        raise Phi4Error(rc, _entry, detail)
     return Handle(ptr, ws, "smc", L, N)
 
 
+def smc_init_kl(L, kappa, lam, N, seed, device="cuda:0"):
+    """Eq. 2's (kappa, lambda) parameterisation (include/phi4smc.h: smc_init_kl)."""
+    return smc_init(L, kappa, lam, N, seed, device, _entry="smc_init_kl")
+
+
 def ns_init(L, m0sq, lam, n_live, k_delete, n_walk, seed, stop_frac=1e-3, max_iters=4096,
-            device="cuda:0"):
+            device="cuda:0", _entry="ns_init"):
     lib = load()
     nbytes = lib.ns_workspace_bytes(L, n_live, k_delete, max_iters)
     if nbytes == 0:
@@ -204,14 +211,21 @@ def ns_init(L, m0sq, lam, n_live, k_delete, n_walk, seed, stop_frac=1e-3, max_it
     ws = _device_workspace(nbytes, device)
     base = _aligned(ws)
     ptr = C.c_void_p()
-    rc = lib.ns_init(C.byref(ptr), L, m0sq, lam, n_live, k_delete, n_walk, seed, stop_frac,
-                     max_iters, C.c_void_p(base), nbytes, _stream_ptr(device))
+    rc = getattr(lib, _entry)(C.byref(ptr), L, m0sq, lam, n_live, k_delete, n_walk, seed, stop_frac,
+                              max_iters, C.c_void_p(base), nbytes, _stream_ptr(device))
     if rc != 0:
         detail = lib.phi4_last_cuda_error(ptr if ptr else None).decode()
         if ptr:
             lib.smc_destroy(ptr)
-        raise Phi4Error(rc, "ns_init", detail)
+        raise Phi4Error(rc, _entry, detail)
     return Handle(ptr, ws, "ns", L, n_live, k_delete=k_delete, n_walk=n_walk, max_iters=max_iters)
+
+
+def ns_init_kl(L, kappa, lam, n_live, k_delete, n_walk, seed, stop_frac=1e-3, max_iters=4096,
+               device="cuda:0"):
+    """Eq. 2's (kappa, lambda) parameterisation (include/phi4smc.h: ns_init_kl)."""
+    return ns_init(L, kappa, lam, n_live, k_delete, n_walk, seed, stop_frac, max_iters, device,
+                   _entry="ns_init_kl")
 
 
 def smc_reset(h, seed):

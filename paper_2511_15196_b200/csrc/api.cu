@@ -155,12 +155,14 @@ static int carve_ns(phi4smc* h, char* base, size_t* total) {
   return 0;
 }
 
-static phi4smc* new_handle(int kind, int L, float m0sq, float lambda, int N, uint64_t seed) {
+static phi4smc* new_handle(int kind, int L, float kappa, float m0sq, float lambda, int N,
+                           uint64_t seed) {
   phi4smc* h = new (std::nothrow) phi4smc;
   if (!h) return nullptr;
   memset(h, 0, sizeof(*h));
   h->kind = kind;
   h->md.L = L; h->md.V = L * L; h->md.m0sq = m0sq; h->md.lam = lambda;
+  h->md.kappa = kappa;
   h->N = N; h->ld = round_up(N, 128);
   h->seed = seed;
   h->prm.k_steps = 10; h->prm.ess_target = 0.5f; h->prm.step_scale = 0.f; h->prm.mutation_path = 0;
@@ -253,15 +255,16 @@ static int push_ctrl(phi4smc* h) {
 }
 
 // ------------------------------------------------------------------------------ SMC ----------
-PHI4_API int smc_init(phi4smc** out, int L, float m0sq, float lambda, int N, uint64_t seed,
-                        void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
+static int smc_init_impl(phi4smc** out, int L, float kappa, float m0sq, float lambda, int N,
+                         uint64_t seed, void* d_workspace, size_t workspace_bytes,
+                         void* cuda_stream) {
   if (!out) return PHI4_EINVAL;
   *out = nullptr;
   size_t need = smc_workspace_bytes(L, N);
   if (need == 0 || !d_workspace || workspace_bytes < need ||
       (reinterpret_cast<uintptr_t>(d_workspace) % ALIGN) != 0)
     return PHI4_EINVAL;
-  phi4smc* h = new_handle(KIND_SMC, L, m0sq, lambda, N, seed);
+  phi4smc* h = new_handle(KIND_SMC, L, kappa, m0sq, lambda, N, seed);
   if (!h) return PHI4_ENOMEM;
   h->st = reinterpret_cast<cudaStream_t>(cuda_stream);
   h->max_rec = MAX_RECORDS;
@@ -277,6 +280,21 @@ PHI4_API int smc_init(phi4smc** out, int L, float m0sq, float lambda, int N, uin
   launch_set_identity(h->Lc, h->md.V, h->st);
   CU(cudaGetLastError());
   return PHI4_OK;
+}
+
+PHI4_API int smc_init(phi4smc** out, int L, float m0sq, float lambda, int N, uint64_t seed,
+                        void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
+  return smc_init_impl(out, L, 1.0f, m0sq, lambda, N, seed, d_workspace, workspace_bytes,
+                       cuda_stream);
+}
+
+// Eq. 2 -> Eq. 1 coefficients by Eq. 4 (reading A18): kinetic kappa,
+// m0^2 = 2 (1 - 2 lambda), quartic lambda; the constant V lambda is dropped as in Eq. 5.
+PHI4_API int smc_init_kl(phi4smc** out, int L, float kappa, float lambda, int N, uint64_t seed,
+                           void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (!(kappa >= 0.f) || !(lambda >= 0.f)) { if (out) *out = nullptr; return PHI4_EINVAL; }
+  return smc_init_impl(out, L, kappa, 2.0f * (1.0f - 2.0f * lambda), lambda, N, seed, d_workspace,
+                       workspace_bytes, cuda_stream);
 }
 
 PHI4_API int smc_reset(phi4smc* h, uint64_t seed) {
@@ -544,9 +562,9 @@ static NsArgs ns_args(phi4smc* h) {
   return a;
 }
 
-PHI4_API int ns_init(phi4smc** out, int L, float m0sq, float lambda, int n_live, int k_delete,
-                       int n_walk, uint64_t seed, double stop_frac, int max_iters,
-                       void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
+static int ns_init_impl(phi4smc** out, int L, float kappa, float m0sq, float lambda, int n_live,
+                        int k_delete, int n_walk, uint64_t seed, double stop_frac, int max_iters,
+                        void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
   if (!out) return PHI4_EINVAL;
   *out = nullptr;
   if (n_live > 16384 || k_delete > 1024 || n_walk < 1 || !(stop_frac > 0.0)) return PHI4_EINVAL;
@@ -554,7 +572,7 @@ PHI4_API int ns_init(phi4smc** out, int L, float m0sq, float lambda, int n_live,
   if (need == 0 || !d_workspace || workspace_bytes < need ||
       (reinterpret_cast<uintptr_t>(d_workspace) % ALIGN) != 0)
     return PHI4_EINVAL;
-  phi4smc* h = new_handle(KIND_NS, L, m0sq, lambda, n_live, seed);
+  phi4smc* h = new_handle(KIND_NS, L, kappa, m0sq, lambda, n_live, seed);
   if (!h) return PHI4_ENOMEM;
   h->st = reinterpret_cast<cudaStream_t>(cuda_stream);
   h->k_del = k_delete; h->ldw = round_up(k_delete, 128); h->n_walk = n_walk;
@@ -576,6 +594,22 @@ PHI4_API int ns_init(phi4smc** out, int L, float m0sq, float lambda, int n_live,
   CU(cudaStreamSynchronize(h->st));
   CU(cudaGetLastError());
   return PHI4_OK;
+}
+
+PHI4_API int ns_init(phi4smc** out, int L, float m0sq, float lambda, int n_live, int k_delete,
+                       int n_walk, uint64_t seed, double stop_frac, int max_iters,
+                       void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
+  return ns_init_impl(out, L, 1.0f, m0sq, lambda, n_live, k_delete, n_walk, seed, stop_frac,
+                      max_iters, d_workspace, workspace_bytes, cuda_stream);
+}
+
+PHI4_API int ns_init_kl(phi4smc** out, int L, float kappa, float lambda, int n_live, int k_delete,
+                          int n_walk, uint64_t seed, double stop_frac, int max_iters,
+                          void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (!(kappa >= 0.f) || !(lambda >= 0.f)) { if (out) *out = nullptr; return PHI4_EINVAL; }
+  return ns_init_impl(out, L, kappa, 2.0f * (1.0f - 2.0f * lambda), lambda, n_live, k_delete,
+                      n_walk, seed, stop_frac, max_iters, d_workspace, workspace_bytes,
+                      cuda_stream);
 }
 
 static void enqueue_ns_step(phi4smc* h) {

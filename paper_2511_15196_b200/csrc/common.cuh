@@ -44,9 +44,11 @@ struct StepRecord {
   int n_unique, chol_status, index, done;
 };
 
+// kappa: coefficient of the kinetic term (1 = Eq. 1; Eq. 2 scales it, reading A18).
+// With kappa = 1 every kernel computes bit-for-bit what it computed before the field existed.
 struct Model {
   int L, V;
-  float m0sq, lam;
+  float m0sq, lam, kappa;
 };
 
 __host__ __device__ inline int round_up(int a, int b) { return (a + b - 1) / b * b; }

@@ -47,7 +47,7 @@ action_kernel(const float* __restrict__ phi, int N, int ld, Model md, float* __r
         float b = row[(size_t)cn * ld];
         float d = rown[(size_t)c * ld];
         float e = b - a, f = d - a, a2 = a * a;
-        s += 0.5f * (e * e + f * f) + a2 * (0.5f * md.m0sq + md.lam * a2);
+        s += 0.5f * md.kappa * (e * e + f * f) + a2 * (0.5f * md.m0sq + md.lam * a2);
         u += 0.5f * a2;
         a = b;
       }

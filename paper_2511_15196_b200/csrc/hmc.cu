@@ -49,7 +49,7 @@ __device__ __forceinline__ void cta_sync() { asm volatile("bar.sync 0;" ::: "mem
 template <int LT, int NR, int R>
 __device__ __forceinline__ void hmc_kick(const float (&q)[R * LT], float (&p)[R * LT],
                                          const float* hn, const float* hs, float h, float beta,
-                                         float m0sq, float lam4) {
+                                         float m0sq, float lam4, float kap) {
 #pragma unroll
   for (int jr = 0; jr < NR; ++jr)
 #pragma unroll
@@ -60,7 +60,7 @@ __device__ __forceinline__ void hmc_kick(const float (&q)[R * LT], float (&p)[R 
       const float n = jr == 0 ? hn[c * hm::P] : q[jr == 0 ? j : j - LT];
       const float s = jr == NR - 1 ? hs[c * hm::P] : q[jr == NR - 1 ? j : j + LT];
       // grad S_E = (4 a - neighbours) + m0^2 a + 4 lambda a^3;  grad U = a + beta grad S_E
-      const float gs = fmaf(4.0f, a, -((e + w) + (n + s))) + a * fmaf(lam4, a * a, m0sq);
+      const float gs = fmaf(kap, fmaf(4.0f, a, -((e + w) + (n + s))), a * fmaf(lam4, a * a, m0sq));
       p[j] = fmaf(-h, fmaf(beta, gs, a), p[j]);
     }
 }
@@ -77,7 +77,8 @@ __device__ __forceinline__ void hmc_band(const HmcArgs& A, float* cur, float* ha
   const bool live = i < A.N;
   const int r0 = w * R, x0 = r0 * LT;
   const int rn = (r0 + LT - 1) % LT, rs = (r0 + NR) % LT;       // halo rows
-  const float beta = (float)A.ctrl->beta, m0sq = A.md.m0sq, lam = A.md.lam, lam4 = 4.0f * A.md.lam;
+  const float beta = (float)A.ctrl->beta, m0sq = A.md.m0sq, lam = A.md.lam, lam4 = 4.0f * A.md.lam,
+              kap = A.md.kappa, hk = 0.5f * A.md.kappa;
   const float eps = A.eps;
   float q[R * LT], p[R * LT], ev[R * LT];
 #pragma unroll
@@ -116,7 +117,7 @@ __device__ __forceinline__ void hmc_band(const HmcArgs& A, float* cur, float* ha
       K0 = fmaf(0.5f * z, z, K0);
     }
     hmc_kick<LT, NR, R>(q, p, hal0 + rn * LT * P + lane, hal0 + rs * LT * P + lane, 0.5f * eps, beta,
-                     m0sq, lam4);
+                     m0sq, lam4, kap);
     cta_sync();                       // hal1 (the staged normals) is free from here on
     for (int s = 0; s < A.nfrog; ++s) {
       float* const own = (s & 1) ? own0 : own1;
@@ -128,7 +129,7 @@ __device__ __forceinline__ void hmc_band(const HmcArgs& A, float* cur, float* ha
       }
       cta_sync();
       hmc_kick<LT, NR, R>(q, p, hb + rn * LT * P + lane, hb + rs * LT * P + lane,
-                       (s + 1 == A.nfrog) ? 0.5f * eps : eps, beta, m0sq, lam4);
+                       (s + 1 == A.nfrog) ? 0.5f * eps : eps, beta, m0sq, lam4, kap);
     }
     // H_new: kinetic, S_E (Eq. 1, forward neighbours), U0 over this band
     const float* const hs = (((A.nfrog - 1) & 1) ? hal0 : hal1) + rs * LT * P + lane;
@@ -142,7 +143,7 @@ __device__ __forceinline__ void hmc_band(const HmcArgs& A, float* cur, float* ha
         const float a = q[j], b = q[jr * LT + (c + 1) % LT];
         const float d = jr == NR - 1 ? hs[c * P] : q[jr == NR - 1 ? j : j + LT];
         const float e1 = b - a, e2 = d - a, a2 = a * a;
-        rowS += 0.5f * (e1 * e1 + e2 * e2) + a2 * (0.5f * m0sq + lam * a2);
+        rowS += hk * (e1 * e1 + e2 * e2) + a2 * (0.5f * m0sq + lam * a2);
         Up = fmaf(0.5f, a2, Up);
         K1 = fmaf(0.5f * ev[j] * p[j], p[j], K1);
       }
@@ -314,7 +315,7 @@ hmc_g_kick_kernel(const float* __restrict__ q, float* __restrict__ p, int N, int
   const float e = q[(size_t)(r * L + ce) * ld + i], w = q[(size_t)(r * L + cw) * ld + i];
   const float n = q[(size_t)(rn * L + c) * ld + i], s = q[(size_t)(rs * L + c) * ld + i];
   const float beta = (float)ctrl->beta;
-  const float gs = fmaf(4.0f, a, -((e + w) + (n + s))) + a * fmaf(4.0f * md.lam, a * a, md.m0sq);
+  const float gs = fmaf(md.kappa, fmaf(4.0f, a, -((e + w) + (n + s))), a * fmaf(4.0f * md.lam, a * a, md.m0sq));
   const size_t o = (size_t)x * ld + i;
   p[o] = fmaf(-h, fmaf(beta, gs, a), p[o]);
 }
@@ -346,7 +347,7 @@ hmc_g_accept_kernel(float* __restrict__ phi, const float* __restrict__ q,
   const int lane = threadIdx.x & 31, g = threadIdx.x >> 5;
   const int i = blockIdx.x * 32 + lane;
   const int L = md.L, V = md.V;
-  const float hm = 0.5f * md.m0sq, lam = md.lam;
+  const float hm = 0.5f * md.m0sq, lam = md.lam, hk = 0.5f * md.kappa;
   const int band = (L + 7) >> 3, r_lo = min(L, g * band), r_hi = min(L, r_lo + band);
   float Sp = 0.f, Up = 0.f, K1 = 0.f;
   if (i < N) {
@@ -359,7 +360,7 @@ hmc_g_accept_kernel(float* __restrict__ phi, const float* __restrict__ q,
         const float b = q[(size_t)(r * L + ce) * ld + i], d = q[(size_t)(rs * L + c) * ld + i];
         const float pp = p[(size_t)x * ld + i];
         const float e1 = b - a, e2 = d - a, a2 = a * a;
-        rowS += 0.5f * (e1 * e1 + e2 * e2) + a2 * (hm + lam * a2);
+        rowS += hk * (e1 * e1 + e2 * e2) + a2 * (hm + lam * a2);
         rowU = fmaf(0.5f, a2, rowU);
         rowK = fmaf(0.5f * Sigma[(size_t)x * V + x] * pp, pp, rowK);
         a = b;

@@ -105,13 +105,13 @@ propose_kernel(const float* __restrict__ Lc, const float* __restrict__ Z,
 
 // Per-site differences of Eq. 1 and U0 between phi' and phi, written so that nothing cancels
 // (SURVEY H3): with a = phi_x, b / c its forward neighbours and primes for the proposal,
-//   d kin  = 1/2 [(e'-e)(e'+e) + (f'-f)(f'+f)],  e = b-a, f = c-a
+//   d kin  = kappa/2 [(e'-e)(e'+e) + (f'-f)(f'+f)],  e = b-a, f = c-a   (hk = kappa/2; 1/2 for Eq. 1)
 //   d mass + d quartic = (a'^2-a^2) (1/2 m0^2 + lambda (a'^2+a^2)),   dU0 = 1/2 (a'^2-a^2)
 __device__ __forceinline__ void site_diff(float a, float b, float c, float a2, float b2, float c2,
-                                          float hm, float lam, float& dS, float& dU) {
+                                          float hk, float hm, float lam, float& dS, float& dU) {
   float q = (a2 - a) * (a2 + a);
   float e = b - a, e2 = b2 - a2, f = c - a, f2 = c2 - a2;
-  dS += 0.5f * ((e2 - e) * (e2 + e) + (f2 - f) * (f2 + f)) + q * (hm + lam * (a2 * a2 + a * a));
+  dS += hk * ((e2 - e) * (e2 + e) + (f2 - f) * (f2 + f)) + q * (hm + lam * (a2 * a2 + a * a));
   dU += 0.5f * q;
 }
 
@@ -134,7 +134,7 @@ accept_kernel(float* __restrict__ phi, const float* __restrict__ phip, float* __
   const int lane = threadIdx.x & 31, g = threadIdx.x >> 5;
   const int i = blockIdx.x * 32 + lane;
   const int L = md.L;
-  const float hm = 0.5f * md.m0sq, lam = md.lam;
+  const float hm = 0.5f * md.m0sq, lam = md.lam, hk = 0.5f * md.kappa;
   // each warp owns a contiguous band of lattice rows
   const int band = (L + G - 1) / G, r_lo = min(L, g * band), r_hi = min(L, r_lo + band);
   float dS = 0.f, dU = 0.f, z2 = 0.f;
@@ -174,7 +174,7 @@ accept_kernel(float* __restrict__ phi, const float* __restrict__ phip, float* __
             if (q < nr) {
               const float d = (q + 1 < nr) ? A[q + 1 < 8 ? q + 1 : 8] : A[8];
               const float d2 = (q + 1 < nr) ? A2[q + 1 < 8 ? q + 1 : 8] : A2[8];
-              site_diff(A[q], Bn[q], d, A2[q], B2[q], d2, hm, lam, rS[q], rU[q]);
+              site_diff(A[q], Bn[q], d, A2[q], B2[q], d2, hk, hm, lam, rS[q], rU[q]);
             }
 #pragma unroll
           for (int q = 0; q < 9; ++q) { A[q] = Bn[q]; A2[q] = B2[q]; }
@@ -193,7 +193,7 @@ accept_kernel(float* __restrict__ phi, const float* __restrict__ phip, float* __
           int cn = (c + 1 == L) ? 0 : c + 1;
           float b = phi[ro + (size_t)cn * ld], b2 = phip[ro + (size_t)cn * ld];
           float d = phi[rno + (size_t)c * ld], d2 = phip[rno + (size_t)c * ld];
-          site_diff(a, b, d, a2, b2, d2, hm, lam, rS, rU);
+          site_diff(a, b, d, a2, b2, d2, hk, hm, lam, rS, rU);
           a = b;
           a2 = b2;
         }
@@ -407,8 +407,8 @@ slice_kernel(float* __restrict__ phi, const float* __restrict__ dir, float* __re
         v[q] = a;
       }
       const float lam = md.lam, m0 = md.m0sq;
-      const float c1 = v[2] + m0 * v[0] + 4.f * lam * v[4];
-      const float c2 = 0.5f * v[3] + 0.5f * m0 * v[1] + 6.f * lam * v[5];
+      const float c1 = md.kappa * v[2] + m0 * v[0] + 4.f * lam * v[4];
+      const float c2 = 0.5f * md.kappa * v[3] + 0.5f * m0 * v[1] + 6.f * lam * v[5];
       const float c3 = 4.f * lam * v[6], c4 = lam * v[7];
       const float u1 = v[0], u2 = 0.5f * v[1];
       const float S0 = S[i], Ub = U0[i], S_star = (float)ctrl->S_star;

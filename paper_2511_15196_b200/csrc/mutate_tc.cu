@@ -77,7 +77,7 @@ struct TcParams {
   Ctrl* ctrl;
   uint8_t* acc_out; float* margin_out;
   int N, ld, L, V, Vn, Kp;
-  float m0sq, lam;
+  float m0sq, lam, kappa;
   int mode;
   uint64_t seed;
   uint32_t tag_prop, tag_acc, t0;
@@ -112,18 +112,20 @@ __global__ void lsplit_kernel(const float* __restrict__ Lc, int V, int Vn, int K
 
 // Per-site difference of Eq. 1 between phi' (a2; forward neighbours b2, c2) and phi (a; b, c) in
 // the lattice-Laplacian form: on the periodic lattice
-//   S_E = sum_x [ (2 + m0^2/2) phi_x^2 + lambda phi_x^4 - phi_x (phi_{x+1} + phi_{x+2}) ],
-// which is Eq. 1 with the squares expanded (each site appears in four bonds).  With
+//   S_E = sum_x [ (2 kappa + m0^2/2) phi_x^2 + lambda phi_x^4 - kappa phi_x (phi_{x+1} + phi_{x+2}) ],
+// which is Eq. 1 with the squares expanded (each site appears in four bonds; kappa = 1 for Eq. 1,
+// Eq. 5 of PAPER.md:313 is this form).  The bond sum dB is kept apart and scaled once at the end.  With
 // q = a2^2 - a^2 formed as (a2-a)(a2+a), the potential part does not cancel; the bond part
 // a2 (b2+c2) - a (b+c) carries an fp32 rounding of ~3e-7 per site, 3e-6 over the V <= 112 sites
 // of this kernel -- far inside the 1e-4 decision band.  (The generic path, used up to V = 4096,
 // keeps the fully difference-based form.)
 __device__ __forceinline__ void tc_site_diff(float a, float b, float c, float a2, float b2,
-                                             float c2, float c2m, float lam, float& dS, float& dU) {
+                                             float c2, float c2m, float lam, float& dS, float& dB,
+                                             float& dU) {
   const float q = (a2 - a) * (a2 + a);
   dS = fmaf(q, fmaf(lam, fmaf(a2, a2, a * a), c2m), dS);
-  dS = fmaf(a, b + c, dS);
-  dS = fmaf(-a2, b2 + c2, dS);
+  dB = fmaf(a, b + c, dB);
+  dB = fmaf(-a2, b2 + c2, dB);
   dU = fmaf(0.5f, q, dU);
 }
 
@@ -133,10 +135,10 @@ __device__ __forceinline__ void tc_site_diff(float a, float b, float c, float a2
 // flight before the arithmetic.  LT = 0: any L, one site at a time.
 template <int LT>
 __device__ __forceinline__ void tc_stencil(const float* cur, const float* oth, int g, int Lrt,
-                                           float c2m, float lam, float& dS, float& dU) {
+                                           float c2m, float lam, float kap, float& dS, float& dU) {
   using namespace tc;
   if constexpr (LT > 0) {
-    float s0 = 0.f, u0 = 0.f, s1 = 0.f, u1 = 0.f;
+    float s0 = 0.f, u0 = 0.f, s1 = 0.f, u1 = 0.f, b0 = 0.f, b1 = 0.f;
     for (int r = g; r < LT; r += EPI_PARTS) {
       const int rn = (r + 1 == LT) ? 0 : r + 1;
       const float* c0 = cur + r * LT * TILE; const float* c1 = cur + rn * LT * TILE;
@@ -151,14 +153,15 @@ __device__ __forceinline__ void tc_stencil(const float* cur, const float* oth, i
       for (int c = 0; c < LT; ++c) {
         constexpr int dummy = 0; (void)dummy;
         const int cn = (c + 1 == LT) ? 0 : c + 1;
-        if (c & 1) tc_site_diff(a[c], a[cn], d[c], a2[c], a2[cn], d2[c], c2m, lam, s1, u1);
-        else tc_site_diff(a[c], a[cn], d[c], a2[c], a2[cn], d2[c], c2m, lam, s0, u0);
+        if (c & 1) tc_site_diff(a[c], a[cn], d[c], a2[c], a2[cn], d2[c], c2m, lam, s1, b1, u1);
+        else tc_site_diff(a[c], a[cn], d[c], a2[c], a2[cn], d2[c], c2m, lam, s0, b0, u0);
       }
     }
-    dS = s0 + s1;
+    dS = fmaf(kap, b0 + b1, s0 + s1);
     dU = u0 + u1;
   } else {
     const int L = Lrt;
+    float dB = 0.f;
     for (int r = g; r < L; r += EPI_PARTS) {
       const int rn = (r + 1 == L) ? 0 : r + 1;
       const float* c0 = cur + r * L * TILE; const float* c1 = cur + rn * L * TILE;
@@ -168,11 +171,12 @@ __device__ __forceinline__ void tc_stencil(const float* cur, const float* oth, i
         const int cn = (c + 1 == L) ? 0 : c + 1;
         float b = c0[cn * TILE], b2 = o0[cn * TILE];
         float d = c1[c * TILE], d2 = o1[c * TILE];
-        tc_site_diff(a, b, d, a2, b2, d2, c2m, lam, dS, dU);
+        tc_site_diff(a, b, d, a2, b2, d2, c2m, lam, dS, dB, dU);
         a = b;
         a2 = b2;
       }
     }
+    dS = fmaf(kap, dB, dS);
   }
 }
 
@@ -374,7 +378,7 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
     const int i = i0 + pr;
     const bool live = i < p.N;
     const int L = LT > 0 ? LT : p.L;
-    const float hm = 2.0f + 0.5f * p.m0sq, lam = p.lam;   // coefficient of phi^2 in the Laplacian form
+    const float hm = 2.0f * p.kappa + 0.5f * p.m0sq, lam = p.lam, kap = p.kappa;   // coefficient of phi^2 in the Laplacian form
     float* cur = tile0 + pr;
     float* oth = tile1 + pr;
     for (int x = g; x < V; x += EPI_PARTS) cur[x * TILE] = live ? p.phi[(size_t)x * p.ld + i] : 0.f;
@@ -467,7 +471,7 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
       TC_TRACE(2, tr);
       // pass 2: per-site differences of Eq. 1 and U0 over this part's lattice rows
       float dS = 0.f, dU = 0.f;
-      tc_stencil<LT>(cur, oth, g, L, hm, lam, dS, dU);
+      tc_stencil<LT>(cur, oth, g, L, hm, lam, kap, dS, dU);
       part[g * TILE + pr] = make_float2(dS, dU);
       if (g == 0) lus[pr] = log_uniform(p.seed, p.tag_acc, p.t0 + (uint32_t)t, (uint32_t)i);
       TC_TRACE(2, tr);
@@ -547,7 +551,7 @@ void launch_mutate_tc(const MutateArgs& a, float* Lsplit, cudaStream_t st) {
   p.phi = a.phi; p.S = a.S; p.U0 = a.U0; p.Lsplit = Lsplit; p.ctrl = a.ctrl;
   p.acc_out = a.acc_out; p.margin_out = a.margin_out;
   p.N = a.N; p.ld = a.ld; p.L = a.md.L; p.V = V; p.Vn = Vn; p.Kp = Kp;
-  p.m0sq = a.md.m0sq; p.lam = a.md.lam; p.mode = a.mode; p.seed = a.seed;
+  p.m0sq = a.md.m0sq; p.lam = a.md.lam; p.kappa = a.md.kappa; p.mode = a.mode; p.seed = a.seed;
   p.tag_prop = a.tag_prop; p.tag_acc = a.tag_acc; p.t0 = a.t0; p.k = a.k;
   p.respect_done = a.respect_done;
   p.rk = philox_round_keys(a.seed);

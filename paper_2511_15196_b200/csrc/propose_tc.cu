@@ -43,24 +43,30 @@ constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 256;
 // z of step t for every particle, hi/lo split, tile-major interleave layout:
 // float4 index ((part * ntm + m) * nkc + q) * 128 + pr, part 0 = hi, 1 = lo.
 __global__ void __launch_bounds__(128)
-normals_split_kernel(float4* __restrict__ Zs, int N, int ntm, int V, int Kp, uint64_t seed,
+normals_split_kernel(float4* __restrict__ Zs, int N, int ntm, int V, int Kp, int qpb, uint64_t seed,
                      uint32_t tag, uint32_t t, const Ctrl* ctrl, int respect_done) {
   pdl_enter();
   if (respect_done && ctrl->done) return;
-  const int m = blockIdx.x, q = blockIdx.y, pr = threadIdx.x;
+  const int m = blockIdx.x, pr = threadIdx.x;
   const int i = m * lg::TILE + pr, nkc = Kp >> 2;
-  float z[4] = {0.f, 0.f, 0.f, 0.f};
-  // SFU Box-Muller (philox.cuh, R2): this kernel is instruction-issue bound.  Quads
-  // beyond the lattice (K padding) stay zero; sites >= V inside the last quad meet zero columns.
-  if (i < N && 4 * q < V) normals4_fast(seed, tag, t, (uint32_t)i, (uint32_t)q, z);
-  float4 hi, lo;
-  hi.x = tc::tf32_rna(z[0]); lo.x = z[0] - hi.x;
-  hi.y = tc::tf32_rna(z[1]); lo.y = z[1] - hi.y;
-  hi.z = tc::tf32_rna(z[2]); lo.z = z[2] - hi.z;
-  hi.w = tc::tf32_rna(z[3]); lo.w = z[3] - hi.w;
-  const size_t o = ((size_t)m * nkc + q) * lg::TILE + pr;
-  Zs[o] = hi;
-  Zs[(size_t)ntm * nkc * lg::TILE + o] = lo;
+  const size_t lo_off = (size_t)ntm * nkc * lg::TILE;
+  // SFU Box-Muller (philox.cuh, R2).  Quads beyond the lattice (K padding) stay zero;
+  // sites >= V inside the last quad meet zero columns.
+#pragma unroll 2
+  for (int qq = 0; qq < qpb; ++qq) {
+    const int q = blockIdx.y * qpb + qq;
+    if (q >= nkc) break;
+    float z[4] = {0.f, 0.f, 0.f, 0.f};
+    if (i < N && 4 * q < V) normals4_fast(seed, tag, t, (uint32_t)i, (uint32_t)q, z);
+    float4 hi, lo;
+    hi.x = tc::tf32_rna(z[0]); lo.x = z[0] - hi.x;
+    hi.y = tc::tf32_rna(z[1]); lo.y = z[1] - hi.y;
+    hi.z = tc::tf32_rna(z[2]); lo.z = z[2] - hi.z;
+    hi.w = tc::tf32_rna(z[3]); lo.w = z[3] - hi.w;
+    const size_t o = ((size_t)m * nkc + q) * lg::TILE + pr;
+    Zs[o] = hi;
+    Zs[lo_off + o] = lo;
+  }
 }
 
 struct ProposeTcParams {
@@ -319,10 +325,14 @@ size_t propose_tc_lsplit_floats(int V) {
 void launch_normals_split(float* Zs, int N, int ld, int V, uint64_t seed, uint32_t tag, uint32_t t,
                           const Ctrl* ctrl, int respect_done, cudaStream_t st) {
   const int Kp = round_up(V, 16);
-  dim3 grid(ld / lg::TILE, Kp / 4);
+  // quads per thread: one quad per block made 1 M blocks at C4 (block-launch-rate bound); a small
+  // population keeps one quad per thread so that the grid still fills the GPU
+  int qpb = (ld / lg::TILE) * (Kp / 4) / (148 * 16);
+  qpb = qpb < 1 ? 1 : qpb > 8 ? 8 : qpb;
+  dim3 grid(ld / lg::TILE, (Kp / 4 + qpb - 1) / qpb);
   ++g_launches;
   launch_pdl(normals_split_kernel, grid, 128, 0, st, reinterpret_cast<float4*>(Zs), N, ld / lg::TILE, V, Kp,
-             seed, tag, t, ctrl, respect_done);
+             qpb, seed, tag, t, ctrl, respect_done);
 }
 
 void launch_propose_tc(const float* phi, float* phip, const float* Zs, const float* Lsplit, int ld,

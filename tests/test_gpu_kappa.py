@@ -1,0 +1,173 @@
+"""GPU parity for the kappa-lambda parameterisation (Eqs. 2-5;
+reading A18): smc_init_kl / ns_init_kl through the C ABI against the FP64 oracle with the same
+kinetic coefficient, on the same seeded inputs.  Same tolerances as the Eq. 1 tests: decisions exact
+outside |g| < 1e-4 (HMC: 1e-3), S_E within 2e-5 * A (A12), statistics within 3 combined SE."""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+from paper_2511_15196_b200 import binding as B
+from paper_2511_15196_b200 import build, inputs
+
+pytestmark = pytest.mark.gpu
+
+BAND, BAND_HMC, BAND_SLICE = 1e-4, 1e-3, 2e-3
+KAPPA, LAM2 = 0.8, 1.5            # broken-phase point of Eq. 2: m0^2 = 2 (1 - 2 lambda) = -4
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    build.build()
+    B.load()
+
+
+@pytest.mark.parametrize("L,N", [(4, 1024), (10, 4096), (7, 257), (2, 33), (16, 512)])
+def test_action_with_kappa(L, N):
+    kin, m0sq, lam, _ = O.kl_to_eq1(KAPPA, LAM2)
+    h = B.smc_init_kl(L, KAPPA, LAM2, N, 11 + L)
+    st = B.smc_get_state(h)
+    with O.kinetic(kin):
+        S, U0, A = O.action_batch(st["phi"].astype(np.float64), L, m0sq, lam, with_abs=True)
+    S1 = O.action_batch(st["phi"].astype(np.float64), L, m0sq, lam)[0]
+    assert np.all(np.abs(st["S"] - S) <= 2e-5 * A + 1e-12)
+    if L > 1:
+        assert np.abs(S - S1).max() > 0.1                  # kappa = 1 would be caught
+    # Eq. 2 verbatim, constant V lambda included, for a few particles
+    for i in range(0, N, max(1, N // 7)):
+        s2 = O.action_eq2_field(st["phi"][:, i].astype(np.float64), L, KAPPA, LAM2)
+        assert abs(st["S"][i] - (s2 - L * L * LAM2)) <= 2e-5 * A[i] + 1e-9
+    h.close()
+
+
+def test_kl_argument_errors():
+    with pytest.raises(B.Phi4Error):
+        B.smc_init_kl(4, -0.1, 1.0, 64, 0)
+    with pytest.raises(B.Phi4Error):
+        B.smc_init_kl(4, 1.0, float("nan"), 64, 0)
+    with pytest.raises(B.Phi4Error):
+        B.ns_init_kl(4, 1.0, -2.0, 64, 8, 4, 0)
+
+
+@pytest.mark.parametrize("path", [1, 2], ids=["generic", "tcgen05"])
+@pytest.mark.parametrize("L,N,k,beta", [(4, 1024, 10, 0.4), (10, 4096, 12, 0.3), (9, 640, 7, 0.6),
+                                        (2, 129, 6, 0.5), (12, 700, 3, 0.5), (16, 1024, 3, 0.2)])
+def test_rw_mutation_lockstep_with_kappa(L, N, k, beta, path):
+    V, seed, t_start = L * L, 5 + L, 2 * k
+    kin, m0sq, lam, _ = O.kl_to_eq1(KAPPA, LAM2)
+    h = B.smc_init_kl(L, KAPPA, LAM2, N, seed)
+    B.smc_set_params(h, k_steps=k, mutation_path=path)
+    B.smc_set_state(h, inputs.smooth_fields(L, N, seed=seed + 1), beta, t_start)
+    B.estimate_cov_chol(h)
+    Lc, st0 = B.smc_get_chol(h), B.smc_get_state(h)
+    acc, mar = B.smc_mutate(h, k)
+    st1 = B.smc_get_state(h)
+    with O.kinetic(kin):
+        S0, U00 = O.action_batch(st0["phi"].astype(np.float64), L, m0sq, lam)
+        p, S, U0, oacc, omar, _ = O.mutate(st0["phi"], S0, U00, L, m0sq, lam, Lc,
+                                           np.float32(2.38 / math.sqrt(V)), beta, seed, t_start + 1, k)
+        Sx, Ux, A = O.action_batch(st1["phi"].astype(np.float64), L, m0sq, lam, with_abs=True)
+    amb = np.abs(omar) < BAND
+    first = np.where(amb.any(axis=0), amb.argmax(axis=0), k)
+    valid = np.arange(k)[:, None] < first[None, :]
+    assert valid.mean() > 0.98
+    assert np.array_equal(acc[valid], oacc[valid]), "accept decisions differ outside the band"
+    assert np.all(np.abs(mar[valid] - omar[valid]) < BAND + 1e-5 * np.abs(omar[valid]))
+    clean = first == k
+    assert np.abs(st1["phi"][:, clean] - p[:, clean]).max() < 2e-5
+    assert np.all(np.abs(st1["S"] - Sx) <= 2e-5 * A + 2e-5)
+    assert 0.0 < acc.mean() < 1.0
+    h.close()
+
+
+@pytest.mark.parametrize("L,N,k,nfrog", [(10, 2048, 2, 10), (4, 512, 3, 8), (23, 96, 1, 4)])
+def test_hmc_lockstep_with_kappa(L, N, k, nfrog):
+    """On-chip kernel (L <= 22) and the HBM-resident per-half-step kernels (L = 23)."""
+    seed, beta, eps = 3 + L, 0.5, 0.08
+    kin, m0sq, lam, _ = O.kl_to_eq1(KAPPA, LAM2)
+    h = B.smc_init_kl(L, KAPPA, LAM2, N, seed)
+    B.smc_set_params(h, k_steps=k, kernel=1, hmc_eps=eps, hmc_leapfrog=nfrog)
+    B.smc_set_state(h, inputs.smooth_fields(L, N, seed=seed + 1), beta, 0)
+    B.estimate_cov_chol(h)
+    st0 = B.smc_get_state(h)
+    acc, mar = B.smc_mutate(h, k)
+    st1 = B.smc_get_state(h)
+    f0 = st0["phi"].astype(np.float64)
+    with O.kinetic(kin):
+        S0, U00 = O.action_batch(f0, L, m0sq, lam)
+        _, Sig = O.covariance(f0)
+        p, S, U0, oacc, omar = O.hmc_mutate(f0, S0, U00, L, m0sq, lam, np.diag(Sig).copy(),
+                                            float(np.float32(eps)), nfrog, beta, seed, 1, k)
+    amb = np.abs(omar) < BAND_HMC
+    first = np.where(amb.any(axis=0), amb.argmax(axis=0), k)
+    valid = np.arange(k)[:, None] < first[None, :]
+    assert valid.mean() > 0.9
+    assert np.array_equal(acc[valid], oacc[valid])
+    d, go = np.abs(mar[valid] - omar[valid]), np.abs(omar[valid])
+    assert np.all(d < np.where(go < 20.0, 0.5 * BAND_HMC + 1e-5 * go, 1e-3 * go))
+    clean = first == k
+    assert np.abs(st1["phi"][:, clean] - p[:, clean]).max() < 1e-4
+    assert 0.05 < acc.mean() <= 1.0
+    h.close()
+
+
+@pytest.mark.parametrize("inner", [0, 1], ids=["walk", "slice"])
+def test_ns_first_iteration_lockstep_with_kappa(inner):
+    L, n, kd, nw, seed = 6, 1024, 256, 6, 41
+    kin, m0sq, lam, _ = O.kl_to_eq1(KAPPA, LAM2)
+    h = B.ns_init_kl(L, KAPPA, LAM2, n, kd, nw, seed, max_iters=16)
+    B.ns_set_params(h, inner=inner)
+    st0 = B.smc_get_state(h)
+    info = B.ns_step(h)
+    st1 = B.smc_get_state(h)
+    S0 = st0["S"].astype(np.float64)
+    dead = O.ns_select(S0, kd)
+    assert np.array_equal(B.ns_get_dead(h)["last_dead"], dead)
+    Lc = B.smc_get_chol(h)
+    surv = np.setdiff1d(np.arange(n), dead)
+    start = np.array([surv[O.word0(seed, O.TAG_NS_START, 0, j) % (n - kd)] for j in range(kd)])
+    f0 = st0["phi"][:, start].astype(np.float64)
+    with O.kinetic(kin):
+        Ss, Us = O.action_batch(f0, L, m0sq, lam)
+        if inner == 1:
+            p, S, U0, t, nexp, nshr, amb = O.slice_walk(f0, Ss, Us, L, m0sq, lam, Lc, info["S_star"],
+                                                        seed, 1, nw, width=np.float32(1.0), m_expand=8)
+            clean = amb.min(axis=0) > BAND_SLICE
+        else:
+            p, S, U0, oacc, omar, ocon = O.mutate(f0, Ss, Us, L, m0sq, lam, Lc,
+                                                  np.float32(2.38 / L), 0.0, seed, 1, nw,
+                                                  mode=O.MODE_NS, S_star=info["S_star"])
+            amb = (np.abs(omar) < BAND) | (np.abs(ocon) < 1e-4 * max(1.0, abs(info["S_star"])))
+            clean = ~amb.any(axis=0)
+    assert clean.mean() > 0.6
+    got = st1["phi"][:, dead]
+    assert np.abs(got[:, clean] - p[:, clean]).max() < 1e-4
+    assert np.all(st1["S"] < info["S_star"] + 1e-3)
+    h.close()
+
+
+def logZ_gauss_kappa(L, kappa, m0sq):
+    k = np.arange(L)
+    kh = 4 * np.sin(np.pi * k / L) ** 2
+    return -0.5 * np.sum(np.log1p(m0sq + kappa * (kh[:, None] + kh[None, :])))
+
+
+def _mean_se(v):
+    v = np.asarray(v, float)
+    return v.mean(), v.std(ddof=1) / math.sqrt(v.size)
+
+
+def test_smc_eq2_gaussian_closed_form():
+    """Eq. 2 at lambda = 0 (m0^2 = 2) is Gaussian: log Z = -1/2 sum_k ln(3 + kappa khat_k^2)."""
+    kappa, want = 0.5, logZ_gauss_kappa(4, 0.5, 2.0)
+    out = []
+    for s in range(8):
+        h = B.smc_init_kl(4, kappa, 0.0, 2048, s)
+        B.smc_set_params(h, k_steps=48, ess_target=0.9)
+        B.smc_run(h)
+        out.append(B.log_Z(h))
+        h.close()
+    m, se = _mean_se(out)
+    assert abs(m - want) < 3 * se + 0.01, (m, se, want)
+    assert abs(m - logZ_gauss_kappa(4, 1.0, 2.0)) > 10 * se
