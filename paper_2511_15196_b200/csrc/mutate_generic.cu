@@ -258,9 +258,7 @@ void launch_mutate_generic(const MutateArgs& a, float* Lsplit, cudaStream_t st) 
   dim3 gz((a.ld + 127) / 128, (V + 3) / 4);
   dim3 gp(a.ld / 64, (V + 63) / 64);
   if (Lsplit) {
-    int Vn, Kp;
-    propose_tc_dims(V, &Vn, &Kp);
-    launch_lsplit(a.Lc, V, Vn, Kp, a.s, Lsplit, a.ctrl, a.respect_done, st);
+    launch_propose_lsplit(a.Lc, V, a.ld, a.s, Lsplit, a.ctrl, a.respect_done, st);
   }
   for (int j = 0; j < a.k; ++j) {
     uint32_t t = a.t0 + (uint32_t)j;

@@ -43,8 +43,8 @@ constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 256;
 // z of step t for every particle, hi/lo split, tile-major interleave layout:
 // float4 index ((part * ntm + m) * nkc + q) * 128 + pr, part 0 = hi, 1 = lo.
 __global__ void __launch_bounds__(128)
-normals_split_kernel(float4* __restrict__ Zs, int N, int ntm, int V, int Kp, int qpb, uint64_t seed,
-                     uint32_t tag, uint32_t t, const Ctrl* ctrl, int respect_done) {
+normals_split_kernel(float4* __restrict__ Zs, int N, int ntm, int V, int Kp, int qpb, int stage_major,
+                     uint64_t seed, uint32_t tag, uint32_t t, const Ctrl* ctrl, int respect_done) {
   pdl_enter();
   if (respect_done && ctrl->done) return;
   const int m = blockIdx.x, pr = threadIdx.x;
@@ -63,9 +63,16 @@ normals_split_kernel(float4* __restrict__ Zs, int N, int ntm, int V, int Kp, int
     hi.y = tc::tf32_rna(z[1]); lo.y = z[1] - hi.y;
     hi.z = tc::tf32_rna(z[2]); lo.z = z[2] - hi.z;
     hi.w = tc::tf32_rna(z[3]); lo.w = z[3] - hi.w;
-    const size_t o = ((size_t)m * nkc + q) * lg::TILE + pr;
-    Zs[o] = hi;
-    Zs[lo_off + o] = lo;
+    if (stage_major) {
+      // pair kernel (propose_tc2.cu): [m][stage][part][4 chunks][128][4], one copy per stage
+      const size_t o = ((((size_t)m * (nkc >> 2) + (q >> 2)) * 2) * 4 + (q & 3)) * lg::TILE + pr;
+      Zs[o] = hi;
+      Zs[o + 4 * lg::TILE] = lo;
+    } else {
+      const size_t o = ((size_t)m * nkc + q) * lg::TILE + pr;
+      Zs[o] = hi;
+      Zs[lo_off + o] = lo;
+    }
   }
 }
 
@@ -139,8 +146,12 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
 
   if (warp == 8) {
     // ================================ producer: bulk copies into the ring =====================
-    if (lane == 0) {
+    // One lane per copy of a stage (a single thread issuing all ten, with their 64-bit address
+    // arithmetic, took longer than the 768 tensor cycles of a stage): lanes 0-1 the hi / lo
+    // normals, lanes 2-9 the (K-step kk, chunk c, part h) runs of s*Lc.
+    {
       const size_t lpart = l_floats_vk(Vn, Kp);
+      const int kk = (lane - 2) >> 2 & 1, c = (lane - 2) >> 1 & 1, h = lane & 1;
       int s = 0;
       uint32_t ph = 0;
       for (TileIter ti(p.ntm, p.ntn, p.pair); ti.valid(); ti.next()) {
@@ -148,40 +159,27 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
         ti.tile(m, tn);
         const int n0 = tn * TN;
         const int nst = min(n0 + TN, Kp) >> 4;               // K-stages up to the tile's last row
+        const float* za = p.Zs + ((size_t)h * p.ntm + m) * nkc * (TILE * 4);
         for (int it = 0; it < nst; ++it) {
-          mbar_wait(empty(s), ph ^ 1);
           const uint32_t st = ring + (uint32_t)s * STAGE_BYTES;
-          // bytes of this stage: A is always whole, B shrinks inside the diagonal block
-          uint32_t bytes = 2 * A_PART;
-          int rowstart[2], nrows[2];
-#pragma unroll
-          for (int kk = 0; kk < 2; ++kk) {
-            const int xs = xs_of(2 * it + kk);
-            rowstart[kk] = max(n0, xs);
-            nrows[kk] = n0 + TN - rowstart[kk];
-            bytes += 4u * (uint32_t)nrows[kk] * 16u;            // 2 chunks x hi, lo
+          // A is always whole, B shrinks inside the diagonal block
+          const int xs0 = xs_of(2 * it), xs1 = xs_of(2 * it + 1);
+          const int nr0 = n0 + TN - max(n0, xs0), nr1 = n0 + TN - max(n0, xs1);
+          if (lane == 0) {
+            mbar_wait(empty(s), ph ^ 1);
+            mbar_expect_tx(full(s), 2 * A_PART + 64u * (uint32_t)(nr0 + nr1));   // 2 chunks x hi, lo x 16 B
           }
-          mbar_expect_tx(full(s), bytes);
-#pragma unroll
-          for (int h = 0; h < 2; ++h) {
-            const float* za = p.Zs + (((size_t)h * p.ntm + m) * nkc + 4 * it) * (TILE * 4);
-            bulk_g2s(st + (uint32_t)h * A_PART, za, A_PART, full(s));
-          }
-#pragma unroll
-          for (int kk = 0; kk < 2; ++kk) {
-            const int ks = 2 * it + kk, xs = xs_of(ks);
-            const size_t blk = (size_t)rows_before(ks, Vn) * 8;
-#pragma unroll
-            for (int c = 0; c < 2; ++c)
-#pragma unroll
-              for (int h = 0; h < 2; ++h) {
-                const float* src = p.Lsplit + (size_t)h * lpart + blk + (size_t)c * (Vn - xs) * 4 +
-                                   (size_t)(rowstart[kk] - xs) * 4;
-                const uint32_t dst = st + 2 * A_PART + (uint32_t)h * B_PART +
-                                     (uint32_t)(kk * 2 + c) * CHUNK_B +
-                                     (uint32_t)(rowstart[kk] - n0) * 16u;
-                bulk_g2s(dst, src, (uint32_t)nrows[kk] * 16u, full(s));
-              }
+          __syncwarp();
+          if (lane < 2) {
+            bulk_g2s(st + (uint32_t)h * A_PART, za + (size_t)(4 * it) * (TILE * 4), A_PART, full(s));
+          } else if (lane < 10) {
+            const int ks = 2 * it + kk, xs = kk ? xs1 : xs0, nr = kk ? nr1 : nr0;
+            const int rowstart = max(n0, xs);
+            const float* src = p.Lsplit + (size_t)h * lpart + (size_t)rows_before(ks, Vn) * 8 +
+                               (size_t)c * (Vn - xs) * 4 + (size_t)(rowstart - xs) * 4;
+            const uint32_t dst = st + 2 * A_PART + (uint32_t)h * B_PART +
+                                 (uint32_t)(kk * 2 + c) * CHUNK_B + (uint32_t)(rowstart - n0) * 16u;
+            bulk_g2s(dst, src, (uint32_t)nr * 16u, full(s));
           }
           if (++s == STAGES) { s = 0; ph ^= 1; }
         }
@@ -311,6 +309,28 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
 
 bool propose_tc_supported(int V) { return V > 112; }
 
+static int num_sms_cached() {
+  static int n = 0;
+  if (!n) {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev);
+  }
+  return n;
+}
+
+// s*Lc split hi / lo in the layout of the kernel that launch_propose_tc will pick
+void launch_propose_lsplit(const float* Lc, int V, int ld, float s, float* Lsplit, const Ctrl* ctrl,
+                           int respect_done, cudaStream_t st) {
+  if (propose_tc2_usable(V, ld, num_sms_cached())) {
+    launch_lsplit_tiled(Lc, V, s, Lsplit, ctrl, respect_done, st);
+    return;
+  }
+  int Vn, Kp;
+  propose_tc_dims(V, &Vn, &Kp);
+  launch_lsplit(Lc, V, Vn, Kp, s, Lsplit, ctrl, respect_done, st);
+}
+
 void propose_tc_dims(int V, int* Vn, int* Kp) {
   *Vn = round_up(V, lg::TN);
   *Kp = round_up(V, 16);
@@ -319,7 +339,9 @@ void propose_tc_dims(int V, int* Vn, int* Kp) {
 size_t propose_tc_zsplit_floats(int V, int ld) { return (size_t)2 * round_up(V, 16) * ld; }
 
 size_t propose_tc_lsplit_floats(int V) {
-  return 2 * tc::l_floats_vk(round_up(V, lg::TN), round_up(V, 16));
+  const size_t a = 2 * tc::l_floats_vk(round_up(V, lg::TN), round_up(V, 16));
+  const size_t b = propose_tc2_lsplit_floats(V);
+  return a > b ? a : b;
 }
 
 void launch_normals_split(float* Zs, int N, int ld, int V, uint64_t seed, uint32_t tag, uint32_t t,
@@ -332,18 +354,21 @@ void launch_normals_split(float* Zs, int N, int ld, int V, uint64_t seed, uint32
   dim3 grid(ld / lg::TILE, (Kp / 4 + qpb - 1) / qpb);
   ++g_launches;
   launch_pdl(normals_split_kernel, grid, 128, 0, st, reinterpret_cast<float4*>(Zs), N, ld / lg::TILE, V, Kp,
-             qpb, seed, tag, t, ctrl, respect_done);
+             qpb, (int)propose_tc2_usable(V, ld, num_sms_cached()), seed, tag, t, ctrl, respect_done);
 }
 
 void launch_propose_tc(const float* phi, float* phip, const float* Zs, const float* Lsplit, int ld,
                        int V, const Ctrl* ctrl, int respect_done, cudaStream_t st) {
-  static int num_sms = 0;
-  if (!num_sms) {
+  static bool attr_done = false;
+  if (!attr_done) {
     cudaFuncSetAttribute(propose_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                          lg::SMEM_BYTES);
-    int dev = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev);
+    attr_done = true;
+  }
+  const int num_sms = num_sms_cached();
+  if (propose_tc2_usable(V, ld, num_sms)) {
+    launch_propose_tc2(phi, phip, Zs, Lsplit, ld, V, ctrl, respect_done, num_sms, st);
+    return;
   }
   ProposeTcParams p;
   p.phi = phi; p.phip = phip; p.Zs = Zs; p.Lsplit = Lsplit; p.ctrl = ctrl;
