@@ -57,16 +57,8 @@ size_t propose_tc_lsplit_floats(int V);
 void propose_tc_dims(int V, int* Vn, int* Kp);
 void launch_normals_split(float* Zs, int N, int ld, int V, uint64_t seed, uint32_t tag, uint32_t t,
                           const Ctrl* ctrl, int respect_done, cudaStream_t st);
-// propose_tc2.cu -- the same GEMM on CTA pairs (cta_group::2): a third less L2 -> SM traffic
-bool propose_tc2_usable(int V, int ld, int num_sms);
-size_t propose_tc2_lsplit_floats(int V);
-void launch_lsplit_tiled(const float* Lc, int V, float s, float* Lsplit, const Ctrl* ctrl,
-                         int respect_done, cudaStream_t st);
 void launch_propose_lsplit(const float* Lc, int V, int ld, float s, float* Lsplit, const Ctrl* ctrl,
                            int respect_done, cudaStream_t st);
-void launch_propose_tc2(const float* phi, float* phip, const float* Zs, const float* Lsplit,
-                        int ld, int V, const Ctrl* ctrl, int respect_done, int num_sms,
-                        cudaStream_t st);
 void launch_propose_tc(const float* phi, float* phip, const float* Zs, const float* Lsplit, int ld,
                        int V, const Ctrl* ctrl, int respect_done, cudaStream_t st);
 

@@ -40,16 +40,15 @@ constexpr int SUB_STAGES = 64;               // one TMEM accumulation chain cove
 constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 256;
 }  // namespace lg
 
-// z of step t for every particle, hi/lo split, tile-major interleave layout:
-// float4 index ((part * ntm + m) * nkc + q) * 128 + pr, part 0 = hi, 1 = lo.
+// z of step t for every particle, hi/lo split, stage-major interleave layout:
+// float4 index (((m * nst + q / 4) * 2 + part) * 4 + q % 4) * 128 + pr, part 0 = hi, 1 = lo.
 __global__ void __launch_bounds__(128)
-normals_split_kernel(float4* __restrict__ Zs, int N, int ntm, int V, int Kp, int qpb, int stage_major,
+normals_split_kernel(float4* __restrict__ Zs, int N, int ntm, int V, int Kp, int qpb,
                      uint64_t seed, uint32_t tag, uint32_t t, const Ctrl* ctrl, int respect_done) {
   pdl_enter();
   if (respect_done && ctrl->done) return;
   const int m = blockIdx.x, pr = threadIdx.x;
   const int i = m * lg::TILE + pr, nkc = Kp >> 2;
-  const size_t lo_off = (size_t)ntm * nkc * lg::TILE;
   // SFU Box-Muller (philox.cuh, R2).  Quads beyond the lattice (K padding) stay zero;
   // sites >= V inside the last quad meet zero columns.
 #pragma unroll 2
@@ -63,17 +62,48 @@ normals_split_kernel(float4* __restrict__ Zs, int N, int ntm, int V, int Kp, int
     hi.y = tc::tf32_rna(z[1]); lo.y = z[1] - hi.y;
     hi.z = tc::tf32_rna(z[2]); lo.z = z[2] - hi.z;
     hi.w = tc::tf32_rna(z[3]); lo.w = z[3] - hi.w;
-    if (stage_major) {
-      // pair kernel (propose_tc2.cu): [m][stage][part][4 chunks][128][4], one copy per stage
-      const size_t o = ((((size_t)m * (nkc >> 2) + (q >> 2)) * 2) * 4 + (q & 3)) * lg::TILE + pr;
-      Zs[o] = hi;
-      Zs[o + 4 * lg::TILE] = lo;
-    } else {
-      const size_t o = ((size_t)m * nkc + q) * lg::TILE + pr;
-      Zs[o] = hi;
-      Zs[lo_off + o] = lo;
-    }
+    const size_t o = ((((size_t)m * (nkc >> 2) + (q >> 2)) * 2) * 4 + (q & 3)) * lg::TILE + pr;
+    Zs[o] = hi;
+    Zs[o + 4 * lg::TILE] = lo;
   }
+}
+
+// ---- operand layouts: one bulk copy per operand per stage ------------------------------------
+// (Round 1 issued ten copies per stage -- 2 parts of normals, 2 K-steps x 2 chunks x 2 parts of
+// s*Lc; the ncu source view showed the producer warp never waiting for a free stage while the
+// MMA thread polled "stage full" ~30 times per stage: the copy issue was the bottleneck.)
+// Normals: Zs[m][it][part][4 chunks][128 rows][4] -- 16 KB per (particle tile, stage).
+// s*Lc:    Lt[tn][it][part][kk][c][nrows][4], nrows = the rows of site tile tn that K-stage it
+//          can reach: 256 below the diagonal block, 256 - 16 j in its j-th stage (both K-steps of
+//          a stage start at row xs = 16 it).  32 nrows floats per stage; rows above the diagonal
+//          are never stored or multiplied.
+__host__ __device__ inline size_t lt_tile_base(int tn) {          // floats before site tile tn
+  return (size_t)8192 * 16 * ((size_t)tn * (tn - 1) / 2) + (size_t)69632 * tn;
+}
+__host__ __device__ inline size_t lt_stage_off(int tn, int it) {  // floats before stage it of tile tn
+  const int d0 = 16 * tn;
+  if (it < d0) return lt_tile_base(tn) + (size_t)it * 8192;
+  const int j = it - d0;
+  return lt_tile_base(tn) + (size_t)d0 * 8192 + (size_t)32 * (256 * j - 8 * j * (j - 1));
+}
+
+__global__ void lsplit_tiled_kernel(const float* __restrict__ Lc, int V, int Vn, int Kp, float s,
+                                    float* __restrict__ out, const Ctrl* ctrl, int respect_done) {
+  pdl_enter();
+  if (respect_done && ctrl->done) return;
+  const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= (size_t)Kp * Vn) return;
+  const int y = (int)(idx / Vn), x = (int)(idx - (size_t)y * Vn);
+  const int tn = x >> 8, n0 = tn << 8, it = y >> 4;
+  const int rs = max(n0, 16 * it);
+  if (x < rs) return;                                // above the diagonal: never multiplied
+  const int nrows = n0 + 256 - rs;
+  const int kk = (y >> 3) & 1, c = (y >> 2) & 1, e = y & 3;
+  const float v = (x < V && y < V && y <= x) ? s * Lc[(size_t)x * V + y] : 0.f;
+  const float hi = tc::tf32_rna(v), lo = tc::tf32_rna(v - hi);
+  const size_t o = lt_stage_off(tn, it) + ((size_t)((kk * 2 + c) * nrows + (x - rs))) * 4 + e;
+  out[o] = hi;
+  out[o + (size_t)16 * nrows] = lo;                  // part stride: 2 kk x 2 c x nrows rows x 4
 }
 
 struct ProposeTcParams {
@@ -125,7 +155,7 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
   auto dempty = [&](int b) { return bar0 + 8u * (2 * STAGES + 2 + b); };
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * STAGES + 4);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int V = p.V, Vn = p.Vn, Kp = p.Kp, nkc = Kp >> 2;
+  const int V = p.V, Kp = p.Kp;
 
   if (warp == 8 && lane == 0) {
     for (int s = 0; s < STAGES; ++s) { mbar_init(full(s), 1); mbar_init(empty(s), 1); }
@@ -145,42 +175,25 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
   }
 
   if (warp == 8) {
-    // ================================ producer: bulk copies into the ring =====================
-    // One lane per copy of a stage (a single thread issuing all ten, with their 64-bit address
-    // arithmetic, took longer than the 768 tensor cycles of a stage): lanes 0-1 the hi / lo
-    // normals, lanes 2-9 the (K-step kk, chunk c, part h) runs of s*Lc.
-    {
-      const size_t lpart = l_floats_vk(Vn, Kp);
-      const int kk = (lane - 2) >> 2 & 1, c = (lane - 2) >> 1 & 1, h = lane & 1;
+    // ================================ producer: two bulk copies per stage =====================
+    if (lane == 0) {
       int s = 0;
       uint32_t ph = 0;
+      const int nstz = Kp >> 4;
       for (TileIter ti(p.ntm, p.ntn, p.pair); ti.valid(); ti.next()) {
         int m, tn;
         ti.tile(m, tn);
         const int n0 = tn * TN;
         const int nst = min(n0 + TN, Kp) >> 4;               // K-stages up to the tile's last row
-        const float* za = p.Zs + ((size_t)h * p.ntm + m) * nkc * (TILE * 4);
+        const float* za = p.Zs + (size_t)m * nstz * (2 * A_PART / 4);
         for (int it = 0; it < nst; ++it) {
           const uint32_t st = ring + (uint32_t)s * STAGE_BYTES;
-          // A is always whole, B shrinks inside the diagonal block
-          const int xs0 = xs_of(2 * it), xs1 = xs_of(2 * it + 1);
-          const int nr0 = n0 + TN - max(n0, xs0), nr1 = n0 + TN - max(n0, xs1);
-          if (lane == 0) {
-            mbar_wait(empty(s), ph ^ 1);
-            mbar_expect_tx(full(s), 2 * A_PART + 64u * (uint32_t)(nr0 + nr1));   // 2 chunks x hi, lo x 16 B
-          }
-          __syncwarp();
-          if (lane < 2) {
-            bulk_g2s(st + (uint32_t)h * A_PART, za + (size_t)(4 * it) * (TILE * 4), A_PART, full(s));
-          } else if (lane < 10) {
-            const int ks = 2 * it + kk, xs = kk ? xs1 : xs0, nr = kk ? nr1 : nr0;
-            const int rowstart = max(n0, xs);
-            const float* src = p.Lsplit + (size_t)h * lpart + (size_t)rows_before(ks, Vn) * 8 +
-                               (size_t)c * (Vn - xs) * 4 + (size_t)(rowstart - xs) * 4;
-            const uint32_t dst = st + 2 * A_PART + (uint32_t)h * B_PART +
-                                 (uint32_t)(kk * 2 + c) * CHUNK_B + (uint32_t)(rowstart - n0) * 16u;
-            bulk_g2s(dst, src, (uint32_t)nr * 16u, full(s));
-          }
+          const int nrows = n0 + TN - max(n0, 16 * it);      // rows of the s*Lc block of this stage
+          const uint32_t bbytes = 128u * (uint32_t)nrows;    // 2 parts x 2 kk x 2 c x nrows x 16 B
+          mbar_wait(empty(s), ph ^ 1);
+          mbar_expect_tx(full(s), 2 * A_PART + bbytes);
+          bulk_g2s(st, za + (size_t)it * (2 * A_PART / 4), 2 * A_PART, full(s));
+          bulk_g2s(st + 2 * A_PART, p.Lsplit + lt_stage_off(tn, it), bbytes, full(s));
           if (++s == STAGES) { s = 0; ph ^= 1; }
         }
       }
@@ -192,7 +205,6 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
       int s = 0, cnt = 0;
       uint32_t ph = 0;
       const uint64_t a_base = smem_desc(ring, CHUNK_A, 128);
-      const uint64_t b_base = smem_desc(ring + 2 * A_PART, CHUNK_B, 128);
       for (TileIter ti(p.ntm, p.ntn, p.pair); ti.valid(); ti.next()) {
         int m, tn;
         ti.tile(m, tn);
@@ -208,17 +220,18 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
             mbar_wait(full(s), ph);
             tc_fence_after();
             const uint32_t so = (uint32_t)s * (STAGE_BYTES >> 4);
+            // both K-steps of a stage reach the same rows (xs = 16 it); the block sits packed in
+            // the stage as [part][kk][c][nrows][16 B], so LBO and the part stride follow nrows
+            const int rowstart = max(n0, 16 * it), nrows = n0 + TN - rowstart;
+            const uint32_t idesc = instr_desc(TILE, nrows);
+            const uint32_t d = dbase + (uint32_t)(rowstart - n0);
+            const uint64_t b_st = smem_desc(ring + 2 * A_PART, (uint32_t)nrows * 16u, 128) + so;
 #pragma unroll
             for (int kk = 0; kk < 2; ++kk) {
-              const int xs = xs_of(2 * it + kk);
-              const int rowstart = max(n0, xs), nrows = n0 + TN - rowstart;
-              const uint32_t idesc = instr_desc(TILE, nrows);
-              const uint32_t d = dbase + (uint32_t)(rowstart - n0);
               const uint64_t a_hi = a_base + so + (uint32_t)(2 * kk) * (CHUNK_A >> 4);
               const uint64_t a_lo = a_hi + (A_PART >> 4);
-              const uint64_t b_hi = b_base + so + (uint32_t)(2 * kk) * (CHUNK_B >> 4) +
-                                    (uint32_t)(rowstart - n0);
-              const uint64_t b_lo = b_hi + (B_PART >> 4);
+              const uint64_t b_hi = b_st + (uint32_t)(2 * kk * nrows);
+              const uint64_t b_lo = b_hi + (uint32_t)(4 * nrows);
               // The first K-step of a chain overwrites the accumulator.  Only the chain that ends
               // in the diagonal block has shrunk K-steps, and it starts with a full-width one
               // (n0 is a multiple of 256 <= 16 it0 whenever it0 > 0), so no column is left stale.
@@ -319,16 +332,15 @@ static int num_sms_cached() {
   return n;
 }
 
-// s*Lc split hi / lo in the layout of the kernel that launch_propose_tc will pick
+// s*Lc split hi / lo in the tiled layout propose_tc_kernel streams (lt_stage_off)
 void launch_propose_lsplit(const float* Lc, int V, int ld, float s, float* Lsplit, const Ctrl* ctrl,
                            int respect_done, cudaStream_t st) {
-  if (propose_tc2_usable(V, ld, num_sms_cached())) {
-    launch_lsplit_tiled(Lc, V, s, Lsplit, ctrl, respect_done, st);
-    return;
-  }
+  (void)ld;
   int Vn, Kp;
   propose_tc_dims(V, &Vn, &Kp);
-  launch_lsplit(Lc, V, Vn, Kp, s, Lsplit, ctrl, respect_done, st);
+  ++g_launches;
+  launch_pdl(lsplit_tiled_kernel, (unsigned)(((size_t)Kp * Vn + 255) / 256), 256, 0, st, Lc, V, Vn,
+             Kp, s, Lsplit, ctrl, respect_done);
 }
 
 void propose_tc_dims(int V, int* Vn, int* Kp) {
@@ -339,9 +351,7 @@ void propose_tc_dims(int V, int* Vn, int* Kp) {
 size_t propose_tc_zsplit_floats(int V, int ld) { return (size_t)2 * round_up(V, 16) * ld; }
 
 size_t propose_tc_lsplit_floats(int V) {
-  const size_t a = 2 * tc::l_floats_vk(round_up(V, lg::TN), round_up(V, 16));
-  const size_t b = propose_tc2_lsplit_floats(V);
-  return a > b ? a : b;
+  return lt_tile_base(round_up(V, lg::TN) / lg::TN);
 }
 
 void launch_normals_split(float* Zs, int N, int ld, int V, uint64_t seed, uint32_t tag, uint32_t t,
@@ -354,7 +364,7 @@ void launch_normals_split(float* Zs, int N, int ld, int V, uint64_t seed, uint32
   dim3 grid(ld / lg::TILE, (Kp / 4 + qpb - 1) / qpb);
   ++g_launches;
   launch_pdl(normals_split_kernel, grid, 128, 0, st, reinterpret_cast<float4*>(Zs), N, ld / lg::TILE, V, Kp,
-             qpb, (int)propose_tc2_usable(V, ld, num_sms_cached()), seed, tag, t, ctrl, respect_done);
+             qpb, seed, tag, t, ctrl, respect_done);
 }
 
 void launch_propose_tc(const float* phi, float* phip, const float* Zs, const float* Lsplit, int ld,
@@ -366,10 +376,6 @@ void launch_propose_tc(const float* phi, float* phip, const float* Zs, const flo
     attr_done = true;
   }
   const int num_sms = num_sms_cached();
-  if (propose_tc2_usable(V, ld, num_sms)) {
-    launch_propose_tc2(phi, phip, Zs, Lsplit, ld, V, ctrl, respect_done, num_sms, st);
-    return;
-  }
   ProposeTcParams p;
   p.phi = phi; p.phip = phip; p.Zs = Zs; p.Lsplit = Lsplit; p.ctrl = ctrl;
   p.ld = ld; p.V = V;
