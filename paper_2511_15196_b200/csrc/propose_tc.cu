@@ -261,22 +261,31 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
       const size_t col = (size_t)m * TILE + Q * 32 + lane;
       const int x0 = n0 + hc * 128;
       if (nst <= SUB_STAGES) {
-        // one chain: accumulator -> phi' directly, 16 columns (16 loads in flight) at a time
+        // one chain: phi does not depend on the product, so all 128 loads of this warp's columns
+        // are issued BEFORE the wait for the accumulator -- their HBM latency hides behind the
+        // MMAs of the tile (issued after the wait, 8 batches x ~1.5 us made a short tile's
+        // epilogue longer than the next tile's MMAs)
         const int buf = cnt & 1;
+        float f[128];
+#pragma unroll
+        for (int j = 0; j < 128; ++j)
+          f[j] = (x0 + j < V) ? p.phi[(size_t)(x0 + j) * p.ld + col] : 0.f;
         mbar_wait_relaxed(dfull(buf), (cnt >> 1) & 1);
         tc_fence_after();
-        for (int cb = 0; cb < 128; cb += 16) {
-          uint32_t r[16];
-          tmem_ld16(tlane + (uint32_t)(buf * TN + hc * 128 + cb), r);
-          float f[16];
 #pragma unroll
-          for (int jj = 0; jj < 16; ++jj)
-            f[jj] = (x0 + cb + jj < V) ? p.phi[(size_t)(x0 + cb + jj) * p.ld + col] : 0.f;
+        for (int cb = 0; cb < 128; cb += 32) {
+          uint32_t r0[16], r1[16];
+          tmem_ld16(tlane + (uint32_t)(buf * TN + hc * 128 + cb), r0);
+          tmem_ld16(tlane + (uint32_t)(buf * TN + hc * 128 + cb + 16), r1);
           tmem_ld_wait();
 #pragma unroll
           for (int jj = 0; jj < 16; ++jj)
             if (x0 + cb + jj < V)
-              p.phip[(size_t)(x0 + cb + jj) * p.ld + col] = f[jj] + __uint_as_float(r[jj]);
+              p.phip[(size_t)(x0 + cb + jj) * p.ld + col] = f[cb + jj] + __uint_as_float(r0[jj]);
+#pragma unroll
+          for (int jj = 0; jj < 16; ++jj)
+            if (x0 + cb + 16 + jj < V)
+              p.phip[(size_t)(x0 + cb + 16 + jj) * p.ld + col] = f[cb + 16 + jj] + __uint_as_float(r1[jj]);
         }
         tc_fence_before();
         __syncwarp();
