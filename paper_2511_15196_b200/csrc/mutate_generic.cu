@@ -118,9 +118,10 @@ __device__ __forceinline__ void site_diff(float a, float b, float c, float a2, f
 // Block = 32 particles x 8 row groups (one warp per group).  Phase 1: partial dS, dU0 over the
 // group's lattice rows.  Phase 2: warp 0 decides (R4 margin; NS: also S' < S_star).  Phase 3:
 // every group commits its rows of the accepted particles.
-// G row groups (8 or 32 warps): a small population does not fill the GPU with 8-warp blocks and a
-// warp then walks a long band of rows with ~L2-latency per site; 32 groups shorten the band.
-template <bool IRMH, int G>
+// G row groups (8, 16 or 32 warps): a small population does not fill the GPU with 8-warp blocks and
+// a warp then walks a long band of rows with ~L2-latency per site; 32 groups shorten the band.
+// NR > 0: column walk over bands of at most NR rows (large populations); NR = 0: row walk.
+template <bool IRMH, int G, int NR>
 __global__ void __launch_bounds__(32 * G)
 accept_kernel(float* __restrict__ phi, const float* __restrict__ phip, float* __restrict__ S,
               float* __restrict__ U0, int N, int ld, Model md, int mode, uint64_t seed,
@@ -145,42 +146,46 @@ accept_kernel(float* __restrict__ phi, const float* __restrict__ phip, float* __
         z2 = fmaf(z, z, z2);
       }
     }
-    if (G == 8 && band >= 4 && band <= 8 && ld >= 8192) {
-      // Column walk (large populations; a small one is latency-bound and prefers the row walk): the band's rows (<= 8) and the halo row below it are held for two adjacent
-      // lattice columns in registers, so every site of phi and phi' is loaded once (plus the
-      // halo row and the wrap-around column) instead of once as a site and again as the "down"
-      // neighbour of the row above -- the kernel is HBM-bound at C3 / C4.
+    if constexpr (NR > 0) {
+      // Column walk (large populations; a small one is latency-bound and prefers the row walk):
+      // the band's rows (<= NR) and the halo row below it are held in registers for the current
+      // column and the two columns to its right, so every site of phi and phi' is loaded once
+      // (plus the halo row and the wrap-around column) instead of once as a site and again as the
+      // "down" neighbour of the row above.  The kernel is HBM-bound at C3 / C4 and the bytes in
+      // flight are what its registers can hold: loads run two columns ahead of the arithmetic
+      // (one column ahead with 8-row bands: 30-55 KB in flight per SM, 3.4-4.8 TB/s, round 1).
       const int nr = r_hi - r_lo;
       const int rh = (r_hi == L) ? 0 : r_hi;              // halo row below the band
-      float A[9], A2[9], Bn[9], B2[9], rS[8], rU[8];
+      float A[NR + 1], A2[NR + 1], Bn[NR + 1], B2[NR + 1], Cn[NR + 1], C2[NR + 1], rS[NR], rU[NR];
 #pragma unroll
-      for (int q = 0; q < 8; ++q) { rS[q] = 0.f; rU[q] = 0.f; }
-      auto load_col = [&](int c, float (&X)[9], float (&X2)[9]) {
+      for (int q = 0; q < NR; ++q) { rS[q] = 0.f; rU[q] = 0.f; }
+      auto load_col = [&](int c, float (&X)[NR + 1], float (&X2)[NR + 1]) {
 #pragma unroll
-        for (int q = 0; q < 8; ++q)
+        for (int q = 0; q < NR; ++q)
           if (q < nr) {
             const size_t o = ((size_t)(r_lo + q) * L + c) * ld + i;
             X[q] = phi[o]; X2[q] = phip[o];
           }
         const size_t o = ((size_t)rh * L + c) * ld + i;
-        X[8] = phi[o]; X2[8] = phip[o];
+        X[NR] = phi[o]; X2[NR] = phip[o];
       };
       if (nr > 0) {
         load_col(0, A, A2);
+        load_col(1 % L, Bn, B2);
         for (int c = 0; c < L; ++c) {
-          load_col(c + 1 == L ? 0 : c + 1, Bn, B2);
+          if (c + 2 <= L) load_col(c + 2 == L ? 0 : c + 2, Cn, C2);
 #pragma unroll
-          for (int q = 0; q < 8; ++q)
+          for (int q = 0; q < NR; ++q)
             if (q < nr) {
-              const float d = (q + 1 < nr) ? A[q + 1 < 8 ? q + 1 : 8] : A[8];
-              const float d2 = (q + 1 < nr) ? A2[q + 1 < 8 ? q + 1 : 8] : A2[8];
+              const float d = (q + 1 < nr) ? A[q + 1 < NR ? q + 1 : NR] : A[NR];
+              const float d2 = (q + 1 < nr) ? A2[q + 1 < NR ? q + 1 : NR] : A2[NR];
               site_diff(A[q], Bn[q], d, A2[q], B2[q], d2, hk, hm, lam, rS[q], rU[q]);
             }
 #pragma unroll
-          for (int q = 0; q < 9; ++q) { A[q] = Bn[q]; A2[q] = B2[q]; }
+          for (int q = 0; q <= NR; ++q) { A[q] = Bn[q]; A2[q] = B2[q]; Bn[q] = Cn[q]; B2[q] = C2[q]; }
         }
 #pragma unroll
-        for (int q = 0; q < 8; ++q)
+        for (int q = 0; q < NR; ++q)
           if (q < nr) { dS += rS[q]; dU += rU[q]; }
       }
     } else {
@@ -255,6 +260,8 @@ void launch_mutate_generic(const MutateArgs& a, float* Lsplit, cudaStream_t st) 
   const int V = a.md.V;
   // fewer than two 8-warp blocks per SM and more than 8 lattice rows: one warp per row instead
   const bool wide = a.md.L > 8 && a.ld / 32 < 2 * 148;
+  // large populations: column walk over bands of <= 4 lattice rows (8, 16 or 32 row groups)
+  const bool colwalk = !wide && a.ld >= 8192 && a.md.L >= 25 && a.md.L <= 128;
   dim3 gz((a.ld + 127) / 128, (V + 3) / 4);
   dim3 gp(a.ld / 64, (V + 63) / 64);
   if (Lsplit) {
@@ -272,18 +279,18 @@ void launch_mutate_generic(const MutateArgs& a, float* Lsplit, cudaStream_t st) 
                                          0, a.ctrl, a.respect_done);
     }
     ++g_launches;
-    if (wide)
-      launch_pdl(accept_kernel<false, 32>, a.ld / 32, 1024, 0, st,
+    auto launch_accept = [&](auto kern, int G) {
+      launch_pdl(kern, a.ld / 32, 32 * G, 0, st,
                  a.phi, a.phip, a.S, a.U0, a.N, a.ld, a.md, a.mode, a.seed, a.tag_acc, t, a.ctrl,
                  a.acc_out ? a.acc_out + (size_t)j * a.N : nullptr,
                  a.margin_out ? a.margin_out + (size_t)j * a.N : nullptr, a.respect_done,
                  (const float*)nullptr, (float*)nullptr);
-    else
-      launch_pdl(accept_kernel<false, 8>, a.ld / 32, 256, 0, st,
-                 a.phi, a.phip, a.S, a.U0, a.N, a.ld, a.md, a.mode, a.seed, a.tag_acc, t, a.ctrl,
-                 a.acc_out ? a.acc_out + (size_t)j * a.N : nullptr,
-                 a.margin_out ? a.margin_out + (size_t)j * a.N : nullptr, a.respect_done,
-                 (const float*)nullptr, (float*)nullptr);
+    };
+    if (wide) launch_accept(accept_kernel<false, 32, 0>, 32);
+    else if (colwalk && a.md.L <= 32) launch_accept(accept_kernel<false, 8, 4>, 8);
+    else if (colwalk && a.md.L <= 64) launch_accept(accept_kernel<false, 16, 4>, 16);
+    else if (colwalk) launch_accept(accept_kernel<false, 32, 4>, 32);
+    else launch_accept(accept_kernel<false, 8, 0>, 8);
   }
 }
 
@@ -332,7 +339,7 @@ void launch_mutate_irmh(const MutateArgs& a, const float* mu, float* W2, cudaStr
                                        a.respect_done);
     ++g_launches; propose_kernel<<<gp, 256, 0, st>>>(a.Lc, a.Z, a.phi, a.phip, V, a.ld, 1.0f, mu,
                                        0, a.ctrl, a.respect_done);
-    ++g_launches; accept_kernel<true, 8><<<a.ld / 32, 256, 0, st>>>(
+    ++g_launches; accept_kernel<true, 8, 0><<<a.ld / 32, 256, 0, st>>>(
         a.phi, a.phip, a.S, a.U0, a.N, a.ld, a.md, MODE_IRMH, a.seed, a.tag_acc, t, a.ctrl,
         a.acc_out ? a.acc_out + (size_t)j * a.N : nullptr,
         a.margin_out ? a.margin_out + (size_t)j * a.N : nullptr, a.respect_done, a.Z, W2);
