@@ -302,9 +302,17 @@ def ns_run(h, max_iters=4096):
     return n.value
 
 
-def smc_get_state(h, want_phi=True):
-    phi = np.empty((h.V, h.N), np.float32) if want_phi else None
-    S, U0 = np.empty(h.N, np.float32), np.empty(h.N, np.float32)
+def smc_get_state(h, want_phi=True, out=None):
+    """out: optional dict of caller-owned C-contiguous fp32 arrays "phi" (V, N), "S" (N,), "U0" (N,)
+    to receive the copies (e.g. views of pinned host memory: the device-to-host copies then run at
+    full PCIe rate instead of through the driver's staging of pageable memory)."""
+    if out is not None:
+        phi, S, U0 = (out["phi"] if want_phi else None), out["S"], out["U0"]
+        for a, shp in ((phi, (h.V, h.N)), (S, (h.N,)), (U0, (h.N,))):
+            assert a is None or (a.dtype == np.float32 and a.shape == shp and a.flags["C_CONTIGUOUS"])
+    else:
+        phi = np.empty((h.V, h.N), np.float32) if want_phi else None
+        S, U0 = np.empty(h.N, np.float32), np.empty(h.N, np.float32)
     beta, t = C.c_double(0), C.c_uint64(0)
     h._check(load().smc_get_state(h.ptr, _np_ptr(phi), _np_ptr(S), _np_ptr(U0), C.byref(beta),
                                   C.byref(t)), "smc_get_state")
