@@ -27,7 +27,8 @@ ALU_OPS_PER_SITE_UPDATE = 40          # Philox ~20 int + Box-Muller
 # *a 1, + 1, beta*gs+a 1, kick 1, drift 1
 ALU_OPS_PER_LEAPFROG_SITE = 11
 # dram__bytes_read.sum + dram__bytes_write.sum of one mutation launch (profiles/, ncu --set full)
-NCU_DRAM_BYTES = {"C1": 6815488}
+# (C1: the fused kernel; C3 / C4: the proposal GEMM, the dominant kernel of the large-V step)
+NCU_DRAM_BYTES = {"C1": 6815744, "C3": 1127837175, "C4": 15380342000}
 
 
 def peaks():

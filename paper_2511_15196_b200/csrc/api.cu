@@ -369,7 +369,9 @@ static bool use_tc_propose(const phi4smc* h) {
 
 static void enqueue_mutation(phi4smc* h, const MutateArgs& a) {
   if (h->prm.kernel == 1 && a.mode == MODE_SMC && !hmc_supported(a.md.V)) {
-    launch_hmc_generic(a.phi, a.S, a.U0, h->Sigma, a.phip, a.Z, h->W2, a.N, a.ld, a.md, h->prm.hmc_eps,
+    // positions double-buffered in phip and the second half of the normal scratch (2 V ld floats
+    // whenever the tcgen05 proposal exists, i.e. for every V this path serves), momenta in its first
+    launch_hmc_generic(a.phi, a.S, a.U0, h->Sigma, a.phip, a.Z + (size_t)a.md.V * a.ld, a.Z, h->W2, a.N, a.ld, a.md, h->prm.hmc_eps,
                        h->prm.hmc_leapfrog, a.seed, a.t0, a.k, a.ctrl, a.acc_out, a.margin_out,
                        a.respect_done, h->st);
     return;

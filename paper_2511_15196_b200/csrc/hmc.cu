@@ -320,17 +320,29 @@ hmc_g_kick_kernel(const float* __restrict__ q, float* __restrict__ p, int N, int
   p[o] = fmaf(-h, fmaf(beta, gs, a), p[o]);
 }
 
-// q += eps var p
+// Kick and the drift that follows it in one pass: p -= h grad U(q_in); q_out = q_in + eps var p.
+// The drift must not overwrite positions that other threads still read as neighbours, so q is
+// double-buffered; the arithmetic is that of the two separate kernels, bit for bit.  16 B per
+// site and leapfrog step instead of 24 (the path is HBM-bound).
 __global__ void __launch_bounds__(256)
-hmc_g_drift_kernel(float* __restrict__ q, const float* __restrict__ p,
-                   const float* __restrict__ Sigma, int N, int ld, int V, float eps,
-                   const Ctrl* ctrl, int respect_done) {
+hmc_g_kickdrift_kernel(const float* __restrict__ qin, float* __restrict__ qout, float* __restrict__ p,
+                       const float* __restrict__ Sigma, int N, int ld, Model md, float h, float eps,
+                       const Ctrl* ctrl, int respect_done) {
   if (respect_done && ctrl->done) return;
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= N) return;
-  const int x = blockIdx.y;
+  const int L = md.L, V = md.V, x = blockIdx.y, r = x / L, c = x - r * L;
+  const int ce = c + 1 == L ? 0 : c + 1, cw = c == 0 ? L - 1 : c - 1;
+  const int rs = r + 1 == L ? 0 : r + 1, rn = r == 0 ? L - 1 : r - 1;
+  const float a = qin[(size_t)x * ld + i];
+  const float e = qin[(size_t)(r * L + ce) * ld + i], w = qin[(size_t)(r * L + cw) * ld + i];
+  const float n = qin[(size_t)(rn * L + c) * ld + i], s = qin[(size_t)(rs * L + c) * ld + i];
+  const float beta = (float)ctrl->beta;
+  const float gs = fmaf(md.kappa, fmaf(4.0f, a, -((e + w) + (n + s))), a * fmaf(4.0f * md.lam, a * a, md.m0sq));
   const size_t o = (size_t)x * ld + i;
-  q[o] = fmaf(eps * Sigma[(size_t)x * V + x], p[o], q[o]);
+  const float pn = fmaf(-h, fmaf(beta, gs, a), p[o]);
+  p[o] = pn;
+  qout[o] = fmaf(eps * Sigma[(size_t)x * V + x], pn, a);
 }
 
 // H_new, margin, accept, commit.  Block = 32 particles x 8 row groups (as accept_kernel).
@@ -398,9 +410,9 @@ hmc_g_accept_kernel(float* __restrict__ phi, const float* __restrict__ q,
   }
 }
 
-// q, p: [V][ld] scratch each; K0: [ld] scratch
-void launch_hmc_generic(float* phi, float* S, float* U0, const float* Sigma, float* q, float* p,
-                        float* K0, int N, int ld, Model md, float eps, int nfrog, uint64_t seed,
+// q, q2, p: [V][ld] scratch each; K0: [ld] scratch
+void launch_hmc_generic(float* phi, float* S, float* U0, const float* Sigma, float* q, float* q2,
+                        float* p, float* K0, int N, int ld, Model md, float eps, int nfrog, uint64_t seed,
                         uint32_t t0, int k, Ctrl* ctrl, uint8_t* acc_out, float* margin_out,
                         int respect_done, cudaStream_t st) {
   const int V = md.V;
@@ -409,18 +421,21 @@ void launch_hmc_generic(float* phi, float* S, float* U0, const float* Sigma, flo
     const uint32_t t = t0 + (uint32_t)j;
     ++g_launches;
     hmc_g_init_kernel<<<ld / 32, 256, 0, st>>>(phi, q, p, Sigma, K0, N, ld, V, seed, t, ctrl, respect_done);
-    ++g_launches;
-    hmc_g_kick_kernel<<<gs, 256, 0, st>>>(q, p, N, ld, md, 0.5f * eps, ctrl, respect_done);
+    // p -= eps/2 grad U; nfrog x { q += eps var p; p -= eps grad U (eps/2 after the last drift) }
+    // as nfrog fused (kick, drift) passes between the two position buffers and one last kick
+    float* qa = q;
+    float* qb = q2;
     for (int s = 0; s < nfrog; ++s) {
       ++g_launches;
-      hmc_g_drift_kernel<<<gs, 256, 0, st>>>(q, p, Sigma, N, ld, V, eps, ctrl, respect_done);
-      ++g_launches;
-      hmc_g_kick_kernel<<<gs, 256, 0, st>>>(q, p, N, ld, md, (s + 1 == nfrog) ? 0.5f * eps : eps, ctrl,
-                                            respect_done);
+      hmc_g_kickdrift_kernel<<<gs, 256, 0, st>>>(qa, qb, p, Sigma, N, ld, md, s == 0 ? 0.5f * eps : eps, eps,
+                                                 ctrl, respect_done);
+      float* tmp = qa; qa = qb; qb = tmp;
     }
     ++g_launches;
+    hmc_g_kick_kernel<<<gs, 256, 0, st>>>(qa, p, N, ld, md, 0.5f * eps, ctrl, respect_done);
+    ++g_launches;
     hmc_g_accept_kernel<<<ld / 32, 256, 0, st>>>(
-        phi, q, p, Sigma, K0, S, U0, N, ld, md, seed, t, ctrl,
+        phi, qa, p, Sigma, K0, S, U0, N, ld, md, seed, t, ctrl,
         acc_out ? acc_out + (size_t)j * N : nullptr, margin_out ? margin_out + (size_t)j * N : nullptr,
         respect_done);
   }

@@ -130,8 +130,8 @@ void launch_ns_finish(const NsArgs& a, StepRecord* rec, int n_walk, cudaStream_t
 namespace phi4 {
 // hmc.cu -- NEXT f1: k HMC transitions with mass matrix diag(1/Sigma_xx) (reading A14)
 bool hmc_supported(int V);   // the on-chip kernel (L <= 22); larger lattices take launch_hmc_generic
-void launch_hmc_generic(float* phi, float* S, float* U0, const float* Sigma, float* q, float* p,
-                        float* K0, int N, int ld, Model md, float eps, int nfrog, uint64_t seed,
+void launch_hmc_generic(float* phi, float* S, float* U0, const float* Sigma, float* q, float* q2,
+                        float* p, float* K0, int N, int ld, Model md, float eps, int nfrog, uint64_t seed,
                         uint32_t t0, int k, Ctrl* ctrl, uint8_t* acc_out, float* margin_out,
                         int respect_done, cudaStream_t st);
 void launch_hmc(float* phi, float* S, float* U0, const float* Sigma, int N, int ld, Model md,

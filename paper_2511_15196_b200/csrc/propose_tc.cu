@@ -5,15 +5,17 @@
 // proposal product L*z ... as tcgen05/TMEM tiles in 3xTF32 split precision"; PAPER.md:53(i), :172).
 //
 //   normals_split_kernel  Philox normals of one step, split hi/lo, written straight in the UMMA
-//                         K-major interleave layout, tile-major: Zs[part][particle tile][K-chunk]
-//                         [128 rows][4] -- a ring stage is one contiguous 8 KB run per part.
+//                         K-major interleave layout, stage-major: Zs[particle tile][K-stage][part]
+//                         [4 chunks][128 rows][4] -- a ring stage is one contiguous 16 KB run.
+//   lsplit_tiled_kernel   s*Lc split hi/lo once per temperature, stored per (site tile, K-stage):
+//                         only the rows the stage can reach (lower-triangular), one run per stage.
 //   propose_tc_kernel     one CTA per SM loops over (particle tile 128) x (site tile 256) output
-//                         tiles.  Warp 8 streams A (normals) and B (s Lc, packed lower-triangular
-//                         blocks of tcgen05.cuh) into a 4-stage shared-memory ring with
-//                         cp.async.bulk + mbarrier; warp 9 issues tcgen05.mma kind::tf32 (three
-//                         products per K-step into one FP32 TMEM accumulator, K-steps above the
-//                         diagonal skipped, N shrunk inside the diagonal block); warps 0-7 read the
-//                         accumulator with tcgen05.ld (lane = particle) and write phi' = phi + d,
+//                         tiles, in pairs of site tiles of equal total length.  Warp 8 streams A
+//                         (normals) and B (s Lc) into a 4-stage shared-memory ring with two
+//                         cp.async.bulk per stage + mbarrier; warp 9 issues tcgen05.mma kind::tf32
+//                         (three products per K-step into one FP32 TMEM accumulator, K-steps above
+//                         the diagonal skipped, N shrunk inside the diagonal block); warps 0-7 read
+//                         the accumulator with tcgen05.ld (lane = particle) and write phi' = phi + d,
 //                         coalesced along particles.  The accumulator is double-buffered (2 x 256
 //                         TMEM columns), so the epilogue of a tile overlaps the MMAs of the next.
 // The tensor core's FP32 accumulation truncates (measured in syrk_tc.cu: -1e-4 relative over 3000
