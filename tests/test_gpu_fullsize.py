@@ -19,9 +19,22 @@ def _built():
     B.load()
 
 
-@pytest.mark.parametrize("name,k,n_sub", [("C1", 20, 512), ("C3", 2, 256), ("C4", 1, 96)])
+# Ragged shapes that still fill the GPU (the launch configurations of the large-V kernels depend on
+# the population: paired site tiles in the proposal GEMM once there are more tiles than SMs, the
+# column-walk accept with 8 / 16 row groups): V not a multiple of 256 or 16, an odd number of site
+# tiles, N not a multiple of 128, row groups with fewer rows than the others or none, K > 1024
+# (several TMEM accumulation chains).
+RAGGED = {
+    "R20": dict(L=20, N=19200, m0sq=-4.0, lam=1.0, ess=0.5),     # V = 400: 2 site tiles, 25 K-stages
+    "R27": dict(L=27, N=10000, m0sq=-4.0, lam=1.0, ess=0.5),     # V = 729: 3 site tiles, ld = 10112
+    "R40": dict(L=40, N=8192, m0sq=-4.0, lam=1.0, ess=0.5),      # V = 1600: 7 site tiles, 2 chains
+}
+
+
+@pytest.mark.parametrize("name,k,n_sub", [("C1", 20, 512), ("C3", 2, 256), ("C4", 1, 96),
+                                          ("R20", 3, 256), ("R27", 2, 192), ("R40", 2, 128)])
 def test_full_size_transition(name, k, n_sub):
-    c = inputs.CONFIGS[name]
+    c = inputs.CONFIGS[name] if name in inputs.CONFIGS else RAGGED[name]
     L, N, V, seed = c["L"], c["N"], c["L"] ** 2, 0
     rng = np.random.default_rng(123)
     h = B.smc_init(L, c["m0sq"], c["lam"], N, seed)
