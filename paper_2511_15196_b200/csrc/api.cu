@@ -67,6 +67,10 @@ struct phi4smc {
   Ctrl* h_ctrl;              // pinned staging
   Ctrl* h_poll;              // pinned, 2 slots: smc_run / ns_run poll one step behind the GPU
   cudaEvent_t poll_ev[2];
+  // nested sampling: the dead-point selection does not depend on the covariance chain, so it runs
+  // on a side stream (fork / join by events on the caller's stream; host resources only)
+  cudaStream_t side;
+  cudaEvent_t fork_ev, join_ev;
   StepRecord* h_rec;         // pinned staging (one record)
   double* h_obs;             // pinned staging (85 doubles)
   char err[256];
@@ -222,6 +226,11 @@ static int host_staging(phi4smc* h) {
   CU(cudaMallocHost((void**)&h->h_ctrl, sizeof(Ctrl)));
   CU(cudaMallocHost((void**)&h->h_poll, 2 * sizeof(Ctrl)));
   for (int e = 0; e < 2; ++e) CU(cudaEventCreateWithFlags(&h->poll_ev[e], cudaEventDisableTiming));
+  if (h->kind == KIND_NS) {
+    CU(cudaStreamCreateWithFlags(&h->side, cudaStreamNonBlocking));
+    CU(cudaEventCreateWithFlags(&h->fork_ev, cudaEventDisableTiming));
+    CU(cudaEventCreateWithFlags(&h->join_ev, cudaEventDisableTiming));
+  }
   CU(cudaMallocHost((void**)&h->h_rec, sizeof(StepRecord)));
   CU(cudaMallocHost((void**)&h->h_obs, sizeof(double) * (5 + PHI4_HIST_BINS)));
   return PHI4_OK;
@@ -324,6 +333,9 @@ PHI4_API int smc_destroy(phi4smc* h) {
   if (h->h_ctrl) cudaFreeHost(h->h_ctrl);
   if (h->h_poll) cudaFreeHost(h->h_poll);
   for (int e = 0; e < 2; ++e) if (h->poll_ev[e]) cudaEventDestroy(h->poll_ev[e]);
+  if (h->side) { cudaStreamSynchronize(h->side); cudaStreamDestroy(h->side); }
+  if (h->fork_ev) cudaEventDestroy(h->fork_ev);
+  if (h->join_ev) cudaEventDestroy(h->join_ev);
   if (h->h_rec) cudaFreeHost(h->h_rec);
   if (h->h_obs) cudaFreeHost(h->h_obs);
   delete h;
@@ -616,9 +628,16 @@ PHI4_API int ns_init_kl(phi4smc** out, int L, float kappa, float lambda, int n_l
 
 static void enqueue_ns_step(phi4smc* h) {
   NsArgs a = ns_args(h);
+  // N1 / N2 and the walker gather (S_E order, evidence, start points) read nothing the covariance
+  // chain writes: they run beside it on the side stream (38 + 8 us hidden behind mean / syrk /
+  // Cholesky, 50 us, at C2)
+  cudaEventRecord(h->fork_ev, h->st);
+  cudaStreamWaitEvent(h->side, h->fork_ev, 0);
+  launch_ns_select_evidence(a, h->side);
+  launch_ns_load_walkers(a, h->side);
+  cudaEventRecord(h->join_ev, h->side);
   launch_cov_chol(cov_args(h, 1), h->st);
-  launch_ns_select_evidence(a, h->st);
-  launch_ns_load_walkers(a, h->st);
+  cudaStreamWaitEvent(h->st, h->join_ev, 0);
   MutateArgs m;
   m.phi = h->wphi; m.phip = h->phip; m.Z = h->Z; m.S = h->wS; m.U0 = h->wU; m.Lc = h->Lc;
   m.ctrl = h->ctrl; m.acc_out = nullptr; m.margin_out = nullptr;
