@@ -18,6 +18,9 @@
  *    and the CUDA stream (a cudaStream_t passed as void*; NULL = the legacy default stream).  The
  *    library owns the opaque handle, keeps all state inside the workspace and never allocates
  *    device memory after *_init.  The workspace must outlive the handle.
+ *  - The handle also owns one internal side stream (a host resource): independent branches of a
+ *    step run there, forked from and joined back into the caller's stream by events inside the
+ *    same call, so the caller's stream order is all a caller ever needs to reason about.
  *  - Work is enqueued on the handle's stream.  A function synchronises the stream only when it
  *    returns host values (an info struct, a host array, a double); this is stated per function.
  *  - Host-visible particle arrays are fp32, site-major and dense: h_phi[x*N + i], x = site,
@@ -123,7 +126,7 @@ uint64_t phi4_kernel_launches(void);
 
 /* ---------------------------------------------------------------- SMC-RW (PAPER.md:53(i)) ----
  * smc_workspace_bytes: bytes of device memory smc_init needs for an L x L lattice and N particles
- * (0 if L < 1 or N < 2).  Sized for 180 GB parts: C4 (L=64, N=131072) needs about 11 GB.          */
+ * (0 if L < 1 or N < 2).  Sized for 180 GB parts: C4 (L=64, N=131072) needs about 15 GB.          */
 size_t smc_workspace_bytes(int L, int N);
 
 /* Creates an SMC sampler: particles phi_i ~ N(0,I) from Philox stream INIT, S_E and U0 evaluated,

@@ -46,7 +46,7 @@ struct phi4smc {
   // device state (inside the workspace)
   float* phi[2]; float* S[2]; float* U0[2];
   int cur;
-  float *phip, *Z, *w, *W2, *mu, *Sigma, *Lc, *Lsplit, *partial, *M, *margins;
+  float *phip, *Z, *Z2, *w, *W2, *mu, *Sigma, *Lc, *Lsplit, *partial, *M, *margins;
   unsigned long long* C;
   int32_t* anc;
   uint8_t* acc_flags;
@@ -67,8 +67,9 @@ struct phi4smc {
   Ctrl* h_ctrl;              // pinned staging
   Ctrl* h_poll;              // pinned, 2 slots: smc_run / ns_run poll one step behind the GPU
   cudaEvent_t poll_ev[2];
-  // nested sampling: the dead-point selection does not depend on the covariance chain, so it runs
-  // on a side stream (fork / join by events on the caller's stream; host resources only)
+  // side stream (fork / join by events on the caller's stream; host resources only): nested
+  // sampling runs the dead-point selection beside the covariance chain, the large-V mutation draws
+  // the normals of the next step beside the proposal GEMM of the current one
   cudaStream_t side;
   cudaEvent_t fork_ev, join_ev;
   StepRecord* h_rec;         // pinned staging (one record)
@@ -102,6 +103,8 @@ static int carve_smc(phi4smc* h, char* base, size_t* total) {
     if (propose_tc_supported(V) && propose_tc_zsplit_floats(V, ld) > zf) zf = propose_tc_zsplit_floats(V, ld);
     if (syrk_tc_supported(V, ld) && syrk_tc_scratch_floats(V, ld) > zf) zf = syrk_tc_scratch_floats(V, ld);
     h->Z = c.take<float>(zf);
+    // second buffer of split normals: step t+1 is drawn while step t multiplies (launch_mutate_generic)
+    h->Z2 = propose_tc_supported(V) ? c.take<float>(propose_tc_zsplit_floats(V, ld)) : nullptr;
   }
   h->w = c.take<float>(ld);
   h->W2 = c.take<float>(ld);                               // IRMH: |Lc^-1 (phi - mu)|^2
@@ -134,6 +137,7 @@ static int carve_ns(phi4smc* h, char* base, size_t* total) {
   h->wU = c.take<float>(ldw);
   h->phip = c.take<float>((size_t)V * ldw);
   h->Z = c.take<float>(propose_tc_supported(V) ? propose_tc_zsplit_floats(V, ldw) : (size_t)V * ldw);
+  h->Z2 = propose_tc_supported(V) ? c.take<float>(propose_tc_zsplit_floats(V, ldw)) : nullptr;
   h->mu = c.take<float>(V);
   h->Sigma = c.take<float>((size_t)V * V);
   h->Lc = c.take<float>((size_t)V * V);
@@ -226,7 +230,7 @@ static int host_staging(phi4smc* h) {
   CU(cudaMallocHost((void**)&h->h_ctrl, sizeof(Ctrl)));
   CU(cudaMallocHost((void**)&h->h_poll, 2 * sizeof(Ctrl)));
   for (int e = 0; e < 2; ++e) CU(cudaEventCreateWithFlags(&h->poll_ev[e], cudaEventDisableTiming));
-  if (h->kind == KIND_NS) {
+  {
     CU(cudaStreamCreateWithFlags(&h->side, cudaStreamNonBlocking));
     CU(cudaEventCreateWithFlags(&h->fork_ev, cudaEventDisableTiming));
     CU(cudaEventCreateWithFlags(&h->join_ev, cudaEventDisableTiming));
@@ -361,6 +365,7 @@ PHI4_API int smc_set_params(phi4smc* h, const smc_params* p) {
 static MutateArgs smc_mutate_args(phi4smc* h, int k, uint8_t* acc, float* mar, int respect_done) {
   MutateArgs a;
   a.phi = h->phi[h->cur]; a.phip = h->phip; a.Z = h->Z;
+  a.Z2 = h->Z2; a.side = h->side; a.fork_ev = h->fork_ev; a.join_ev = h->join_ev;
   a.S = h->S[h->cur]; a.U0 = h->U0[h->cur]; a.Lc = h->Lc; a.ctrl = h->ctrl;
   a.acc_out = acc; a.margin_out = mar;
   a.N = h->N; a.ld = h->ld; a.md = h->md; a.s = h->s; a.mode = MODE_SMC; a.seed = h->seed;
@@ -639,6 +644,7 @@ static void enqueue_ns_step(phi4smc* h) {
   launch_cov_chol(cov_args(h, 1), h->st);
   cudaStreamWaitEvent(h->st, h->join_ev, 0);
   MutateArgs m;
+  m.Z2 = h->Z2; m.side = h->side; m.fork_ev = h->fork_ev; m.join_ev = h->join_ev;
   m.phi = h->wphi; m.phip = h->phip; m.Z = h->Z; m.S = h->wS; m.U0 = h->wU; m.Lc = h->Lc;
   m.ctrl = h->ctrl; m.acc_out = nullptr; m.margin_out = nullptr;
   m.N = h->k_del; m.ld = h->ldw; m.md = h->md; m.s = h->s; m.mode = MODE_NS; m.seed = h->seed;

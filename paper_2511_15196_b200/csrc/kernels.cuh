@@ -35,6 +35,12 @@ struct MutateArgs {
   uint32_t t0;       // step counter of the first step
   int k;             // number of steps
   int respect_done;  // 1: every kernel is a no-op once ctrl->done is set
+  // Large-V tcgen05 path only (nullptr / 0 otherwise): a second buffer for the split normals and a
+  // side stream with two events, so that the normals of step t+1 are drawn while the proposal GEMM
+  // and the accept kernel of step t run (the normals depend on nothing but the counters).
+  float* Z2;
+  cudaStream_t side;
+  cudaEvent_t fork_ev, join_ev;
 };
 void launch_mutate_generic(const MutateArgs& a, float* Lsplit, cudaStream_t st);
 // NEXT f3: k constrained slice-sampling steps of the NS walkers (reading A16); a.phip = direction
