@@ -62,7 +62,7 @@ typedef struct {
    * HMC: mass matrix diag(1/var_x) from the particle covariance, hmc_leapfrog >= 1 leapfrog steps
    * of size hmc_eps > 0 per transition, k_steps transitions per temperature.  L <= 22 runs in one
    * register/shared-memory resident kernel per temperature; larger lattices keep position and
-   * momentum in HBM scratch with one launch per leapfrog half-step.                             */
+   * momentum in HBM scratch with one launch per leapfrog step (kick + drift in one pass).          */
   int kernel;
   float hmc_eps;
   int hmc_leapfrog;

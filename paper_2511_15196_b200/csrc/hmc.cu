@@ -259,9 +259,10 @@ void launch_hmc(float* phi, float* S, float* U0, const float* Sigma, int N, int 
 
 // ---------------------------------------------------------------------------------------------
 // Any lattice size: the fields of a trajectory no longer fit on one SM (L > 22), so position and
-// momentum live in HBM scratch ([V][ld] each) and every leapfrog half-step is its own launch
-// (the stencil needs the neighbours' updated positions: a grid-wide dependency).  HBM-bound:
-// ~28 B per site per leapfrog step.  Same arithmetic, streams and reading A14 as hmc_kernel.
+// momentum live in HBM scratch ([V][ld] each, positions double-buffered) and every leapfrog step
+// is its own launch (the stencil needs the neighbours' updated positions: a grid-wide
+// dependency): a kick and the drift after it in one pass.  HBM-bound: 16 B per site per leapfrog
+// step.  Same arithmetic, streams and reading A14 as hmc_kernel.
 namespace phi4 {
 
 // momentum refresh, q <- phi, K0 = 1/2 sum z^2.  Block = 32 particles x 8 quad groups.
