@@ -74,8 +74,11 @@ struct SyrkTcParams {
 // item -> (tile row tm, tile col tn, split z); only tiles that touch the lower triangle
 __device__ __forceinline__ void syrk_item(const SyrkTcParams& p, int item, int& m0, int& n0,
                                           int& z) {
-  z = item % p.nsplit;
-  int t = item / p.nsplit;
+  // K range slow, tile fast: the CTAs of a wave walk the same particles in step, so the operand
+  // panels they share are read from HBM once and from L2 afterwards
+  const int ntiles = p.nitems / p.nsplit;
+  z = item / ntiles;
+  int t = item - z * ntiles;
   // enumerate tm = 0..ntm-1, tn = 0..floor((tm*128+127)/256)
   int tm = 0;
   for (;;) {
@@ -241,13 +244,23 @@ static int syrk_tc_tiles(int V) {
   return t;
 }
 
-// K split: enough items for ~2 waves of 148 SMs; every split is a whole number of K = 256 chains.
+// K split: every split is a whole number of K = 256 chains; among the admissible counts (at most
+// ld / V, so that the partial tiles stay small beside the operands) the one whose items fill whole
+// waves of 148 CTAs best (round 1 took "about two waves": 160 items at C3, a second wave of 12).
 int syrk_tc_nsplit(int V, int ld) {
   const int nkc = round_up(ld, 256) >> 2, tiles = syrk_tc_tiles(V);
-  int ns = (2 * 148 + tiles - 1) / tiles;
-  if (ns < 1) ns = 1;
-  while (ns > 1 && (nkc % (4 * sy::SUB_STAGES * ns)) != 0) --ns;
-  return ns;
+  const int chains = nkc / (4 * sy::SUB_STAGES);            // K = 256 chains in the whole population
+  int cap = ld / V;
+  cap = cap < 1 ? 1 : cap > 64 ? 64 : cap;
+  int best = 1;
+  double best_eff = 0.0;
+  for (int ns = 1; ns <= chains && ns <= cap; ++ns) {
+    if (chains % ns) continue;
+    const int items = tiles * ns, waves = (items + 147) / 148;
+    const double eff = (double)items / (148.0 * waves);
+    if (eff > best_eff + 1e-9) { best_eff = eff; best = ns; }
+  }
+  return best;
 }
 
 size_t syrk_tc_scratch_floats(int V, int ld) {
