@@ -412,6 +412,7 @@ static CovCholArgs cov_args(phi4smc* h, int respect_done) {
   c.mu = h->mu; c.Sigma = h->Sigma; c.Lc = h->Lc; c.partial = h->partial; c.ctrl = h->ctrl;
   // the split-normal scratch of the large-V proposal doubles as the centred-split scratch
   c.tc_scratch = (h->prm.mutation_path != 1 && propose_tc_supported(h->md.V) && h->kind == KIND_SMC) ? h->Z : nullptr;
+  c.tc_small = h->prm.mutation_path != 1;
   c.respect_done = respect_done;
   return c;
 }

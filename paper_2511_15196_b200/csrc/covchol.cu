@@ -472,6 +472,7 @@ size_t cov_partial_floats(int V, int N) {
   int ns = cov_nsplit(V, N);
   const int ld = round_up(N, 128);
   if (syrk_tc_supported(V, ld) && syrk_tc_nsplit(V, ld) > ns) ns = syrk_tc_nsplit(V, ld);
+  if (syrk_tc_small_supported(V, ld) && syrk_tc_small_nsplit(ld) > ns) ns = syrk_tc_small_nsplit(ld);
   return (size_t)ns * V * V;
 }
 
@@ -481,6 +482,14 @@ void launch_cov_chol(const CovCholArgs& a, cudaStream_t st) {
   if (a.tc_scratch && syrk_tc_supported(V, a.ld)) {
     launch_syrk_tc(a.phi, a.N, a.ld, V, a.mu, a.tc_scratch, a.partial, a.ctrl, a.respect_done, st);
     launch_syrk_reduce(a.partial, syrk_tc_nsplit(V, a.ld), V, a.N, a.Sigma, a.ctrl, a.respect_done, st);
+    launch_cholesky(a.Sigma, a.Lc, V, a.ctrl, a.respect_done, st);
+    return;
+  }
+  // (populations below 8192 stay on the SIMT tiles: at n_live = 4096 the 32 tensor-core CTAs take
+  // 11 us against 10 for the 3 x 94 SIMT blocks; at N = 16384 it is 11 against 19)
+  if (a.tc_small && a.ld >= 8192 && syrk_tc_small_supported(V, a.ld)) {
+    launch_syrk_tc_small(a.phi, a.N, a.ld, V, a.mu, a.partial, a.ctrl, a.respect_done, st);
+    launch_syrk_reduce(a.partial, syrk_tc_small_nsplit(a.ld), V, a.N, a.Sigma, a.ctrl, a.respect_done, st);
     launch_cholesky(a.Sigma, a.Lc, V, a.ctrl, a.respect_done, st);
     return;
   }

@@ -89,6 +89,7 @@ struct CovCholArgs {
   float* Lc;         // [V][V]
   float* partial;    // split-K scratch, >= cov_partial_floats(V, N) floats
   float* tc_scratch; // >= syrk_tc_scratch_floats(V, ld) floats, or nullptr: FP32 SIMT syrk
+  int tc_small;      // V <= 128: 1 = tcgen05 syrk (syrk_tc_small.cu), 0 = FP32 SIMT reference
   Ctrl* ctrl;
   int respect_done;
 };
@@ -99,6 +100,11 @@ void launch_cholesky(const float* Sigma, float* Lc, int V, Ctrl* ctrl, int respe
 
 // syrk_tc.cu -- C1 for large V: centred 3xTF32 tcgen05 syrk with K split
 bool syrk_tc_supported(int V, int ld);
+// syrk_tc_small.cu -- C1 for V <= 128 on tcgen05 (3xTF32), one CTA per 128 particles
+bool syrk_tc_small_supported(int V, int ld);
+int syrk_tc_small_nsplit(int ld);
+void launch_syrk_tc_small(const float* phi, int N, int ld, int V, const float* mu, float* partial,
+                          const Ctrl* ctrl, int respect_done, cudaStream_t st);
 int syrk_tc_nsplit(int V, int ld);
 size_t syrk_tc_scratch_floats(int V, int ld);
 void launch_syrk_tc(const float* phi, int N, int ld, int V, const float* mu, float* Ps,
