@@ -252,13 +252,20 @@ int syrk_tc_nsplit(int V, int ld) {
   const int chains = nkc / (4 * sy::SUB_STAGES);            // K = 256 chains in the whole population
   int cap = ld / V;
   cap = cap < 1 ? 1 : cap > 64 ? 64 : cap;
-  int best = 1;
+  // best wave efficiency first, then the smallest count within 2 % of it (the partial tiles cost
+  // 4 V^2 bytes per split to write and to reduce)
   double best_eff = 0.0;
   for (int ns = 1; ns <= chains && ns <= cap; ++ns) {
     if (chains % ns) continue;
     const int items = tiles * ns, waves = (items + 147) / 148;
     const double eff = (double)items / (148.0 * waves);
-    if (eff > best_eff + 1e-9) { best_eff = eff; best = ns; }
+    if (eff > best_eff) best_eff = eff;
+  }
+  int best = 1;
+  for (int ns = 1; ns <= chains && ns <= cap; ++ns) {
+    if (chains % ns) continue;
+    const int items = tiles * ns, waves = (items + 147) / 148;
+    if ((double)items / (148.0 * waves) >= best_eff - 0.02) { best = ns; break; }
   }
   return best;
 }
