@@ -308,9 +308,21 @@ chol_small_kernel(const float* __restrict__ Sigma, float* __restrict__ Lc, int V
   for (int attempt = 0; attempt < 2; ++attempt) {
     const float add = attempt ? 1e-6f * (float)tr / (float)V : 0.f;
     if (tid == 0) failed_s = 0;
-    for (int idx = tid; idx < V * V; idx += blockDim.x) {
-      int x = idx / V, y = idx - x * V;
-      sm[x * P + y] = Sigma[idx] + (x == y ? add : 0.f);
+    // warp w: rows w, w + nw, ...; lanes along the row -- no index division, and the loads of a
+    // row batch (<= 5 x 32 columns, V <= 160) are all in flight before the first store
+    {
+      const int lane = tid & 31, w = tid >> 5, nw = blockDim.x >> 5;
+      for (int x = w; x < V; x += nw) {
+        const float* row = Sigma + (size_t)x * V;
+        float v[5];
+#pragma unroll
+        for (int j = 0; j < 5; ++j) v[j] = (lane + 32 * j < V) ? row[lane + 32 * j] : 0.f;
+#pragma unroll
+        for (int j = 0; j < 5; ++j) {
+          const int y = lane + 32 * j;
+          if (y < V) sm[x * P + y] = v[j] + (x == y ? add : 0.f);
+        }
+      }
     }
     __syncthreads();
     chol_panels(sm, P, V, &failed_s);
@@ -319,9 +331,10 @@ chol_small_kernel(const float* __restrict__ Sigma, float* __restrict__ Lc, int V
     if (!failed) { status = attempt; break; }
     status = -1;
   }
-  for (int idx = tid; idx < V * V; idx += blockDim.x) {
-    int x = idx / V, y = idx - x * V;
-    Lc[idx] = (y <= x) ? sm[x * P + y] : 0.f;
+  {
+    const int lane = tid & 31, w = tid >> 5, nw = blockDim.x >> 5;
+    for (int x = w; x < V; x += nw)
+      for (int y = lane; y < V; y += 32) Lc[(size_t)x * V + y] = (y <= x) ? sm[x * P + y] : 0.f;
   }
   if (tid == 0) { ctrl->chol_status = status; ctrl->chol_fail = 0; ctrl->trace = (float)tr; }
 }
