@@ -271,20 +271,39 @@ __device__ __forceinline__ void chol_panels(float* sm, int P, int V, int* failed
           if (jb + k < V) sm[r * P + jb + k] = x[k];
       }
       __syncthreads();
-      // ---- trailing update: A[r][c] -= sum_k l_rk l_ck for jb+8 <= c <= r < V
+      // ---- trailing update: A[r][c] -= sum_k l_rk l_ck for jb+8 <= c <= r < V, one 2 x 2 tile of
+      // the lower triangle per thread: its 36 shared-memory loads are independent and the four
+      // FMA chains interleave (a warp per row with one element per lane ran nine dependent
+      // load-FMA-store rounds per thread)
       const int j1 = jb + CS_NB;
       if (j1 < V) {
-        const int tx = tid & 31, ty = tid >> 5;
-        for (int rr = j1 + ty; rr < V; rr += (int)(blockDim.x >> 5)) {
-          float lr[CS_NB];
+        const int nt = (V - j1 + 1) >> 1, ntiles = nt * (nt + 1) / 2;
+        for (int t = tid; t < ntiles; t += (int)blockDim.x) {
+          int tr, tc;
+          tri_tile(t, tr, tc);
+          const int r0 = j1 + 2 * tr, c0 = j1 + 2 * tc;
+          const bool r1ok = r0 + 1 < V, c1ok = c0 + 1 < V;
+          const float* pr0 = sm + r0 * P + jb; const float* pr1 = sm + (r1ok ? r0 + 1 : r0) * P + jb;
+          const float* pc0 = sm + c0 * P + jb; const float* pc1 = sm + (c1ok ? c0 + 1 : c0) * P + jb;
+          float lr0[CS_NB], lr1[CS_NB], lc0[CS_NB], lc1[CS_NB];
 #pragma unroll
-          for (int k = 0; k < CS_NB; ++k) lr[k] = sm[rr * P + jb + k];
-          for (int cc = j1 + tx; cc <= rr; cc += 32) {
-            float acc = sm[rr * P + cc];
+          for (int k = 0; k < CS_NB; ++k) { lr0[k] = pr0[k]; lr1[k] = pr1[k]; lc0[k] = pc0[k]; lc1[k] = pc1[k]; }
+          float a00 = sm[r0 * P + c0], a01 = 0.f, a10 = 0.f, a11 = 0.f;
+          const bool e01 = c1ok && c0 + 1 <= r0, e10 = r1ok, e11 = r1ok && c1ok;
+          if (e01) a01 = sm[r0 * P + c0 + 1];
+          if (e10) a10 = sm[(r0 + 1) * P + c0];
+          if (e11) a11 = sm[(r0 + 1) * P + c0 + 1];
 #pragma unroll
-            for (int k = 0; k < CS_NB; ++k) acc = fmaf(-lr[k], sm[cc * P + jb + k], acc);
-            sm[rr * P + cc] = acc;
+          for (int k = 0; k < CS_NB; ++k) {
+            a00 = fmaf(-lr0[k], lc0[k], a00);
+            a01 = fmaf(-lr0[k], lc1[k], a01);
+            a10 = fmaf(-lr1[k], lc0[k], a10);
+            a11 = fmaf(-lr1[k], lc1[k], a11);
           }
+          sm[r0 * P + c0] = a00;
+          if (e01) sm[r0 * P + c0 + 1] = a01;
+          if (e10) sm[(r0 + 1) * P + c0] = a10;
+          if (e11) sm[(r0 + 1) * P + c0 + 1] = a11;
         }
       }
       __syncthreads();
