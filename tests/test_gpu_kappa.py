@@ -171,3 +171,32 @@ def test_smc_eq2_gaussian_closed_form():
     m, se = _mean_se(out)
     assert abs(m - want) < 3 * se + 0.01, (m, se, want)
     assert abs(m - logZ_gauss_kappa(4, 1.0, 2.0)) > 10 * se
+
+
+def test_smc_eq2_statistical_parity_12_seeds():
+    """Broken-phase Eq. 2 point (kappa = 0.8, lambda = 1.5) at L = 10, N = 4096, k = 20, ESS 0.5 -- the
+    fused tcgen05 kernel with kappa != 1 end to end: log Z, <|M|>, <M^2>, <S_E> and the schedule length
+    of 12 GPU runs against 12 oracle runs within 3 combined standard errors."""
+    L, N, k, n = 10, 4096, 20, 12
+    kin, m0sq, lam, _ = O.kl_to_eq1(KAPPA, LAM2)
+    g = []
+    for s in range(n):
+        h = B.smc_init_kl(L, KAPPA, LAM2, N, s)
+        B.smc_set_params(h, k_steps=k, ess_target=0.5)
+        T = B.smc_run(h)
+        g.append({"T": T, "logZ": B.log_Z(h), "obs": B.observables(h)})
+        h.close()
+    with O.kinetic(kin):
+        o = [O.smc_run(L, m0sq, lam, N, s, k, ess_target=0.5) for s in range(n)]
+    oobs = [O.observables(r["phi"], r["S"]) for r in o]
+    pairs = {"logZ": ([r["logZ"] for r in g], [r["logZ"] for r in o]),
+             "absM": ([r["obs"]["absM"] for r in g], [x["absM"] for x in oobs]),
+             "M2": ([r["obs"]["M2"] for r in g], [x["M2"] for x in oobs]),
+             "mean_SE": ([r["obs"]["mean_SE"] for r in g], [x["mean_SE"] for x in oobs])}
+    for key, (a, b) in pairs.items():
+        (ma, sa), (mb, sb) = _mean_se(a), _mean_se(b)
+        assert abs(ma - mb) < 3 * math.hypot(sa, sb) + 1e-6, (key, ma, sa, mb, sb)
+    assert abs(np.mean([r["T"] for r in g]) - np.mean([r["T"] for r in o])) < 1.0
+    # and it is not the kappa = 1 model: same seeds, Eq. 1 coefficients with kappa = 1
+    o1 = [O.smc_run(L, m0sq, lam, N, s, k, ess_target=0.5) for s in range(4)]
+    assert abs(np.mean([r["logZ"] for r in g]) - np.mean([r["logZ"] for r in o1])) > 1.0
