@@ -465,7 +465,11 @@ int orc_cov_chol(const double* phi, int N, int V, double* Sigma, double* Lc) {
  * O (reading A13): magnetisation observables with
  * optional log-weights logw (NULL = equal weights).
  * out[0]=<|M|>, out[1]=<M^2>, out[2]=chi=V(<M^2>-<|M|>^2), out[3]=<S_E>,
- * out[4]=mode balance (#M>0 / #M<0, zeros ignored; +inf if no negatives),
+ * out[4]=mode balance (positive over negative samples, zeros
+ *   ignored; +inf if no negatives, 0 if no positives).  With log-weights the
+ *   "number of samples" on a side is its weight mass (reading A19): an
+ *   unweighted count of nested-sampling dead points would describe the prior,
+ *   not the weighted sample the other outputs describe.
  * out[5..84] = 80-bin normalised weighted histogram of M on [-1.6, 1.6],
  * out-of-range values clamped into the end bins.
  * ---------------------------------------------------------------------- */
@@ -482,7 +486,7 @@ void orc_observables_from_M(const double* M, const double* S,
   double mx = -INFINITY;
   if (logw) for (int i = 0; i < N; ++i) if (logw[i] > mx) mx = logw[i];
   double W = 0.0, a = 0.0, m2 = 0.0, se = 0.0;
-  long npos = 0, nneg = 0;
+  double wpos = 0.0, wneg = 0.0;
   for (int b = 0; b < 85; ++b) out[b] = 0.0;
   for (int i = 0; i < N; ++i) {
     double wi = logw ? exp(logw[i] - mx) : 1.0;
@@ -490,7 +494,7 @@ void orc_observables_from_M(const double* M, const double* S,
     a += wi * fabs(M[i]);
     m2 += wi * M[i] * M[i];
     if (S) se += wi * S[i];
-    if (M[i] > 0.0) ++npos; else if (M[i] < 0.0) ++nneg;
+    if (M[i] > 0.0) wpos += wi; else if (M[i] < 0.0) wneg += wi;
     int b = (int)floor((M[i] + 1.6) / (3.2 / 80.0));
     if (b < 0) b = 0;
     if (b > 79) b = 79;
@@ -500,7 +504,7 @@ void orc_observables_from_M(const double* M, const double* S,
   out[1] = m2 / W;
   out[2] = (double)V * (out[1] - out[0] * out[0]);
   out[3] = se / W;
-  out[4] = nneg ? (double)npos / (double)nneg : INFINITY;
+  out[4] = wneg > 0.0 ? wpos / wneg : INFINITY;
   for (int b = 0; b < 80; ++b) out[5 + b] /= W;
 }
 

@@ -51,7 +51,7 @@ observables_reduce_kernel(const float* __restrict__ M, const float* __restrict__
     a += wi * fabs(m);
     m2 += wi * m * m;
     if (S) se += wi * (double)S[i];
-    if (m > 0.0) npos += 1.0; else if (m < 0.0) nneg += 1.0;
+    if (m > 0.0) npos += wi; else if (m < 0.0) nneg += wi;   // weight mass per side (reading A19)
     int b = (int)floor((m + 1.6) / (3.2 / 80.0));
     b = b < 0 ? 0 : (b > 79 ? 79 : b);
     atomicAdd(&hist[b], wi);
