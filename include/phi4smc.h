@@ -45,9 +45,15 @@ extern "C" {
 #define PHI4_ENOTPD (-3)  /* particle covariance not positive definite even after the jitter retry */
 #define PHI4_ENAN (-4)    /* a non-finite action or weight was produced                           */
 #define PHI4_ECUDA (-5)   /* a CUDA call failed or no device; see phi4_last_cuda_error()          */
+#define PHI4_ETRUNC (-6)  /* ns_step / ns_run: the dead-point log (max_iters) filled up before the
+                             stop rule fired.  Everything computed so far is valid, but log_Z()
+                             is the dead-point evidence only (no live-point term was added).     */
 
 #define PHI4_HIST_BINS 80 /* B = 80 bins; fixed range [-1.6, 1.6] (reading A13)     */
 #define PHI4_MAX_HOOK_STEPS 64 /* largest k accepted by smc_mutate when flags/margins are wanted  */
+#define PHI4_MAX_L 255    /* largest lattice side: several launches index sites by a grid
+                             dimension limited to 65535 (V = 65025); *_workspace_bytes returns 0
+                             and *_init PHI4_EINVAL beyond it                                    */
 
 typedef struct phi4smc phi4smc; /* opaque sampler handle (SMC or NS) */
 
@@ -105,7 +111,9 @@ typedef struct {
   double remaining_frac; /* X mean_live(e^-S) / (Z + X mean_live(e^-S))                          */
   int chol_status;
   int iter_index;
-  int done; /* 1 when remaining_frac < stop_frac; the live term has then been added to logZ      */
+  int done; /* 0 running; 1 remaining_frac < stop_frac: the live term has been added to logZ;
+             * 2 truncated: max_iters iterations were logged before the stop rule fired, logZ is
+             * the dead-point evidence only (ns_step / ns_run then return PHI4_ETRUNC)            */
 } ns_step_info;
 
 typedef struct {
@@ -113,7 +121,8 @@ typedef struct {
   double M2;           /* <M^2>                                                                  */
   double chi;          /* V (<M^2> - <|M|>^2)                                                    */
   double mean_SE;      /* <S_E>                                                                  */
-  double mode_balance; /* #(M>0) / #(M<0), zeros ignored, +inf if no negatives    */
+  double mode_balance; /* #(M>0) / #(M<0), zeros ignored, +inf if no negatives, 0 if no positives
+                        * (PAPER.md:293); NS: weight mass on each side (reading A19)             */
   double hist[PHI4_HIST_BINS]; /* normalised (weighted) histogram of M on [-1.6, 1.6]            */
 } phi4_observables;
 
@@ -126,7 +135,8 @@ uint64_t phi4_kernel_launches(void);
 
 /* ---------------------------------------------------------------- SMC-RW (PAPER.md:53(i)) ----
  * smc_workspace_bytes: bytes of device memory smc_init needs for an L x L lattice and N particles
- * (0 if L < 1 or N < 2).  Sized for 180 GB parts: C4 (L=64, N=131072) needs about 15 GB.          */
+ * (0 if L < 1, L > PHI4_MAX_L or N < 2).  Sized for 180 GB parts: C4 (L=64, N=131072) needs
+ * about 15 GB.  m0sq, lambda (and kappa) must be finite, else *_init returns PHI4_EINVAL.        */
 size_t smc_workspace_bytes(int L, int N);
 
 /* Creates an SMC sampler: particles phi_i ~ N(0,I) from Philox stream INIT, S_E and U0 evaluated,
@@ -199,12 +209,33 @@ int ns_init_kl(phi4smc** out, int L, float kappa, float lambda, int n_live, int 
 /* One iteration N1-N4.  info != NULL synchronises.  No-op once done.              */
 int ns_set_params(phi4smc* h, const ns_params* p); /* defaults: inner 0, width 1, 8, 32          */
 int ns_step(phi4smc* h, ns_step_info* info);
-int ns_run(phi4smc* h, int max_iters, int* n_iters); /* until done; synchronises                 */
+/* Until done or max_iters more iterations; synchronises.  PHI4_ETRUNC if the handle's dead-point
+ * log filled up first (see ns_step_info.done).                                                  */
+int ns_run(phi4smc* h, int max_iters, int* n_iters);
 
 /* ------------------------------------------------- test / checkpoint hooks (all synchronise) --
- * Needed for lockstep parity with the oracle; they also serve as checkpoint / resume, since the
- * RNG is counter-based: the whole sampler state is (phi, beta, logZ, step counter).
+ * Needed for lockstep parity with the oracle.  Checkpoint / resume: the RNG is counter-based, so
+ * the whole sampler state is the particles with their cached S_E, U0 (smc_get_state) plus the
+ * scalars of phi4_run_state (smc_get_run_state); smc_restore puts both back and the run then
+ * continues bit for bit as the uninterrupted one would (NS: add ns_get_dead / ns_set_dead).
  * Any output pointer may be NULL.  N below is the particle count (n_live for NS).               */
+typedef struct {
+  double beta;           /* SMC: current inverse temperature                                     */
+  double delta;          /* SMC: last increment (the starting point of the next ESS root solve)  */
+  double logZ;           /* SMC: running sum; NS: evidence of the dead points so far             */
+  double logX;           /* NS: log prior volume                                                 */
+  double S_star;         /* NS: last threshold                                                   */
+  double remaining_frac; /* NS                                                                   */
+  int32_t index;         /* transitions / iterations completed: keys the RESAMPLE, Z2 and NS
+                            start-point streams                                                  */
+  int32_t done;
+  uint64_t step_counter; /* mutation steps made: keys the PROP / ACC streams                     */
+} phi4_run_state;
+int smc_get_run_state(phi4smc* h, phi4_run_state* out);
+/* Replaces particles, cached actions and control scalars.  h_SE and h_U0 are either both given
+ * (taken as they are: a bit-exact resume) or both NULL (recomputed from h_phi).                 */
+int smc_restore(phi4smc* h, const float* h_phi, const float* h_SE, const float* h_U0,
+                const phi4_run_state* rs);
 int smc_get_state(phi4smc* h, float* h_phi, float* h_SE, float* h_U0, double* beta,
                   uint64_t* step_counter);
 /* Replaces the particles (S_E, U0 are recomputed on the device), beta and the step counter.      */
@@ -231,6 +262,9 @@ int smc_resample(phi4smc* h, const float* h_w, int32_t* h_ancestors);
  * log so far (S_E, M, log w per dead point; n_dead = iterations * k_delete).                     */
 int ns_get_dead(phi4smc* h, int32_t* h_last_dead_idx, float* h_dead_S, float* h_dead_M,
                 double* h_dead_logw, int cap, int* n_dead);
+/* Restores the first n_dead entries of the dead-point log (checkpoint / resume of observables). */
+int ns_set_dead(phi4smc* h, const float* h_dead_S, const float* h_dead_M,
+                const double* h_dead_logw, int n_dead);
 
 #ifdef __cplusplus
 }

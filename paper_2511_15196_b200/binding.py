@@ -16,7 +16,8 @@ HIST_BINS = 80
 MAX_HOOK_STEPS = 64
 
 ERRORS = {0: "PHI4_OK", -1: "PHI4_EINVAL", -2: "PHI4_ENOMEM", -3: "PHI4_ENOTPD", -4: "PHI4_ENAN",
-          -5: "PHI4_ECUDA"}
+          -5: "PHI4_ECUDA", -6: "PHI4_ETRUNC"}
+ETRUNC = -6
 
 
 class Phi4Error(RuntimeError):
@@ -50,6 +51,15 @@ class ns_step_info(C.Structure):
     _fields_ = [("logX", C.c_double), ("logZ", C.c_double), ("S_star", C.c_double),
                 ("accept_rate", C.c_double), ("remaining_frac", C.c_double),
                 ("chol_status", C.c_int), ("iter_index", C.c_int), ("done", C.c_int)]
+
+    def asdict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+class phi4_run_state(C.Structure):
+    _fields_ = [("beta", C.c_double), ("delta", C.c_double), ("logZ", C.c_double),
+                ("logX", C.c_double), ("S_star", C.c_double), ("remaining_frac", C.c_double),
+                ("index", C.c_int32), ("done", C.c_int32), ("step_counter", C.c_uint64)]
 
     def asdict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
@@ -101,6 +111,9 @@ SIGNATURES = {
     "smc_reweight": (_i, [_vp, _d, _vp, C.POINTER(smc_step_info)]),
     "smc_resample": (_i, [_vp, _vp, _vp]),
     "ns_get_dead": (_i, [_vp, _vp, _vp, _vp, _vp, _i, C.POINTER(_i)]),
+    "ns_set_dead": (_i, [_vp, _vp, _vp, _vp, _i]),
+    "smc_get_run_state": (_i, [_vp, C.POINTER(phi4_run_state)]),
+    "smc_restore": (_i, [_vp, _vp, _vp, _vp, C.POINTER(phi4_run_state)]),
 }
 
 _lib = None
@@ -288,17 +301,24 @@ def ns_set_params(h, inner=0, slice_width=1.0, max_expand=8, max_shrink=32):
 
 
 def ns_step(h, want_info=True):
+    """PHI4_ETRUNC (dead-point log full) is not raised: the info then carries done = 2."""
     if not want_info:
         h._check(load().ns_step(h.ptr, None), "ns_step")
         return None
     info = ns_step_info()
-    h._check(load().ns_step(h.ptr, C.byref(info)), "ns_step")
+    rc = load().ns_step(h.ptr, C.byref(info))
+    if rc != ETRUNC:
+        h._check(rc, "ns_step")
     return info.asdict()
 
 
 def ns_run(h, max_iters=4096):
+    """Returns the iterations made; h.truncated says whether the run ended with PHI4_ETRUNC."""
     n = C.c_int(0)
-    h._check(load().ns_run(h.ptr, max_iters, C.byref(n)), "ns_run")
+    rc = load().ns_run(h.ptr, max_iters, C.byref(n))
+    h.truncated = rc == ETRUNC
+    if rc != ETRUNC:
+        h._check(rc, "ns_run")
     return n.value
 
 
@@ -323,6 +343,27 @@ def smc_set_state(h, phi, beta, step):
     phi = np.ascontiguousarray(phi, np.float32)
     assert phi.shape == (h.V, h.N)
     h._check(load().smc_set_state(h.ptr, _np_ptr(phi), beta, step), "smc_set_state")
+
+
+def smc_get_run_state(h):
+    rs = phi4_run_state()
+    h._check(load().smc_get_run_state(h.ptr, C.byref(rs)), "smc_get_run_state")
+    return rs.asdict()
+
+
+def smc_restore(h, phi, S, U0, run_state):
+    phi = np.ascontiguousarray(phi, np.float32)
+    assert phi.shape == (h.V, h.N)
+    S = None if S is None else np.ascontiguousarray(S, np.float32)
+    U0 = None if U0 is None else np.ascontiguousarray(U0, np.float32)
+    rs = phi4_run_state(**run_state)
+    h._check(load().smc_restore(h.ptr, _np_ptr(phi), _np_ptr(S), _np_ptr(U0), C.byref(rs)), "smc_restore")
+
+
+def ns_set_dead(h, dead_S, dead_M, dead_logw):
+    dS, dM = np.ascontiguousarray(dead_S, np.float32), np.ascontiguousarray(dead_M, np.float32)
+    dW = np.ascontiguousarray(dead_logw, np.float64)
+    h._check(load().ns_set_dead(h.ptr, _np_ptr(dS), _np_ptr(dM), _np_ptr(dW), dS.size), "ns_set_dead")
 
 
 def smc_get_chol(h):

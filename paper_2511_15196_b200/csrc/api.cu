@@ -62,7 +62,9 @@ struct phi4smc {
   int32_t *dead, *surv, *start;
   // host side
   uint64_t step_counter;     // mutation steps enqueued so far (next step uses counter + 1)
+  uint64_t step_base;        // steps not counted by the device: set_state / restore base + hook steps
   uint32_t iters_enqueued;   // NS iterations enqueued
+  int64_t iter_base;         // NS: iters_enqueued - ctrl->temp_index after a set_state
   int known_done;
   Ctrl* h_ctrl;              // pinned staging
   Ctrl* h_poll;              // pinned, 2 slots: smc_run / ns_run poll one step behind the GPU
@@ -188,6 +190,7 @@ PHI4_API const char* phi4_strerror(int code) {
     case PHI4_ENOTPD: return "particle covariance not positive definite";
     case PHI4_ENAN: return "non-finite action or weight";
     case PHI4_ECUDA: return "CUDA error or no device";
+    case PHI4_ETRUNC: return "nested sampling stopped by max_iters: log_Z lacks the live-point term";
     default: return "unknown error";
   }
 }
@@ -205,7 +208,7 @@ static int init_failed(phi4smc* h, int rc) {
 PHI4_API const char* phi4_last_cuda_error(const phi4smc* h) { return h ? h->err : g_init_err; }
 
 PHI4_API size_t smc_workspace_bytes(int L, int N) {
-  if (L < 1 || N < 2 || L > 4096) return 0;
+  if (L < 1 || N < 2 || L > PHI4_MAX_L) return 0;
   phi4smc tmp;
   memset(&tmp, 0, sizeof(tmp));
   tmp.md.L = L; tmp.md.V = L * L; tmp.N = N; tmp.ld = round_up(N, 128); tmp.max_rec = MAX_RECORDS;
@@ -215,7 +218,8 @@ PHI4_API size_t smc_workspace_bytes(int L, int N) {
 }
 
 PHI4_API size_t ns_workspace_bytes(int L, int n_live, int k_delete, int max_iters) {
-  if (L < 1 || n_live < 2 || k_delete < 1 || k_delete >= n_live || max_iters < 1) return 0;
+  if (L < 1 || L > PHI4_MAX_L || n_live < 2 || k_delete < 1 || k_delete >= n_live || max_iters < 1)
+    return 0;
   phi4smc tmp;
   memset(&tmp, 0, sizeof(tmp));
   tmp.md.L = L; tmp.md.V = L * L; tmp.N = n_live; tmp.ld = round_up(n_live, 128);
@@ -256,6 +260,10 @@ static int sync_ctrl(phi4smc* h) {
   CU(cudaStreamSynchronize(h->st));
   CU(cudaGetLastError());
   if (h->h_ctrl->done) h->known_done = 1;
+  // the stream is idle: what the device counted is what ran (steps enqueued past the end of the
+  // run were no-ops and are not in these counts)
+  if (h->kind == KIND_SMC) h->step_counter = h->step_base + h->h_ctrl->mut_steps;
+  else h->iters_enqueued = (uint32_t)(h->iter_base + (int64_t)h->h_ctrl->temp_index);
   if (h->h_ctrl->nan_flag) return PHI4_ENAN;
   if (h->h_ctrl->chol_status < 0) return PHI4_ENOTPD;
   return PHI4_OK;
@@ -273,6 +281,7 @@ static int smc_init_impl(phi4smc** out, int L, float kappa, float m0sq, float la
                          void* cuda_stream) {
   if (!out) return PHI4_EINVAL;
   *out = nullptr;
+  if (!isfinite(kappa) || !isfinite(m0sq) || !isfinite(lambda)) return PHI4_EINVAL;
   size_t need = smc_workspace_bytes(L, N);
   if (need == 0 || !d_workspace || workspace_bytes < need ||
       (reinterpret_cast<uintptr_t>(d_workspace) % ALIGN) != 0)
@@ -315,7 +324,9 @@ PHI4_API int smc_reset(phi4smc* h, uint64_t seed) {
   h->seed = seed;
   h->cur = 0;
   h->step_counter = 0;
+  h->step_base = 0;
   h->iters_enqueued = 0;
+  h->iter_base = 0;
   h->known_done = 0;
   // h_ctrl is pinned staging that an earlier async copy may still be reading: use a memset for
   // the zero state and a tiny kernel-free patch for the NS evidence (-inf) via a second copy.
@@ -463,11 +474,16 @@ PHI4_API int smc_step(phi4smc* h, smc_step_info* info) {
   if (rc == PHI4_ECUDA) return rc;
   memset(info, 0, sizeof(*info));
   int last = h->h_ctrl->temp_index - 1;
-  if (last >= 0) {
+  if (last >= 0 && last < h->max_rec) {
     StepRecord r;
-    int rr = fetch_record(h, last < h->max_rec ? last : h->max_rec - 1, &r);
+    int rr = fetch_record(h, last, &r);
     if (rr != PHI4_OK) return rr;
     fill_info(r, info);
+  } else if (last >= 0) {
+    // the history is full: report the control block (accept_rate / n_unique are not kept there)
+    const Ctrl& c = *h->h_ctrl;
+    info->beta = c.beta; info->delta = c.delta; info->ess_frac = c.ess_frac; info->dlogZ = c.dlogZ;
+    info->logZ = c.logZ; info->chol_status = c.chol_status; info->temp_index = last;
   }
   info->done = h->h_ctrl->done ? 1 : 0;
   return rc;
@@ -504,9 +520,9 @@ PHI4_API int smc_run(phi4smc* h, int max_temps, int* n_temps) {
   const int start = h->h_ctrl->temp_index;
   int enq = 0;
   rc = run_pipelined(h, max_temps, &enq, enqueue_smc_step);
+  // (steps enqueued past beta = 1 were no-ops; sync_ctrl took the step counter from the device)
   const int made = h->h_ctrl->temp_index - start;
-  // steps enqueued past beta = 1 were no-ops: take them out of the step counter
-  if (enq > made) h->step_counter -= (uint64_t)(enq - made) * (uint64_t)h->prm.k_steps;
+  (void)enq;
   if (n_temps) *n_temps = made;
   return rc;
 }
@@ -588,6 +604,7 @@ static int ns_init_impl(phi4smc** out, int L, float kappa, float m0sq, float lam
   if (!out) return PHI4_EINVAL;
   *out = nullptr;
   if (n_live > 16384 || k_delete > 1024 || n_walk < 1 || !(stop_frac > 0.0)) return PHI4_EINVAL;
+  if (!isfinite(kappa) || !isfinite(m0sq) || !isfinite(lambda)) return PHI4_EINVAL;
   size_t need = ns_workspace_bytes(L, n_live, k_delete, max_iters);
   if (need == 0 || !d_workspace || workspace_bytes < need ||
       (reinterpret_cast<uintptr_t>(d_workspace) % ALIGN) != 0)
@@ -691,8 +708,8 @@ PHI4_API int ns_step(phi4smc* h, ns_step_info* info) {
     if (rr != PHI4_OK) return rr;
     fill_ns_info(r, info);
   }
-  info->done = h->h_ctrl->done ? 1 : 0;
-  return rc;
+  info->done = h->h_ctrl->done;                  // 0 running, 1 converged, 2 truncated
+  return (rc == PHI4_OK && h->h_ctrl->done == 2) ? PHI4_ETRUNC : rc;
 }
 
 PHI4_API int ns_run(phi4smc* h, int max_iters, int* n_iters) {
@@ -703,9 +720,9 @@ PHI4_API int ns_run(phi4smc* h, int max_iters, int* n_iters) {
   int enq = 0;
   rc = run_pipelined(h, max_iters, &enq, enqueue_ns_step);
   const int made = h->h_ctrl->temp_index - start;
-  if (enq > made) h->iters_enqueued -= (uint32_t)(enq - made);
+  (void)enq;
   if (n_iters) *n_iters = made;
-  return rc;
+  return (rc == PHI4_OK && h->h_ctrl->done == 2) ? PHI4_ETRUNC : rc;
 }
 
 PHI4_API int ns_get_dead(phi4smc* h, int32_t* h_last_dead_idx, float* h_dead_S, float* h_dead_M,
@@ -721,6 +738,19 @@ PHI4_API int ns_get_dead(phi4smc* h, int32_t* h_last_dead_idx, float* h_dead_S, 
   if (h_dead_S && m > 0) CU(cudaMemcpy(h_dead_S, h->dead_S, sizeof(float) * m, cudaMemcpyDeviceToHost));
   if (h_dead_M && m > 0) CU(cudaMemcpy(h_dead_M, h->dead_M, sizeof(float) * m, cudaMemcpyDeviceToHost));
   if (h_dead_logw && m > 0) CU(cudaMemcpy(h_dead_logw, h->dead_logw, sizeof(double) * m, cudaMemcpyDeviceToHost));
+  return PHI4_OK;
+}
+
+PHI4_API int ns_set_dead(phi4smc* h, const float* h_dead_S, const float* h_dead_M,
+                           const double* h_dead_logw, int n_dead) {
+  if (!h || h->kind != KIND_NS || n_dead < 0 || !h_dead_S || !h_dead_M || !h_dead_logw) return PHI4_EINVAL;
+  if ((size_t)n_dead > (size_t)h->max_iters * h->k_del) return PHI4_EINVAL;
+  CU(cudaStreamSynchronize(h->st));
+  if (n_dead > 0) {
+    CU(cudaMemcpy(h->dead_S, h_dead_S, sizeof(float) * n_dead, cudaMemcpyHostToDevice));
+    CU(cudaMemcpy(h->dead_M, h_dead_M, sizeof(float) * n_dead, cudaMemcpyHostToDevice));
+    CU(cudaMemcpy(h->dead_logw, h_dead_logw, sizeof(double) * n_dead, cudaMemcpyHostToDevice));
+  }
   return PHI4_OK;
 }
 
@@ -753,12 +783,69 @@ PHI4_API int smc_set_state(phi4smc* h, const float* h_phi, double beta, uint64_t
   h->h_ctrl->beta = beta;
   h->h_ctrl->done = (h->kind == KIND_SMC && beta >= 1.0) ? 1 : 0;
   h->h_ctrl->nan_flag = 0;
+  h->h_ctrl->mut_steps = 0;
   h->known_done = h->h_ctrl->done;
   rc = push_ctrl(h);
   if (rc != PHI4_OK) return rc;
   launch_action(h->phi[c], N, h->ld, h->md, h->S[c], h->U0[c], h->ctrl, h->st);
-  if (h->kind == KIND_SMC) h->step_counter = step_counter;
-  else h->iters_enqueued = (uint32_t)(step_counter / (uint64_t)h->n_walk);
+  if (h->kind == KIND_SMC) {
+    h->step_counter = h->step_base = step_counter;
+  } else {
+    h->iters_enqueued = (uint32_t)(step_counter / (uint64_t)h->n_walk);
+    h->iter_base = (int64_t)h->iters_enqueued - (int64_t)h->h_ctrl->temp_index;
+  }
+  CU(cudaStreamSynchronize(h->st));
+  CU(cudaGetLastError());
+  return PHI4_OK;
+}
+
+// Checkpoint / resume (bit for bit): the scalars of the control block that smc_get_state does not
+// return, and a restore that also takes the cached S_E / U0 (recomputing them would differ from
+// the incrementally updated values by fp32 rounding, and the weights are formed from them).
+PHI4_API int smc_get_run_state(phi4smc* h, phi4_run_state* out) {
+  if (!h || !out) return PHI4_EINVAL;
+  int rc = sync_ctrl(h);
+  if (rc == PHI4_ECUDA) return rc;
+  const Ctrl& c = *h->h_ctrl;
+  memset(out, 0, sizeof(*out));
+  out->beta = c.beta; out->delta = c.delta; out->logZ = c.logZ; out->logX = c.logX;
+  out->S_star = c.S_star; out->remaining_frac = c.remaining;
+  out->index = c.temp_index; out->done = c.done;
+  out->step_counter = h->kind == KIND_SMC ? h->step_counter
+                                          : (uint64_t)h->iters_enqueued * (uint64_t)h->n_walk;
+  return PHI4_OK;
+}
+
+PHI4_API int smc_restore(phi4smc* h, const float* h_phi, const float* h_SE, const float* h_U0,
+                           const phi4_run_state* rs) {
+  if (!h || !h_phi || !rs || rs->index < 0 || !(rs->beta >= 0.0 && rs->beta <= 1.0)) return PHI4_EINVAL;
+  if ((h_SE == nullptr) != (h_U0 == nullptr)) return PHI4_EINVAL;
+  int rc = sync_ctrl(h);
+  if (rc == PHI4_ECUDA) return rc;
+  const int V = h->md.V, N = h->N, c = h->cur;
+  CU(cudaMemcpy2DAsync(h->phi[c], sizeof(float) * h->ld, h_phi, sizeof(float) * N,
+                       sizeof(float) * N, V, cudaMemcpyHostToDevice, h->st));
+  Ctrl z;
+  memset(&z, 0, sizeof(z));
+  z.beta = rs->beta; z.delta = rs->delta; z.logZ = rs->logZ; z.logX = rs->logX;
+  z.S_star = rs->S_star; z.remaining = rs->remaining_frac; z.temp_index = rs->index;
+  z.done = rs->done;
+  *h->h_ctrl = z;
+  h->known_done = z.done ? 1 : 0;
+  rc = push_ctrl(h);
+  if (rc != PHI4_OK) return rc;
+  if (h_SE) {
+    CU(cudaMemcpyAsync(h->S[c], h_SE, sizeof(float) * N, cudaMemcpyHostToDevice, h->st));
+    CU(cudaMemcpyAsync(h->U0[c], h_U0, sizeof(float) * N, cudaMemcpyHostToDevice, h->st));
+  } else {
+    launch_action(h->phi[c], N, h->ld, h->md, h->S[c], h->U0[c], h->ctrl, h->st);
+  }
+  if (h->kind == KIND_SMC) {
+    h->step_counter = h->step_base = rs->step_counter;
+  } else {
+    h->iters_enqueued = (uint32_t)(rs->step_counter / (uint64_t)h->n_walk);
+    h->iter_base = (int64_t)h->iters_enqueued - (int64_t)rs->index;
+  }
   CU(cudaStreamSynchronize(h->st));
   CU(cudaGetLastError());
   return PHI4_OK;
@@ -801,6 +888,7 @@ PHI4_API int smc_mutate(phi4smc* h, int k, uint8_t* h_accept, float* h_margin) {
   enqueue_mutation(h, smc_mutate_args(h, k, want ? h->acc_flags : nullptr,
                                       want ? h->margins : nullptr, 0));
   h->step_counter += (uint64_t)k;
+  h->step_base += (uint64_t)k;
   const size_t n = (size_t)k * h->N;
   if (h_accept) CU(cudaMemcpyAsync(h_accept, h->acc_flags, n, cudaMemcpyDeviceToHost, h->st));
   if (h_margin) CU(cudaMemcpyAsync(h_margin, h->margins, n * sizeof(float), cudaMemcpyDeviceToHost, h->st));
@@ -820,6 +908,7 @@ PHI4_API int smc_time_mutation(phi4smc* h, int k, int reps, float* h_ms_per_call
   for (int r = 0; r < reps; ++r) {
     enqueue_mutation(h, smc_mutate_args(h, k, nullptr, nullptr, 0));
     h->step_counter += (uint64_t)k;
+    h->step_base += (uint64_t)k;
   }
   CU(cudaEventRecord(e1, h->st));
   launch_reset_counters(h->ctrl, h->st);

@@ -36,6 +36,7 @@ struct Ctrl {
   unsigned int n_accept;  // acceptances of the current mutation batch
   unsigned int n_unique;  // distinct ancestors of the last resampling
   unsigned long long q_total;  // T of reading R5
+  unsigned long long mut_steps;  // SMC: mutation steps of the transitions completed since init / reset / restore
 };
 
 // One record per temperature / iteration, written by the device at the end of each step.

@@ -63,14 +63,6 @@ __host__ __device__ inline Smem smem_layout(int V) {
 
 }  // namespace tc
 
-#ifdef PHI4_TC_TRACE
-// Debug build only (never defined by build.py): per-role clock64 stamps of CTA 0.
-__device__ long long g_tc_trace[3 * 4096];
-#define TC_TRACE(role, cnt) do { if (blockIdx.x == 0 && (cnt) < 4096) g_tc_trace[(role) * 4096 + (cnt)++] = clock64(); } while (0)
-#else
-#define TC_TRACE(role, cnt) do { } while (0)
-#endif
-
 struct TcParams {
   float* phi; float* S; float* U0;
   const float* Lsplit;         // [2][Kp/4][Vn][4]: s*Lc split hi/lo, UMMA K-major interleave layout
@@ -270,13 +262,10 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
       const uint64_t a_base = smem_desc(smem_u32(smem + lay.zring), CHUNK_BYTES, 128);
       int s = 0;
       uint32_t ph = 0;
-      int tr = 0; (void)tr;
       for (int t = 0; t < p.k; ++t) {
         const int buf = t & 1;
-        TC_TRACE(0, tr);
         mbar_wait(dempty(buf), ((t >> 1) & 1) ^ 1);
         tc_fence_after();
-        TC_TRACE(0, tr);
         const uint32_t dbase = taddr + (uint32_t)(buf * Vn);
         for (int it = 0; it < nit; ++it) {
           const KStep e0 = tab[2 * it];
@@ -284,7 +273,6 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
           const uint64_t a0 = a_base + (uint64_t)((uint32_t)s * (SLAB_BYTES >> 4));
           mbar_wait(zfull(s), ph);
           tc_fence_after();
-          TC_TRACE(0, tr);
           // the first K-step (xs = 0) overwrites all Vn columns; later ones accumulate
           tc_mma_tf32(dbase + e0.xs, a0 + (4 * CHUNK_BYTES >> 4), e0.b_hi, e0.idesc, it > 0);
           tc_mma_tf32(dbase + e0.xs, a0, e0.b_lo, e0.idesc, 1);
@@ -296,7 +284,6 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
             tc_mma_tf32(dbase + e1.xs, a1, e1.b_hi, e1.idesc, 1);
           }
           tc_commit(zempty(s));
-          TC_TRACE(0, tr);
           if (++s == STAGES) { s = 0; ph ^= 1; }
         }
         tc_commit(dfull(buf));
@@ -310,13 +297,11 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
     const int i = i0 + pr;
     const int nq = (V + 3) >> 2;
     uint8_t* zr = smem + lay.zring;
-    int tr = (j == 0) ? 0 : 4096; (void)tr;
     for (int t = 0; t < p.k; ++t) {
       const uint32_t tt = p.t0 + (uint32_t)t;
       // two ring stages (four Philox chains) per pass: the chains are independent, so their
       // latencies overlap inside the warp
       for (int it = 0; it < nitP; it += 2) {
-        TC_TRACE(1, tr);
         const bool second = it + 1 < nitP;
         U4 w[4];
         bool ok[4];
@@ -335,7 +320,6 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
             w[c] = philox4x32_10_rk((uint32_t)(4 * (nitE + it) + 2 * c + half), (uint32_t)i, tt, p.tag_prop, p.rk);
           w[2] = w[0]; w[3] = w[1];
         }
-        TC_TRACE(1, tr);
 #pragma unroll
         for (int st2 = 0; st2 < 2; ++st2) {
           if (st2 == 1 && !second) break;
@@ -367,8 +351,6 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
           __syncwarp();
           if (lane == 0) mbar_arrive_n(zfull(s), 2);         // 8 warps x 2 = the 16 expected
         }
-        TC_TRACE(1, tr);
-        TC_TRACE(1, tr);
       }
     }
   } else {
@@ -426,13 +408,10 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
     // step t + 1 then never wait for a warp that is itself waiting for the MMAs of step t
     fill(0);
     if (p.k > 1) fill(1);
-    int tr = (threadIdx.x == 0) ? 0 : 4096; (void)tr;
     for (int t = 0; t < p.k; ++t) {
       const int buf = t & 1;
-      TC_TRACE(2, tr);
       mbar_wait_relaxed(dfull(buf), (t >> 1) & 1);
       tc_fence_after();
-      TC_TRACE(2, tr);
       // pass 1: phi' = phi + d on this part's 16-column blocks (d carries the step scale s); two
       // TMEM loads in flight per wait
       for (int cb = 16 * g; cb < Vn; cb += 32 * EPI_PARTS) {
@@ -466,17 +445,13 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive(dempty(buf));
-      TC_TRACE(2, tr);
       named_bar_sync(1 + Q, 32 * EPI_PARTS);       // the whole proposal of these 32 particles is in smem
-      TC_TRACE(2, tr);
       // pass 2: per-site differences of Eq. 1 and U0 over this part's lattice rows
       float dS = 0.f, dU = 0.f;
       tc_stencil<LT>(cur, oth, g, L, hm, lam, kap, dS, dU);
       part[g * TILE + pr] = make_float2(dS, dU);
       if (g == 0) lus[pr] = log_uniform(p.seed, p.tag_acc, p.t0 + (uint32_t)t, (uint32_t)i);
-      TC_TRACE(2, tr);
       named_bar_sync(1 + Q, 32 * EPI_PARTS);
-      TC_TRACE(2, tr);
       // every part sums the four partials in the same order and takes the same decision (M4)
       dS = 0.f; dU = 0.f;
 #pragma unroll
@@ -528,12 +503,6 @@ bool mutate_tc_supported(int V) {
 }
 
 size_t mutate_tc_lsplit_floats(int V) { return 2 * tc::l_floats(V); }
-
-#ifdef PHI4_TC_TRACE
-extern "C" __attribute__((visibility("default"))) int phi4_debug_tc_trace(long long* out) {
-  return (int)cudaMemcpyFromSymbol(out, g_tc_trace, sizeof(long long) * 3 * 4096);
-}
-#endif
 
 // Packed hi / lo split of s*Lc with Vn rows (>= V, multiple of 16) and Kp columns (>= V, multiple
 // of 8); the lo part starts l_floats_vk(Vn, Kp) floats after the hi part.

@@ -2,9 +2,6 @@
 // incremental weights + log Z, exact integer systematic resampling, gather.
 #include "kernels.cuh"
 #include "philox.cuh"
-#ifdef PHI4_RW_TRACE
-#include <cstdio>
-#endif
 
 namespace phi4 {
 
@@ -177,9 +174,6 @@ __device__ __forceinline__ void next_delta_reweight_body(const float* __restrict
       delta = x;
       const int fl = bcast_flags;
       final_step = fl >> 1;
-#ifdef PHI4_RW_TRACE
-      if (threadIdx.x == 0) printf("rw it=%d x=%.9g stop=%d\n", it, x, fl);
-#endif
       if (fl & 1) break;
     }
   }
@@ -564,6 +558,7 @@ __global__ void finish_step_kernel(Ctrl* ctrl, StepRecord* rec, int max_rec, int
     rec[t] = r;
   }
   ctrl->temp_index = t + 1;
+  ctrl->mut_steps += (unsigned long long)k;   // steps enqueued past beta = 1 never get here
   ctrl->n_accept = 0u;
   ctrl->n_unique = 0u;
   if (ctrl->beta >= 1.0) ctrl->done = 1;

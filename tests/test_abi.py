@@ -39,6 +39,7 @@ def test_struct_sizes_match_header(lib):
     assert C.sizeof(B.smc_step_info) == 6 * 8 + 4 * 4
     assert C.sizeof(B.ns_step_info) == 56   # 5 doubles + 3 ints, padded to 8
     assert C.sizeof(B.phi4_observables) == (5 + 80) * 8
+    assert C.sizeof(B.phi4_run_state) == 6 * 8 + 2 * 4 + 8
 
 
 def test_workspace_sizes(lib):
