@@ -133,6 +133,22 @@ const char* phi4_last_cuda_error(const phi4smc* h);
 /* Diagnostic: number of CUDA kernels this library has launched in this process so far. */
 uint64_t phi4_kernel_launches(void);
 
+/* Measurement aid: the roofline denominators that MEASURED_PEAKS.json does not hold,
+ * measured on the current device with kernels that do nothing else: dense tcgen05 kind::tf32
+ * throughput (burst: best short launch; sustained: back-to-back launches for `seconds`, 0 < seconds
+ * <= 30), FP32 FMA and 32x32->64 integer multiply rates in 1e12 lane-operations per second.
+ * d_scratch: >= 4096 bytes of device memory (contents destroyed).  Synchronises.               */
+typedef struct {
+  double tf32_tflops_burst;
+  double tf32_tflops_sustained;
+  double ffma_tlaneops;       /* 1e12 FMA lane-operations / s (x2 for flop)                        */
+  double imad_wide_tlaneops;  /* 1e12 IMAD.WIDE + LOP3 pairs / s: the unit of a Philox round       */
+  int32_t sms;
+  int32_t reserved;
+} phi4_peaks;
+int phi4_measure_peaks(double seconds, phi4_peaks* out, void* d_scratch, size_t scratch_bytes,
+                       void* cuda_stream);
+
 /* ---------------------------------------------------------------- SMC-RW (PAPER.md:53(i)) ----
  * smc_workspace_bytes: bytes of device memory smc_init needs for an L x L lattice and N particles
  * (0 if L < 1, L > PHI4_MAX_L or N < 2).  Sized for 180 GB parts: C4 (L=64, N=131072) needs

@@ -65,6 +65,12 @@ class phi4_run_state(C.Structure):
         return {k: getattr(self, k) for k, _ in self._fields_}
 
 
+class phi4_peaks(C.Structure):
+    _fields_ = [("tf32_tflops_burst", C.c_double), ("tf32_tflops_sustained", C.c_double),
+                ("ffma_tlaneops", C.c_double), ("imad_wide_tlaneops", C.c_double),
+                ("sms", C.c_int32), ("reserved", C.c_int32)]
+
+
 class phi4_observables(C.Structure):
     _fields_ = [("absM", C.c_double), ("M2", C.c_double), ("chi", C.c_double),
                 ("mean_SE", C.c_double), ("mode_balance", C.c_double),
@@ -82,6 +88,7 @@ SIGNATURES = {
     "phi4_strerror": (C.c_char_p, [_i]),
     "phi4_last_cuda_error": (C.c_char_p, [_vp]),
     "phi4_kernel_launches": (_u64, []),
+    "phi4_measure_peaks": (_i, [_d, C.POINTER(phi4_peaks), _vp, _sz, _vp]),
     "smc_workspace_bytes": (_sz, [_i, _i]),
     "smc_init": (_i, [C.POINTER(_vp), _i, _f, _f, _i, _u64, _vp, _sz, _vp]),
     "smc_init_kl": (_i, [C.POINTER(_vp), _i, _f, _f, _i, _u64, _vp, _sz, _vp]),
@@ -182,6 +189,15 @@ def _aligned(ws):
 
 def phi4_kernel_launches():
     return load().phi4_kernel_launches()
+
+
+def phi4_measure_peaks(seconds=2.0, device="cuda:0"):
+    ws = _device_workspace(1 << 16, device)
+    out = phi4_peaks()
+    rc = load().phi4_measure_peaks(seconds, C.byref(out), C.c_void_p(_aligned(ws)), 1 << 16, _stream_ptr(device))
+    if rc != 0:
+        raise Phi4Error(rc, "phi4_measure_peaks")
+    return {k: getattr(out, k) for k, _ in phi4_peaks._fields_ if k != "reserved"}
 
 
 def smc_workspace_bytes(L, N):

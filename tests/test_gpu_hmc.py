@@ -51,6 +51,9 @@ def hmc_lockstep(L, N, k, beta, seed, eps, nfrog, m0sq=-4.0, lam=1.0, t_start=0,
     # a diverging trajectory (|g| beyond any acceptable energy error) amplifies rounding along the
     # way: relative 1e-3 there; the decision (reject) is exact either way
     d, go = np.abs(mar[valid] - omar[valid]), np.abs(omar[valid])
+    sane = go < 20.0
+    print("hmc L=%d N=%d: worst |dg| %.2e on |g| < 20 (band %.0e), valid fraction %.3f"
+          % (L, N, d[sane].max() if sane.any() else 0.0, BAND_HMC, valid.mean()))
     assert np.all(d < np.where(go < 20.0, 0.5 * BAND_HMC + 1e-5 * go, 1e-3 * go))
     clean = first == k
     assert np.abs(st1["phi"][:, clean] - p[:, clean]).max() < 1e-4

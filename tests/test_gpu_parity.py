@@ -128,7 +128,14 @@ def lockstep(L, N, k, beta, seed, m0sq=-4.0, lam=1.0, path=0, fields="init", t_s
     Sx, Ux, A = O.action_batch(st1["phi"].astype(np.float64), L, m0sq, lam, with_abs=True)
     # the cached S_E is updated incrementally (S += dS): relative 2e-5 of the action
     # scale plus an absolute floor for the fp32 rounding picked up along the k-step path
-    assert np.all(np.abs(st1["S"] - Sx) <= 2e-5 * A + 2e-5)
+    eS = np.abs(st1["S"] - Sx)
+    # measured worst cases (pytest -s; profiles/r02_parity_margins.md keeps the table): the floor
+    # matters only where 2e-5 A is itself ~1e-4 or less (L <= 2)
+    print("lockstep L=%d N=%d k=%d path=%d: worst |dg| %.2e, worst |S_cached - S| %.2e = %.2f of "
+          "(2e-5 A + 2e-5), %.2f of 2e-5 A alone"
+          % (L, N, k, path, np.abs(mar[valid] - omar[valid]).max(), eS.max(),
+             (eS / (2e-5 * A + 2e-5)).max(), (eS / np.maximum(2e-5 * A, 1e-300)).max()))
+    assert np.all(eS <= 2e-5 * A + 2e-5)
     assert np.all(np.abs(st1["U0"] - Ux) <= 2e-5 * Ux + 2e-5)
     rate = acc.mean()
     h.close()

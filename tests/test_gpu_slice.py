@@ -54,8 +54,12 @@ def test_slice_first_iteration_lockstep(L, n, kd, nw, width, mexp):
     p, S, U0, t, nexp, nshr, amb = O.slice_walk(f0, Ss, Us, L, m0sq, lam, Lc, info["S_star"], seed, 1,
                                                 nw, width=np.float32(width), m_expand=mexp)
     clean = amb.min(axis=0) > BAND_SLICE
-    assert clean.mean() > 0.6
     got = st1["phi"][:, dead]
+    same = np.abs(got - p).max(axis=0) < 1e-4
+    print("slice L=%d n=%d: clean fraction %.3f (walkers whose closest decision is > %.0e away), "
+          "walkers reproduced %.3f, worst field error on clean walkers %.2e"
+          % (L, n, clean.mean(), BAND_SLICE, same.mean(), np.abs(got[:, clean] - p[:, clean]).max()))
+    assert clean.mean() > 0.6
     assert np.abs(got[:, clean] - p[:, clean]).max() < 1e-4
     gS = st1["S"][dead]
     A = O.action_batch(p, L, m0sq, lam, with_abs=True)[2]
