@@ -9,11 +9,16 @@ configuration (default C1 = configs[1]: L=10, N=16384, k=20, ESS 0.5).  value = 
 executed) / time, summed over ranks.  The path does not shard ("replicas only"): with
 --gpus N every rank runs an independent replica with its own seed, no collective on the data path.
 
-One JSON line on stdout (rank 0).  --impl reference times the FP64 CPU oracle on the host cores.
+One JSON line on stdout (rank 0).  Besides the headline workload it carries
+  peaks_measured  dense tcgen05 kind::tf32, FP32 FMA and IMAD.WIDE rates measured in this run through
+                  phi4_measure_peaks (the roofline denominators MEASURED_PEAKS.json does not hold)
+  large_v         the same measurement on C3 and C4 (first --max-temps temperatures per step), where
+                  the rooflines mean something: the tcgen05 proposal GEMM against the TF32 peak and
+                  the population step against the HBM peak, with per-phase device times
+--impl reference times the FP64 CPU oracle on the host cores.
 """
 import argparse
 import json
-import math
 import os
 import sys
 import threading
@@ -26,9 +31,12 @@ ALU_OPS_PER_SITE_UPDATE = 40          # Philox ~20 int + Box-Muller
 # HMC: per site per leapfrog step: neighbour sum 3, 4a-nb 1, a^2 1, lam4*a^2+m0sq 1,
 # *a 1, + 1, beta*gs+a 1, kick 1, drift 1
 ALU_OPS_PER_LEAPFROG_SITE = 11
-# dram__bytes_read.sum + dram__bytes_write.sum of one mutation launch (profiles/, ncu --set full)
-# (C1: the fused kernel; C3 / C4: the proposal GEMM, the dominant kernel of the large-V step)
-NCU_DRAM_BYTES = {"C1": 6815744, "C3": 1127837175, "C4": 15380342000}
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, copied from the
+# committed `ncu --set full` captures (not measured by this run): C1 the fused mutation kernel,
+# C3 / C4 the proposal GEMM.
+NCU_TRAFFIC = {"C1": (6815744, "profiles/r01_mutate_tc_C1.md"),
+               "C3": (1127837175, "profiles/r01_large_V.md"),
+               "C4": (15380342000, "profiles/r01_large_V.md")}
 
 
 def peaks():
@@ -37,9 +45,9 @@ def peaks():
         d = json.load(open(p))
         return {"hbm_gbs": d["hbm_gbs"], "bf16_tflops": d["bf16_tflops"],
                 "bf16_tflops_sustained": d.get("bf16_tflops_sustained", d["bf16_tflops"]),
-                "sm_max_mhz": d.get("sm_max_mhz", 1965.0), "source": "measured"}
+                "sm_max_mhz": d.get("sm_max_mhz", 1965.0), "source": "MEASURED_PEAKS.json"}
     return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0,
-            "sm_max_mhz": 1965.0, "source": "fallback"}
+            "sm_max_mhz": 1965.0, "source": "fallback (B200_PROFILING.md)"}
 
 
 class ClockSampler(threading.Thread):
@@ -69,7 +77,9 @@ class ClockSampler(threading.Thread):
         except Exception as e:                      # pragma: no cover - depends on the box
             self.reasons.add("nvml_unavailable:%s" % type(e).__name__)
 
-    def result(self):
+    def finish(self):
+        self.stop_flag = True
+        self.join()
         s = sorted(self.samples)
         return {"sm_mhz": s[len(s) // 2] if s else None, "sm_max_mhz": self.max_mhz,
                 "reasons": sorted(self.reasons)}
@@ -100,14 +110,18 @@ def units_per_step(cfg):
     return cfg["hmc"][1] if cfg.get("hmc") else 1
 
 
+def default_max_temps(cfg, arg):
+    return arg if arg > 0 else (6 if cfg["L"] ** 2 >= 1024 else 4096)
+
+
 def run_reference(args, cfg):
     """--impl reference: the oracle as it stands, on the host cores, bounded sample per step."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     V = cfg["L"] ** 2
-    n_sample = min(cfg["N"], args.ref_particles if V < 1024 else 256)
-    max_temps = args.max_temps if args.max_temps > 0 else (6 if V >= 1024 else 4096)
+    n_sample = min(cfg["N"], args.ref_particles if V < 1024 else 128)
+    max_temps = args.max_temps if args.max_temps > 0 else (1 if V >= 1024 else 4096)
     for w in range(args.warmup):
         oracle_run(cfg, n_sample, 1000 + w, max_temps)
     tot_su, tot_t, Ts = 0, 0.0, []
@@ -117,12 +131,14 @@ def run_reference(args, cfg):
         tot_t += dt
         Ts.append(T)
     value = tot_su / tot_t
-    sample = "N=%d of %d particles, full adaptive tempering run to beta=1 per step" % (n_sample, cfg["N"])
+    sample = "N=%d of %d particles, %s per step" % (
+        n_sample, cfg["N"], "full adaptive tempering run to beta=1" if max_temps >= 4096
+        else "first %d temperature(s)" % max_temps)
     line = {"impl": "reference", "metric": "site-updates/s", "value": value, "unit": "site-updates/s",
             "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": 1e3 * tot_t / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": workload_config(args, cfg, temps=Ts),
+            "config": workload_config(args.workload, cfg, args.gpus, temps=Ts),
             "cpu_baseline": {"value": value, "unit": "site-updates/s", "cores": thr, "kind": "oracle",
                              "sample": sample},
             "e2e": {"value": value, "unit": "site-updates/s", "h2d_bytes_per_step": 0,
@@ -131,10 +147,10 @@ def run_reference(args, cfg):
     print(json.dumps(line))
 
 
-def workload_config(args, cfg, temps=None):
+def workload_config(name, cfg, gpus, temps=None, max_temps=None):
     c = {"workload": "%s: phi^4 L=%d (V=%d) m0sq=%g lambda=%g, N=%d particles from N(0,I), adaptive "
                      "tempering to beta=1 at ESS %.2f, %d %s per temperature, systematic resampling"
-                     % (args.workload, cfg["L"], cfg["L"] ** 2, cfg["m0sq"], cfg["lam"], cfg["N"],
+                     % (name, cfg["L"], cfg["L"] ** 2, cfg["m0sq"], cfg["lam"], cfg["N"],
                         cfg["ess"], cfg["k"],
                         "HMC transitions (%d leapfrog steps of %g, diagonal mass matrix; a site-update "
                         "is one site in one leapfrog step)" % (cfg["hmc"][1], cfg["hmc"][0])
@@ -142,14 +158,179 @@ def workload_config(args, cfg, temps=None):
                         "independent-MH steps from the fitted Gaussian N(mu, Sigma)" if cfg.get("irmh") else
                         "RW-Metropolis steps, dense VxV covariance-Cholesky proposal"),
          "L": cfg["L"], "V": cfg["L"] ** 2, "N": cfg["N"], "k_steps": cfg["k"], "ess_target": cfg["ess"],
-         "parallelism": "replicas x%d (no sharding)" % args.gpus,
+         "parallelism": "replicas x%d (no sharding)" % gpus,
          "l2": "flushed between timed steps (256 MiB write)"}
     if temps is not None:
         c["temperatures_per_step"] = temps
     if cfg["L"] ** 2 >= 1024:
-        c["note"] = "full schedule to beta=1 takes 100+ temperatures at this size: each step runs the first max_temps"
-
+        c["note"] = ("the full schedule to beta=1 takes 100+ temperatures at this size: a step runs the "
+                     "first %s temperatures" % (max_temps if max_temps else "max_temps"))
     return c
+
+
+def rooflines(name, cfg, ph, pk, mp, timed_region_s):
+    """Roofline records of the dominant mutation kernel and of the population step.
+    ph: per-phase device times in ms; pk: MEASURED_PEAKS.json; mp: phi4_measure_peaks of this run."""
+    L, N, k = cfg["L"], cfg["N"], cfg["k"]
+    V, upm = L * L, units_per_step(cfg)
+    mut_ms = ph["mutation_k_steps"]
+    traffic, tsrc = NCU_TRAFFIC.get(name, (None, None))
+    derived_alu = 148 * 128 * pk["sm_max_mhz"] * 1e6 / 1e12
+    if cfg.get("hmc") or V <= 112:
+        # plain-ALU bound (DESIGN.md 5.1 / 5.5): lane-ops, an FMA = 1
+        per = ALU_OPS_PER_LEAPFROG_SITE if cfg.get("hmc") else ALU_OPS_PER_SITE_UPDATE
+        work = per * float(N) * V * k * upm
+        achieved = work / (mut_ms * 1e-3) / 1e12
+        peak = mp["ffma_tlaneops"]
+        roof = {"bound": "alu", "kernel": ("hmc_kernel" if cfg.get("hmc") else "mutate_tc_kernel") +
+                " x%d steps, one launch" % k,
+                "achieved": achieved, "peak": peak, "unit": "T lane-op/s", "frac": achieved / peak,
+                "ops": "lane-ops (FMA = 1), %d per site-update" % per,
+                "peak_source": "phi4_measure_peaks FP32 FMA rate of this run (derived 148 SM x 128 lanes x "
+                               "%.0f MHz = %.1f; IMAD.WIDE rate %.1f)" % (pk["sm_max_mhz"], derived_alu,
+                                                                         mp["imad_wide_tlaneops"]),
+                "traffic": traffic if not cfg.get("hmc") else None,
+                "traffic_source": tsrc if not cfg.get("hmc") else None,
+                "site_updates_per_s": float(N) * V * k * upm / (mut_ms * 1e-3), "ms": mut_ms}
+    else:
+        # tensor bound (DESIGN.md 5.2): the proposal GEMM of ONE step, timed alone.  Algorithmic
+        # work: the triangular product in 3xTF32 split precision (north_star), 3 products x 2 flop x
+        # N V (V+1) / 2; the FP32-equivalent ("useful") flop are a third of that.
+        t = ph["proposal_gemm"] * 1e-3
+        issued = 3.0 * float(N) * V * (V + 1)
+        achieved = issued / t / 1e12
+        sustained = timed_region_s >= 0.25
+        peak = mp["tf32_tflops_sustained"] if sustained else mp["tf32_tflops_burst"]
+        roof = {"bound": "tensor", "kernel": "propose_tc_kernel, one launch = one mutation step",
+                "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+                "useful_frac": achieved / 3.0 / peak,
+                "ops": "TF32 flop of the triangular L*z in 3xTF32 split precision, 3 N V (V+1) per "
+                       "step; useful_frac counts the FP32-equivalent N V (V+1)",
+                "peak_source": "phi4_measure_peaks dense tcgen05 kind::tf32 of this run, %s (burst %.0f, "
+                               "sustained %.0f; bf16 x 1/2 would be %.0f)"
+                               % ("sustained: the launch was timed inside a >= 0.25 s region" if sustained
+                                  else "burst", mp["tf32_tflops_burst"], mp["tf32_tflops_sustained"],
+                                  0.5 * pk["bf16_tflops"]),
+                "traffic": traffic, "traffic_source": tsrc,
+                "site_updates_per_s": float(N) * V / t, "ms": ph["proposal_gemm"],
+                "mutation_step_ms": mut_ms / k}
+    pop_ms = ph["resample_gather"]
+    pop_bytes = 8.0 * N * V + 12.0 * N                 # 4 read + 4 written per site, 12 per particle
+    gat = 8.0 * N * V / (ph["gather"] * 1e-3) / 1e9
+    population = {"bound": "hbm", "kernel": "resample (scan, ancestors) + gather",
+                  "achieved": pop_bytes / (pop_ms * 1e-3) / 1e9, "peak": pk["hbm_gbs"], "unit": "GB/s",
+                  "frac": pop_bytes / (pop_ms * 1e-3) / 1e9 / pk["hbm_gbs"], "ms": pop_ms,
+                  "gather_alone": {"achieved": gat, "frac": gat / pk["hbm_gbs"], "ms": ph["gather"]},
+                  "peak_source": pk["source"], "state_in_l2": bool(8.0 * N * V < 126e6)}
+    return roof, population
+
+
+def measure_workload(name, cfg, args, env, steps, warmup, max_temps, want_e2e):
+    """Times `steps` whole runs of one workload on this rank; returns raw times and records."""
+    import torch
+    B, replicas, dev, rank, local, flush = (env[k] for k in ("B", "replicas", "dev", "rank", "local", "flush"))
+    L, N, k, V = cfg["L"], cfg["N"], cfg["k"], cfg["L"] ** 2
+    upm = units_per_step(cfg)
+    h = B.smc_init(L, cfg["m0sq"], cfg["lam"], N, 0, device=dev)
+    if cfg.get("hmc"):
+        B.smc_set_params(h, k_steps=k, ess_target=cfg["ess"], kernel=1, hmc_eps=cfg["hmc"][0],
+                         hmc_leapfrog=cfg["hmc"][1])
+    elif cfg.get("irmh"):
+        B.smc_set_params(h, k_steps=k, ess_target=cfg["ess"], kernel=2)
+    else:
+        B.smc_set_params(h, k_steps=k, ess_target=cfg["ess"], mutation_path=args.path)
+
+    def device_step(seed):
+        """inputs resident in HBM: particles are drawn on the device by the INIT Philox stream."""
+        flush.fill_(seed & 0xFF)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        B.smc_reset(h, seed)
+        T = B.smc_run(h, max_temps)
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1), T
+
+    for w in range(warmup):
+        device_step(replicas.replica_seed(1000 + w, rank))
+    env["barrier"]()
+    sampler = ClockSampler(local)
+    sampler.start()
+    l0 = B.phi4_kernel_launches()
+    ms, Ts = 0.0, []
+    for s in range(steps):
+        dt, T = device_step(replicas.replica_seed(s, rank))
+        ms += dt
+        Ts.append(T)
+    launches = B.phi4_kernel_launches() - l0
+    env["barrier"]()
+    clocks = sampler.finish()
+    out = {"ms": ms, "Ts": Ts, "launches": int(launches), "clocks": clocks,
+           "site_updates": float(N) * V * k * upm * sum(Ts), "logZ": B.log_Z(h)}
+
+    if want_e2e:
+        # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
+        h_in = torch.empty((V, N), dtype=torch.float32, pin_memory=True)
+        h_in.normal_(generator=torch.Generator().manual_seed(1234 + rank))
+        phi_in = h_in.numpy()
+        h_out = {"phi": torch.empty((V, N), dtype=torch.float32, pin_memory=True).numpy(),
+                 "S": torch.empty(N, dtype=torch.float32, pin_memory=True).numpy(),
+                 "U0": torch.empty(N, dtype=torch.float32, pin_memory=True).numpy()}
+
+        def e2e_step(seed):
+            flush.fill_(seed & 0xFF)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            B.smc_reset(h, seed)
+            B.smc_set_state(h, phi_in, 0.0, 0)            # H2D: V*N fp32 initial particles
+            T = B.smc_run(h, max_temps)
+            B.smc_get_state(h, out=h_out)                 # D2H: final particles, S_E, U0
+            B.log_Z(h)
+            torch.cuda.synchronize()
+            return (time.perf_counter() - t0) * 1e3, T
+
+        e2e_step(999)
+        e2e_ms, e2e_T = 0.0, []
+        env["barrier"]()
+        for s in range(steps):
+            dt, T = e2e_step(replicas.replica_seed(s, rank))
+            e2e_ms += dt
+            e2e_T.append(T)
+        env["barrier"]()
+        out["e2e_ms"] = e2e_ms
+        out["e2e_su"] = float(N) * V * k * upm * sum(e2e_T)
+
+    # ---- phases, timed alone at a mid-schedule state with CUDA events on the library's stream ----
+    B.smc_reset(h, 4242)
+    for _ in range(3):
+        B.smc_step(h, want_info=False)
+    torch.cuda.synchronize()
+    reps = 5
+    ph = {}
+    B.smc_time_phase(h, "mutation", 1)                         # warm
+    t0 = time.perf_counter()
+    ph["mutation_k_steps"] = B.smc_time_phase(h, "mutation", reps)
+    region_s = time.perf_counter() - t0
+    if V > 112 and not cfg.get("hmc") and not cfg.get("irmh") and args.path != 1:
+        for key, p in (("proposal_gemm", "proposal"), ("normals", "normals"), ("accept", "accept")):
+            B.smc_time_phase(h, p, 1)
+            t0 = time.perf_counter()
+            ph[key] = B.smc_time_phase(h, p, reps * 2)
+            if key == "proposal_gemm":
+                region_s = time.perf_counter() - t0
+    B.smc_reset(h, 4242)
+    for _ in range(3):
+        B.smc_step(h, want_info=False)
+    B.smc_reweight(h)                                          # weights at the ESS target
+    B.smc_resample(h)
+    ph["resample_gather"] = B.smc_time_phase(h, "resample", reps)
+    ph["gather"] = B.smc_time_phase(h, "gather", reps)
+    ph["cov_chol"] = B.smc_time_phase(h, "covchol", reps)
+    ph["reweight"] = B.smc_time_phase(h, "reweight", reps)
+    out["phases_ms"] = ph
+    out["phase_region_s"] = region_s
+    h.close()
+    return out
 
 
 def main():
@@ -171,6 +352,11 @@ def main():
     ap.add_argument("--max-temps", type=int, default=-1,
                     help="temperatures per step; -1: to beta=1 (C0-C2), 6 for C3/C4 whose full schedule "
                          "takes 100+ temperatures")
+    ap.add_argument("--large-v", default="C3,C4",
+                    help="workloads measured beside the headline one as `large_v` sub-records (1 GPU "
+                         "only); '' to skip")
+    ap.add_argument("--peak-seconds", type=float, default=2.0,
+                    help="length of the sustained tcgen05 TF32 peak measurement")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
 
@@ -188,7 +374,6 @@ def main():
         run_reference(args, cfg)
         return
 
-    import numpy as np
     import torch
     import torch.distributed as dist
     from paper_2511_15196_b200 import binding as B
@@ -207,174 +392,58 @@ def main():
         dist.barrier()
     B.load()
 
-    L, N, k, V = cfg["L"], cfg["N"], cfg["k"], cfg["L"] ** 2
-    max_temps = args.max_temps if args.max_temps > 0 else (6 if V >= 1024 else 4096)
-    h = B.smc_init(L, cfg["m0sq"], cfg["lam"], N, 0, device=dev)
-    upm = units_per_step(cfg)
-    if cfg.get("hmc"):
-        B.smc_set_params(h, k_steps=k, ess_target=cfg["ess"], kernel=1, hmc_eps=cfg["hmc"][0],
-                         hmc_leapfrog=cfg["hmc"][1])
-    elif cfg.get("irmh"):
-        B.smc_set_params(h, k_steps=k, ess_target=cfg["ess"], kernel=2)
-    else:
-        B.smc_set_params(h, k_steps=k, ess_target=cfg["ess"], mutation_path=args.path)
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
-
     def barrier():
         torch.cuda.synchronize()
         if world > 1:
             dist.barrier()
             torch.cuda.synchronize()
 
-    def device_step(seed):
-        """inputs resident in HBM: particles are drawn on the device by the INIT Philox stream."""
-        flush.fill_(seed & 0xFF)
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record()
-        B.smc_reset(h, seed)
-        T = B.smc_run(h, max_temps)
-        e1.record()
-        torch.cuda.synchronize()
-        return e0.elapsed_time(e1), T
+    env = {"B": B, "replicas": replicas, "dev": dev, "rank": rank, "local": local, "barrier": barrier,
+           "flush": torch.empty(256 << 20, dtype=torch.uint8, device=dev)}
+    pk = peaks()
+    mp = B.phi4_measure_peaks(args.peak_seconds, device=dev)      # every rank: keeps the ranks in step
 
-    # ---- device-resident timing -------------------------------------------------------------
-    for w in range(args.warmup):
-        device_step(replicas.replica_seed(1000 + w, rank))
-    barrier()
-    sampler = ClockSampler(local)
-    sampler.start()
-    l0 = B.phi4_kernel_launches()
-    ms, Ts = 0.0, []
-    for s in range(args.steps):
-        dt, T = device_step(replicas.replica_seed(s, rank))
-        ms += dt
-        Ts.append(T)
-    launches = B.phi4_kernel_launches() - l0
-    barrier()
-    sampler.stop_flag = True
-    sampler.join()
-    site_updates = float(N) * V * k * upm * sum(Ts)
-    logZ = B.log_Z(h)
-
-    # ---- end to end through the C ABI with HOST buffers ---------------------------------------
-    h_in = torch.empty((V, N), dtype=torch.float32, pin_memory=True)
-    h_in.normal_(generator=torch.Generator().manual_seed(1234 + rank))
-    phi_in = h_in.numpy()
-    # results land in pinned host memory too (pageable destinations are staged by the driver)
-    h_out = {"phi": torch.empty((V, N), dtype=torch.float32, pin_memory=True).numpy(),
-             "S": torch.empty(N, dtype=torch.float32, pin_memory=True).numpy(),
-             "U0": torch.empty(N, dtype=torch.float32, pin_memory=True).numpy()}
-
-    def e2e_step(seed):
-        flush.fill_(seed & 0xFF)
-        torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        B.smc_reset(h, seed)
-        B.smc_set_state(h, phi_in, 0.0, 0)            # H2D: V*N fp32 initial particles
-        T = B.smc_run(h, max_temps)
-        st = B.smc_get_state(h, out=h_out)            # D2H: final particles, S_E, U0
-        lz = B.log_Z(h)
-        torch.cuda.synchronize()
-        return (time.perf_counter() - t0) * 1e3, T, lz
-
-    e2e_step(999)
-    e2e_ms, e2e_T = 0.0, []
-    barrier()
-    for s in range(args.steps):
-        dt, T, _ = e2e_step(replicas.replica_seed(s, rank))
-        e2e_ms += dt
-        e2e_T.append(T)
-    barrier()
-    e2e_su = float(N) * V * k * upm * sum(e2e_T)
-
-    # ---- dominant kernel: the mutation, timed alone at a mid-schedule state -------------------
-    B.smc_reset(h, 4242)
-    for _ in range(3):
-        B.smc_step(h, want_info=False)
-    torch.cuda.synchronize()
-    for _ in range(2):
-        B.smc_mutate(h, k, want=False)
-    reps = 5
-    l1 = B.phi4_kernel_launches()
-    # CUDA events on the library's own stream around `reps` back-to-back k-step mutations
-    mut_ms = B.smc_time_mutation(h, k, reps)                  # k steps
-    mut_launches = (B.phi4_kernel_launches() - l1 - 2) // reps    # minus the two counter resets
-
-    # ---- population step: resample (integer scan, ancestors) + gather, device-resident weights ----
-    B.smc_reweight(h)                                          # weights at the ESS target
-    B.smc_resample(h)
-    pe0, pe1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    pe0.record()
-    for _ in range(reps):
-        B.smc_resample(h, want=False)                          # P3 + P4, nothing but the control block read back
-    pe1.record()
-    torch.cuda.synchronize()
-    pop_ms = pe0.elapsed_time(pe1) / reps
+    L, N, k, V = cfg["L"], cfg["N"], cfg["k"], cfg["L"] ** 2
+    max_temps = default_max_temps(cfg, args.max_temps)
+    m = measure_workload(args.workload, cfg, args, env, args.steps, args.warmup, max_temps, True)
 
     # ---- reduce over ranks: MAX of the times, SUM of the work (no data-path collective) ---------
-    tmax, usum = replicas.reduce_stats({"ms": ms, "e2e_ms": e2e_ms, "mut_ms": mut_ms, "pop_ms": pop_ms},
-                                       {"su": site_updates, "e2e_su": e2e_su}, device=dev)
-    ms, e2e_ms, mut_ms, pop_ms = tmax["ms"], tmax["e2e_ms"], tmax["mut_ms"], tmax["pop_ms"]
+    tmax, usum = replicas.reduce_stats({"ms": m["ms"], "e2e_ms": m["e2e_ms"]},
+                                       {"su": m["site_updates"], "e2e_su": m["e2e_su"]}, device=dev)
+    ms, e2e_ms = tmax["ms"], tmax["e2e_ms"]
     site_updates, e2e_su = usum["su"], usum["e2e_su"]
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
 
-    pk = peaks()
-    # Roofline of the dominant kernel, the fused mutation (DESIGN.md 5.1): plain-ALU bound; the
-    # algorithmic work is 40 lane-ops per site-update (Philox ~20, Box-Muller ~6, action ~14;
-    # SURVEY 8(d)); the proposal product rides on the tensor pipe.  Peak: 148 SM x 128 lanes x clock
-    # (an FMA counts as one lane-op).  traffic: dram bytes per launch from the committed ncu capture.
-    work = ALU_OPS_PER_SITE_UPDATE * float(N) * V * k
-    alu_peak = 148 * 128 * pk["sm_max_mhz"] * 1e6 / 1e12
-    achieved = work / (mut_ms * 1e-3) / 1e12
-    if cfg.get("hmc"):
-        work = ALU_OPS_PER_LEAPFROG_SITE * float(N) * V * k * upm
-        achieved = work / (mut_ms * 1e-3) / 1e12
-        roofline = {"bound": "alu", "kernel": "hmc_kernel x%d transitions (%d launches)" % (k, mut_launches),
-                    "achieved": achieved, "peak": alu_peak, "unit": "TFLOP/s", "frac": achieved / alu_peak,
-                    "ops": "lane-ops (FMA = 1), 11 per site per leapfrog step", "traffic": None,
-                    "peak_source": "derived: 148 SM x 128 lanes x %.0f MHz (%s clocks)"
-                    % (pk["sm_max_mhz"], pk["source"]),
-                    "site_updates_per_s": float(N) * V * k * upm / (mut_ms * 1e-3), "ms": mut_ms}
-    elif V <= 112:
-        roofline = {"bound": "alu", "kernel": "mutation x%d steps (%d launches)" % (k, mut_launches),
-                    "achieved": achieved, "peak": alu_peak, "unit": "TFLOP/s", "frac": achieved / alu_peak,
-                    "ops": "lane-ops (FMA = 1), 40 per site-update",
-                    "traffic": NCU_DRAM_BYTES.get(args.workload),
-                    "peak_source": "derived: 148 SM x 128 lanes x %.0f MHz (%s clocks)"
-                    % (pk["sm_max_mhz"], pk["source"]),
-                    "site_updates_per_s": float(N) * V * k / (mut_ms * 1e-3), "ms": mut_ms}
-    else:
-        # Large V (DESIGN.md 5.2): the mutation is the 3xTF32 tcgen05 proposal GEMM plus HBM-bound
-        # normals / accept kernels.  Algorithmic work = the triangular product, (V+1) flop per
-        # site-update in FP32-equivalent flop; every such flop costs three TF32 MMAs, so 1/3 is the
-        # ceiling of this fraction.  Peak: measured dense BF16 x 1/2 (nominal TF32 : BF16 ratio).
-        tf32_peak = 0.5 * pk["bf16_tflops"]
-        achieved = (V + 1) * float(N) * V * k / (mut_ms * 1e-3) / 1e12
-        roofline = {"bound": "tensor", "kernel": "mutation x%d steps (%d launches)" % (k, mut_launches),
-                    "achieved": achieved, "peak": tf32_peak, "unit": "TFLOP/s", "frac": achieved / tf32_peak,
-                    "ops": "FP32-equivalent flop of the triangular L*z, (V+1) per site-update; 3xTF32 "
-                           "issues 3 MMAs per flop (ceiling 1/3)",
-                    "traffic": NCU_DRAM_BYTES.get(args.workload),
-                    "peak_source": "%s bf16 %.0f TFLOP/s x 1/2" % (pk["source"], pk["bf16_tflops"]),
-                    "site_updates_per_s": float(N) * V * k / (mut_ms * 1e-3), "ms": mut_ms}
-    # Population step (P3 + P4): 8 bytes per site (4 read + 4 written) + 12 bytes per particle.
-    pop_bytes = 8.0 * N * V + 12.0 * N
-    population = {"bound": "hbm", "kernel": "resample + gather", "achieved": pop_bytes / (pop_ms * 1e-3) / 1e9,
-                  "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": pop_bytes / (pop_ms * 1e-3) / 1e9 / pk["hbm_gbs"],
-                  "ms": pop_ms, "state_in_l2": bool(8.0 * N * V < 126e6),
-                  "note": "integer CDF scan + ancestor search + gather, one control-block readback per call"}
+    roof, population = rooflines(args.workload, cfg, m["phases_ms"], pk, mp, m["phase_region_s"])
+
+    # ---- large-V sub-records: where the rooflines mean something ------------------
+    large = {}
+    if world == 1 and args.kernel == "rw" and args.large_v:
+        for name in [x for x in args.large_v.split(",") if x and x != args.workload]:
+            c = dict(inputs.CONFIGS[name])
+            mt = default_max_temps(c, args.max_temps)
+            st, wu = (3, 3) if c["L"] >= 64 else (5, 3)
+            r = measure_workload(name, c, args, env, st, wu, mt, False)
+            rf, pop = rooflines(name, c, r["phases_ms"], pk, mp, r["phase_region_s"])
+            large[name] = {"config": workload_config(name, c, 1, temps=r["Ts"], max_temps=mt),
+                           "steps": st, "warmup": wu, "ms_per_step": r["ms"] / st,
+                           "value": r["site_updates"] / (r["ms"] * 1e-3), "unit": "site-updates/s",
+                           "ms_per_temperature": r["ms"] / max(1, sum(r["Ts"])),
+                           "gpu_launches": r["launches"], "clocks": r["clocks"], "roofline": rf,
+                           "population_step": pop, "phases_ms": r["phases_ms"]}
 
     cpu = None
     if not args.no_cpu_baseline:
         # the oracle as it stands on the host cores: full runs of the same workload until ~10 s of
         # CPU work (large lattices: a reduced population, the per-particle work is independent)
-        n_s = min(N, args.ref_particles if V < 1024 else 256)
+        n_s = min(N, args.ref_particles if V < 1024 else 128)
+        mt = max_temps if V < 1024 else 1
         su_tot, dt_tot, runs, T, thr = 0.0, 0.0, 0, 0, 1
         while dt_tot < 10.0 and runs < 12:
-            su, dt, T, thr = oracle_run(cfg, n_s, runs, max_temps)
+            su, dt, T, thr = oracle_run(cfg, n_s, runs, mt)
             su_tot += su
             dt_tot += dt
             runs += 1
@@ -385,13 +454,22 @@ def main():
     line = {"metric": "site-updates/s", "value": site_updates / (ms * 1e-3), "unit": "site-updates/s",
             "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
-            "data": "synthetic", "config": workload_config(args, cfg, temps=Ts),
-            "smc_wall_clock_ms_to_beta1": ms / args.steps, "logZ_last": logZ,
+            "data": "synthetic",
+            "config": workload_config(args.workload, cfg, world, temps=m["Ts"], max_temps=max_temps),
+            "smc_wall_clock_ms_to_beta1": ms / args.steps if max_temps >= 4096 else None,
+            "logZ_last": m["logZ"],
             "e2e": {"value": e2e_su / (e2e_ms * 1e-3), "unit": "site-updates/s",
                     "h2d_bytes_per_step": V * N * 4, "d2h_bytes_per_step": V * N * 4 + 8 * N + 8,
                     "ms_per_step": e2e_ms / args.steps},
-            "gpu_launches": int(launches), "clocks": sampler.result(), "roofline": roofline,
-            "population_step": population, "cpu_baseline": cpu}
+            "gpu_launches": m["launches"], "clocks": m["clocks"], "roofline": roof,
+            "population_step": population, "phases_ms": m["phases_ms"],
+            "peaks_measured": dict(mp, hbm_gbs=pk["hbm_gbs"], bf16_tflops=pk["bf16_tflops"],
+                                   hbm_bf16_source=pk["source"],
+                                   how="phi4_measure_peaks (csrc/measure.cu): dense tcgen05 kind::tf32 "
+                                       "M128 N256 K8 from resident smem operands on all SMs, burst = best "
+                                       "of 5 launches, sustained = back to back for %.1f s; FP32 FMA and "
+                                       "IMAD.WIDE+LOP3: 8 chains/thread, 2048 threads/SM" % args.peak_seconds),
+            "large_v": large, "cpu_baseline": cpu}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

@@ -270,6 +270,20 @@ int smc_mutate(phi4smc* h, int k, uint8_t* h_accept, float* h_margin);
  * flags, no host synchronisation in between) bracketed by CUDA events on the handle's stream and
  * returns the average device time of one k-step mutation in milliseconds.                        */
 int smc_time_mutation(phi4smc* h, int k, int reps, float* h_ms_per_call);
+/* Measurement hook: one phase of the step, `reps` times back to back between two CUDA events on
+ * the handle's stream; returns the average device time of one call in milliseconds.  Phases 1-3
+ * exist only where a mutation step is three kernels (L*L > 112, mutation_path != 1).  The state
+ * afterwards is valid but meaningless (e.g. a resampling without its reweighting): smc_reset or
+ * smc_restore before using the handle for anything else.  PHASE_REWEIGHT advances beta.       */
+#define PHI4_PHASE_MUTATION 0 /* k_steps x (M1-M4), as smc_step enqueues them                  */
+#define PHI4_PHASE_PROPOSAL 1 /* M2: the tcgen05 proposal GEMM of one step, operands in place  */
+#define PHI4_PHASE_NORMALS 2  /* M1: the normals of one step                                   */
+#define PHI4_PHASE_ACCEPT 3   /* M3 + M4: action differences, decision, commit of one step     */
+#define PHI4_PHASE_RESAMPLE 4 /* P3 + P4: integer scan, ancestors, gather                      */
+#define PHI4_PHASE_GATHER 5   /* P4 alone (with the ancestors of the last resampling)          */
+#define PHI4_PHASE_COVCHOL 6  /* C1 + C2                                                       */
+#define PHI4_PHASE_REWEIGHT 7 /* P1 + P2                                                       */
+int smc_time_phase(phi4smc* h, int phase, int reps, float* h_ms_per_call);
 int smc_reweight(phi4smc* h, double delta, float* h_w, smc_step_info* info);
 /* P3+P4: systematic resampling of the device weights (or of h_w if non-NULL) with the Philox
  * offset of the current temperature index, then the gather.  h_ancestors receives a_j.           */

@@ -115,6 +115,7 @@ SIGNATURES = {
     "smc_get_mean": (_i, [_vp, _vp]),
     "smc_mutate": (_i, [_vp, _i, _vp, _vp]),
     "smc_time_mutation": (_i, [_vp, _i, _i, C.POINTER(_f)]),
+    "smc_time_phase": (_i, [_vp, _i, _i, C.POINTER(_f)]),
     "smc_reweight": (_i, [_vp, _d, _vp, C.POINTER(smc_step_info)]),
     "smc_resample": (_i, [_vp, _vp, _vp]),
     "ns_get_dead": (_i, [_vp, _vp, _vp, _vp, _vp, _i, C.POINTER(_i)]),
@@ -416,6 +417,16 @@ def smc_mutate(h, k, want=True):
 def smc_time_mutation(h, k, reps=5):
     ms = C.c_float(0.0)
     h._check(load().smc_time_mutation(h.ptr, k, reps, C.byref(ms)), "smc_time_mutation")
+    return ms.value
+
+
+PHASES = {"mutation": 0, "proposal": 1, "normals": 2, "accept": 3, "resample": 4, "gather": 5,
+          "covchol": 6, "reweight": 7}
+
+
+def smc_time_phase(h, phase, reps=5):
+    ms = C.c_float(0.0)
+    h._check(load().smc_time_phase(h.ptr, PHASES[phase], reps, C.byref(ms)), "smc_time_phase")
     return ms.value
 
 

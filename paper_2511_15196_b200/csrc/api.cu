@@ -922,6 +922,73 @@ PHI4_API int smc_time_mutation(phi4smc* h, int k, int reps, float* h_ms_per_call
   return PHI4_OK;
 }
 
+// Measurement hook: one phase of the step, `reps` times back to back between two CUDA events on
+// the handle's stream.  The state it leaves behind is valid but not meaningful (a proposal that
+// was never accepted, a resampling without its reweighting): reset or restore afterwards.
+PHI4_API int smc_time_phase(phi4smc* h, int phase, int reps, float* h_ms_per_call) {
+  if (!h || h->kind != KIND_SMC || reps < 1 || !h_ms_per_call) return PHI4_EINVAL;
+  const int V = h->md.V;
+  const bool large = use_tc_propose(h) && !use_tc_path(h);
+  if ((phase == PHI4_PHASE_PROPOSAL || phase == PHI4_PHASE_NORMALS || phase == PHI4_PHASE_ACCEPT) && !large)
+    return PHI4_EINVAL;
+  if (phase < 0 || phase > PHI4_PHASE_REWEIGHT) return PHI4_EINVAL;
+  cudaEvent_t e0, e1;
+  CU(cudaEventCreate(&e0));
+  CU(cudaEventCreate(&e1));
+  launch_reset_counters(h->ctrl, h->st);
+  MutateArgs a = smc_mutate_args(h, h->prm.k_steps, nullptr, nullptr, 0);
+  if (phase == PHI4_PHASE_PROPOSAL || phase == PHI4_PHASE_ACCEPT) {
+    // operands of a real step: the factor split and one set of normals, one proposal
+    launch_propose_lsplit(a.Lc, V, a.ld, a.s, h->Lsplit, a.ctrl, 0, h->st);
+    launch_normals_split(a.Z, a.N, a.ld, V, a.seed, a.tag_prop, a.t0, a.ctrl, 0, h->st);
+    launch_propose_tc(a.phi, a.phip, a.Z, h->Lsplit, a.ld, V, a.ctrl, 0, h->st);
+  }
+  CU(cudaEventRecord(e0, h->st));
+  for (int r = 0; r < reps; ++r) {
+    switch (phase) {
+      case PHI4_PHASE_MUTATION:
+        enqueue_mutation(h, smc_mutate_args(h, h->prm.k_steps, nullptr, nullptr, 0));
+        h->step_counter += (uint64_t)h->prm.k_steps;
+        h->step_base += (uint64_t)h->prm.k_steps;
+        break;
+      case PHI4_PHASE_PROPOSAL:
+        launch_propose_tc(a.phi, a.phip, a.Z, h->Lsplit, a.ld, V, a.ctrl, 0, h->st);
+        break;
+      case PHI4_PHASE_NORMALS:
+        launch_normals_split(a.Z, a.N, a.ld, V, a.seed, a.tag_prop, a.t0 + (uint32_t)r, a.ctrl, 0, h->st);
+        break;
+      case PHI4_PHASE_ACCEPT:
+        launch_accept_step(a, 0, h->st);
+        break;
+      case PHI4_PHASE_RESAMPLE:
+        enqueue_resample(h);
+        break;
+      case PHI4_PHASE_GATHER: {
+        const int o = h->cur ^ 1;
+        launch_gather(h->phi[h->cur], h->phi[o], h->S[h->cur], h->S[o], h->U0[h->cur], h->U0[o], h->anc,
+                      nullptr, h->N, h->ld, V, h->ctrl, h->st);
+        break;
+      }
+      case PHI4_PHASE_COVCHOL:
+        launch_cov_chol(cov_args(h, 0), h->st);
+        break;
+      default:   // PHI4_PHASE_REWEIGHT: P1 + P2 at the current beta (beta is put back below)
+        launch_next_delta_reweight(h->S[h->cur], h->N, h->prm.ess_target, -1.0, h->w, nullptr, h->ctrl, h->st);
+        break;
+    }
+  }
+  CU(cudaEventRecord(e1, h->st));
+  launch_reset_counters(h->ctrl, h->st);
+  CU(cudaStreamSynchronize(h->st));
+  float ms = 0.f;
+  CU(cudaEventElapsedTime(&ms, e0, e1));
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  CU(cudaGetLastError());
+  *h_ms_per_call = ms / (float)reps;
+  return PHI4_OK;
+}
+
 PHI4_API int smc_reweight(phi4smc* h, double delta, float* h_w, smc_step_info* info) {
   if (!h || h->kind != KIND_SMC) return PHI4_EINVAL;
   launch_next_delta_reweight(h->S[h->cur], h->N, h->prm.ess_target, delta < 0.0 ? -1.0 : delta,

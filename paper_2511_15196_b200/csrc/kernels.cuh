@@ -43,6 +43,7 @@ struct MutateArgs {
   cudaEvent_t fork_ev, join_ev;
 };
 void launch_mutate_generic(const MutateArgs& a, float* Lsplit, cudaStream_t st);
+void launch_accept_step(const MutateArgs& a, int j, cudaStream_t st);
 // NEXT f3: k constrained slice-sampling steps of the NS walkers (reading A16); a.phip = direction
 void launch_ns_slice(const MutateArgs& a, float width, int m_expand, int max_shrink, cudaStream_t st);
 // NEXT f2: k independent-MH steps from N(mu, Lc Lc^T) (reading A15); W2 [ld] scratch

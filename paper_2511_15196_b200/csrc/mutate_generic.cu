@@ -254,14 +254,33 @@ accept_kernel(float* __restrict__ phi, const float* __restrict__ phip, float* __
   }
 }
 
-// Lsplit != nullptr selects the tcgen05 proposal (propose_tc.cu) for M1 + M2; a.Z must then hold
-// 2 V ld floats.  The accept / commit step is the same either way.
-void launch_mutate_generic(const MutateArgs& a, float* Lsplit, cudaStream_t st) {
-  const int V = a.md.V;
+// M3 + M4 of step j (step counter a.t0 + j): action differences between a.phip and a.phi,
+// decision, commit.
+void launch_accept_step(const MutateArgs& a, int j, cudaStream_t st) {
+  const uint32_t t = a.t0 + (uint32_t)j;
   // fewer than two 8-warp blocks per SM and more than 8 lattice rows: one warp per row instead
   const bool wide = a.md.L > 8 && a.ld / 32 < 2 * 148;
   // large populations: column walk over bands of <= 4 lattice rows (8, 16 or 32 row groups)
   const bool colwalk = !wide && a.ld >= 8192 && a.md.L >= 25 && a.md.L <= 128;
+  ++g_launches;
+  auto launch_accept = [&](auto kern, int G) {
+    launch_pdl(kern, a.ld / 32, 32 * G, 0, st,
+               a.phi, a.phip, a.S, a.U0, a.N, a.ld, a.md, a.mode, a.seed, a.tag_acc, t, a.ctrl,
+               a.acc_out ? a.acc_out + (size_t)j * a.N : nullptr,
+               a.margin_out ? a.margin_out + (size_t)j * a.N : nullptr, a.respect_done,
+               (const float*)nullptr, (float*)nullptr);
+  };
+  if (wide) launch_accept(accept_kernel<false, 32, 0>, 32);
+  else if (colwalk && a.md.L <= 32) launch_accept(accept_kernel<false, 8, 4>, 8);
+  else if (colwalk && a.md.L <= 64) launch_accept(accept_kernel<false, 16, 4>, 16);
+  else if (colwalk) launch_accept(accept_kernel<false, 32, 4>, 32);
+  else launch_accept(accept_kernel<false, 8, 0>, 8);
+}
+
+// Lsplit != nullptr selects the tcgen05 proposal (propose_tc.cu) for M1 + M2; a.Z must then hold
+// 2 V ld floats.  The accept / commit step is the same either way.
+void launch_mutate_generic(const MutateArgs& a, float* Lsplit, cudaStream_t st) {
+  const int V = a.md.V;
   dim3 gz((a.ld + 127) / 128, (V + 3) / 4);
   dim3 gp(a.ld / 64, (V + 63) / 64);
   if (Lsplit) {
@@ -299,19 +318,7 @@ void launch_mutate_generic(const MutateArgs& a, float* Lsplit, cudaStream_t st) 
       ++g_launches; propose_kernel<<<gp, 256, 0, st>>>(a.Lc, a.Z, a.phi, a.phip, V, a.ld, a.s, nullptr,
                                          0, a.ctrl, a.respect_done);
     }
-    ++g_launches;
-    auto launch_accept = [&](auto kern, int G) {
-      launch_pdl(kern, a.ld / 32, 32 * G, 0, st,
-                 a.phi, a.phip, a.S, a.U0, a.N, a.ld, a.md, a.mode, a.seed, a.tag_acc, t, a.ctrl,
-                 a.acc_out ? a.acc_out + (size_t)j * a.N : nullptr,
-                 a.margin_out ? a.margin_out + (size_t)j * a.N : nullptr, a.respect_done,
-                 (const float*)nullptr, (float*)nullptr);
-    };
-    if (wide) launch_accept(accept_kernel<false, 32, 0>, 32);
-    else if (colwalk && a.md.L <= 32) launch_accept(accept_kernel<false, 8, 4>, 8);
-    else if (colwalk && a.md.L <= 64) launch_accept(accept_kernel<false, 16, 4>, 16);
-    else if (colwalk) launch_accept(accept_kernel<false, 32, 4>, 32);
-    else launch_accept(accept_kernel<false, 8, 0>, 8);
+    launch_accept_step(a, j, st);
   }
 }
 
