@@ -51,6 +51,7 @@ extern "C" {
 
 #define PHI4_HIST_BINS 80 /* B = 80 bins; fixed range [-1.6, 1.6] (reading A13)     */
 #define PHI4_MAX_HOOK_STEPS 64 /* largest k accepted by smc_mutate when flags/margins are wanted  */
+#define PHI4_NS_MAX_LIVE (1 << 20) /* nested sampling: largest n_live (k_delete: any value < n_live) */
 #define PHI4_MAX_L 255    /* largest lattice side: several launches index sites by a grid
                              dimension limited to 65535 (V = 65025); *_workspace_bytes returns 0
                              and *_init PHI4_EINVAL beyond it                                    */
@@ -214,7 +215,9 @@ size_t ns_workspace_bytes(int L, int n_live, int k_delete, int max_iters);
  * points are deleted and each replaced by an n_walk-step covariance-preconditioned constrained
  * walk (accept iff S_E' < S_star and log u < -dU0, reading A5).  stop_frac: remaining-evidence
  * fraction at which the run ends (BASELINE configs: 1e-3).  max_iters bounds the dead-point log.
- * Requires 2 <= n_live <= 16384 and 1 <= k_delete < n_live.                                      */
+ * Requires 2 <= n_live <= PHI4_NS_MAX_LIVE and 1 <= k_delete < n_live (the paper's own setting,
+ * N = 5000 with delete fraction 0.5, is ns_init(.., 5000, 2500, ..)); up to
+ * 16384 live points are ordered by one CTA in shared memory, more by a multi-block network.      */
 int ns_init(phi4smc** out, int L, float m0sq, float lambda, int n_live, int k_delete, int n_walk,
             uint64_t seed, double stop_frac, int max_iters, void* d_workspace,
             size_t workspace_bytes, void* cuda_stream);

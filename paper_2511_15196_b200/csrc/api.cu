@@ -59,7 +59,8 @@ struct phi4smc {
   double stop_frac;
   float *wphi, *wS, *wU, *dead_S, *dead_M, *M_all, *S_all;
   double *dead_logw, *logw_all, *hsum;
-  int32_t *dead, *surv, *start;
+  int32_t *dead, *surv, *start, *gflag;
+  unsigned long long* gkeys;
   // host side
   uint64_t step_counter;     // mutation steps enqueued so far (next step uses counter + 1)
   uint64_t step_base;        // steps not counted by the device: set_state / restore base + hook steps
@@ -148,6 +149,8 @@ static int carve_ns(phi4smc* h, char* base, size_t* total) {
   h->dead = c.take<int32_t>(kd);
   h->surv = c.take<int32_t>(N);
   h->start = c.take<int32_t>(kd);
+  h->gkeys = c.take<unsigned long long>(ns_sort_scratch_keys(N));
+  h->gflag = c.take<int32_t>(ns_sort_scratch_keys(N) ? N : 0);
   const size_t nlog = (size_t)h->max_iters * kd;
   h->dead_S = c.take<float>(nlog);
   h->dead_M = c.take<float>(nlog);
@@ -218,7 +221,8 @@ PHI4_API size_t smc_workspace_bytes(int L, int N) {
 }
 
 PHI4_API size_t ns_workspace_bytes(int L, int n_live, int k_delete, int max_iters) {
-  if (L < 1 || L > PHI4_MAX_L || n_live < 2 || k_delete < 1 || k_delete >= n_live || max_iters < 1)
+  if (L < 1 || L > PHI4_MAX_L || n_live < 2 || n_live > PHI4_NS_MAX_LIVE || k_delete < 1 ||
+      k_delete >= n_live || max_iters < 1)
     return 0;
   phi4smc tmp;
   memset(&tmp, 0, sizeof(tmp));
@@ -595,6 +599,7 @@ static NsArgs ns_args(phi4smc* h) {
   a.seed = h->seed; a.dead = h->dead; a.surv = h->surv; a.start = h->start;
   a.dead_S = h->dead_S; a.dead_M = h->dead_M; a.dead_logw = h->dead_logw;
   a.max_iters = h->max_iters; a.stop_frac = h->stop_frac; a.ctrl = h->ctrl; a.hsum = h->hsum;
+  a.gkeys = h->gkeys; a.gflag = h->gflag;
   return a;
 }
 
@@ -603,7 +608,7 @@ static int ns_init_impl(phi4smc** out, int L, float kappa, float m0sq, float lam
                         void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
   if (!out) return PHI4_EINVAL;
   *out = nullptr;
-  if (n_live > 16384 || k_delete > 1024 || n_walk < 1 || !(stop_frac > 0.0)) return PHI4_EINVAL;
+  if (n_live > PHI4_NS_MAX_LIVE || n_walk < 1 || !(stop_frac > 0.0)) return PHI4_EINVAL;
   if (!isfinite(kappa) || !isfinite(m0sq) || !isfinite(lambda)) return PHI4_EINVAL;
   size_t need = ns_workspace_bytes(L, n_live, k_delete, max_iters);
   if (need == 0 || !d_workspace || workspace_bytes < need ||

@@ -12,73 +12,118 @@ __device__ __forceinline__ double logaddexp_d(double a, double b) {
   return m + log(exp(a - m) + exp(b - m));
 }
 
-// Ascending bitonic sort of 1024 E composite keys (descending S_E, ascending index; pad keys sort
-// last) by one block of 1024 threads.  Thread t holds keys t E .. t E + E - 1 in registers:
+// Bitonic network on 64-bit composite keys (descending S_E, ascending index; pad keys sort last).
+// A block of 1024 threads holds 1024 E keys, thread t the keys t E .. t E + E - 1 in registers:
 // partners inside the thread are exchanged in registers, partners inside the warp by shuffles,
 // and only the strides that cross warps (j >= 32 E) go through shared memory -- 15 of the 78
-// stages at n = 4096 instead of a barrier after every stage.  The sorted keys end in `keys`.
+// stages at n = 4096 instead of a barrier after every stage.
+__device__ __forceinline__ unsigned long long ns_key(float S, int i) {
+  const uint32_t b = __float_as_uint(S);
+  const uint32_t asc = (b & 0x80000000u) ? ~b : (b | 0x80000000u);   // ascending-orderable
+  return ((unsigned long long)(~asc) << 32) | (uint32_t)i;           // descending S, ascending i
+}
+
+// The strides jstart, jstart / 2, ..., 1 of merge stage k for the block's 1024 E keys, whose global
+// positions start at `base` (a multiple of 1024 E): position gi sorts ascending iff (gi & k) == 0.
+template <int E>
+__device__ __forceinline__ void bitonic_strides(unsigned long long (&kr)[E], unsigned long long* keys,
+                                                int k, int jstart, int base) {
+  const int tid = threadIdx.x;
+  for (int j = jstart; j >= E && j > 0; j >>= 1) {
+    if (j >= 32 * E) {
+      // partner in another warp: through shared memory
+#pragma unroll
+      for (int e = 0; e < E; ++e) keys[tid * E + e] = kr[e];
+      __syncthreads();
+#pragma unroll
+      for (int e = 0; e < E; ++e) {
+        const int i = tid * E + e;
+        const unsigned long long y = keys[i ^ j];
+        const bool keep_min = ((i & j) == 0) == (((base + i) & k) == 0);
+        kr[e] = keep_min ? (kr[e] < y ? kr[e] : y) : (kr[e] > y ? kr[e] : y);
+      }
+      __syncthreads();
+    } else {
+      // partner in another lane of this warp, same register slot
+      const int lm = j / E;
+#pragma unroll
+      for (int e = 0; e < E; ++e) {
+        const int i = tid * E + e;
+        const unsigned long long y = __shfl_xor_sync(0xffffffffu, kr[e], lm);
+        const bool keep_min = ((i & j) == 0) == (((base + i) & k) == 0);
+        kr[e] = keep_min ? (kr[e] < y ? kr[e] : y) : (kr[e] > y ? kr[e] : y);
+      }
+    }
+  }
+  // partners inside this thread: strides E/2 .. 1 (compile-time register indices)
+#pragma unroll
+  for (int jj = E >> 1; jj > 0; jj >>= 1) {
+    if (jj <= jstart) {
+#pragma unroll
+      for (int e = 0; e < E; ++e) {
+        if ((e & jj) == 0) {
+          const int i = tid * E + e;
+          const bool up = ((base + i) & k) == 0;
+          const unsigned long long x = kr[e], y = kr[e | jj];
+          if ((x > y) == up) { kr[e] = y; kr[e | jj] = x; }
+        }
+      }
+    }
+  }
+}
+
+// Full sort of the block's 1024 E keys (built from S; positions >= n are pad keys); the sorted keys
+// end in `keys` (shared memory).
 template <int E>
 __device__ __forceinline__ void bitonic_sort_block(const float* __restrict__ S, int n,
-                                                   unsigned long long* keys) {
+                                                   unsigned long long* keys, int base = 0) {
   const int tid = threadIdx.x, NP = 1024 * E;
   unsigned long long kr[E];
 #pragma unroll
   for (int e = 0; e < E; ++e) {
-    const int i = tid * E + e;
-    unsigned long long key = ~0ull;
-    if (i < n) {
-      uint32_t b = __float_as_uint(S[i]);
-      uint32_t asc = (b & 0x80000000u) ? ~b : (b | 0x80000000u);   // ascending-orderable
-      key = ((unsigned long long)(~asc) << 32) | (uint32_t)i;        // descending S, ascending i
-    }
-    kr[e] = key;
+    const int i = base + tid * E + e;
+    kr[e] = i < n ? ns_key(S[i], i) : ~0ull;
   }
-  for (int k = 2; k <= NP; k <<= 1) {
-    for (int j = k >> 1; j >= E && j > 0; j >>= 1) {
-      if (j >= 32 * E) {
-        // partner in another warp: through shared memory
-#pragma unroll
-        for (int e = 0; e < E; ++e) keys[tid * E + e] = kr[e];
-        __syncthreads();
-#pragma unroll
-        for (int e = 0; e < E; ++e) {
-          const int i = tid * E + e;
-          const unsigned long long y = keys[i ^ j];
-          const bool keep_min = ((i & j) == 0) == ((i & k) == 0);
-          kr[e] = keep_min ? (kr[e] < y ? kr[e] : y) : (kr[e] > y ? kr[e] : y);
-        }
-        __syncthreads();
-      } else {
-        // partner in another lane of this warp, same register slot
-        const int lm = j / E;
-#pragma unroll
-        for (int e = 0; e < E; ++e) {
-          const int i = tid * E + e;
-          const unsigned long long y = __shfl_xor_sync(0xffffffffu, kr[e], lm);
-          const bool keep_min = ((i & j) == 0) == ((i & k) == 0);
-          kr[e] = keep_min ? (kr[e] < y ? kr[e] : y) : (kr[e] > y ? kr[e] : y);
-        }
-      }
-    }
-    // partners inside this thread: strides E/2 .. 1 (compile-time register indices)
-#pragma unroll
-    for (int jj = E >> 1; jj > 0; jj >>= 1) {
-      if (jj <= (k >> 1)) {
-#pragma unroll
-        for (int e = 0; e < E; ++e) {
-          if ((e & jj) == 0) {
-            const int i = tid * E + e;
-            const bool up = (i & k) == 0;
-            const unsigned long long x = kr[e], y = kr[e | jj];
-            if ((x > y) == up) { kr[e] = y; kr[e | jj] = x; }
-          }
-        }
-      }
-    }
-  }
+  for (int k = 2; k <= NP; k <<= 1) bitonic_strides<E>(kr, keys, k, k >> 1, base);
 #pragma unroll
   for (int e = 0; e < E; ++e) keys[tid * E + e] = kr[e];
   __syncthreads();
+}
+
+// ---- more than 16384 live points: the same network across blocks, keys in global memory --------
+constexpr int NS_BLOCK_KEYS = 16384;
+__global__ void __launch_bounds__(1024)
+ns_sort_local_kernel(const float* __restrict__ S, int n, unsigned long long* __restrict__ gkeys,
+                     const Ctrl* ctrl) {
+  extern __shared__ unsigned long long keys[];
+  if (ctrl->done) return;
+  const int base = blockIdx.x * NS_BLOCK_KEYS;
+  bitonic_sort_block<16>(S, n, keys, base);
+  for (int i = threadIdx.x; i < NS_BLOCK_KEYS; i += blockDim.x) gkeys[base + i] = keys[i];
+}
+// one stride j >= 16384 of merge stage k: thread = the lower element of a pair
+__global__ void ns_merge_global_kernel(unsigned long long* __restrict__ gkeys, int j, int k, int np2,
+                                       const Ctrl* ctrl) {
+  if (ctrl->done) return;
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= np2 / 2) return;
+  const int i = ((t & ~(j - 1)) << 1) | (t & (j - 1));          // bit j clear
+  const unsigned long long x = gkeys[i], y = gkeys[i | j];
+  const bool up = (i & k) == 0;
+  if ((x > y) == up) { gkeys[i] = y; gkeys[i | j] = x; }
+}
+// the strides 8192 .. 1 of merge stage k, block-local
+__global__ void __launch_bounds__(1024)
+ns_merge_local_kernel(unsigned long long* __restrict__ gkeys, int k, const Ctrl* ctrl) {
+  extern __shared__ unsigned long long keys[];
+  if (ctrl->done) return;
+  const int base = blockIdx.x * NS_BLOCK_KEYS, tid = threadIdx.x;
+  unsigned long long kr[16];
+#pragma unroll
+  for (int e = 0; e < 16; ++e) kr[e] = gkeys[base + tid * 16 + e];
+  bitonic_strides<16>(kr, keys, k, NS_BLOCK_KEYS >> 1, base);
+#pragma unroll
+  for (int e = 0; e < 16; ++e) gkeys[base + tid * 16 + e] = kr[e];
 }
 
 // N1 + N2 + survivors + start choice in one CTA.
@@ -88,46 +133,49 @@ __device__ __forceinline__ void bitonic_sort_block(const float* __restrict__ S, 
 //      do not depend on the data, so the batch is one parallel log-sum-exp.
 //  N3 (choice): survivors in index order by a flag scan; walker j starts from survivor number
 //      (word0 mod (n - k_del)) of Philox stream NS_START (c1 = j, c2 = iteration).
+// More than 16384 live points: the keys arrive sorted in global memory (a.gkeys, multi-block
+// network above) and the survivor flags live in global memory too (a.gflag).
 __global__ void __launch_bounds__(1024)
 ns_select_evidence_kernel(NsArgs a) {
   pdl_enter();
-  extern __shared__ unsigned long long keys[];   // npow2 keys; later reused as int flags
+  extern __shared__ unsigned long long skeys[];  // npow2 keys; later reused as int flags
   __shared__ double scratch[33];
   __shared__ int wsum[32];
   Ctrl* ctrl = a.ctrl;
   if (ctrl->done) return;
   const int n = a.n, kd = a.k_del, tid = threadIdx.x, nt = blockDim.x;
-  int np2 = 1024;                    // padded to the block: thread t holds keys t E .. t E + E - 1
-  while (np2 < n) np2 <<= 1;
-  switch (np2 >> 10) {
-    case 1: bitonic_sort_block<1>(a.S, n, keys); break;
-    case 2: bitonic_sort_block<2>(a.S, n, keys); break;
-    case 4: bitonic_sort_block<4>(a.S, n, keys); break;
-    case 8: bitonic_sort_block<8>(a.S, n, keys); break;
-    default: bitonic_sort_block<16>(a.S, n, keys); break;
+  const bool big = n > NS_BLOCK_KEYS;
+  const unsigned long long* keys = big ? a.gkeys : skeys;
+  if (!big) {
+    int np2 = 1024;                  // padded to the block: thread t holds keys t E .. t E + E - 1
+    while (np2 < n) np2 <<= 1;
+    switch (np2 >> 10) {
+      case 1: bitonic_sort_block<1>(a.S, n, skeys); break;
+      case 2: bitonic_sort_block<2>(a.S, n, skeys); break;
+      case 4: bitonic_sort_block<4>(a.S, n, skeys); break;
+      case 8: bitonic_sort_block<8>(a.S, n, skeys); break;
+      default: bitonic_sort_block<16>(a.S, n, skeys); break;
+    }
   }
   const int it = ctrl->temp_index;
   const double logX0 = ctrl->logX;
   // dead list, threshold
   for (int j = tid; j < kd; j += nt) a.dead[j] = (int)(uint32_t)keys[j];
   const float S_star = a.S[(int)(uint32_t)keys[kd - 1]];
-  // evidence of the batch
+  // evidence of the batch: two passes (max, then sum) over the dead points, k_del / 1024 per thread
   double best = -INFINITY;
-  double term_mine[1];   // kd <= 1024 = blockDim: one dead point per thread at most
-  term_mine[0] = -INFINITY;
-  if (tid < kd) {
-    const double lx = logX0 - a.hsum[tid];                                // logX_{j-1}, j = tid+1
-    double step = 1.0 / (double)(n - tid);                                // 1/(n-j+1)
-    double logw = lx + log1p(-exp(-step));
-    int d = (int)(uint32_t)keys[tid];
-    float Sd = a.S[d];
-    term_mine[0] = logw - (double)Sd;
+  for (int j = tid; j < kd; j += nt) {
+    const double lx = logX0 - a.hsum[j];                                  // logX_{j'-1}, j' = j+1
+    const double step = 1.0 / (double)(n - j);                            // 1/(n-j'+1)
+    const double logw = lx + log1p(-exp(-step));
+    const int d = (int)(uint32_t)keys[j];
+    const float Sd = a.S[d];
     if (it < a.max_iters) {
-      size_t slot = (size_t)it * kd + tid;
+      const size_t slot = (size_t)it * kd + j;
       a.dead_S[slot] = Sd;
       a.dead_logw[slot] = logw;
     }
-    best = term_mine[0];
+    best = fmax(best, logw - (double)Sd);
   }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) best = fmax(best, __shfl_xor_sync(0xffffffffu, best, o));
@@ -140,16 +188,20 @@ ns_select_evidence_kernel(NsArgs a) {
   }
   __syncthreads();
   best = scratch[32];
-  double e = (tid < kd) ? exp(term_mine[0] - best) : 0.0;
+  double e = 0.0;
+  for (int j = tid; j < kd; j += nt) {
+    const double logw = logX0 - a.hsum[j] + log1p(-exp(-1.0 / (double)(n - j)));
+    e += exp(logw - (double)a.S[(int)(uint32_t)keys[j]] - best);
+  }
   e = block_sum(e, scratch);
   __syncthreads();
   // survivors: flags over n, contiguous run per thread, block scan
-  int* flags = reinterpret_cast<int*>(keys);
-  unsigned long long mykey = (tid < kd) ? keys[tid] : 0ull;
+  // (the dead indices were written to a.dead above: the keys' storage becomes the flag array)
+  int* flags = big ? a.gflag : reinterpret_cast<int*>(skeys);
   __syncthreads();
   for (int i = tid; i < n; i += nt) flags[i] = 1;
   __syncthreads();
-  if (tid < kd) flags[(int)(uint32_t)mykey] = 0;
+  for (int j = tid; j < kd; j += nt) flags[a.dead[j]] = 0;
   __syncthreads();
   const int ipt = (n + nt - 1) / nt;
   const int lo = min(n, tid * ipt), hi = min(n, lo + ipt);
@@ -191,17 +243,40 @@ ns_select_evidence_kernel(NsArgs a) {
   }
 }
 
+size_t ns_sort_scratch_keys(int n) {          // global keys of the multi-block sort (0: not needed)
+  if (n <= NS_BLOCK_KEYS) return 0;
+  size_t np2 = NS_BLOCK_KEYS;
+  while (np2 < (size_t)n) np2 <<= 1;
+  return np2;
+}
+
 void launch_ns_select_evidence(const NsArgs& a, cudaStream_t st) {
-  int np2 = 1024;
-  while (np2 < a.n) np2 <<= 1;
-  size_t smem = (size_t)np2 * sizeof(unsigned long long);
   static bool attr_done = false;
+  const int kb = NS_BLOCK_KEYS * (int)sizeof(unsigned long long);
   if (!attr_done) {
-    cudaFuncSetAttribute(ns_select_evidence_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                         16384 * (int)sizeof(unsigned long long));
+    cudaFuncSetAttribute(ns_select_evidence_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kb);
+    cudaFuncSetAttribute(ns_sort_local_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kb);
+    cudaFuncSetAttribute(ns_merge_local_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kb);
     attr_done = true;
   }
-  ++g_launches; launch_pdl(ns_select_evidence_kernel, 1, 1024, smem, st, a);
+  if (a.n <= NS_BLOCK_KEYS) {
+    int np2 = 1024;
+    while (np2 < a.n) np2 <<= 1;
+    ++g_launches;
+    launch_pdl(ns_select_evidence_kernel, 1, 1024, (size_t)np2 * sizeof(unsigned long long), st, a);
+    return;
+  }
+  // multi-block bitonic network: block-local sorts of 16384 keys, then per merge stage k the
+  // strides >= 16384 one launch each over global memory and the rest block-local
+  const int np2 = (int)ns_sort_scratch_keys(a.n), nb = np2 / NS_BLOCK_KEYS;
+  ++g_launches; ns_sort_local_kernel<<<nb, 1024, kb, st>>>(a.S, a.n, a.gkeys, a.ctrl);
+  for (int k = 2 * NS_BLOCK_KEYS; k <= np2; k <<= 1) {
+    for (int j = k >> 1; j >= NS_BLOCK_KEYS; j >>= 1) {
+      ++g_launches; ns_merge_global_kernel<<<np2 / 2 / 256, 256, 0, st>>>(a.gkeys, j, k, np2, a.ctrl);
+    }
+    ++g_launches; ns_merge_local_kernel<<<nb, 1024, kb, st>>>(a.gkeys, k, a.ctrl);
+  }
+  ++g_launches; ns_select_evidence_kernel<<<1, 1024, 0, st>>>(a);
 }
 
 // hsum[j] = sum_{m=1..j} 1/(n-m+1), j = 0..k_del: the data-independent volume shrinkage of

@@ -20,6 +20,13 @@ CONFIGS = {
     "P10": dict(kind="smc", L=10, N=5000, k=300, m0sq=-4.0, lam=1.0, ess=0.9),
     "P15": dict(kind="smc", L=15, N=5000, k=675, m0sq=-4.0, lam=1.0, ess=0.9),
     "P18": dict(kind="smc", L=18, N=5000, k=972, m0sq=-4.0, lam=1.0, ess=0.9),
+    # the paper's ESS sweep (Table 3: ESS 0.90 / 0.99 / 0.999 with 5 V inner steps)
+    "P10e99": dict(kind="smc", L=10, N=5000, k=500, m0sq=-4.0, lam=1.0, ess=0.99),
+    "P10e999": dict(kind="smc", L=10, N=5000, k=500, m0sq=-4.0, lam=1.0, ess=0.999),
+    # the paper's own nested-sampling setting: N = 5000 live points, delete
+    # fraction 0.5, slice-sampling inner kernel, n_MCMC = 3 V slice steps per replacement
+    "PNS10": dict(kind="ns", L=10, n_live=5000, k_del=2500, n_walk=300, inner="slice", m0sq=-4.0,
+                  lam=1.0, stop_frac=1e-3),
 }
 
 

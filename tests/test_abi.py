@@ -74,7 +74,7 @@ def test_init_argument_checks_and_no_cpu_fallback(lib):
     assert lib.smc_init(C.byref(ptr), 4, -4.0, 1.0, 1024, 0, fake, need - 1, None) == -1
     assert lib.smc_init(C.byref(ptr), 4, -4.0, 1.0, 1024, 0, C.c_void_p((1 << 20) + 4), need, None) == -1
     assert lib.smc_init(C.byref(ptr), 4, -4.0, 1.0, 1024, 0, None, need, None) == -1
-    assert lib.ns_init(C.byref(ptr), 4, -4.0, 1.0, 100000, 10, 5, 0, 1e-3, 10, fake, 1 << 40, None) == -1
+    assert lib.ns_init(C.byref(ptr), 4, -4.0, 1.0, (1 << 20) + 1, 10, 5, 0, 1e-3, 10, fake, 1 << 40, None) == -1
     if not torch.cuda.is_available():
         assert lib.smc_init(C.byref(ptr), 4, -4.0, 1.0, 1024, 0, fake, need, None) == -5   # PHI4_ECUDA
         with pytest.raises(RuntimeError, match="no CPU fallback"):

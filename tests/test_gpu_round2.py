@@ -191,3 +191,93 @@ def test_argument_limits():
         B.smc_init_kl(4, float("inf"), 0.5, 256, 0)
     with pytest.raises(B.Phi4Error):
         B.ns_init_kl(4, float("inf"), 0.5, 256, 32, 4, 0)
+
+
+# ---------------------------------------------------------------- NS at the paper's settings ----
+def test_ns_paper_setting_first_iteration_lockstep():
+    """N = 5000 live points, delete fraction 0.5 (2500 deletions per iteration,
+    more dead points than one CTA has threads), slice-sampling inner kernel (reading A16)."""
+    c = inputs.CONFIGS["PNS10"]
+    L, n, kd, nw, seed = c["L"], c["n_live"], c["k_del"], 4, 17
+    h = B.ns_init(L, c["m0sq"], c["lam"], n, kd, nw, seed, max_iters=8)
+    B.ns_set_params(h, inner=1)
+    st0 = B.smc_get_state(h)
+    info = B.ns_step(h)
+    S0 = st0["S"].astype(np.float64)
+    dead = O.ns_select(S0, kd)
+    got = B.ns_get_dead(h)
+    assert np.array_equal(got["last_dead"], dead)                             # N1 exact
+    assert info["S_star"] == S0[dead[-1]]
+    lw = np.array([-sum(1.0 / (n - m + 1) for m in range(1, j)) +
+                   math.log1p(-math.exp(-1.0 / (n - j + 1))) for j in range(1, kd + 1)])
+    assert np.allclose(got["dead_logw"], lw, rtol=1e-12, atol=1e-14)          # N2, reading A6
+    from scipy.special import logsumexp
+    assert info["logZ"] == pytest.approx(logsumexp(lw - S0[dead]), rel=1e-10)
+    assert info["logX"] == pytest.approx(-sum(1.0 / (n - j + 1) for j in range(1, kd + 1)), rel=1e-12)
+    # N3: slice walks replayed by the oracle from the GPU's start state and factor
+    Lc = B.smc_get_chol(h)
+    surv = np.setdiff1d(np.arange(n), dead)
+    start = np.array([surv[O.word0(seed, O.TAG_NS_START, 0, j) % (n - kd)] for j in range(kd)])
+    f0 = st0["phi"][:, start].astype(np.float64)
+    Ss, Us = O.action_batch(f0, L, c["m0sq"], c["lam"])
+    p, S, U0, t, nexp, nshr, amb = O.slice_walk(f0, Ss, Us, L, c["m0sq"], c["lam"], Lc, info["S_star"],
+                                                seed, 1, nw, width=np.float32(1.0), m_expand=8)
+    st1 = B.smc_get_state(h)
+    clean = amb.min(axis=0) > 2e-3
+    assert clean.mean() > 0.6
+    assert np.abs(st1["phi"][:, dead][:, clean] - p[:, clean]).max() < 1e-4
+    assert np.array_equal(st1["phi"][:, surv], st0["phi"][:, surv])           # survivors untouched
+    assert np.all(st1["S"] < info["S_star"] + 1e-3)
+    h.close()
+
+
+def test_ns_paper_setting_statistical_parity():
+    """N = 5000, delete fraction 0.5, slice kernel (10 slice steps per replacement instead of 3 V,
+    so that eight oracle runs stay affordable): log Z and iterations within 3 combined SE."""
+    c = inputs.CONFIGS["PNS10"]
+    L, n, kd, nw = c["L"], c["n_live"], c["k_del"], 10
+
+    def gpu(seed):
+        h = B.ns_init(L, c["m0sq"], c["lam"], n, kd, nw, seed, max_iters=512)
+        B.ns_set_params(h, inner=1)
+        it = B.ns_run(h)
+        out = (B.log_Z(h), it, B.observables(h)["absM"])
+        h.close()
+        return out
+    g = [gpu(s) for s in range(8)]
+    o = [O.ns_run(L, c["m0sq"], c["lam"], n, kd, nw, s, inner="slice") for s in range(8)]
+    for key, a, b in (("logZ", [x[0] for x in g], [r["logZ"] for r in o]),
+                      ("iters", [x[1] for x in g], [r["iters"] for r in o])):
+        a, b = np.asarray(a, float), np.asarray(b, float)
+        se = math.hypot(a.std(ddof=1), b.std(ddof=1)) / math.sqrt(8)
+        print("PNS10 %s: gpu %.4f oracle %.4f (%.2f combined SE)" % (key, a.mean(), b.mean(),
+                                                                    abs(a.mean() - b.mean()) / max(se, 1e-12)))
+        assert abs(a.mean() - b.mean()) < 3 * se + (0.5 if key == "iters" else 0.0)
+
+
+@pytest.mark.parametrize("n,kd", [(40000, 20000), (70000, 1000)])
+def test_ns_select_beyond_one_cta(n, kd):
+    """More than 16384 live points: the multi-block bitonic network orders the keys; dead list,
+    threshold, evidence and start points are still exact."""
+    L, nw, seed = 4, 2, 3
+    h = B.ns_init(L, -4.0, 1.0, n, kd, nw, seed, max_iters=4)
+    st0 = B.smc_get_state(h)
+    info = B.ns_step(h)
+    S0 = st0["S"].astype(np.float64)
+    dead = O.ns_select(S0, kd)
+    got = B.ns_get_dead(h)
+    assert np.array_equal(got["last_dead"], dead)
+    assert info["S_star"] == S0[dead[-1]]
+    assert np.array_equal(got["dead_S"], st0["S"][dead])
+    st1 = B.smc_get_state(h)
+    surv = np.setdiff1d(np.arange(n), dead)
+    assert np.array_equal(st1["phi"][:, surv], st0["phi"][:, surv])
+    assert np.all(st1["S"] < info["S_star"] + 1e-3)
+    # walkers that did not move (2 steps only) sit exactly on their start points: the rule of R1
+    start = np.array([surv[O.word0(seed, O.TAG_NS_START, 0, j) % (n - kd)] for j in range(0, kd, 97)])
+    moved = 0
+    for j, s in zip(range(0, kd, 97), start):
+        if not np.array_equal(st1["phi"][:, dead[j]], st0["phi"][:, s]):
+            moved += 1
+    assert moved < len(start)                     # some walkers stay; the others have moved off
+    h.close()
