@@ -49,6 +49,9 @@ extern "C" {
                              stop rule fired.  Everything computed so far is valid, but log_Z()
                              is the dead-point evidence only (no live-point term was added).     */
 
+#define PHI4_ETOOBIG (-7) /* a no-allocation entry point was given a size beyond its fixed capacity
+                             (phi4_resample_noalloc: N > PHI4_NOALLOC_MAX_N)                     */
+
 #define PHI4_HIST_BINS 80 /* B = 80 bins; fixed range [-1.6, 1.6] (reading A13)     */
 #define PHI4_MAX_HOOK_STEPS 64 /* largest k accepted by smc_mutate when flags/margins are wanted  */
 #define PHI4_NS_MAX_LIVE (1 << 20) /* nested sampling: largest n_live (k_delete: any value < n_live) */
@@ -298,6 +301,29 @@ int ns_get_dead(phi4smc* h, int32_t* h_last_dead_idx, float* h_dead_S, float* h_
 /* Restores the first n_dead entries of the dead-point log (checkpoint / resume of observables). */
 int ns_set_dead(phi4smc* h, const float* h_dead_S, const float* h_dead_M,
                 const double* h_dead_logw, int n_dead);
+
+/* ------------------------------------------------------------- no-allocation entry point ------
+ * For callers that cannot allocate device memory (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): exact systematic resampling (P3; reading
+ * R5) without a handle or a workspace.  The scratch of the kernels (64-bit integer CDF, block sums,
+ * control block) is a file-scope __device__ array of PHI4_NOALLOC_SCRATCH_BYTES inside the library:
+ * every GPU that loads libphi4smc.so holds that much until the process exits.  The call performs no
+ * cudaMalloc / cudaFree and calls no allocating library routine; it only enqueues kernels.
+ *   d_w          DEVICE, N fp32 weights in [0, 1] (the resampler's contract: max-shifted, max = 1)
+ *   N            1 <= N <= PHI4_NOALLOC_MAX_N, else PHI4_ETOOBIG (nothing is enqueued)
+ *   seed, t      the offset U is word 0 of the Philox draw (tag RESAMPLE, step t, slot 0): the same
+ *                ancestors as smc_resample on a handle with this seed at temperature index t
+ *   d_ancestors  DEVICE, receives N int32 ancestor indices (identity map if every weight is 0)
+ * Enqueues on cuda_stream and returns without synchronising.  All calls share the one array, which
+ * keeps the last call's contents (each call re-initialises what it reads): calls that overlap on
+ * the GPU -- different streams or host threads -- race; serialise them.
+ * phi4_noalloc_setup() looks up the array's device address for the CURRENT device (done lazily by
+ * the first call otherwise; call it once per device before graph capture begins).              */
+#define PHI4_NOALLOC_MAX_N 131072
+#define PHI4_NOALLOC_SCRATCH_BYTES 1181952
+int phi4_noalloc_setup(void);
+int phi4_resample_noalloc(const float* d_w, int N, uint64_t seed, uint32_t t, int32_t* d_ancestors,
+                          void* cuda_stream);
 
 #ifdef __cplusplus
 }

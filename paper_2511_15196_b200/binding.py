@@ -16,7 +16,8 @@ HIST_BINS = 80
 MAX_HOOK_STEPS = 64
 
 ERRORS = {0: "PHI4_OK", -1: "PHI4_EINVAL", -2: "PHI4_ENOMEM", -3: "PHI4_ENOTPD", -4: "PHI4_ENAN",
-          -5: "PHI4_ECUDA", -6: "PHI4_ETRUNC"}
+          -5: "PHI4_ECUDA", -6: "PHI4_ETRUNC", -7: "PHI4_ETOOBIG"}
+NOALLOC_MAX_N = 131072
 ETRUNC = -6
 
 
@@ -89,6 +90,8 @@ SIGNATURES = {
     "phi4_last_cuda_error": (C.c_char_p, [_vp]),
     "phi4_kernel_launches": (_u64, []),
     "phi4_measure_peaks": (_i, [_d, C.POINTER(phi4_peaks), _vp, _sz, _vp]),
+    "phi4_noalloc_setup": (_i, []),
+    "phi4_resample_noalloc": (_i, [_vp, _i, _u64, C.c_uint32, _vp, _vp]),
     "smc_workspace_bytes": (_sz, [_i, _i]),
     "smc_init": (_i, [C.POINTER(_vp), _i, _f, _f, _i, _u64, _vp, _sz, _vp]),
     "smc_init_kl": (_i, [C.POINTER(_vp), _i, _f, _f, _i, _u64, _vp, _sz, _vp]),
@@ -199,6 +202,20 @@ def phi4_measure_peaks(seconds=2.0, device="cuda:0"):
     if rc != 0:
         raise Phi4Error(rc, "phi4_measure_peaks")
     return {k: getattr(out, k) for k, _ in phi4_peaks._fields_ if k != "reserved"}
+
+
+def phi4_resample_noalloc(w, seed, t, out):
+    """w: CUDA float32 tensor (N,), out: CUDA int32 tensor (N,) on the same device; enqueues on
+    torch's current stream of that device, allocates nothing.  Raises Phi4Error(-7) if N > NOALLOC_MAX_N."""
+    import torch
+    assert w.is_cuda and out.is_cuda and w.device == out.device
+    assert w.dtype == torch.float32 and out.dtype == torch.int32 and w.is_contiguous() and out.is_contiguous()
+    assert out.numel() >= w.numel()
+    with torch.cuda.device(w.device):
+        rc = load().phi4_resample_noalloc(C.c_void_p(w.data_ptr()), w.numel(), seed, t,
+                                          C.c_void_p(out.data_ptr()), _stream_ptr(w.device))
+    if rc != 0:
+        raise Phi4Error(rc, "phi4_resample_noalloc", load().phi4_strerror(rc).decode())
 
 
 def smc_workspace_bytes(L, N):

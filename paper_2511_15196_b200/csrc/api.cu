@@ -194,6 +194,7 @@ PHI4_API const char* phi4_strerror(int code) {
     case PHI4_ENAN: return "non-finite action or weight";
     case PHI4_ECUDA: return "CUDA error or no device";
     case PHI4_ETRUNC: return "nested sampling stopped by max_iters: log_Z lacks the live-point term";
+    case PHI4_ETOOBIG: return "size exceeds the fixed capacity of a no-allocation entry point (N > PHI4_NOALLOC_MAX_N = 131072)";
     default: return "unknown error";
   }
 }
