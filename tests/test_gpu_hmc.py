@@ -5,8 +5,9 @@ Tolerance.  An HMC proposal is a whole trajectory, not a small perturbation, so 
 fp32 evaluation of S_E, U0 and the kinetic energy: the margin g = (H_old - H_new) - ln u carries
 the 2e-5 * A error of reading A12 (A = sum of the absolute terms of S_E, a few hundred at V = 100)
 plus the fp32 rounding of nfrog leapfrog steps.  Decisions are therefore compared outside
-|g| < BAND_HMC = 1e-3 and margins within BAND_HMC / 2 + 1e-5 |g| (measured: 3e-5 at C1's
-shape, 2.3e-4 worst case on unit-normal fields at L = 4)."""
+|g| < BAND_HMC = 6e-4 and margins within BAND_HMC / 2 + 1e-5 |g| (measured: 3e-5 at C1's
+shape, 1.1e-4 worst case over the twelve lock-step shapes in round 2 -- profiles/r02_parity_margins.md --
+and 2.3e-4 on unit-normal fields at L = 4; the band was 1e-3 in round 1)."""
 import numpy as np
 import pytest
 
@@ -16,7 +17,7 @@ from paper_2511_15196_b200 import build, inputs
 
 pytestmark = pytest.mark.gpu
 
-BAND_HMC = 1e-3
+BAND_HMC = 6e-4
 
 
 @pytest.fixture(scope="module", autouse=True)

@@ -4,7 +4,7 @@ PAPER.md:53(iv), :174; reading A16): the CUDA path through the C ABI against the
 Tolerance.  The kernel evaluates S_E and U0 along the line phi + t d from polynomial coefficients
 in fp32, the oracle evaluates both directly in FP64; every stepping-out / shrinkage decision is a
 comparison of such a value against S_star or log y.  A walker is compared when the oracle's
-closest decision over all its steps was further than BAND_SLICE = 2e-3 from flipping (the
+closest decision over all its steps was further than BAND_SLICE = 3e-4 from flipping (the
 oracle reports that distance); for those the whole decision sequence must agree, so the final
 fields agree to fp32 rounding."""
 import math
@@ -18,7 +18,7 @@ from paper_2511_15196_b200 import build
 
 pytestmark = pytest.mark.gpu
 
-BAND_SLICE = 2e-3
+BAND_SLICE = 3e-4
 
 
 @pytest.fixture(scope="module", autouse=True)
@@ -59,7 +59,10 @@ def test_slice_first_iteration_lockstep(L, n, kd, nw, width, mexp):
     print("slice L=%d n=%d: clean fraction %.3f (walkers whose closest decision is > %.0e away), "
           "walkers reproduced %.3f, worst field error on clean walkers %.2e"
           % (L, n, clean.mean(), BAND_SLICE, same.mean(), np.abs(got[:, clean] - p[:, clean]).max()))
-    assert clean.mean() > 0.6
+    # measured in round 2 (profiles/r02_parity_margins.md): at a band of 2e-3 the clean fraction was
+    # 0.67-0.98 and EVERY walker, clean or not, reproduced the oracle to 1e-6; the band is now 3e-4
+    assert clean.mean() > 0.85
+    assert same.mean() > 0.99
     assert np.abs(got[:, clean] - p[:, clean]).max() < 1e-4
     gS = st1["S"][dead]
     A = O.action_batch(p, L, m0sq, lam, with_abs=True)[2]
