@@ -34,9 +34,9 @@ ALU_OPS_PER_LEAPFROG_SITE = 11
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, copied from the
 # committed `ncu --set full` captures (not measured by this run): C1 the fused mutation kernel,
 # C3 / C4 the proposal GEMM.
-NCU_TRAFFIC = {"C1": (6815744, "profiles/r01_mutate_tc_C1.md"),
-               "C3": (1127837175, "profiles/r01_large_V.md"),
-               "C4": (15380342000, "profiles/r01_large_V.md")}
+NCU_TRAFFIC = {"C1": (6815000, "profiles/r02_ncu_tables.md"),
+               "C3": (1132800000, "profiles/r02_ncu_tables.md"),
+               "C4": (14304000000, "profiles/r02_ncu_tables.md")}
 
 
 def peaks():
