@@ -196,21 +196,13 @@ __device__ __forceinline__ bool chol_skip(const Ctrl* ctrl, int attempt, int res
   return attempt == 1 && !(ctrl->chol_fail & 1);
 }
 
-// ------------------------------------------------------------------ small V: one CTA ---------
-// Panel-blocked right-looking factorisation in shared memory (row stride V+1: conflict free).
-// Per 8-column panel: every row thread re-factorises the 8x8 diagonal block in registers (170
-// FMAs, no barrier) and solves its own row against it; then all 1024 threads apply the rank-8
-// update to the trailing lower triangle.  Three barriers per panel instead of two per column.
-// Both attempts of reading A4 (plain, then jitter 1e-6 tr/V) run inside this one launch.
+// ------------------------------------------------------------------ panel routine -----------
 constexpr int CS_NB = 8;
-#ifndef PHI4_CS_THREADS
-#define PHI4_CS_THREADS 1024
-#endif
-constexpr int CS_THREADS = PHI4_CS_THREADS;
 // In-place lower Cholesky of the n x n matrix in shared memory (row stride P), 8-column panels:
-// every row thread re-factorises the 8x8 diagonal block in registers and solves its own row,
-// then the whole block applies the rank-8 update to the trailing lower triangle.  *failed_s is
-// set if a pivot is <= 0 (the factorisation then continues with a unit pivot).
+// every row thread re-factorises the 8x8 diagonal block in registers (170 FMAs, no barrier) and
+// solves its own row, then the whole block applies the rank-8 update to the trailing lower
+// triangle.  *failed_s is set if a pivot is <= 0 (the factorisation then continues with a unit
+// pivot).  Used for the 64 x 64 diagonal blocks of the large-V path (chol_diag_kernel).
 __device__ __forceinline__ void chol_panels(float* sm, int P, int V, int* failed_s) {
   const int tid = threadIdx.x;
     for (int jb = 0; jb < V; jb += CS_NB) {
@@ -310,52 +302,271 @@ __device__ __forceinline__ void chol_panels(float* sm, int P, int V, int* failed
     }
 }
 
-__global__ void __launch_bounds__(1024)
+// ---- V <= 160 in one CTA: register-resident state, warp-specialised --------------------------
+// Right-looking factorisation in 8-column panels (column block q = columns 8q .. 8q+7), no matrix
+// in shared memory.  Two groups of warps:
+//  * ROW warps: thread r owns matrix row r.  At panel p it holds x = A[r][8p..8p+7] with every
+//    earlier panel applied, re-factorises the 8 x 8 diagonal block in registers with its own row
+//    riding along as a ninth row (the pivots are the only serial chain), publishes its eight new
+//    L entries k-major (Lp), and then applies panel p to its own entries of the NEXT column block
+//    itself: x' = Ap - sum_k x[k] L[8(p+1)+c][k].  The eight rows of the next diagonal block go
+//    through shared memory (Dn).  Two row-group barriers per panel; nothing else is on the
+//    critical path.
+//  * TILE warps: the lower triangle is cut into 4 x 4 tiles, one per thread, in registers for the
+//    whole factorisation (<= 820 tiles: 26 warps).  A tile of column block q receives the
+//    updates of panels 0 .. q-2 from Lp (sixteen 16-byte shared loads, 128 FMAs per panel) and
+//    is then published k-major (Ap) for the row warps, which need it one whole panel later.
+//  * one housekeeping warp copies Lp to Lc and writes the zeros above the diagonal.
+// Named barriers: AP_FULL (tiles -> rows), LP_FULL (rows -> tiles), LP_EMPTY (tiles -> rows, two
+// Lp buffers), ROW_A / ROW_B (row group).  Both attempts of reading A4 run inside this launch.
+constexpr int CT_LD = 160;                 // leading dimension of Ap / Lp (rows), V <= 160
+constexpr int CT_ROW_WARPS = 5;            // 160 rows
+constexpr int CT_TILE_WARPS = 26;          // 40 * 41 / 2 = 820 tiles
+constexpr int CT_THREADS = 32 * (CT_TILE_WARPS + CT_ROW_WARPS + 1);   // + 1 housekeeping warp
+constexpr int CT_RWT = 32 * CT_ROW_WARPS;
+// named barriers: M(p) = "panel p of L is in Lp, column block p + 1 of A is in Ap" (rows, tile
+// warps that still hold a tile of a block >= p + 1, housekeeping); B(p) = "the diagonal block of
+// panel p + 1 is in Dn, and Lp of panel p - 1 has been read" (rows sync; tile warps and
+// housekeeping arrive); AP0 / B_PRO: the same two for the prologue.  M and B alternate ids.
+enum { BAR_M = 1, BAR_B = 3, BAR_AP0 = 5, BAR_B_PRO = 6 };
+
+__device__ __forceinline__ void bar_sync(int id, int nthreads) {
+  asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+__device__ __forceinline__ void bar_arrive(int id, int nthreads) {
+  asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+__device__ __forceinline__ float rsqrt_ftz(float x) {
+  float y;
+  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+
+struct CholTiles {
+  int nT;                                   // tile rows = ceil(V / 4)
+  __device__ int first(int C) const { return C * nT - C * (C - 1) / 2; }   // first tile of column C
+  __device__ int ntiles() const { return nT * (nT + 1) / 2; }
+  __device__ int nwarps() const { return (ntiles() + 31) >> 5; }
+  // tile warps that hold a tile in a column >= C: warps [warp_lo(C), nwarps())
+  __device__ int warp_lo(int C) const { return C >= nT ? nwarps() : first(C) >> 5; }
+  // number of warps holding a tile of columns C, C + 1 (first of them: warp_lo(C)); 0 if none
+  __device__ int owners(int C) const {
+    if (C >= nT) return 0;
+    const int last = first(min(C + 2, nT)) - 1;
+    return (last >> 5) - (first(C) >> 5) + 1;
+  }
+};
+
+__global__ void __launch_bounds__(CT_THREADS)
 chol_small_kernel(const float* __restrict__ Sigma, float* __restrict__ Lc, int V, Ctrl* ctrl,
                   int respect_done) {
   pdl_enter();
-  extern __shared__ float sm[];   // V x (V+1)
+  __shared__ __align__(16) float Ap[2][CS_NB * CT_LD];   // column block q of A, k-major, buffer q & 1
+  __shared__ __align__(16) float Lp[2][CS_NB * CT_LD];   // panel p of L, k-major, buffer p & 1
+  __shared__ __align__(16) float Dn[2][CS_NB * CS_NB];   // diagonal block of panel p, k-major
   __shared__ int failed_s;
-  __shared__ double red[33];
   if (respect_done && ctrl->done) return;
-  const int P = V + 1, tid = threadIdx.x;
-  // tr(Sigma) for the jitter scale
-  double tr = 0.0;
-  for (int x = tid; x < V; x += blockDim.x) tr += (double)Sigma[(size_t)x * V + x];
-  tr = block_sum(tr, red);
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  CholTiles T;
+  T.nT = (V + 3) >> 2;
+  const int ntiles = T.ntiles(), ntw = T.nwarps();
+  const int nP = (V + CS_NB - 1) / CS_NB;
+  const bool is_tile = warp < CT_TILE_WARPS, is_row = !is_tile && warp < CT_TILE_WARPS + CT_ROW_WARPS;
+
+  // tile of this thread (numbered column by column: t -> column C ascending, rows R >= C)
+  int R = 0, C = 0;
+  const bool has_tile = is_tile && tid < ntiles;
+  if (has_tile) {
+    int ur, uc;
+    tri_tile(ntiles - 1 - tid, ur, uc);      // row-major lower index of the mirrored tile
+    C = T.nT - 1 - ur;
+    R = T.nT - 1 - uc;
+  }
+  const int r0 = 4 * R, c0 = 4 * C, q = C >> 1;
+
+  float tr = 0.f;
   int status = 0;
   for (int attempt = 0; attempt < 2; ++attempt) {
-    const float add = attempt ? 1e-6f * (float)tr / (float)V : 0.f;
-    if (tid == 0) failed_s = 0;
-    // warp w: rows w, w + nw, ...; lanes along the row -- no index division, and the loads of a
-    // row batch (<= 5 x 32 columns, V <= 160) are all in flight before the first store
-    {
-      const int lane = tid & 31, w = tid >> 5, nw = blockDim.x >> 5;
-      for (int x = w; x < V; x += nw) {
-        const float* row = Sigma + (size_t)x * V;
-        float v[5];
+    if (attempt) {                            // jitter scale of reading A4 (only if attempt 0 failed)
+      double t2 = 0.0;
+      for (int x = lane; x < V; x += 32) t2 += (double)Sigma[(size_t)x * V + x];
 #pragma unroll
-        for (int j = 0; j < 5; ++j) v[j] = (lane + 32 * j < V) ? row[lane + 32 * j] : 0.f;
+      for (int o = 16; o > 0; o >>= 1) t2 += __shfl_xor_sync(0xffffffffu, t2, o);
+      tr = (float)t2;
+    }
+    const float add = attempt ? 1e-6f * tr / (float)V : 0.f;
+    if (is_tile) {
+      if (warp >= ntw && attempt == 0)        // idle tile warps: zeros above the diagonal
+        for (int x = warp - ntw; x < V; x += CT_TILE_WARPS - ntw)
+          for (int y = x + 1 + lane; y < V; y += 32) Lc[(size_t)x * V + y] = 0.f;
+      if (warp < ntw) {
+        float a[4][4];
 #pragma unroll
-        for (int j = 0; j < 5; ++j) {
-          const int y = lane + 32 * j;
-          if (y < V) sm[x * P + y] = v[j] + (x == y ? add : 0.f);
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {
+            const int x = r0 + i, y = c0 + j;
+            const float v = Sigma[(size_t)min(x, V - 1) * V + min(y, V - 1)];   // always in range
+            a[i][j] = (x < V && y < V) ? v + (x == y ? add : 0.f) : (x == y ? 1.f : 0.f);
+          }
+        // column blocks 0 and 1 receive no update from a tile warp: publish them right away
+        if (has_tile && q <= 1) {
+          float* dst = &Ap[q][(c0 - 8 * q) * CT_LD + r0];
+#pragma unroll
+          for (int j = 0; j < 4; ++j)
+            *reinterpret_cast<float4*>(dst + j * CT_LD) = make_float4(a[0][j], a[1][j], a[2][j], a[3][j]);
         }
+        if (warp < T.owners(0)) bar_arrive(BAR_AP0, 32 * T.owners(0) + CT_RWT);
+        for (int p = 0; p < nP; ++p) {
+          const int lo1 = T.warp_lo(2 * p + 2), alo = T.warp_lo(2 * p + 4), buf = p & 1;
+          const int nM = 32 * (ntw - lo1) + 32 + CT_RWT;
+          if (warp < alo) {                                   // every tile of this warp is final
+            if (warp >= lo1) bar_arrive(BAR_M + buf, nM);     // (its block p + 1 tiles are in Ap)
+            break;
+          }
+          bar_sync(BAR_M + buf, nM);
+          // update from panel p for the tiles of column blocks >= p + 2
+          if (has_tile && q >= p + 2) {
+            const float* lp = &Lp[buf][0];
+#pragma unroll
+            for (int k = 0; k < CS_NB; ++k) {
+              const float4 lr = *reinterpret_cast<const float4*>(lp + k * CT_LD + r0);
+              const float4 lc = *reinterpret_cast<const float4*>(lp + k * CT_LD + c0);
+              const float lrv[4] = {lr.x, lr.y, lr.z, lr.w}, lcv[4] = {lc.x, lc.y, lc.z, lc.w};
+#pragma unroll
+              for (int i = 0; i < 4; ++i)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) a[i][j] = fmaf(-lrv[i], lcv[j], a[i][j]);
+            }
+          }
+          bar_arrive(BAR_B + (buf ^ 1), 32 * (ntw - alo) + 32 + CT_RWT);   // B(p + 1): Lp[buf] read
+          // column block p + 2 is complete now: publish it (visible through M(p + 1))
+          if (has_tile && q == p + 2) {
+            float* dst = &Ap[q & 1][(c0 - 8 * q) * CT_LD + r0];
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+              *reinterpret_cast<float4*>(dst + j * CT_LD) = make_float4(a[0][j], a[1][j], a[2][j], a[3][j]);
+          }
+        }
+      }
+    } else if (is_row) {
+      const int r = tid - 32 * CT_TILE_WARPS;          // matrix row of this thread (fixed)
+      const bool live = r < CS_NB * nP;                // rows of the matrix padded to whole panels
+      if (r == 0) failed_s = 0;
+      // rows [V, 4 nT) exist in the tiles as identity padding: their L entries are zero
+      if (r >= V) {
+#pragma unroll
+        for (int k = 0; k < 2 * CS_NB; ++k) (&Lp[0][0])[k * CT_LD + r] = 0.f;
+      }
+      float x[CS_NB];
+      bar_sync(BAR_AP0, 32 * T.owners(0) + CT_RWT);
+#pragma unroll
+      for (int k = 0; k < CS_NB; ++k) x[k] = (r < V) ? Ap[0][k * CT_LD + r] : (k == r ? 1.f : 0.f);
+      if (r < CS_NB) {
+#pragma unroll
+        for (int k = 0; k < CS_NB; ++k) Dn[0][k * CS_NB + r] = x[k];
+      }
+      bar_sync(BAR_B_PRO, CT_RWT);
+      for (int p = 0; p < nP; ++p) {
+        const int buf = p & 1, jb = CS_NB * p, ri = r - jb;
+        if (ri >= 0 && live) {
+          const float* dn = &Dn[buf][0];
+          float D[CS_NB][CS_NB];
+#pragma unroll
+          for (int k = 0; k < CS_NB; ++k) {
+            const float4 lo = *reinterpret_cast<const float4*>(dn + k * CS_NB);
+            const float4 hi = *reinterpret_cast<const float4*>(dn + k * CS_NB + 4);
+            D[0][k] = lo.x; D[1][k] = lo.y; D[2][k] = lo.z; D[3][k] = lo.w;
+            D[4][k] = hi.x; D[5][k] = hi.y; D[6][k] = hi.z; D[7][k] = hi.w;
+          }
+          bool bad = false;
+#pragma unroll
+          for (int k = 0; k < CS_NB; ++k) {
+            // pivots below the smallest normal number count as failures (the reciprocal square
+            // root flushes them); 1/sqrt(d) = SFU seed + one Newton step (~1 ulp)
+            const float d0 = D[k][k];
+            const bool ok = d0 >= 1.17549435e-38f;
+            bad |= !ok;
+            const float d = ok ? d0 : 1.f;
+            float inv = rsqrt_ftz(d0);
+            inv = ok ? inv : 1.f;
+            inv = inv * fmaf(-0.5f * d * inv, inv, 1.5f);
+            D[k][k] = d * inv;
+#pragma unroll
+            for (int i = k + 1; i < CS_NB; ++i) D[i][k] *= inv;
+            x[k] *= inv;
+#pragma unroll
+            for (int i = k + 1; i < CS_NB; ++i)
+#pragma unroll
+              for (int c = k + 1; c <= i; ++c) D[i][c] = fmaf(-D[i][k], D[c][k], D[i][c]);
+#pragma unroll
+            for (int c = k + 1; c < CS_NB; ++c) x[c] = fmaf(-x[k], D[c][k], x[c]);
+          }
+          if (bad) failed_s = 1;
+          // rows of the diagonal block: their elimination reproduces the factor; zero above it
+#pragma unroll
+          for (int k = 1; k < CS_NB; ++k) if (k > ri) x[k] = 0.f;
+          float* lp = &Lp[buf][0];
+#pragma unroll
+          for (int k = 0; k < CS_NB; ++k) lp[k * CT_LD + r] = x[k];
+        }
+        const int nM = 32 * (ntw - T.warp_lo(2 * p + 2)) + 32 + CT_RWT;
+        if (p + 1 == nP) { bar_arrive(BAR_M + buf, nM); break; }
+        bar_sync(BAR_M + buf, nM);
+        if (ri >= CS_NB && live) {
+          // own entries of column block p + 1: A (panels < p applied by the tiles) minus panel p
+          const float* lp = &Lp[buf][jb + CS_NB];
+          const float* ap = &Ap[buf ^ 1][0];
+          float xn[CS_NB];
+#pragma unroll
+          for (int c = 0; c < CS_NB; ++c)
+            xn[c] = (r < V) ? ap[c * CT_LD + r] : (c == ri - CS_NB ? 1.f : 0.f);
+#pragma unroll
+          for (int k = 0; k < CS_NB; ++k) {
+            const float4 lo = *reinterpret_cast<const float4*>(lp + k * CT_LD);
+            const float4 hi = *reinterpret_cast<const float4*>(lp + k * CT_LD + 4);
+            const float l[CS_NB] = {lo.x, lo.y, lo.z, lo.w, hi.x, hi.y, hi.z, hi.w};
+#pragma unroll
+            for (int c = 0; c < CS_NB; ++c) xn[c] = fmaf(-x[k], l[c], xn[c]);
+          }
+#pragma unroll
+          for (int c = 0; c < CS_NB; ++c) x[c] = xn[c];
+          if (ri < 2 * CS_NB) {
+#pragma unroll
+            for (int c = 0; c < CS_NB; ++c) Dn[buf ^ 1][c * CS_NB + ri - CS_NB] = x[c];
+          }
+        }
+        // B(p): next diagonal block visible; readers of Lp[buf ^ 1] (panel p - 1) are done
+        bar_sync(BAR_B + buf, CT_RWT + (p >= 1 ? 32 * (ntw - T.warp_lo(2 * p + 2)) + 32 : 0));
+      }
+    } else {
+      // housekeeping warp: L from Lp to Lc panel by panel (and the zeros above the diagonal if
+      // every tile warp holds tiles)
+      if (attempt == 0 && ntw == CT_TILE_WARPS)
+        for (int x = 0; x < V; ++x)
+          for (int y = x + 1 + lane; y < V; y += 32) Lc[(size_t)x * V + y] = 0.f;
+      for (int p = 0; p < nP; ++p) {
+        const int buf = p & 1, jb = CS_NB * p;
+        bar_sync(BAR_M + buf, 32 * (ntw - T.warp_lo(2 * p + 2)) + 32 + CT_RWT);
+        const float* lp = &Lp[buf][0];
+        for (int r = jb + lane; r < V; r += 32) {
+#pragma unroll
+          for (int k = 0; k < CS_NB; ++k)
+            if (jb + k < V && jb + k <= r) Lc[(size_t)r * V + jb + k] = lp[k * CT_LD + r];
+        }
+        if (p + 2 < nP) bar_arrive(BAR_B + (buf ^ 1), 32 * (ntw - T.warp_lo(2 * p + 4)) + 32 + CT_RWT);
       }
     }
     __syncthreads();
-    chol_panels(sm, P, V, &failed_s);
     const int failed = failed_s;
     __syncthreads();
     if (!failed) { status = attempt; break; }
     status = -1;
   }
-  {
-    const int lane = tid & 31, w = tid >> 5, nw = blockDim.x >> 5;
-    for (int x = w; x < V; x += nw)
-      for (int y = lane; y < V; y += 32) Lc[(size_t)x * V + y] = (y <= x) ? sm[x * P + y] : 0.f;
+  if (tid == 0) {
+    ctrl->chol_status = status; ctrl->chol_fail = 0;
+    if (status != 0) ctrl->trace = tr;
   }
-  if (tid == 0) { ctrl->chol_status = status; ctrl->chol_fail = 0; ctrl->trace = (float)tr; }
 }
 
 // ------------------------------------------------------------------ large V: blocked ---------
@@ -458,15 +669,8 @@ __global__ void chol_finalize_kernel(Ctrl* ctrl, int respect_done) {
 
 void launch_cholesky(const float* Sigma, float* Lc, int V, Ctrl* ctrl, int respect_done,
                      cudaStream_t st) {
-  if (V <= 160) {
-    size_t smem = (size_t)V * (V + 1) * sizeof(float);
-    static bool attr_done = false;
-    if (!attr_done) {
-      cudaFuncSetAttribute(chol_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                           160 * 161 * (int)sizeof(float));
-      attr_done = true;
-    }
-    ++g_launches; launch_pdl(chol_small_kernel, 1, CS_THREADS, smem, st, Sigma, Lc, V, ctrl, respect_done);
+  if (V <= CT_LD) {
+    ++g_launches; launch_pdl(chol_small_kernel, 1, CT_THREADS, 0, st, Sigma, Lc, V, ctrl, respect_done);
     return;
   }
   ++g_launches; trace_kernel<<<1, 256, 0, st>>>(Sigma, V, ctrl, respect_done);

@@ -1,5 +1,7 @@
 // population.cu -- the population step P1-P4: next beta by ESS bisection,
 // incremental weights + log Z, exact integer systematic resampling, gather.
+#include <cooperative_groups.h>
+
 #include "kernels.cuh"
 #include "philox.cuh"
 
@@ -86,6 +88,16 @@ __device__ __forceinline__ EssSums ess_sums(const float (&xs)[rw::RC], int cnt,
   return r;
 }
 
+// h(d) = log(a^2 / (b N target)) and h'(d) without FP64 logarithms or divisions: the ratio minus
+// one is formed from an FP64 numerator (exact cancellation near the root) and goes through
+// log1pf, whose error is relative to h itself; h' only steers the iteration.
+__device__ __forceinline__ void ess_h(const EssSums& q, double NT, float& h, float& dh) {
+  const double den = q.b * NT;
+  const double num = q.a * q.a - den;
+  h = log1pf((float)num / (float)den);
+  dh = 2.f * (float)q.da / (float)q.a - (float)q.db / (float)q.b;
+}
+
 template <bool CACHED>
 __device__ __forceinline__ void next_delta_reweight_body(const float* __restrict__ S, int N,
                                                          float ess_target, double delta_fixed,
@@ -96,48 +108,56 @@ __device__ __forceinline__ void next_delta_reweight_body(const float* __restrict
   __shared__ float smin_s[33];
   __shared__ double bcast_x;
   __shared__ int bcast_flags;
+  __shared__ unsigned long long wsum[32];
   float xs[rw::RC];
   int cnt = 0;
   float m = INFINITY;
-  // cached layout: warp w owns the contiguous span [w 32 ipt, (w+1) 32 ipt), lane l its elements
-  // l, l + 32, ...: every load / store instruction covers 32 consecutive entries, and the integer
-  // scan of P3 is a warp scan per row plus a running carry
+  // cached layout: thread t owns the contiguous run [t ipt, (t+1) ipt): 16-byte loads and stores
+  // when the run is whole and aligned, and the integer scan of P3 is a serial prefix per thread
+  // plus ONE warp scan of the run totals
   const int ipt = min(rw::RC, (N + rw::THREADS - 1) / rw::THREADS);
-  const int run0 = (int)(threadIdx.x >> 5) * 32 * ipt + (int)(threadIdx.x & 31);
+  const int run0 = (int)threadIdx.x * ipt;
+  const bool vec = CACHED && (ipt & 3) == 0 && run0 + ipt <= N;
   if (CACHED) {
-    cnt = max(0, min(ipt, (N - run0 + 31) >> 5));
+    cnt = max(0, min(ipt, N - run0));
+    if (vec) {
+      const float4* s4 = reinterpret_cast<const float4*>(S + run0);
 #pragma unroll
-    for (int j = 0; j < rw::RC; ++j) {
-      xs[j] = j < cnt ? S[run0 + 32 * j] : INFINITY;
-      m = fminf(m, xs[j]);
+      for (int j = 0; j < rw::RC / 4; ++j)
+        if (4 * j < ipt) {
+          const float4 v = s4[j];
+          xs[4 * j] = v.x; xs[4 * j + 1] = v.y; xs[4 * j + 2] = v.z; xs[4 * j + 3] = v.w;
+        } else {
+          xs[4 * j] = xs[4 * j + 1] = xs[4 * j + 2] = xs[4 * j + 3] = INFINITY;
+        }
+    } else {
+#pragma unroll
+      for (int j = 0; j < rw::RC; ++j) xs[j] = j < cnt ? S[run0 + j] : INFINITY;
     }
+#pragma unroll
+    for (int j = 0; j < rw::RC; ++j) m = fminf(m, xs[j]);
   } else {
     for (int i = threadIdx.x; i < N; i += rw::THREADS) m = fminf(m, S[i]);
   }
   m = warp_min(m);
   if ((threadIdx.x & 31) == 0) smin_s[threadIdx.x >> 5] = m;
   __syncthreads();
-  if (threadIdx.x < 32) {
-    float v = warp_min(smin_s[threadIdx.x]);
-    if (threadIdx.x == 0) smin_s[32] = v;
-  }
-  __syncthreads();
-  const float smin = smin_s[32];
+  const float smin = warp_min(smin_s[threadIdx.x & 31]);    // every warp reduces the 32 minima
   if (CACHED) {
 #pragma unroll
     for (int j = 0; j < rw::RC; ++j) xs[j] -= smin;
   }
   const double beta = ctrl->beta;
   const double rest = 1.0 - beta;
-  const double ltarget = log((double)ess_target), lN = log((double)N);
+  const double NT = (double)N * (double)ess_target, lN = log((double)N);
   double delta;
   int final_step = 0;
   if (delta_fixed >= 0.0) {
     delta = delta_fixed;
     final_step = (beta + delta >= 1.0);
   } else {
-    // thread 0 owns the bracket and the Newton step (FP64 logs and divisions once, not 1024
-    // times); the next abscissa and the stop flag go through shared memory
+    // thread 0 owns the bracket and the Newton step; the next abscissa and the stop flag go
+    // through shared memory
     double lo = 0.0, hi = rest;
     bool hi_known = false;                           // sign of h(rest) not evaluated yet
     const double prev = ctrl->delta;
@@ -148,17 +168,17 @@ __device__ __forceinline__ void next_delta_reweight_body(const float* __restrict
       if (threadIdx.x == 0) {
         int stop = 0, fin = 0;
         double xn = x;
-        const double h = 2.0 * log(q.a) - log(q.b) - lN - ltarget;
+        float h, dh;
+        ess_h(q, NT, h, dh);
         if (x >= rest && !hi_known) {
-          if (h >= 0.0) { stop = 1; fin = 1; xn = rest; }
+          if (h >= 0.f) { stop = 1; fin = 1; xn = rest; }
           hi_known = true;
         }
         if (!stop) {
-          if (h > 0.0) lo = x; else hi = x;
-          if (fabs(h) < 1e-9) stop = 1;
+          if (h > 0.f) lo = x; else hi = x;
+          if (fabsf(h) < 1e-9f) stop = 1;
           else {
-            const double dh = 2.0 * q.da / q.a - q.db / q.b;
-            xn = x - h / dh;
+            xn = x - (double)(h / dh);
             if (!(xn > lo && xn < hi)) {
               if (!hi_known && xn >= hi) xn = rest;      // probe the end of the interval
               else if (hi_known) xn = 0.5 * (lo + hi);
@@ -179,55 +199,26 @@ __device__ __forceinline__ void next_delta_reweight_body(const float* __restrict
   }
   const float df = (float)delta;
   double a = 0.0, b = 0.0;
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  unsigned long long run = 0;
   if (CACHED) {
-    unsigned long long run = 0;
 #pragma unroll
     for (int j = 0; j < rw::RC; ++j)
       if (j < cnt) {
         const float e = expf(-df * xs[j]);
         xs[j] = e;                                   // kept for the scan below
-        w[run0 + 32 * j] = e;
         a += (double)e;
         b += (double)e * (double)e;
         run += quantise40(e);
       }
-    if (C) {
-      // P3 fused (reading R5): inclusive integer scan of q_i = floor(w_i 2^40).  Warp totals ->
-      // exclusive offsets of the warp spans; inside a span, one warp scan per row of 32.
-      __shared__ unsigned long long wsum[32];
-      const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-      unsigned long long tot = run;
+    if (vec) {
+      float4* w4 = reinterpret_cast<float4*>(w + run0);
 #pragma unroll
-      for (int o = 16; o > 0; o >>= 1) tot += __shfl_xor_sync(0xffffffffu, tot, o);
-      if (lane == 0) wsum[wid] = tot;
-      __syncthreads();
-      if (wid == 0) {
-        unsigned long long v = wsum[lane], sc = v;
+      for (int j = 0; j < rw::RC / 4; ++j)
+        if (4 * j < ipt) w4[j] = make_float4(xs[4 * j], xs[4 * j + 1], xs[4 * j + 2], xs[4 * j + 3]);
+    } else {
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-          unsigned long long u = __shfl_up_sync(0xffffffffu, sc, o);
-          if (lane >= o) sc += u;
-        }
-        wsum[lane] = sc - v;  // exclusive
-      }
-      __syncthreads();
-      unsigned long long carry = wsum[wid];
-#pragma unroll
-      for (int j = 0; j < rw::RC; ++j)
-        if (j < ipt) {                               // block-uniform bound: shuffles stay convergent
-          unsigned long long inc = j < cnt ? quantise40(xs[j]) : 0ull;
-#pragma unroll
-          for (int o = 1; o < 32; o <<= 1) {
-            unsigned long long v = __shfl_up_sync(0xffffffffu, inc, o);
-            if (lane >= o) inc += v;
-          }
-          if (j < cnt) C[run0 + 32 * j] = carry + inc;
-          carry += __shfl_sync(0xffffffffu, inc, 31);
-        }
-      if (threadIdx.x == rw::THREADS - 1) {
-        ctrl->q_total = carry;
-        if (carry == 0ull) ctrl->nan_flag = 1;
-      }
+      for (int j = 0; j < rw::RC; ++j) if (j < cnt) w[run0 + j] = xs[j];
     }
   } else {
     for (int i = threadIdx.x; i < N; i += rw::THREADS) {
@@ -237,22 +228,54 @@ __device__ __forceinline__ void next_delta_reweight_body(const float* __restrict
       b += (double)e * (double)e;
     }
   }
-  {
-    const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5;
-    a = warp_sum(a);
-    b = warp_sum(b);
-    __syncthreads();
-    if (lane == 0) scratch[wi] = make_double4(a, b, 0.0, 0.0);
-    __syncthreads();
-    if (wi == 0) {
-      double4 t = scratch[lane];
-      t.x = warp_sum(t.x);
-      t.y = warp_sum(t.y);
-      if (lane == 0) scratch[32] = t;
+  // one round for both block reductions: sum w, sum w^2, and (P3 fused, reading R5) the
+  // inclusive integer scan of the run totals q = sum floor(w_i 2^40)
+  unsigned long long inc = run;
+  if (CACHED && C) {
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      unsigned long long v = __shfl_up_sync(0xffffffffu, inc, o);
+      if (lane >= o) inc += v;
     }
-    __syncthreads();
-    a = scratch[32].x;
-    b = scratch[32].y;
+    if (lane == 31) wsum[wid] = inc;
+  }
+  a = warp_sum(a);
+  b = warp_sum(b);
+  if (lane == 0) scratch[wid] = make_double4(a, b, 0.0, 0.0);
+  __syncthreads();
+  {
+    double4 t = scratch[lane];                       // every warp reduces the 32 partial sums
+    a = warp_sum(t.x);
+    b = warp_sum(t.y);
+  }
+  if (CACHED && C) {
+    unsigned long long v = wsum[lane], sc = v;       // ... and scans the 32 warp totals
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      unsigned long long u = __shfl_up_sync(0xffffffffu, sc, o);
+      if (lane >= o) sc += u;
+    }
+    const unsigned long long warp_off = __shfl_sync(0xffffffffu, sc - v, wid);
+    unsigned long long pre = warp_off + inc - run;
+    if (vec) {
+      ulonglong2* C2 = reinterpret_cast<ulonglong2*>(C + run0);
+#pragma unroll
+      for (int j = 0; j < rw::RC / 2; ++j)
+        if (2 * j < ipt) {
+          ulonglong2 c;
+          pre += quantise40(xs[2 * j]); c.x = pre;
+          pre += quantise40(xs[2 * j + 1]); c.y = pre;
+          C2[j] = c;
+        }
+    } else {
+#pragma unroll
+      for (int j = 0; j < rw::RC; ++j)
+        if (j < cnt) { pre += quantise40(xs[j]); C[run0 + j] = pre; }
+    }
+    if (threadIdx.x == rw::THREADS - 1) {
+      ctrl->q_total = pre;
+      if (pre == 0ull) ctrl->nan_flag = 1;
+    }
   }
   if (threadIdx.x == 0) {
     double dlz = -delta * (double)smin + log(a) - lN;
@@ -276,12 +299,254 @@ next_delta_reweight_kernel(const float* __restrict__ S, int N, float ess_target,
   else next_delta_reweight_body<false>(S, N, ess_target, delta_fixed, w, nullptr, ctrl);
 }
 
+// ---------------------------------------------------------------------------------------------
+// P1 + P2 (+ the integer scan of P3) for N <= 16384 on a CLUSTER of 8 CTAs.  One CTA holding all
+// 16384 actions spends ~2000 cycles per Newton evaluation on instruction issue alone (16 actions
+// x 7 instructions x 32 warps on one SM).  Here CTA c of the cluster holds the contiguous chunk
+// [c chunk, (c+1) chunk), 8 actions per thread in registers; per evaluation every warp writes
+// its four partial sums into the shared memory of ALL eight CTAs (distributed shared memory),
+// one cluster barrier, and every thread reduces the 64 partials in the same fixed order and takes
+// the Newton step itself: the same numbers in every thread of every CTA, no broadcast.
+// Same algorithm (reading R3) and the same stopping rule as next_delta_reweight_body.
+// ---------------------------------------------------------------------------------------------
+namespace rwc {
+constexpr int G = 8, THREADS = 256, WARPS = THREADS / 32, RC = 8, NP = G * WARPS;   // 64 partials
+}
+
+__device__ __forceinline__ double4 rwc_reduce64(const double4* slot, int lane) {
+  const double4 u = slot[lane], v = slot[lane + 32];
+  double4 t = make_double4(u.x + v.x, u.y + v.y, u.z + v.z, u.w + v.w);
+  t.x = warp_sum(t.x); t.y = warp_sum(t.y); t.z = warp_sum(t.z); t.w = warp_sum(t.w);
+  return t;
+}
+
+__global__ void __launch_bounds__(rwc::THREADS)
+next_delta_reweight_cluster_kernel(const float* __restrict__ S, int N, float ess_target,
+                                   double delta_fixed, float* __restrict__ w,
+                                   unsigned long long* __restrict__ C, Ctrl* ctrl) {
+  namespace cg = cooperative_groups;
+  pdl_enter();
+  __shared__ __align__(32) double4 slot[2][rwc::NP];       // partial sums, double-buffered by evaluation
+  __shared__ unsigned long long qslot[rwc::NP];            // integer totals of the warps (P3)
+  __shared__ float cmin[rwc::G];
+  __shared__ float wmin[rwc::WARPS];
+  if (ctrl->done) return;                                  // (uniform over the cluster)
+  cg::cluster_group cluster = cg::this_cluster();
+  const int rank = (int)cluster.block_rank();
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  const int ipt = (N + rwc::G * rwc::THREADS - 1) / (rwc::G * rwc::THREADS);      // <= 8
+  const int run0 = (rank * rwc::THREADS + tid) * ipt;
+  const int cnt = max(0, min(ipt, N - run0));
+  const bool vec = (ipt & 3) == 0 && run0 + ipt <= N;
+  float xs[rwc::RC];
+  if (vec) {
+    const float4* s4 = reinterpret_cast<const float4*>(S + run0);
+#pragma unroll
+    for (int j = 0; j < rwc::RC / 4; ++j)
+      if (4 * j < ipt) {
+        const float4 v = s4[j];
+        xs[4 * j] = v.x; xs[4 * j + 1] = v.y; xs[4 * j + 2] = v.z; xs[4 * j + 3] = v.w;
+      } else {
+        xs[4 * j] = xs[4 * j + 1] = xs[4 * j + 2] = xs[4 * j + 3] = INFINITY;
+      }
+  } else {
+#pragma unroll
+    for (int j = 0; j < rwc::RC; ++j) xs[j] = j < cnt ? S[run0 + j] : INFINITY;
+  }
+  float m = INFINITY;
+#pragma unroll
+  for (int j = 0; j < rwc::RC; ++j) m = fminf(m, xs[j]);
+  m = warp_min(m);
+  if (lane == 0) wmin[wid] = m;
+  __syncthreads();
+  if (tid < rwc::G) {                                      // thread g: this CTA's minimum to CTA g
+    float v = wmin[0];
+#pragma unroll
+    for (int k = 1; k < rwc::WARPS; ++k) v = fminf(v, wmin[k]);
+    *cluster.map_shared_rank(&cmin[rank], tid) = v;
+  }
+  cluster.sync();
+  float smin = cmin[0];
+#pragma unroll
+  for (int g = 1; g < rwc::G; ++g) smin = fminf(smin, cmin[g]);
+#pragma unroll
+  for (int j = 0; j < rwc::RC; ++j) xs[j] -= smin;
+
+  const double beta = ctrl->beta;
+  const double rest = 1.0 - beta;
+  const double NT = (double)N * (double)ess_target, lN = log((double)N);
+  double delta;
+  int final_step = 0;
+  int par = 0;
+  if (delta_fixed >= 0.0) {
+    delta = delta_fixed;
+    final_step = (beta + delta >= 1.0);
+  } else {
+    double lo = 0.0, hi = rest;
+    bool hi_known = false;
+    const double prev = ctrl->delta;
+    double x = (prev > 0.0 && prev < rest) ? prev : rest;
+    delta = rest;
+    for (int it = 0; it < 64; ++it) {
+      const float df = (float)x * 1.4426950408889634f;
+      float a = 0.f, b = 0.f, da = 0.f, db = 0.f;
+#pragma unroll
+      for (int j = 0; j < rwc::RC; ++j)
+        if (j < cnt) {
+          float e;
+          asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(-df * xs[j]));
+          const float e2 = e * e;
+          a += e; b += e2;
+          da = fmaf(xs[j], e, da); db = fmaf(xs[j], e2, db);
+        }
+      double4 t = make_double4(warp_sum((double)a), warp_sum((double)b), warp_sum((double)da),
+                               warp_sum((double)db));
+      if (lane < rwc::G) *cluster.map_shared_rank(&slot[par][rank * rwc::WARPS + wid], lane) = t;
+      cluster.sync();
+      t = rwc_reduce64(slot[par], lane);
+      par ^= 1;
+      EssSums q{t.x, t.y, -t.z, -2.0 * t.w};
+      int stop = 0, fin = 0;
+      double xn = x;
+      float h, dh;
+      ess_h(q, NT, h, dh);
+      if (x >= rest && !hi_known) {
+        if (h >= 0.f) { stop = 1; fin = 1; xn = rest; }
+        hi_known = true;
+      }
+      if (!stop) {
+        if (h > 0.f) lo = x; else hi = x;
+        if (fabsf(h) < 1e-9f) stop = 1;
+        else {
+          xn = x - (double)(h / dh);
+          if (!(xn > lo && xn < hi)) {
+            if (!hi_known && xn >= hi) xn = rest;
+            else if (hi_known) xn = 0.5 * (lo + hi);
+            else xn = fmin(rest, 2.0 * x);
+          }
+          if (fabs(xn - x) <= 1e-7 * xn && !(xn >= rest && !hi_known)) stop = 1;
+        }
+      }
+      x = xn;
+      delta = x;
+      final_step = fin;
+      if (stop) break;
+    }
+  }
+  // P2: weights, their sums, and (P3, reading R5) the integer scan of q_i = floor(w_i 2^40)
+  const float df = (float)delta;
+  double a = 0.0, b = 0.0;
+  unsigned long long run = 0;
+#pragma unroll
+  for (int j = 0; j < rwc::RC; ++j)
+    if (j < cnt) {
+      const float e = expf(-df * xs[j]);
+      xs[j] = e;
+      a += (double)e;
+      b += (double)e * (double)e;
+      run += quantise40(e);
+    }
+  if (vec) {
+    float4* w4 = reinterpret_cast<float4*>(w + run0);
+#pragma unroll
+    for (int j = 0; j < rwc::RC / 4; ++j)
+      if (4 * j < ipt) w4[j] = make_float4(xs[4 * j], xs[4 * j + 1], xs[4 * j + 2], xs[4 * j + 3]);
+  } else {
+#pragma unroll
+    for (int j = 0; j < rwc::RC; ++j) if (j < cnt) w[run0 + j] = xs[j];
+  }
+  unsigned long long inc = run;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    unsigned long long v = __shfl_up_sync(0xffffffffu, inc, o);
+    if (lane >= o) inc += v;
+  }
+  const unsigned long long wtot = __shfl_sync(0xffffffffu, inc, 31);
+  {
+    const double4 t = make_double4(warp_sum(a), warp_sum(b), 0.0, 0.0);
+    const int me = rank * rwc::WARPS + wid;
+    if (lane < rwc::G) {
+      *cluster.map_shared_rank(&slot[par][me], lane) = t;
+      *cluster.map_shared_rank(&qslot[me], lane) = wtot;
+    }
+  }
+  cluster.sync();
+  {
+    const double4 t = rwc_reduce64(slot[par], lane);
+    a = t.x; b = t.y;
+  }
+  if (C) {
+    // exclusive prefix of the 64 warp totals at this warp's position (warps are numbered in
+    // element order: rank-major), then the serial prefix inside the thread's run
+    const int me = rank * rwc::WARPS + wid;
+    const unsigned long long q0 = qslot[lane], q1 = qslot[lane + 32];
+    unsigned long long part = (lane < me ? q0 : 0ull) + (lane + 32 < me ? q1 : 0ull);
+    unsigned long long tot = q0 + q1;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      part += __shfl_xor_sync(0xffffffffu, part, o);
+      tot += __shfl_xor_sync(0xffffffffu, tot, o);
+    }
+    unsigned long long pre = part + inc - run;
+    if (vec) {
+      ulonglong2* C2 = reinterpret_cast<ulonglong2*>(C + run0);
+#pragma unroll
+      for (int j = 0; j < rwc::RC / 2; ++j)
+        if (2 * j < ipt) {
+          ulonglong2 c;
+          pre += quantise40(xs[2 * j]); c.x = pre;
+          pre += quantise40(xs[2 * j + 1]); c.y = pre;
+          C2[j] = c;
+        }
+    } else {
+#pragma unroll
+      for (int j = 0; j < rwc::RC; ++j)
+        if (j < cnt) { pre += quantise40(xs[j]); C[run0 + j] = pre; }
+    }
+    if (rank == 0 && tid == 0) {
+      ctrl->q_total = tot;
+      if (tot == 0ull) ctrl->nan_flag = 1;
+    }
+  }
+  if (rank == 0 && tid == 0) {
+    double dlz = -delta * (double)smin + log(a) - lN;
+    ctrl->delta = delta;
+    ctrl->beta = final_step ? 1.0 : beta + delta;
+    ctrl->ess_frac = a * a / (b * (double)N);
+    ctrl->dlogZ = dlz;
+    ctrl->logZ += dlz;
+    ctrl->S_min = smin;
+    if (!isfinite(dlz)) ctrl->nan_flag = 1;
+  }
+  cluster.sync();          // no CTA exits while another may still write into its shared memory
+}
+
+template <typename... KArgs, typename... Args>
+static cudaError_t launch_pdl_cluster(void (*kernel)(KArgs...), int cluster, int threads, cudaStream_t st,
+                                      Args&&... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(cluster); cfg.blockDim = dim3(threads); cfg.dynamicSmemBytes = 0; cfg.stream = st;
+  cudaLaunchAttribute at[2];
+  at[0].id = cudaLaunchAttributeClusterDimension;
+  at[0].val.clusterDim.x = cluster; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+  at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[1].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = pdl_enabled() ? 2 : 1;
+  return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
 // C != nullptr and N <= 16384: the integer scan of P3 runs in the same kernel (the weights are
 // still in registers); returns whether it did, so that the caller can skip launch_quantise_scan.
 bool launch_next_delta_reweight(const float* S, int N, float ess_target, double delta_fixed,
                                 float* w, unsigned long long* C, Ctrl* ctrl, cudaStream_t st) {
   const bool fused = C != nullptr && N <= rw::THREADS * rw::RC;
   ++g_launches;
+  if (N <= rwc::G * rwc::THREADS * rwc::RC) {
+    launch_pdl_cluster(next_delta_reweight_cluster_kernel, rwc::G, rwc::THREADS, st, S, N, ess_target,
+                       delta_fixed, w, C, ctrl);
+    return fused;
+  }
   launch_pdl(next_delta_reweight_kernel, 1, rw::THREADS, 0, st, S, N, ess_target, delta_fixed, w,
              fused ? C : (unsigned long long*)nullptr, ctrl);
   return fused;
