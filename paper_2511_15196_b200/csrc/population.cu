@@ -712,26 +712,69 @@ void launch_quantise_scan(const float* w, int N, unsigned long long* C, Ctrl* ct
 // identity, so that a step enqueued past beta = 1 leaves the particles unchanged.
 // flip[j] (NEXT row f4, reading A17): with z2 set, slot j is sign-flipped by the gather iff the top
 // bit of word 0 of the Z2 stream at this temperature is set.
+// t_j exactly, without a 128-bit division: (P T) >> 32 is a 74-bit number (P < 2^49, T < 2^57);
+// long division by N in base 2^32 (N < 2^21, so every partial remainder fits 64 bits).
+__device__ __forceinline__ unsigned long long resample_threshold(int j, uint32_t U, unsigned long long T,
+                                                                 int N) {
+  const unsigned long long P = ((unsigned long long)j << 32) + U;
+  const unsigned long long lo = P * T, hi = __umul64hi(P, T);
+  const unsigned long long x2 = hi >> 32, x1 = hi & 0xffffffffull, x0 = lo >> 32;
+  const unsigned long long n = (unsigned long long)N;
+  unsigned long long r = x2 % n;                    // (x2 / n = 0: t_j < T < 2^64)
+  r = (r << 32) + x1;
+  const unsigned long long q1 = r / n;
+  r = ((r % n) << 32) + x0;
+  return (q1 << 32) + r / n;
+}
+
+// a_j for K consecutive slots j0 .. j0+K-1 (slots >= N: -1): K binary searches in lock step, so
+// that their loads overlap
+template <int K>
+__device__ __forceinline__ void ancestors_of(const unsigned long long* __restrict__ C, int N, uint64_t seed,
+                                             const Ctrl* ctrl, int j0, int (&a)[K]) {
+  const unsigned long long T = ctrl->q_total;
+  if (ctrl->done || T == 0ull) {
+#pragma unroll
+    for (int m = 0; m < K; ++m) a[m] = (j0 + m >= 0 && j0 + m < N) ? j0 + m : -1;
+    return;
+  }
+  const uint32_t U = philox_draw(seed, TAG_RESAMPLE, (uint32_t)ctrl->temp_index, 0u, 0u).x;
+  unsigned long long t[K];
+  int lo[K], hi[K];
+#pragma unroll
+  for (int m = 0; m < K; ++m) {
+    const bool in = j0 + m >= 0 && j0 + m < N;
+    t[m] = in ? resample_threshold(j0 + m, U, T, N) : 0ull;
+    lo[m] = 0; hi[m] = in ? N : 0;                  // first index with C > t
+  }
+  for (int span = N; span > 0; span >>= 1) {        // ceil(log2(N + 1)) halvings bound every search
+#pragma unroll
+    for (int m = 0; m < K; ++m) {
+      const int mid = (lo[m] + hi[m]) >> 1;
+      if (lo[m] < hi[m]) {
+        if (C[mid] <= t[m]) lo[m] = mid + 1; else hi[m] = mid;
+      }
+    }
+  }
+#pragma unroll
+  for (int m = 0; m < K; ++m) a[m] = (j0 + m >= 0 && j0 + m < N) ? min(lo[m], N - 1) : -1;
+}
+
+__device__ __forceinline__ uint8_t z2_flip_of(uint64_t seed, const Ctrl* ctrl, int j, int z2) {
+  if (!z2 || ctrl->done || ctrl->q_total == 0ull) return 0;
+  return (uint8_t)(philox_draw(seed, TAG_Z2, (uint32_t)ctrl->temp_index, (uint32_t)j, 0u).x >> 31);
+}
+
 __global__ void ancestors_kernel(const unsigned long long* __restrict__ C, int N, uint64_t seed,
                                  int32_t* __restrict__ anc, uint8_t* __restrict__ flip, int z2,
                                  const Ctrl* ctrl) {
   pdl_enter();
   int j = blockIdx.x * blockDim.x + threadIdx.x;
   if (j >= N) return;
-  if (ctrl->done || ctrl->q_total == 0ull) { anc[j] = j; flip[j] = 0; return; }
-  flip[j] = z2 ? (uint8_t)(philox_draw(seed, TAG_Z2, (uint32_t)ctrl->temp_index, (uint32_t)j, 0u).x >> 31)
-               : (uint8_t)0;
-  const uint32_t U = philox_draw(seed, TAG_RESAMPLE, (uint32_t)ctrl->temp_index, 0u, 0u).x;
-  const unsigned long long T = ctrl->q_total;
-  unsigned __int128 num = (unsigned __int128)(((unsigned long long)j << 32) + U) *
-                          (unsigned __int128)T;
-  unsigned long long tj = (unsigned long long)(num / ((unsigned __int128)((unsigned long long)N << 32)));
-  int lo = 0, hi = N;  // first index with C > tj
-  while (lo < hi) {
-    int mid = (lo + hi) >> 1;
-    if (C[mid] <= tj) lo = mid + 1; else hi = mid;
-  }
-  anc[j] = min(lo, N - 1);
+  int a[1];
+  ancestors_of<1>(C, N, seed, ctrl, j, a);
+  anc[j] = a[0];
+  flip[j] = z2_flip_of(seed, ctrl, j, z2);
 }
 
 void launch_ancestors(const unsigned long long* C, int N, uint64_t seed, int32_t* anc, uint8_t* flip,
