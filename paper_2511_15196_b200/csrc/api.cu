@@ -68,7 +68,8 @@ struct phi4smc {
   int64_t iter_base;         // NS: iters_enqueued - ctrl->temp_index after a set_state
   int known_done;
   Ctrl* h_ctrl;              // pinned staging
-  Ctrl* h_poll;              // pinned, 2 slots: smc_run / ns_run poll one step behind the GPU
+  Ctrl* h_poll;              // pinned, 2 slots: ns_run polls one step behind the GPU
+  HostPoll* h_hp;            // pinned, written by the device at the end of every SMC temperature
   cudaEvent_t poll_ev[2];
   // side stream (fork / join by events on the caller's stream; host resources only): nested
   // sampling runs the dead-point selection beside the covariance chain, the large-V mutation draws
@@ -238,6 +239,8 @@ PHI4_API size_t ns_workspace_bytes(int L, int n_live, int k_delete, int max_iter
 static int host_staging(phi4smc* h) {
   CU(cudaMallocHost((void**)&h->h_ctrl, sizeof(Ctrl)));
   CU(cudaMallocHost((void**)&h->h_poll, 2 * sizeof(Ctrl)));
+  CU(cudaMallocHost((void**)&h->h_hp, sizeof(HostPoll)));
+  memset(h->h_hp, 0, sizeof(HostPoll));
   for (int e = 0; e < 2; ++e) CU(cudaEventCreateWithFlags(&h->poll_ev[e], cudaEventDisableTiming));
   {
     CU(cudaStreamCreateWithFlags(&h->side, cudaStreamNonBlocking));
@@ -352,6 +355,7 @@ PHI4_API int smc_destroy(phi4smc* h) {
   cudaStreamSynchronize(h->st);
   if (h->h_ctrl) cudaFreeHost(h->h_ctrl);
   if (h->h_poll) cudaFreeHost(h->h_poll);
+  if (h->h_hp) cudaFreeHost(h->h_hp);
   for (int e = 0; e < 2; ++e) if (h->poll_ev[e]) cudaEventDestroy(h->poll_ev[e]);
   if (h->side) { cudaStreamSynchronize(h->side); cudaStreamDestroy(h->side); }
   if (h->fork_ev) cudaEventDestroy(h->fork_ev);
@@ -449,9 +453,14 @@ static void enqueue_smc_step(phi4smc* h) {
                                                   h->C, h->ctrl, h->st);
   enqueue_resample(h, scanned);
   launch_cov_chol(cov_args(h, 1), h->st);
-  enqueue_mutation(h, smc_mutate_args(h, h->prm.k_steps, nullptr, nullptr, 1));
+  MutateArgs a = smc_mutate_args(h, h->prm.k_steps, nullptr, nullptr, 1);
+  // the fused tcgen05 mutation closes the temperature itself (its last CTA); the other mutation
+  // paths are several launches, so the step is closed by a kernel of its own
+  const bool fused_finish = h->prm.kernel == 0 && use_tc_path(h);
+  if (fused_finish) { a.finish_rec = h->rec; a.finish_max_rec = h->max_rec; a.finish_poll = h->h_hp; }
+  enqueue_mutation(h, a);
   h->step_counter += (uint64_t)h->prm.k_steps;
-  launch_finish_step(h->ctrl, h->rec, h->max_rec, h->prm.k_steps, h->N, h->st);
+  if (!fused_finish) launch_finish_step(h->ctrl, h->rec, h->max_rec, h->prm.k_steps, h->N, h->h_hp, h->st);
 }
 
 static void fill_info(const StepRecord& r, smc_step_info* info) {
@@ -524,7 +533,30 @@ PHI4_API int smc_run(phi4smc* h, int max_temps, int* n_temps) {
   if (rc != PHI4_OK) return rc;
   const int start = h->h_ctrl->temp_index;
   int enq = 0;
-  rc = run_pipelined(h, max_temps, &enq, enqueue_smc_step);
+  // The device reports every finished temperature in pinned host memory (HostPoll): no copy or
+  // event sits in the stream between two temperatures.  Keep one step queued behind the one
+  // whose report the host is waiting for.
+  volatile HostPoll* hp = h->h_hp;
+  hp->seq = start; hp->done = h->h_ctrl->done; hp->nan_flag = h->h_ctrl->nan_flag;
+  hp->chol_status = h->h_ctrl->chol_status;
+  if (h->h_ctrl->done) h->known_done = 1;
+  while (!h->known_done && enq < max_temps) {
+    enqueue_smc_step(h);
+    ++enq;
+    if (enq >= 2) {
+      const int target = start + enq - 1;        // the step before the one just enqueued
+      for (unsigned spin = 1; hp->seq < target && !hp->done; ++spin) {
+        if ((spin & 1023u) == 0) {               // a dead stream must not hang the host
+          cudaError_t q = cudaStreamQuery(h->st);
+          if (q == cudaSuccess) break;
+          if (q != cudaErrorNotReady) { snprintf(h->err, sizeof(h->err), "smc_run: %s", cudaGetErrorString(q)); return PHI4_ECUDA; }
+        }
+      }
+      if (hp->done) h->known_done = 1;
+      if (hp->nan_flag || hp->chol_status < 0) break;
+    }
+  }
+  rc = sync_ctrl(h);
   // (steps enqueued past beta = 1 were no-ops; sync_ctrl took the step counter from the device)
   const int made = h->h_ctrl->temp_index - start;
   (void)enq;

@@ -37,6 +37,7 @@ struct Ctrl {
   unsigned int n_unique;  // distinct ancestors of the last resampling
   unsigned long long q_total;  // T of reading R5
   unsigned long long mut_steps;  // SMC: mutation steps of the transitions completed since init / reset / restore
+  unsigned int cta_done;  // CTAs of the fused mutation kernel that have finished (the last one closes the step)
 };
 
 // One record per temperature / iteration, written by the device at the end of each step.
@@ -44,6 +45,37 @@ struct StepRecord {
   double beta, delta, ess_frac, dlogZ, logZ, accept_rate;   // NS: logX, logZ, S_star, acc, rem
   int n_unique, chol_status, index, done;
 };
+
+// What the host needs to see of a finished temperature, written by the device straight into
+// pinned host memory (seq last, after a system-wide fence): the run loop polls it without a
+// copy in the stream, so the kernels of consecutive temperatures stay chained.
+struct HostPoll { int seq, done, nan_flag, chol_status; };
+
+// End of a temperature (one thread): record it, advance the index, latch done at beta == 1.
+__device__ __forceinline__ void finish_step_device(Ctrl* ctrl, StepRecord* rec, int max_rec, int k, int N,
+                                                   HostPoll* hp) {
+  int t = ctrl->temp_index;
+  if (t < max_rec) {
+    StepRecord r;
+    r.beta = ctrl->beta; r.delta = ctrl->delta; r.ess_frac = ctrl->ess_frac;
+    r.dlogZ = ctrl->dlogZ; r.logZ = ctrl->logZ;
+    r.accept_rate = (double)ctrl->n_accept / ((double)k * (double)N);
+    r.n_unique = (int)ctrl->n_unique; r.chol_status = ctrl->chol_status;
+    r.index = t; r.done = ctrl->beta >= 1.0;
+    rec[t] = r;
+  }
+  ctrl->temp_index = t + 1;
+  ctrl->mut_steps += (unsigned long long)k;   // steps enqueued past beta = 1 never get here
+  ctrl->n_accept = 0u;
+  ctrl->n_unique = 0u;
+  if (ctrl->beta >= 1.0) ctrl->done = 1;
+  if (hp) {
+    volatile HostPoll* v = hp;
+    v->done = ctrl->done; v->nan_flag = ctrl->nan_flag; v->chol_status = ctrl->chol_status;
+    __threadfence_system();
+    v->seq = t + 1;
+  }
+}
 
 // kappa: coefficient of the kinetic term (1 = Eq. 1; Eq. 2 scales it, reading A18).
 // With kappa = 1 every kernel computes bit-for-bit what it computed before the field existed.

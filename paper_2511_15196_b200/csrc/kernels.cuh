@@ -41,6 +41,11 @@ struct MutateArgs {
   float* Z2;
   cudaStream_t side;
   cudaEvent_t fork_ev, join_ev;
+  // Fused tcgen05 path only: if set, the last CTA to finish closes the temperature itself
+  // (finish_step_device) and the caller launches no finish_step_kernel.
+  StepRecord* finish_rec = nullptr;
+  int finish_max_rec = 0;
+  HostPoll* finish_poll = nullptr;
 };
 void launch_mutate_generic(const MutateArgs& a, float* Lsplit, cudaStream_t st);
 void launch_accept_step(const MutateArgs& a, int j, cudaStream_t st);
@@ -79,7 +84,7 @@ void launch_ancestors(const unsigned long long* C, int N, uint64_t seed, int32_t
 void launch_gather(const float* phi_in, float* phi_out, const float* S_in, float* S_out,
                    const float* U_in, float* U_out, const int32_t* anc, const uint8_t* flip, int N,
                    int ld, int V, Ctrl* ctrl, cudaStream_t st);
-void launch_finish_step(Ctrl* ctrl, StepRecord* rec, int max_rec, int k, int N, cudaStream_t st);
+void launch_finish_step(Ctrl* ctrl, StepRecord* rec, int max_rec, int k, int N, HostPoll* hp, cudaStream_t st);
 
 // covchol.cu -- C1, C2
 struct CovCholArgs {

@@ -75,6 +75,9 @@ struct TcParams {
   uint32_t tag_prop, tag_acc, t0;
   int k, respect_done;
   PhiloxKeys rk;               // round keys of `seed` (constant-bank operands of the Philox XORs)
+  StepRecord* finish_rec;      // not null: the last CTA closes the temperature (finish_step_device)
+  int finish_max_rec;
+  HostPoll* finish_poll;
 };
 
 // (s Lc) -> hi/lo TF32 split in the layout the MMA reads.  K-step ks is a block of two 16-byte
@@ -450,7 +453,7 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
       float dS = 0.f, dU = 0.f;
       tc_stencil<LT>(cur, oth, g, L, hm, lam, kap, dS, dU);
       part[g * TILE + pr] = make_float2(dS, dU);
-      if (g == 0) lus[pr] = log_uniform(p.seed, p.tag_acc, p.t0 + (uint32_t)t, (uint32_t)i);
+      if (g == EPI_PARTS - 1) lus[pr] = log_uniform(p.seed, p.tag_acc, p.t0 + (uint32_t)t, (uint32_t)i);
       named_bar_sync(1 + Q, 32 * EPI_PARTS);
       // every part sums the four partials in the same order and takes the same decision (M4)
       dS = 0.f; dU = 0.f;
@@ -491,11 +494,21 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) nacc += __shfl_xor_sync(0xffffffffu, nacc, o);
       if (lane == 0 && nacc) atomicAdd(&p.ctrl->n_accept, nacc);
+      if (lane == 0) __threadfence();
     }
   }
   tc_fence_before();
   __syncthreads();
   if (warp == 0) tmem_dealloc(taddr, ncols);
+  if (p.finish_rec && threadIdx.x == 0) {
+    // the CTA that counts in last has seen every other CTA's acceptances (fence, then counter)
+    __threadfence();
+    if (atomicAdd(&p.ctrl->cta_done, 1u) == gridDim.x - 1) {
+      __threadfence();
+      p.ctrl->cta_done = 0u;
+      finish_step_device(p.ctrl, p.finish_rec, p.finish_max_rec, p.k, p.N, p.finish_poll);
+    }
+  }
 }
 
 bool mutate_tc_supported(int V) {
@@ -523,6 +536,7 @@ void launch_mutate_tc(const MutateArgs& a, float* Lsplit, cudaStream_t st) {
   p.m0sq = a.md.m0sq; p.lam = a.md.lam; p.kappa = a.md.kappa; p.mode = a.mode; p.seed = a.seed;
   p.tag_prop = a.tag_prop; p.tag_acc = a.tag_acc; p.t0 = a.t0; p.k = a.k;
   p.respect_done = a.respect_done;
+  p.finish_rec = a.finish_rec; p.finish_max_rec = a.finish_max_rec; p.finish_poll = a.finish_poll;
   p.rk = philox_round_keys(a.seed);
   const size_t smem = tc::smem_layout(V).total;
   static bool attr_done = false;

@@ -852,28 +852,14 @@ void launch_gather(const float* phi_in, float* phi_out, const float* S_in, float
 }
 
 // End of a temperature: record it, advance the index, latch done at beta == 1.
-__global__ void finish_step_kernel(Ctrl* ctrl, StepRecord* rec, int max_rec, int k, int N) {
+__global__ void finish_step_kernel(Ctrl* ctrl, StepRecord* rec, int max_rec, int k, int N, HostPoll* hp) {
   pdl_enter();
   if (ctrl->done) return;
-  int t = ctrl->temp_index;
-  if (t < max_rec) {
-    StepRecord r;
-    r.beta = ctrl->beta; r.delta = ctrl->delta; r.ess_frac = ctrl->ess_frac;
-    r.dlogZ = ctrl->dlogZ; r.logZ = ctrl->logZ;
-    r.accept_rate = (double)ctrl->n_accept / ((double)k * (double)N);
-    r.n_unique = (int)ctrl->n_unique; r.chol_status = ctrl->chol_status;
-    r.index = t; r.done = ctrl->beta >= 1.0;
-    rec[t] = r;
-  }
-  ctrl->temp_index = t + 1;
-  ctrl->mut_steps += (unsigned long long)k;   // steps enqueued past beta = 1 never get here
-  ctrl->n_accept = 0u;
-  ctrl->n_unique = 0u;
-  if (ctrl->beta >= 1.0) ctrl->done = 1;
+  finish_step_device(ctrl, rec, max_rec, k, N, hp);
 }
 
-void launch_finish_step(Ctrl* ctrl, StepRecord* rec, int max_rec, int k, int N, cudaStream_t st) {
-  ++g_launches; launch_pdl(finish_step_kernel, 1, 1, 0, st, ctrl, rec, max_rec, k, N);
+void launch_finish_step(Ctrl* ctrl, StepRecord* rec, int max_rec, int k, int N, HostPoll* hp, cudaStream_t st) {
+  ++g_launches; launch_pdl(finish_step_kernel, 1, 1, 0, st, ctrl, rec, max_rec, k, N, hp);
 }
 
 }  // namespace phi4
