@@ -419,7 +419,8 @@ static void enqueue_mutation(phi4smc* h, const MutateArgs& a) {
     return;
   }
   if (h->prm.kernel == 2 && a.mode == MODE_SMC) {
-    launch_mutate_irmh(a, h->mu, h->W2, h->st);
+    launch_mutate_irmh(a, h->mu, h->W2,
+                       (h->prm.mutation_path != 1 && mutate_tc_supported(a.md.V, true)) ? h->Lsplit : nullptr, h->st);
     return;
   }
   if (use_tc_path(h)) launch_mutate_tc(a, h->Lsplit, h->st);
@@ -456,7 +457,8 @@ static void enqueue_smc_step(phi4smc* h) {
   MutateArgs a = smc_mutate_args(h, h->prm.k_steps, nullptr, nullptr, 1);
   // the fused tcgen05 mutation closes the temperature itself (its last CTA); the other mutation
   // paths are several launches, so the step is closed by a kernel of its own
-  const bool fused_finish = h->prm.kernel == 0 && use_tc_path(h);
+  const bool fused_finish = (h->prm.kernel == 0 && use_tc_path(h)) ||
+                            (h->prm.kernel == 2 && h->prm.mutation_path != 1 && mutate_tc_supported(h->md.V, true));
   if (fused_finish) { a.finish_rec = h->rec; a.finish_max_rec = h->max_rec; a.finish_poll = h->h_hp; }
   enqueue_mutation(h, a);
   h->step_counter += (uint64_t)h->prm.k_steps;

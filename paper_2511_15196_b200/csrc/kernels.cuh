@@ -53,12 +53,15 @@ void launch_accept_step(const MutateArgs& a, int j, cudaStream_t st);
 void launch_ns_slice(const MutateArgs& a, float width, int m_expand, int max_shrink, cudaStream_t st);
 // NEXT f2: k independent-MH steps from N(mu, Lc Lc^T) (reading A15); W2 [ld] scratch
 bool irmh_supported(int V);
-void launch_mutate_irmh(const MutateArgs& a, const float* mu, float* W2, cudaStream_t st);
+// Lsplit != nullptr: the k steps run in the fused tcgen05 kernel (V <= 112)
+void launch_mutate_irmh(const MutateArgs& a, const float* mu, float* W2, float* Lsplit, cudaStream_t st);
 
 // mutate_tc.cu -- M1-M4 fused over k steps on tcgen05 (3xTF32), phi tile resident on-chip
-bool mutate_tc_supported(int V);
+bool mutate_tc_supported(int V, bool irmh = false);
 size_t mutate_tc_lsplit_floats(int V);
-void launch_mutate_tc(const MutateArgs& a, float* Lsplit, cudaStream_t st);
+// mu != nullptr: SMC-IRMH (independent proposal mu + Lc z, W2 = |Lc^-1 (phi - mu)|^2 per particle)
+void launch_mutate_tc(const MutateArgs& a, float* Lsplit, cudaStream_t st, const float* mu = nullptr,
+                      float* W2 = nullptr);
 void launch_lsplit(const float* Lc, int V, int Vn, int Kp, float s, float* Lsplit, const Ctrl* ctrl,
                    int respect_done, cudaStream_t st);
 

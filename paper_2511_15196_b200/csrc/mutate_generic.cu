@@ -327,38 +327,195 @@ void launch_mutate_generic(const MutateArgs& a, float* Lsplit, cudaStream_t st) 
 // (PAPER.md:53(ii), :200; reading A15).  whiten_kernel: W2[i] = |Lc^-1 (phi_i - mu)|^2 by forward
 // substitution, one warp per 32 particles, w in shared memory; FP64 accumulation (once per
 // temperature: the solve amplifies rounding by cond(Lc), and W2 enters every margin).
+// V <= 128.  FP64 arithmetic runs at ~1.5 TFLOP/s on this part (measured: the FP64 version of
+// this kernel took 111 us at C1 for 82 M FMAs), so the solve is carried in double-float
+// arithmetic on the FP32 pipe: w and every accumulator are (hi, lo) pairs, products and sums are
+// error-free transformations (Dekker / Knuth: two-product by FMA, two-sum), ~2^-44 relative.
+// Rows are taken four at a time: the products with the part of w already known run as eight
+// independent chains (four rows x even / odd columns), only the 4 x 4 diagonal block is serial.
+// The factor sits in shared memory (rows padded to a multiple of four, zeros beyond the row end)
+// and is read as broadcasts; a block serves WH_P particles.
+constexpr int WH_P = 64;
+__host__ __device__ inline int wh_vp(int V) { return (V + 3) & ~3; }
+__host__ __device__ inline size_t whiten_smem(int V) {
+  return ((size_t)wh_vp(V) * wh_vp(V) + (size_t)2 * V * WH_P) * sizeof(float);
+}
+struct df2 { float h, l; };
+__device__ __forceinline__ df2 df_two_sum(float a, float b) {          // a + b exactly
+  const float t = __fadd_rn(a, b), z = __fsub_rn(t, a);
+  return {t, __fadd_rn(__fsub_rn(a, __fsub_rn(t, z)), __fsub_rn(b, z))};
+}
+__device__ __forceinline__ df2 df_add(df2 a, df2 b) {
+  df2 s = df_two_sum(a.h, b.h);
+  s.l = __fadd_rn(s.l, __fadd_rn(a.l, b.l));
+  return df_two_sum(s.h, s.l);
+}
+// s += L * w (L a float, w a pair): the chain through s.h is one addition long
+__device__ __forceinline__ void df_fma(float L, df2 w, df2& s) {
+  const float ph = __fmul_rn(L, w.h);
+  float pe = __fmaf_rn(L, w.h, -ph);
+  pe = __fmaf_rn(L, w.l, pe);
+  const float t = __fadd_rn(s.h, ph), z = __fsub_rn(t, s.h);
+  const float e = __fadd_rn(__fsub_rn(s.h, __fsub_rn(t, z)), __fsub_rn(ph, z));
+  s.h = t;
+  s.l = __fadd_rn(s.l, __fadd_rn(e, pe));
+}
+__device__ __forceinline__ df2 df_div(df2 a, float b) {               // a / b
+  const float q1 = __fdiv_rn(a.h, b);
+  const float r = __fadd_rn(__fmaf_rn(-q1, b, a.h), a.l);
+  return df_two_sum(q1, __fdiv_rn(r, b));
+}
+// Block = WH_P particles x 4 row lanes (256 threads): thread (p, j) carries row x0 + j of the
+// current 4-row block for particle p (four chains: the column phases); the j = 0 threads then
+// finish the 4 x 4 diagonal block serially.  Two block barriers per row block.
+__global__ void __launch_bounds__(4 * WH_P)
+whiten_small_kernel(const float* __restrict__ phi, const float* __restrict__ mu,
+                    const float* __restrict__ Lc, float* __restrict__ W2, int N, int ld, int V,
+                    const Ctrl* ctrl, int respect_done) {
+  if (respect_done && ctrl->done) return;
+  extern __shared__ float whs[];
+  __shared__ float2 accs[3][WH_P];                             // row sums of rows x0 + 1 .. x0 + 3
+  const int Vp = wh_vp(V);
+  float* Lf = whs;                                             // [Vp][Vp], zero outside the lower triangle
+  float2* wsm = reinterpret_cast<float2*>(Lf + (size_t)Vp * Vp);   // [V][WH_P] (hi, lo)
+  const int tid = threadIdx.x, p = tid & (WH_P - 1), j = tid >> 6;   // j is warp-uniform
+  const int i = blockIdx.x * WH_P + p;
+  const bool live = i < N;
+  // eight loads in flight per thread (the factor comes from L2: one round trip per batch)
+  for (int e0 = 0; e0 < Vp * Vp; e0 += 8 * 4 * WH_P) {
+    float v[8];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      const int e = e0 + u * 4 * WH_P + tid, x = e / Vp, y = e - x * Vp;
+      v[u] = (x < V && y <= x) ? Lc[(size_t)x * V + y] : 0.f;
+    }
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      const int e = e0 + u * 4 * WH_P + tid;
+      if (e < Vp * Vp) Lf[e] = v[u];
+    }
+  }
+  __syncthreads();
+  df2 w2 = {0.f, 0.f};
+  for (int x0 = 0; x0 < V; x0 += 4) {
+    // the j = 0 threads need this row block's right-hand sides after the product loop
+    float fx[4], mx[4];
+    if (j == 0) {
+#pragma unroll
+      for (int m = 0; m < 4; ++m) {
+        const int x = min(x0 + m, V - 1);
+        fx[m] = live ? phi[(size_t)x * ld + i] : 0.f;
+        mx[m] = mu[x];
+      }
+    }
+    const float* row = Lf + (size_t)(x0 + j) * Vp;
+    df2 ac[4] = {{0.f, 0.f}, {0.f, 0.f}, {0.f, 0.f}, {0.f, 0.f}};
+    for (int y = 0; y < x0; y += 4) {          // x0 is a multiple of 4
+      const float4 l = *reinterpret_cast<const float4*>(row + y);
+      const float2 u0 = wsm[y * WH_P + p], u1 = wsm[(y + 1) * WH_P + p];
+      const float2 u2 = wsm[(y + 2) * WH_P + p], u3 = wsm[(y + 3) * WH_P + p];
+      df_fma(l.x, df2{u0.x, u0.y}, ac[0]); df_fma(l.y, df2{u1.x, u1.y}, ac[1]);
+      df_fma(l.z, df2{u2.x, u2.y}, ac[2]); df_fma(l.w, df2{u3.x, u3.y}, ac[3]);
+    }
+    const df2 acc = df_add(df_add(ac[0], ac[1]), df_add(ac[2], ac[3]));
+    if (j > 0) accs[j - 1][p] = make_float2(acc.h, acc.l);
+    __syncthreads();
+    if (j == 0) {
+      df2 wl[4];
+#pragma unroll
+      for (int m = 0; m < 4; ++m) {
+        const int x = x0 + m;
+        if (x < V) {
+          df2 s = acc;
+          if (m > 0) { const float2 t = accs[m - 1][p]; s = df2{t.x, t.y}; }
+          const float* rm = Lf + (size_t)x * Vp + x0;
+#pragma unroll
+          for (int q = 0; q < 4; ++q)
+            if (q < m) df_fma(rm[q], wl[q], s);
+          // v = ((phi - mu) - s) / L_xx, the difference formed exactly
+          df2 v = df_add(df_two_sum(fx[m], -mx[m]), df2{-s.h, -s.l});
+          v = df_div(v, rm[m]);
+          wl[m] = v;
+          wsm[x * WH_P + p] = make_float2(v.h, v.l);
+          // w2 += v^2 = v.h^2 + 2 v.h v.l (+ v.l^2, below the pair's precision)
+          df_fma(v.h, v, w2);
+          w2.l = __fmaf_rn(v.l, v.h, w2.l);
+        }
+      }
+    }
+    __syncthreads();
+  }
+  if (j == 0 && live) W2[i] = __fadd_rn(w2.h, w2.l);
+}
+
+// Any V <= 800: one warp per 32 particles, the factor read through the read-only cache.
 __global__ void __launch_bounds__(32)
 whiten_kernel(const float* __restrict__ phi, const float* __restrict__ mu,
               const float* __restrict__ Lc, float* __restrict__ W2, int N, int ld, int V,
               const Ctrl* ctrl, int respect_done) {
   if (respect_done && ctrl->done) return;
-  extern __shared__ double wsm[];          // [V][32]
+  extern __shared__ double wsm[];          // [V][32] w, then [V] 1 / L_xx
+  double* invd = wsm + (size_t)V * 32;
   const int lane = threadIdx.x, i = blockIdx.x * 32 + lane;
+  for (int x = lane; x < V; x += 32) invd[x] = 1.0 / (double)Lc[(size_t)x * V + x];
+  __syncwarp();
   if (i >= N) return;
   double w2 = 0.0;
-  for (int x = 0; x < V; ++x) {
-    const float* row = Lc + (size_t)x * V;
-    double a = (double)phi[(size_t)x * ld + i] - (double)mu[x];
-    for (int y = 0; y < x; ++y) a -= (double)row[y] * wsm[y * 32 + lane];
-    a /= (double)row[x];
-    wsm[x * 32 + lane] = a;
-    w2 += a * a;
+  for (int x0 = 0; x0 < V; x0 += 4) {
+    const int nb = min(4, V - x0);
+    const float* r0 = Lc + (size_t)x0 * V;
+    const float* r1 = Lc + (size_t)min(x0 + 1, V - 1) * V;
+    const float* r2 = Lc + (size_t)min(x0 + 2, V - 1) * V;
+    const float* r3 = Lc + (size_t)min(x0 + 3, V - 1) * V;
+    double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0, c0 = 0.0, c1 = 0.0, c2 = 0.0, c3 = 0.0;
+    for (int y = 0; y < x0; y += 2) {        // x0 is a multiple of 4: whole pairs
+      const double w0 = wsm[y * 32 + lane], w1 = wsm[(y + 1) * 32 + lane];
+      a0 = fma((double)__ldg(r0 + y), w0, a0); c0 = fma((double)__ldg(r0 + y + 1), w1, c0);
+      a1 = fma((double)__ldg(r1 + y), w0, a1); c1 = fma((double)__ldg(r1 + y + 1), w1, c1);
+      a2 = fma((double)__ldg(r2 + y), w0, a2); c2 = fma((double)__ldg(r2 + y + 1), w1, c2);
+      a3 = fma((double)__ldg(r3 + y), w0, a3); c3 = fma((double)__ldg(r3 + y + 1), w1, c3);
+    }
+    const double acc[4] = {a0 + c0, a1 + c1, a2 + c2, a3 + c3};
+    const float* rows[4] = {r0, r1, r2, r3};
+    double wl[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j)
+      if (j < nb) {
+        const int x = x0 + j;
+        double v = (double)phi[(size_t)x * ld + i] - (double)mu[x] - acc[j];
+#pragma unroll
+        for (int m = 0; m < 4; ++m)
+          if (m < j) v -= (double)__ldg(rows[j] + x0 + m) * wl[m];
+        v *= invd[x];
+        wl[j] = v;
+        wsm[x * 32 + lane] = v;
+        w2 = fma(v, v, w2);
+      }
   }
   W2[i] = (float)w2;
 }
 
-bool irmh_supported(int V) { return (size_t)V * 32 * sizeof(double) <= 200 * 1024; }
+bool irmh_supported(int V) { return V >= 1 && V <= 800; }     // w [V][32] + 1 / L_xx [V] in FP64: 211 KB
 
-void launch_mutate_irmh(const MutateArgs& a, const float* mu, float* W2, cudaStream_t st) {
+void launch_mutate_irmh(const MutateArgs& a, const float* mu, float* W2, float* Lsplit, cudaStream_t st) {
   const int V = a.md.V;
   static bool attr_done = false;
   if (!attr_done) {
-    cudaFuncSetAttribute(whiten_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    cudaFuncSetAttribute(whiten_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 800 * 33 * (int)sizeof(double));
+    cudaFuncSetAttribute(whiten_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
     attr_done = true;
   }
   ++g_launches;
-  whiten_kernel<<<(a.N + 31) / 32, 32, (size_t)V * 32 * sizeof(double), st>>>(
-      a.phi, mu, a.Lc, W2, a.N, a.ld, V, a.ctrl, a.respect_done);
+  if (whiten_smem(V) <= (size_t)224 * 1024)
+    whiten_small_kernel<<<(a.N + WH_P - 1) / WH_P, 4 * WH_P, whiten_smem(V), st>>>(
+        a.phi, mu, a.Lc, W2, a.N, a.ld, V, a.ctrl, a.respect_done);
+  else
+    whiten_kernel<<<(a.N + 31) / 32, 32, (size_t)V * 33 * sizeof(double), st>>>(
+        a.phi, mu, a.Lc, W2, a.N, a.ld, V, a.ctrl, a.respect_done);
+  if (Lsplit) {                      // the k steps in the fused tcgen05 kernel
+    launch_mutate_tc(a, Lsplit, st, mu, W2);
+    return;
+  }
   dim3 gz((a.ld + 127) / 128, (V + 3) / 4);
   dim3 gp(a.ld / 64, (V + 63) / 64);
   for (int j = 0; j < a.k; ++j) {

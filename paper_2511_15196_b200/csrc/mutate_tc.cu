@@ -42,10 +42,12 @@ constexpr int CHUNK_BYTES = TILE * 16;           // one 16-byte K-chunk of all 1
 constexpr int SLAB_BYTES = 2 * 4 * CHUNK_BYTES;  // {hi,lo} x 4 K-chunks
 constexpr int MAX_SMEM = 232448;
 
+constexpr int ZSQ_BUFS = 4;          // IRMH: |z|^2 accumulators, one per step in flight
+constexpr float ZSQ_SCALE = 4194304.f;   // 2^22: |z|^2 < 1024 in 32-bit fixed point, 2.4e-7 resolution
 struct Smem {
-  size_t tile0, tile1, lhi, llo, zring, part, dtab, bars, total;
+  size_t tile0, tile1, lhi, llo, zring, part, dtab, bars, zsq, zzs, total;
 };
-__host__ __device__ inline Smem smem_layout(int V) {
+__host__ __device__ inline Smem smem_layout(int V, bool irmh = false) {
   Smem s;
   size_t o = 0;
   const size_t tile = (size_t)V * TILE * 4, lmat = l_floats(V) * 4;
@@ -55,8 +57,12 @@ __host__ __device__ inline Smem smem_layout(int V) {
   s.llo = o; o += round_up((int)lmat, 128);
   s.zring = o; o += (size_t)STAGES * SLAB_BYTES;
   s.part = o; o += (size_t)EPI_PARTS * TILE * 8 + TILE * 4;   // partial (dS, dU0) per part and particle; ln u
-  s.dtab = o; o += 32 * 32;                        // per-K-step operand descriptors
+  s.dtab = o; o += round_up(32 * (kp_of(V) >> 3), 128);   // per-K-step operand descriptors (32 B each)
   s.bars = o; o += 128;
+  // IRMH (reading A15): |z|^2 per particle and step in fixed point (integer atomics: the sum does
+  // not depend on the order of the six threads that draw a particle's normals), and its float copy
+  s.zsq = o; if (irmh) o += (size_t)ZSQ_BUFS * TILE * 4;
+  s.zzs = o; if (irmh) o += (size_t)TILE * 4;
   s.total = o;
   return s;
 }
@@ -75,6 +81,7 @@ struct TcParams {
   uint32_t tag_prop, tag_acc, t0;
   int k, respect_done;
   PhiloxKeys rk;               // round keys of `seed` (constant-bank operands of the Philox XORs)
+  const float* mu; float* W2;  // IRMH: proposal mean [V]; |Lc^-1 (phi - mu)|^2 per particle [ld]
   StepRecord* finish_rec;      // not null: the last CTA closes the temperature (finish_step_device)
   int finish_max_rec;
   HostPoll* finish_poll;
@@ -188,14 +195,18 @@ __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
 //                 stage, two stages (four independent chains) per pass.
 //   warp 24       one thread issues every tcgen05.mma and the bulk copy of Lc; the operand
 //                 descriptors of all K-steps are tabulated once in shared memory by its 32 lanes.
-template <int LT>
+// IRMH (NEXT row f2, reading A15): the proposal is mu + Lc z (the factor is packed with s = 1), the
+// margin gains log q(phi) - log q(phi') = 1/2 |z|^2 - 1/2 |w|^2, and an accepted particle's |w|^2
+// becomes |z|^2.  |z|^2 is summed where the normals are drawn.
+template <int LT, bool IRMH>
 __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParams p) {
   // programmatic dependent launch: barrier setup and the TMEM allocation touch nothing the
   // predecessor writes, so they run before the wait
   pdl_trigger();
   using namespace tc;
   extern __shared__ __align__(1024) uint8_t smem[];
-  const Smem lay = smem_layout(p.V);
+  const Smem lay = smem_layout(p.V, IRMH);
+  uint32_t* zsq = reinterpret_cast<uint32_t*>(smem + lay.zsq);
   float* tile0 = reinterpret_cast<float*>(smem + lay.tile0);
   float* tile1 = reinterpret_cast<float*>(smem + lay.tile1);
   float2* part = reinterpret_cast<float2*>(smem + lay.part);
@@ -225,6 +236,8 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
     fence_mbar_init();
   }
   if (warp == 0) tmem_alloc(smem_u32(tmem_slot), ncols);
+  if (IRMH)
+    for (int e = threadIdx.x; e < ZSQ_BUFS * TILE; e += THREADS) zsq[e] = 0u;
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
@@ -327,6 +340,7 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
         for (int st2 = 0; st2 < 2; ++st2) {
           if (st2 == 1 && !second) break;
           float4 hv[2], lv[2];
+          float zz = 0.f;
 #pragma unroll
           for (int e = 0; e < 2; ++e) {
             const int c = 2 * st2 + e;
@@ -334,6 +348,11 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
             if (ok[c]) {
               box_muller_fast(w[c].x, w[c].y, z[0], z[1]);
               box_muller_fast(w[c].z, w[c].w, z[2], z[3]);
+            }
+            if (IRMH) {                                  // R1: a ragged last quad is truncated at V
+              const int x0 = 4 * (4 * (nitE + it + (c >> 1)) + 2 * (c & 1) + half);
+#pragma unroll
+              for (int m = 0; m < 4; ++m) if (x0 + m < V) zz = fmaf(z[m], z[m], zz);
             }
             // hi = rna_tf32(z); lo = z - hi is exact and |lo| <= 2^-12 |z|: the tensor core's own
             // truncation of lo to 11 bits costs 2^-23 |z|, below the dropped lo*lo term
@@ -350,6 +369,7 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
           *reinterpret_cast<float4*>(st + 2 * CHUNK_BYTES) = hv[1];
           *reinterpret_cast<float4*>(st + 4 * CHUNK_BYTES) = lv[0];
           *reinterpret_cast<float4*>(st + 6 * CHUNK_BYTES) = lv[1];
+          if (IRMH) atomicAdd(&zsq[(t & (ZSQ_BUFS - 1)) * TILE + pr], __float2uint_rn(zz * ZSQ_SCALE));
           fence_proxy_async();
           __syncwarp();
           if (lane == 0) mbar_arrive_n(zfull(s), 2);         // 8 warps x 2 = the 16 expected
@@ -368,6 +388,8 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
     float* oth = tile1 + pr;
     for (int x = g; x < V; x += EPI_PARTS) cur[x * TILE] = live ? p.phi[(size_t)x * p.ld + i] : 0.f;
     float Si = live ? p.S[i] : 0.f, Ui = live ? p.U0[i] : 0.f;
+    float Wi = (IRMH && live) ? p.W2[i] : 0.f;          // |Lc^-1 (phi - mu)|^2 of the current state
+    float* zzs = reinterpret_cast<float*>(smem + lay.zzs);
     const float beta = (float)p.ctrl->beta, S_star = (float)p.ctrl->S_star;
     unsigned nacc = 0;
     const uint32_t tlane = taddr + ((uint32_t)(Q * 32) << 16);
@@ -391,6 +413,12 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
           if (live && q < nq) {
             box_muller_fast(w[e].x, w[e].y, z[0], z[1]);
             box_muller_fast(w[e].z, w[e].w, z[2], z[3]);
+          }
+          if (IRMH) {                                    // R1: a ragged last quad is truncated at V
+            float zz = 0.f;
+#pragma unroll
+            for (int m = 0; m < 4; ++m) if (4 * q + m < V) zz = fmaf(z[m], z[m], zz);
+            atomicAdd(&zsq[(t & (ZSQ_BUFS - 1)) * TILE + pr], __float2uint_rn(zz * ZSQ_SCALE));
           }
           float4 hv, lv;
           hv.x = tf32_rna(z[0]); lv.x = z[0] - hv.x;  hv.y = tf32_rna(z[1]); lv.y = z[1] - hv.y;
@@ -427,21 +455,21 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
         const float* ci = cur + cb * TILE; float* oi = oth + cb * TILE;
         if (cb + 16 <= V) {
 #pragma unroll
-          for (int jj = 0; jj < 16; ++jj) oi[jj * TILE] = ci[jj * TILE] + __uint_as_float(r0[jj]);
+          for (int jj = 0; jj < 16; ++jj) oi[jj * TILE] = (IRMH ? __ldg(p.mu + cb + jj) : ci[jj * TILE]) + __uint_as_float(r0[jj]);
         } else {
 #pragma unroll
           for (int jj = 0; jj < 16; ++jj)
-            if (cb + jj < V) oi[jj * TILE] = ci[jj * TILE] + __uint_as_float(r0[jj]);
+            if (cb + jj < V) oi[jj * TILE] = (IRMH ? __ldg(p.mu + cb + jj) : ci[jj * TILE]) + __uint_as_float(r0[jj]);
         }
         if (two) {
           ci = cur + cb1 * TILE; oi = oth + cb1 * TILE;
           if (cb1 + 16 <= V) {
 #pragma unroll
-            for (int jj = 0; jj < 16; ++jj) oi[jj * TILE] = ci[jj * TILE] + __uint_as_float(r1[jj]);
+            for (int jj = 0; jj < 16; ++jj) oi[jj * TILE] = (IRMH ? __ldg(p.mu + cb1 + jj) : ci[jj * TILE]) + __uint_as_float(r1[jj]);
           } else {
 #pragma unroll
             for (int jj = 0; jj < 16; ++jj)
-              if (cb1 + jj < V) oi[jj * TILE] = ci[jj * TILE] + __uint_as_float(r1[jj]);
+              if (cb1 + jj < V) oi[jj * TILE] = (IRMH ? __ldg(p.mu + cb1 + jj) : ci[jj * TILE]) + __uint_as_float(r1[jj]);
           }
         }
       }
@@ -453,7 +481,14 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
       float dS = 0.f, dU = 0.f;
       tc_stencil<LT>(cur, oth, g, L, hm, lam, kap, dS, dU);
       part[g * TILE + pr] = make_float2(dS, dU);
-      if (g == EPI_PARTS - 1) lus[pr] = log_uniform(p.seed, p.tag_acc, p.t0 + (uint32_t)t, (uint32_t)i);
+      if (g == EPI_PARTS - 1) {
+        lus[pr] = log_uniform(p.seed, p.tag_acc, p.t0 + (uint32_t)t, (uint32_t)i);
+        if (IRMH) {                                  // |z|^2 of this step; the slot is free again
+          uint32_t* zq = &zsq[(t & (ZSQ_BUFS - 1)) * TILE + pr];
+          zzs[pr] = (float)*zq * (1.0f / ZSQ_SCALE);
+          *zq = 0u;
+        }
+      }
       named_bar_sync(1 + Q, 32 * EPI_PARTS);
       // every part sums the four partials in the same order and takes the same decision (M4)
       dS = 0.f; dU = 0.f;
@@ -466,7 +501,12 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
       const float lu = lus[pr];
       float margin;
       bool acc;
-      if (p.mode == MODE_SMC) {
+      float tZ = 0.f;
+      if (IRMH) {
+        tZ = zzs[pr];
+        margin = -(dU + beta * dS) + 0.5f * (tZ - Wi) - lu;
+        acc = margin > 0.f;
+      } else if (p.mode == MODE_SMC) {
         margin = -(dU + beta * dS) - lu;
         acc = margin > 0.f;
       } else {
@@ -478,6 +518,7 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
         float* tmp = cur; cur = oth; oth = tmp;
         Si += dS;
         Ui += dU;
+        if (IRMH) Wi = tZ;
         ++nacc;
       }
       if (live && g == 0) {
@@ -488,7 +529,7 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
     }
     if (live) {
       for (int x = g; x < V; x += EPI_PARTS) p.phi[(size_t)x * p.ld + i] = cur[x * TILE];
-      if (g == 0) { p.S[i] = Si; p.U0[i] = Ui; }
+      if (g == 0) { p.S[i] = Si; p.U0[i] = Ui; if (IRMH) p.W2[i] = Wi; }
     }
     if (g == 0) {
 #pragma unroll
@@ -511,8 +552,8 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
   }
 }
 
-bool mutate_tc_supported(int V) {
-  return V >= 1 && tc::vn_of(V) <= 256 && tc::smem_layout(V).total <= (size_t)tc::MAX_SMEM;
+bool mutate_tc_supported(int V, bool irmh) {
+  return V >= 1 && tc::vn_of(V) <= 256 && tc::smem_layout(V, irmh).total <= (size_t)tc::MAX_SMEM;
 }
 
 size_t mutate_tc_lsplit_floats(int V) { return 2 * tc::l_floats(V); }
@@ -526,9 +567,10 @@ void launch_lsplit(const float* Lc, int V, int Vn, int Kp, float s, float* Lspli
       Lc, V, Vn, Kp, s, Lsplit, tc::l_floats_vk(Vn, Kp), ctrl, respect_done);
 }
 
-void launch_mutate_tc(const MutateArgs& a, float* Lsplit, cudaStream_t st) {
+void launch_mutate_tc(const MutateArgs& a, float* Lsplit, cudaStream_t st, const float* mu, float* W2) {
   const int V = a.md.V, Vn = tc::vn_of(V), Kp = tc::kp_of(V);
-  launch_lsplit(a.Lc, V, Vn, Kp, a.s, Lsplit, a.ctrl, a.respect_done, st);
+  const bool irmh = mu != nullptr;                 // independent proposal mu + Lc z: no step scale
+  launch_lsplit(a.Lc, V, Vn, Kp, irmh ? 1.0f : a.s, Lsplit, a.ctrl, a.respect_done, st);
   TcParams p;
   p.phi = a.phi; p.S = a.S; p.U0 = a.U0; p.Lsplit = Lsplit; p.ctrl = a.ctrl;
   p.acc_out = a.acc_out; p.margin_out = a.margin_out;
@@ -536,22 +578,28 @@ void launch_mutate_tc(const MutateArgs& a, float* Lsplit, cudaStream_t st) {
   p.m0sq = a.md.m0sq; p.lam = a.md.lam; p.kappa = a.md.kappa; p.mode = a.mode; p.seed = a.seed;
   p.tag_prop = a.tag_prop; p.tag_acc = a.tag_acc; p.t0 = a.t0; p.k = a.k;
   p.respect_done = a.respect_done;
+  p.mu = mu; p.W2 = W2;
   p.finish_rec = a.finish_rec; p.finish_max_rec = a.finish_max_rec; p.finish_poll = a.finish_poll;
   p.rk = philox_round_keys(a.seed);
-  const size_t smem = tc::smem_layout(V).total;
+  const size_t smem = tc::smem_layout(V, irmh).total;
   static bool attr_done = false;
   if (!attr_done) {
-    cudaFuncSetAttribute(mutate_tc_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::MAX_SMEM);
-    cudaFuncSetAttribute(mutate_tc_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::MAX_SMEM);
-    cudaFuncSetAttribute(mutate_tc_kernel<10>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::MAX_SMEM);
+    cudaFuncSetAttribute(mutate_tc_kernel<0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::MAX_SMEM);
+    cudaFuncSetAttribute(mutate_tc_kernel<4, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::MAX_SMEM);
+    cudaFuncSetAttribute(mutate_tc_kernel<10, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::MAX_SMEM);
+    cudaFuncSetAttribute(mutate_tc_kernel<0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::MAX_SMEM);
+    cudaFuncSetAttribute(mutate_tc_kernel<10, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::MAX_SMEM);
     attr_done = true;
   }
   const dim3 grid(a.ld / tc::TILE);
   ++g_launches;
   // lattice sizes of the BASELINE configs get a fully unrolled stencil; any other L the loop
-  if (p.L == 10) launch_pdl(mutate_tc_kernel<10>, grid, tc::THREADS, smem, st, p);
-  else if (p.L == 4) launch_pdl(mutate_tc_kernel<4>, grid, tc::THREADS, smem, st, p);
-  else launch_pdl(mutate_tc_kernel<0>, grid, tc::THREADS, smem, st, p);
+  if (irmh) {
+    if (p.L == 10) launch_pdl(mutate_tc_kernel<10, true>, grid, tc::THREADS, smem, st, p);
+    else launch_pdl(mutate_tc_kernel<0, true>, grid, tc::THREADS, smem, st, p);
+  } else if (p.L == 10) launch_pdl(mutate_tc_kernel<10, false>, grid, tc::THREADS, smem, st, p);
+  else if (p.L == 4) launch_pdl(mutate_tc_kernel<4, false>, grid, tc::THREADS, smem, st, p);
+  else launch_pdl(mutate_tc_kernel<0, false>, grid, tc::THREADS, smem, st, p);
 }
 
 }  // namespace phi4
