@@ -68,9 +68,7 @@ struct phi4smc {
   int64_t iter_base;         // NS: iters_enqueued - ctrl->temp_index after a set_state
   int known_done;
   Ctrl* h_ctrl;              // pinned staging
-  Ctrl* h_poll;              // pinned, 2 slots: ns_run polls one step behind the GPU
   HostPoll* h_hp;            // pinned, written by the device at the end of every SMC temperature
-  cudaEvent_t poll_ev[2];
   // side stream (fork / join by events on the caller's stream; host resources only): nested
   // sampling runs the dead-point selection beside the covariance chain, the large-V mutation draws
   // the normals of the next step beside the proposal GEMM of the current one
@@ -156,7 +154,7 @@ static int carve_ns(phi4smc* h, char* base, size_t* total) {
   h->dead_S = c.take<float>(nlog);
   h->dead_M = c.take<float>(nlog);
   h->dead_logw = c.take<double>(nlog);
-  h->hsum = c.take<double>(kd + 1);
+  h->hsum = c.take<double>(2 * kd + 1);
   h->M_all = c.take<float>(nlog + N);
   h->S_all = c.take<float>(nlog + N);
   h->logw_all = c.take<double>(nlog + N);
@@ -238,10 +236,8 @@ PHI4_API size_t ns_workspace_bytes(int L, int n_live, int k_delete, int max_iter
 
 static int host_staging(phi4smc* h) {
   CU(cudaMallocHost((void**)&h->h_ctrl, sizeof(Ctrl)));
-  CU(cudaMallocHost((void**)&h->h_poll, 2 * sizeof(Ctrl)));
   CU(cudaMallocHost((void**)&h->h_hp, sizeof(HostPoll)));
   memset(h->h_hp, 0, sizeof(HostPoll));
-  for (int e = 0; e < 2; ++e) CU(cudaEventCreateWithFlags(&h->poll_ev[e], cudaEventDisableTiming));
   {
     CU(cudaStreamCreateWithFlags(&h->side, cudaStreamNonBlocking));
     CU(cudaEventCreateWithFlags(&h->fork_ev, cudaEventDisableTiming));
@@ -354,9 +350,7 @@ PHI4_API int smc_destroy(phi4smc* h) {
   if (!h) return PHI4_OK;
   cudaStreamSynchronize(h->st);
   if (h->h_ctrl) cudaFreeHost(h->h_ctrl);
-  if (h->h_poll) cudaFreeHost(h->h_poll);
   if (h->h_hp) cudaFreeHost(h->h_hp);
-  for (int e = 0; e < 2; ++e) if (h->poll_ev[e]) cudaEventDestroy(h->poll_ev[e]);
   if (h->side) { cudaStreamSynchronize(h->side); cudaStreamDestroy(h->side); }
   if (h->fork_ev) cudaEventDestroy(h->fork_ev);
   if (h->join_ev) cudaEventDestroy(h->join_ev);
@@ -505,45 +499,19 @@ PHI4_API int smc_step(phi4smc* h, smc_step_info* info) {
   return rc;
 }
 
-// Shared by smc_run / ns_run: keep one step queued behind the one whose control block the host
-// is looking at, so the GPU never idles on the host's poll.  `enqueue` enqueues one step.
+// Shared by smc_run / ns_run.  The device reports every finished step in pinned host memory
+// (HostPoll, written by the kernel that closes the step): no copy or event sits in the stream
+// between two steps, so their kernels stay chained.  One step is kept queued behind the one whose
+// report the host is waiting for.  `start` = steps completed before this call.
 template <typename F>
-static int run_pipelined(phi4smc* h, int max_steps, int* enq_out, F enqueue) {
-  int enq = 0, rc = PHI4_OK;
-  while (!h->known_done && enq < max_steps) {
-    enqueue(h);
-    const int slot = enq & 1;
-    ++enq;
-    CU(cudaMemcpyAsync(&h->h_poll[slot], h->ctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost, h->st));
-    CU(cudaEventRecord(h->poll_ev[slot], h->st));
-    if (enq >= 2) {
-      const int prev = (enq - 2) & 1;            // the step before the one just enqueued
-      CU(cudaEventSynchronize(h->poll_ev[prev]));
-      const Ctrl& c = h->h_poll[prev];
-      if (c.done) h->known_done = 1;
-      if (c.nan_flag || c.chol_status < 0) break;
-    }
-  }
-  *enq_out = enq;
-  rc = sync_ctrl(h);
-  return rc;
-}
-
-PHI4_API int smc_run(phi4smc* h, int max_temps, int* n_temps) {
-  if (!h || h->kind != KIND_SMC || max_temps < 0) return PHI4_EINVAL;
-  int rc = sync_ctrl(h);
-  if (rc != PHI4_OK) return rc;
-  const int start = h->h_ctrl->temp_index;
-  int enq = 0;
-  // The device reports every finished temperature in pinned host memory (HostPoll): no copy or
-  // event sits in the stream between two temperatures.  Keep one step queued behind the one
-  // whose report the host is waiting for.
+static int run_polled(phi4smc* h, int max_steps, int start, F enqueue) {
   volatile HostPoll* hp = h->h_hp;
   hp->seq = start; hp->done = h->h_ctrl->done; hp->nan_flag = h->h_ctrl->nan_flag;
   hp->chol_status = h->h_ctrl->chol_status;
   if (h->h_ctrl->done) h->known_done = 1;
-  while (!h->known_done && enq < max_temps) {
-    enqueue_smc_step(h);
+  int enq = 0;
+  while (!h->known_done && enq < max_steps) {
+    enqueue(h);
     ++enq;
     if (enq >= 2) {
       const int target = start + enq - 1;        // the step before the one just enqueued
@@ -551,17 +519,27 @@ PHI4_API int smc_run(phi4smc* h, int max_temps, int* n_temps) {
         if ((spin & 1023u) == 0) {               // a dead stream must not hang the host
           cudaError_t q = cudaStreamQuery(h->st);
           if (q == cudaSuccess) break;
-          if (q != cudaErrorNotReady) { snprintf(h->err, sizeof(h->err), "smc_run: %s", cudaGetErrorString(q)); return PHI4_ECUDA; }
+          if (q != cudaErrorNotReady) {
+            snprintf(h->err, sizeof(h->err), "run: %s", cudaGetErrorString(q));
+            return PHI4_ECUDA;
+          }
         }
       }
       if (hp->done) h->known_done = 1;
       if (hp->nan_flag || hp->chol_status < 0) break;
     }
   }
-  rc = sync_ctrl(h);
+  return sync_ctrl(h);
+}
+
+PHI4_API int smc_run(phi4smc* h, int max_temps, int* n_temps) {
+  if (!h || h->kind != KIND_SMC || max_temps < 0) return PHI4_EINVAL;
+  int rc = sync_ctrl(h);
+  if (rc != PHI4_OK) return rc;
+  const int start = h->h_ctrl->temp_index;
+  rc = run_polled(h, max_temps, start, enqueue_smc_step);
   // (steps enqueued past beta = 1 were no-ops; sync_ctrl took the step counter from the device)
   const int made = h->h_ctrl->temp_index - start;
-  (void)enq;
   if (n_temps) *n_temps = made;
   return rc;
 }
@@ -711,7 +689,7 @@ static void enqueue_ns_step(phi4smc* h) {
   if (h->nsp.inner == 1) launch_ns_slice(m, h->nsp.slice_width, h->nsp.max_expand, h->nsp.max_shrink, h->st);
   else enqueue_mutation(h, m);
   launch_ns_store_walkers(a, h->st);
-  launch_ns_finish(a, h->rec, h->n_walk, h->st);
+  launch_ns_finish(a, h->rec, h->n_walk, h->h_hp, h->st);
   h->iters_enqueued += 1;
 }
 
@@ -757,10 +735,8 @@ PHI4_API int ns_run(phi4smc* h, int max_iters, int* n_iters) {
   int rc = sync_ctrl(h);
   if (rc != PHI4_OK) return rc;
   const int start = h->h_ctrl->temp_index;
-  int enq = 0;
-  rc = run_pipelined(h, max_iters, &enq, enqueue_ns_step);
+  rc = run_polled(h, max_iters, start, enqueue_ns_step);
   const int made = h->h_ctrl->temp_index - start;
-  (void)enq;
   if (n_iters) *n_iters = made;
   return (rc == PHI4_OK && h->h_ctrl->done == 2) ? PHI4_ETRUNC : rc;
 }

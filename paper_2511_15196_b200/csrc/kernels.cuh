@@ -135,7 +135,7 @@ struct NsArgs {
   int32_t* surv;                         // [n] survivors in index order
   int32_t* start;                        // [k_del] chosen start points
   float* dead_S; float* dead_M; double* dead_logw;   // dead-point log [max_iters*k_del]
-  const double* hsum;                    // [k_del+1] partial sums of 1/(n-m+1) (reading A6)
+  const double* hsum;                    // [k_del+1] partial sums of 1/(n-m+1) (reading A6), then [k_del] log(1 - e^{-1/(n-j)})
   unsigned long long* gkeys;             // n > 16384: sort keys in global memory (ns_sort_scratch_keys)
   int32_t* gflag;                        // n > 16384: [n] survivor flags
   int max_iters;
@@ -147,7 +147,7 @@ void launch_ns_hsum(double* hsum, int n, int k_del, cudaStream_t st);
 void launch_ns_select_evidence(const NsArgs& a, cudaStream_t st);   // N1 + N2 + start choice
 void launch_ns_load_walkers(const NsArgs& a, cudaStream_t st);      // N3 gather
 void launch_ns_store_walkers(const NsArgs& a, cudaStream_t st);     // N3 scatter
-void launch_ns_finish(const NsArgs& a, StepRecord* rec, int n_walk, cudaStream_t st);  // N4
+void launch_ns_finish(const NsArgs& a, StepRecord* rec, int n_walk, HostPoll* hp, cudaStream_t st);  // N4
 
 }  // namespace phi4
 

@@ -166,8 +166,7 @@ ns_select_evidence_kernel(NsArgs a) {
   double best = -INFINITY;
   for (int j = tid; j < kd; j += nt) {
     const double lx = logX0 - a.hsum[j];                                  // logX_{j'-1}, j' = j+1
-    const double step = 1.0 / (double)(n - j);                            // 1/(n-j'+1)
-    const double logw = lx + log1p(-exp(-step));
+    const double logw = lx + a.hsum[kd + 1 + j];                          // + log(1 - e^{-1/(n-j'+1)})
     const int d = (int)(uint32_t)keys[j];
     const float Sd = a.S[d];
     if (it < a.max_iters) {
@@ -190,7 +189,7 @@ ns_select_evidence_kernel(NsArgs a) {
   best = scratch[32];
   double e = 0.0;
   for (int j = tid; j < kd; j += nt) {
-    const double logw = logX0 - a.hsum[j] + log1p(-exp(-1.0 / (double)(n - j)));
+    const double logw = logX0 - a.hsum[j] + a.hsum[kd + 1 + j];
     e += exp(logw - (double)a.S[(int)(uint32_t)keys[j]] - best);
   }
   e = block_sum(e, scratch);
@@ -282,13 +281,17 @@ void launch_ns_select_evidence(const NsArgs& a, cudaStream_t st) {
 // hsum[j] = sum_{m=1..j} 1/(n-m+1), j = 0..k_del: the data-independent volume shrinkage of
 // reading A6, tabulated once at ns_init.
 __global__ void ns_hsum_kernel(double* hsum, int n, int k_del) {
-  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  // second table (FP64 transcendentals are slow on this part: once, not per iteration):
+  // hsum[k_del + 1 + j] = log(1 - e^{-1/(n-j)}), the log width factor of dead point j
+  for (int j = threadIdx.x; j < k_del; j += blockDim.x)
+    hsum[k_del + 1 + j] = log1p(-exp(-1.0 / (double)(n - j)));
+  if (threadIdx.x != 0) return;
   double acc = 0.0;
   hsum[0] = 0.0;
   for (int m = 1; m <= k_del; ++m) { acc += 1.0 / (double)(n - m + 1); hsum[m] = acc; }
 }
 void launch_ns_hsum(double* hsum, int n, int k_del, cudaStream_t st) {
-  ++g_launches; ns_hsum_kernel<<<1, 32, 0, st>>>(hsum, n, k_del);
+  ++g_launches; ns_hsum_kernel<<<1, 256, 0, st>>>(hsum, n, k_del);
 }
 
 // N3 gather: walker j <- live point start[j].  One thread per (site, walker): the walker index is
@@ -350,7 +353,7 @@ void launch_ns_store_walkers(const NsArgs& a, cudaStream_t st) {
 
 // N4: remaining = X mean_live(e^-S) / (Z + X mean_live(e^-S)); record; stop rule; live term.
 __global__ void __launch_bounds__(1024)
-ns_finish_kernel(NsArgs a, StepRecord* rec, int n_walk) {
+ns_finish_kernel(NsArgs a, StepRecord* rec, int n_walk, HostPoll* hp) {
   pdl_enter();
   __shared__ double scratch[33];
   __shared__ float smin_s[33];
@@ -394,11 +397,17 @@ ns_finish_kernel(NsArgs a, StepRecord* rec, int n_walk) {
     } else if (it + 1 >= a.max_iters) {
       ctrl->done = 2;   // dead-point log is full: stop without the live term
     }
+    if (hp) {           // report to the host's run loop (see HostPoll)
+      volatile HostPoll* v = hp;
+      v->done = ctrl->done; v->nan_flag = ctrl->nan_flag; v->chol_status = ctrl->chol_status;
+      __threadfence_system();
+      v->seq = it + 1;
+    }
   }
 }
 
-void launch_ns_finish(const NsArgs& a, StepRecord* rec, int n_walk, cudaStream_t st) {
-  ++g_launches; launch_pdl(ns_finish_kernel, 1, 1024, 0, st, a, rec, n_walk);
+void launch_ns_finish(const NsArgs& a, StepRecord* rec, int n_walk, HostPoll* hp, cudaStream_t st) {
+  ++g_launches; launch_pdl(ns_finish_kernel, 1, 1024, 0, st, a, rec, n_walk, hp);
 }
 
 // Posterior sample for `observables`: dead points (weight w_j e^{-S_j}) followed by the live
