@@ -58,8 +58,10 @@ def test_set_state_roundtrip_and_action_large_fields():
 
 
 # ------------------------------------------------------------------ C1 + C2 -------------------
+# (V <= 160: the one-CTA register-tile Cholesky, incl. V not a multiple of 4 or 8; above: blocked)
 @pytest.mark.parametrize("L,N", [(4, 1024), (10, 16384), (10, 1000), (15, 2000), (16, 4096), (18, 5000),
-                                 (11, 700), (12, 400)])
+                                 (11, 700), (12, 400), (1, 64), (2, 100), (3, 500), (5, 333), (6, 900),
+                                 (7, 777), (8, 2048), (9, 640)])
 def test_cov_chol(L, N):
     V = L * L
     phi = inputs.smooth_fields(L, N, seed=L)
@@ -165,7 +167,10 @@ def test_every_lattice_size_has_a_tensor_core_path():
 
 
 # ------------------------------------------------------------------ P1 + P2 -------------------
-@pytest.mark.parametrize("L,N,beta", [(4, 1024, 0.0), (10, 16384, 0.0), (10, 5000, 0.3)])
+# (N <= 16384: the 8-CTA cluster kernel, whole and ragged runs; above: the single-CTA kernel)
+@pytest.mark.parametrize("L,N,beta", [(4, 1024, 0.0), (10, 16384, 0.0), (10, 5000, 0.3), (4, 37, 0.0),
+                                      (5, 300, 0.2), (10, 2049, 0.0), (10, 8193, 0.1), (10, 16383, 0.0),
+                                      (4, 20000, 0.0), (4, 65536, 0.0)])
 def test_next_beta_and_weights(L, N, beta):
     h = new_smc(L, N, seed=5)
     if beta > 0:
@@ -184,6 +189,20 @@ def test_next_beta_and_weights(L, N, beta):
     assert info["dlogZ"] == pytest.approx(dlz_ref, abs=2e-5 * max(1.0, abs(dlz_ref)))
     assert B.log_Z(h) == pytest.approx(info["dlogZ"], rel=1e-12)
     h.close()
+
+
+@pytest.mark.parametrize("L,N", [(4, 1000), (10, 16384), (10, 5001)])
+def test_fused_scan_of_a_whole_step_matches_the_separate_scan(L, N):
+    """smc_step takes the integer CDF from the reweight kernel (P3 fused into P1 + P2); smc_reweight +
+    smc_resample run the stand-alone scan.  Same state, same seed: the same ancestors, so the same
+    number of distinct ones (the stand-alone path is bit-exact against the oracle, below)."""
+    ha, hb = new_smc(L, N, seed=9), new_smc(L, N, seed=9)
+    info = B.smc_step(ha)
+    w, _ = B.smc_reweight(hb)
+    anc = B.smc_resample(hb)
+    assert info["n_unique"] == len(np.unique(anc))
+    assert np.array_equal(anc, O.resample_systematic(w, O.word0(9, O.TAG_RESAMPLE, 0, 0)))
+    ha.close(); hb.close()
 
 
 def test_final_step_rule_and_fixed_delta():
