@@ -357,22 +357,19 @@ struct CholTiles {
   }
 };
 
-__global__ void __launch_bounds__(CT_THREADS)
-chol_small_kernel(const float* __restrict__ Sigma, float* __restrict__ Lc, int V, Ctrl* ctrl,
-                  int respect_done) {
-  pdl_enter();
-  __shared__ __align__(16) float Ap[2][CS_NB * CT_LD];   // column block q of A, k-major, buffer q & 1
-  __shared__ __align__(16) float Lp[2][CS_NB * CT_LD];   // panel p of L, k-major, buffer p & 1
-  __shared__ __align__(16) float Dn[2][CS_NB * CS_NB];   // diagonal block of panel p, k-major
-  __shared__ int failed_s;
-  if (respect_done && ctrl->done) return;
+// One factorisation pass of the V x V matrix S (row stride s_ld, lower triangle read) by a CTA of
+// CT_THREADS threads; L goes to `out` (row stride o_ld: global or shared memory), with zeros above
+// the diagonal if zero_upper.  *failed_s is set if a pivot fails.  Ends without a block barrier.
+__device__ __forceinline__ void chol_tiles_pass(const float* __restrict__ S, int s_ld, float* out, int o_ld,
+                                                int V, float add, bool zero_upper,
+                                                float (*Ap)[CS_NB * CT_LD], float (*Lp)[CS_NB * CT_LD],
+                                                float (*Dn)[CS_NB * CS_NB], int* failed_s) {
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   CholTiles T;
   T.nT = (V + 3) >> 2;
   const int ntiles = T.ntiles(), ntw = T.nwarps();
   const int nP = (V + CS_NB - 1) / CS_NB;
   const bool is_tile = warp < CT_TILE_WARPS, is_row = !is_tile && warp < CT_TILE_WARPS + CT_ROW_WARPS;
-
   // tile of this thread (numbered column by column: t -> column C ascending, rows R >= C)
   int R = 0, C = 0;
   const bool has_tile = is_tile && tid < ntiles;
@@ -383,7 +380,180 @@ chol_small_kernel(const float* __restrict__ Sigma, float* __restrict__ Lc, int V
     R = T.nT - 1 - uc;
   }
   const int r0 = 4 * R, c0 = 4 * C, q = C >> 1;
+  if (is_tile) {
+    if (warp >= ntw && zero_upper)        // idle tile warps: zeros above the diagonal
+      for (int x = warp - ntw; x < V; x += CT_TILE_WARPS - ntw)
+        for (int y = x + 1 + lane; y < V; y += 32) out[(size_t)x * o_ld + y] = 0.f;
+    if (warp < ntw) {
+      float a[4][4];
+#pragma unroll
+      for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const int x = r0 + i, y = c0 + j;
+          const float v = S[(size_t)min(x, V - 1) * s_ld + min(y, V - 1)];   // always in range
+          a[i][j] = (x < V && y < V) ? v + (x == y ? add : 0.f) : (x == y ? 1.f : 0.f);
+        }
+      // column blocks 0 and 1 receive no update from a tile warp: publish them right away
+      if (has_tile && q <= 1) {
+        float* dst = &Ap[q][(c0 - 8 * q) * CT_LD + r0];
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+          *reinterpret_cast<float4*>(dst + j * CT_LD) = make_float4(a[0][j], a[1][j], a[2][j], a[3][j]);
+      }
+      if (warp < T.owners(0)) bar_arrive(BAR_AP0, 32 * T.owners(0) + CT_RWT);
+      for (int p = 0; p < nP; ++p) {
+        const int lo1 = T.warp_lo(2 * p + 2), alo = T.warp_lo(2 * p + 4), buf = p & 1;
+        const int nM = 32 * (ntw - lo1) + 32 + CT_RWT;
+        if (warp < alo) {                                   // every tile of this warp is final
+          if (warp >= lo1) bar_arrive(BAR_M + buf, nM);     // (its block p + 1 tiles are in Ap)
+          break;
+        }
+        bar_sync(BAR_M + buf, nM);
+        // update from panel p for the tiles of column blocks >= p + 2
+        if (has_tile && q >= p + 2) {
+          const float* lp = &Lp[buf][0];
+#pragma unroll
+          for (int k = 0; k < CS_NB; ++k) {
+            const float4 lr = *reinterpret_cast<const float4*>(lp + k * CT_LD + r0);
+            const float4 lc = *reinterpret_cast<const float4*>(lp + k * CT_LD + c0);
+            const float lrv[4] = {lr.x, lr.y, lr.z, lr.w}, lcv[4] = {lc.x, lc.y, lc.z, lc.w};
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+#pragma unroll
+              for (int j = 0; j < 4; ++j) a[i][j] = fmaf(-lrv[i], lcv[j], a[i][j]);
+          }
+        }
+        bar_arrive(BAR_B + (buf ^ 1), 32 * (ntw - alo) + 32 + CT_RWT);   // B(p + 1): Lp[buf] read
+        // column block p + 2 is complete now: publish it (visible through M(p + 1))
+        if (has_tile && q == p + 2) {
+          float* dst = &Ap[q & 1][(c0 - 8 * q) * CT_LD + r0];
+#pragma unroll
+          for (int j = 0; j < 4; ++j)
+            *reinterpret_cast<float4*>(dst + j * CT_LD) = make_float4(a[0][j], a[1][j], a[2][j], a[3][j]);
+        }
+      }
+    }
+  } else if (is_row) {
+    const int r = tid - 32 * CT_TILE_WARPS;          // matrix row of this thread (fixed)
+    const bool live = r < CS_NB * nP;                // rows of the matrix padded to whole panels
+    if (r == 0) *failed_s = 0;
+    // rows [V, 4 nT) exist in the tiles as identity padding: their L entries are zero
+    if (r >= V) {
+#pragma unroll
+      for (int k = 0; k < 2 * CS_NB; ++k) (&Lp[0][0])[k * CT_LD + r] = 0.f;
+    }
+    float x[CS_NB];
+    bar_sync(BAR_AP0, 32 * T.owners(0) + CT_RWT);
+#pragma unroll
+    for (int k = 0; k < CS_NB; ++k) x[k] = (r < V) ? Ap[0][k * CT_LD + r] : (k == r ? 1.f : 0.f);
+    if (r < CS_NB) {
+#pragma unroll
+      for (int k = 0; k < CS_NB; ++k) Dn[0][k * CS_NB + r] = x[k];
+    }
+    bar_sync(BAR_B_PRO, CT_RWT);
+    for (int p = 0; p < nP; ++p) {
+      const int buf = p & 1, jb = CS_NB * p, ri = r - jb;
+      if (ri >= 0 && live) {
+        const float* dn = &Dn[buf][0];
+        float D[CS_NB][CS_NB];
+#pragma unroll
+        for (int k = 0; k < CS_NB; ++k) {
+          const float4 lo = *reinterpret_cast<const float4*>(dn + k * CS_NB);
+          const float4 hi = *reinterpret_cast<const float4*>(dn + k * CS_NB + 4);
+          D[0][k] = lo.x; D[1][k] = lo.y; D[2][k] = lo.z; D[3][k] = lo.w;
+          D[4][k] = hi.x; D[5][k] = hi.y; D[6][k] = hi.z; D[7][k] = hi.w;
+        }
+        bool bad = false;
+#pragma unroll
+        for (int k = 0; k < CS_NB; ++k) {
+          // pivots below the smallest normal number count as failures (the reciprocal square
+          // root flushes them); 1/sqrt(d) = SFU seed + one Newton step (~1 ulp)
+          const float d0 = D[k][k];
+          const bool ok = d0 >= 1.17549435e-38f;
+          bad |= !ok;
+          const float d = ok ? d0 : 1.f;
+          float inv = rsqrt_ftz(d0);
+          inv = ok ? inv : 1.f;
+          inv = inv * fmaf(-0.5f * d * inv, inv, 1.5f);
+          D[k][k] = d * inv;
+#pragma unroll
+          for (int i = k + 1; i < CS_NB; ++i) D[i][k] *= inv;
+          x[k] *= inv;
+#pragma unroll
+          for (int i = k + 1; i < CS_NB; ++i)
+#pragma unroll
+            for (int c = k + 1; c <= i; ++c) D[i][c] = fmaf(-D[i][k], D[c][k], D[i][c]);
+#pragma unroll
+          for (int c = k + 1; c < CS_NB; ++c) x[c] = fmaf(-x[k], D[c][k], x[c]);
+        }
+        if (bad) *failed_s = 1;
+        // rows of the diagonal block: their elimination reproduces the factor; zero above it
+#pragma unroll
+        for (int k = 1; k < CS_NB; ++k) if (k > ri) x[k] = 0.f;
+        float* lp = &Lp[buf][0];
+#pragma unroll
+        for (int k = 0; k < CS_NB; ++k) lp[k * CT_LD + r] = x[k];
+      }
+      const int nM = 32 * (ntw - T.warp_lo(2 * p + 2)) + 32 + CT_RWT;
+      if (p + 1 == nP) { bar_arrive(BAR_M + buf, nM); break; }
+      bar_sync(BAR_M + buf, nM);
+      if (ri >= CS_NB && live) {
+        // own entries of column block p + 1: A (panels < p applied by the tiles) minus panel p
+        const float* lp = &Lp[buf][jb + CS_NB];
+        const float* ap = &Ap[buf ^ 1][0];
+        float xn[CS_NB];
+#pragma unroll
+        for (int c = 0; c < CS_NB; ++c)
+          xn[c] = (r < V) ? ap[c * CT_LD + r] : (c == ri - CS_NB ? 1.f : 0.f);
+#pragma unroll
+        for (int k = 0; k < CS_NB; ++k) {
+          const float4 lo = *reinterpret_cast<const float4*>(lp + k * CT_LD);
+          const float4 hi = *reinterpret_cast<const float4*>(lp + k * CT_LD + 4);
+          const float l[CS_NB] = {lo.x, lo.y, lo.z, lo.w, hi.x, hi.y, hi.z, hi.w};
+#pragma unroll
+          for (int c = 0; c < CS_NB; ++c) xn[c] = fmaf(-x[k], l[c], xn[c]);
+        }
+#pragma unroll
+        for (int c = 0; c < CS_NB; ++c) x[c] = xn[c];
+        if (ri < 2 * CS_NB) {
+#pragma unroll
+          for (int c = 0; c < CS_NB; ++c) Dn[buf ^ 1][c * CS_NB + ri - CS_NB] = x[c];
+        }
+      }
+      // B(p): next diagonal block visible; readers of Lp[buf ^ 1] (panel p - 1) are done
+      bar_sync(BAR_B + buf, CT_RWT + (p >= 1 ? 32 * (ntw - T.warp_lo(2 * p + 2)) + 32 : 0));
+    }
+  } else {
+    // housekeeping warp: L from Lp to Lc panel by panel (and the zeros above the diagonal if
+    // every tile warp holds tiles)
+    if (zero_upper && ntw == CT_TILE_WARPS)
+      for (int x = 0; x < V; ++x)
+        for (int y = x + 1 + lane; y < V; y += 32) out[(size_t)x * o_ld + y] = 0.f;
+    for (int p = 0; p < nP; ++p) {
+      const int buf = p & 1, jb = CS_NB * p;
+      bar_sync(BAR_M + buf, 32 * (ntw - T.warp_lo(2 * p + 2)) + 32 + CT_RWT);
+      const float* lp = &Lp[buf][0];
+      for (int r = jb + lane; r < V; r += 32) {
+#pragma unroll
+        for (int k = 0; k < CS_NB; ++k)
+          if (jb + k < V && jb + k <= r) out[(size_t)r * o_ld + jb + k] = lp[k * CT_LD + r];
+      }
+      if (p + 2 < nP) bar_arrive(BAR_B + (buf ^ 1), 32 * (ntw - T.warp_lo(2 * p + 4)) + 32 + CT_RWT);
+    }
+  }
+}
 
+__global__ void __launch_bounds__(CT_THREADS)
+chol_small_kernel(const float* __restrict__ Sigma, float* __restrict__ Lc, int V, Ctrl* ctrl,
+                  int respect_done) {
+  pdl_enter();
+  __shared__ __align__(16) float Ap[2][CS_NB * CT_LD];   // column block q of A, k-major, buffer q & 1
+  __shared__ __align__(16) float Lp[2][CS_NB * CT_LD];   // panel p of L, k-major, buffer p & 1
+  __shared__ __align__(16) float Dn[2][CS_NB * CS_NB];   // diagonal block of panel p, k-major
+  __shared__ int failed_s;
+  if (respect_done && ctrl->done) return;
+  const int tid = threadIdx.x, lane = tid & 31;
   float tr = 0.f;
   int status = 0;
   for (int attempt = 0; attempt < 2; ++attempt) {
@@ -395,168 +565,7 @@ chol_small_kernel(const float* __restrict__ Sigma, float* __restrict__ Lc, int V
       tr = (float)t2;
     }
     const float add = attempt ? 1e-6f * tr / (float)V : 0.f;
-    if (is_tile) {
-      if (warp >= ntw && attempt == 0)        // idle tile warps: zeros above the diagonal
-        for (int x = warp - ntw; x < V; x += CT_TILE_WARPS - ntw)
-          for (int y = x + 1 + lane; y < V; y += 32) Lc[(size_t)x * V + y] = 0.f;
-      if (warp < ntw) {
-        float a[4][4];
-#pragma unroll
-        for (int i = 0; i < 4; ++i)
-#pragma unroll
-          for (int j = 0; j < 4; ++j) {
-            const int x = r0 + i, y = c0 + j;
-            const float v = Sigma[(size_t)min(x, V - 1) * V + min(y, V - 1)];   // always in range
-            a[i][j] = (x < V && y < V) ? v + (x == y ? add : 0.f) : (x == y ? 1.f : 0.f);
-          }
-        // column blocks 0 and 1 receive no update from a tile warp: publish them right away
-        if (has_tile && q <= 1) {
-          float* dst = &Ap[q][(c0 - 8 * q) * CT_LD + r0];
-#pragma unroll
-          for (int j = 0; j < 4; ++j)
-            *reinterpret_cast<float4*>(dst + j * CT_LD) = make_float4(a[0][j], a[1][j], a[2][j], a[3][j]);
-        }
-        if (warp < T.owners(0)) bar_arrive(BAR_AP0, 32 * T.owners(0) + CT_RWT);
-        for (int p = 0; p < nP; ++p) {
-          const int lo1 = T.warp_lo(2 * p + 2), alo = T.warp_lo(2 * p + 4), buf = p & 1;
-          const int nM = 32 * (ntw - lo1) + 32 + CT_RWT;
-          if (warp < alo) {                                   // every tile of this warp is final
-            if (warp >= lo1) bar_arrive(BAR_M + buf, nM);     // (its block p + 1 tiles are in Ap)
-            break;
-          }
-          bar_sync(BAR_M + buf, nM);
-          // update from panel p for the tiles of column blocks >= p + 2
-          if (has_tile && q >= p + 2) {
-            const float* lp = &Lp[buf][0];
-#pragma unroll
-            for (int k = 0; k < CS_NB; ++k) {
-              const float4 lr = *reinterpret_cast<const float4*>(lp + k * CT_LD + r0);
-              const float4 lc = *reinterpret_cast<const float4*>(lp + k * CT_LD + c0);
-              const float lrv[4] = {lr.x, lr.y, lr.z, lr.w}, lcv[4] = {lc.x, lc.y, lc.z, lc.w};
-#pragma unroll
-              for (int i = 0; i < 4; ++i)
-#pragma unroll
-                for (int j = 0; j < 4; ++j) a[i][j] = fmaf(-lrv[i], lcv[j], a[i][j]);
-            }
-          }
-          bar_arrive(BAR_B + (buf ^ 1), 32 * (ntw - alo) + 32 + CT_RWT);   // B(p + 1): Lp[buf] read
-          // column block p + 2 is complete now: publish it (visible through M(p + 1))
-          if (has_tile && q == p + 2) {
-            float* dst = &Ap[q & 1][(c0 - 8 * q) * CT_LD + r0];
-#pragma unroll
-            for (int j = 0; j < 4; ++j)
-              *reinterpret_cast<float4*>(dst + j * CT_LD) = make_float4(a[0][j], a[1][j], a[2][j], a[3][j]);
-          }
-        }
-      }
-    } else if (is_row) {
-      const int r = tid - 32 * CT_TILE_WARPS;          // matrix row of this thread (fixed)
-      const bool live = r < CS_NB * nP;                // rows of the matrix padded to whole panels
-      if (r == 0) failed_s = 0;
-      // rows [V, 4 nT) exist in the tiles as identity padding: their L entries are zero
-      if (r >= V) {
-#pragma unroll
-        for (int k = 0; k < 2 * CS_NB; ++k) (&Lp[0][0])[k * CT_LD + r] = 0.f;
-      }
-      float x[CS_NB];
-      bar_sync(BAR_AP0, 32 * T.owners(0) + CT_RWT);
-#pragma unroll
-      for (int k = 0; k < CS_NB; ++k) x[k] = (r < V) ? Ap[0][k * CT_LD + r] : (k == r ? 1.f : 0.f);
-      if (r < CS_NB) {
-#pragma unroll
-        for (int k = 0; k < CS_NB; ++k) Dn[0][k * CS_NB + r] = x[k];
-      }
-      bar_sync(BAR_B_PRO, CT_RWT);
-      for (int p = 0; p < nP; ++p) {
-        const int buf = p & 1, jb = CS_NB * p, ri = r - jb;
-        if (ri >= 0 && live) {
-          const float* dn = &Dn[buf][0];
-          float D[CS_NB][CS_NB];
-#pragma unroll
-          for (int k = 0; k < CS_NB; ++k) {
-            const float4 lo = *reinterpret_cast<const float4*>(dn + k * CS_NB);
-            const float4 hi = *reinterpret_cast<const float4*>(dn + k * CS_NB + 4);
-            D[0][k] = lo.x; D[1][k] = lo.y; D[2][k] = lo.z; D[3][k] = lo.w;
-            D[4][k] = hi.x; D[5][k] = hi.y; D[6][k] = hi.z; D[7][k] = hi.w;
-          }
-          bool bad = false;
-#pragma unroll
-          for (int k = 0; k < CS_NB; ++k) {
-            // pivots below the smallest normal number count as failures (the reciprocal square
-            // root flushes them); 1/sqrt(d) = SFU seed + one Newton step (~1 ulp)
-            const float d0 = D[k][k];
-            const bool ok = d0 >= 1.17549435e-38f;
-            bad |= !ok;
-            const float d = ok ? d0 : 1.f;
-            float inv = rsqrt_ftz(d0);
-            inv = ok ? inv : 1.f;
-            inv = inv * fmaf(-0.5f * d * inv, inv, 1.5f);
-            D[k][k] = d * inv;
-#pragma unroll
-            for (int i = k + 1; i < CS_NB; ++i) D[i][k] *= inv;
-            x[k] *= inv;
-#pragma unroll
-            for (int i = k + 1; i < CS_NB; ++i)
-#pragma unroll
-              for (int c = k + 1; c <= i; ++c) D[i][c] = fmaf(-D[i][k], D[c][k], D[i][c]);
-#pragma unroll
-            for (int c = k + 1; c < CS_NB; ++c) x[c] = fmaf(-x[k], D[c][k], x[c]);
-          }
-          if (bad) failed_s = 1;
-          // rows of the diagonal block: their elimination reproduces the factor; zero above it
-#pragma unroll
-          for (int k = 1; k < CS_NB; ++k) if (k > ri) x[k] = 0.f;
-          float* lp = &Lp[buf][0];
-#pragma unroll
-          for (int k = 0; k < CS_NB; ++k) lp[k * CT_LD + r] = x[k];
-        }
-        const int nM = 32 * (ntw - T.warp_lo(2 * p + 2)) + 32 + CT_RWT;
-        if (p + 1 == nP) { bar_arrive(BAR_M + buf, nM); break; }
-        bar_sync(BAR_M + buf, nM);
-        if (ri >= CS_NB && live) {
-          // own entries of column block p + 1: A (panels < p applied by the tiles) minus panel p
-          const float* lp = &Lp[buf][jb + CS_NB];
-          const float* ap = &Ap[buf ^ 1][0];
-          float xn[CS_NB];
-#pragma unroll
-          for (int c = 0; c < CS_NB; ++c)
-            xn[c] = (r < V) ? ap[c * CT_LD + r] : (c == ri - CS_NB ? 1.f : 0.f);
-#pragma unroll
-          for (int k = 0; k < CS_NB; ++k) {
-            const float4 lo = *reinterpret_cast<const float4*>(lp + k * CT_LD);
-            const float4 hi = *reinterpret_cast<const float4*>(lp + k * CT_LD + 4);
-            const float l[CS_NB] = {lo.x, lo.y, lo.z, lo.w, hi.x, hi.y, hi.z, hi.w};
-#pragma unroll
-            for (int c = 0; c < CS_NB; ++c) xn[c] = fmaf(-x[k], l[c], xn[c]);
-          }
-#pragma unroll
-          for (int c = 0; c < CS_NB; ++c) x[c] = xn[c];
-          if (ri < 2 * CS_NB) {
-#pragma unroll
-            for (int c = 0; c < CS_NB; ++c) Dn[buf ^ 1][c * CS_NB + ri - CS_NB] = x[c];
-          }
-        }
-        // B(p): next diagonal block visible; readers of Lp[buf ^ 1] (panel p - 1) are done
-        bar_sync(BAR_B + buf, CT_RWT + (p >= 1 ? 32 * (ntw - T.warp_lo(2 * p + 2)) + 32 : 0));
-      }
-    } else {
-      // housekeeping warp: L from Lp to Lc panel by panel (and the zeros above the diagonal if
-      // every tile warp holds tiles)
-      if (attempt == 0 && ntw == CT_TILE_WARPS)
-        for (int x = 0; x < V; ++x)
-          for (int y = x + 1 + lane; y < V; y += 32) Lc[(size_t)x * V + y] = 0.f;
-      for (int p = 0; p < nP; ++p) {
-        const int buf = p & 1, jb = CS_NB * p;
-        bar_sync(BAR_M + buf, 32 * (ntw - T.warp_lo(2 * p + 2)) + 32 + CT_RWT);
-        const float* lp = &Lp[buf][0];
-        for (int r = jb + lane; r < V; r += 32) {
-#pragma unroll
-          for (int k = 0; k < CS_NB; ++k)
-            if (jb + k < V && jb + k <= r) Lc[(size_t)r * V + jb + k] = lp[k * CT_LD + r];
-        }
-        if (p + 2 < nP) bar_arrive(BAR_B + (buf ^ 1), 32 * (ntw - T.warp_lo(2 * p + 4)) + 32 + CT_RWT);
-      }
-    }
+    chol_tiles_pass(Sigma, V, Lc, V, V, add, attempt == 0, Ap, Lp, Dn, &failed_s);
     __syncthreads();
     const int failed = failed_s;
     __syncthreads();
@@ -580,59 +589,71 @@ __global__ void chol_copy_kernel(const float* __restrict__ Sigma, float* __restr
   Lc[idx] = (y <= x) ? Sigma[idx] + add : 0.f;
 }
 
-// Diagonal block [j0, j0+nb) factorised in shared memory by one CTA (panel algorithm above).
-__global__ void __launch_bounds__(256)
+// Diagonal block [j0, j0+nb) factorised in place by one CTA (register tiles, chol_tiles_pass: every
+// entry is in registers before the first result is stored).
+__global__ void __launch_bounds__(CT_THREADS)
 chol_diag_kernel(float* __restrict__ A, int V, int j0, Ctrl* ctrl, int attempt,
                  int respect_done) {
-  __shared__ float T[64 * 65];
+  __shared__ __align__(16) float Ap[2][CS_NB * CT_LD];
+  __shared__ __align__(16) float Lp[2][CS_NB * CT_LD];
+  __shared__ __align__(16) float Dn[2][CS_NB * CS_NB];
   __shared__ int failed_s;
   if (chol_skip(ctrl, attempt, respect_done)) return;
   const int nb = min(64, V - j0);
-  if (threadIdx.x == 0) failed_s = 0;
-  for (int e = threadIdx.x; e < nb * nb; e += blockDim.x) {
-    const int r = e / nb, c = e - r * nb;
-    T[r * 65 + c] = (c <= r) ? A[(size_t)(j0 + r) * V + j0 + c] : 0.f;
-  }
+  float* blk = A + (size_t)j0 * V + j0;
+  chol_tiles_pass(blk, V, blk, V, nb, 0.f, false, Ap, Lp, Dn, &failed_s);
   __syncthreads();
-  chol_panels(T, 65, nb, &failed_s);
-  __syncthreads();
-  for (int e = threadIdx.x; e < nb * nb; e += blockDim.x) {
-    const int r = e / nb, c = e - r * nb;
-    if (c <= r) A[(size_t)(j0 + r) * V + j0 + c] = T[r * 65 + c];
-  }
   if (threadIdx.x == 0 && failed_s) atomicOr(&ctrl->chol_fail, attempt ? 2 : 1);
 }
 
-// Rows below the diagonal block: X L11^T = A21, one thread per row, L11 in shared memory.
+// Rows below the diagonal block: X L11^T = A21, one thread per row.  Right-looking: once x_c is
+// known (one multiplication by the tabulated 1 / l_cc) the 63 - c updates x_m -= x_c l_mc are
+// independent; L11 sits transposed in shared memory (Tt[c][m] = l_mc: 16-byte broadcast loads).
 __global__ void __launch_bounds__(64)
 chol_trsm_kernel(float* __restrict__ A, int V, int j0, const Ctrl* ctrl, int attempt,
                  int respect_done) {
-  __shared__ float T[64][65];
+  __shared__ __align__(16) float Tt[64][64];
+  __shared__ float inv[64];
   if (chol_skip(ctrl, attempt, respect_done)) return;
-  const int nb = min(64, V - j0);
-  for (int c = 0; c < nb; ++c)
-    T[threadIdx.x][c] = (threadIdx.x < nb && c <= threadIdx.x)
-                            ? A[(size_t)(j0 + threadIdx.x) * V + j0 + c] : 0.f;
+  const int nb = min(64, V - j0), t = threadIdx.x;
+  for (int c = 0; c < 64; ++c)                       // thread t: row t of L11 -> column t of Tt
+    Tt[c][t] = (t < nb && c <= t) ? A[(size_t)(j0 + t) * V + j0 + c] : 0.f;
+  inv[t] = t < nb ? 1.0f / A[(size_t)(j0 + t) * V + j0 + t] : 0.f;
   __syncthreads();
-  const int row = j0 + nb + blockIdx.x * 64 + threadIdx.x;
+  const int row = j0 + nb + blockIdx.x * 64 + t;
   if (row >= V) return;
   float x[64];
   float* a = A + (size_t)row * V + j0;
+  if (nb == 64 && (V & 3) == 0) {
 #pragma unroll
-  for (int c = 0; c < 64; ++c) x[c] = c < nb ? a[c] : 0.f;
-#pragma unroll
-  for (int c = 0; c < 64; ++c) {
-    if (c < nb) {
-      float v = x[c];
-#pragma unroll
-      for (int m = 0; m < 64; ++m)
-        if (m < c) v = fmaf(-x[m], T[c][m], v);
-      x[c] = v / T[c][c];
+    for (int c = 0; c < 64; c += 4) {
+      const float4 v = *reinterpret_cast<const float4*>(a + c);
+      x[c] = v.x; x[c + 1] = v.y; x[c + 2] = v.z; x[c + 3] = v.w;
     }
+  } else {
+#pragma unroll
+    for (int c = 0; c < 64; ++c) x[c] = c < nb ? a[c] : 0.f;
   }
 #pragma unroll
-  for (int c = 0; c < 64; ++c)
-    if (c < nb) a[c] = x[c];
+  for (int c = 0; c < 64; ++c) {
+    x[c] *= inv[c];                                  // (columns >= nb: inv = 0, x = 0)
+#pragma unroll
+    for (int m4 = (c + 1) & ~3; m4 < 64; m4 += 4) {
+      const float4 l = *reinterpret_cast<const float4*>(&Tt[c][m4]);
+      if (m4 > c) x[m4] = fmaf(-x[c], l.x, x[m4]);
+      if (m4 + 1 > c) x[m4 + 1] = fmaf(-x[c], l.y, x[m4 + 1]);
+      if (m4 + 2 > c) x[m4 + 2] = fmaf(-x[c], l.z, x[m4 + 2]);
+      x[m4 + 3] = fmaf(-x[c], l.w, x[m4 + 3]);
+    }
+  }
+  if (nb == 64 && (V & 3) == 0) {
+#pragma unroll
+    for (int c = 0; c < 64; c += 4) *reinterpret_cast<float4*>(a + c) = make_float4(x[c], x[c + 1], x[c + 2], x[c + 3]);
+  } else {
+#pragma unroll
+    for (int c = 0; c < 64; ++c)
+      if (c < nb) a[c] = x[c];
+  }
 }
 
 // Trailing update A22 -= L21 L21^T on the lower-triangular 64x64 tiles of rows/cols >= j1.
@@ -679,7 +700,7 @@ void launch_cholesky(const float* Sigma, float* Lc, int V, Ctrl* ctrl, int respe
                                                           respect_done);
     for (int j0 = 0; j0 < V; j0 += 64) {
       int j1 = min(V, j0 + 64);
-      ++g_launches; chol_diag_kernel<<<1, 256, 0, st>>>(Lc, V, j0, ctrl, attempt, respect_done);
+      ++g_launches; chol_diag_kernel<<<1, CT_THREADS, 0, st>>>(Lc, V, j0, ctrl, attempt, respect_done);
       int rows = V - j1;
       if (rows > 0) {
         ++g_launches; chol_trsm_kernel<<<(rows + 63) / 64, 64, 0, st>>>(Lc, V, j0, ctrl, attempt,
