@@ -196,111 +196,7 @@ __device__ __forceinline__ bool chol_skip(const Ctrl* ctrl, int attempt, int res
   return attempt == 1 && !(ctrl->chol_fail & 1);
 }
 
-// ------------------------------------------------------------------ panel routine -----------
-constexpr int CS_NB = 8;
-// In-place lower Cholesky of the n x n matrix in shared memory (row stride P), 8-column panels:
-// every row thread re-factorises the 8x8 diagonal block in registers (170 FMAs, no barrier) and
-// solves its own row, then the whole block applies the rank-8 update to the trailing lower
-// triangle.  *failed_s is set if a pivot is <= 0 (the factorisation then continues with a unit
-// pivot).  Used for the 64 x 64 diagonal blocks of the large-V path (chol_diag_kernel).
-__device__ __forceinline__ void chol_panels(float* sm, int P, int V, int* failed_s) {
-  const int tid = threadIdx.x;
-    for (int jb = 0; jb < V; jb += CS_NB) {
-      // ---- panel: rows r >= jb, one thread per row
-      const int r = jb + tid;
-      float D[CS_NB][CS_NB], x[CS_NB];
-      if (r < V) {
-#pragma unroll
-        for (int i = 0; i < CS_NB; ++i)
-#pragma unroll
-          for (int k = 0; k < CS_NB; ++k)
-            if (k <= i) D[i][k] = (jb + i < V) ? sm[(jb + i) * P + jb + k] : (i == k ? 1.f : 0.f);
-#pragma unroll
-        for (int k = 0; k < CS_NB; ++k) x[k] = (jb + k < V) ? sm[r * P + jb + k] : 0.f;
-      }
-      __syncthreads();        // every thread has read the diagonal block before its rows change
-      if (r < V) {
-        bool bad = false;
-        float invd[CS_NB];                   // 1 / l_kk: the solves multiply instead of dividing
-#pragma unroll
-        for (int k = 0; k < CS_NB; ++k) {
-          float d = D[k][k];
-          if (!(d > 0.f)) { bad = true; d = 1.f; }
-          // 1/sqrt(d) from the SFU seed plus one Newton step (~1 ulp), l_kk = d * that: two
-          // short dependent chains per pivot instead of an IEEE sqrt followed by an IEEE divide
-          float inv = rsqrtf(d);
-          inv = inv * fmaf(-0.5f * d * inv, inv, 1.5f);
-          const float sd = d * inv;
-          D[k][k] = sd;
-          invd[k] = inv;
-#pragma unroll
-          for (int i = k + 1; i < CS_NB; ++i) D[i][k] *= inv;
-#pragma unroll
-          for (int i = k + 1; i < CS_NB; ++i)
-#pragma unroll
-            for (int c = k + 1; c <= i; ++c) D[i][c] = fmaf(-D[i][k], D[c][k], D[i][c]);
-        }
-        if (bad) *failed_s = 1;
-        const int ri = r - jb;               // row inside the diagonal block if < CS_NB
-#pragma unroll
-        for (int k = 0; k < CS_NB; ++k) {
-          float v = x[k];
-#pragma unroll
-          for (int m = 0; m < k; ++m) v = fmaf(-x[m], D[k][m], v);
-          v = v * invd[k];
-          // rows of the diagonal block take the factor itself (their solve reproduces it up to
-          // rounding; use the shared value so that every thread sees the same l_ck)
-          if (ri < CS_NB) {
-            float dv = 0.f;
-#pragma unroll
-            for (int i = 0; i < CS_NB; ++i) if (i == ri) dv = (k <= i) ? D[i][k] : 0.f;
-            v = dv;
-          }
-          x[k] = v;
-        }
-#pragma unroll
-        for (int k = 0; k < CS_NB; ++k)
-          if (jb + k < V) sm[r * P + jb + k] = x[k];
-      }
-      __syncthreads();
-      // ---- trailing update: A[r][c] -= sum_k l_rk l_ck for jb+8 <= c <= r < V, one 2 x 2 tile of
-      // the lower triangle per thread: its 36 shared-memory loads are independent and the four
-      // FMA chains interleave (a warp per row with one element per lane ran nine dependent
-      // load-FMA-store rounds per thread)
-      const int j1 = jb + CS_NB;
-      if (j1 < V) {
-        const int nt = (V - j1 + 1) >> 1, ntiles = nt * (nt + 1) / 2;
-        for (int t = tid; t < ntiles; t += (int)blockDim.x) {
-          int tr, tc;
-          tri_tile(t, tr, tc);
-          const int r0 = j1 + 2 * tr, c0 = j1 + 2 * tc;
-          const bool r1ok = r0 + 1 < V, c1ok = c0 + 1 < V;
-          const float* pr0 = sm + r0 * P + jb; const float* pr1 = sm + (r1ok ? r0 + 1 : r0) * P + jb;
-          const float* pc0 = sm + c0 * P + jb; const float* pc1 = sm + (c1ok ? c0 + 1 : c0) * P + jb;
-          float lr0[CS_NB], lr1[CS_NB], lc0[CS_NB], lc1[CS_NB];
-#pragma unroll
-          for (int k = 0; k < CS_NB; ++k) { lr0[k] = pr0[k]; lr1[k] = pr1[k]; lc0[k] = pc0[k]; lc1[k] = pc1[k]; }
-          float a00 = sm[r0 * P + c0], a01 = 0.f, a10 = 0.f, a11 = 0.f;
-          const bool e01 = c1ok && c0 + 1 <= r0, e10 = r1ok, e11 = r1ok && c1ok;
-          if (e01) a01 = sm[r0 * P + c0 + 1];
-          if (e10) a10 = sm[(r0 + 1) * P + c0];
-          if (e11) a11 = sm[(r0 + 1) * P + c0 + 1];
-#pragma unroll
-          for (int k = 0; k < CS_NB; ++k) {
-            a00 = fmaf(-lr0[k], lc0[k], a00);
-            a01 = fmaf(-lr0[k], lc1[k], a01);
-            a10 = fmaf(-lr1[k], lc0[k], a10);
-            a11 = fmaf(-lr1[k], lc1[k], a11);
-          }
-          sm[r0 * P + c0] = a00;
-          if (e01) sm[r0 * P + c0 + 1] = a01;
-          if (e10) sm[(r0 + 1) * P + c0] = a10;
-          if (e11) sm[(r0 + 1) * P + c0 + 1] = a11;
-        }
-      }
-      __syncthreads();
-    }
-}
+constexpr int CS_NB = 8;               // panel width of the factorisations below
 
 // ---- V <= 160 in one CTA: register-resident state, warp-specialised --------------------------
 // Right-looking factorisation in 8-column panels (column block q = columns 8q .. 8q+7), no matrix

@@ -61,7 +61,8 @@ def irmh_lockstep(L, N, k, beta, seed, m0sq=-4.0, lam=1.0, t_start=0, fields="sm
 @pytest.mark.parametrize("L,N,k,beta,fields", [
     (4, 1024, 6, 0.4, "init"), (10, 4096, 4, 0.3, "smooth"), (10, 1000, 3, 1.0, "smooth"),
     (5, 333, 5, 0.7, "smooth"), (1, 200, 6, 1.0, "init"), (2, 129, 6, 0.5, "init"),
-    (9, 640, 3, 0.6, "smooth"), (16, 2048, 2, 0.2, "smooth"), (12, 700, 2, 0.1, "init")])
+    (9, 640, 3, 0.6, "smooth"), (16, 2048, 2, 0.2, "smooth"), (12, 700, 2, 0.1, "init"),
+    (10, 16384, 2, 0.5, "smooth"), (3, 77, 4, 0.3, "init"), (7, 500, 3, 0.8, "smooth")])
 def test_irmh_lockstep(L, N, k, beta, fields):
     rate = irmh_lockstep(L, N, k, beta, seed=53 + L, fields=fields, t_start=2 * k)
     assert 0.05 < rate < 1.0
