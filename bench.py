@@ -147,6 +147,156 @@ def run_reference(args, cfg):
     print(json.dumps(line))
 
 
+# ------------------------------------------------------------------ nested sampling workloads --
+def ns_config(name, cfg, gpus, iters):
+    return {"workload": "%s: nested sampling, phi^4 L=%d (V=%d) m0sq=%g lambda=%g, %d live points from "
+                        "N(0,I), %d deleted per iteration, %d %s steps per replacement, run to remaining "
+                        "evidence < %g" % (name, cfg["L"], cfg["L"] ** 2, cfg["m0sq"], cfg["lam"],
+                                           cfg["n_live"], cfg["k_del"], cfg["n_walk"],
+                                           "slice-sampling" if cfg.get("inner") == "slice"
+                                           else "constrained RW-Metropolis", cfg["stop_frac"]),
+            "L": cfg["L"], "V": cfg["L"] ** 2, "n_live": cfg["n_live"], "k_delete": cfg["k_del"],
+            "n_walk": cfg["n_walk"], "parallelism": "replicas x%d (no sharding)" % gpus,
+            "l2": "flushed between timed steps (256 MiB write)", "iterations_per_step": iters,
+            "unit_definition": "one site of one walker in one inner step"}
+
+
+def ns_oracle_run(cfg, seed, max_iter):
+    from oracle import oracle as O
+    t0 = time.perf_counter()
+    r = O.ns_run(cfg["L"], cfg["m0sq"], cfg["lam"], cfg["n_live"], cfg["k_del"], cfg["n_walk"], seed,
+                 stop_frac=cfg["stop_frac"], max_iter=max_iter, inner=cfg.get("inner", "rw"))
+    dt = time.perf_counter() - t0
+    return float(r["iters"]) * cfg["k_del"] * cfg["n_walk"] * cfg["L"] ** 2, dt, r["iters"], O.num_threads()
+
+
+def run_ns_reference(args, cfg):
+    """--impl reference on a nested-sampling workload: the oracle, a bounded number of iterations."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    max_iter = 8 if cfg.get("inner") == "slice" else 64
+    for w in range(args.warmup):
+        ns_oracle_run(cfg, 1000 + w, 2)
+    su, tt, its, thr = 0.0, 0.0, [], 1
+    for s in range(args.steps):
+        a, dt, it, thr = ns_oracle_run(cfg, s, max_iter)
+        su += a; tt += dt; its.append(it)
+    value = su / tt
+    print(json.dumps({"impl": "reference", "metric": "site-updates/s", "value": value,
+                      "unit": "site-updates/s", "n_gpus": args.gpus, "steps": args.steps,
+                      "warmup": args.warmup, "ms_per_step": 1e3 * tt / args.steps, "higher_is_better": True,
+                      "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                      "config": ns_config(args.workload, cfg, args.gpus, its),
+                      "cpu_baseline": {"value": value, "unit": "site-updates/s", "cores": thr,
+                                       "kind": "oracle",
+                                       "sample": "first %d iterations of the run per step" % max_iter},
+                      "e2e": {"value": value, "unit": "site-updates/s", "h2d_bytes_per_step": 0,
+                              "d2h_bytes_per_step": 0}, "gpu_launches": 0}))
+
+
+def run_ns(args, cfg):
+    """A nested-sampling workload (BASELINE configs[2] = C2, or PNS10): a step is one whole run."""
+    import torch
+    import torch.distributed as dist
+    from paper_2511_15196_b200 import binding as B
+    from paper_2511_15196_b200 import build, replicas
+    rank, world, local = replicas.rank_info()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --impl ours needs a CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = "cuda:%d" % local
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(dev))
+    if rank == 0:
+        build.build()
+    if world > 1:
+        dist.barrier()
+    B.load()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    pk = peaks()
+    mp = B.phi4_measure_peaks(args.peak_seconds, device=dev)
+    L, V, n, kd, nw = cfg["L"], cfg["L"] ** 2, cfg["n_live"], cfg["k_del"], cfg["n_walk"]
+    h = B.ns_init(L, cfg["m0sq"], cfg["lam"], n, kd, nw, 0, cfg["stop_frac"], 4096, device=dev)
+    if cfg.get("inner") == "slice":
+        B.ns_set_params(h, inner=1)
+
+    def step(seed, e2e):
+        flush.fill_(seed & 0xFF)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t0 = time.perf_counter()
+        e0.record()
+        B.smc_reset(h, seed)
+        it = B.ns_run(h)
+        e1.record()
+        nbytes = 0
+        if e2e:                                   # D2H: the dead-point log (S_E, M, log w) and log Z
+            d = B.ns_get_dead(h)
+            B.log_Z(h)
+            nbytes = sum(v.nbytes for v in d.values() if hasattr(v, "nbytes")) + 8
+        torch.cuda.synchronize()
+        return (time.perf_counter() - t0) * 1e3 if e2e else e0.elapsed_time(e1), it, nbytes
+
+    for w in range(max(args.warmup, 1)):
+        step(replicas.replica_seed(1000 + w, rank), False)
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    l0 = B.phi4_kernel_launches()
+    ms, its = 0.0, []
+    for s in range(args.steps):
+        dt, it, _ = step(replicas.replica_seed(s, rank), False)
+        ms += dt; its.append(it)
+    launches = B.phi4_kernel_launches() - l0
+    barrier()
+    clocks = sampler.finish()
+    e2e_ms, e2e_its, nbytes = 0.0, [], 0
+    for s in range(args.steps):
+        dt, it, nbytes = step(replicas.replica_seed(s, rank), True)
+        e2e_ms += dt; e2e_its.append(it)
+    barrier()
+    su, e2e_su = float(sum(its)) * kd * nw * V, float(sum(e2e_its)) * kd * nw * V
+    tmax, usum = replicas.reduce_stats({"ms": ms, "e2e_ms": e2e_ms}, {"su": su, "e2e_su": e2e_su}, device=dev)
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    ms, e2e_ms, su, e2e_su = tmax["ms"], tmax["e2e_ms"], usum["su"], usum["e2e_su"]
+    cpu = None
+    if not args.no_cpu_baseline:
+        a, dt, it, thr = ns_oracle_run(cfg, 0, 4 if cfg.get("inner") == "slice" else 48)
+        cpu = {"value": a / dt, "unit": "site-updates/s", "cores": thr, "kind": "oracle",
+               "sample": "first %d iterations of one run, %.1f s of CPU time" % (it, dt)}
+    achieved = ALU_OPS_PER_SITE_UPDATE * su / world / (ms * 1e-3) / 1e12
+    line = {"metric": "site-updates/s", "value": su / (ms * 1e-3), "unit": "site-updates/s", "n_gpus": world,
+            "steps": args.steps, "warmup": max(args.warmup, 1), "ms_per_step": ms / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+            "data": "synthetic", "config": ns_config(args.workload, cfg, world, its),
+            "us_per_iteration": 1e3 * ms / max(1, sum(its)), "logZ_last": B.log_Z(h),
+            "e2e": {"value": e2e_su / (e2e_ms * 1e-3), "unit": "site-updates/s", "h2d_bytes_per_step": 0,
+                    "d2h_bytes_per_step": int(nbytes), "ms_per_step": e2e_ms / args.steps,
+                    "note": "the live points are drawn on the device (INIT Philox stream): no host input"},
+            "gpu_launches": int(launches), "clocks": clocks,
+            "roofline": {"bound": "alu", "kernel": "whole iteration (select, evidence, covariance, Cholesky, "
+                         "walk): the walk runs on k_delete / 128 CTAs and is latency-bound",
+                         "achieved": achieved, "peak": mp["ffma_tlaneops"], "unit": "T lane-op/s",
+                         "frac": achieved / mp["ffma_tlaneops"],
+                         "ops": "lane-ops (FMA = 1), %d per walker site-update" % ALU_OPS_PER_SITE_UPDATE,
+                         "peak_source": "phi4_measure_peaks FP32 FMA rate of this run", "traffic": None},
+            "peaks_measured": dict(mp, hbm_gbs=pk["hbm_gbs"], bf16_tflops=pk["bf16_tflops"]),
+            "cpu_baseline": cpu}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def workload_config(name, cfg, gpus, temps=None, max_temps=None):
     c = {"workload": "%s: phi^4 L=%d (V=%d) m0sq=%g lambda=%g, N=%d particles from N(0,I), adaptive "
                      "tempering to beta=1 at ESS %.2f, %d %s per temperature, systematic resampling"
@@ -362,7 +512,12 @@ def main():
 
     from paper_2511_15196_b200 import inputs
     cfg = dict(inputs.CONFIGS[args.workload])
-    assert cfg["kind"] == "smc", "bench.py times SMC workloads (C0, C0g, C1, C3, C4, P10, P15, P18)"
+    if cfg["kind"] == "ns":                            # C2 (BASELINE configs[2]), PNS10
+        if args.impl == "reference":
+            run_ns_reference(args, cfg)
+        else:
+            run_ns(args, cfg)
+        return
     if args.kernel == "hmc":
         cfg["hmc"] = (args.hmc_eps, args.hmc_leapfrog)
         cfg["k"] = 2                                   # "short HMC trajectories"
