@@ -16,14 +16,24 @@ mean_kernel(const float* __restrict__ phi, int N, int ld, float* __restrict__ mu
   __shared__ double scratch[33];
   if (respect_done && ctrl->done) return;
   const float* row = phi + (size_t)blockIdx.x * ld;
-  // ld is a multiple of 128 and pad particles hold zeros: whole float4s, four partial sums
-  double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+  // ld is a multiple of 128 and pad particles hold zeros: whole float4s.  Two-level sums: at most 32
+  // terms in FP32 (four partial sums of eight), folded into FP64 (FP64 adds and conversions are
+  // ~40 times slower than FP32 on this part: one per term was half of this kernel's time at C1)
+  double a = 0.0;
   const float4* row4 = reinterpret_cast<const float4*>(row);
-  for (int i = threadIdx.x; i < ld / 4; i += blockDim.x) {
-    float4 v = row4[i];
-    a0 += (double)v.x; a1 += (double)v.y; a2 += (double)v.z; a3 += (double)v.w;
+  const int n4 = ld / 4, stride = blockDim.x;
+  for (int i0 = threadIdx.x; i0 < n4; i0 += 8 * stride) {
+    float f0 = 0.f, f1 = 0.f, f2 = 0.f, f3 = 0.f;
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      const int i = i0 + u * stride;
+      if (i < n4) {
+        const float4 v = row4[i];
+        f0 += v.x; f1 += v.y; f2 += v.z; f3 += v.w;
+      }
+    }
+    a += (double)((f0 + f1) + (f2 + f3));
   }
-  double a = (a0 + a1) + (a2 + a3);
   a = block_sum(a, scratch);
   if (threadIdx.x == 0) mu[blockIdx.x] = (float)(a / (double)N);
 }

@@ -49,21 +49,22 @@ syrk_tc_small_kernel(const float* __restrict__ phi, int N, int ld, int V,
     return;
   }
   const int i0 = blockIdx.x * TILE;
-  // centre + split: lane = site row (conflict-free 512-byte shared-memory stores), warp + loop =
-  // K-chunk of four particles (16-byte global loads; the tile is L2-resident)
+  // centre + split: a warp instruction covers 8 site rows x 4 K-chunks of four particles: 64
+  // contiguous bytes per row from global memory (whole 32-byte sectors; the tile is L2-resident)
+  // and, in shared memory, 8 x 16 B = all 32 banks per chunk (four wavefronts for 512 bytes)
   constexpr int NLD = ROWS * (TILE / 4) / THREADS;          // 16 loads per thread, all in flight
   float4 g[NLD];
 #pragma unroll
   for (int k = 0; k < NLD; ++k) {
     const int e = threadIdx.x + k * THREADS;
-    const int x = (e & 31) | ((e >> 10) << 5), c = (e >> 5) & 31;      // x = 32 (e / 1024) + lane
+    const int u = (e >> 5), x = 8 * (u & 15) + (e & 7), c = 4 * (u >> 4) + ((e >> 3) & 3);
     g[k] = x < V ? *reinterpret_cast<const float4*>(phi + (size_t)x * ld + i0 + 4 * c)
                  : make_float4(0.f, 0.f, 0.f, 0.f);
   }
 #pragma unroll
   for (int k = 0; k < NLD; ++k) {
     const int e = threadIdx.x + k * THREADS;
-    const int x = (e & 31) | ((e >> 10) << 5), c = (e >> 5) & 31;
+    const int u = (e >> 5), x = 8 * (u & 15) + (e & 7), c = 4 * (u >> 4) + ((e >> 3) & 3);
     float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
     if (x < V) {
       const float m = mu[x];
@@ -100,23 +101,29 @@ syrk_tc_small_kernel(const float* __restrict__ phi, int N, int ld, int V,
   }
   mbar_wait_relaxed(smem_u32(bar), 0);
   tc_fence_after();
-  // warp w: TMEM lane quarter w % 4 (rows x = 32 (w % 4) + lane), column half w / 4
-  const int x = (warp & 3) * 32 + lane, y0 = (warp >> 2) * 64;
-  float* out = partial + (size_t)blockIdx.x * V * V + (size_t)x * V;
-  const uint32_t tl = taddr + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)y0;
+  // warp w: TMEM lane quarter w % 4 (rows x = 32 (w % 4) + lane), column half w / 4.  The tile goes
+  // through shared memory (the operand space is free once the MMAs have committed; row stride 129:
+  // conflict-free both ways), so that the partial tile is written with whole 128-byte rows instead
+  // of one 4-byte store per lane and row (13 x the sectors)
+  float* stage = reinterpret_cast<float*>(smem);
+  constexpr int SP = ROWS + 1;
+  {
+    const int x = (warp & 3) * 32 + lane, y0 = (warp >> 2) * 64;
+    const uint32_t tl = taddr + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)y0;
 #pragma unroll
-  for (int cb = 0; cb < 64; cb += 16) {
-    uint32_t r[16];
-    tmem_ld16(tl + (uint32_t)cb, r);
-    tmem_ld_wait();
-    if (x < V) {
+    for (int cb = 0; cb < 64; cb += 16) {
+      uint32_t r[16];
+      tmem_ld16(tl + (uint32_t)cb, r);
+      tmem_ld_wait();
 #pragma unroll
-      for (int j = 0; j < 16; ++j) {
-        const int y = y0 + cb + j;
-        if (y <= x) out[y] = __uint_as_float(r[j]);
-      }
+      for (int j = 0; j < 16; ++j) stage[x * SP + y0 + cb + j] = __uint_as_float(r[j]);
     }
   }
+  tc_fence_before();
+  __syncthreads();
+  float* out = partial + (size_t)blockIdx.x * V * V;
+  for (int x = warp; x < V; x += THREADS / 32)
+    for (int y = lane; y <= x; y += 32) out[(size_t)x * V + y] = stage[x * SP + y];
   tc_fence_before();
   __syncthreads();
   if (warp == 0) tmem_dealloc(taddr, 128);
