@@ -727,53 +727,49 @@ __device__ __forceinline__ unsigned long long resample_threshold(int j, uint32_t
   return (q1 << 32) + r / n;
 }
 
-// a_j for K consecutive slots j0 .. j0+K-1 (slots >= N: -1): K binary searches in lock step, so
-// that their loads overlap
-template <int K>
-__device__ __forceinline__ void ancestors_of(const unsigned long long* __restrict__ C, int N, uint64_t seed,
-                                             const Ctrl* ctrl, int j0, int (&a)[K]) {
-  const unsigned long long T = ctrl->q_total;
-  if (ctrl->done || T == 0ull) {
-#pragma unroll
-    for (int m = 0; m < K; ++m) a[m] = (j0 + m >= 0 && j0 + m < N) ? j0 + m : -1;
-    return;
-  }
-  const uint32_t U = philox_draw(seed, TAG_RESAMPLE, (uint32_t)ctrl->temp_index, 0u, 0u).x;
-  unsigned long long t[K];
-  int lo[K], hi[K];
-#pragma unroll
-  for (int m = 0; m < K; ++m) {
-    const bool in = j0 + m >= 0 && j0 + m < N;
-    t[m] = in ? resample_threshold(j0 + m, U, T, N) : 0ull;
-    lo[m] = 0; hi[m] = in ? N : 0;                  // first index with C > t
-  }
-  for (int span = N; span > 0; span >>= 1) {        // ceil(log2(N + 1)) halvings bound every search
-#pragma unroll
-    for (int m = 0; m < K; ++m) {
-      const int mid = (lo[m] + hi[m]) >> 1;
-      if (lo[m] < hi[m]) {
-        if (C[mid] <= t[m]) lo[m] = mid + 1; else hi[m] = mid;
-      }
-    }
-  }
-#pragma unroll
-  for (int m = 0; m < K; ++m) a[m] = (j0 + m >= 0 && j0 + m < N) ? min(lo[m], N - 1) : -1;
-}
-
 __device__ __forceinline__ uint8_t z2_flip_of(uint64_t seed, const Ctrl* ctrl, int j, int z2) {
   if (!z2 || ctrl->done || ctrl->q_total == 0ull) return 0;
   return (uint8_t)(philox_draw(seed, TAG_Z2, (uint32_t)ctrl->temp_index, (uint32_t)j, 0u).x >> 31);
 }
 
-__global__ void ancestors_kernel(const unsigned long long* __restrict__ C, int N, uint64_t seed,
-                                 int32_t* __restrict__ anc, uint8_t* __restrict__ flip, int z2,
-                                 const Ctrl* ctrl) {
+// Two-level search: the block first reads 256 samples of the CDF (the last entry of each of 256
+// equal segments: one round trip to L2), every thread finds its segment in shared memory and
+// finishes inside it -- log2(N / 256) dependent global loads instead of log2(N).
+__global__ void __launch_bounds__(256)
+ancestors_kernel(const unsigned long long* __restrict__ C, int N, uint64_t seed,
+                 int32_t* __restrict__ anc, uint8_t* __restrict__ flip, int z2, const Ctrl* ctrl) {
   pdl_enter();
-  int j = blockIdx.x * blockDim.x + threadIdx.x;
+  __shared__ unsigned long long samp[256];
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  const unsigned long long T = ctrl->q_total;
+  if (ctrl->done || T == 0ull) {                   // (block-uniform) identity map
+    if (j < N) { anc[j] = j; flip[j] = 0; }
+    return;
+  }
+  const int seg = (N + 255) >> 8;                   // entries per segment
+  {
+    const long long e = (long long)(threadIdx.x + 1) * seg - 1;
+    samp[threadIdx.x] = C[e < N ? e : N - 1];
+  }
+  __syncthreads();
   if (j >= N) return;
-  int a[1];
-  ancestors_of<1>(C, N, seed, ctrl, j, a);
-  anc[j] = a[0];
+  const uint32_t U = philox_draw(seed, TAG_RESAMPLE, (uint32_t)ctrl->temp_index, 0u, 0u).x;
+  const unsigned long long t = resample_threshold(j, U, T, N);
+  int s0 = 0, s1 = 255;                             // first segment whose last entry is > t (one exists:
+                                                    // t < T): 256 outcomes, eight halvings
+#pragma unroll
+  for (int step = 0; step < 8; ++step) {
+    const int mid = (s0 + s1) >> 1;
+    if (samp[mid] <= t) s0 = mid + 1; else s1 = mid;
+  }
+  int lo = min(N, s0 * seg), hi = min(N, lo + seg);  // first index with C > t lies in [lo, hi]
+  for (int span = seg; span > 0; span >>= 1) {
+    const int mid = (lo + hi) >> 1;
+    if (lo < hi) {
+      if (C[mid] <= t) lo = mid + 1; else hi = mid;
+    }
+  }
+  anc[j] = min(lo, N - 1);
   flip[j] = z2_flip_of(seed, ctrl, j, z2);
 }
 
