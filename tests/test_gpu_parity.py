@@ -82,6 +82,36 @@ def test_cov_chol(L, N):
     h.close()
 
 
+@pytest.mark.parametrize("L,N", [(10, 4096), (12, 1000), (7, 300), (16, 3000)])
+def test_cholesky_is_deterministic_under_repetition(L, N):
+    """The one-CTA factorisation synchronises its warps with named barriers and keeps the matrix in
+    registers; the cluster reweight kernel exchanges partial sums through distributed shared memory.
+    A missing hand-off would show as run-to-run differences: 40 repetitions on the same state must give
+    the same bits, and 8 different states must all reconstruct."""
+    V = L * L
+    h = new_smc(L, N)
+    phi = inputs.smooth_fields(L, N, seed=3, corr=0.3)
+    B.smc_set_state(h, phi, 0.0, 0)
+    B.estimate_cov_chol(h)
+    L0, S0 = B.smc_get_chol(h).copy(), B.smc_get_cov(h).copy()
+    w0, i0 = B.smc_reweight(h)
+    for _ in range(40):
+        B.smc_reset(h, 0)                 # (the Newton iteration starts from the last delta: clear it)
+        B.smc_set_state(h, phi, 0.0, 0)
+        B.estimate_cov_chol(h)
+        assert np.array_equal(B.smc_get_chol(h), L0) and np.array_equal(B.smc_get_cov(h), S0)
+        w, i1 = B.smc_reweight(h)
+        assert np.array_equal(w, w0) and i1["delta"] == i0["delta"] and i1["dlogZ"] == i0["dlogZ"]
+    for seed in range(8):
+        f = inputs.smooth_fields(L, N, seed=20 + seed, corr=0.3)
+        B.smc_set_state(h, f, 0.0, 0)
+        B.estimate_cov_chol(h)
+        Lc = B.smc_get_chol(h).astype(np.float64)
+        _, Sref = O.covariance(f.astype(np.float64))
+        assert np.linalg.norm(Lc @ Lc.T - Sref) / np.linalg.norm(Sref) < 1e-5
+    h.close()
+
+
 def test_cholesky_jitter_retry_and_failure():
     L, N = 4, 8                         # N < V: rank-deficient covariance -> jitter retry (A4)
     phi = inputs.random_fields(16, N, seed=3)
