@@ -623,7 +623,8 @@ def main():
                                    how="phi4_measure_peaks (csrc/measure.cu): dense tcgen05 kind::tf32 "
                                        "M128 N256 K8 from resident smem operands on all SMs, burst = best "
                                        "of 5 launches, sustained = back to back for %.1f s; FP32 FMA and "
-                                       "IMAD.WIDE+LOP3: 8 chains/thread, 2048 threads/SM" % args.peak_seconds),
+                                       "IMAD.WIDE+LOP3 (and FP64 FMA, dfma_tlaneops): 8 chains/thread, 2048 "
+                                       "threads/SM" % args.peak_seconds),
             "large_v": large, "cpu_baseline": cpu}
     print(json.dumps(line))
     if world > 1:

@@ -149,6 +149,7 @@ typedef struct {
   double imad_wide_tlaneops;  /* 1e12 IMAD.WIDE + LOP3 pairs / s: the unit of a Philox round       */
   int32_t sms;
   int32_t reserved;
+  double dfma_tlaneops;       /* 1e12 FP64 FMA lane-operations / s (8 chains per thread): half the FP32 rate on a B200 */
 } phi4_peaks;
 int phi4_measure_peaks(double seconds, phi4_peaks* out, void* d_scratch, size_t scratch_bytes,
                        void* cuda_stream);

@@ -17,8 +17,8 @@ mean_kernel(const float* __restrict__ phi, int N, int ld, float* __restrict__ mu
   if (respect_done && ctrl->done) return;
   const float* row = phi + (size_t)blockIdx.x * ld;
   // ld is a multiple of 128 and pad particles hold zeros: whole float4s.  Two-level sums: at most 32
-  // terms in FP32 (four partial sums of eight), folded into FP64 (FP64 adds and conversions are
-  // ~40 times slower than FP32 on this part: one per term was half of this kernel's time at C1)
+  // terms in FP32 (four partial sums of eight), folded into FP64 -- one conversion and one FP64 add per
+  // 32 terms instead of per term (half of this latency-sized kernel's instructions at C1)
   double a = 0.0;
   const float4* row4 = reinterpret_cast<const float4*>(row);
   const int n4 = ld / 4, stride = blockDim.x;

@@ -88,6 +88,24 @@ __global__ void __launch_bounds__(1024, 2) peak_ffma_kernel(int iters, float* si
   if (s == 123456.789f) sink[0] = s;
 }
 
+__global__ void __launch_bounds__(1024, 2) peak_dfma_kernel(int iters, double* sink) {
+  double a[8];
+  const double x = 1.0 + 1e-12 * (double)threadIdx.x, y = 1e-3 * (double)(blockIdx.x & 7);
+#pragma unroll
+  for (int j = 0; j < 8; ++j) a[j] = (double)j + (double)threadIdx.x;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int u = 0; u < 16; ++u) {
+#pragma unroll
+      for (int j = 0; j < 8; ++j) a[j] = fma(a[j], x, y);
+    }
+  }
+  double s = 0.0;
+#pragma unroll
+  for (int j = 0; j < 8; ++j) s += a[j];
+  if (s == 123456.789) sink[0] = s;
+}
+
 __global__ void __launch_bounds__(1024, 2) peak_imad_kernel(int iters, uint32_t* sink) {
   uint32_t a[8];
 #pragma unroll
@@ -166,6 +184,14 @@ int phi4_measure_peaks(double seconds, phi4_peaks* out, void* d_scratch, size_t 
     best = 1e30;
     for (int r = 0; r < 5; ++r) { double t = timed(li, 1); if (t < best) best = t; }
     out->imad_wide_tlaneops = ops / best * 1e-12;
+    // FP64 FMA rate (half the FP32 rate on a B200: 64 lanes per SM)
+    const int itd = 64;
+    const double opsd = 8.0 * 16.0 * itd * 1024.0 * grid;
+    auto ld = [&]() { ++g_launches; peak_dfma_kernel<<<grid, 1024, 0, st>>>(itd, reinterpret_cast<double*>(sink)); };
+    timed(ld, 2);
+    best = 1e30;
+    for (int r = 0; r < 5; ++r) { double t = timed(ld, 1); if (t < best) best = t; }
+    out->dfma_tlaneops = opsd / best * 1e-12;
   }
   cudaEventDestroy(e0);
   cudaEventDestroy(e1);

@@ -327,57 +327,29 @@ void launch_mutate_generic(const MutateArgs& a, float* Lsplit, cudaStream_t st) 
 // (PAPER.md:53(ii), :200; reading A15).  whiten_kernel: W2[i] = |Lc^-1 (phi_i - mu)|^2 by forward
 // substitution, one warp per 32 particles, w in shared memory; FP64 accumulation (once per
 // temperature: the solve amplifies rounding by cond(Lc), and W2 enters every margin).
-// V <= 128.  FP64 arithmetic runs at ~1.5 TFLOP/s on this part (measured: the FP64 version of
-// this kernel took 111 us at C1 for 82 M FMAs), so the solve is carried in double-float
-// arithmetic on the FP32 pipe: w and every accumulator are (hi, lo) pairs, products and sums are
-// error-free transformations (Dekker / Knuth: two-product by FMA, two-sum), ~2^-44 relative.
-// Rows are taken four at a time: the products with the part of w already known run as eight
-// independent chains (four rows x even / odd columns), only the 4 x 4 diagonal block is serial.
-// The factor sits in shared memory (rows padded to a multiple of four, zeros beyond the row end)
-// and is read as broadcasts; a block serves WH_P particles.
+// V <= 128.  FP64 accumulation (the solve amplifies rounding by cond(Lc) and W2 enters every margin).
+// One thread per particle is a single dependent chain per SM sub-partition (16384 particles are 512
+// warps on 592 sub-partitions): 111 us at C1.  Here a block is WH_P particles x 4 row lanes (256
+// threads): thread (p, j) carries row x0 + j of the current 4-row block for particle p -- four
+// independent FP64 chains over the column phases -- and the j = 0 threads then finish the 4 x 4
+// diagonal block serially; two block barriers per row block.  The factor sits in shared memory as
+// FP32 (rows padded to a multiple of four, zeros beyond the row end) and is read as broadcasts.
 constexpr int WH_P = 64;
 __host__ __device__ inline int wh_vp(int V) { return (V + 3) & ~3; }
 __host__ __device__ inline size_t whiten_smem(int V) {
-  return ((size_t)wh_vp(V) * wh_vp(V) + (size_t)2 * V * WH_P) * sizeof(float);
+  return (size_t)wh_vp(V) * wh_vp(V) * sizeof(float) + ((size_t)V * WH_P + wh_vp(V)) * sizeof(double);
 }
-struct df2 { float h, l; };
-__device__ __forceinline__ df2 df_two_sum(float a, float b) {          // a + b exactly
-  const float t = __fadd_rn(a, b), z = __fsub_rn(t, a);
-  return {t, __fadd_rn(__fsub_rn(a, __fsub_rn(t, z)), __fsub_rn(b, z))};
-}
-__device__ __forceinline__ df2 df_add(df2 a, df2 b) {
-  df2 s = df_two_sum(a.h, b.h);
-  s.l = __fadd_rn(s.l, __fadd_rn(a.l, b.l));
-  return df_two_sum(s.h, s.l);
-}
-// s += L * w (L a float, w a pair): the chain through s.h is one addition long
-__device__ __forceinline__ void df_fma(float L, df2 w, df2& s) {
-  const float ph = __fmul_rn(L, w.h);
-  float pe = __fmaf_rn(L, w.h, -ph);
-  pe = __fmaf_rn(L, w.l, pe);
-  const float t = __fadd_rn(s.h, ph), z = __fsub_rn(t, s.h);
-  const float e = __fadd_rn(__fsub_rn(s.h, __fsub_rn(t, z)), __fsub_rn(ph, z));
-  s.h = t;
-  s.l = __fadd_rn(s.l, __fadd_rn(e, pe));
-}
-__device__ __forceinline__ df2 df_div(df2 a, float b) {               // a / b
-  const float q1 = __fdiv_rn(a.h, b);
-  const float r = __fadd_rn(__fmaf_rn(-q1, b, a.h), a.l);
-  return df_two_sum(q1, __fdiv_rn(r, b));
-}
-// Block = WH_P particles x 4 row lanes (256 threads): thread (p, j) carries row x0 + j of the
-// current 4-row block for particle p (four chains: the column phases); the j = 0 threads then
-// finish the 4 x 4 diagonal block serially.  Two block barriers per row block.
 __global__ void __launch_bounds__(4 * WH_P)
 whiten_small_kernel(const float* __restrict__ phi, const float* __restrict__ mu,
                     const float* __restrict__ Lc, float* __restrict__ W2, int N, int ld, int V,
                     const Ctrl* ctrl, int respect_done) {
   if (respect_done && ctrl->done) return;
-  extern __shared__ float whs[];
-  __shared__ float2 accs[3][WH_P];                             // row sums of rows x0 + 1 .. x0 + 3
+  extern __shared__ double whd[];
+  __shared__ double accs[3][WH_P];                              // row sums of rows x0 + 1 .. x0 + 3
   const int Vp = wh_vp(V);
-  float* Lf = whs;                                             // [Vp][Vp], zero outside the lower triangle
-  float2* wsm = reinterpret_cast<float2*>(Lf + (size_t)Vp * Vp);   // [V][WH_P] (hi, lo)
+  double* wsm = whd;                                            // [V][WH_P]
+  double* invd = wsm + (size_t)V * WH_P;                        // [Vp] 1 / L_xx
+  float* Lf = reinterpret_cast<float*>(invd + Vp);              // [Vp][Vp], zero outside the lower triangle
   const int tid = threadIdx.x, p = tid & (WH_P - 1), j = tid >> 6;   // j is warp-uniform
   const int i = blockIdx.x * WH_P + p;
   const bool live = i < N;
@@ -395,57 +367,52 @@ whiten_small_kernel(const float* __restrict__ phi, const float* __restrict__ mu,
       if (e < Vp * Vp) Lf[e] = v[u];
     }
   }
+  for (int x = tid; x < Vp; x += 4 * WH_P) invd[x] = x < V ? 1.0 / (double)Lc[(size_t)x * V + x] : 0.0;
   __syncthreads();
-  df2 w2 = {0.f, 0.f};
+  double w2 = 0.0;
   for (int x0 = 0; x0 < V; x0 += 4) {
     // the j = 0 threads need this row block's right-hand sides after the product loop
-    float fx[4], mx[4];
+    double rhs[4];
     if (j == 0) {
 #pragma unroll
       for (int m = 0; m < 4; ++m) {
         const int x = min(x0 + m, V - 1);
-        fx[m] = live ? phi[(size_t)x * ld + i] : 0.f;
-        mx[m] = mu[x];
+        rhs[m] = live ? (double)phi[(size_t)x * ld + i] - (double)mu[x] : 0.0;
       }
     }
     const float* row = Lf + (size_t)(x0 + j) * Vp;
-    df2 ac[4] = {{0.f, 0.f}, {0.f, 0.f}, {0.f, 0.f}, {0.f, 0.f}};
+    double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
     for (int y = 0; y < x0; y += 4) {          // x0 is a multiple of 4
       const float4 l = *reinterpret_cast<const float4*>(row + y);
-      const float2 u0 = wsm[y * WH_P + p], u1 = wsm[(y + 1) * WH_P + p];
-      const float2 u2 = wsm[(y + 2) * WH_P + p], u3 = wsm[(y + 3) * WH_P + p];
-      df_fma(l.x, df2{u0.x, u0.y}, ac[0]); df_fma(l.y, df2{u1.x, u1.y}, ac[1]);
-      df_fma(l.z, df2{u2.x, u2.y}, ac[2]); df_fma(l.w, df2{u3.x, u3.y}, ac[3]);
+      a0 = fma((double)l.x, wsm[y * WH_P + p], a0);
+      a1 = fma((double)l.y, wsm[(y + 1) * WH_P + p], a1);
+      a2 = fma((double)l.z, wsm[(y + 2) * WH_P + p], a2);
+      a3 = fma((double)l.w, wsm[(y + 3) * WH_P + p], a3);
     }
-    const df2 acc = df_add(df_add(ac[0], ac[1]), df_add(ac[2], ac[3]));
-    if (j > 0) accs[j - 1][p] = make_float2(acc.h, acc.l);
+    const double acc = (a0 + a1) + (a2 + a3);
+    if (j > 0) accs[j - 1][p] = acc;
     __syncthreads();
     if (j == 0) {
-      df2 wl[4];
+      double wl[4];
 #pragma unroll
       for (int m = 0; m < 4; ++m) {
         const int x = x0 + m;
         if (x < V) {
-          df2 s = acc;
-          if (m > 0) { const float2 t = accs[m - 1][p]; s = df2{t.x, t.y}; }
+          double s = m > 0 ? accs[m - 1][p] : acc;
           const float* rm = Lf + (size_t)x * Vp + x0;
 #pragma unroll
           for (int q = 0; q < 4; ++q)
-            if (q < m) df_fma(rm[q], wl[q], s);
-          // v = ((phi - mu) - s) / L_xx, the difference formed exactly
-          df2 v = df_add(df_two_sum(fx[m], -mx[m]), df2{-s.h, -s.l});
-          v = df_div(v, rm[m]);
+            if (q < m) s = fma((double)rm[q], wl[q], s);
+          const double v = (rhs[m] - s) * invd[x];
           wl[m] = v;
-          wsm[x * WH_P + p] = make_float2(v.h, v.l);
-          // w2 += v^2 = v.h^2 + 2 v.h v.l (+ v.l^2, below the pair's precision)
-          df_fma(v.h, v, w2);
-          w2.l = __fmaf_rn(v.l, v.h, w2.l);
+          wsm[x * WH_P + p] = v;
+          w2 = fma(v, v, w2);
         }
       }
     }
     __syncthreads();
   }
-  if (j == 0 && live) W2[i] = __fadd_rn(w2.h, w2.l);
+  if (j == 0 && live) W2[i] = (float)w2;
 }
 
 // Any V <= 800: one warp per 32 particles, the factor read through the read-only cache.

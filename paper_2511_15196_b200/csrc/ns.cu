@@ -281,7 +281,7 @@ void launch_ns_select_evidence(const NsArgs& a, cudaStream_t st) {
 // hsum[j] = sum_{m=1..j} 1/(n-m+1), j = 0..k_del: the data-independent volume shrinkage of
 // reading A6, tabulated once at ns_init.
 __global__ void ns_hsum_kernel(double* hsum, int n, int k_del) {
-  // second table (FP64 transcendentals are slow on this part: once, not per iteration):
+  // second table (data-independent, so once and not per iteration: an FP64 exp and log1p per dead point):
   // hsum[k_del + 1 + j] = log(1 - e^{-1/(n-j)}), the log width factor of dead point j
   for (int j = threadIdx.x; j < k_del; j += blockDim.x)
     hsum[k_del + 1 + j] = log1p(-exp(-1.0 / (double)(n - j)));
