@@ -200,7 +200,7 @@ def test_every_lattice_size_has_a_tensor_core_path():
 # (N <= 16384: the 8-CTA cluster kernel, whole and ragged runs; above: the single-CTA kernel)
 @pytest.mark.parametrize("L,N,beta", [(4, 1024, 0.0), (10, 16384, 0.0), (10, 5000, 0.3), (4, 37, 0.0),
                                       (5, 300, 0.2), (10, 2049, 0.0), (10, 8193, 0.1), (10, 16383, 0.0),
-                                      (4, 20000, 0.0), (4, 65536, 0.0)])
+                                      (4, 16385, 0.0), (4, 20000, 0.0), (4, 65536, 0.0), (10, 16384, 0.6)])
 def test_next_beta_and_weights(L, N, beta):
     h = new_smc(L, N, seed=5)
     if beta > 0:
