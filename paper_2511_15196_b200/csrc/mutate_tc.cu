@@ -198,7 +198,14 @@ __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
 // IRMH (NEXT row f2, reading A15): the proposal is mu + Lc z (the factor is packed with s = 1), the
 // margin gains log q(phi) - log q(phi') = 1/2 |z|^2 - 1/2 |w|^2, and an accepted particle's |w|^2
 // becomes |z|^2.  |z|^2 is summed where the normals are drawn.
-template <int LT, bool IRMH>
+// NARROW (populations of at most 148 x 32 particles: nested-sampling walkers, C0): a CTA owns 32
+// particles instead of 128.  They sit in TMEM lanes 0-31 (rows 32-127 of the A operand stay zero),
+// so only the four warps of lane quarter 0 can read the accumulator, but the proposal then lies
+// in shared memory and ALL sixteen epilogue warps share the stencil rows, the ring fills and the
+// tile copies of those 32 particles (lane = particle in every warp), and the eight producer
+// warps draw one quad per thread instead of four: a step is a latency chain, and the chain gets
+// shorter; four times as many SMs take part.
+template <int LT, bool IRMH, bool NARROW>
 __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParams p) {
   // programmatic dependent launch: barrier setup and the TMEM allocation touch nothing the
   // predecessor writes, so they run before the wait
@@ -225,7 +232,7 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
   // the first nitE ring fills of every step are produced by the epilogue warps (one quad per
   // thread, two steps ahead), the other nitP by the dedicated producers (two quads per thread)
   const int nitE = min(EPI_FILLS, nit - 1), nitP = nit - nitE;
-  const int i0 = blockIdx.x * TILE;
+  const int i0 = blockIdx.x * (NARROW ? 32 : TILE);
   uint32_t ncols = 32;
   while ((int)ncols < 2 * Vn) ncols <<= 1;
 
@@ -238,6 +245,11 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
   if (warp == 0) tmem_alloc(smem_u32(tmem_slot), ncols);
   if (IRMH)
     for (int e = threadIdx.x; e < ZSQ_BUFS * TILE; e += THREADS) zsq[e] = 0u;
+  if (NARROW) {            // rows 32..127 of every ring stage are never written again: zero once
+    float4* z4 = reinterpret_cast<float4*>(smem + lay.zring);
+    for (int e = threadIdx.x; e < STAGES * SLAB_BYTES / 16; e += THREADS) z4[e] = make_float4(0.f, 0.f, 0.f, 0.f);
+    fence_proxy_async();
+  }
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
@@ -308,234 +320,426 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
     __syncwarp();
   } else if (warp >= PROD_WARP0) {
     // ================================ normal producers =======================================
-    const int j = threadIdx.x - PROD_WARP0 * 32;         // 0..255
-    const int pr = j & (TILE - 1), half = j >> 7;
-    const int i = i0 + pr;
-    const int nq = (V + 3) >> 2;
-    uint8_t* zr = smem + lay.zring;
-    for (int t = 0; t < p.k; ++t) {
-      const uint32_t tt = p.t0 + (uint32_t)t;
-      // two ring stages (four Philox chains) per pass: the chains are independent, so their
-      // latencies overlap inside the warp
-      for (int it = 0; it < nitP; it += 2) {
-        const bool second = it + 1 < nitP;
-        U4 w[4];
-        bool ok[4];
-#pragma unroll
-        for (int c = 0; c < 4; ++c) {
-          const int q = 4 * (nitE + it + (c >> 1)) + 2 * (c & 1) + half;   // slab nitE + it + c/2, chunk 2 (c%2) + half
-          ok[c] = (i < p.N) && (q < nq) && (c < 2 || second);
-        }
-        if (second) {
-#pragma unroll
-          for (int c = 0; c < 4; ++c)
-            w[c] = philox4x32_10_rk((uint32_t)(4 * (nitE + it + (c >> 1)) + 2 * (c & 1) + half), (uint32_t)i, tt, p.tag_prop, p.rk);
-        } else {
-#pragma unroll
-          for (int c = 0; c < 2; ++c)
-            w[c] = philox4x32_10_rk((uint32_t)(4 * (nitE + it) + 2 * c + half), (uint32_t)i, tt, p.tag_prop, p.rk);
-          w[2] = w[0]; w[3] = w[1];
-        }
-#pragma unroll
-        for (int st2 = 0; st2 < 2; ++st2) {
-          if (st2 == 1 && !second) break;
-          float4 hv[2], lv[2];
-          float zz = 0.f;
-#pragma unroll
-          for (int e = 0; e < 2; ++e) {
-            const int c = 2 * st2 + e;
-            float z[4] = {0.f, 0.f, 0.f, 0.f};
-            if (ok[c]) {
-              box_muller_fast(w[c].x, w[c].y, z[0], z[1]);
-              box_muller_fast(w[c].z, w[c].w, z[2], z[3]);
-            }
-            if (IRMH) {                                  // R1: a ragged last quad is truncated at V
-              const int x0 = 4 * (4 * (nitE + it + (c >> 1)) + 2 * (c & 1) + half);
-#pragma unroll
-              for (int m = 0; m < 4; ++m) if (x0 + m < V) zz = fmaf(z[m], z[m], zz);
-            }
-            // hi = rna_tf32(z); lo = z - hi is exact and |lo| <= 2^-12 |z|: the tensor core's own
-            // truncation of lo to 11 bits costs 2^-23 |z|, below the dropped lo*lo term
-            hv[e].x = tf32_rna(z[0]); lv[e].x = z[0] - hv[e].x;
-            hv[e].y = tf32_rna(z[1]); lv[e].y = z[1] - hv[e].y;
-            hv[e].z = tf32_rna(z[2]); lv[e].z = z[2] - hv[e].z;
-            hv[e].w = tf32_rna(z[3]); lv[e].w = z[3] - hv[e].w;
+    if constexpr (NARROW) {
+      // thread (particle row, sub): one quad per pass -- warps 0-3 fill stage `it`, warps 4-7 stage
+      // `it + 1`, sub & 3 = the stage's 16-byte K-chunk
+      const int j = threadIdx.x - PROD_WARP0 * 32;       // 0..255
+      const int pr = j & 31, sub = j >> 5, so = sub >> 2, c = sub & 3;
+      const int i = i0 + pr;
+      const int nq = (V + 3) >> 2;
+      uint8_t* zr = smem + lay.zring;
+      for (int t = 0; t < p.k; ++t) {
+        const uint32_t tt = p.t0 + (uint32_t)t;
+        for (int it = 0; it < nitP; it += 2) {
+          if (it + so >= nitP) continue;                  // (warp-uniform: so is)
+          const int q = 4 * (nitE + it + so) + c;
+          float z[4] = {0.f, 0.f, 0.f, 0.f};
+          if (i < p.N && q < nq) {
+            const U4 w = philox4x32_10_rk((uint32_t)q, (uint32_t)i, tt, p.tag_prop, p.rk);
+            box_muller_fast(w.x, w.y, z[0], z[1]);
+            box_muller_fast(w.z, w.w, z[2], z[3]);
           }
-          const int n = t * nit + nitE + it + st2, s = n % STAGES;    // ring slot and use of fill n
+          float4 hv, lv;
+          hv.x = tf32_rna(z[0]); lv.x = z[0] - hv.x;  hv.y = tf32_rna(z[1]); lv.y = z[1] - hv.y;
+          hv.z = tf32_rna(z[2]); lv.z = z[2] - hv.z;  hv.w = tf32_rna(z[3]); lv.w = z[3] - hv.w;
+          const int n = t * nit + nitE + it + so, sl = n % STAGES;
           const uint32_t ph = (uint32_t)(n / STAGES) & 1u;
-          mbar_wait_relaxed(zempty(s), ph ^ 1);
-          uint8_t* st = zr + (size_t)s * SLAB_BYTES + (size_t)half * CHUNK_BYTES + (size_t)pr * 16;
-          *reinterpret_cast<float4*>(st) = hv[0];
-          *reinterpret_cast<float4*>(st + 2 * CHUNK_BYTES) = hv[1];
-          *reinterpret_cast<float4*>(st + 4 * CHUNK_BYTES) = lv[0];
-          *reinterpret_cast<float4*>(st + 6 * CHUNK_BYTES) = lv[1];
-          if (IRMH) atomicAdd(&zsq[(t & (ZSQ_BUFS - 1)) * TILE + pr], __float2uint_rn(zz * ZSQ_SCALE));
+          mbar_wait_relaxed(zempty(sl), ph ^ 1);
+          uint8_t* st = zr + (size_t)sl * SLAB_BYTES + (size_t)c * CHUNK_BYTES + (size_t)pr * 16;
+          *reinterpret_cast<float4*>(st) = hv;
+          *reinterpret_cast<float4*>(st + 4 * CHUNK_BYTES) = lv;
           fence_proxy_async();
           __syncwarp();
-          if (lane == 0) mbar_arrive_n(zfull(s), 2);         // 8 warps x 2 = the 16 expected
+          if (lane == 0) mbar_arrive_n(zfull(sl), 4);       // 4 warps x 4 = the 16 expected
+        }
+      }
+    } else {
+      const int j = threadIdx.x - PROD_WARP0 * 32;         // 0..255
+      const int pr = j & (TILE - 1), half = j >> 7;
+      const int i = i0 + pr;
+      const int nq = (V + 3) >> 2;
+      uint8_t* zr = smem + lay.zring;
+      for (int t = 0; t < p.k; ++t) {
+        const uint32_t tt = p.t0 + (uint32_t)t;
+        // two ring stages (four Philox chains) per pass: the chains are independent, so their
+        // latencies overlap inside the warp
+        for (int it = 0; it < nitP; it += 2) {
+          const bool second = it + 1 < nitP;
+          U4 w[4];
+          bool ok[4];
+  #pragma unroll
+          for (int c = 0; c < 4; ++c) {
+            const int q = 4 * (nitE + it + (c >> 1)) + 2 * (c & 1) + half;   // slab nitE + it + c/2, chunk 2 (c%2) + half
+            ok[c] = (i < p.N) && (q < nq) && (c < 2 || second);
+          }
+          if (second) {
+  #pragma unroll
+            for (int c = 0; c < 4; ++c)
+              w[c] = philox4x32_10_rk((uint32_t)(4 * (nitE + it + (c >> 1)) + 2 * (c & 1) + half), (uint32_t)i, tt, p.tag_prop, p.rk);
+          } else {
+  #pragma unroll
+            for (int c = 0; c < 2; ++c)
+              w[c] = philox4x32_10_rk((uint32_t)(4 * (nitE + it) + 2 * c + half), (uint32_t)i, tt, p.tag_prop, p.rk);
+            w[2] = w[0]; w[3] = w[1];
+          }
+  #pragma unroll
+          for (int st2 = 0; st2 < 2; ++st2) {
+            if (st2 == 1 && !second) break;
+            float4 hv[2], lv[2];
+            float zz = 0.f;
+  #pragma unroll
+            for (int e = 0; e < 2; ++e) {
+              const int c = 2 * st2 + e;
+              float z[4] = {0.f, 0.f, 0.f, 0.f};
+              if (ok[c]) {
+                box_muller_fast(w[c].x, w[c].y, z[0], z[1]);
+                box_muller_fast(w[c].z, w[c].w, z[2], z[3]);
+              }
+              if (IRMH) {                                  // R1: a ragged last quad is truncated at V
+                const int x0 = 4 * (4 * (nitE + it + (c >> 1)) + 2 * (c & 1) + half);
+  #pragma unroll
+                for (int m = 0; m < 4; ++m) if (x0 + m < V) zz = fmaf(z[m], z[m], zz);
+              }
+              // hi = rna_tf32(z); lo = z - hi is exact and |lo| <= 2^-12 |z|: the tensor core's own
+              // truncation of lo to 11 bits costs 2^-23 |z|, below the dropped lo*lo term
+              hv[e].x = tf32_rna(z[0]); lv[e].x = z[0] - hv[e].x;
+              hv[e].y = tf32_rna(z[1]); lv[e].y = z[1] - hv[e].y;
+              hv[e].z = tf32_rna(z[2]); lv[e].z = z[2] - hv[e].z;
+              hv[e].w = tf32_rna(z[3]); lv[e].w = z[3] - hv[e].w;
+            }
+            const int n = t * nit + nitE + it + st2, s = n % STAGES;    // ring slot and use of fill n
+            const uint32_t ph = (uint32_t)(n / STAGES) & 1u;
+            mbar_wait_relaxed(zempty(s), ph ^ 1);
+            uint8_t* st = zr + (size_t)s * SLAB_BYTES + (size_t)half * CHUNK_BYTES + (size_t)pr * 16;
+            *reinterpret_cast<float4*>(st) = hv[0];
+            *reinterpret_cast<float4*>(st + 2 * CHUNK_BYTES) = hv[1];
+            *reinterpret_cast<float4*>(st + 4 * CHUNK_BYTES) = lv[0];
+            *reinterpret_cast<float4*>(st + 6 * CHUNK_BYTES) = lv[1];
+            if (IRMH) atomicAdd(&zsq[(t & (ZSQ_BUFS - 1)) * TILE + pr], __float2uint_rn(zz * ZSQ_SCALE));
+            fence_proxy_async();
+            __syncwarp();
+            if (lane == 0) mbar_arrive_n(zfull(s), 2);         // 8 warps x 2 = the 16 expected
+          }
         }
       }
     }
   } else {
     // ================================ epilogue ==============================================
-    const int Q = warp & 3, g = warp >> 2;       // lane quarter, site part
-    const int pr = Q * 32 + lane;                // particle row = TMEM lane
-    const int i = i0 + pr;
-    const bool live = i < p.N;
-    const int L = LT > 0 ? LT : p.L;
-    const float hm = 2.0f * p.kappa + 0.5f * p.m0sq, lam = p.lam, kap = p.kappa;   // coefficient of phi^2 in the Laplacian form
-    float* cur = tile0 + pr;
-    float* oth = tile1 + pr;
-    for (int x = g; x < V; x += EPI_PARTS) cur[x * TILE] = live ? p.phi[(size_t)x * p.ld + i] : 0.f;
-    float Si = live ? p.S[i] : 0.f, Ui = live ? p.U0[i] : 0.f;
-    float Wi = (IRMH && live) ? p.W2[i] : 0.f;          // |Lc^-1 (phi - mu)|^2 of the current state
-    float* zzs = reinterpret_cast<float*>(smem + lay.zzs);
-    const float beta = (float)p.ctrl->beta, S_star = (float)p.ctrl->S_star;
-    unsigned nacc = 0;
-    const uint32_t tlane = taddr + ((uint32_t)(Q * 32) << 16);
-    named_bar_sync(1 + Q, 32 * EPI_PARTS);
-    float* lus = reinterpret_cast<float*>(part + EPI_PARTS * TILE);
-    uint8_t* zr = smem + lay.zring;
-    const int nq = (V + 3) >> 2;
-    // this thread's share of the normals of step t: quad 4 it + g of its own particle row
-    auto fill = [&](int t) {
-      // two stages per pass: both Philox chains first, then the maps and the stores
-      for (int e0 = 0; e0 < nitE; e0 += 2) {
-        U4 w[2];
-#pragma unroll
-        for (int e = 0; e < 2; ++e)
-          if (e0 + e < nitE) w[e] = philox4x32_10_rk((uint32_t)(4 * (e0 + e) + g), (uint32_t)i, p.t0 + (uint32_t)t, p.tag_prop, p.rk);
-#pragma unroll
-        for (int e = 0; e < 2; ++e) {
-          if (e0 + e >= nitE) break;
-          const int it = e0 + e, q = 4 * it + g;
-          float z[4] = {0.f, 0.f, 0.f, 0.f};
-          if (live && q < nq) {
-            box_muller_fast(w[e].x, w[e].y, z[0], z[1]);
-            box_muller_fast(w[e].z, w[e].w, z[2], z[3]);
-          }
-          if (IRMH) {                                    // R1: a ragged last quad is truncated at V
-            float zz = 0.f;
-#pragma unroll
-            for (int m = 0; m < 4; ++m) if (4 * q + m < V) zz = fmaf(z[m], z[m], zz);
-            atomicAdd(&zsq[(t & (ZSQ_BUFS - 1)) * TILE + pr], __float2uint_rn(zz * ZSQ_SCALE));
-          }
-          float4 hv, lv;
-          hv.x = tf32_rna(z[0]); lv.x = z[0] - hv.x;  hv.y = tf32_rna(z[1]); lv.y = z[1] - hv.y;
-          hv.z = tf32_rna(z[2]); lv.z = z[2] - hv.z;  hv.w = tf32_rna(z[3]); lv.w = z[3] - hv.w;
-          const int n = t * nit + it, s = n % STAGES;
+    if constexpr (NARROW) {
+      // ---- 32 particles: lane = particle in every warp; warp e = 4 g + Q of 16 shares the work
+      const int Q = warp & 3, g = warp >> 2, e16 = 4 * g + Q;
+      const int pr = lane, i = i0 + pr;
+      const bool live = i < p.N;
+      const int L = LT > 0 ? LT : p.L;
+      const float hm = 2.0f * p.kappa + 0.5f * p.m0sq, lam = p.lam, kap = p.kappa;
+      float* cur = tile0 + pr;
+      float* oth = tile1 + pr;
+      for (int x = e16; x < V; x += EPI_WARPS) cur[x * TILE] = live ? p.phi[(size_t)x * p.ld + i] : 0.f;
+      float Si = live ? p.S[i] : 0.f, Ui = live ? p.U0[i] : 0.f;
+      const float beta = (float)p.ctrl->beta, S_star = (float)p.ctrl->S_star;
+      unsigned nacc = 0;
+      const uint32_t tlane = taddr;                         // TMEM lanes 0..31
+      constexpr int NB_ALL = 6;                             // named barrier of the 16 epilogue warps
+      named_bar_sync(NB_ALL, 32 * EPI_WARPS);
+      float* lus = reinterpret_cast<float*>(part + EPI_PARTS * TILE);
+      uint8_t* zr = smem + lay.zring;
+      const int nq = (V + 3) >> 2;
+      // ring fills of step t by the epilogue warps: stage `it` (< nitE <= 2) chunk g by the warps with
+      // Q == it; every warp arrives once per stage (the barrier expects all sixteen)
+      auto fill = [&](int t) {
+        for (int it = 0; it < nitE; ++it) {
+          const int n = t * nit + it, sl = n % STAGES;
           const uint32_t ph = (uint32_t)(n / STAGES) & 1u;
-          mbar_wait_relaxed(zempty(s), ph ^ 1);
-          uint8_t* st = zr + (size_t)s * SLAB_BYTES + (size_t)g * CHUNK_BYTES + (size_t)pr * 16;
-          *reinterpret_cast<float4*>(st) = hv;
-          *reinterpret_cast<float4*>(st + 4 * CHUNK_BYTES) = lv;
-          fence_proxy_async();
+          mbar_wait_relaxed(zempty(sl), ph ^ 1);       // (every arriver: the slot's last use is over)
+          if (Q == it) {
+            const int q = 4 * it + g;
+            float z[4] = {0.f, 0.f, 0.f, 0.f};
+            if (live && q < nq) {
+              const U4 w = philox4x32_10_rk((uint32_t)q, (uint32_t)i, p.t0 + (uint32_t)t, p.tag_prop, p.rk);
+              box_muller_fast(w.x, w.y, z[0], z[1]);
+              box_muller_fast(w.z, w.w, z[2], z[3]);
+            }
+            float4 hv, lv;
+            hv.x = tf32_rna(z[0]); lv.x = z[0] - hv.x;  hv.y = tf32_rna(z[1]); lv.y = z[1] - hv.y;
+            hv.z = tf32_rna(z[2]); lv.z = z[2] - hv.z;  hv.w = tf32_rna(z[3]); lv.w = z[3] - hv.w;
+            uint8_t* st = zr + (size_t)sl * SLAB_BYTES + (size_t)g * CHUNK_BYTES + (size_t)pr * 16;
+            *reinterpret_cast<float4*>(st) = hv;
+            *reinterpret_cast<float4*>(st + 4 * CHUNK_BYTES) = lv;
+            fence_proxy_async();
+          }
           __syncwarp();
-          if (lane == 0) mbar_arrive(zfull(s));
+          if (lane == 0) mbar_arrive(zfull(sl));
         }
-      }
-    };
-    // the epilogue warps produce the FIRST slabs of a step and run two steps ahead: the MMAs of
-    // step t + 1 then never wait for a warp that is itself waiting for the MMAs of step t
-    fill(0);
-    if (p.k > 1) fill(1);
-    for (int t = 0; t < p.k; ++t) {
-      const int buf = t & 1;
-      mbar_wait_relaxed(dfull(buf), (t >> 1) & 1);
-      tc_fence_after();
-      // pass 1: phi' = phi + d on this part's 16-column blocks (d carries the step scale s); two
-      // TMEM loads in flight per wait
-      for (int cb = 16 * g; cb < Vn; cb += 32 * EPI_PARTS) {
-        uint32_t r0[16], r1[16];
-        const int cb1 = cb + 16 * EPI_PARTS;
-        const bool two = cb1 < Vn;
-        tmem_ld16(tlane + (uint32_t)(buf * Vn + cb), r0);
-        if (two) tmem_ld16(tlane + (uint32_t)(buf * Vn + cb1), r1);
-        tmem_ld_wait();
-        const float* ci = cur + cb * TILE; float* oi = oth + cb * TILE;
-        if (cb + 16 <= V) {
-#pragma unroll
-          for (int jj = 0; jj < 16; ++jj) oi[jj * TILE] = (IRMH ? __ldg(p.mu + cb + jj) : ci[jj * TILE]) + __uint_as_float(r0[jj]);
-        } else {
-#pragma unroll
-          for (int jj = 0; jj < 16; ++jj)
-            if (cb + jj < V) oi[jj * TILE] = (IRMH ? __ldg(p.mu + cb + jj) : ci[jj * TILE]) + __uint_as_float(r0[jj]);
-        }
-        if (two) {
-          ci = cur + cb1 * TILE; oi = oth + cb1 * TILE;
-          if (cb1 + 16 <= V) {
-#pragma unroll
-            for (int jj = 0; jj < 16; ++jj) oi[jj * TILE] = (IRMH ? __ldg(p.mu + cb1 + jj) : ci[jj * TILE]) + __uint_as_float(r1[jj]);
-          } else {
+      };
+      fill(0);
+      if (p.k > 1) fill(1);
+      for (int t = 0; t < p.k; ++t) {
+        const int buf = t & 1;
+        mbar_wait_relaxed(dfull(buf), (t >> 1) & 1);
+        tc_fence_after();
+        // pass 1 (the four warps of lane quarter 0): phi' = phi + d on 16-column blocks
+        if (Q == 0) {
+          for (int cb = 16 * g; cb < Vn; cb += 32 * EPI_PARTS) {
+            uint32_t r0[16], r1[16];
+            const int cb1 = cb + 16 * EPI_PARTS;
+            const bool two = cb1 < Vn;
+            tmem_ld16(tlane + (uint32_t)(buf * Vn + cb), r0);
+            if (two) tmem_ld16(tlane + (uint32_t)(buf * Vn + cb1), r1);
+            tmem_ld_wait();
+            const float* ci = cur + cb * TILE; float* oi = oth + cb * TILE;
 #pragma unroll
             for (int jj = 0; jj < 16; ++jj)
-              if (cb1 + jj < V) oi[jj * TILE] = (IRMH ? __ldg(p.mu + cb1 + jj) : ci[jj * TILE]) + __uint_as_float(r1[jj]);
+              if (cb + jj < V) oi[jj * TILE] = ci[jj * TILE] + __uint_as_float(r0[jj]);
+            if (two) {
+              ci = cur + cb1 * TILE; oi = oth + cb1 * TILE;
+#pragma unroll
+              for (int jj = 0; jj < 16; ++jj)
+                if (cb1 + jj < V) oi[jj * TILE] = ci[jj * TILE] + __uint_as_float(r1[jj]);
+            }
           }
         }
-      }
-      tc_fence_before();
-      __syncwarp();
-      if (lane == 0) mbar_arrive(dempty(buf));
-      named_bar_sync(1 + Q, 32 * EPI_PARTS);       // the whole proposal of these 32 particles is in smem
-      // pass 2: per-site differences of Eq. 1 and U0 over this part's lattice rows
-      float dS = 0.f, dU = 0.f;
-      tc_stencil<LT>(cur, oth, g, L, hm, lam, kap, dS, dU);
-      part[g * TILE + pr] = make_float2(dS, dU);
-      if (g == EPI_PARTS - 1) {
-        lus[pr] = log_uniform(p.seed, p.tag_acc, p.t0 + (uint32_t)t, (uint32_t)i);
-        if (IRMH) {                                  // |z|^2 of this step; the slot is free again
-          uint32_t* zq = &zsq[(t & (ZSQ_BUFS - 1)) * TILE + pr];
-          zzs[pr] = (float)*zq * (1.0f / ZSQ_SCALE);
-          *zq = 0u;
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(dempty(buf));
+        named_bar_sync(NB_ALL, 32 * EPI_WARPS);        // the proposal of the 32 particles is in smem
+        // pass 2: lattice rows e16, e16 + 16, ... of every particle
+        float dS = 0.f, dU = 0.f;
+        {
+          float dB = 0.f;
+          for (int r = e16; r < L; r += EPI_WARPS) {
+            const int rn = (r + 1 == L) ? 0 : r + 1;
+            const float* c0 = cur + r * L * TILE; const float* c1 = cur + rn * L * TILE;
+            const float* o0 = oth + r * L * TILE; const float* o1 = oth + rn * L * TILE;
+            if constexpr (LT > 0) {
+              float a[LT], a2[LT], d[LT], d2[LT];
+#pragma unroll
+              for (int c = 0; c < LT; ++c) {
+                a[c] = c0[c * TILE]; a2[c] = o0[c * TILE];
+                d[c] = c1[c * TILE]; d2[c] = o1[c * TILE];
+              }
+#pragma unroll
+              for (int c = 0; c < LT; ++c) {
+                const int cn = (c + 1 == LT) ? 0 : c + 1;
+                tc_site_diff(a[c], a[cn], d[c], a2[c], a2[cn], d2[c], hm, lam, dS, dB, dU);
+              }
+            } else {
+              float a = c0[0], a2 = o0[0];
+              for (int c = 0; c < L; ++c) {
+                const int cn = (c + 1 == L) ? 0 : c + 1;
+                const float b = c0[cn * TILE], b2 = o0[cn * TILE];
+                tc_site_diff(a, b, c1[c * TILE], a2, b2, o1[c * TILE], hm, lam, dS, dB, dU);
+                a = b;
+                a2 = b2;
+              }
+            }
+          }
+          dS = fmaf(kap, dB, dS);
         }
+        // sixteen partials per particle: part[e16 * 32 + lane] (the 4 x 128 slots of the wide layout)
+        part[e16 * 32 + pr] = make_float2(dS, dU);
+        if (e16 == EPI_WARPS - 1) lus[pr] = log_uniform(p.seed, p.tag_acc, p.t0 + (uint32_t)t, (uint32_t)i);
+        named_bar_sync(NB_ALL, 32 * EPI_WARPS);
+        dS = 0.f; dU = 0.f;
+#pragma unroll
+        for (int m = 0; m < EPI_WARPS; ++m) {
+          const float2 v = part[m * 32 + pr];
+          dS += v.x;
+          dU += v.y;
+        }
+        const float lu = lus[pr];
+        float margin;
+        bool acc;
+        if (p.mode == MODE_SMC) {
+          margin = -(dU + beta * dS) - lu;
+          acc = margin > 0.f;
+        } else {
+          margin = -dU - lu;
+          acc = (margin > 0.f) && (Si + dS < S_star);
+        }
+        acc = acc && live;
+        if (acc) {
+          float* tmp = cur; cur = oth; oth = tmp;
+          Si += dS;
+          Ui += dU;
+          ++nacc;
+        }
+        if (live && e16 == 0) {
+          if (p.acc_out) p.acc_out[(size_t)t * p.N + i] = (uint8_t)acc;
+          if (p.margin_out) p.margin_out[(size_t)t * p.N + i] = margin;
+        }
+        if (t + 2 < p.k) fill(t + 2);
       }
+      if (live) {
+        for (int x = e16; x < V; x += EPI_WARPS) p.phi[(size_t)x * p.ld + i] = cur[x * TILE];
+        if (e16 == 0) { p.S[i] = Si; p.U0[i] = Ui; }
+      }
+      if (e16 == 0) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) nacc += __shfl_xor_sync(0xffffffffu, nacc, o);
+        if (lane == 0 && nacc) atomicAdd(&p.ctrl->n_accept, nacc);
+        if (lane == 0) __threadfence();
+      }
+    } else {
+      const int Q = warp & 3, g = warp >> 2;       // lane quarter, site part
+      const int pr = Q * 32 + lane;                // particle row = TMEM lane
+      const int i = i0 + pr;
+      const bool live = i < p.N;
+      const int L = LT > 0 ? LT : p.L;
+      const float hm = 2.0f * p.kappa + 0.5f * p.m0sq, lam = p.lam, kap = p.kappa;   // coefficient of phi^2 in the Laplacian form
+      float* cur = tile0 + pr;
+      float* oth = tile1 + pr;
+      for (int x = g; x < V; x += EPI_PARTS) cur[x * TILE] = live ? p.phi[(size_t)x * p.ld + i] : 0.f;
+      float Si = live ? p.S[i] : 0.f, Ui = live ? p.U0[i] : 0.f;
+      float Wi = (IRMH && live) ? p.W2[i] : 0.f;          // |Lc^-1 (phi - mu)|^2 of the current state
+      float* zzs = reinterpret_cast<float*>(smem + lay.zzs);
+      const float beta = (float)p.ctrl->beta, S_star = (float)p.ctrl->S_star;
+      unsigned nacc = 0;
+      const uint32_t tlane = taddr + ((uint32_t)(Q * 32) << 16);
       named_bar_sync(1 + Q, 32 * EPI_PARTS);
-      // every part sums the four partials in the same order and takes the same decision (M4)
-      dS = 0.f; dU = 0.f;
-#pragma unroll
-      for (int m = 0; m < EPI_PARTS; ++m) {
-        float2 v = part[m * TILE + pr];
-        dS += v.x;
-        dU += v.y;
+      float* lus = reinterpret_cast<float*>(part + EPI_PARTS * TILE);
+      uint8_t* zr = smem + lay.zring;
+      const int nq = (V + 3) >> 2;
+      // this thread's share of the normals of step t: quad 4 it + g of its own particle row
+      auto fill = [&](int t) {
+        // two stages per pass: both Philox chains first, then the maps and the stores
+        for (int e0 = 0; e0 < nitE; e0 += 2) {
+          U4 w[2];
+  #pragma unroll
+          for (int e = 0; e < 2; ++e)
+            if (e0 + e < nitE) w[e] = philox4x32_10_rk((uint32_t)(4 * (e0 + e) + g), (uint32_t)i, p.t0 + (uint32_t)t, p.tag_prop, p.rk);
+  #pragma unroll
+          for (int e = 0; e < 2; ++e) {
+            if (e0 + e >= nitE) break;
+            const int it = e0 + e, q = 4 * it + g;
+            float z[4] = {0.f, 0.f, 0.f, 0.f};
+            if (live && q < nq) {
+              box_muller_fast(w[e].x, w[e].y, z[0], z[1]);
+              box_muller_fast(w[e].z, w[e].w, z[2], z[3]);
+            }
+            if (IRMH) {                                    // R1: a ragged last quad is truncated at V
+              float zz = 0.f;
+  #pragma unroll
+              for (int m = 0; m < 4; ++m) if (4 * q + m < V) zz = fmaf(z[m], z[m], zz);
+              atomicAdd(&zsq[(t & (ZSQ_BUFS - 1)) * TILE + pr], __float2uint_rn(zz * ZSQ_SCALE));
+            }
+            float4 hv, lv;
+            hv.x = tf32_rna(z[0]); lv.x = z[0] - hv.x;  hv.y = tf32_rna(z[1]); lv.y = z[1] - hv.y;
+            hv.z = tf32_rna(z[2]); lv.z = z[2] - hv.z;  hv.w = tf32_rna(z[3]); lv.w = z[3] - hv.w;
+            const int n = t * nit + it, s = n % STAGES;
+            const uint32_t ph = (uint32_t)(n / STAGES) & 1u;
+            mbar_wait_relaxed(zempty(s), ph ^ 1);
+            uint8_t* st = zr + (size_t)s * SLAB_BYTES + (size_t)g * CHUNK_BYTES + (size_t)pr * 16;
+            *reinterpret_cast<float4*>(st) = hv;
+            *reinterpret_cast<float4*>(st + 4 * CHUNK_BYTES) = lv;
+            fence_proxy_async();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(zfull(s));
+          }
+        }
+      };
+      // the epilogue warps produce the FIRST slabs of a step and run two steps ahead: the MMAs of
+      // step t + 1 then never wait for a warp that is itself waiting for the MMAs of step t
+      fill(0);
+      if (p.k > 1) fill(1);
+      for (int t = 0; t < p.k; ++t) {
+        const int buf = t & 1;
+        mbar_wait_relaxed(dfull(buf), (t >> 1) & 1);
+        tc_fence_after();
+        // pass 1: phi' = phi + d on this part's 16-column blocks (d carries the step scale s); two
+        // TMEM loads in flight per wait
+        for (int cb = 16 * g; cb < Vn; cb += 32 * EPI_PARTS) {
+          uint32_t r0[16], r1[16];
+          const int cb1 = cb + 16 * EPI_PARTS;
+          const bool two = cb1 < Vn;
+          tmem_ld16(tlane + (uint32_t)(buf * Vn + cb), r0);
+          if (two) tmem_ld16(tlane + (uint32_t)(buf * Vn + cb1), r1);
+          tmem_ld_wait();
+          const float* ci = cur + cb * TILE; float* oi = oth + cb * TILE;
+          if (cb + 16 <= V) {
+  #pragma unroll
+            for (int jj = 0; jj < 16; ++jj) oi[jj * TILE] = (IRMH ? __ldg(p.mu + cb + jj) : ci[jj * TILE]) + __uint_as_float(r0[jj]);
+          } else {
+  #pragma unroll
+            for (int jj = 0; jj < 16; ++jj)
+              if (cb + jj < V) oi[jj * TILE] = (IRMH ? __ldg(p.mu + cb + jj) : ci[jj * TILE]) + __uint_as_float(r0[jj]);
+          }
+          if (two) {
+            ci = cur + cb1 * TILE; oi = oth + cb1 * TILE;
+            if (cb1 + 16 <= V) {
+  #pragma unroll
+              for (int jj = 0; jj < 16; ++jj) oi[jj * TILE] = (IRMH ? __ldg(p.mu + cb1 + jj) : ci[jj * TILE]) + __uint_as_float(r1[jj]);
+            } else {
+  #pragma unroll
+              for (int jj = 0; jj < 16; ++jj)
+                if (cb1 + jj < V) oi[jj * TILE] = (IRMH ? __ldg(p.mu + cb1 + jj) : ci[jj * TILE]) + __uint_as_float(r1[jj]);
+            }
+          }
+        }
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(dempty(buf));
+        named_bar_sync(1 + Q, 32 * EPI_PARTS);       // the whole proposal of these 32 particles is in smem
+        // pass 2: per-site differences of Eq. 1 and U0 over this part's lattice rows
+        float dS = 0.f, dU = 0.f;
+        tc_stencil<LT>(cur, oth, g, L, hm, lam, kap, dS, dU);
+        part[g * TILE + pr] = make_float2(dS, dU);
+        if (g == EPI_PARTS - 1) {
+          lus[pr] = log_uniform(p.seed, p.tag_acc, p.t0 + (uint32_t)t, (uint32_t)i);
+          if (IRMH) {                                  // |z|^2 of this step; the slot is free again
+            uint32_t* zq = &zsq[(t & (ZSQ_BUFS - 1)) * TILE + pr];
+            zzs[pr] = (float)*zq * (1.0f / ZSQ_SCALE);
+            *zq = 0u;
+          }
+        }
+        named_bar_sync(1 + Q, 32 * EPI_PARTS);
+        // every part sums the four partials in the same order and takes the same decision (M4)
+        dS = 0.f; dU = 0.f;
+  #pragma unroll
+        for (int m = 0; m < EPI_PARTS; ++m) {
+          float2 v = part[m * TILE + pr];
+          dS += v.x;
+          dU += v.y;
+        }
+        const float lu = lus[pr];
+        float margin;
+        bool acc;
+        float tZ = 0.f;
+        if (IRMH) {
+          tZ = zzs[pr];
+          margin = -(dU + beta * dS) + 0.5f * (tZ - Wi) - lu;
+          acc = margin > 0.f;
+        } else if (p.mode == MODE_SMC) {
+          margin = -(dU + beta * dS) - lu;
+          acc = margin > 0.f;
+        } else {
+          margin = -dU - lu;
+          acc = (margin > 0.f) && (Si + dS < S_star);
+        }
+        acc = acc && live;
+        if (acc) {
+          float* tmp = cur; cur = oth; oth = tmp;
+          Si += dS;
+          Ui += dU;
+          if (IRMH) Wi = tZ;
+          ++nacc;
+        }
+        if (live && g == 0) {
+          if (p.acc_out) p.acc_out[(size_t)t * p.N + i] = (uint8_t)acc;
+          if (p.margin_out) p.margin_out[(size_t)t * p.N + i] = margin;
+        }
+        if (t + 2 < p.k) fill(t + 2);
       }
-      const float lu = lus[pr];
-      float margin;
-      bool acc;
-      float tZ = 0.f;
-      if (IRMH) {
-        tZ = zzs[pr];
-        margin = -(dU + beta * dS) + 0.5f * (tZ - Wi) - lu;
-        acc = margin > 0.f;
-      } else if (p.mode == MODE_SMC) {
-        margin = -(dU + beta * dS) - lu;
-        acc = margin > 0.f;
-      } else {
-        margin = -dU - lu;
-        acc = (margin > 0.f) && (Si + dS < S_star);
+      if (live) {
+        for (int x = g; x < V; x += EPI_PARTS) p.phi[(size_t)x * p.ld + i] = cur[x * TILE];
+        if (g == 0) { p.S[i] = Si; p.U0[i] = Ui; if (IRMH) p.W2[i] = Wi; }
       }
-      acc = acc && live;
-      if (acc) {
-        float* tmp = cur; cur = oth; oth = tmp;
-        Si += dS;
-        Ui += dU;
-        if (IRMH) Wi = tZ;
-        ++nacc;
+      if (g == 0) {
+  #pragma unroll
+        for (int o = 16; o > 0; o >>= 1) nacc += __shfl_xor_sync(0xffffffffu, nacc, o);
+        if (lane == 0 && nacc) atomicAdd(&p.ctrl->n_accept, nacc);
+        if (lane == 0) __threadfence();
       }
-      if (live && g == 0) {
-        if (p.acc_out) p.acc_out[(size_t)t * p.N + i] = (uint8_t)acc;
-        if (p.margin_out) p.margin_out[(size_t)t * p.N + i] = margin;
-      }
-      if (t + 2 < p.k) fill(t + 2);
-    }
-    if (live) {
-      for (int x = g; x < V; x += EPI_PARTS) p.phi[(size_t)x * p.ld + i] = cur[x * TILE];
-      if (g == 0) { p.S[i] = Si; p.U0[i] = Ui; if (IRMH) p.W2[i] = Wi; }
-    }
-    if (g == 0) {
-#pragma unroll
-      for (int o = 16; o > 0; o >>= 1) nacc += __shfl_xor_sync(0xffffffffu, nacc, o);
-      if (lane == 0 && nacc) atomicAdd(&p.ctrl->n_accept, nacc);
-      if (lane == 0) __threadfence();
+  
     }
   }
   tc_fence_before();
@@ -582,24 +786,33 @@ void launch_mutate_tc(const MutateArgs& a, float* Lsplit, cudaStream_t st, const
   p.finish_rec = a.finish_rec; p.finish_max_rec = a.finish_max_rec; p.finish_poll = a.finish_poll;
   p.rk = philox_round_keys(a.seed);
   const size_t smem = tc::smem_layout(V, irmh).total;
+  // at most one wave of 32-particle CTAs: the narrow variant (nested-sampling walkers, C0)
+  const bool narrow = !irmh && a.ld / 32 <= 148;
   static bool attr_done = false;
   if (!attr_done) {
-    cudaFuncSetAttribute(mutate_tc_kernel<0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::MAX_SMEM);
-    cudaFuncSetAttribute(mutate_tc_kernel<4, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::MAX_SMEM);
-    cudaFuncSetAttribute(mutate_tc_kernel<10, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::MAX_SMEM);
-    cudaFuncSetAttribute(mutate_tc_kernel<0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::MAX_SMEM);
-    cudaFuncSetAttribute(mutate_tc_kernel<10, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::MAX_SMEM);
+    cudaFuncSetAttribute(mutate_tc_kernel<0, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::MAX_SMEM);
+    cudaFuncSetAttribute(mutate_tc_kernel<4, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::MAX_SMEM);
+    cudaFuncSetAttribute(mutate_tc_kernel<10, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::MAX_SMEM);
+    cudaFuncSetAttribute(mutate_tc_kernel<0, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::MAX_SMEM);
+    cudaFuncSetAttribute(mutate_tc_kernel<10, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::MAX_SMEM);
+    cudaFuncSetAttribute(mutate_tc_kernel<0, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::MAX_SMEM);
+    cudaFuncSetAttribute(mutate_tc_kernel<4, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::MAX_SMEM);
+    cudaFuncSetAttribute(mutate_tc_kernel<10, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::MAX_SMEM);
     attr_done = true;
   }
-  const dim3 grid(a.ld / tc::TILE);
+  const dim3 grid(narrow ? a.ld / 32 : a.ld / tc::TILE);
   ++g_launches;
   // lattice sizes of the BASELINE configs get a fully unrolled stencil; any other L the loop
   if (irmh) {
-    if (p.L == 10) launch_pdl(mutate_tc_kernel<10, true>, grid, tc::THREADS, smem, st, p);
-    else launch_pdl(mutate_tc_kernel<0, true>, grid, tc::THREADS, smem, st, p);
-  } else if (p.L == 10) launch_pdl(mutate_tc_kernel<10, false>, grid, tc::THREADS, smem, st, p);
-  else if (p.L == 4) launch_pdl(mutate_tc_kernel<4, false>, grid, tc::THREADS, smem, st, p);
-  else launch_pdl(mutate_tc_kernel<0, false>, grid, tc::THREADS, smem, st, p);
+    if (p.L == 10) launch_pdl(mutate_tc_kernel<10, true, false>, grid, tc::THREADS, smem, st, p);
+    else launch_pdl(mutate_tc_kernel<0, true, false>, grid, tc::THREADS, smem, st, p);
+  } else if (narrow) {
+    if (p.L == 10) launch_pdl(mutate_tc_kernel<10, false, true>, grid, tc::THREADS, smem, st, p);
+    else if (p.L == 4) launch_pdl(mutate_tc_kernel<4, false, true>, grid, tc::THREADS, smem, st, p);
+    else launch_pdl(mutate_tc_kernel<0, false, true>, grid, tc::THREADS, smem, st, p);
+  } else if (p.L == 10) launch_pdl(mutate_tc_kernel<10, false, false>, grid, tc::THREADS, smem, st, p);
+  else if (p.L == 4) launch_pdl(mutate_tc_kernel<4, false, false>, grid, tc::THREADS, smem, st, p);
+  else launch_pdl(mutate_tc_kernel<0, false, false>, grid, tc::THREADS, smem, st, p);
 }
 
 }  // namespace phi4
