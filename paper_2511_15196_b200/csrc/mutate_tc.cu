@@ -198,15 +198,16 @@ __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
 // IRMH (NEXT row f2, reading A15): the proposal is mu + Lc z (the factor is packed with s = 1), the
 // margin gains log q(phi) - log q(phi') = 1/2 |z|^2 - 1/2 |w|^2, and an accepted particle's |w|^2
 // becomes |z|^2.  |z|^2 is summed where the normals are drawn.
-// NARROW (populations of at most 148 x 32 particles: nested-sampling walkers, C0): a CTA owns 32
-// particles instead of 128.  They sit in TMEM lanes 0-31 (rows 32-127 of the A operand stay zero),
-// so only the four warps of lane quarter 0 can read the accumulator, but the proposal then lies
-// in shared memory and ALL sixteen epilogue warps share the stencil rows, the ring fills and the
-// tile copies of those 32 particles (lane = particle in every warp), and the eight producer
-// warps draw one quad per thread instead of four: a step is a latency chain, and the chain gets
-// shorter; four times as many SMs take part.
-template <int LT, bool IRMH, bool NARROW>
+// NG > 0 (small populations: nested-sampling walkers, C0, the paper's N = 5000): a CTA owns NG
+// groups of 32 particles (NG = 1 or 2) instead of 128.  They sit in TMEM lanes 0 .. 32 NG - 1 (the
+// other rows of the A operand stay zero), so only the four warps of a group's lane quarter can
+// read its accumulator rows, but the proposal then lies in shared memory and the group's 16 / NG
+// epilogue warps share the stencil rows, the ring fills and the tile copies of its 32 particles
+// (lane = particle in every warp), and the producer threads draw 1 or 2 quads per pass instead of
+// four: a step is a latency chain, and the chain gets shorter; more SMs take part.
+template <int LT, bool IRMH, int NG>
 __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParams p) {
+  constexpr bool NARROW = NG > 0;
   // programmatic dependent launch: barrier setup and the TMEM allocation touch nothing the
   // predecessor writes, so they run before the wait
   pdl_trigger();
@@ -232,7 +233,7 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
   // the first nitE ring fills of every step are produced by the epilogue warps (one quad per
   // thread, two steps ahead), the other nitP by the dedicated producers (two quads per thread)
   const int nitE = min(EPI_FILLS, nit - 1), nitP = nit - nitE;
-  const int i0 = blockIdx.x * (NARROW ? 32 : TILE);
+  const int i0 = blockIdx.x * (NARROW ? 32 * NG : TILE);
   uint32_t ncols = 32;
   while ((int)ncols < 2 * Vn) ncols <<= 1;
 
@@ -245,7 +246,7 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
   if (warp == 0) tmem_alloc(smem_u32(tmem_slot), ncols);
   if (IRMH)
     for (int e = threadIdx.x; e < ZSQ_BUFS * TILE; e += THREADS) zsq[e] = 0u;
-  if (NARROW) {            // rows 32..127 of every ring stage are never written again: zero once
+  if (NARROW) {            // rows 32 NG..127 of every ring stage are never written again: zero once
     float4* z4 = reinterpret_cast<float4*>(smem + lay.zring);
     for (int e = threadIdx.x; e < STAGES * SLAB_BYTES / 16; e += THREADS) z4[e] = make_float4(0.f, 0.f, 0.f, 0.f);
     fence_proxy_async();
@@ -321,10 +322,12 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
   } else if (warp >= PROD_WARP0) {
     // ================================ normal producers =======================================
     if constexpr (NARROW) {
-      // thread (particle row, sub): one quad per pass -- warps 0-3 fill stage `it`, warps 4-7 stage
-      // `it + 1`, sub & 3 = the stage's 16-byte K-chunk
+      // thread (particle row, sub): 8 / TPR quads per pass (a pass = two ring stages of four
+      // 16-byte K-chunks), TPR = threads per row; all quads of a thread lie in ONE stage, so a
+      // stage is written by four warps
+      constexpr int TP = 32 * (NG > 0 ? NG : 1), TPR = 256 / TP, QPT = 8 / TPR;
       const int j = threadIdx.x - PROD_WARP0 * 32;       // 0..255
-      const int pr = j & 31, sub = j >> 5, so = sub >> 2, c = sub & 3;
+      const int pr = j % TP, sub = j / TP, so = (sub * QPT) >> 2;
       const int i = i0 + pr;
       const int nq = (V + 3) >> 2;
       uint8_t* zr = smem + lay.zring;
@@ -332,22 +335,29 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
         const uint32_t tt = p.t0 + (uint32_t)t;
         for (int it = 0; it < nitP; it += 2) {
           if (it + so >= nitP) continue;                  // (warp-uniform: so is)
-          const int q = 4 * (nitE + it + so) + c;
-          float z[4] = {0.f, 0.f, 0.f, 0.f};
-          if (i < p.N && q < nq) {
-            const U4 w = philox4x32_10_rk((uint32_t)q, (uint32_t)i, tt, p.tag_prop, p.rk);
-            box_muller_fast(w.x, w.y, z[0], z[1]);
-            box_muller_fast(w.z, w.w, z[2], z[3]);
+          float4 hv[QPT], lv[QPT];
+#pragma unroll
+          for (int u = 0; u < QPT; ++u) {
+            const int c = (sub * QPT + u) & 3, q = 4 * (nitE + it + so) + c;
+            float z[4] = {0.f, 0.f, 0.f, 0.f};
+            if (i < p.N && q < nq) {
+              const U4 w = philox4x32_10_rk((uint32_t)q, (uint32_t)i, tt, p.tag_prop, p.rk);
+              box_muller_fast(w.x, w.y, z[0], z[1]);
+              box_muller_fast(w.z, w.w, z[2], z[3]);
+            }
+            hv[u].x = tf32_rna(z[0]); lv[u].x = z[0] - hv[u].x;  hv[u].y = tf32_rna(z[1]); lv[u].y = z[1] - hv[u].y;
+            hv[u].z = tf32_rna(z[2]); lv[u].z = z[2] - hv[u].z;  hv[u].w = tf32_rna(z[3]); lv[u].w = z[3] - hv[u].w;
           }
-          float4 hv, lv;
-          hv.x = tf32_rna(z[0]); lv.x = z[0] - hv.x;  hv.y = tf32_rna(z[1]); lv.y = z[1] - hv.y;
-          hv.z = tf32_rna(z[2]); lv.z = z[2] - hv.z;  hv.w = tf32_rna(z[3]); lv.w = z[3] - hv.w;
           const int n = t * nit + nitE + it + so, sl = n % STAGES;
           const uint32_t ph = (uint32_t)(n / STAGES) & 1u;
           mbar_wait_relaxed(zempty(sl), ph ^ 1);
-          uint8_t* st = zr + (size_t)sl * SLAB_BYTES + (size_t)c * CHUNK_BYTES + (size_t)pr * 16;
-          *reinterpret_cast<float4*>(st) = hv;
-          *reinterpret_cast<float4*>(st + 4 * CHUNK_BYTES) = lv;
+#pragma unroll
+          for (int u = 0; u < QPT; ++u) {
+            const int c = (sub * QPT + u) & 3;
+            uint8_t* st = zr + (size_t)sl * SLAB_BYTES + (size_t)c * CHUNK_BYTES + (size_t)pr * 16;
+            *reinterpret_cast<float4*>(st) = hv[u];
+            *reinterpret_cast<float4*>(st + 4 * CHUNK_BYTES) = lv[u];
+          }
           fence_proxy_async();
           __syncwarp();
           if (lane == 0) mbar_arrive_n(zfull(sl), 4);       // 4 warps x 4 = the 16 expected
@@ -426,33 +436,35 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
   } else {
     // ================================ epilogue ==============================================
     if constexpr (NARROW) {
-      // ---- 32 particles: lane = particle in every warp; warp e = 4 g + Q of 16 shares the work
-      const int Q = warp & 3, g = warp >> 2, e16 = 4 * g + Q;
-      const int pr = lane, i = i0 + pr;
+      // ---- group gq of 32 particles: lane = particle in each of its WPG warps; warp e16 of the group
+      constexpr int NGc = NG > 0 ? NG : 1, WPG = EPI_WARPS / NGc;
+      const int Q = warp & 3, g = warp >> 2, gq = Q % NGc, e16 = g * (4 / NGc) + Q / NGc;
+      const int pr = 32 * gq + lane, i = i0 + pr;
       const bool live = i < p.N;
       const int L = LT > 0 ? LT : p.L;
       const float hm = 2.0f * p.kappa + 0.5f * p.m0sq, lam = p.lam, kap = p.kappa;
       float* cur = tile0 + pr;
       float* oth = tile1 + pr;
-      for (int x = e16; x < V; x += EPI_WARPS) cur[x * TILE] = live ? p.phi[(size_t)x * p.ld + i] : 0.f;
+      for (int x = e16; x < V; x += WPG) cur[x * TILE] = live ? p.phi[(size_t)x * p.ld + i] : 0.f;
       float Si = live ? p.S[i] : 0.f, Ui = live ? p.U0[i] : 0.f;
       const float beta = (float)p.ctrl->beta, S_star = (float)p.ctrl->S_star;
       unsigned nacc = 0;
-      const uint32_t tlane = taddr;                         // TMEM lanes 0..31
-      constexpr int NB_ALL = 6;                             // named barrier of the 16 epilogue warps
-      named_bar_sync(NB_ALL, 32 * EPI_WARPS);
+      const uint32_t tlane = taddr + ((uint32_t)(32 * gq) << 16);   // TMEM lanes of the group
+      const int NB_ALL = 6 + gq;                            // named barrier of the group's warps
+      named_bar_sync(NB_ALL, 32 * WPG);
       float* lus = reinterpret_cast<float*>(part + EPI_PARTS * TILE);
       uint8_t* zr = smem + lay.zring;
       const int nq = (V + 3) >> 2;
-      // ring fills of step t by the epilogue warps: stage `it` (< nitE <= 2) chunk g by the warps with
-      // Q == it; every warp arrives once per stage (the barrier expects all sixteen)
+      // ring fills of step t by the epilogue warps: stage `it` (< nitE <= 2), chunk e16 & 3 by the
+      // group's warps with e16 < 8 and e16 >> 2 == it; every warp arrives once per stage (the barrier
+      // expects all sixteen)
       auto fill = [&](int t) {
         for (int it = 0; it < nitE; ++it) {
           const int n = t * nit + it, sl = n % STAGES;
           const uint32_t ph = (uint32_t)(n / STAGES) & 1u;
           mbar_wait_relaxed(zempty(sl), ph ^ 1);       // (every arriver: the slot's last use is over)
-          if (Q == it) {
-            const int q = 4 * it + g;
+          if (e16 < 8 && (e16 >> 2) == it) {
+            const int q = 4 * it + (e16 & 3);
             float z[4] = {0.f, 0.f, 0.f, 0.f};
             if (live && q < nq) {
               const U4 w = philox4x32_10_rk((uint32_t)q, (uint32_t)i, p.t0 + (uint32_t)t, p.tag_prop, p.rk);
@@ -462,7 +474,7 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
             float4 hv, lv;
             hv.x = tf32_rna(z[0]); lv.x = z[0] - hv.x;  hv.y = tf32_rna(z[1]); lv.y = z[1] - hv.y;
             hv.z = tf32_rna(z[2]); lv.z = z[2] - hv.z;  hv.w = tf32_rna(z[3]); lv.w = z[3] - hv.w;
-            uint8_t* st = zr + (size_t)sl * SLAB_BYTES + (size_t)g * CHUNK_BYTES + (size_t)pr * 16;
+            uint8_t* st = zr + (size_t)sl * SLAB_BYTES + (size_t)(e16 & 3) * CHUNK_BYTES + (size_t)pr * 16;
             *reinterpret_cast<float4*>(st) = hv;
             *reinterpret_cast<float4*>(st + 4 * CHUNK_BYTES) = lv;
             fence_proxy_async();
@@ -477,8 +489,8 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
         const int buf = t & 1;
         mbar_wait_relaxed(dfull(buf), (t >> 1) & 1);
         tc_fence_after();
-        // pass 1 (the four warps of lane quarter 0): phi' = phi + d on 16-column blocks
-        if (Q == 0) {
+        // pass 1 (the four warps of the group's lane quarter): phi' = phi + d on 16-column blocks
+        if (Q == gq) {
           for (int cb = 16 * g; cb < Vn; cb += 32 * EPI_PARTS) {
             uint32_t r0[16], r1[16];
             const int cb1 = cb + 16 * EPI_PARTS;
@@ -501,12 +513,12 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(dempty(buf));
-        named_bar_sync(NB_ALL, 32 * EPI_WARPS);        // the proposal of the 32 particles is in smem
-        // pass 2: lattice rows e16, e16 + 16, ... of every particle
+        named_bar_sync(NB_ALL, 32 * WPG);              // the proposal of the 32 particles is in smem
+        // pass 2: lattice rows e16, e16 + WPG, ... of every particle
         float dS = 0.f, dU = 0.f;
         {
           float dB = 0.f;
-          for (int r = e16; r < L; r += EPI_WARPS) {
+          for (int r = e16; r < L; r += WPG) {
             const int rn = (r + 1 == L) ? 0 : r + 1;
             const float* c0 = cur + r * L * TILE; const float* c1 = cur + rn * L * TILE;
             const float* o0 = oth + r * L * TILE; const float* o1 = oth + rn * L * TILE;
@@ -535,14 +547,14 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
           }
           dS = fmaf(kap, dB, dS);
         }
-        // sixteen partials per particle: part[e16 * 32 + lane] (the 4 x 128 slots of the wide layout)
-        part[e16 * 32 + pr] = make_float2(dS, dU);
-        if (e16 == EPI_WARPS - 1) lus[pr] = log_uniform(p.seed, p.tag_acc, p.t0 + (uint32_t)t, (uint32_t)i);
-        named_bar_sync(NB_ALL, 32 * EPI_WARPS);
+        // WPG partials per particle: part[(gq WPG + e16) 32 + lane] (the 4 x 128 slots of the wide layout)
+        part[(gq * WPG + e16) * 32 + lane] = make_float2(dS, dU);
+        if (e16 == WPG - 1) lus[pr] = log_uniform(p.seed, p.tag_acc, p.t0 + (uint32_t)t, (uint32_t)i);
+        named_bar_sync(NB_ALL, 32 * WPG);
         dS = 0.f; dU = 0.f;
 #pragma unroll
-        for (int m = 0; m < EPI_WARPS; ++m) {
-          const float2 v = part[m * 32 + pr];
+        for (int m = 0; m < WPG; ++m) {
+          const float2 v = part[(gq * WPG + m) * 32 + lane];
           dS += v.x;
           dU += v.y;
         }
@@ -570,7 +582,7 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
         if (t + 2 < p.k) fill(t + 2);
       }
       if (live) {
-        for (int x = e16; x < V; x += EPI_WARPS) p.phi[(size_t)x * p.ld + i] = cur[x * TILE];
+        for (int x = e16; x < V; x += WPG) p.phi[(size_t)x * p.ld + i] = cur[x * TILE];
         if (e16 == 0) { p.S[i] = Si; p.U0[i] = Ui; }
       }
       if (e16 == 0) {
@@ -786,33 +798,30 @@ void launch_mutate_tc(const MutateArgs& a, float* Lsplit, cudaStream_t st, const
   p.finish_rec = a.finish_rec; p.finish_max_rec = a.finish_max_rec; p.finish_poll = a.finish_poll;
   p.rk = philox_round_keys(a.seed);
   const size_t smem = tc::smem_layout(V, irmh).total;
-  // at most one wave of 32-particle CTAs: the narrow variant (nested-sampling walkers, C0)
-  const bool narrow = !irmh && a.ld / 32 <= 148;
+  // at most one wave of 32- or 64-particle CTAs: the narrow variants (nested-sampling walkers, C0,
+  // the paper's N = 5000)
+  const int ng = irmh ? 0 : (a.ld / 32 <= 148 ? 1 : (a.ld / 64 <= 148 ? 2 : 0));
   static bool attr_done = false;
   if (!attr_done) {
-    cudaFuncSetAttribute(mutate_tc_kernel<0, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::MAX_SMEM);
-    cudaFuncSetAttribute(mutate_tc_kernel<4, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::MAX_SMEM);
-    cudaFuncSetAttribute(mutate_tc_kernel<10, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::MAX_SMEM);
-    cudaFuncSetAttribute(mutate_tc_kernel<0, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::MAX_SMEM);
-    cudaFuncSetAttribute(mutate_tc_kernel<10, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::MAX_SMEM);
-    cudaFuncSetAttribute(mutate_tc_kernel<0, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::MAX_SMEM);
-    cudaFuncSetAttribute(mutate_tc_kernel<4, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::MAX_SMEM);
-    cudaFuncSetAttribute(mutate_tc_kernel<10, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::MAX_SMEM);
+    auto big = [](auto kern) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::MAX_SMEM); };
+    big(mutate_tc_kernel<0, false, 0>); big(mutate_tc_kernel<4, false, 0>); big(mutate_tc_kernel<10, false, 0>);
+    big(mutate_tc_kernel<0, true, 0>); big(mutate_tc_kernel<10, true, 0>);
+    big(mutate_tc_kernel<0, false, 1>); big(mutate_tc_kernel<4, false, 1>); big(mutate_tc_kernel<10, false, 1>);
+    big(mutate_tc_kernel<0, false, 2>); big(mutate_tc_kernel<4, false, 2>); big(mutate_tc_kernel<10, false, 2>);
     attr_done = true;
   }
-  const dim3 grid(narrow ? a.ld / 32 : a.ld / tc::TILE);
+  const dim3 grid(ng ? a.ld / (32 * ng) : a.ld / tc::TILE);
   ++g_launches;
   // lattice sizes of the BASELINE configs get a fully unrolled stencil; any other L the loop
-  if (irmh) {
-    if (p.L == 10) launch_pdl(mutate_tc_kernel<10, true, false>, grid, tc::THREADS, smem, st, p);
-    else launch_pdl(mutate_tc_kernel<0, true, false>, grid, tc::THREADS, smem, st, p);
-  } else if (narrow) {
-    if (p.L == 10) launch_pdl(mutate_tc_kernel<10, false, true>, grid, tc::THREADS, smem, st, p);
-    else if (p.L == 4) launch_pdl(mutate_tc_kernel<4, false, true>, grid, tc::THREADS, smem, st, p);
-    else launch_pdl(mutate_tc_kernel<0, false, true>, grid, tc::THREADS, smem, st, p);
-  } else if (p.L == 10) launch_pdl(mutate_tc_kernel<10, false, false>, grid, tc::THREADS, smem, st, p);
-  else if (p.L == 4) launch_pdl(mutate_tc_kernel<4, false, false>, grid, tc::THREADS, smem, st, p);
-  else launch_pdl(mutate_tc_kernel<0, false, false>, grid, tc::THREADS, smem, st, p);
+  auto go = [&](auto k0, auto k4, auto k10) {
+    if (p.L == 10) launch_pdl(k10, grid, tc::THREADS, smem, st, p);
+    else if (p.L == 4) launch_pdl(k4, grid, tc::THREADS, smem, st, p);
+    else launch_pdl(k0, grid, tc::THREADS, smem, st, p);
+  };
+  if (irmh) go(mutate_tc_kernel<0, true, 0>, mutate_tc_kernel<0, true, 0>, mutate_tc_kernel<10, true, 0>);
+  else if (ng == 1) go(mutate_tc_kernel<0, false, 1>, mutate_tc_kernel<4, false, 1>, mutate_tc_kernel<10, false, 1>);
+  else if (ng == 2) go(mutate_tc_kernel<0, false, 2>, mutate_tc_kernel<4, false, 2>, mutate_tc_kernel<10, false, 2>);
+  else go(mutate_tc_kernel<0, false, 0>, mutate_tc_kernel<4, false, 0>, mutate_tc_kernel<10, false, 0>);
 }
 
 }  // namespace phi4
