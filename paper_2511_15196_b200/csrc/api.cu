@@ -1,5 +1,6 @@
 // api.cu -- the C ABI of include/phi4smc.h: handle, workspace carve-up, step sequencing.
 // No torch types, no device allocation: all device state lives in the caller's workspace.
+#include <chrono>
 #include <math.h>
 #include <stdio.h>
 #include <stdlib.h>
@@ -503,6 +504,7 @@ PHI4_API int smc_step(phi4smc* h, smc_step_info* info) {
 // (HostPoll, written by the kernel that closes the step): no copy or event sits in the stream
 // between two steps, so their kernels stay chained.  One step is kept queued behind the one whose
 // report the host is waiting for.  `start` = steps completed before this call.
+constexpr int RUN_STALL_SECONDS = 120;
 template <typename F>
 static int run_polled(phi4smc* h, int max_steps, int start, F enqueue) {
   volatile HostPoll* hp = h->h_hp;
@@ -515,12 +517,22 @@ static int run_polled(phi4smc* h, int max_steps, int start, F enqueue) {
     ++enq;
     if (enq >= 2) {
       const int target = start + enq - 1;        // the step before the one just enqueued
+      int seen = hp->seq;
+      auto moved = std::chrono::steady_clock::now();
       for (unsigned spin = 1; hp->seq < target && !hp->done; ++spin) {
         if ((spin & 1023u) == 0) {               // a dead stream must not hang the host
           cudaError_t q = cudaStreamQuery(h->st);
           if (q == cudaSuccess) break;
           if (q != cudaErrorNotReady) {
             snprintf(h->err, sizeof(h->err), "run: %s", cudaGetErrorString(q));
+            return PHI4_ECUDA;
+          }
+          // ... nor a stream that stopped making progress (no step takes anywhere near this long)
+          const auto now = std::chrono::steady_clock::now();
+          if (hp->seq != seen) { seen = hp->seq; moved = now; }
+          else if (now - moved > std::chrono::seconds(RUN_STALL_SECONDS)) {
+            snprintf(h->err, sizeof(h->err), "run: no step finished for %d s (device stalled at step %d)",
+                     RUN_STALL_SECONDS, seen);
             return PHI4_ECUDA;
           }
         }

@@ -324,7 +324,10 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
     if constexpr (NARROW) {
       // thread (particle row, sub): 8 / TPR quads per pass (a pass = two ring stages of four
       // 16-byte K-chunks), TPR = threads per row; all quads of a thread lie in ONE stage, so a
-      // stage is written by four warps
+      // stage is written by four warps.  EVERY producer warp waits for and arrives at EVERY
+      // producer stage, writer or not: a parity wait only tells "one phase behind" from "level",
+      // and a warp that skipped the stages of the other four could meet a slot two phases on
+      // (its wait then passes at once, and it overwrites a stage the MMA has not read).
       constexpr int TP = 32 * (NG > 0 ? NG : 1), TPR = 256 / TP, QPT = 8 / TPR;
       const int j = threadIdx.x - PROD_WARP0 * 32;       // 0..255
       const int pr = j % TP, sub = j / TP, so = (sub * QPT) >> 2;
@@ -334,33 +337,41 @@ __global__ void __launch_bounds__(tc::THREADS, 1) mutate_tc_kernel(const TcParam
       for (int t = 0; t < p.k; ++t) {
         const uint32_t tt = p.t0 + (uint32_t)t;
         for (int it = 0; it < nitP; it += 2) {
-          if (it + so >= nitP) continue;                  // (warp-uniform: so is)
+          const bool mine = it + so < nitP;               // (warp-uniform: so is)
           float4 hv[QPT], lv[QPT];
+          if (mine) {
 #pragma unroll
-          for (int u = 0; u < QPT; ++u) {
-            const int c = (sub * QPT + u) & 3, q = 4 * (nitE + it + so) + c;
-            float z[4] = {0.f, 0.f, 0.f, 0.f};
-            if (i < p.N && q < nq) {
-              const U4 w = philox4x32_10_rk((uint32_t)q, (uint32_t)i, tt, p.tag_prop, p.rk);
-              box_muller_fast(w.x, w.y, z[0], z[1]);
-              box_muller_fast(w.z, w.w, z[2], z[3]);
+            for (int u = 0; u < QPT; ++u) {
+              const int c = (sub * QPT + u) & 3, q = 4 * (nitE + it + so) + c;
+              float z[4] = {0.f, 0.f, 0.f, 0.f};
+              if (i < p.N && q < nq) {
+                const U4 w = philox4x32_10_rk((uint32_t)q, (uint32_t)i, tt, p.tag_prop, p.rk);
+                box_muller_fast(w.x, w.y, z[0], z[1]);
+                box_muller_fast(w.z, w.w, z[2], z[3]);
+              }
+              hv[u].x = tf32_rna(z[0]); lv[u].x = z[0] - hv[u].x;  hv[u].y = tf32_rna(z[1]); lv[u].y = z[1] - hv[u].y;
+              hv[u].z = tf32_rna(z[2]); lv[u].z = z[2] - hv[u].z;  hv[u].w = tf32_rna(z[3]); lv[u].w = z[3] - hv[u].w;
             }
-            hv[u].x = tf32_rna(z[0]); lv[u].x = z[0] - hv[u].x;  hv[u].y = tf32_rna(z[1]); lv[u].y = z[1] - hv[u].y;
-            hv[u].z = tf32_rna(z[2]); lv[u].z = z[2] - hv[u].z;  hv[u].w = tf32_rna(z[3]); lv[u].w = z[3] - hv[u].w;
           }
-          const int n = t * nit + nitE + it + so, sl = n % STAGES;
-          const uint32_t ph = (uint32_t)(n / STAGES) & 1u;
-          mbar_wait_relaxed(zempty(sl), ph ^ 1);
 #pragma unroll
-          for (int u = 0; u < QPT; ++u) {
-            const int c = (sub * QPT + u) & 3;
-            uint8_t* st = zr + (size_t)sl * SLAB_BYTES + (size_t)c * CHUNK_BYTES + (size_t)pr * 16;
-            *reinterpret_cast<float4*>(st) = hv[u];
-            *reinterpret_cast<float4*>(st + 4 * CHUNK_BYTES) = lv[u];
+          for (int st2 = 0; st2 < 2; ++st2) {
+            if (it + st2 >= nitP) break;
+            const int n = t * nit + nitE + it + st2, sl = n % STAGES;
+            const uint32_t ph = (uint32_t)(n / STAGES) & 1u;
+            mbar_wait_relaxed(zempty(sl), ph ^ 1);
+            if (st2 == so) {
+#pragma unroll
+              for (int u = 0; u < QPT; ++u) {
+                const int c = (sub * QPT + u) & 3;
+                uint8_t* st = zr + (size_t)sl * SLAB_BYTES + (size_t)c * CHUNK_BYTES + (size_t)pr * 16;
+                *reinterpret_cast<float4*>(st) = hv[u];
+                *reinterpret_cast<float4*>(st + 4 * CHUNK_BYTES) = lv[u];
+              }
+              fence_proxy_async();
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive_n(zfull(sl), 2);     // 8 warps x 2 = the 16 expected
           }
-          fence_proxy_async();
-          __syncwarp();
-          if (lane == 0) mbar_arrive_n(zfull(sl), 4);       // 4 warps x 4 = the 16 expected
         }
       }
     } else {

@@ -90,6 +90,96 @@ __device__ __forceinline__ void bitonic_sort_block(const float* __restrict__ S, 
   __syncthreads();
 }
 
+// The kd smallest keys (= the dead points) of the block's 1024 E keys, sorted, without sorting the
+// rest: radix select of the kd-th smallest key (8 bits per pass from the top; the keys are distinct,
+// so at the latest the eighth pass isolates it; the pass stops as soon as a whole bin is taken),
+// compaction of the selected keys, and a 1024-key bitonic sort of those.  For kd <= 1024.
+template <int E>
+__device__ __forceinline__ void topk_sort_block(const float* __restrict__ S, int n, int kd,
+                                                unsigned long long* keys) {
+  __shared__ int hist[256];
+  __shared__ int sel_digit, sel_before, sel_all;
+  __shared__ int wcnt[32];
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  unsigned long long kr[E];
+#pragma unroll
+  for (int e = 0; e < E; ++e) {
+    const int i = tid * E + e;
+    kr[e] = i < n ? ns_key(S[i], i) : ~0ull;
+  }
+  unsigned long long prefix = 0ull, mask = 0ull;
+  int remaining = kd;                                    // rank of the threshold among the candidates
+  for (int pass = 0; pass < 8; ++pass) {
+    const int shift = 56 - 8 * pass;
+    if (tid < 256) hist[tid] = 0;
+    __syncthreads();
+#pragma unroll
+    for (int e = 0; e < E; ++e)
+      if ((kr[e] & mask) == prefix) atomicAdd(&hist[(int)((kr[e] >> shift) & 255ull)], 1);
+    __syncthreads();
+    if (wid == 0) {
+      // lane l: bins 8 l .. 8 l + 7; find the bin that holds rank `remaining`
+      int c[8], tot = 0;
+#pragma unroll
+      for (int b = 0; b < 8; ++b) { c[b] = hist[8 * lane + b]; tot += c[b]; }
+      int inc = tot;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const int v = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += v;
+      }
+      int before = inc - tot;                            // candidates in the bins of lower lanes
+      if (before < remaining && remaining <= inc) {      // exactly one lane
+        int b = 0;
+        while (before + c[b] < remaining) { before += c[b]; ++b; }
+        sel_digit = 8 * lane + b;
+        sel_before = before;
+        sel_all = (remaining - before == c[b]);          // the whole bin is taken: done
+      }
+    }
+    __syncthreads();
+    prefix |= (unsigned long long)sel_digit << shift;
+    mask |= 255ull << shift;
+    remaining -= sel_before;
+    if (sel_all) break;
+  }
+  // selected: (key & mask) <= prefix -- exactly kd keys; compact them in index order of the threads
+  int cnt = 0;
+#pragma unroll
+  for (int e = 0; e < E; ++e) cnt += ((kr[e] & mask) <= prefix) ? 1 : 0;
+  int inc = cnt;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const int v = __shfl_up_sync(0xffffffffu, inc, o);
+    if (lane >= o) inc += v;
+  }
+  if (lane == 31) wcnt[wid] = inc;
+  __syncthreads();
+  if (wid == 0) {
+    const int v = wcnt[lane];
+    int sc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int u = __shfl_up_sync(0xffffffffu, sc, o);
+      if (lane >= o) sc += u;
+    }
+    wcnt[lane] = sc - v;
+  }
+  __syncthreads();
+  int pos = wcnt[wid] + inc - cnt;
+#pragma unroll
+  for (int e = 0; e < E; ++e)
+    if ((kr[e] & mask) <= prefix) keys[pos++] = kr[e];
+  __syncthreads();
+  // sort the kd selected keys (padded to 1024 with keys that sort last)
+  unsigned long long k1[1];
+  k1[0] = tid < kd ? keys[tid] : ~0ull;
+  __syncthreads();
+  for (int k = 2; k <= 1024; k <<= 1) bitonic_strides<1>(k1, keys, k, k >> 1, 0);
+  keys[tid] = k1[0];
+  __syncthreads();
+}
+
 // ---- more than 16384 live points: the same network across blocks, keys in global memory --------
 constexpr int NS_BLOCK_KEYS = 16384;
 __global__ void __launch_bounds__(1024)
@@ -149,12 +239,23 @@ ns_select_evidence_kernel(NsArgs a) {
   if (!big) {
     int np2 = 1024;                  // padded to the block: thread t holds keys t E .. t E + E - 1
     while (np2 < n) np2 <<= 1;
-    switch (np2 >> 10) {
-      case 1: bitonic_sort_block<1>(a.S, n, skeys); break;
-      case 2: bitonic_sort_block<2>(a.S, n, skeys); break;
-      case 4: bitonic_sort_block<4>(a.S, n, skeys); break;
-      case 8: bitonic_sort_block<8>(a.S, n, skeys); break;
-      default: bitonic_sort_block<16>(a.S, n, skeys); break;
+    if (kd <= 1024 && 4 * kd <= n) {
+      // few dead points: select them, sort only them (the order of the survivors is never used)
+      switch (np2 >> 10) {
+        case 1: topk_sort_block<1>(a.S, n, kd, skeys); break;
+        case 2: topk_sort_block<2>(a.S, n, kd, skeys); break;
+        case 4: topk_sort_block<4>(a.S, n, kd, skeys); break;
+        case 8: topk_sort_block<8>(a.S, n, kd, skeys); break;
+        default: topk_sort_block<16>(a.S, n, kd, skeys); break;
+      }
+    } else {
+      switch (np2 >> 10) {
+        case 1: bitonic_sort_block<1>(a.S, n, skeys); break;
+        case 2: bitonic_sort_block<2>(a.S, n, skeys); break;
+        case 4: bitonic_sort_block<4>(a.S, n, skeys); break;
+        case 8: bitonic_sort_block<8>(a.S, n, skeys); break;
+        default: bitonic_sort_block<16>(a.S, n, skeys); break;
+      }
     }
   }
   const int it = ctrl->temp_index;
