@@ -193,7 +193,8 @@ int smc_step(phi4smc* h, smc_step_info* info);
 
 /* Runs smc_step until beta == 1 or max_temps transitions were made; termination is decided on
  * the device, the host only polls a flag.  Synchronises.  *n_temps (may be NULL) = transitions
- * made by this call.  Returns PHI4_ENOTPD / PHI4_ENAN if a step failed.                          */
+ * made by this call.  Returns PHI4_ENOTPD / PHI4_ENAN if a step failed, PHI4_ECUDA if the
+ * stream reports an error or no step finishes for 120 s (the same holds for ns_run).            */
 int smc_run(phi4smc* h, int max_temps, int* n_temps);
 
 /* Per-temperature records of all transitions made so far (at most cap entries are copied;
