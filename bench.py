@@ -10,10 +10,11 @@ executed) / time, summed over ranks.  The path does not shard ("replicas only", 
 --gpus N every rank runs an independent replica with its own seed, no collective on the data path.
 
 One JSON line on stdout (rank 0).  Besides the headline workload it carries
-  peaks_measured  dense tcgen05 kind::tf32, FP32 FMA and IMAD.WIDE rates measured in this run through
+  peaks_measured  dense tcgen05 kind::tf32 / kind::f16, FP32 FMA and IMAD.WIDE rates measured in this run through
                   phi4_measure_peaks (the roofline denominators MEASURED_PEAKS.json does not hold)
   large_v         the same measurement on C3 and C4 (first --max-temps temperatures per step), where
-                  the rooflines mean something: the tcgen05 proposal GEMM against the TF32 peak and
+                  the rooflines mean something: the tcgen05 proposal GEMM against the measured peak of the
+                  MMA kind it issues (kind::f16 for the scaled 3xFP16 split, kind::tf32 with --path 3) and
                   the population step against the HBM peak, with per-phase device times
 --impl reference times the FP64 CPU oracle on the host cores.
 """
@@ -318,7 +319,7 @@ def workload_config(name, cfg, gpus, temps=None, max_temps=None):
     return c
 
 
-def rooflines(name, cfg, ph, pk, mp, timed_region_s):
+def rooflines(name, cfg, ph, pk, mp, timed_region_s, path=0):
     """Roofline records of the dominant mutation kernel and of the population step.
     ph: per-phase device times in ms; pk: MEASURED_PEAKS.json; mp: phi4_measure_peaks of this run."""
     L, N, k = cfg["L"], cfg["N"], cfg["k"]
@@ -344,23 +345,29 @@ def rooflines(name, cfg, ph, pk, mp, timed_region_s):
                 "site_updates_per_s": float(N) * V * k * upm / (mut_ms * 1e-3), "ms": mut_ms}
     else:
         # tensor bound: the proposal GEMM of ONE step, timed alone.  Algorithmic
-        # work: the triangular product in 3xTF32 split precision (north_star), 3 products x 2 flop x
-        # N V (V+1) / 2; the FP32-equivalent ("useful") flop are a third of that.
+        # work: the triangular product in three-product split precision (north_star), 3 products x
+        # 2 flop x N V (V+1) / 2; the FP32-equivalent ("useful") flop are a third of that.  The
+        # operands are FP16 pairs (scaled 3xFP16, same 11-bit significands as TF32) unless
+        # --path 3 asks for 3xTF32: the peak is the measured dense rate of the kind the kernel issues.
         t = ph["proposal_gemm"] * 1e-3
         issued = 3.0 * float(N) * V * (V + 1)
         achieved = issued / t / 1e12
         sustained = timed_region_s >= 0.25
-        peak = mp["tf32_tflops_sustained"] if sustained else mp["tf32_tflops_burst"]
-        roof = {"bound": "tensor", "kernel": "propose_tc_kernel, one launch = one mutation step",
+        kind = "tf32" if path == 3 else "f16"
+        peak = mp[kind + "_tflops_sustained"] if sustained else mp[kind + "_tflops_burst"]
+        roof = {"bound": "tensor", "kernel": "propose_tc_kernel<%s>, one launch = one mutation step"
+                                             % ("false" if path == 3 else "true"),
                 "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                 "useful_frac": achieved / 3.0 / peak,
-                "ops": "TF32 flop of the triangular L*z in 3xTF32 split precision, 3 N V (V+1) per "
-                       "step; useful_frac counts the FP32-equivalent N V (V+1)",
-                "peak_source": "phi4_measure_peaks dense tcgen05 kind::tf32 of this run, %s (burst %.0f, "
-                               "sustained %.0f; bf16 x 1/2 would be %.0f)"
-                               % ("sustained: the launch was timed inside a >= 0.25 s region" if sustained
-                                  else "burst", mp["tf32_tflops_burst"], mp["tf32_tflops_sustained"],
-                                  0.5 * pk["bf16_tflops"]),
+                "ops": "%s flop of the triangular L*z in %s split precision, 3 N V (V+1) per "
+                       "step; useful_frac counts the FP32-equivalent N V (V+1)"
+                       % (("TF32", "3xTF32") if path == 3 else ("FP16", "scaled 3xFP16")),
+                "peak_source": "phi4_measure_peaks dense tcgen05 kind::%s of this run, %s (burst %.0f, "
+                               "sustained %.0f; kind::tf32 %.0f / %.0f; bf16 of MEASURED_PEAKS.json %.0f)"
+                               % (kind, "sustained: the launch was timed inside a >= 0.25 s region" if sustained
+                                  else "burst", mp[kind + "_tflops_burst"], mp[kind + "_tflops_sustained"],
+                                  mp["tf32_tflops_burst"], mp["tf32_tflops_sustained"], pk["bf16_tflops"]),
+                "proposal_gemm_3xtf32_ms": ph.get("proposal_gemm_3xtf32"),
                 "traffic": traffic, "traffic_source": tsrc,
                 "site_updates_per_s": float(N) * V / t, "ms": ph["proposal_gemm"],
                 "mutation_step_ms": mut_ms / k}
@@ -468,6 +475,12 @@ def measure_workload(name, cfg, args, env, steps, warmup, max_temps, want_e2e):
             ph[key] = B.smc_time_phase(h, p, reps * 2)
             if key == "proposal_gemm":
                 region_s = time.perf_counter() - t0
+        if args.path != 3:
+            # the same product in 3xTF32 (mutation_path 3), for the record: same accuracy, twice the MMAs
+            B.smc_set_params(h, k_steps=k, ess_target=cfg["ess"], mutation_path=3)
+            B.smc_time_phase(h, "proposal", 1)
+            ph["proposal_gemm_3xtf32"] = B.smc_time_phase(h, "proposal", reps * 2)
+            B.smc_set_params(h, k_steps=k, ess_target=cfg["ess"], mutation_path=args.path)
     B.smc_reset(h, 4242)
     for _ in range(3):
         B.smc_step(h, want_info=False)
@@ -490,7 +503,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="C1")
-    ap.add_argument("--path", type=int, default=0, help="mutation path: 0 auto, 1 generic, 2 fused")
+    ap.add_argument("--path", type=int, default=0, help="mutation path: 0 auto, 1 generic, 2 fused, 3 auto with the large-V proposal in 3xTF32")
     ap.add_argument("--ref-particles", type=int, default=16384)
     ap.add_argument("--kernel", default="rw", choices=["rw", "hmc", "irmh"],
                     help="rejuvenation kernel: RW-Metropolis (BASELINE metric), HMC (NEXT row f1) or "
@@ -572,7 +585,7 @@ def main():
             dist.destroy_process_group()
         return
 
-    roof, population = rooflines(args.workload, cfg, m["phases_ms"], pk, mp, m["phase_region_s"])
+    roof, population = rooflines(args.workload, cfg, m["phases_ms"], pk, mp, m["phase_region_s"], args.path)
 
     # ---- large-V sub-records: where the rooflines mean something ------------------
     large = {}
@@ -582,7 +595,7 @@ def main():
             mt = default_max_temps(c, args.max_temps)
             st, wu = (3, 3) if c["L"] >= 64 else (5, 3)
             r = measure_workload(name, c, args, env, st, wu, mt, False)
-            rf, pop = rooflines(name, c, r["phases_ms"], pk, mp, r["phase_region_s"])
+            rf, pop = rooflines(name, c, r["phases_ms"], pk, mp, r["phase_region_s"], args.path)
             large[name] = {"config": workload_config(name, c, 1, temps=r["Ts"], max_temps=mt),
                            "steps": st, "warmup": wu, "ms_per_step": r["ms"] / st,
                            "value": r["site_updates"] / (r["ms"] * 1e-3), "unit": "site-updates/s",
@@ -621,7 +634,7 @@ def main():
             "peaks_measured": dict(mp, hbm_gbs=pk["hbm_gbs"], bf16_tflops=pk["bf16_tflops"],
                                    hbm_bf16_source=pk["source"],
                                    how="phi4_measure_peaks (csrc/measure.cu): dense tcgen05 kind::tf32 "
-                                       "M128 N256 K8 from resident smem operands on all SMs, burst = best "
+                                       "M128 N256 K8 (and kind::f16, K16) from resident smem operands on all SMs, burst = best "
                                        "of 5 launches, sustained = back to back for %.1f s; FP32 FMA and "
                                        "IMAD.WIDE+LOP3 (and FP64 FMA, dfma_tlaneops): 8 chains/thread, 2048 "
                                        "threads/SM" % args.peak_seconds),

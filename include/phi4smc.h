@@ -66,7 +66,9 @@ typedef struct {
   int k_steps;      /* MCMC steps per tempering transition, n_MCMC >= 1           */
   float ess_target; /* target ESS fraction in (0,1) for adaptive tempering        */
   float step_scale; /* s in phi' = phi + s*Lc*z; 0 selects 2.38/sqrt(V) (A3)       */
-  int mutation_path; /* 0 = automatic, 1 = generic (any V), 2 = fused tcgen05 (if it supports V) */
+  int mutation_path; /* 0 = automatic, 1 = generic (any V), 2 = fused tcgen05 (if it supports V),
+                      * 3 = automatic with the large-V proposal product (L*L > 112) in 3xTF32
+                      * instead of the scaled 3xFP16 split of the same accuracy   */
   /* Rejuvenation kernel: 0 = RW-Metropolis (i), 1 = HMC (iii, :172; reading A14),
    * 2 = independent MH from the fitted Gaussian N(mu, Sigma) (ii, :200; reading A15; L*L <= 800).
    * HMC: mass matrix diag(1/var_x) from the particle covariance, hmc_leapfrog >= 1 leapfrog steps
@@ -150,6 +152,8 @@ typedef struct {
   int32_t sms;
   int32_t reserved;
   double dfma_tlaneops;       /* 1e12 FP64 FMA lane-operations / s (8 chains per thread): half the FP32 rate on a B200 */
+  double f16_tflops_burst;    /* dense tcgen05.mma kind::f16 (FP16 operands, FP32 accumulator)     */
+  double f16_tflops_sustained;
 } phi4_peaks;
 int phi4_measure_peaks(double seconds, phi4_peaks* out, void* d_scratch, size_t scratch_bytes,
                        void* cuda_stream);

@@ -69,7 +69,8 @@ class phi4_run_state(C.Structure):
 class phi4_peaks(C.Structure):
     _fields_ = [("tf32_tflops_burst", C.c_double), ("tf32_tflops_sustained", C.c_double),
                 ("ffma_tlaneops", C.c_double), ("imad_wide_tlaneops", C.c_double),
-                ("sms", C.c_int32), ("reserved", C.c_int32), ("dfma_tlaneops", C.c_double)]
+                ("sms", C.c_int32), ("reserved", C.c_int32), ("dfma_tlaneops", C.c_double),
+                ("f16_tflops_burst", C.c_double), ("f16_tflops_sustained", C.c_double)]
 
 
 class phi4_observables(C.Structure):

@@ -364,10 +364,11 @@ PHI4_API int smc_destroy(phi4smc* h) {
 PHI4_API int smc_set_params(phi4smc* h, const smc_params* p) {
   if (!h || !p) return PHI4_EINVAL;
   if (p->k_steps < 1 || !(p->ess_target > 0.f && p->ess_target < 1.f) || p->step_scale < 0.f ||
-      p->mutation_path < 0 || p->mutation_path > 2)
+      p->mutation_path < 0 || p->mutation_path > 3)
     return PHI4_EINVAL;
   if (p->mutation_path == 2 && !mutate_tc_supported(h->md.V) && !propose_tc_supported(h->md.V))
     return PHI4_EINVAL;
+  if (p->mutation_path == 3 && !propose_tc_supported(h->md.V)) return PHI4_EINVAL;
   if (p->kernel < 0 || p->kernel > 2 || p->z2_flip < 0 || p->z2_flip > 1) return PHI4_EINVAL;
   if (p->kernel == 2 && (h->kind != KIND_SMC || !irmh_supported(h->md.V))) return PHI4_EINVAL;
   if (p->kernel == 1 && (h->kind != KIND_SMC || !(p->hmc_eps > 0.f) || p->hmc_leapfrog < 1))
@@ -386,6 +387,7 @@ static MutateArgs smc_mutate_args(phi4smc* h, int k, uint8_t* acc, float* mar, i
   a.N = h->N; a.ld = h->ld; a.md = h->md; a.s = h->s; a.mode = MODE_SMC; a.seed = h->seed;
   a.tag_prop = TAG_PROP; a.tag_acc = TAG_ACC;
   a.t0 = (uint32_t)(h->step_counter + 1); a.k = k; a.respect_done = respect_done;
+  a.tc_f16 = h->prm.mutation_path != 3;
   return a;
 }
 
@@ -967,9 +969,9 @@ PHI4_API int smc_time_phase(phi4smc* h, int phase, int reps, float* h_ms_per_cal
   MutateArgs a = smc_mutate_args(h, h->prm.k_steps, nullptr, nullptr, 0);
   if (phase == PHI4_PHASE_PROPOSAL || phase == PHI4_PHASE_ACCEPT) {
     // operands of a real step: the factor split and one set of normals, one proposal
-    launch_propose_lsplit(a.Lc, V, a.ld, a.s, h->Lsplit, a.ctrl, 0, h->st);
-    launch_normals_split(a.Z, a.N, a.ld, V, a.seed, a.tag_prop, a.t0, a.ctrl, 0, h->st);
-    launch_propose_tc(a.phi, a.phip, a.Z, h->Lsplit, a.ld, V, a.ctrl, 0, h->st);
+    launch_propose_lsplit(a.Lc, V, a.ld, a.s, h->Lsplit, a.ctrl, 0, h->st, a.tc_f16);
+    launch_normals_split(a.Z, a.N, a.ld, V, a.seed, a.tag_prop, a.t0, a.ctrl, 0, h->st, a.tc_f16);
+    launch_propose_tc(a.phi, a.phip, a.Z, h->Lsplit, a.ld, V, a.ctrl, 0, h->st, a.tc_f16);
   }
   CU(cudaEventRecord(e0, h->st));
   for (int r = 0; r < reps; ++r) {
@@ -980,10 +982,10 @@ PHI4_API int smc_time_phase(phi4smc* h, int phase, int reps, float* h_ms_per_cal
         h->step_base += (uint64_t)h->prm.k_steps;
         break;
       case PHI4_PHASE_PROPOSAL:
-        launch_propose_tc(a.phi, a.phip, a.Z, h->Lsplit, a.ld, V, a.ctrl, 0, h->st);
+        launch_propose_tc(a.phi, a.phip, a.Z, h->Lsplit, a.ld, V, a.ctrl, 0, h->st, a.tc_f16);
         break;
       case PHI4_PHASE_NORMALS:
-        launch_normals_split(a.Z, a.N, a.ld, V, a.seed, a.tag_prop, a.t0 + (uint32_t)r, a.ctrl, 0, h->st);
+        launch_normals_split(a.Z, a.N, a.ld, V, a.seed, a.tag_prop, a.t0 + (uint32_t)r, a.ctrl, 0, h->st, a.tc_f16);
         break;
       case PHI4_PHASE_ACCEPT:
         launch_accept_step(a, 0, h->st);

@@ -46,6 +46,8 @@ struct MutateArgs {
   StepRecord* finish_rec = nullptr;
   int finish_max_rec = 0;
   HostPoll* finish_poll = nullptr;
+  // Large-V tcgen05 path: operand format of the split-precision proposal GEMM (propose_tc.cu)
+  bool tc_f16 = true;
 };
 void launch_mutate_generic(const MutateArgs& a, float* Lsplit, cudaStream_t st);
 void launch_accept_step(const MutateArgs& a, int j, cudaStream_t st);
@@ -65,17 +67,18 @@ void launch_mutate_tc(const MutateArgs& a, float* Lsplit, cudaStream_t st, const
 void launch_lsplit(const float* Lc, int V, int Vn, int Kp, float s, float* Lsplit, const Ctrl* ctrl,
                    int respect_done, cudaStream_t st);
 
-// propose_tc.cu -- M1 + M2 for large V: persistent 3xTF32 tcgen05 GEMM, normals in UMMA layout
+// propose_tc.cu -- M1 + M2 for large V: persistent split-precision tcgen05 GEMM, normals in UMMA
+// layout.  f16 = true: 3xFP16 with power-of-two scales (default); false: 3xTF32.
 bool propose_tc_supported(int V);
 size_t propose_tc_zsplit_floats(int V, int ld);
 size_t propose_tc_lsplit_floats(int V);
-void propose_tc_dims(int V, int* Vn, int* Kp);
+void propose_tc_dims(int V, int* Vn, int* Kp, bool f16);
 void launch_normals_split(float* Zs, int N, int ld, int V, uint64_t seed, uint32_t tag, uint32_t t,
-                          const Ctrl* ctrl, int respect_done, cudaStream_t st);
+                          const Ctrl* ctrl, int respect_done, cudaStream_t st, bool f16);
 void launch_propose_lsplit(const float* Lc, int V, int ld, float s, float* Lsplit, const Ctrl* ctrl,
-                           int respect_done, cudaStream_t st);
+                           int respect_done, cudaStream_t st, bool f16);
 void launch_propose_tc(const float* phi, float* phip, const float* Zs, const float* Lsplit, int ld,
-                       int V, const Ctrl* ctrl, int respect_done, cudaStream_t st);
+                       int V, const Ctrl* ctrl, int respect_done, cudaStream_t st, bool f16);
 
 // population.cu -- P1-P4
 bool launch_next_delta_reweight(const float* S, int N, float ess_target, double delta_fixed,

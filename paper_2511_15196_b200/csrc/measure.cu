@@ -4,6 +4,7 @@
 //          CTA per SM issuing from shared-memory operands that never change (no loads: the
 //          tensor pipe alone), two alternating TMEM accumulators.  Burst: best of a few ~10 ms
 //          launches after warm-up; sustained: launches back to back for `seconds`.
+//   f16    the same with kind::f16 (FP16 operands, FP32 accumulator), K = 16 per instruction.
 //   ffma   FP32 fused multiply-adds, 8 independent chains per thread, 2 x 1024 threads per SM.
 //   imad   the Philox round's integer work: 32 x 32 -> 64 multiplies (IMAD.WIDE) with a LOP3.
 // Rates are returned per second; lane-ops count one FMA / one IMAD.WIDE as one operation.
@@ -19,7 +20,8 @@ constexpr int MM_N = 256, MM_K8 = 8;
 constexpr int MM_A_BYTES = 128 * 32, MM_B_BYTES = MM_N * 32;          // K = 8 tf32 = 32 B per row
 constexpr int MM_SETS = 4;                                            // operand sets cycled through
 
-__global__ void __launch_bounds__(128, 1) peak_tf32_kernel(int iters, float* sink) {
+template <bool F16>
+__global__ void __launch_bounds__(128, 1) peak_mma_kernel(int iters, float* sink) {
   using namespace tc;
   extern __shared__ __align__(1024) uint8_t smem[];
   __shared__ uint64_t bar[2];
@@ -28,7 +30,9 @@ __global__ void __launch_bounds__(128, 1) peak_tf32_kernel(int iters, float* sin
   const int nfl = MM_SETS * (MM_A_BYTES + MM_B_BYTES) / 4;
   for (int i = threadIdx.x; i < nfl; i += blockDim.x) {
     uint32_t hsh = (uint32_t)i * 2654435761u + blockIdx.x * 40503u;
+    // (FP16: the same bits read as pairs of halves -- exponent fields 0x3c.. / mantissa noise, all finite)
     f[i] = tf32_rna(((float)(hsh >> 8) * 5.9604644775390625e-8f - 0.5f) * 0.25f);
+    if (F16) reinterpret_cast<uint32_t*>(f)[i] = 0x2c002c00u | (hsh & 0x03ff03ffu);
   }
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   if (threadIdx.x == 0) { mbar_init(smem_u32(&bar[0]), 1); mbar_init(smem_u32(&bar[1]), 1); fence_mbar_init(); }
@@ -40,7 +44,7 @@ __global__ void __launch_bounds__(128, 1) peak_tf32_kernel(int iters, float* sin
   const uint32_t taddr = tmem_slot;
   if (warp == 1 && lane == 0) {
     const uint32_t base = smem_u32(smem);
-    const uint32_t idesc = instr_desc(128, MM_N);
+    const uint32_t idesc = F16 ? instr_desc_f16(128, MM_N) : instr_desc(128, MM_N);
     // batches alternate between two barriers and each barrier is waited on before its next commit
     // is issued, so no phase can be skipped: the queue holds at most two batches of 16 MMAs
     uint32_t ph[2] = {0, 0};
@@ -50,7 +54,8 @@ __global__ void __launch_bounds__(128, 1) peak_tf32_kernel(int iters, float* sin
         const int set = j & (MM_SETS - 1);
         const uint64_t a = smem_desc(base + set * MM_A_BYTES, 128 * 16, 128);
         const uint64_t b = smem_desc(base + MM_SETS * MM_A_BYTES + set * MM_B_BYTES, MM_N * 16, 128);
-        tc_mma_tf32(taddr + (uint32_t)((j & 1) * MM_N), a, b, idesc, (it | (j >> 1)) != 0);
+        if (F16) tc_mma_f16(taddr + (uint32_t)((j & 1) * MM_N), a, b, idesc, (it | (j >> 1)) != 0);
+        else tc_mma_tf32(taddr + (uint32_t)((j & 1) * MM_N), a, b, idesc, (it | (j >> 1)) != 0);
       }
       tc_commit(smem_u32(&bar[it & 1]));
       if (it > 0) { const int b = (it - 1) & 1; mbar_wait(smem_u32(&bar[b]), ph[b]); ph[b] ^= 1; }
@@ -146,7 +151,8 @@ int phi4_measure_peaks(double seconds, phi4_peaks* out, void* d_scratch, size_t 
   cudaEvent_t e0, e1;
   if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return PHI4_ECUDA;
   const int smem = MM_SETS * (MM_A_BYTES + MM_B_BYTES);
-  cudaFuncSetAttribute(peak_tf32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+  cudaFuncSetAttribute(peak_mma_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+  cudaFuncSetAttribute(peak_mma_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
   auto timed = [&](auto launch, int reps) -> double {   // seconds for `reps` launches
     cudaEventRecord(e0, st);
     for (int r = 0; r < reps; ++r) launch();
@@ -156,19 +162,23 @@ int phi4_measure_peaks(double seconds, phi4_peaks* out, void* d_scratch, size_t 
     cudaEventElapsedTime(&ms, e0, e1);
     return (double)ms * 1e-3;
   };
-  // ---- tf32 tensor pipe
-  {
-    const int iters = 4096;                              // 16 MMAs each: ~6 ms per launch
-    const double flop = 2.0 * 128 * MM_N * MM_K8 * 16.0 * iters * sms;
-    auto launch = [&]() { ++g_launches; peak_tf32_kernel<<<sms, 128, smem, st>>>(iters, sink); };
+  // ---- tensor pipe: kind::tf32 (K = 8 per instruction) and kind::f16 (K = 16)
+  for (int f16 = 0; f16 < 2; ++f16) {
+    const int iters = 4096;                              // 16 MMAs each: ~5 ms per launch
+    const double flop = 2.0 * 128 * MM_N * MM_K8 * (f16 ? 2.0 : 1.0) * 16.0 * iters * sms;
+    auto launch = [&]() {
+      ++g_launches;
+      if (f16) peak_mma_kernel<true><<<sms, 128, smem, st>>>(iters, sink);
+      else peak_mma_kernel<false><<<sms, 128, smem, st>>>(iters, sink);
+    };
     timed(launch, 2);                                    // warm-up
     double best = 1e30;
     for (int r = 0; r < 5; ++r) { double t = timed(launch, 1); if (t < best) best = t; }
-    out->tf32_tflops_burst = flop / best * 1e-12;
     const double t1 = timed(launch, 8) / 8.0;
-    int reps = (int)(seconds / t1) + 1;
+    int reps = (int)((f16 ? 0.5 : 1.0) * seconds / t1) + 1;
     const double t = timed(launch, reps);
-    out->tf32_tflops_sustained = flop * reps / t * 1e-12;
+    if (f16) { out->f16_tflops_burst = flop / best * 1e-12; out->f16_tflops_sustained = flop * reps / t * 1e-12; }
+    else { out->tf32_tflops_burst = flop / best * 1e-12; out->tf32_tflops_sustained = flop * reps / t * 1e-12; }
   }
   // ---- FP32 FMA and integer multiply lanes
   {

@@ -284,7 +284,7 @@ void launch_mutate_generic(const MutateArgs& a, float* Lsplit, cudaStream_t st) 
   dim3 gz((a.ld + 127) / 128, (V + 3) / 4);
   dim3 gp(a.ld / 64, (V + 63) / 64);
   if (Lsplit) {
-    launch_propose_lsplit(a.Lc, V, a.ld, a.s, Lsplit, a.ctrl, a.respect_done, st);
+    launch_propose_lsplit(a.Lc, V, a.ld, a.s, Lsplit, a.ctrl, a.respect_done, st, a.tc_f16);
   }
   // Normals of step j+1 on the side stream while the GEMM and the accept kernel of step j run:
   // the GEMM is launched first (one persistent CTA per SM), the normal blocks fill the registers
@@ -295,7 +295,7 @@ void launch_mutate_generic(const MutateArgs& a, float* Lsplit, cudaStream_t st) 
   const bool overlap = Lsplit && a.Z2 && a.side && a.k > 1 && (size_t)a.ld * V >= ((size_t)1 << 24);
   float* zbuf[2] = {a.Z, overlap ? a.Z2 : a.Z};
   if (Lsplit)
-    launch_normals_split(zbuf[0], a.N, a.ld, V, a.seed, a.tag_prop, a.t0, a.ctrl, a.respect_done, st);
+    launch_normals_split(zbuf[0], a.N, a.ld, V, a.seed, a.tag_prop, a.t0, a.ctrl, a.respect_done, st, a.tc_f16);
   for (int j = 0; j < a.k; ++j) {
     uint32_t t = a.t0 + (uint32_t)j;
     if (Lsplit) {
@@ -303,13 +303,13 @@ void launch_mutate_generic(const MutateArgs& a, float* Lsplit, cudaStream_t st) 
         if (j > 0) cudaStreamWaitEvent(st, a.join_ev, 0);          // normals of step j are there
         if (j + 1 < a.k) cudaEventRecord(a.fork_ev, st);
       } else if (j > 0) {
-        launch_normals_split(zbuf[0], a.N, a.ld, V, a.seed, a.tag_prop, t, a.ctrl, a.respect_done, st);
+        launch_normals_split(zbuf[0], a.N, a.ld, V, a.seed, a.tag_prop, t, a.ctrl, a.respect_done, st, a.tc_f16);
       }
-      launch_propose_tc(a.phi, a.phip, zbuf[j & 1], Lsplit, a.ld, V, a.ctrl, a.respect_done, st);
+      launch_propose_tc(a.phi, a.phip, zbuf[j & 1], Lsplit, a.ld, V, a.ctrl, a.respect_done, st, a.tc_f16);
       if (overlap && j + 1 < a.k) {
         cudaStreamWaitEvent(a.side, a.fork_ev, 0);
         launch_normals_split(zbuf[(j + 1) & 1], a.N, a.ld, V, a.seed, a.tag_prop, t + 1, a.ctrl,
-                             a.respect_done, a.side);
+                             a.respect_done, a.side, a.tc_f16);
         cudaEventRecord(a.join_ev, a.side);
       }
     } else {

@@ -1,27 +1,41 @@
 // propose_tc.cu -- M1 + M2 for lattices beyond the fused kernel (V > 112, any V: the packed
-// operands are zero-padded to 256 rows / 16 columns): the proposal product
+// operands are zero-padded to 256 rows / one K-stage of columns): the proposal product
 //   phi'[x][i] = phi[x][i] + sum_{y<=x} (s Lc)[x][y] z[y][i]
-// as a persistent tcgen05 GEMM in 3xTF32 split precision (BASELINE.json north_star: "the N x V x V
-// proposal product L*z ... as tcgen05/TMEM tiles in 3xTF32 split precision"; PAPER.md:53(i), :172).
+// as a persistent tcgen05 GEMM in three-product split precision (BASELINE.json north_star: "the
+// N x V x V proposal product L*z ... as tcgen05/TMEM tiles in 3xTF32 split precision";
+// PAPER.md:53(i), :172).  Two operand formats, template parameter F16:
+//   F16 = false  3xTF32: hi = rna_tf32(v), lo = v - hi; kind::tf32, K = 8 per instruction.
+//   F16 = true   3xFP16, scaled (the default): FP16 has the SAME 11-bit significand as TF32, so
+//                hi = rn_f16(c v), lo = rn_f16(c v - hi) split with the same error bounds, and
+//                kind::f16 multiplies K = 16 per instruction in the same time: half the tensor
+//                work and half the operand bytes.  What FP16 lacks is exponent range, hence the
+//                powers of two c: normals are scaled by 2^3 (|z| < 6.7), s*Lc by 2^(12 - e) with
+//                e = floor(log2 max|s Lc|) measured on the device (labsmax_kernel) -- the largest
+//                entry lands in [2^12, 2^13), entries down to 2^-26 of it stay normal numbers,
+//                smaller ones lose relative, not absolute, accuracy (< 2^-37 of the largest
+//                entry).  The epilogue multiplies the FP32 accumulator by the exact inverse.
 //
 //   normals_split_kernel  Philox normals of one step, split hi/lo, written straight in the UMMA
 //                         K-major interleave layout, stage-major: Zs[particle tile][K-stage][part]
-//                         [4 chunks][128 rows][4] -- a ring stage is one contiguous 16 KB run.
+//                         [4 chunks][128 rows][16 B] -- a ring stage is one contiguous 16 KB run
+//                         (K = 16 TF32 or 32 FP16 columns).
 //   lsplit_tiled_kernel   s*Lc split hi/lo once per temperature, stored per (site tile, K-stage):
 //                         only the rows the stage can reach (lower-triangular), one run per stage.
 //   propose_tc_kernel     one CTA per SM loops over (particle tile 128) x (site tile 256) output
 //                         tiles, in pairs of site tiles of equal total length.  Warp 8 streams A
 //                         (normals) and B (s Lc) into a 4-stage shared-memory ring with two
-//                         cp.async.bulk per stage + mbarrier; warp 9 issues tcgen05.mma kind::tf32
+//                         cp.async.bulk per stage + mbarrier; warp 9 issues tcgen05.mma
 //                         (three products per K-step into one FP32 TMEM accumulator, K-steps above
 //                         the diagonal skipped, N shrunk inside the diagonal block); warps 0-7 read
 //                         the accumulator with tcgen05.ld (lane = particle) and write phi' = phi + d,
 //                         coalesced along particles.  The accumulator is double-buffered (2 x 256
 //                         TMEM columns), so the epilogue of a tile overlaps the MMAs of the next.
 // The tensor core's FP32 accumulation truncates (measured in syrk_tc.cu: -1e-4 relative over 3000
-// MMAs), so one TMEM accumulator only runs over K = 1024 (384 MMAs, ~1e-5 of |d|); the epilogue
-// folds the chains into round-to-nearest FP32 register sums.
+// MMAs), so one TMEM accumulator only runs over K = 1024 (384 / 192 MMAs, ~1e-5 of |d|); the
+// epilogue folds the chains into round-to-nearest FP32 register sums.
 // The accept step stays in accept_kernel (mutate_generic.cu): it needs whole lattice rows of phi'.
+#include <cuda_fp16.h>
+
 #include "kernels.cuh"
 #include "philox.cuh"
 #include "tcgen05.cuh"
@@ -34,37 +48,68 @@ constexpr int TN = 256;                      // sites per output tile = TMEM col
 constexpr int STAGES = 4;
 constexpr int CHUNK_A = TILE * 16;           // one 16-byte K-chunk of 128 rows
 constexpr int CHUNK_B = TN * 16;
-constexpr int A_PART = 4 * CHUNK_A;          // K = 16 per stage: 4 chunks per hi / lo part
+constexpr int A_PART = 4 * CHUNK_A;          // 4 chunks per stage and hi / lo part
 constexpr int B_PART = 4 * CHUNK_B;
 constexpr int STAGE_BYTES = 2 * A_PART + 2 * B_PART;   // 48 KB
 constexpr int THREADS = 320;                 // 8 epilogue warps, producer warp, MMA warp
-constexpr int SUB_STAGES = 64;               // one TMEM accumulation chain covers K = 1024
 constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 256;
+// K columns per ring stage (4 chunks of 16 B: 4 TF32 or 8 FP16 each) and per TMEM chain (1024)
+template <bool F16> struct Fmt {
+  static constexpr int KS = F16 ? 32 : 16, KS_LOG = F16 ? 5 : 4, SUB_STAGES = 1024 / KS;
+  static constexpr int SPB = TN / KS;        // stages of a site tile's diagonal block
+};
+constexpr float Z_SCALE = 8.0f;              // FP16 normals: 2^3 z (|z| < 6.7)
+constexpr int L_TOP = 12;                    // FP16 factor: largest |entry| scaled into [2^12, 2^13)
+constexpr int LMAX_BLOCKS = 148, SCALE_SLOT = 160, SCALE_FLOATS = 256;
 }  // namespace lg
 
-// z of step t for every particle, hi/lo split, stage-major interleave layout:
-// float4 index (((m * nst + q / 4) * 2 + part) * 4 + q % 4) * 128 + pr, part 0 = hi, 1 = lo.
+__device__ __forceinline__ uint32_t pack_half2(__half a, __half b) {
+  return (uint32_t)__half_as_ushort(a) | ((uint32_t)__half_as_ushort(b) << 16);
+}
+// v = hi + lo in FP16 (round to nearest each): |v - hi - lo| <= 2^-22 |v| while lo is a normal number
+__device__ __forceinline__ void split_f16(float v, __half& hi, __half& lo) {
+  hi = __float2half_rn(v);
+  lo = __float2half_rn(v - __half2float(hi));
+}
+
+// z of step t for every particle, hi/lo split, stage-major interleave layout: 16-byte chunk c of
+// particle row pr in tile m sits at chunk index (((m * nst + c / 4) * 2 + part) * 4 + c % 4) * 128 + pr,
+// part 0 = hi, 1 = lo; a chunk is one Philox quad (TF32) or two (FP16: quads 2c, 2c + 1, scaled by 8).
+template <bool F16>
 __global__ void __launch_bounds__(128)
-normals_split_kernel(float4* __restrict__ Zs, int N, int ntm, int V, int Kp, int qpb,
+normals_split_kernel(uint4* __restrict__ Zs, int N, int ntm, int V, int Kp, int cpb,
                      uint64_t seed, uint32_t tag, uint32_t t, const Ctrl* ctrl, int respect_done) {
   pdl_enter();
   if (respect_done && ctrl->done) return;
   const int m = blockIdx.x, pr = threadIdx.x;
-  const int i = m * lg::TILE + pr, nkc = Kp >> 2;
+  const int i = m * lg::TILE + pr, nch = F16 ? Kp >> 3 : Kp >> 2;
   // SFU Box-Muller (philox.cuh, R2).  Quads beyond the lattice (K padding) stay zero;
   // sites >= V inside the last quad meet zero columns.
 #pragma unroll 2
-  for (int qq = 0; qq < qpb; ++qq) {
-    const int q = blockIdx.y * qpb + qq;
-    if (q >= nkc) break;
-    float z[4] = {0.f, 0.f, 0.f, 0.f};
-    if (i < N && 4 * q < V) normals4_fast(seed, tag, t, (uint32_t)i, (uint32_t)q, z);
-    float4 hi, lo;
-    hi.x = tc::tf32_rna(z[0]); lo.x = z[0] - hi.x;
-    hi.y = tc::tf32_rna(z[1]); lo.y = z[1] - hi.y;
-    hi.z = tc::tf32_rna(z[2]); lo.z = z[2] - hi.z;
-    hi.w = tc::tf32_rna(z[3]); lo.w = z[3] - hi.w;
-    const size_t o = ((((size_t)m * (nkc >> 2) + (q >> 2)) * 2) * 4 + (q & 3)) * lg::TILE + pr;
+  for (int cc = 0; cc < cpb; ++cc) {
+    const int c = blockIdx.y * cpb + cc;
+    if (c >= nch) break;
+    uint4 hi, lo;
+    if constexpr (F16) {
+      float z[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+      if (i < N && 8 * c < V) normals4_fast(seed, tag, t, (uint32_t)i, (uint32_t)(2 * c), z);
+      if (i < N && 8 * c + 4 < V) normals4_fast(seed, tag, t, (uint32_t)i, (uint32_t)(2 * c + 1), z + 4);
+      __half h[8], l[8];
+#pragma unroll
+      for (int e = 0; e < 8; ++e) split_f16(lg::Z_SCALE * z[e], h[e], l[e]);
+      hi = make_uint4(pack_half2(h[0], h[1]), pack_half2(h[2], h[3]), pack_half2(h[4], h[5]), pack_half2(h[6], h[7]));
+      lo = make_uint4(pack_half2(l[0], l[1]), pack_half2(l[2], l[3]), pack_half2(l[4], l[5]), pack_half2(l[6], l[7]));
+    } else {
+      float z[4] = {0.f, 0.f, 0.f, 0.f};
+      if (i < N && 4 * c < V) normals4_fast(seed, tag, t, (uint32_t)i, (uint32_t)c, z);
+      float h[4];
+#pragma unroll
+      for (int e = 0; e < 4; ++e) h[e] = tc::tf32_rna(z[e]);
+      hi = make_uint4(__float_as_uint(h[0]), __float_as_uint(h[1]), __float_as_uint(h[2]), __float_as_uint(h[3]));
+      lo = make_uint4(__float_as_uint(z[0] - h[0]), __float_as_uint(z[1] - h[1]), __float_as_uint(z[2] - h[2]),
+                      __float_as_uint(z[3] - h[3]));
+    }
+    const size_t o = ((((size_t)m * (nch >> 2) + (c >> 2)) * 2) * 4 + (c & 3)) * lg::TILE + pr;
     Zs[o] = hi;
     Zs[o + 4 * lg::TILE] = lo;
   }
@@ -74,46 +119,113 @@ normals_split_kernel(float4* __restrict__ Zs, int N, int ntm, int V, int Kp, int
 // (Round 1 issued ten copies per stage -- 2 parts of normals, 2 K-steps x 2 chunks x 2 parts of
 // s*Lc; the ncu source view showed the producer warp never waiting for a free stage while the
 // MMA thread polled "stage full" ~30 times per stage: the copy issue was the bottleneck.)
-// Normals: Zs[m][it][part][4 chunks][128 rows][4] -- 16 KB per (particle tile, stage).
-// s*Lc:    Lt[tn][it][part][kk][c][nrows][4], nrows = the rows of site tile tn that K-stage it
-//          can reach: 256 below the diagonal block, 256 - 16 j in its j-th stage (both K-steps of
-//          a stage start at row xs = 16 it).  32 nrows floats per stage; rows above the diagonal
-//          are never stored or multiplied.
+// Normals: Zs[m][it][part][4 chunks][128 rows][16 B] -- 16 KB per (particle tile, stage).
+// s*Lc:    Lt[tn][it][part][kk][c][nrows][16 B], nrows = the rows of site tile tn that K-stage it
+//          can reach: 256 below the diagonal block, 256 - KS j in its j-th stage (both K-steps of
+//          a stage start at row xs = KS it).  32 nrows floats (128 nrows bytes) per stage; rows
+//          above the diagonal are never stored or multiplied.  Offsets below are in 4-byte units.
+template <bool F16>
 __host__ __device__ inline size_t lt_tile_base(int tn) {          // floats before site tile tn
-  return (size_t)8192 * 16 * ((size_t)tn * (tn - 1) / 2) + (size_t)69632 * tn;
+  using F = lg::Fmt<F16>;
+  const size_t diag = (size_t)32 * (256 * F::SPB - F::KS * (F::SPB * (F::SPB - 1) / 2));
+  return (size_t)8192 * F::SPB * ((size_t)tn * (tn - 1) / 2) + diag * tn;
 }
+template <bool F16>
 __host__ __device__ inline size_t lt_stage_off(int tn, int it) {  // floats before stage it of tile tn
-  const int d0 = 16 * tn;
-  if (it < d0) return lt_tile_base(tn) + (size_t)it * 8192;
+  using F = lg::Fmt<F16>;
+  const int d0 = F::SPB * tn;
+  if (it < d0) return lt_tile_base<F16>(tn) + (size_t)it * 8192;
   const int j = it - d0;
-  return lt_tile_base(tn) + (size_t)d0 * 8192 + (size_t)32 * (256 * j - 8 * j * (j - 1));
+  return lt_tile_base<F16>(tn) + (size_t)d0 * 8192 + (size_t)32 * (256 * j - F::KS * (j * (j - 1) / 2));
 }
 
-__global__ void lsplit_tiled_kernel(const float* __restrict__ Lc, int V, int Vn, int Kp, float s,
-                                    float* __restrict__ out, const Ctrl* ctrl, int respect_done) {
+// max |Lc[x][y]|, y <= x, per block (FP16 path: the scale of the factor); no atomics, no reset
+__global__ void __launch_bounds__(256) labsmax_kernel(const float* __restrict__ Lc, int V,
+                                                      float* __restrict__ blockmax, const Ctrl* ctrl,
+                                                      int respect_done) {
   pdl_enter();
   if (respect_done && ctrl->done) return;
+  float m = 0.f;
+  for (int x = blockIdx.x; x < V; x += gridDim.x)
+    for (int y = threadIdx.x; y <= x; y += blockDim.x) m = fmaxf(m, fabsf(Lc[(size_t)x * V + y]));
+  __shared__ float red[8];
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = m;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < 8; ++w) m = fmaxf(m, red[w]);
+    blockmax[blockIdx.x] = m;
+  }
+}
+
+// c = 2^(L_TOP - floor(log2(s max|Lc|))): the largest scaled entry lies in [2^12, 2^13)
+__device__ inline float l_scale_of(const float* blockmax, float s) {
+  float m = 0.f;
+  for (int b = threadIdx.x & 31; b < lg::LMAX_BLOCKS; b += 32) m = fmaxf(m, blockmax[b]);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+  m *= fabsf(s);
+  if (!(m > 0.f) || !isfinite(m)) return 1.f;
+  return ldexpf(1.f, lg::L_TOP - ilogbf(m));
+}
+
+// one thread per (row x, 16-byte chunk of columns): TF32 4 columns, FP16 8
+template <bool F16>
+__global__ void lsplit_tiled_kernel(const float* __restrict__ Lc, int V, int Vn, int Kp, float s,
+                                    float* __restrict__ out, float* __restrict__ scale,
+                                    const Ctrl* ctrl, int respect_done) {
+  pdl_enter();
+  if (respect_done && ctrl->done) return;
+  using F = lg::Fmt<F16>;
+  constexpr int CW = F16 ? 8 : 4;                      // columns per chunk
+  float c = 1.f;
+  if constexpr (F16) {
+    c = l_scale_of(scale, s);
+    // the GEMM epilogue undoes both scales: exact powers of two
+    if (blockIdx.x == 0 && threadIdx.x == 0) scale[lg::SCALE_SLOT] = 1.0f / (c * lg::Z_SCALE);
+  }
   const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (idx >= (size_t)Kp * Vn) return;
-  const int y = (int)(idx / Vn), x = (int)(idx - (size_t)y * Vn);
-  const int tn = x >> 8, n0 = tn << 8, it = y >> 4;
-  const int rs = max(n0, 16 * it);
+  if (idx >= (size_t)(Kp / CW) * Vn) return;
+  const int yc = (int)(idx / Vn), x = (int)(idx - (size_t)yc * Vn), y0 = yc * CW;
+  const int tn = x >> 8, n0 = tn << 8, it = y0 >> F::KS_LOG;
+  const int rs = max(n0, F::KS * it);
   if (x < rs) return;                                // above the diagonal: never multiplied
   const int nrows = n0 + 256 - rs;
-  const int kk = (y >> 3) & 1, c = (y >> 2) & 1, e = y & 3;
-  const float v = (x < V && y < V && y <= x) ? s * Lc[(size_t)x * V + y] : 0.f;
-  const float hi = tc::tf32_rna(v), lo = tc::tf32_rna(v - hi);
-  const size_t o = lt_stage_off(tn, it) + ((size_t)((kk * 2 + c) * nrows + (x - rs))) * 4 + e;
-  out[o] = hi;
-  out[o + (size_t)16 * nrows] = lo;                  // part stride: 2 kk x 2 c x nrows rows x 4
+  const int kc = (y0 & (F::KS - 1)) / CW;            // chunk of the stage: kk = kc / 2, c = kc % 2
+  float v[CW];
+#pragma unroll
+  for (int e = 0; e < CW; ++e) {
+    const int y = y0 + e;
+    v[e] = (x < V && y < V && y <= x) ? c * s * Lc[(size_t)x * V + y] : 0.f;
+  }
+  uint4 hi, lo;
+  if constexpr (F16) {
+    __half h[8], l[8];
+#pragma unroll
+    for (int e = 0; e < 8; ++e) split_f16(v[e], h[e], l[e]);
+    hi = make_uint4(pack_half2(h[0], h[1]), pack_half2(h[2], h[3]), pack_half2(h[4], h[5]), pack_half2(h[6], h[7]));
+    lo = make_uint4(pack_half2(l[0], l[1]), pack_half2(l[2], l[3]), pack_half2(l[4], l[5]), pack_half2(l[6], l[7]));
+  } else {
+    float h[4];
+#pragma unroll
+    for (int e = 0; e < 4; ++e) h[e] = tc::tf32_rna(v[e]);
+    hi = make_uint4(__float_as_uint(h[0]), __float_as_uint(h[1]), __float_as_uint(h[2]), __float_as_uint(h[3]));
+    lo = make_uint4(__float_as_uint(tc::tf32_rna(v[0] - h[0])), __float_as_uint(tc::tf32_rna(v[1] - h[1])),
+                    __float_as_uint(tc::tf32_rna(v[2] - h[2])), __float_as_uint(tc::tf32_rna(v[3] - h[3])));
+  }
+  uint4* o = reinterpret_cast<uint4*>(out + lt_stage_off<F16>(tn, it)) + (size_t)kc * nrows + (x - rs);
+  o[0] = hi;
+  o[(size_t)4 * nrows] = lo;                         // part stride: 2 kk x 2 c x nrows chunks
 }
 
 struct ProposeTcParams {
   const float* phi; float* phip;     // [V][ld]
   const float* Zs;                   // normals_split_kernel output
-  const float* Lsplit;               // packed s*Lc hi | lo (tcgen05.cuh layout)
+  const float* Lsplit;               // s*Lc hi | lo per (site tile, K-stage): lt_stage_off
+  const float* scale_inv;            // FP16 operands: 1 / (factor scale x normal scale), else unused
   const Ctrl* ctrl;
-  int ld, V, Vn, Kp, ntm, ntn;       // Vn = V rounded up to 256 rows, Kp = V rounded up to 16
+  int ld, V, Vn, Kp, ntm, ntn;       // Vn = V rounded up to 256 rows, Kp = V rounded up to a K-stage
   int respect_done, pair;
 };
 
@@ -143,9 +255,12 @@ struct TileIter {
   }
 };
 
+template <bool F16>
 __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const ProposeTcParams p) {
   using namespace tc;
   using namespace lg;
+  using F = Fmt<F16>;
+  constexpr int KS = F::KS, SUB_STAGES = F::SUB_STAGES;
   extern __shared__ __align__(1024) uint8_t smem[];
   // programmatic dependent launch: barrier setup and the TMEM allocation run before the wait
   pdl_trigger();
@@ -181,21 +296,21 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
     if (lane == 0) {
       int s = 0;
       uint32_t ph = 0;
-      const int nstz = Kp >> 4;
+      const int nstz = Kp >> F::KS_LOG;
       for (TileIter ti(p.ntm, p.ntn, p.pair); ti.valid(); ti.next()) {
         int m, tn;
         ti.tile(m, tn);
         const int n0 = tn * TN;
-        const int nst = min(n0 + TN, Kp) >> 4;               // K-stages up to the tile's last row
+        const int nst = min(n0 + TN, Kp) >> F::KS_LOG;       // K-stages up to the tile's last row
         const float* za = p.Zs + (size_t)m * nstz * (2 * A_PART / 4);
         for (int it = 0; it < nst; ++it) {
           const uint32_t st = ring + (uint32_t)s * STAGE_BYTES;
-          const int nrows = n0 + TN - max(n0, 16 * it);      // rows of the s*Lc block of this stage
+          const int nrows = n0 + TN - max(n0, KS * it);      // rows of the s*Lc block of this stage
           const uint32_t bbytes = 128u * (uint32_t)nrows;    // 2 parts x 2 kk x 2 c x nrows x 16 B
           mbar_wait(empty(s), ph ^ 1);
           mbar_expect_tx(full(s), 2 * A_PART + bbytes);
           bulk_g2s(st, za + (size_t)it * (2 * A_PART / 4), 2 * A_PART, full(s));
-          bulk_g2s(st + 2 * A_PART, p.Lsplit + lt_stage_off(tn, it), bbytes, full(s));
+          bulk_g2s(st + 2 * A_PART, p.Lsplit + lt_stage_off<F16>(tn, it), bbytes, full(s));
           if (++s == STAGES) { s = 0; ph ^= 1; }
         }
       }
@@ -211,7 +326,7 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
         int m, tn;
         ti.tile(m, tn);
         const int n0 = tn * TN;
-        const int nst = min(n0 + TN, Kp) >> 4;
+        const int nst = min(n0 + TN, Kp) >> F::KS_LOG;
         for (int it0 = 0; it0 < nst; it0 += SUB_STAGES, ++cnt) {
           const int buf = cnt & 1;
           mbar_wait(dempty(buf), ((cnt >> 1) & 1) ^ 1);
@@ -222,10 +337,10 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
             mbar_wait(full(s), ph);
             tc_fence_after();
             const uint32_t so = (uint32_t)s * (STAGE_BYTES >> 4);
-            // both K-steps of a stage reach the same rows (xs = 16 it); the block sits packed in
+            // both K-steps of a stage reach the same rows (xs = KS it); the block sits packed in
             // the stage as [part][kk][c][nrows][16 B], so LBO and the part stride follow nrows
-            const int rowstart = max(n0, 16 * it), nrows = n0 + TN - rowstart;
-            const uint32_t idesc = instr_desc(TILE, nrows);
+            const int rowstart = max(n0, KS * it), nrows = n0 + TN - rowstart;
+            const uint32_t idesc = F16 ? instr_desc_f16(TILE, nrows) : instr_desc(TILE, nrows);
             const uint32_t d = dbase + (uint32_t)(rowstart - n0);
             const uint64_t b_st = smem_desc(ring + 2 * A_PART, (uint32_t)nrows * 16u, 128) + so;
 #pragma unroll
@@ -236,10 +351,16 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
               const uint64_t b_lo = b_hi + (uint32_t)(4 * nrows);
               // The first K-step of a chain overwrites the accumulator.  Only the chain that ends
               // in the diagonal block has shrunk K-steps, and it starts with a full-width one
-              // (n0 is a multiple of 256 <= 16 it0 whenever it0 > 0), so no column is left stale.
-              tc_mma_tf32(d, a_lo, b_hi, idesc, (it != it0) || kk);
-              tc_mma_tf32(d, a_hi, b_lo, idesc, 1);
-              tc_mma_tf32(d, a_hi, b_hi, idesc, 1);
+              // (n0 is a multiple of 256 <= KS it0 whenever it0 > 0), so no column is left stale.
+              if constexpr (F16) {
+                tc_mma_f16(d, a_lo, b_hi, idesc, (it != it0) || kk);
+                tc_mma_f16(d, a_hi, b_lo, idesc, 1);
+                tc_mma_f16(d, a_hi, b_hi, idesc, 1);
+              } else {
+                tc_mma_tf32(d, a_lo, b_hi, idesc, (it != it0) || kk);
+                tc_mma_tf32(d, a_hi, b_lo, idesc, 1);
+                tc_mma_tf32(d, a_hi, b_hi, idesc, 1);
+              }
             }
             tc_commit(empty(s));
             if (++s == STAGES) { s = 0; ph ^= 1; }
@@ -255,11 +376,12 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
     int cnt = 0;
     const int Q = warp & 3, hc = warp >> 2;
     const uint32_t tlane = taddr + ((uint32_t)(Q * 32) << 16);
+    const float inv = F16 ? __ldg(p.scale_inv) : 1.f;   // (exact power of two)
     for (TileIter ti(p.ntm, p.ntn, p.pair); ti.valid(); ti.next()) {
       int m, tn;
       ti.tile(m, tn);
       const int n0 = tn * TN;
-      const int nst = min(n0 + TN, Kp) >> 4;
+      const int nst = min(n0 + TN, Kp) >> F::KS_LOG;
       const size_t col = (size_t)m * TILE + Q * 32 + lane;
       const int x0 = n0 + hc * 128;
       if (nst <= SUB_STAGES) {
@@ -283,11 +405,11 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
 #pragma unroll
           for (int jj = 0; jj < 16; ++jj)
             if (x0 + cb + jj < V)
-              p.phip[(size_t)(x0 + cb + jj) * p.ld + col] = f[cb + jj] + __uint_as_float(r0[jj]);
+              p.phip[(size_t)(x0 + cb + jj) * p.ld + col] = fmaf(__uint_as_float(r0[jj]), inv, f[cb + jj]);
 #pragma unroll
           for (int jj = 0; jj < 16; ++jj)
             if (x0 + cb + 16 + jj < V)
-              p.phip[(size_t)(x0 + cb + 16 + jj) * p.ld + col] = f[cb + 16 + jj] + __uint_as_float(r1[jj]);
+              p.phip[(size_t)(x0 + cb + 16 + jj) * p.ld + col] = fmaf(__uint_as_float(r1[jj]), inv, f[cb + 16 + jj]);
         }
         tc_fence_before();
         __syncwarp();
@@ -321,7 +443,7 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
             f[jj] = (x0 + cb + jj < V) ? p.phi[(size_t)(x0 + cb + jj) * p.ld + col] : 0.f;
 #pragma unroll
           for (int jj = 0; jj < 16; ++jj)
-            if (x0 + cb + jj < V) p.phip[(size_t)(x0 + cb + jj) * p.ld + col] = f[jj] + acc[cb + jj];
+            if (x0 + cb + jj < V) p.phip[(size_t)(x0 + cb + jj) * p.ld + col] = fmaf(acc[cb + jj], inv, f[jj]);
         }
       }
     }
@@ -343,60 +465,86 @@ static int num_sms_cached() {
   return n;
 }
 
-// s*Lc split hi / lo in the tiled layout propose_tc_kernel streams (lt_stage_off)
+// s*Lc split hi / lo in the tiled layout propose_tc_kernel streams (lt_stage_off); the FP16 form
+// keeps its per-block maxima and the inverse scale in the SCALE_FLOATS floats behind the operand
+static float* scale_of(float* Lsplit, int V) {
+  return Lsplit + lt_tile_base<true>(round_up(V, lg::TN) / lg::TN);
+}
+
 void launch_propose_lsplit(const float* Lc, int V, int ld, float s, float* Lsplit, const Ctrl* ctrl,
-                           int respect_done, cudaStream_t st) {
+                           int respect_done, cudaStream_t st, bool f16) {
   (void)ld;
   int Vn, Kp;
-  propose_tc_dims(V, &Vn, &Kp);
-  ++g_launches;
-  launch_pdl(lsplit_tiled_kernel, (unsigned)(((size_t)Kp * Vn + 255) / 256), 256, 0, st, Lc, V, Vn,
-             Kp, s, Lsplit, ctrl, respect_done);
+  propose_tc_dims(V, &Vn, &Kp, f16);
+  if (f16) {
+    ++g_launches;
+    launch_pdl(labsmax_kernel, lg::LMAX_BLOCKS, 256, 0, st, Lc, V, scale_of(Lsplit, V), ctrl, respect_done);
+    ++g_launches;
+    launch_pdl(lsplit_tiled_kernel<true>, (unsigned)(((size_t)(Kp / 8) * Vn + 255) / 256), 256, 0, st, Lc, V,
+               Vn, Kp, s, Lsplit, scale_of(Lsplit, V), ctrl, respect_done);
+  } else {
+    ++g_launches;
+    launch_pdl(lsplit_tiled_kernel<false>, (unsigned)(((size_t)(Kp / 4) * Vn + 255) / 256), 256, 0, st, Lc, V,
+               Vn, Kp, s, Lsplit, (float*)nullptr, ctrl, respect_done);
+  }
 }
 
-void propose_tc_dims(int V, int* Vn, int* Kp) {
+void propose_tc_dims(int V, int* Vn, int* Kp, bool f16) {
   *Vn = round_up(V, lg::TN);
-  *Kp = round_up(V, 16);
+  *Kp = round_up(V, f16 ? 32 : 16);
 }
 
+// (sized for either format: the TF32 operands are the larger ones)
 size_t propose_tc_zsplit_floats(int V, int ld) { return (size_t)2 * round_up(V, 16) * ld; }
 
 size_t propose_tc_lsplit_floats(int V) {
-  return lt_tile_base(round_up(V, lg::TN) / lg::TN);
+  const int ntn = round_up(V, lg::TN) / lg::TN;
+  const size_t a = lt_tile_base<false>(ntn), b = lt_tile_base<true>(ntn) + lg::SCALE_FLOATS;
+  return a > b ? a : b;
 }
 
 void launch_normals_split(float* Zs, int N, int ld, int V, uint64_t seed, uint32_t tag, uint32_t t,
-                          const Ctrl* ctrl, int respect_done, cudaStream_t st) {
-  const int Kp = round_up(V, 16);
-  // quads per thread: one quad per block made 1 M blocks at C4 (block-launch-rate bound); a small
-  // population keeps one quad per thread so that the grid still fills the GPU
-  int qpb = (ld / lg::TILE) * (Kp / 4) / (148 * 16);
-  qpb = qpb < 1 ? 1 : qpb > 8 ? 8 : qpb;
-  dim3 grid(ld / lg::TILE, (Kp / 4 + qpb - 1) / qpb);
+                          const Ctrl* ctrl, int respect_done, cudaStream_t st, bool f16) {
+  const int Kp = round_up(V, f16 ? 32 : 16);
+  const int nch = f16 ? Kp / 8 : Kp / 4;             // 16-byte chunks per particle row
+  // chunks per thread: one per block made 1 M blocks at C4 (block-launch-rate bound); a small
+  // population keeps one per thread so that the grid still fills the GPU
+  int cpb = (ld / lg::TILE) * nch / (148 * 16);
+  const int cmax = f16 ? 4 : 8;
+  cpb = cpb < 1 ? 1 : cpb > cmax ? cmax : cpb;
+  dim3 grid(ld / lg::TILE, (nch + cpb - 1) / cpb);
   ++g_launches;
-  launch_pdl(normals_split_kernel, grid, 128, 0, st, reinterpret_cast<float4*>(Zs), N, ld / lg::TILE, V, Kp,
-             qpb, seed, tag, t, ctrl, respect_done);
+  if (f16)
+    launch_pdl(normals_split_kernel<true>, grid, 128, 0, st, reinterpret_cast<uint4*>(Zs), N, ld / lg::TILE, V,
+               Kp, cpb, seed, tag, t, ctrl, respect_done);
+  else
+    launch_pdl(normals_split_kernel<false>, grid, 128, 0, st, reinterpret_cast<uint4*>(Zs), N, ld / lg::TILE, V,
+               Kp, cpb, seed, tag, t, ctrl, respect_done);
 }
 
 void launch_propose_tc(const float* phi, float* phip, const float* Zs, const float* Lsplit, int ld,
-                       int V, const Ctrl* ctrl, int respect_done, cudaStream_t st) {
+                       int V, const Ctrl* ctrl, int respect_done, cudaStream_t st, bool f16) {
   static bool attr_done = false;
   if (!attr_done) {
-    cudaFuncSetAttribute(propose_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    cudaFuncSetAttribute(propose_tc_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                         lg::SMEM_BYTES);
+    cudaFuncSetAttribute(propose_tc_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                          lg::SMEM_BYTES);
     attr_done = true;
   }
   const int num_sms = num_sms_cached();
   ProposeTcParams p;
   p.phi = phi; p.phip = phip; p.Zs = Zs; p.Lsplit = Lsplit; p.ctrl = ctrl;
+  p.scale_inv = f16 ? scale_of(const_cast<float*>(Lsplit), V) + lg::SCALE_SLOT : nullptr;
   p.ld = ld; p.V = V;
-  propose_tc_dims(V, &p.Vn, &p.Kp);
+  propose_tc_dims(V, &p.Vn, &p.Kp, f16);
   p.ntm = ld / lg::TILE; p.ntn = p.Vn / lg::TN; p.respect_done = respect_done;
   p.pair = p.ntm * p.ntn > num_sms;
   const int nunits = p.ntm * (p.pair ? (p.ntn + 1) / 2 : p.ntn);
   const int grid = nunits < num_sms ? nunits : num_sms;
   ++g_launches;
-  launch_pdl(propose_tc_kernel, grid, lg::THREADS, lg::SMEM_BYTES, st, p);
+  if (f16) launch_pdl(propose_tc_kernel<true>, grid, lg::THREADS, lg::SMEM_BYTES, st, p);
+  else launch_pdl(propose_tc_kernel<false>, grid, lg::THREADS, lg::SMEM_BYTES, st, p);
 }
 
 }  // namespace phi4

@@ -187,6 +187,50 @@ def test_mutation_lockstep(L, N, k, beta, fields, path):
     assert 0.0 < rate < 1.0
 
 
+@pytest.mark.parametrize("L,N,k,beta", [(16, 2048, 4, 0.2), (15, 700, 3, 0.5), (18, 1500, 3, 0.4), (23, 900, 3, 0.3)])
+def test_large_v_proposal_in_3xtf32(L, N, k, beta):
+    """mutation_path 3: the large-V proposal product in 3xTF32 (the north_star's wording) instead of the
+    scaled 3xFP16 split that path 0 / 2 take; same lock-step bar."""
+    rate = lockstep(L, N, k, beta, seed=7 + L, fields="smooth", t_start=3 * k, path=3)
+    assert 0.0 < rate < 1.0
+    h = B.smc_init(10, -4.0, 1.0, 256, 0)                      # no large-V product at V <= 112
+    with pytest.raises(B.Phi4Error):
+        B.smc_set_params(h, mutation_path=3)
+    h.close()
+
+
+@pytest.mark.parametrize("path", [0, 3], ids=["3xfp16", "3xtf32"])
+@pytest.mark.parametrize("scale", [1.0 / 64.0, 300.0])
+def test_large_v_proposal_scale_range(scale, path):
+    """The FP16 operands carry a power-of-two scale measured on the device (max |s Lc| into [2^12, 2^13)):
+    a step scale 300 times the default (wild proposals, |g| ~ 1e6: the margins are compared to 1e-5
+    relative, so an overflow or a lost low part shows) and one 64 times smaller."""
+    L, N, k, beta, seed = 16, 1024, 3, 0.3, 11
+    V = L * L
+    s = np.float32(scale * 2.38 / math.sqrt(V))
+    h = B.smc_init(L, -4.0, 1.0, N, seed)
+    B.smc_set_params(h, k_steps=k, ess_target=0.5, step_scale=float(s), mutation_path=path)
+    phi0 = inputs.smooth_fields(L, N, seed=seed + 1)
+    B.smc_set_state(h, phi0, beta, 0)
+    B.estimate_cov_chol(h)
+    Lc = B.smc_get_chol(h)
+    acc, mar = B.smc_mutate(h, k)
+    st1 = B.smc_get_state(h)
+    S0, U00 = O.action_batch(phi0.astype(np.float64), L, -4.0, 1.0)
+    p, S, U0, oacc, omar, _ = O.mutate(phi0, S0, U00, L, -4.0, 1.0, Lc, s, beta, seed, 1, k)
+    amb = np.abs(omar) < BAND + 2e-5 * np.abs(omar)
+    first = np.where(amb.any(axis=0), amb.argmax(axis=0), k)
+    valid = np.arange(k)[:, None] < first[None, :]
+    assert valid.mean() > 0.95 and np.all(np.isfinite(mar))
+    assert np.array_equal(acc[valid], oacc[valid])
+    rel = np.abs(mar[valid] - omar[valid]) / (BAND + 1e-5 * np.abs(omar[valid]))
+    print("scale %.3g path %d: worst margin error %.2f of (1e-4 + 1e-5 |g|), accept %.3f" % (scale, path, rel.max(), acc.mean()))
+    assert rel.max() < 1.0
+    clean = first == k
+    assert np.abs(st1["phi"][:, clean] - p[:, clean]).max() < 2e-5 * max(1.0, scale)
+    h.close()
+
+
 def test_every_lattice_size_has_a_tensor_core_path():
     """V <= 112: fused kernel; V > 112: tcgen05 proposal GEMM on zero-padded operands (the paper's
     own sizes L = 15, 18 included)."""

@@ -20,8 +20,9 @@ def _built():
 
 
 # ---------------------------------------------------------------- correlated L_c at full size ---
-@pytest.mark.parametrize("L,N,k,n_sub", [(32, 65536, 2, 192), (40, 8192, 2, 128), (64, 16384, 1, 64)])
-def test_full_size_correlated_factor(L, N, k, n_sub):
+@pytest.mark.parametrize("L,N,k,n_sub,path", [(32, 65536, 2, 192, 0), (40, 8192, 2, 128, 0), (64, 16384, 1, 64, 0),
+                                              (40, 8192, 2, 128, 3), (64, 16384, 1, 64, 3)])
+def test_full_size_correlated_factor(L, N, k, n_sub, path):
     """C3's and R40's launch shapes (more tiles than SMs: paired site tiles; K > 1024 at V = 1600
     and 4096: several TMEM accumulation chains) with a factor far from the identity: the particles
     are spatially correlated fields with a magnetisation component, so L_c is dense."""
@@ -31,7 +32,7 @@ def test_full_size_correlated_factor(L, N, k, n_sub):
     # zero between lattice momenta and the covariance is singular in fp32 for L >= 32)
     phi0 = inputs.smooth_fields(L, N, seed=5, corr=0.3)
     h = B.smc_init(L, m0sq, lam, N, seed)
-    B.smc_set_params(h, k_steps=k, ess_target=0.5)
+    B.smc_set_params(h, k_steps=k, ess_target=0.5, mutation_path=path)   # 0: scaled 3xFP16, 3: 3xTF32
     B.smc_set_state(h, phi0, beta, 0)
     B.estimate_cov_chol(h)
     Sig, Lc = B.smc_get_cov(h), B.smc_get_chol(h)
@@ -54,8 +55,8 @@ def test_full_size_correlated_factor(L, N, k, n_sub):
     assert valid.mean() > 0.97
     assert np.array_equal(acc[:, sub][valid], oacc[valid])
     err = np.abs(mar[:, sub][valid] - omar[valid]) - 1e-5 * np.abs(omar[valid])
-    print("correlated L=%d: worst margin error %.3g (band 1e-4), off-diagonal weight %.2f, accept %.3f"
-          % (L, err.max(), off, acc.mean()))
+    print("correlated L=%d path %d: worst margin error %.3g (band 1e-4), off-diagonal weight %.2f, accept %.3f"
+          % (L, path, err.max(), off, acc.mean()))
     assert err.max() < 1e-4 * max(1.0, math.sqrt(V / 100.0))
     clean = first == k
     assert np.abs(st1["phi"][:, sub][:, clean] - p[:, clean]).max() < 2e-5
