@@ -381,7 +381,7 @@ PHI4_API int smc_set_params(phi4smc* h, const smc_params* p) {
 static MutateArgs smc_mutate_args(phi4smc* h, int k, uint8_t* acc, float* mar, int respect_done) {
   MutateArgs a;
   a.phi = h->phi[h->cur]; a.phip = h->phip; a.Z = h->Z;
-  a.Z2 = h->Z2; a.side = h->side; a.fork_ev = h->fork_ev; a.join_ev = h->join_ev;
+  a.Z2 = h->Z2;
   a.S = h->S[h->cur]; a.U0 = h->U0[h->cur]; a.Lc = h->Lc; a.ctrl = h->ctrl;
   a.acc_out = acc; a.margin_out = mar;
   a.N = h->N; a.ld = h->ld; a.md = h->md; a.s = h->s; a.mode = MODE_SMC; a.seed = h->seed;
@@ -431,6 +431,7 @@ static CovCholArgs cov_args(phi4smc* h, int respect_done) {
   // the split-normal scratch of the large-V proposal doubles as the centred-split scratch
   c.tc_scratch = (h->prm.mutation_path != 1 && propose_tc_supported(h->md.V) && h->kind == KIND_SMC) ? h->Z : nullptr;
   c.tc_small = h->prm.mutation_path != 1;
+  c.tc_f16 = h->prm.mutation_path != 3;
   c.respect_done = respect_done;
   return c;
 }
@@ -694,7 +695,7 @@ static void enqueue_ns_step(phi4smc* h) {
   launch_cov_chol(cov_args(h, 1), h->st);
   cudaStreamWaitEvent(h->st, h->join_ev, 0);
   MutateArgs m;
-  m.Z2 = h->Z2; m.side = h->side; m.fork_ev = h->fork_ev; m.join_ev = h->join_ev;
+  m.Z2 = h->Z2;
   m.phi = h->wphi; m.phip = h->phip; m.Z = h->Z; m.S = h->wS; m.U0 = h->wU; m.Lc = h->Lc;
   m.ctrl = h->ctrl; m.acc_out = nullptr; m.margin_out = nullptr;
   m.N = h->k_del; m.ld = h->ldw; m.md = h->md; m.s = h->s; m.mode = MODE_NS; m.seed = h->seed;

@@ -9,12 +9,16 @@
 
 namespace phi4 {
 
+// AMAX: also amax[x] = max_i |phi[x][i]| + |mu[x]| >= max_i |phi[x][i] - mu[x]| (the scale of the FP16
+// covariance operands, syrk_tc.cu)
+template <bool AMAX>
 __global__ void __launch_bounds__(256)
 mean_kernel(const float* __restrict__ phi, int N, int ld, float* __restrict__ mu,
-            const Ctrl* ctrl, int respect_done) {
+            float* __restrict__ amax, const Ctrl* ctrl, int respect_done) {
   pdl_enter();
   __shared__ double scratch[33];
   if (respect_done && ctrl->done) return;
+  float big = 0.f;
   const float* row = phi + (size_t)blockIdx.x * ld;
   // ld is a multiple of 128 and pad particles hold zeros: whole float4s.  Two-level sums: at most 32
   // terms in FP32 (four partial sums of eight), folded into FP64 -- one conversion and one FP64 add per
@@ -30,12 +34,24 @@ mean_kernel(const float* __restrict__ phi, int N, int ld, float* __restrict__ mu
       if (i < n4) {
         const float4 v = row4[i];
         f0 += v.x; f1 += v.y; f2 += v.z; f3 += v.w;
+        if (AMAX) big = fmaxf(fmaxf(big, fmaxf(fabsf(v.x), fabsf(v.y))), fmaxf(fabsf(v.z), fabsf(v.w)));
       }
     }
     a += (double)((f0 + f1) + (f2 + f3));
   }
   a = block_sum(a, scratch);
   if (threadIdx.x == 0) mu[blockIdx.x] = (float)(a / (double)N);
+  if (AMAX) {
+    __shared__ float bigs[8];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) big = fmaxf(big, __shfl_xor_sync(0xffffffffu, big, o));
+    if ((threadIdx.x & 31) == 0) bigs[threadIdx.x >> 5] = big;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      for (int w = 1; w < 8; ++w) big = fmaxf(big, bigs[w]);
+      amax[blockIdx.x] = big + fabsf((float)(a / (double)N));
+    }
+  }
 }
 
 // acc[p][r] += sum_{k in [kb,ke)} (A[(x0+ty*4+p)*lda + k] - mx) (A[(y0+tx*4+r)*lda + k] - my)
@@ -634,20 +650,29 @@ static int cov_nsplit(int V, int N) {
 size_t cov_partial_floats(int V, int N) {
   int ns = cov_nsplit(V, N);
   const int ld = round_up(N, 128);
-  if (syrk_tc_supported(V, ld) && syrk_tc_nsplit(V, ld) > ns) ns = syrk_tc_nsplit(V, ld);
+  if (syrk_tc_supported(V, ld) && syrk_tc_nsplit(V, ld, false) > ns) ns = syrk_tc_nsplit(V, ld, false);
+  if (syrk_tc_supported(V, ld) && syrk_tc_nsplit(V, ld, true) > ns) ns = syrk_tc_nsplit(V, ld, true);
   if (syrk_tc_small_supported(V, ld) && syrk_tc_small_nsplit(ld) > ns) ns = syrk_tc_small_nsplit(ld);
   return (size_t)ns * V * V;
 }
 
 void launch_cov_chol(const CovCholArgs& a, cudaStream_t st) {
   const int V = a.V;
-  ++g_launches; launch_pdl(mean_kernel, V, 256, 0, st, a.phi, a.N, a.ld, a.mu, a.ctrl, a.respect_done);
   if (a.tc_scratch && syrk_tc_supported(V, a.ld)) {
-    launch_syrk_tc(a.phi, a.N, a.ld, V, a.mu, a.tc_scratch, a.partial, a.ctrl, a.respect_done, st);
-    launch_syrk_reduce(a.partial, syrk_tc_nsplit(V, a.ld), V, a.N, a.Sigma, a.ctrl, a.respect_done, st);
+    ++g_launches;
+    if (a.tc_f16)
+      launch_pdl(mean_kernel<true>, V, 256, 0, st, a.phi, a.N, a.ld, a.mu, syrk_tc_amax(a.tc_scratch, V, a.ld),
+                 (const Ctrl*)a.ctrl, a.respect_done);
+    else
+      launch_pdl(mean_kernel<false>, V, 256, 0, st, a.phi, a.N, a.ld, a.mu, (float*)nullptr, (const Ctrl*)a.ctrl,
+                 a.respect_done);
+    launch_syrk_tc(a.phi, a.N, a.ld, V, a.mu, a.tc_scratch, a.partial, a.ctrl, a.respect_done, st, a.tc_f16);
+    launch_syrk_reduce(a.partial, syrk_tc_nsplit(V, a.ld, a.tc_f16), V, a.N, a.Sigma, a.ctrl, a.respect_done, st);
     launch_cholesky(a.Sigma, a.Lc, V, a.ctrl, a.respect_done, st);
     return;
   }
+  ++g_launches; launch_pdl(mean_kernel<false>, V, 256, 0, st, a.phi, a.N, a.ld, a.mu, (float*)nullptr,
+                           (const Ctrl*)a.ctrl, a.respect_done);
   // (populations below 8192 stay on the SIMT tiles: at n_live = 4096 the 32 tensor-core CTAs take
   // 11 us against 10 for the 3 x 94 SIMT blocks; at N = 16384 it is 11 against 19)
   if (a.tc_small && a.ld >= 8192 && syrk_tc_small_supported(V, a.ld)) {

@@ -35,12 +35,10 @@ struct MutateArgs {
   uint32_t t0;       // step counter of the first step
   int k;             // number of steps
   int respect_done;  // 1: every kernel is a no-op once ctrl->done is set
-  // Large-V tcgen05 path only (nullptr / 0 otherwise): a second buffer for the split normals and a
-  // side stream with two events, so that the normals of step t+1 are drawn while the proposal GEMM
-  // and the accept kernel of step t run (the normals depend on nothing but the counters).
+  // Large-V tcgen05 path only (nullptr otherwise): a second buffer for the split normals, so that the
+  // normals of step t+1 are drawn inside the proposal GEMM of step t (they depend on nothing but
+  // the counters).
   float* Z2;
-  cudaStream_t side;
-  cudaEvent_t fork_ev, join_ev;
   // Fused tcgen05 path only: if set, the last CTA to finish closes the temperature itself
   // (finish_step_device) and the caller launches no finish_step_kernel.
   StepRecord* finish_rec = nullptr;
@@ -77,8 +75,12 @@ void launch_normals_split(float* Zs, int N, int ld, int V, uint64_t seed, uint32
                           const Ctrl* ctrl, int respect_done, cudaStream_t st, bool f16);
 void launch_propose_lsplit(const float* Lc, int V, int ld, float s, float* Lsplit, const Ctrl* ctrl,
                            int respect_done, cudaStream_t st, bool f16);
+// next != nullptr: two spare warps of every GEMM CTA also draw the normals of step next->t into
+// next->Zs (same layout and numbers as launch_normals_split) while the tensor core works
+struct NextNormals { float* Zs; int N; uint64_t seed; uint32_t tag, t; };
 void launch_propose_tc(const float* phi, float* phip, const float* Zs, const float* Lsplit, int ld,
-                       int V, const Ctrl* ctrl, int respect_done, cudaStream_t st, bool f16);
+                       int V, const Ctrl* ctrl, int respect_done, cudaStream_t st, bool f16,
+                       const NextNormals* next = nullptr);
 
 // population.cu -- P1-P4
 bool launch_next_delta_reweight(const float* S, int N, float ess_target, double delta_fixed,
@@ -104,6 +106,7 @@ struct CovCholArgs {
   int tc_small;      // V <= 128: 1 = tcgen05 syrk (syrk_tc_small.cu), 0 = FP32 SIMT reference
   Ctrl* ctrl;
   int respect_done;
+  bool tc_f16 = true; // large-V tcgen05 syrk: scaled 3xFP16 operands (false: 3xTF32)
 };
 size_t cov_partial_floats(int V, int N);
 void launch_cov_chol(const CovCholArgs& a, cudaStream_t st);
@@ -117,10 +120,11 @@ bool syrk_tc_small_supported(int V, int ld);
 int syrk_tc_small_nsplit(int ld);
 void launch_syrk_tc_small(const float* phi, int N, int ld, int V, const float* mu, float* partial,
                           const Ctrl* ctrl, int respect_done, cudaStream_t st);
-int syrk_tc_nsplit(int V, int ld);
+int syrk_tc_nsplit(int V, int ld, bool f16);
 size_t syrk_tc_scratch_floats(int V, int ld);
+float* syrk_tc_amax(float* Ps, int V, int ld);     // per-site bounds behind the operand (FP16 scale)
 void launch_syrk_tc(const float* phi, int N, int ld, int V, const float* mu, float* Ps,
-                    float* partial, const Ctrl* ctrl, int respect_done, cudaStream_t st);
+                    float* partial, const Ctrl* ctrl, int respect_done, cudaStream_t st, bool f16);
 
 // observables.cu -- O
 void launch_magnetisation(const float* phi, int N, int ld, int V, float* M, cudaStream_t st);

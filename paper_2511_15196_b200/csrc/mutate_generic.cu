@@ -286,32 +286,24 @@ void launch_mutate_generic(const MutateArgs& a, float* Lsplit, cudaStream_t st) 
   if (Lsplit) {
     launch_propose_lsplit(a.Lc, V, a.ld, a.s, Lsplit, a.ctrl, a.respect_done, st, a.tc_f16);
   }
-  // Normals of step j+1 on the side stream while the GEMM and the accept kernel of step j run:
-  // the GEMM is launched first (one persistent CTA per SM), the normal blocks fill the registers
-  // and issue slots it leaves free.  Buffer j & 1; the fork event is recorded after accept(j-1),
-  // i.e. after the last reader (GEMM j-1) of the buffer that step j+1 overwrites.
-  // (only where a step is long enough to pay for the two cross-stream dependencies: at the
-  // paper's N = 5000 a step is 20-40 us and the fork / join cost more than the 5 us they hide)
-  const bool overlap = Lsplit && a.Z2 && a.side && a.k > 1 && (size_t)a.ld * V >= ((size_t)1 << 24);
-  float* zbuf[2] = {a.Z, overlap ? a.Z2 : a.Z};
+  // Normals of step j+1 while the GEMM of step j runs (they depend on nothing but the counters):
+  // drawn by two spare warps inside every GEMM CTA into the other buffer.  (Round 2 first launched
+  // them as a kernel of their own on a side stream: beside a persistent GEMM CTA -- 12 warps' worth
+  // of registers -- no block of another kernel fits, so they only started when GEMM CTAs exited and
+  // then ran against the accept kernel: C3 0.55 ms per step for 0.23 + 0.16 ms of GEMM + accept.)
+  // Only where a CTA's GEMM work is long enough to hide its share of the normals.
+  const bool fuse = Lsplit && a.Z2 && a.k > 1 && (size_t)a.ld * V >= ((size_t)1 << 22);
+  float* zbuf[2] = {a.Z, fuse ? a.Z2 : a.Z};
   if (Lsplit)
     launch_normals_split(zbuf[0], a.N, a.ld, V, a.seed, a.tag_prop, a.t0, a.ctrl, a.respect_done, st, a.tc_f16);
   for (int j = 0; j < a.k; ++j) {
     uint32_t t = a.t0 + (uint32_t)j;
     if (Lsplit) {
-      if (overlap) {
-        if (j > 0) cudaStreamWaitEvent(st, a.join_ev, 0);          // normals of step j are there
-        if (j + 1 < a.k) cudaEventRecord(a.fork_ev, st);
-      } else if (j > 0) {
+      if (!fuse && j > 0)
         launch_normals_split(zbuf[0], a.N, a.ld, V, a.seed, a.tag_prop, t, a.ctrl, a.respect_done, st, a.tc_f16);
-      }
-      launch_propose_tc(a.phi, a.phip, zbuf[j & 1], Lsplit, a.ld, V, a.ctrl, a.respect_done, st, a.tc_f16);
-      if (overlap && j + 1 < a.k) {
-        cudaStreamWaitEvent(a.side, a.fork_ev, 0);
-        launch_normals_split(zbuf[(j + 1) & 1], a.N, a.ld, V, a.seed, a.tag_prop, t + 1, a.ctrl,
-                             a.respect_done, a.side, a.tc_f16);
-        cudaEventRecord(a.join_ev, a.side);
-      }
+      const NextNormals nx = {zbuf[(j + 1) & 1], a.N, a.seed, a.tag_prop, t + 1};
+      launch_propose_tc(a.phi, a.phip, zbuf[j & 1], Lsplit, a.ld, V, a.ctrl, a.respect_done, st, a.tc_f16,
+                        (fuse && j + 1 < a.k) ? &nx : nullptr);
     } else {
       ++g_launches; normals_kernel<<<gz, 128, 0, st>>>(a.Z, a.N, a.ld, V, a.seed, a.tag_prop, t, a.ctrl,
                                          a.respect_done);

@@ -51,7 +51,13 @@ constexpr int CHUNK_B = TN * 16;
 constexpr int A_PART = 4 * CHUNK_A;          // 4 chunks per stage and hi / lo part
 constexpr int B_PART = 4 * CHUNK_B;
 constexpr int STAGE_BYTES = 2 * A_PART + 2 * B_PART;   // 48 KB
-constexpr int THREADS = 320;                 // 8 epilogue warps, producer warp, MMA warp
+// 8 epilogue warps (warpgroups 0-1), producer warp, MMA warp and 10 warps that draw the next step's
+// normals (warpgroups 2-4).  The kernel is compiled for 96 registers per thread; the epilogue
+// warpgroups then take 168 each (setmaxnreg.inc) out of what the other three give back (48 each):
+// 8 x 168 + 12 x 48 = 20 x 96.
+constexpr int THREADS = 640;
+constexpr int GEN_WARP0 = 10, GEN_THREADS = THREADS - 32 * GEN_WARP0;
+constexpr int REGS_EPI = 168, REGS_REST = 48;
 constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 256;
 // K columns per ring stage (4 chunks of 16 B: 4 TF32 or 8 FP16 each) and per TMEM chain (1024)
 template <bool F16> struct Fmt {
@@ -72,6 +78,35 @@ __device__ __forceinline__ void split_f16(float v, __half& hi, __half& lo) {
   lo = __float2half_rn(v - __half2float(hi));
 }
 
+// 16-byte chunk c of particle i: one Philox quad (TF32) or two (FP16: quads 2c, 2c + 1, scaled by 8),
+// split hi / lo.  SFU Box-Muller (philox.cuh, R2).  Quads beyond the lattice (K padding) stay
+// zero; sites >= V inside the last quad meet zero columns.
+template <bool F16>
+__device__ __forceinline__ void normals_chunk(uint64_t seed, uint32_t tag, uint32_t t, int i, int c, int N,
+                                              int V, uint4& hi, uint4& lo) {
+  if constexpr (F16) {
+    // (no branches: several chunks are in flight per thread and their Philox chains must interleave)
+    float z[8];
+    normals4_fast(seed, tag, t, (uint32_t)i, (uint32_t)(2 * c), z);
+    normals4_fast(seed, tag, t, (uint32_t)i, (uint32_t)(2 * c + 1), z + 4);
+    const float s0 = (i < N && 8 * c < V) ? lg::Z_SCALE : 0.f, s1 = (i < N && 8 * c + 4 < V) ? lg::Z_SCALE : 0.f;
+    __half h[8], l[8];
+#pragma unroll
+    for (int e = 0; e < 8; ++e) split_f16((e < 4 ? s0 : s1) * z[e], h[e], l[e]);
+    hi = make_uint4(pack_half2(h[0], h[1]), pack_half2(h[2], h[3]), pack_half2(h[4], h[5]), pack_half2(h[6], h[7]));
+    lo = make_uint4(pack_half2(l[0], l[1]), pack_half2(l[2], l[3]), pack_half2(l[4], l[5]), pack_half2(l[6], l[7]));
+  } else {
+    float z[4] = {0.f, 0.f, 0.f, 0.f};
+    if (i < N && 4 * c < V) normals4_fast(seed, tag, t, (uint32_t)i, (uint32_t)c, z);
+    float h[4];
+#pragma unroll
+    for (int e = 0; e < 4; ++e) h[e] = tc::tf32_rna(z[e]);
+    hi = make_uint4(__float_as_uint(h[0]), __float_as_uint(h[1]), __float_as_uint(h[2]), __float_as_uint(h[3]));
+    lo = make_uint4(__float_as_uint(z[0] - h[0]), __float_as_uint(z[1] - h[1]), __float_as_uint(z[2] - h[2]),
+                    __float_as_uint(z[3] - h[3]));
+  }
+}
+
 // z of step t for every particle, hi/lo split, stage-major interleave layout: 16-byte chunk c of
 // particle row pr in tile m sits at chunk index (((m * nst + c / 4) * 2 + part) * 4 + c % 4) * 128 + pr,
 // part 0 = hi, 1 = lo; a chunk is one Philox quad (TF32) or two (FP16: quads 2c, 2c + 1, scaled by 8).
@@ -90,25 +125,7 @@ normals_split_kernel(uint4* __restrict__ Zs, int N, int ntm, int V, int Kp, int 
     const int c = blockIdx.y * cpb + cc;
     if (c >= nch) break;
     uint4 hi, lo;
-    if constexpr (F16) {
-      float z[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-      if (i < N && 8 * c < V) normals4_fast(seed, tag, t, (uint32_t)i, (uint32_t)(2 * c), z);
-      if (i < N && 8 * c + 4 < V) normals4_fast(seed, tag, t, (uint32_t)i, (uint32_t)(2 * c + 1), z + 4);
-      __half h[8], l[8];
-#pragma unroll
-      for (int e = 0; e < 8; ++e) split_f16(lg::Z_SCALE * z[e], h[e], l[e]);
-      hi = make_uint4(pack_half2(h[0], h[1]), pack_half2(h[2], h[3]), pack_half2(h[4], h[5]), pack_half2(h[6], h[7]));
-      lo = make_uint4(pack_half2(l[0], l[1]), pack_half2(l[2], l[3]), pack_half2(l[4], l[5]), pack_half2(l[6], l[7]));
-    } else {
-      float z[4] = {0.f, 0.f, 0.f, 0.f};
-      if (i < N && 4 * c < V) normals4_fast(seed, tag, t, (uint32_t)i, (uint32_t)c, z);
-      float h[4];
-#pragma unroll
-      for (int e = 0; e < 4; ++e) h[e] = tc::tf32_rna(z[e]);
-      hi = make_uint4(__float_as_uint(h[0]), __float_as_uint(h[1]), __float_as_uint(h[2]), __float_as_uint(h[3]));
-      lo = make_uint4(__float_as_uint(z[0] - h[0]), __float_as_uint(z[1] - h[1]), __float_as_uint(z[2] - h[2]),
-                      __float_as_uint(z[3] - h[3]));
-    }
+    normals_chunk<F16>(seed, tag, t, i, c, N, V, hi, lo);
     const size_t o = ((((size_t)m * (nch >> 2) + (c >> 2)) * 2) * 4 + (c & 3)) * lg::TILE + pr;
     Zs[o] = hi;
     Zs[o + 4 * lg::TILE] = lo;
@@ -224,6 +241,13 @@ struct ProposeTcParams {
   const float* Zs;                   // normals_split_kernel output
   const float* Lsplit;               // s*Lc hi | lo per (site tile, K-stage): lt_stage_off
   const float* scale_inv;            // FP16 operands: 1 / (factor scale x normal scale), else unused
+  // normals of the NEXT step, drawn by warps 10-11 of every CTA while the tensor core works
+  // (nullptr: none).  A separate kernel cannot do this: beside a GEMM CTA no register file has room
+  // for another block, so its blocks only start once GEMM CTAs exit (CUPTI timeline).
+  uint4* Znext;
+  int N;
+  uint64_t seed;
+  uint32_t tag, t_next;
   const Ctrl* ctrl;
   int ld, V, Vn, Kp, ntm, ntn;       // Vn = V rounded up to 256 rows, Kp = V rounded up to a K-stage
   int respect_done, pair;
@@ -291,12 +315,15 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
     return;
   }
 
+  if (warp >= 8) {
+  asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(REGS_REST));
   if (warp == 8) {
     // ================================ producer: two bulk copies per stage =====================
     if (lane == 0) {
       int s = 0;
       uint32_t ph = 0;
       const int nstz = Kp >> F::KS_LOG;
+      const uint64_t keep = l2_policy_evict_last();
       for (TileIter ti(p.ntm, p.ntn, p.pair); ti.valid(); ti.next()) {
         int m, tn;
         ti.tile(m, tn);
@@ -309,13 +336,31 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
           const uint32_t bbytes = 128u * (uint32_t)nrows;    // 2 parts x 2 kk x 2 c x nrows x 16 B
           mbar_wait(empty(s), ph ^ 1);
           mbar_expect_tx(full(s), 2 * A_PART + bbytes);
-          bulk_g2s(st, za + (size_t)it * (2 * A_PART / 4), 2 * A_PART, full(s));
-          bulk_g2s(st + 2 * A_PART, p.Lsplit + lt_stage_off<F16>(tn, it), bbytes, full(s));
+          bulk_g2s_hint(st, za + (size_t)it * (2 * A_PART / 4), 2 * A_PART, full(s), keep);
+          bulk_g2s_hint(st + 2 * A_PART, p.Lsplit + lt_stage_off<F16>(tn, it), bbytes, full(s), keep);
           if (++s == STAGES) { s = 0; ph ^= 1; }
         }
       }
     }
     __syncwarp();
+  } else if (warp >= GEN_WARP0) {
+    // ================================ normals of the next step ================================
+    if (p.Znext) {
+      const int nch = F16 ? Kp >> 3 : Kp >> 2;             // 16-byte chunks per particle row
+      // flat index over (particle tile, chunk, particle row): consecutive threads, consecutive rows
+      const long long total = (long long)p.ntm * nch * TILE;
+      const long long stride = (long long)gridDim.x * GEN_THREADS;
+      for (long long idx = (long long)blockIdx.x * GEN_THREADS + (threadIdx.x - GEN_WARP0 * 32); idx < total;
+           idx += stride) {
+        const int pr = (int)(idx & (TILE - 1)), mc = (int)(idx >> 7);
+        const int m = mc / nch, c = mc - m * nch, i = m * TILE + pr;
+        uint4 hi, lo;
+        normals_chunk<F16>(p.seed, p.tag, p.t_next, i, c, p.N, V, hi, lo);
+        const size_t o = ((((size_t)m * (nch >> 2) + (c >> 2)) * 2) * 4 + (c & 3)) * TILE + pr;
+        p.Znext[o] = hi;
+        p.Znext[o + 4 * TILE] = lo;
+      }
+    }
   } else if (warp == 9) {
     // ================================ MMA issuer ==============================================
     if (lane == 0) {
@@ -370,7 +415,9 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
       }
     }
     __syncwarp();
+  }
   } else {
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(REGS_EPI));
     // ================================ epilogue: phi' = phi + sum of chains ====================
     // warp w: TMEM lane quarter w % 4 (32 particles), column half w / 4 (128 sites)
     int cnt = 0;
@@ -393,7 +440,7 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
         float f[128];
 #pragma unroll
         for (int j = 0; j < 128; ++j)
-          f[j] = (x0 + j < V) ? p.phi[(size_t)(x0 + j) * p.ld + col] : 0.f;
+          f[j] = (x0 + j < V) ? __ldcs(p.phi + (size_t)(x0 + j) * p.ld + col) : 0.f;
         mbar_wait_relaxed(dfull(buf), (cnt >> 1) & 1);
         tc_fence_after();
 #pragma unroll
@@ -405,11 +452,11 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
 #pragma unroll
           for (int jj = 0; jj < 16; ++jj)
             if (x0 + cb + jj < V)
-              p.phip[(size_t)(x0 + cb + jj) * p.ld + col] = fmaf(__uint_as_float(r0[jj]), inv, f[cb + jj]);
+              __stcs(p.phip + (size_t)(x0 + cb + jj) * p.ld + col, fmaf(__uint_as_float(r0[jj]), inv, f[cb + jj]));
 #pragma unroll
           for (int jj = 0; jj < 16; ++jj)
             if (x0 + cb + 16 + jj < V)
-              p.phip[(size_t)(x0 + cb + 16 + jj) * p.ld + col] = fmaf(__uint_as_float(r1[jj]), inv, f[cb + 16 + jj]);
+              __stcs(p.phip + (size_t)(x0 + cb + 16 + jj) * p.ld + col, fmaf(__uint_as_float(r1[jj]), inv, f[cb + 16 + jj]));
         }
         tc_fence_before();
         __syncwarp();
@@ -440,10 +487,10 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
           float f[16];
 #pragma unroll
           for (int jj = 0; jj < 16; ++jj)
-            f[jj] = (x0 + cb + jj < V) ? p.phi[(size_t)(x0 + cb + jj) * p.ld + col] : 0.f;
+            f[jj] = (x0 + cb + jj < V) ? __ldcs(p.phi + (size_t)(x0 + cb + jj) * p.ld + col) : 0.f;
 #pragma unroll
           for (int jj = 0; jj < 16; ++jj)
-            if (x0 + cb + jj < V) p.phip[(size_t)(x0 + cb + jj) * p.ld + col] = fmaf(acc[cb + jj], inv, f[jj]);
+            if (x0 + cb + jj < V) __stcs(p.phip + (size_t)(x0 + cb + jj) * p.ld + col, fmaf(acc[cb + jj], inv, f[jj]));
         }
       }
     }
@@ -523,7 +570,8 @@ void launch_normals_split(float* Zs, int N, int ld, int V, uint64_t seed, uint32
 }
 
 void launch_propose_tc(const float* phi, float* phip, const float* Zs, const float* Lsplit, int ld,
-                       int V, const Ctrl* ctrl, int respect_done, cudaStream_t st, bool f16) {
+                       int V, const Ctrl* ctrl, int respect_done, cudaStream_t st, bool f16,
+                       const NextNormals* next) {
   static bool attr_done = false;
   if (!attr_done) {
     cudaFuncSetAttribute(propose_tc_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -536,6 +584,9 @@ void launch_propose_tc(const float* phi, float* phip, const float* Zs, const flo
   ProposeTcParams p;
   p.phi = phi; p.phip = phip; p.Zs = Zs; p.Lsplit = Lsplit; p.ctrl = ctrl;
   p.scale_inv = f16 ? scale_of(const_cast<float*>(Lsplit), V) + lg::SCALE_SLOT : nullptr;
+  p.Znext = next ? reinterpret_cast<uint4*>(next->Zs) : nullptr;
+  p.N = next ? next->N : 0; p.seed = next ? next->seed : 0; p.tag = next ? next->tag : 0;
+  p.t_next = next ? next->t : 0;
   p.ld = ld; p.V = V;
   propose_tc_dims(V, &p.Vn, &p.Kp, f16);
   p.ntm = ld / lg::TILE; p.ntn = p.Vn / lg::TN; p.respect_done = respect_done;

@@ -1,23 +1,32 @@
 // syrk_tc.cu -- C1 for lattices beyond the single-CTA sizes (V > 112; operands zero-padded to
 // 256 rows and 256 particles): the centred particle covariance
 //   Sigma = (1/(N-1)) sum_i (phi_i - mu)(phi_i - mu)^T
-// as a tcgen05 GEMM in 3xTF32 split precision (BASELINE.json north_star: "the V x V covariance
-// syrk as tcgen05/TMEM tiles in 3xTF32 split precision"; readings A4, R6).
+// as a tcgen05 GEMM in three-product split precision (BASELINE.json north_star: "the V x V
+// covariance syrk as tcgen05/TMEM tiles in 3xTF32 split precision"; readings A4, R6).
+// Operand format, template parameter F16 (as in propose_tc.cu): false = 3xTF32; true (default) =
+// 3xFP16 with a power-of-two scale c = 2^(11 - e), e = floor(log2 of a bound on max |phi - mu|)
+// taken on the device (mean_kernel also returns max_i |phi[x][i]|; syrk_scale_kernel) -- the same
+// 11-bit significands, K = 16 per MMA instead of 8, half the operand bytes; the epilogue multiplies
+// the FP32 sums by the exact 1 / c^2.
 //
-//   centre_split_kernel  phi[x][i] - mu[x] -> hi/lo TF32 parts in the UMMA K-major interleave
-//                        layout with the particle index as contraction index:
-//                        Ps[part][i / 4][x][i % 4]  (a 128-row slice of one K-chunk is 2 KB
-//                        contiguous).  Transposed through shared memory: coalesced both ways.
+//   centre_split_kernel  phi[x][i] - mu[x] -> hi/lo parts in the UMMA K-major interleave layout
+//                        with the particle index as contraction index: 16-byte chunks of 4 (TF32)
+//                        or 8 (FP16) consecutive particles, Ps[part][chunk][x] (a 128-row slice of
+//                        one K-chunk is 2 KB contiguous).  Transposed through shared memory:
+//                        coalesced both ways.
 //   syrk_tc_kernel       work item = (lower-triangular 128 x 256 output tile, K split).  Warp 8
-//                        streams both operand slices of a K = 16 stage with cp.async.bulk into a
-//                        4-stage ring, warp 9 issues tcgen05.mma kind::tf32 (hi*hi + hi*lo + lo*hi
+//                        streams both operand slices of a 4-chunk stage with cp.async.bulk into a
+//                        4-stage ring, warp 9 issues tcgen05.mma (hi*hi + hi*lo + lo*hi
 //                        into one FP32 TMEM accumulator).  The tensor core's FP32 accumulation
 //                        truncates: over the 1e5-term sums of a covariance that is a -1e-4
-//                        relative bias (measured), so an accumulator only runs over K = 256
-//                        (96 MMAs); warps 0-7 then fold it into round-to-nearest FP32 register
-//                        sums (tcgen05.ld, double-buffered TMEM) and write the partial tile once.
+//                        relative bias (measured), so an accumulator only runs over 16 stages
+//                        (96 MMAs: K = 256 or 512); warps 0-7 then fold it into round-to-nearest
+//                        FP32 register sums (tcgen05.ld, double-buffered TMEM) and write the
+//                        partial tile once.
 //   syrk_reduce_kernel   (covchol.cu) sums the K-split partials in a fixed order, scales by
 //                        1/(N-1) and mirrors the lower triangle.
+#include <cuda_fp16.h>
+
 #include "kernels.cuh"
 #include "tcgen05.cuh"
 
@@ -26,38 +35,80 @@ namespace phi4 {
 namespace sy {
 constexpr int TM = 128, TN = 256, STAGES = 4;
 constexpr int CHUNK_A = TM * 16, CHUNK_B = TN * 16;
-constexpr int A_PART = 4 * CHUNK_A, B_PART = 4 * CHUNK_B;       // K = 16 per stage
+constexpr int A_PART = 4 * CHUNK_A, B_PART = 4 * CHUNK_B;       // 4 chunks per stage: K = 16 / 32
 constexpr int STAGE_BYTES = 2 * A_PART + 2 * B_PART;            // 48 KB
 constexpr int THREADS = 320;          // 8 epilogue warps, producer warp, MMA warp
-constexpr int SUB_STAGES = 16;        // TMEM accumulation chain: K = 256 per flush
+constexpr int SUB_STAGES = 16;        // TMEM accumulation chain: 16 stages (96 MMAs) per flush
+constexpr int S_TOP = 11;             // FP16: the bound on max |phi - mu| scaled into [2^11, 2^12)
 constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 256;
 }  // namespace sy
 
+// c and 1 / c^2 from the per-site bounds amax[x] >= max_i |phi[x][i] - mu[x]| (one small block)
+__global__ void __launch_bounds__(256) syrk_scale_kernel(const float* __restrict__ amax, int V,
+                                                         float* __restrict__ slot, const Ctrl* ctrl,
+                                                         int respect_done) {
+  if (respect_done && ctrl->done) return;
+  __shared__ float red[8];
+  float m = 0.f;
+  for (int x = threadIdx.x; x < V; x += blockDim.x) m = fmaxf(m, amax[x]);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = m;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < 8; ++w) m = fmaxf(m, red[w]);
+    const float c = (m > 0.f && isfinite(m)) ? ldexpf(1.f, sy::S_TOP - ilogbf(m)) : 1.f;
+    slot[0] = c;
+    slot[1] = 1.0f / (c * c);
+  }
+}
+
+__device__ __forceinline__ uint32_t syrk_pack_half2(__half a, __half b) {
+  return (uint32_t)__half_as_ushort(a) | ((uint32_t)__half_as_ushort(b) << 16);
+}
+
 // Block = 32 sites x 128 particles.  Pad particles (i >= N) contribute exact zeros.
+template <bool F16>
 __global__ void __launch_bounds__(256)
 centre_split_kernel(const float* __restrict__ phi, int N, int ld, int V, int Vn, int ldp,
-                    const float* __restrict__ mu, float4* __restrict__ Ps, const Ctrl* ctrl,
-                    int respect_done) {
+                    const float* __restrict__ mu, uint4* __restrict__ Ps, const float* __restrict__ slot,
+                    const Ctrl* ctrl, int respect_done) {
   if (respect_done && ctrl->done) return;
   __shared__ float tile[32][129];
   const int x0 = blockIdx.y * 32, i0 = blockIdx.x * 128;
+  const float c = F16 ? slot[0] : 1.f;
   for (int e = threadIdx.x; e < 32 * 128; e += 256) {
     const int xr = e >> 7, ic = e & 127;
     const int i = i0 + ic, x = x0 + xr;
-    tile[xr][ic] = (i < N && x < V) ? phi[(size_t)x * ld + i] - mu[x] : 0.f;   // zero padding
+    tile[xr][ic] = (i < N && x < V) ? c * (phi[(size_t)x * ld + i] - mu[x]) : 0.f;   // zero padding
   }
   __syncthreads();
-  const size_t part = (size_t)(ldp >> 2) * Vn;           // float4s per hi / lo part
-  for (int e = threadIdx.x; e < 32 * 32; e += 256) {
+  constexpr int CW = F16 ? 8 : 4, CSH = F16 ? 3 : 2;     // particles per 16-byte chunk
+  const size_t part = (size_t)(ldp >> CSH) * Vn;         // chunks per hi / lo part
+  for (int e = threadIdx.x; e < 32 * (128 / CW); e += 256) {
     const int kc = e >> 5, xr = e & 31;                  // lanes along x: 512 B contiguous stores
-    float4 hi, lo;
-    const float v0 = tile[xr][4 * kc], v1 = tile[xr][4 * kc + 1], v2 = tile[xr][4 * kc + 2],
-                v3 = tile[xr][4 * kc + 3];
-    hi.x = tc::tf32_rna(v0); lo.x = v0 - hi.x;
-    hi.y = tc::tf32_rna(v1); lo.y = v1 - hi.y;
-    hi.z = tc::tf32_rna(v2); lo.z = v2 - hi.z;
-    hi.w = tc::tf32_rna(v3); lo.w = v3 - hi.w;
-    const size_t o = (size_t)((i0 >> 2) + kc) * Vn + x0 + xr;
+    uint4 hi, lo;
+    if constexpr (F16) {
+      __half h[8], l[8];
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        const float v = tile[xr][8 * kc + j];
+        h[j] = __float2half_rn(v);
+        l[j] = __float2half_rn(v - __half2float(h[j]));
+      }
+      hi = make_uint4(syrk_pack_half2(h[0], h[1]), syrk_pack_half2(h[2], h[3]), syrk_pack_half2(h[4], h[5]),
+                      syrk_pack_half2(h[6], h[7]));
+      lo = make_uint4(syrk_pack_half2(l[0], l[1]), syrk_pack_half2(l[2], l[3]), syrk_pack_half2(l[4], l[5]),
+                      syrk_pack_half2(l[6], l[7]));
+    } else {
+      float v[4], h[4];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) { v[j] = tile[xr][4 * kc + j]; h[j] = tc::tf32_rna(v[j]); }
+      hi = make_uint4(__float_as_uint(h[0]), __float_as_uint(h[1]), __float_as_uint(h[2]), __float_as_uint(h[3]));
+      lo = make_uint4(__float_as_uint(v[0] - h[0]), __float_as_uint(v[1] - h[1]), __float_as_uint(v[2] - h[2]),
+                      __float_as_uint(v[3] - h[3]));
+    }
+    const size_t o = (size_t)((i0 >> CSH) + kc) * Vn + x0 + xr;
     Ps[o] = hi;
     Ps[part + o] = lo;
   }
@@ -65,6 +116,7 @@ centre_split_kernel(const float* __restrict__ phi, int N, int ld, int V, int Vn,
 
 struct SyrkTcParams {
   const float* Ps;       // centre_split_kernel output
+  const float* slot;     // FP16: {c, 1 / c^2}
   float* partial;        // [nsplit][V][V]
   const Ctrl* ctrl;
   int V, Vn, nkc, ntm, nsplit, chunks_per_split, nitems;   // Vn = V rounded up to 256
@@ -92,6 +144,7 @@ __device__ __forceinline__ void syrk_item(const SyrkTcParams& p, int item, int& 
   n0 = t * sy::TN;
 }
 
+template <bool F16>
 __global__ void __launch_bounds__(sy::THREADS, 1) syrk_tc_kernel(const SyrkTcParams p) {
   using namespace tc;
   using namespace sy;
@@ -118,7 +171,7 @@ __global__ void __launch_bounds__(sy::THREADS, 1) syrk_tc_kernel(const SyrkTcPar
   tc_fence_after();
   const uint32_t taddr = *tmem_slot;
   const uint32_t ring = smem_u32(smem);
-  const int nst = p.chunks_per_split >> 2;                 // K = 16 stages per item
+  const int nst = p.chunks_per_split >> 2;                 // stages (4 chunks) per item
 
   if (warp == 8) {
     if (lane == 0) {
@@ -156,7 +209,7 @@ __global__ void __launch_bounds__(sy::THREADS, 1) syrk_tc_kernel(const SyrkTcPar
       uint32_t ph = 0;
       const uint64_t a_base = smem_desc(ring, CHUNK_A, 128);
       const uint64_t b_base = smem_desc(ring + 2 * A_PART, CHUNK_B, 128);
-      const uint32_t idesc = instr_desc(TM, TN);
+      const uint32_t idesc = F16 ? instr_desc_f16(TM, TN) : instr_desc(TM, TN);
       for (int item = blockIdx.x; item < p.nitems; item += gridDim.x) {
         for (int sub = 0; sub < nst / SUB_STAGES; ++sub, ++cnt) {
           const int buf = cnt & 1;
@@ -173,9 +226,15 @@ __global__ void __launch_bounds__(sy::THREADS, 1) syrk_tc_kernel(const SyrkTcPar
               const uint64_t a_lo = a_hi + (A_PART >> 4);
               const uint64_t b_hi = b_base + so + (uint32_t)(2 * kk) * (CHUNK_B >> 4);
               const uint64_t b_lo = b_hi + (B_PART >> 4);
-              tc_mma_tf32(d, a_lo, b_hi, idesc, (it | kk) != 0);
-              tc_mma_tf32(d, a_hi, b_lo, idesc, 1);
-              tc_mma_tf32(d, a_hi, b_hi, idesc, 1);
+              if constexpr (F16) {
+                tc_mma_f16(d, a_lo, b_hi, idesc, (it | kk) != 0);
+                tc_mma_f16(d, a_hi, b_lo, idesc, 1);
+                tc_mma_f16(d, a_hi, b_hi, idesc, 1);
+              } else {
+                tc_mma_tf32(d, a_lo, b_hi, idesc, (it | kk) != 0);
+                tc_mma_tf32(d, a_hi, b_lo, idesc, 1);
+                tc_mma_tf32(d, a_hi, b_hi, idesc, 1);
+              }
             }
             tc_commit(empty(s));
             if (++s == STAGES) { s = 0; ph ^= 1; }
@@ -190,6 +249,7 @@ __global__ void __launch_bounds__(sy::THREADS, 1) syrk_tc_kernel(const SyrkTcPar
     int cnt = 0;
     const int Q = warp & 3, hc = warp >> 2;
     const uint32_t tlane = taddr + ((uint32_t)(Q * 32) << 16);
+    const float inv = F16 ? p.slot[1] : 1.f;               // (exact power of two)
     for (int item = blockIdx.x; item < p.nitems; item += gridDim.x) {
       int m0, n0, z;
       syrk_item(p, item, m0, n0, z);
@@ -218,11 +278,12 @@ __global__ void __launch_bounds__(sy::THREADS, 1) syrk_tc_kernel(const SyrkTcPar
         if ((V & 3) == 0 && y0 + 128 <= V) {
 #pragma unroll
           for (int j = 0; j < 128; j += 4)
-            *reinterpret_cast<float4*>(out + j) = make_float4(acc[j], acc[j + 1], acc[j + 2], acc[j + 3]);
+            *reinterpret_cast<float4*>(out + j) =
+                make_float4(acc[j] * inv, acc[j + 1] * inv, acc[j + 2] * inv, acc[j + 3] * inv);
         } else {
 #pragma unroll
           for (int j = 0; j < 128; ++j)
-            if (y0 + j < V) out[j] = acc[j];
+            if (y0 + j < V) out[j] = acc[j] * inv;
         }
       }
     }
@@ -244,12 +305,15 @@ static int syrk_tc_tiles(int V) {
   return t;
 }
 
-// K split: every split is a whole number of K = 256 chains; among the admissible counts (at most
+// Particles are padded to a whole number of accumulation chains (16 stages x 4 chunks)
+static int syrk_ldp(int ld, bool f16) { return round_up(ld, f16 ? 512 : 256); }
+
+// K split: every split is a whole number of accumulation chains; among the admissible counts (at most
 // ld / V, so that the partial tiles stay small beside the operands) the one whose items fill whole
 // waves of 148 CTAs best (round 1 took "about two waves": 160 items at C3, a second wave of 12).
-int syrk_tc_nsplit(int V, int ld) {
-  const int nkc = round_up(ld, 256) >> 2, tiles = syrk_tc_tiles(V);
-  const int chains = nkc / (4 * sy::SUB_STAGES);            // K = 256 chains in the whole population
+int syrk_tc_nsplit(int V, int ld, bool f16) {
+  const int nkc = syrk_ldp(ld, f16) >> (f16 ? 3 : 2), tiles = syrk_tc_tiles(V);
+  const int chains = nkc / (4 * sy::SUB_STAGES);            // accumulation chains in the whole population
   int cap = ld / V;
   cap = cap < 1 ? 1 : cap > 64 ? 64 : cap;
   // best wave efficiency first, then the smallest count within 2 % of it (the partial tiles cost
@@ -270,35 +334,57 @@ int syrk_tc_nsplit(int V, int ld) {
   return best;
 }
 
-size_t syrk_tc_scratch_floats(int V, int ld) {
-  return (size_t)2 * round_up(V, sy::TN) * round_up(ld, 256);
+// split operand (either format: 2 Vn ldp(256) floats as TF32, Vn ldp(512) as FP16), then the per-site
+// bounds (Vn floats) and the scale slot
+static size_t syrk_operand_floats(int V, int ld) {
+  const size_t Vn = round_up(V, sy::TN);
+  const size_t a = 2 * Vn * syrk_ldp(ld, false), b = Vn * syrk_ldp(ld, true);
+  return a > b ? a : b;
 }
+size_t syrk_tc_scratch_floats(int V, int ld) {
+  return syrk_operand_floats(V, ld) + round_up(V, sy::TN) + 64;
+}
+float* syrk_tc_amax(float* Ps, int V, int ld) { return Ps + syrk_operand_floats(V, ld); }
 
 void launch_syrk_tc(const float* phi, int N, int ld, int V, const float* mu, float* Ps,
-                    float* partial, const Ctrl* ctrl, int respect_done, cudaStream_t st) {
+                    float* partial, const Ctrl* ctrl, int respect_done, cudaStream_t st, bool f16) {
   static int num_sms = 0;
   if (!num_sms) {
-    cudaFuncSetAttribute(syrk_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    cudaFuncSetAttribute(syrk_tc_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                         sy::SMEM_BYTES);
+    cudaFuncSetAttribute(syrk_tc_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                          sy::SMEM_BYTES);
     int dev = 0;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev);
   }
-  const int Vn = round_up(V, sy::TN), ldp = round_up(ld, 256);
+  const int Vn = round_up(V, sy::TN), ldp = syrk_ldp(ld, f16);
+  float* amax = syrk_tc_amax(Ps, V, ld);
+  float* slot = amax + Vn;
   dim3 gc(ldp / 128, Vn / 32);
-  ++g_launches;
-  centre_split_kernel<<<gc, 256, 0, st>>>(phi, N, ld, V, Vn, ldp, mu, reinterpret_cast<float4*>(Ps),
-                                          ctrl, respect_done);
+  if (f16) {
+    ++g_launches;
+    syrk_scale_kernel<<<1, 256, 0, st>>>(amax, V, slot, ctrl, respect_done);
+    ++g_launches;
+    centre_split_kernel<true><<<gc, 256, 0, st>>>(phi, N, ld, V, Vn, ldp, mu, reinterpret_cast<uint4*>(Ps), slot,
+                                                  ctrl, respect_done);
+  } else {
+    ++g_launches;
+    centre_split_kernel<false><<<gc, 256, 0, st>>>(phi, N, ld, V, Vn, ldp, mu, reinterpret_cast<uint4*>(Ps), slot,
+                                                   ctrl, respect_done);
+  }
   SyrkTcParams p;
-  p.Ps = Ps; p.partial = partial; p.ctrl = ctrl; p.V = V; p.Vn = Vn; p.nkc = ldp >> 2;
+  p.Ps = Ps; p.slot = slot; p.partial = partial; p.ctrl = ctrl; p.V = V; p.Vn = Vn;
+  p.nkc = ldp >> (f16 ? 3 : 2);
   p.ntm = Vn / sy::TM;
-  p.nsplit = syrk_tc_nsplit(V, ld);
+  p.nsplit = syrk_tc_nsplit(V, ld, f16);
   p.chunks_per_split = p.nkc / p.nsplit;
   p.nitems = syrk_tc_tiles(V) * p.nsplit;
   p.respect_done = respect_done;
   const int grid = p.nitems < num_sms ? p.nitems : num_sms;
   ++g_launches;
-  syrk_tc_kernel<<<grid, sy::THREADS, sy::SMEM_BYTES, st>>>(p);
+  if (f16) syrk_tc_kernel<true><<<grid, sy::THREADS, sy::SMEM_BYTES, st>>>(p);
+  else syrk_tc_kernel<false><<<grid, sy::THREADS, sy::SMEM_BYTES, st>>>(p);
 }
 
 }  // namespace phi4
