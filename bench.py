@@ -36,8 +36,10 @@ ALU_OPS_PER_LEAPFROG_SITE = 11
 # committed `ncu --set full` captures (not measured by this run): C1 the fused mutation kernel,
 # C3 / C4 the proposal GEMM.
 NCU_TRAFFIC = {"C1": (6815000, "profiles/r02_ncu_tables.md"),
-               "C3": (1132800000, "profiles/r02_ncu_tables.md"),
-               "C4": (14304000000, "profiles/r02_ncu_tables.md")}
+               "C3": (1035600000, "profiles/r02_ncu_tables.md (capture r02d: the launch also writes the next "
+                                  "step's normals, 0.21 GB)"),
+               "C4": (13807000000, "profiles/r02_ncu_tables.md (capture r02d: the launch also writes the next "
+                                   "step's normals, 2.1 GB)")}
 
 
 def peaks():
@@ -57,6 +59,12 @@ class ClockSampler(threading.Thread):
     def __init__(self, index):
         super().__init__(daemon=True)
         self.index, self.stop_flag, self.samples, self.reasons, self.max_mhz = index, False, [], set(), None
+        self.ready = threading.Event()          # NVML is up: the caller waits for this before timing
+
+    def begin(self):
+        self.start()
+        self.ready.wait(10.0)
+        return self
 
     def run(self):
         try:
@@ -68,15 +76,17 @@ class ClockSampler(threading.Thread):
                      nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
                      nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown",
                      nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap"}
+            self.ready.set()
             while not self.stop_flag:
                 self.samples.append(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM))
                 r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(h)
                 for bit, name in names.items():
                     if r & bit:
                         self.reasons.add(name)
-                time.sleep(0.02)
+                time.sleep(0.005)
         except Exception as e:                      # pragma: no cover - depends on the box
             self.reasons.add("nvml_unavailable:%s" % type(e).__name__)
+        self.ready.set()
 
     def finish(self):
         self.stop_flag = True
@@ -248,8 +258,7 @@ def run_ns(args, cfg):
     for w in range(max(args.warmup, 1)):
         step(replicas.replica_seed(1000 + w, rank), False)
     barrier()
-    sampler = ClockSampler(local)
-    sampler.start()
+    sampler = ClockSampler(local).begin()
     l0 = B.phi4_kernel_launches()
     ms, its = 0.0, []
     for s in range(args.steps):
@@ -411,8 +420,7 @@ def measure_workload(name, cfg, args, env, steps, warmup, max_temps, want_e2e):
     for w in range(warmup):
         device_step(replicas.replica_seed(1000 + w, rank))
     env["barrier"]()
-    sampler = ClockSampler(local)
-    sampler.start()
+    sampler = ClockSampler(local).begin()
     l0 = B.phi4_kernel_launches()
     ms, Ts = 0.0, []
     for s in range(steps):
