@@ -232,6 +232,37 @@ def test_ns_paper_setting_first_iteration_lockstep():
     h.close()
 
 
+@pytest.mark.parametrize("L,n,kd,nw", [(16, 32768, 16384, 3), (12, 2048, 1024, 4)])
+def test_ns_large_v_walk_lockstep(L, n, kd, nw):
+    """Constrained RW walks at V > 112: the walkers go through the tcgen05 proposal GEMM (FP16 operands), and
+    with 16384 walkers x 256 sites the GEMM of a step also draws the next step's normals (NS tags, walker
+    slots); the second case takes a kernel of its own for them.  First iteration against the oracle."""
+    seed, m0sq, lam = 23, -4.0, 1.0
+    h = B.ns_init(L, m0sq, lam, n, kd, nw, seed, max_iters=4)
+    st0 = B.smc_get_state(h)
+    info = B.ns_step(h)
+    S0 = st0["S"].astype(np.float64)
+    dead = O.ns_select(S0, kd)
+    assert np.array_equal(B.ns_get_dead(h)["last_dead"], dead)
+    Lc = B.smc_get_chol(h)
+    surv = np.setdiff1d(np.arange(n), dead)
+    start = np.array([surv[O.word0(seed, O.TAG_NS_START, 0, j) % (n - kd)] for j in range(kd)])
+    sub = np.sort(np.random.default_rng(5).choice(kd, 256, replace=False)).astype(np.int32)
+    f0 = st0["phi"][:, start[sub]].astype(np.float64)
+    Ss, Us = O.action_batch(f0, L, m0sq, lam)
+    p, S, U0, oacc, omar, cmar = O.mutate(f0, Ss, Us, L, m0sq, lam, Lc, np.float32(2.38 / math.sqrt(L * L)), 0.0,
+                                          seed, 1, nw, mode=O.MODE_NS, S_star=info["S_star"], slots=sub)
+    amb = np.minimum(np.abs(omar), np.abs(cmar)) < 1e-4
+    clean = ~amb.any(axis=0)
+    assert clean.mean() > 0.9
+    st1 = B.smc_get_state(h)
+    got = st1["phi"][:, dead[sub]]
+    assert np.abs(got[:, clean] - p[:, clean]).max() < 2e-5
+    assert np.array_equal(st1["phi"][:, surv], st0["phi"][:, surv])
+    assert np.all(st1["S"] < info["S_star"] + 1e-3) and 0.0 < oacc.mean() < 1.0
+    h.close()
+
+
 def test_ns_paper_setting_statistical_parity():
     """N = 5000, delete fraction 0.5, slice kernel (10 slice steps per replacement instead of 3 V,
     so that eight oracle runs stay affordable): log Z and iterations within 3 combined SE."""
