@@ -11,13 +11,15 @@
 //
 //   centre_split_kernel  phi[x][i] - mu[x] -> hi/lo parts in the UMMA K-major interleave layout
 //                        with the particle index as contraction index: 16-byte chunks of 4 (TF32)
-//                        or 8 (FP16) consecutive particles, Ps[part][chunk][x] (a 128-row slice of
-//                        one K-chunk is 2 KB contiguous).  Transposed through shared memory:
+//                        or 8 (FP16) consecutive particles, tile-major: Ps[x / 128][chunk][part]
+//                        [x % 128] -- the four chunks of a ring stage of one 128-row tile, hi and
+//                        lo, are ONE contiguous 16 KB run.  Transposed through shared memory:
 //                        coalesced both ways.
 //   syrk_tc_kernel       work item = (lower-triangular 128 x 256 output tile, K split).  Warp 8
-//                        streams both operand slices of a 4-chunk stage with cp.async.bulk into a
-//                        4-stage ring, warp 9 issues tcgen05.mma (hi*hi + hi*lo + lo*hi
-//                        into one FP32 TMEM accumulator).  The tensor core's FP32 accumulation
+//                        streams a stage with three bulk copies (the row tile, the two column
+//                        tiles; sixteen 2-4 KB copies with the part-major layout it replaces kept
+//                        the tensor pipe at 68 %) into a 4-stage ring, warp 9 issues tcgen05.mma
+//                        (hi*hi + hi*lo + lo*hi, two N = 128 halves, into one FP32 TMEM accumulator).  The tensor core's FP32 accumulation
 //                        truncates: over the 1e5-term sums of a covariance that is a -1e-4
 //                        relative bias (measured), so an accumulator only runs over 16 stages
 //                        (96 MMAs: K = 256 or 512); warps 0-7 then fold it into round-to-nearest
@@ -84,7 +86,7 @@ centre_split_kernel(const float* __restrict__ phi, int N, int ld, int V, int Vn,
   }
   __syncthreads();
   constexpr int CW = F16 ? 8 : 4, CSH = F16 ? 3 : 2;     // particles per 16-byte chunk
-  const size_t part = (size_t)(ldp >> CSH) * Vn;         // chunks per hi / lo part
+  const size_t nkc = (size_t)(ldp >> CSH);               // chunks per row
   for (int e = threadIdx.x; e < 32 * (128 / CW); e += 256) {
     const int kc = e >> 5, xr = e & 31;                  // lanes along x: 512 B contiguous stores
     uint4 hi, lo;
@@ -108,9 +110,10 @@ centre_split_kernel(const float* __restrict__ phi, int N, int ld, int V, int Vn,
       lo = make_uint4(__float_as_uint(v[0] - h[0]), __float_as_uint(v[1] - h[1]), __float_as_uint(v[2] - h[2]),
                       __float_as_uint(v[3] - h[3]));
     }
-    const size_t o = (size_t)((i0 >> CSH) + kc) * Vn + x0 + xr;
+    const int x = x0 + xr;
+    const size_t o = (((size_t)(x >> 7) * nkc + (size_t)((i0 >> CSH) + kc)) * 2) * sy::TM + (x & (sy::TM - 1));
     Ps[o] = hi;
-    Ps[part + o] = lo;
+    Ps[o + sy::TM] = lo;
   }
 }
 
@@ -158,7 +161,7 @@ __global__ void __launch_bounds__(sy::THREADS, 1) syrk_tc_kernel(const SyrkTcPar
   auto dempty = [&](int b) { return bar0 + 8u * (2 * STAGES + 2 + b); };
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * STAGES + 4);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int V = p.V, Vn = p.Vn;
+  const int V = p.V;
 
   if (warp == 8 && lane == 0) {
     for (int s = 0; s < STAGES; ++s) { mbar_init(full(s), 1); mbar_init(empty(s), 1); }
@@ -175,29 +178,24 @@ __global__ void __launch_bounds__(sy::THREADS, 1) syrk_tc_kernel(const SyrkTcPar
 
   if (warp == 8) {
     if (lane == 0) {
-      const size_t part = (size_t)p.nkc * Vn * 4;          // floats per hi / lo part
+      const size_t tile_f = (size_t)p.nkc * 2 * TM * 4;    // floats per 128-row tile
+      const uint64_t keep = l2_policy_evict_last();        // a wave of CTAs shares its operand panels
       int s = 0;
       uint32_t ph = 0;
       for (int item = blockIdx.x; item < p.nitems; item += gridDim.x) {
         int m0, n0, z;
         syrk_item(p, item, m0, n0, z);
         const int kc0 = z * p.chunks_per_split;
+        const float* a_src = p.Ps + (size_t)(m0 / TM) * tile_f;
+        const float* b_src = p.Ps + (size_t)(n0 / TM) * tile_f;
         for (int it = 0; it < nst; ++it) {
           mbar_wait(empty(s), ph ^ 1);
           const uint32_t st = ring + (uint32_t)s * STAGE_BYTES;
+          const size_t off = (size_t)(kc0 + 4 * it) * 2 * TM * 4;     // floats before this stage's chunks
           mbar_expect_tx(full(s), STAGE_BYTES);
-#pragma unroll
-          for (int c = 0; c < 4; ++c) {
-            const size_t row = (size_t)(kc0 + 4 * it + c) * Vn;
-#pragma unroll
-            for (int h = 0; h < 2; ++h) {
-              const float* base = p.Ps + (size_t)h * part + row * 4;
-              bulk_g2s(st + (uint32_t)h * A_PART + (uint32_t)c * CHUNK_A, base + (size_t)m0 * 4,
-                       CHUNK_A, full(s));
-              bulk_g2s(st + 2 * A_PART + (uint32_t)h * B_PART + (uint32_t)c * CHUNK_B,
-                       base + (size_t)n0 * 4, CHUNK_B, full(s));
-            }
-          }
+          bulk_g2s_hint(st, a_src + off, 2 * A_PART, full(s), keep);
+          bulk_g2s_hint(st + 2 * A_PART, b_src + off, 2 * A_PART, full(s), keep);
+          bulk_g2s_hint(st + 4 * A_PART, b_src + tile_f + off, 2 * A_PART, full(s), keep);
           if (++s == STAGES) { s = 0; ph ^= 1; }
         }
       }
@@ -207,9 +205,10 @@ __global__ void __launch_bounds__(sy::THREADS, 1) syrk_tc_kernel(const SyrkTcPar
     if (lane == 0) {
       int s = 0, cnt = 0;
       uint32_t ph = 0;
-      const uint64_t a_base = smem_desc(ring, CHUNK_A, 128);
-      const uint64_t b_base = smem_desc(ring + 2 * A_PART, CHUNK_B, 128);
-      const uint32_t idesc = F16 ? instr_desc_f16(TM, TN) : instr_desc(TM, TN);
+      // a tile's stage in shared memory: [chunk c][part][128 rows][16 B]; the two K-chunks of an MMA
+      // are 2 CHUNK_A apart (LBO), hi and lo of a chunk CHUNK_A
+      const uint64_t t_base = smem_desc(ring, 2 * CHUNK_A, 128);
+      const uint32_t idesc = F16 ? instr_desc_f16(TM, TM) : instr_desc(TM, TM);
       for (int item = blockIdx.x; item < p.nitems; item += gridDim.x) {
         for (int sub = 0; sub < nst / SUB_STAGES; ++sub, ++cnt) {
           const int buf = cnt & 1;
@@ -222,18 +221,22 @@ __global__ void __launch_bounds__(sy::THREADS, 1) syrk_tc_kernel(const SyrkTcPar
             const uint32_t so = (uint32_t)s * (STAGE_BYTES >> 4);
 #pragma unroll
             for (int kk = 0; kk < 2; ++kk) {
-              const uint64_t a_hi = a_base + so + (uint32_t)(2 * kk) * (CHUNK_A >> 4);
-              const uint64_t a_lo = a_hi + (A_PART >> 4);
-              const uint64_t b_hi = b_base + so + (uint32_t)(2 * kk) * (CHUNK_B >> 4);
-              const uint64_t b_lo = b_hi + (B_PART >> 4);
-              if constexpr (F16) {
-                tc_mma_f16(d, a_lo, b_hi, idesc, (it | kk) != 0);
-                tc_mma_f16(d, a_hi, b_lo, idesc, 1);
-                tc_mma_f16(d, a_hi, b_hi, idesc, 1);
-              } else {
-                tc_mma_tf32(d, a_lo, b_hi, idesc, (it | kk) != 0);
-                tc_mma_tf32(d, a_hi, b_lo, idesc, 1);
-                tc_mma_tf32(d, a_hi, b_hi, idesc, 1);
+              const uint64_t a_hi = t_base + so + (uint32_t)(4 * kk) * (CHUNK_A >> 4);
+              const uint64_t a_lo = a_hi + (CHUNK_A >> 4);
+#pragma unroll
+              for (int hb = 0; hb < 2; ++hb) {             // column tiles n0, n0 + 128
+                const uint64_t b_hi = a_hi + (uint32_t)((2 + 2 * hb) * (A_PART >> 4));
+                const uint64_t b_lo = b_hi + (CHUNK_A >> 4);
+                const uint32_t dh = d + (uint32_t)(hb * TM);
+                if constexpr (F16) {
+                  tc_mma_f16(dh, a_lo, b_hi, idesc, (it | kk) != 0);
+                  tc_mma_f16(dh, a_hi, b_lo, idesc, 1);
+                  tc_mma_f16(dh, a_hi, b_hi, idesc, 1);
+                } else {
+                  tc_mma_tf32(dh, a_lo, b_hi, idesc, (it | kk) != 0);
+                  tc_mma_tf32(dh, a_hi, b_lo, idesc, 1);
+                  tc_mma_tf32(dh, a_hi, b_hi, idesc, 1);
+                }
               }
             }
             tc_commit(empty(s));
