@@ -69,13 +69,15 @@ constexpr int L_TOP = 12;                    // FP16 factor: largest |entry| sca
 constexpr int LMAX_BLOCKS = 148, SCALE_SLOT = 160, SCALE_FLOATS = 256;
 }  // namespace lg
 
-__device__ __forceinline__ uint32_t pack_half2(__half a, __half b) {
-  return (uint32_t)__half_as_ushort(a) | ((uint32_t)__half_as_ushort(b) << 16);
-}
-// v = hi + lo in FP16 (round to nearest each): |v - hi - lo| <= 2^-22 |v| while lo is a normal number
-__device__ __forceinline__ void split_f16(float v, __half& hi, __half& lo) {
-  hi = __float2half_rn(v);
-  lo = __float2half_rn(v - __half2float(hi));
+// v = hi + lo in FP16 (round to nearest each): |v - hi - lo| <= 2^-22 |v| while lo is a normal number.
+// Two values at a time: cvt.rn.f16x2.f32 (F2FP.PACK_AB) runs on the ALU pipe at full rate; the scalar
+// conversion (F2F) shares the quarter-rate unit with the SFU calls of Box-Muller, which bounds the normals.
+__device__ __forceinline__ void split_f16x2(float a, float b, uint32_t& hi, uint32_t& lo) {
+  const __half2 h = __floats2half2_rn(a, b);
+  const float2 f = __half22float2(h);
+  const __half2 l = __floats2half2_rn(a - f.x, b - f.y);
+  hi = *reinterpret_cast<const uint32_t*>(&h);
+  lo = *reinterpret_cast<const uint32_t*>(&l);
 }
 
 // 16-byte chunk c of particle i: one Philox quad (TF32) or two (FP16: quads 2c, 2c + 1, scaled by 8),
@@ -90,11 +92,10 @@ __device__ __forceinline__ void normals_chunk(uint64_t seed, uint32_t tag, uint3
     normals4_fast(seed, tag, t, (uint32_t)i, (uint32_t)(2 * c), z);
     normals4_fast(seed, tag, t, (uint32_t)i, (uint32_t)(2 * c + 1), z + 4);
     const float s0 = (i < N && 8 * c < V) ? lg::Z_SCALE : 0.f, s1 = (i < N && 8 * c + 4 < V) ? lg::Z_SCALE : 0.f;
-    __half h[8], l[8];
-#pragma unroll
-    for (int e = 0; e < 8; ++e) split_f16((e < 4 ? s0 : s1) * z[e], h[e], l[e]);
-    hi = make_uint4(pack_half2(h[0], h[1]), pack_half2(h[2], h[3]), pack_half2(h[4], h[5]), pack_half2(h[6], h[7]));
-    lo = make_uint4(pack_half2(l[0], l[1]), pack_half2(l[2], l[3]), pack_half2(l[4], l[5]), pack_half2(l[6], l[7]));
+    split_f16x2(s0 * z[0], s0 * z[1], hi.x, lo.x);
+    split_f16x2(s0 * z[2], s0 * z[3], hi.y, lo.y);
+    split_f16x2(s1 * z[4], s1 * z[5], hi.z, lo.z);
+    split_f16x2(s1 * z[6], s1 * z[7], hi.w, lo.w);
   } else {
     float z[4] = {0.f, 0.f, 0.f, 0.f};
     if (i < N && 4 * c < V) normals4_fast(seed, tag, t, (uint32_t)i, (uint32_t)c, z);
@@ -218,11 +219,10 @@ __global__ void lsplit_tiled_kernel(const float* __restrict__ Lc, int V, int Vn,
   }
   uint4 hi, lo;
   if constexpr (F16) {
-    __half h[8], l[8];
-#pragma unroll
-    for (int e = 0; e < 8; ++e) split_f16(v[e], h[e], l[e]);
-    hi = make_uint4(pack_half2(h[0], h[1]), pack_half2(h[2], h[3]), pack_half2(h[4], h[5]), pack_half2(h[6], h[7]));
-    lo = make_uint4(pack_half2(l[0], l[1]), pack_half2(l[2], l[3]), pack_half2(l[4], l[5]), pack_half2(l[6], l[7]));
+    split_f16x2(v[0], v[1], hi.x, lo.x);
+    split_f16x2(v[2], v[3], hi.y, lo.y);
+    split_f16x2(v[4], v[5], hi.z, lo.z);
+    split_f16x2(v[6], v[7], hi.w, lo.w);
   } else {
     float h[4];
 #pragma unroll

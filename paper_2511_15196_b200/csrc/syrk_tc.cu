@@ -65,8 +65,13 @@ __global__ void __launch_bounds__(256) syrk_scale_kernel(const float* __restrict
   }
 }
 
-__device__ __forceinline__ uint32_t syrk_pack_half2(__half a, __half b) {
-  return (uint32_t)__half_as_ushort(a) | ((uint32_t)__half_as_ushort(b) << 16);
+// (as split_f16x2 in propose_tc.cu: packed conversions on the ALU pipe)
+__device__ __forceinline__ void syrk_split_f16x2(float a, float b, uint32_t& hi, uint32_t& lo) {
+  const __half2 h = __floats2half2_rn(a, b);
+  const float2 f = __half22float2(h);
+  const __half2 l = __floats2half2_rn(a - f.x, b - f.y);
+  hi = *reinterpret_cast<const uint32_t*>(&h);
+  lo = *reinterpret_cast<const uint32_t*>(&l);
 }
 
 // Block = 32 sites x 128 particles.  Pad particles (i >= N) contribute exact zeros.
@@ -91,17 +96,13 @@ centre_split_kernel(const float* __restrict__ phi, int N, int ld, int V, int Vn,
     const int kc = e >> 5, xr = e & 31;                  // lanes along x: 512 B contiguous stores
     uint4 hi, lo;
     if constexpr (F16) {
-      __half h[8], l[8];
+      float v[8];
 #pragma unroll
-      for (int j = 0; j < 8; ++j) {
-        const float v = tile[xr][8 * kc + j];
-        h[j] = __float2half_rn(v);
-        l[j] = __float2half_rn(v - __half2float(h[j]));
-      }
-      hi = make_uint4(syrk_pack_half2(h[0], h[1]), syrk_pack_half2(h[2], h[3]), syrk_pack_half2(h[4], h[5]),
-                      syrk_pack_half2(h[6], h[7]));
-      lo = make_uint4(syrk_pack_half2(l[0], l[1]), syrk_pack_half2(l[2], l[3]), syrk_pack_half2(l[4], l[5]),
-                      syrk_pack_half2(l[6], l[7]));
+      for (int j = 0; j < 8; ++j) v[j] = tile[xr][8 * kc + j];
+      syrk_split_f16x2(v[0], v[1], hi.x, lo.x);
+      syrk_split_f16x2(v[2], v[3], hi.y, lo.y);
+      syrk_split_f16x2(v[4], v[5], hi.z, lo.z);
+      syrk_split_f16x2(v[6], v[7], hi.w, lo.w);
     } else {
       float v[4], h[4];
 #pragma unroll
