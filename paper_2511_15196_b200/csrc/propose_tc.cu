@@ -323,6 +323,8 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
       int s = 0;
       uint32_t ph = 0;
       const int nstz = Kp >> F::KS_LOG;
+      // s*Lc blocks are re-read by every particle tile for the whole launch: evict_last.  The normals of
+      // a particle tile are dead after one work item; with the same hint they crowded the factor out.
       const uint64_t keep = l2_policy_evict_last();
       for (TileIter ti(p.ntm, p.ntn, p.pair); ti.valid(); ti.next()) {
         int m, tn;
@@ -336,7 +338,7 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
           const uint32_t bbytes = 128u * (uint32_t)nrows;    // 2 parts x 2 kk x 2 c x nrows x 16 B
           mbar_wait(empty(s), ph ^ 1);
           mbar_expect_tx(full(s), 2 * A_PART + bbytes);
-          bulk_g2s_hint(st, za + (size_t)it * (2 * A_PART / 4), 2 * A_PART, full(s), keep);
+          bulk_g2s(st, za + (size_t)it * (2 * A_PART / 4), 2 * A_PART, full(s));
           bulk_g2s_hint(st + 2 * A_PART, p.Lsplit + lt_stage_off<F16>(tn, it), bbytes, full(s), keep);
           if (++s == STAGES) { s = 0; ph ^= 1; }
         }
