@@ -82,6 +82,27 @@ def test_cov_chol(L, N):
     h.close()
 
 
+@pytest.mark.parametrize("path", [0, 3], ids=["3xfp16", "3xtf32"])
+@pytest.mark.parametrize("L,N,offset,amp", [(16, 4096, 3.0, 0.05), (15, 3000, -40.0, 0.5), (23, 2500, 0.0, 30.0),
+                                            (18, 8192, 0.3, 1e-3)])
+def test_large_v_covariance_scale_and_offset(L, N, offset, amp, path):
+    """The tcgen05 covariance (V > 112) on fields with a large common offset or a small / large spread: the
+    FP16 operand is c (phi - mu) with c from the device-side bound max |phi| + |mu| (far above |phi - mu| when
+    the offset dominates), the sums are centred before the split (R6); both operand formats, ragged V."""
+    phi = (offset + amp * inputs.smooth_fields(L, N, seed=31 + L, corr=0.3)).astype(np.float32)
+    h = new_smc(L, N, path=path)
+    B.smc_set_state(h, phi, 0.0, 0)
+    B.estimate_cov_chol(h)
+    Sig = B.smc_get_cov(h).astype(np.float64)
+    _, Sref = O.covariance(phi.astype(np.float64))
+    rel = np.linalg.norm(Sig - Sref) / np.linalg.norm(Sref)
+    print("cov L=%d offset %g amp %g path %d: relative error %.2e" % (L, offset, amp, path, rel))
+    # the inputs themselves carry 2^-24 |offset| of rounding against a spread of amp
+    assert rel < 1e-5 + 4.0 * 2.0 ** -24 * abs(offset) / amp
+    assert np.array_equal(Sig, Sig.T)
+    h.close()
+
+
 @pytest.mark.parametrize("L,N", [(10, 4096), (12, 1000), (7, 300), (16, 3000)])
 def test_cholesky_is_deterministic_under_repetition(L, N):
     """The one-CTA factorisation synchronises its warps with named barriers and keeps the matrix in
