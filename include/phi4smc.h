@@ -67,8 +67,9 @@ typedef struct {
   float ess_target; /* target ESS fraction in (0,1) for adaptive tempering        */
   float step_scale; /* s in phi' = phi + s*Lc*z; 0 selects 2.38/sqrt(V) (A3)       */
   int mutation_path; /* 0 = automatic, 1 = generic (any V), 2 = fused tcgen05 (if it supports V),
-                      * 3 = automatic with the large-V proposal product (L*L > 112) in 3xTF32
-                      * instead of the scaled 3xFP16 split of the same accuracy   */
+                      * 3 = automatic with the large-V products (proposal L*z and covariance,
+                      * L*L > 112) in 3xTF32 instead of the scaled 3xFP16 split of the same
+                      * accuracy (reading A20, 5.2, 5.4); PHI4_EINVAL for L*L <= 112     */
   /* Rejuvenation kernel: 0 = RW-Metropolis (i), 1 = HMC (iii, :172; reading A14),
    * 2 = independent MH from the fitted Gaussian N(mu, Sigma) (ii, :200; reading A15; L*L <= 800).
    * HMC: mass matrix diag(1/var_x) from the particle covariance, hmc_leapfrog >= 1 leapfrog steps
@@ -140,7 +141,7 @@ const char* phi4_last_cuda_error(const phi4smc* h);
 uint64_t phi4_kernel_launches(void);
 
 /* Measurement aid: the roofline denominators that MEASURED_PEAKS.json does not hold,
- * measured on the current device with kernels that do nothing else: dense tcgen05 kind::tf32
+ * measured on the current device with kernels that do nothing else: dense tcgen05 kind::tf32 and kind::f16
  * throughput (burst: best short launch; sustained: back-to-back launches for `seconds`, 0 < seconds
  * <= 30), FP32 FMA and 32x32->64 integer multiply rates in 1e12 lane-operations per second.
  * d_scratch: >= 4096 bytes of device memory (contents destroyed).  Synchronises.               */
