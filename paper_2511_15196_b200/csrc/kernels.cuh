@@ -71,8 +71,11 @@ bool propose_tc_supported(int V);
 size_t propose_tc_zsplit_floats(int V, int ld);
 size_t propose_tc_lsplit_floats(int V);
 void propose_tc_dims(int V, int* Vn, int* Kp, bool f16);
+// nsteps > 1: steps t .. t + nsteps - 1, one after the other in Zs (propose_tc_zstep_floats apart)
 void launch_normals_split(float* Zs, int N, int ld, int V, uint64_t seed, uint32_t tag, uint32_t t,
-                          const Ctrl* ctrl, int respect_done, cudaStream_t st, bool f16);
+                          const Ctrl* ctrl, int respect_done, cudaStream_t st, bool f16, int nsteps = 1);
+size_t propose_tc_zstep_floats(int V, int ld, bool f16);
+int propose_tc_zbatch(int V, int ld, bool f16);
 void launch_propose_lsplit(const float* Lc, int V, int ld, float s, float* Lsplit, const Ctrl* ctrl,
                            int respect_done, cudaStream_t st, bool f16);
 // next != nullptr: two spare warps of every GEMM CTA also draw the normals of step next->t into

@@ -320,16 +320,21 @@ void launch_mutate_generic(const MutateArgs& a, float* Lsplit, cudaStream_t st) 
   // Only where a CTA's GEMM work is long enough to hide its share of the normals.
   const bool fuse = Lsplit && a.Z2 && a.k > 1 && (size_t)a.ld * V >= ((size_t)1 << 22);
   float* zbuf[2] = {a.Z, fuse ? a.Z2 : a.Z};
-  if (Lsplit)
+  // small populations: the normals of a batch of steps per launch (one step alone is a launch-latency-sized
+  // kernel: 4.5 us at N = 5000, L = 15 for 1.7 us of work)
+  const int zb = (Lsplit && !fuse) ? propose_tc_zbatch(V, a.ld, a.tc_f16) : 1;
+  const size_t zstep = Lsplit ? propose_tc_zstep_floats(V, a.ld, a.tc_f16) : 0;
+  if (Lsplit && fuse)
     launch_normals_split(zbuf[0], a.N, a.ld, V, a.seed, a.tag_prop, a.t0, a.ctrl, a.respect_done, st, a.tc_f16);
   for (int j = 0; j < a.k; ++j) {
     uint32_t t = a.t0 + (uint32_t)j;
     if (Lsplit) {
-      if (!fuse && j > 0)
-        launch_normals_split(zbuf[0], a.N, a.ld, V, a.seed, a.tag_prop, t, a.ctrl, a.respect_done, st, a.tc_f16);
+      if (!fuse && j % zb == 0)
+        launch_normals_split(zbuf[0], a.N, a.ld, V, a.seed, a.tag_prop, t, a.ctrl, a.respect_done, st, a.tc_f16,
+                             a.k - j < zb ? a.k - j : zb);
       const NextNormals nx = {zbuf[(j + 1) & 1], a.N, a.seed, a.tag_prop, t + 1};
-      launch_propose_tc(a.phi, a.phip, zbuf[j & 1], Lsplit, a.ld, V, a.ctrl, a.respect_done, st, a.tc_f16,
-                        (fuse && j + 1 < a.k) ? &nx : nullptr);
+      launch_propose_tc(a.phi, a.phip, fuse ? zbuf[j & 1] : zbuf[0] + (size_t)(j % zb) * zstep, Lsplit, a.ld, V,
+                        a.ctrl, a.respect_done, st, a.tc_f16, (fuse && j + 1 < a.k) ? &nx : nullptr);
     } else {
       ++g_launches; normals_kernel<<<gz, 128, 0, st>>>(a.Z, a.N, a.ld, V, a.seed, a.tag_prop, t, a.ctrl,
                                          a.respect_done);

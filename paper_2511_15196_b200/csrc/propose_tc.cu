@@ -117,6 +117,10 @@ normals_split_kernel(uint4* __restrict__ Zs, int N, int ntm, int V, int Kp, int 
                      uint64_t seed, uint32_t tag, uint32_t t, const Ctrl* ctrl, int respect_done) {
   pdl_enter();
   if (respect_done && ctrl->done) return;
+  // blockIdx.z: step t + z of a batch, written behind the z steps before it (small populations draw
+  // several steps per launch: one step alone is a launch-latency-sized kernel)
+  t += blockIdx.z;
+  Zs += (size_t)blockIdx.z * ((size_t)ntm * lg::TILE * (size_t)(F16 ? Kp >> 2 : Kp >> 1));
   const int m = blockIdx.x, pr = threadIdx.x;
   const int i = m * lg::TILE + pr, nch = F16 ? Kp >> 3 : Kp >> 2;
   // SFU Box-Muller (philox.cuh, R2).  Quads beyond the lattice (K padding) stay zero;
@@ -543,8 +547,21 @@ void propose_tc_dims(int V, int* Vn, int* Kp, bool f16) {
   *Kp = round_up(V, f16 ? 32 : 16);
 }
 
-// (sized for either format: the TF32 operands are the larger ones)
-size_t propose_tc_zsplit_floats(int V, int ld) { return (size_t)2 * round_up(V, 16) * ld; }
+// floats of the split normals of ONE step
+size_t propose_tc_zstep_floats(int V, int ld, bool f16) {
+  return f16 ? (size_t)round_up(V, 32) * ld : (size_t)2 * round_up(V, 16) * ld;
+}
+// steps of normals drawn per launch: small populations (whose GEMM cannot hide the next step's normals)
+// draw a batch, FP16 only
+int propose_tc_zbatch(int V, int ld, bool f16) {
+  return (f16 && (size_t)ld * V < ((size_t)1 << 22)) ? 8 : 1;
+}
+// (sized for either format: one TF32 step or the FP16 batch)
+size_t propose_tc_zsplit_floats(int V, int ld) {
+  const size_t a = propose_tc_zstep_floats(V, ld, false);
+  const size_t b = propose_tc_zstep_floats(V, ld, true) * propose_tc_zbatch(V, ld, true);
+  return a > b ? a : b;
+}
 
 size_t propose_tc_lsplit_floats(int V) {
   const int ntn = round_up(V, lg::TN) / lg::TN;
@@ -553,15 +570,15 @@ size_t propose_tc_lsplit_floats(int V) {
 }
 
 void launch_normals_split(float* Zs, int N, int ld, int V, uint64_t seed, uint32_t tag, uint32_t t,
-                          const Ctrl* ctrl, int respect_done, cudaStream_t st, bool f16) {
+                          const Ctrl* ctrl, int respect_done, cudaStream_t st, bool f16, int nsteps) {
   const int Kp = round_up(V, f16 ? 32 : 16);
   const int nch = f16 ? Kp / 8 : Kp / 4;             // 16-byte chunks per particle row
   // chunks per thread: one per block made 1 M blocks at C4 (block-launch-rate bound); a small
   // population keeps one per thread so that the grid still fills the GPU
-  int cpb = (ld / lg::TILE) * nch / (148 * 16);
+  int cpb = (ld / lg::TILE) * nch * nsteps / (148 * 16);
   const int cmax = f16 ? 4 : 8;
   cpb = cpb < 1 ? 1 : cpb > cmax ? cmax : cpb;
-  dim3 grid(ld / lg::TILE, (nch + cpb - 1) / cpb);
+  dim3 grid(ld / lg::TILE, (nch + cpb - 1) / cpb, nsteps);
   ++g_launches;
   if (f16)
     launch_pdl(normals_split_kernel<true>, grid, 128, 0, st, reinterpret_cast<uint4*>(Zs), N, ld / lg::TILE, V,
