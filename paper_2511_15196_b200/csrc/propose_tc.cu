@@ -458,11 +458,11 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
 #pragma unroll
           for (int jj = 0; jj < 16; ++jj)
             if (x0 + cb + jj < V)
-              __stcs(p.phip + (size_t)(x0 + cb + jj) * p.ld + col, fmaf(__uint_as_float(r0[jj]), inv, f[cb + jj]));
+              p.phip[(size_t)(x0 + cb + jj) * p.ld + col] = fmaf(__uint_as_float(r0[jj]), inv, f[cb + jj]);
 #pragma unroll
           for (int jj = 0; jj < 16; ++jj)
             if (x0 + cb + 16 + jj < V)
-              __stcs(p.phip + (size_t)(x0 + cb + 16 + jj) * p.ld + col, fmaf(__uint_as_float(r1[jj]), inv, f[cb + 16 + jj]));
+              p.phip[(size_t)(x0 + cb + 16 + jj) * p.ld + col] = fmaf(__uint_as_float(r1[jj]), inv, f[cb + 16 + jj]);
         }
         tc_fence_before();
         __syncwarp();
@@ -496,7 +496,7 @@ __global__ void __launch_bounds__(lg::THREADS, 1) propose_tc_kernel(const Propos
             f[jj] = (x0 + cb + jj < V) ? __ldcs(p.phi + (size_t)(x0 + cb + jj) * p.ld + col) : 0.f;
 #pragma unroll
           for (int jj = 0; jj < 16; ++jj)
-            if (x0 + cb + jj < V) __stcs(p.phip + (size_t)(x0 + cb + jj) * p.ld + col, fmaf(acc[cb + jj], inv, f[jj]));
+            if (x0 + cb + jj < V) p.phip[(size_t)(x0 + cb + jj) * p.ld + col] = fmaf(acc[cb + jj], inv, f[jj]);
         }
       }
     }
