@@ -71,8 +71,7 @@ struct phi4smc {
   Ctrl* h_ctrl;              // pinned staging
   HostPoll* h_hp;            // pinned, written by the device at the end of every SMC temperature
   // side stream (fork / join by events on the caller's stream; host resources only): nested
-  // sampling runs the dead-point selection beside the covariance chain, the large-V mutation draws
-  // the normals of the next step beside the proposal GEMM of the current one
+  // sampling runs the dead-point selection beside the covariance chain
   cudaStream_t side;
   cudaEvent_t fork_ev, join_ev;
   StepRecord* h_rec;         // pinned staging (one record)
